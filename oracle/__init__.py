@@ -1,0 +1,198 @@
+"""CPU oracle — TEST INFRASTRUCTURE ONLY (see the header of ll_oracle.c).
+
+Thin ctypes marshalling over `libll_oracle.so` (built from ll_oracle.c by `oracle.build()` /
+`__graft_entry__.build()`).  No arithmetic of the method lives in this file.  Only tests/,
+`__graft_entry__.smoke()` and bench.py's cpu_baseline / --impl reference legs may import it; it never
+imports the CUDA package.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from typing import Optional
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "libll_oracle.so")
+_SRC = os.path.join(_HERE, "ll_oracle.c")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """gcc -O2 -fopenmp; plain C, no flags that reorder floating point."""
+    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-O2", "-std=c11", "-fopenmp", "-fPIC", "-shared", "-fno-fast-math",
+               "-o", _SO, _SRC, "-lm"]
+        subprocess.run(cmd, check=True)
+    return _SO
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        build()
+        _lib = C.CDLL(_SO)
+    return _lib
+
+
+def _p(a: Optional[np.ndarray], dtype=np.float64):
+    if a is None:
+        return None
+    assert a.dtype == dtype and a.flags["C_CONTIGUOUS"], (a.dtype, a.flags)
+    return a.ctypes.data_as(C.c_void_p)
+
+
+def _f64(a) -> np.ndarray:
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _i32(a) -> np.ndarray:
+    return np.ascontiguousarray(a, dtype=np.int32)
+
+
+def _check(rc: int, what: str):
+    if rc != 0:
+        raise RuntimeError(f"oracle {what} failed with status {rc}")
+
+
+def n_threads() -> int:
+    """Threads the OpenMP loops will use (for bench.py's cpu_baseline `cores`)."""
+    env = os.environ.get("OMP_NUM_THREADS")
+    return int(env) if env else (os.cpu_count() or 1)
+
+
+# ------------------------------------------------------------------ spline
+def spline_natural(x, y) -> np.ndarray:
+    x, y = _f64(x), _f64(y)
+    M = np.empty_like(x)
+    _check(lib().orc_spline_natural(C.c_int(len(x)), _p(x), _p(y), _p(M)), "spline_natural")
+    return M
+
+
+def spline_eval(x, y, f_q) -> np.ndarray:
+    x, y, f_q = _f64(x), _f64(y), _f64(f_q)
+    out = np.empty_like(f_q)
+    _check(lib().orc_spline_eval(C.c_int(len(x)), _p(x), _p(y), C.c_int64(f_q.size), _p(f_q), _p(out)), "spline_eval")
+    return out
+
+
+# ------------------------------------------------------------------ stand-in waveform
+def standin_fisco(p) -> float:
+    p = _f64(p)
+    out = C.c_double()
+    _check(lib().orc_standin_fisco(_p(p), C.byref(out)), "standin_fisco")
+    return out.value
+
+
+def standin_nodes(params, mode_m, c_lm, kappa, f, f_grid_lo, f_grid_hi, n_c=2):
+    """-> amp, phase [n_w][n_m][n_freq], tf [n_w][n_m][n_c][2], band [n_w][2]"""
+    params, f, c_lm, mode_m = _f64(params), _f64(f), _f64(c_lm), _i32(mode_m)
+    n_w, n_m, n = params.shape[0], len(mode_m), len(f)
+    assert params.shape[1] == 5 + 2 * n_c * n_m
+    amp = np.empty((n_w, n_m, n))
+    phase = np.empty((n_w, n_m, n))
+    tf = np.empty((n_w, n_m, n_c, 2))
+    band = np.empty((n_w, 2))
+    _check(lib().orc_standin_nodes(C.c_int64(n_w), C.c_int(n_m), C.c_int(n_c), _p(mode_m, np.int32), _p(c_lm),
+                                   C.c_double(kappa), _p(params), C.c_int(n), _p(f),
+                                   C.c_double(f_grid_lo), C.c_double(f_grid_hi),
+                                   _p(amp), _p(phase), _p(tf), _p(band)), "standin_nodes")
+    return amp, phase, tf, band
+
+
+def standin_direct(p, mode_m, c_lm, kappa, f, f_lo, f_hi, n_c=2) -> np.ndarray:
+    """stand-in template of ONE parameter row evaluated directly at f: [n_c][n_freq][2]"""
+    p, f, c_lm, mode_m = _f64(p), _f64(f), _f64(c_lm), _i32(mode_m)
+    n_m = len(mode_m)
+    assert p.shape == (5 + 2 * n_c * n_m,)
+    h = np.empty((n_c, len(f), 2))
+    _check(lib().orc_standin_direct(C.c_int(n_m), C.c_int(n_c), _p(mode_m, np.int32), _p(c_lm), C.c_double(kappa),
+                                    _p(p), C.c_int64(len(f)), _p(f), C.c_double(f_lo), C.c_double(f_hi), _p(h)),
+           "standin_direct")
+    return h
+
+
+# ------------------------------------------------------------------ inner products
+def dd(d, W) -> float:
+    d, W = _f64(d), _f64(W)
+    out = C.c_double()
+    _check(lib().orc_dd(C.c_int(d.shape[0]), C.c_int64(d.shape[1]), _p(d), _p(W), C.byref(out)), "dd")
+    return out.value
+
+
+def inner(a, b, W) -> complex:
+    """sum_c sum_k W_k conj(a_k) b_k; the real part is <a|b> (Eq. 3)."""
+    a, b, W = _f64(a), _f64(b), _f64(W)
+    re, im = C.c_double(), C.c_double()
+    _check(lib().orc_inner(C.c_int(a.shape[0]), C.c_int64(a.shape[1]), _p(a), _p(b), _p(W), C.byref(re), C.byref(im)),
+           "inner")
+    return complex(re.value, im.value)
+
+
+# ------------------------------------------------------------------ full-grid path
+def full_batch(f_nodes, amp, phase, tf, band, k_min, df, d, W, want_template=False):
+    """-> dict(logL, d_h, h_h, logL_direct[, h]) for amp/phase [n_w][n_m][n_nodes]."""
+    f_nodes, amp, phase, tf, W = _f64(f_nodes), _f64(amp), _f64(phase), _f64(tf), _f64(W)
+    n_w, n_m, n_nodes = amp.shape
+    n_c = tf.shape[2]
+    n_f = W.shape[0]
+    band = None if band is None else _f64(band)
+    d = None if d is None else _f64(d)
+    out = {k: np.empty(n_w) for k in ("logL", "d_h", "h_h", "logL_direct")}
+    h = np.empty((n_c, n_f, 2)) if want_template else None
+    _check(lib().orc_full_batch(C.c_int64(n_w), C.c_int(n_m), C.c_int(n_c), C.c_int(n_nodes), _p(f_nodes),
+                                _p(amp), _p(phase), _p(tf), _p(band), C.c_int64(n_f), C.c_int64(k_min),
+                                C.c_double(df), _p(d), _p(W), _p(out["logL"]), _p(out["d_h"]), _p(out["h_h"]),
+                                _p(out["logL_direct"]), _p(h)), "full_batch")
+    if want_template:
+        out["h"] = h
+    return out
+
+
+def full_batch_standin(wl_modes_m, c_lm, kappa, params, f_nodes, k_min, df, n_f, d, W, want_template=False):
+    """parameters -> node arrays (stand-in, rounded to fp64) -> full_batch."""
+    f_lo, f_hi = float(k_min) * df, float(k_min + n_f - 1) * df
+    amp, phase, tf, band = standin_nodes(params, wl_modes_m, c_lm, kappa, f_nodes, f_lo, f_hi)
+    return full_batch(f_nodes, amp, phase, tf, band, k_min, df, d, W, want_template)
+
+
+# ------------------------------------------------------------------ heterodyned path
+def het_prepare(k_min, df, d, W, h0_dense, f_edges):
+    d, W, h0_dense, f_edges = _f64(d), _f64(W), _f64(h0_dense), _f64(f_edges)
+    n_c, n_f = d.shape[0], d.shape[1]
+    n_b = len(f_edges) - 1
+    A0, A1 = np.empty((n_c, n_b, 2)), np.empty((n_c, n_b, 2))
+    B0, B1, B2 = np.empty((n_c, n_b)), np.empty((n_c, n_b)), np.empty((n_c, n_b))
+    ddb = C.c_double()
+    _check(lib().orc_het_prepare(C.c_int(n_c), C.c_int64(n_f), C.c_int64(k_min), C.c_double(df), _p(d), _p(W),
+                                 _p(h0_dense), C.c_int(len(f_edges)), _p(f_edges),
+                                 _p(A0), _p(A1), _p(B0), _p(B1), _p(B2), C.byref(ddb)), "het_prepare")
+    return dict(A0=A0, A1=A1, B0=B0, B1=B1, B2=B2, dd_band=ddb.value)
+
+
+def het_batch(f_edges, amp_e, phase_e, tf, h0_edges, summ):
+    f_edges, amp_e, phase_e, tf, h0_edges = _f64(f_edges), _f64(amp_e), _f64(phase_e), _f64(tf), _f64(h0_edges)
+    n_w, n_m, n_e = amp_e.shape
+    n_c = tf.shape[2]
+    out = {k: np.empty(n_w) for k in ("logL", "d_h", "h_h")}
+    _check(lib().orc_het_batch(C.c_int64(n_w), C.c_int(n_m), C.c_int(n_c), C.c_int(n_e), _p(f_edges),
+                               _p(amp_e), _p(phase_e), _p(tf), _p(h0_edges),
+                               _p(_f64(summ["A0"])), _p(_f64(summ["A1"])), _p(_f64(summ["B0"])), _p(_f64(summ["B1"])),
+                               C.c_double(summ["dd_band"]), _p(out["logL"]), _p(out["d_h"]), _p(out["h_h"])),
+           "het_batch")
+    return out
+
+
+def het_batch_standin(mode_m, c_lm, kappa, params, f_edges, h0_edges, summ, chunk=8192):
+    """parameters -> amp/phase at the edges (stand-in evaluated directly, no spline) -> het_batch."""
+    params = _f64(params)
+    outs = []
+    for lo in range(0, params.shape[0], chunk):
+        amp, phase, tf, _ = standin_nodes(params[lo:lo + chunk], mode_m, c_lm, kappa, f_edges,
+                                          float(f_edges[0]), float(f_edges[-1]))
+        outs.append(het_batch(f_edges, amp, phase, tf, h0_edges, summ))
+    if not outs:
+        return {k: np.empty(0) for k in ("logL", "d_h", "h_h")}
+    return {k: np.concatenate([o[k] for o in outs]) for k in outs[0]}

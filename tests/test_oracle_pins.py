@@ -1,0 +1,536 @@
+"""Pins for the CPU oracle (oracle/ll_oracle.c) against things OTHER than itself:
+library routines (SciPy CubicSpline, numpy.linalg), closed forms, textbook numbers, invariants the
+paper states, and brute force written a different way (numpy complex arithmetic, math.fsum, mpmath).
+All CPU-only (-m "not gpu").  Citations: PAPER.md line numbers; R<n> = DESIGN.md §3 readings.
+"""
+import math
+
+import mpmath
+import numpy as np
+import pytest
+from scipy.interpolate import CubicSpline
+
+from paper_2111_01064_b200 import workloads as wlm
+
+TWO_PI = 2.0 * math.pi
+
+
+# --------------------------------------------------------------------------- helpers (independent formulation)
+def _brute_full(f_nodes, amp, phase, tf, band, k_min, df, d, W):
+    """SciPy natural spline + numpy complex arithmetic + math.fsum.  One walker at a time."""
+    n_w, n_m, _ = amp.shape
+    n_c = tf.shape[2]
+    n_f = W.shape[0]
+    f = np.arange(k_min, k_min + n_f, dtype=np.float64) * df
+    dc = d[..., 0] + 1j * d[..., 1]
+    out = {k: np.zeros(n_w) for k in ("logL", "d_h", "h_h")}
+    dd = math.fsum((W[None, :] * np.abs(dc) ** 2).ravel())
+    for w in range(n_w):
+        mask = np.ones(n_f, bool) if band is None else (f >= band[w, 0]) & (f <= band[w, 1])
+        h = np.zeros((n_c, n_f), complex)
+        for m in range(n_m):
+            A = CubicSpline(f_nodes, amp[w, m], bc_type="natural")(f)
+            P = CubicSpline(f_nodes, phase[w, m], bc_type="natural")(f)
+            hm = A * np.exp(-1j * P)
+            for c in range(n_c):
+                h[c] += (tf[w, m, c, 0] + 1j * tf[w, m, c, 1]) * hm
+        h[:, ~mask] = 0.0
+        out["d_h"][w] = math.fsum((W[None, :] * (np.conj(dc) * h).real).ravel())
+        out["h_h"][w] = math.fsum((W[None, :] * np.abs(h) ** 2).ravel())
+        out["logL"][w] = out["d_h"][w] - 0.5 * out["h_h"][w] - 0.5 * dd
+    return out
+
+
+def _rand_smooth_nodes(rng, n_w, n_m, f_nodes):
+    """Smooth random amp/phase node arrays with a LISA-like dynamic range (phase ~1e3 rad)."""
+    x = np.log(f_nodes / f_nodes[0])
+    amp = np.empty((n_w, n_m, len(f_nodes)))
+    ph = np.empty_like(amp)
+    for w in range(n_w):
+        for m in range(n_m):
+            a, b, c = rng.uniform(0.5, 2.0), rng.uniform(-1, 1), rng.uniform(-300, 300)
+            amp[w, m] = a * np.exp(-0.7 * x) * (1.0 + 0.1 * np.sin(b + x))
+            ph[w, m] = c * x + 40.0 * np.cos(0.3 * x + b) + 900.0 * f_nodes / f_nodes[-1]
+    return amp, ph
+
+
+def _unit_tf(rng, n_w, n_m, n_c=2):
+    ang = rng.uniform(0, TWO_PI, (n_w, n_m, n_c))
+    return np.stack([np.cos(ang), np.sin(ang)], axis=-1)
+
+
+def _c(a):
+    return a[..., 0] + 1j * a[..., 1]
+
+
+# --------------------------------------------------------------------------- spline (R1, R21)
+@pytest.mark.parametrize("n", [3, 4, 7, 16, 257])
+def test_spline_matches_scipy_natural(orc, n):
+    rng = np.random.default_rng(n)
+    x = np.sort(rng.uniform(1e-4, 5e-2, n))
+    x[0], x[-1] = 1e-4, 5e-2
+    y = rng.standard_normal(n).cumsum()
+    cs = CubicSpline(x, y, bc_type="natural")
+    M = orc.spline_natural(x, y)
+    np.testing.assert_allclose(M, cs(x, 2), rtol=1e-10, atol=1e-10 * np.abs(cs(x, 2)).max())
+    assert M[0] == 0.0 and M[-1] == 0.0
+    q = rng.uniform(x[0], x[-1], 500)
+    np.testing.assert_allclose(orc.spline_eval(x, y, q), cs(q), rtol=0, atol=1e-12 * np.abs(y).max())
+
+
+def test_spline_dense_gaussian_elimination(orc):
+    """The tridiagonal system of R1 solved as a dense matrix (numpy.linalg.solve)."""
+    rng = np.random.default_rng(1)
+    for n in (3, 5, 12, 16):
+        x = np.cumsum(rng.uniform(0.1, 1.0, n))
+        y = rng.standard_normal(n)
+        h = np.diff(x)
+        A = np.zeros((n, n))
+        r = np.zeros(n)
+        A[0, 0] = A[-1, -1] = 1.0
+        for j in range(1, n - 1):
+            A[j, j - 1], A[j, j], A[j, j + 1] = h[j - 1] / 6, (h[j - 1] + h[j]) / 3, h[j] / 6
+            r[j] = (y[j + 1] - y[j]) / h[j] - (y[j] - y[j - 1]) / h[j - 1]
+        np.testing.assert_allclose(orc.spline_natural(x, y), np.linalg.solve(A, r), rtol=1e-11, atol=1e-12)
+
+
+def test_spline_reproduces_linear_and_interpolates_nodes(orc):
+    x = wlm.geomspace_exact(1e-4, 5e-2, 64)
+    y = 3.0e6 * x - 17.0                      # 2 pi f t_c like term: any cubic spline is exact (R2)
+    q = np.linspace(x[0], x[-1], 1001)
+    np.testing.assert_allclose(orc.spline_eval(x, y, q), 3.0e6 * q - 17.0, rtol=0, atol=1e-10)
+    np.testing.assert_allclose(orc.spline_natural(x, y), 0.0, atol=1e-3)  # |M| ~ rounding of y / h^2
+    y2 = np.sin(200 * x) + x ** -0.5
+    np.testing.assert_allclose(orc.spline_eval(x, y2, x), y2, rtol=1e-15, atol=0)
+
+
+def test_spline_c2_continuity_and_clamped_lookup(orc):
+    rng = np.random.default_rng(5)
+    x = np.cumsum(rng.uniform(0.5, 1.5, 9))
+    y = rng.standard_normal(9)
+    eps = 1e-6
+    for xi in x[1:-1]:
+        lo, mid, hi = orc.spline_eval(x, y, [xi - eps, xi, xi + eps])
+        # value and first derivative continuous: symmetric difference is O(eps^2)
+        assert abs(hi - 2 * mid + lo) < 1e-9
+    M = orc.spline_natural(x, y)
+    # second derivative is piecewise linear between the M_j: midpoint value equals the mean
+    xm = 0.5 * (x[:-1] + x[1:])
+    e2 = 1e-4
+    num2 = (orc.spline_eval(x, y, xm + e2) - 2 * orc.spline_eval(x, y, xm) + orc.spline_eval(x, y, xm - e2)) / e2 ** 2
+    np.testing.assert_allclose(num2, 0.5 * (M[:-1] + M[1:]), atol=1e-6)
+    # a query exactly on the last node uses the last interval (clamp, R21)
+    assert orc.spline_eval(x, y, [x[-1]])[0] == pytest.approx(y[-1], abs=1e-14)
+
+
+# --------------------------------------------------------------------------- stand-in waveform (R9)
+def _row(mc_msun=3e5, q=0.5, t_c=7.0e4, phi_c=1.2, inv_d=1.0, n_m=1, ang=None):
+    p = np.zeros(5 + 4 * n_m)
+    p[:5] = [mc_msun * wlm.GMSUN_S, q, t_c, phi_c, inv_d]
+    ang = np.linspace(0.3, 2.9, 2 * n_m) if ang is None else ang
+    p[5::2], p[6::2] = np.cos(ang), np.sin(ang)
+    return p
+
+
+def test_fisco_textbook_number(orc):
+    """f_ISCO = c^3/(6^{3/2} pi G M) = 4397 Hz for M = 1 Msun (textbook, ~4.4 kHz Msun/M)."""
+    p = _row(mc_msun=0.25 ** 0.6, q=1.0)      # eta = 1/4 -> M = Mc eta^{-3/5} = 1 Msun
+    assert orc.standin_fisco(p) == pytest.approx(4397.0, rel=2e-4)
+    # scales as 1/M
+    p2 = _row(mc_msun=1e6 * 0.25 ** 0.6, q=1.0)
+    assert orc.standin_fisco(p2) == pytest.approx(orc.standin_fisco(p) / 1e6, rel=1e-14)
+
+
+def test_standin_phase_derivative_is_newtonian_chirp_time(orc):
+    """(1/2pi) dPsi/df = t_c - tau(f),  tau = (5/256) Mc^{-5/3} (pi f)^{-8/3}  (Peters' time to coalescence).
+    Fails on a wrong sign or power in the PN term, a wrong eta/M relation, or a missing 2 pi f t_c."""
+    p = _row(mc_msun=4e5, q=0.3, t_c=9.0e4)
+    mc = p[0]
+    f = np.array([2e-4, 5e-4, 1e-3, 3e-3])
+    hstep = f * 1e-5
+    kw = dict(mode_m=[2], c_lm=[1.0], kappa=0.5, f_grid_lo=0.0, f_grid_hi=1.0)
+    _, php, _, _ = orc.standin_nodes(p[None], f=f + hstep, **kw)
+    _, phm, _, _ = orc.standin_nodes(p[None], f=f - hstep, **kw)
+    t_of_f = (php[0, 0] - phm[0, 0]) / (2 * hstep) / TWO_PI
+    tau = 5.0 / 256.0 * mc ** (-5.0 / 3.0) * (math.pi * f) ** (-8.0 / 3.0)
+    np.testing.assert_allclose(p[2] - t_of_f, tau, rtol=1e-6)
+
+
+def test_standin_q_enters_phase_only_through_fisco(orc):
+    """eta v^5 = (pi Mc f)^{5/3}: at fixed chirp mass the phase is independent of q."""
+    f = wlm.geomspace_exact(1e-4, 2e-3, 40)
+    kw = dict(mode_m=[2], c_lm=[1.0], kappa=0.5, f=f, f_grid_lo=0.0, f_grid_hi=1.0)
+    _, ph1, _, b1 = orc.standin_nodes(_row(q=0.2)[None], **kw)
+    _, ph2, _, b2 = orc.standin_nodes(_row(q=0.9)[None], **kw)
+    np.testing.assert_allclose(ph1, ph2, rtol=0, atol=1e-9 * np.abs(ph1).max())
+    assert b1[0, 1] != b2[0, 1]
+
+
+def test_standin_amplitude_powerlaw_and_taper(orc):
+    p = _row(mc_msun=5e5, q=1.0, inv_d=2.0)
+    fi = orc.standin_fisco(p)
+    kw = dict(mode_m=[2], c_lm=[1.0], kappa=0.5, f_grid_lo=0.0, f_grid_hi=1.0)
+    f = np.array([0.1, 0.5, 1.0]) * fi
+    a, _, _, band = orc.standin_nodes(p[None], f=f, **kw)
+    np.testing.assert_allclose(a[0, 0], 2.0 * f ** (-7.0 / 6.0), rtol=1e-14)          # untapered below f_ISCO
+    assert band[0, 1] == pytest.approx(1.5 * fi, rel=1e-15)
+    # taper: 1/2 at the midpoint, 0 at and beyond (1+kappa) f_ISCO, smooth (C^2) at both ends
+    f2 = np.array([1.25, 1.5, 1.7]) * fi
+    a2, _, _, _ = orc.standin_nodes(p[None], f=f2, **kw)
+    np.testing.assert_allclose(a2[0, 0] / (2.0 * f2 ** (-7.0 / 6.0)), [0.5, 0.0, 0.0], atol=1e-15)
+    for x0 in (1.0, 1.5):
+        e = 1e-4
+        fx = np.array([x0 - 2 * e, x0 - e, x0, x0 + e, x0 + 2 * e]) * fi
+        t = orc.standin_nodes(p[None], f=fx, **kw)[0][0, 0] / (2.0 * fx ** (-7.0 / 6.0))
+        assert abs(t[1] - 2 * t[2] + t[3]) / e ** 2 < 1e-2 * 60   # second derivative -> 0 (s^3 factor), not O(1)/kappa^2
+        assert abs((t[3] - t[1]) / (2 * e)) < 1e-3
+    # monotone on the taper
+    fx = np.linspace(1.0, 1.5, 50) * fi
+    t = orc.standin_nodes(p[None], f=fx, **kw)[0][0, 0] / (2.0 * fx ** (-7.0 / 6.0))
+    assert np.all(np.diff(t) <= 1e-15)
+
+
+def test_standin_mode_relation(orc):
+    """Psi_lm(f) = (m/2) Psi_22(2f/m);  A_lm(f) = c_lm f^{-7/6}/D taper(2f/(m f_ISCO))  (BASELINE config 3)."""
+    p6 = _row(n_m=3)
+    p1 = np.concatenate([p6[:5], p6[5:9]])
+    f = wlm.geomspace_exact(2e-4, 3e-3, 17)
+    kw = dict(kappa=0.5, f_grid_lo=0.0, f_grid_hi=1.0)
+    a, ph, tf, band = orc.standin_nodes(p6[None], mode_m=[2, 1, 3], c_lm=[1.0, 0.3, 0.2], f=f, **kw)
+    for i, (m, c) in enumerate([(2, 1.0), (1, 0.3), (3, 0.2)]):
+        a22, ph22, _, _ = orc.standin_nodes(p1[None], mode_m=[2], c_lm=[1.0], f=2 * f / m, **kw)
+        np.testing.assert_allclose(ph[0, i], (m / 2) * ph22[0, 0], rtol=1e-15)
+        # amplitude: same taper argument as the (2,2) mode at 2f/m, power law taken at f
+        np.testing.assert_allclose(a[0, i], c * a22[0, 0] * (f / (2 * f / m)) ** (-7.0 / 6.0), rtol=1e-14)
+    assert tf.shape == (1, 3, 2, 2) and np.all(tf.ravel() == p6[5:])
+    assert band[0, 1] == pytest.approx(1.5 * orc.standin_fisco(p6) * 1.5, rel=1e-15)  # max m/2 = 3/2
+
+
+# --------------------------------------------------------------------------- <h|h> closed form (Eq. 3)
+def _flat_setup(orc, t_obs, n_nodes, S0=3.0e-40):
+    grid = wlm.make_grid(t_obs)
+    f = grid.freqs()
+    w = np.ones(grid.n_f)
+    w[0] = w[-1] = 0.5
+    W = 4.0 * grid.df * w / S0
+    p = _row(mc_msun=50.0, q=1.0, t_c=0.6 * t_obs, inv_d=1.0)   # f_ISCO ~ 50 Hz >> band: no taper
+    assert orc.standin_fisco(p) > 1.0
+    return grid, f, W, p, S0
+
+
+def test_hh_closed_form_flat_psd_direct(orc):
+    """<h|h> = (6/(D^2 S0)) (f_lo^{-4/3} - f_hi^{-4/3}) for |T^A| = |T^E| = 1, no taper, flat PSD.
+    The discrete trapezoid sum differs from the integral by the Euler-Maclaurin term
+    (df^2/12)[g'(f_hi) - g'(f_lo)], g = f^{-7/3}; after adding it the residual is ~1e-6 (cfg-0 grid)."""
+    grid, f, W, p, S0 = _flat_setup(orc, 2.0 ** 17, 0)
+    h = orc.standin_direct(p, [2], [1.0], 0.5, f, f[0], f[-1])
+    hh = orc.inner(h, h, W).real
+    flo, fhi = f[0], f[-1]
+    integral = 6.0 / S0 * (flo ** (-4.0 / 3.0) - fhi ** (-4.0 / 3.0))
+    gp = lambda x: -7.0 / 3.0 * x ** (-10.0 / 3.0)
+    em = 8.0 / S0 * grid.df ** 2 / 12.0 * (gp(fhi) - gp(flo))
+    assert hh == pytest.approx(integral, rel=2e-3)
+    assert abs(hh - integral) / integral > 5e-4            # the trapezoid bias is really there (+1.3e-3)
+    assert hh == pytest.approx(integral + em, rel=5e-6)
+    # exact discrete sum with mpmath (50 digits)
+    mpmath.mp.dps = 50
+    s = mpmath.fsum(mpmath.mpf(float(Wk)) * mpmath.mpf(float(fk)) ** (mpmath.mpf(-7) / 3) for Wk, fk in zip(W, f))
+    assert hh == pytest.approx(float(2 * s), rel=1e-14)
+
+
+def test_hh_closed_form_through_spline_path(orc):
+    grid, f, W, p, S0 = _flat_setup(orc, 2.0 ** 17, 256)
+    f_nodes = wlm.geomspace_exact(1e-4, 0.05, 256)
+    r = orc.full_batch_standin([2], [1.0], 0.5, p[None], f_nodes, grid.k_min, grid.df, grid.n_f, None, W)
+    flo, fhi = f[0], f[-1]
+    integral = 6.0 / S0 * (flo ** (-4.0 / 3.0) - fhi ** (-4.0 / 3.0))
+    gp = lambda x: -7.0 / 3.0 * x ** (-10.0 / 3.0)
+    em = 8.0 / S0 * grid.df ** 2 / 12.0 * (gp(fhi) - gp(flo))
+    assert r["h_h"][0] == pytest.approx(integral + em, rel=2e-4)     # spline amplitude error <= 7e-5 (natural BC)
+    # 1024 nodes on the cfg-1 grid: 1e-5
+    grid2, f2, W2, p2, _ = _flat_setup(orc, 2.0 ** 22, 1024)
+    f_nodes2 = wlm.geomspace_exact(1e-4, 0.05, 1024)
+    r2 = orc.full_batch_standin([2], [1.0], 0.5, p2[None], f_nodes2, grid2.k_min, grid2.df, grid2.n_f, None, W2)
+    integral2 = 6.0 / S0 * (f2[0] ** (-4.0 / 3.0) - f2[-1] ** (-4.0 / 3.0))
+    assert r2["h_h"][0] == pytest.approx(integral2, rel=1e-5)
+
+
+# --------------------------------------------------------------------------- log L invariants (Eq. 2)
+@pytest.fixture(scope="module")
+def cfg0(orc):
+    wl = wlm.make_workload(0)
+    g = wl.grid
+    run = lambda params, d, tmpl=False: orc.full_batch_standin(
+        wl.modes_m, wl.c_lm, wl.kappa, params, wl.f_nodes, g.k_min, g.df, g.n_f, d, wl.W, want_template=tmpl)
+    wl.finish_distance(run(wl.inj[None], None)["h_h"][0])
+    h = run(wl.inj[None], None, True)["h"]
+    d = wl.make_data(h)
+    return wl, d, run
+
+
+def test_logL_zero_at_truth_noiseless(cfg0):
+    """noiseless data, correct model => the maximum log L = 0 at Theta_true."""
+    wl, d, run = cfg0
+    r = run(wl.params, d)
+    assert abs(r["logL"][0]) <= 1e-6
+    assert abs(r["logL_direct"][0]) <= 1e-20
+    assert math.sqrt(r["h_h"][0]) == pytest.approx(500.0, rel=1e-12)        # R18
+    assert np.all(r["logL"][1:] < -1.0)
+    np.testing.assert_allclose(r["logL"], r["logL_direct"], rtol=1e-9, atol=1e-6)   # R8: both forms of Eq. 2
+    # Cauchy-Schwarz: <d|h>^2 <= <d|d><h|h>
+    dd = -2.0 * r["logL"] + 2.0 * r["d_h"] - r["h_h"]
+    assert np.all(r["d_h"] ** 2 <= dd * r["h_h"] * (1 + 1e-12))
+
+
+def test_scaling_laws(cfg0):
+    """d_h ∝ 1/D, h_h ∝ 1/D^2; phi_c -> phi_c + delta rotates the complex overlap, h_h unchanged."""
+    wl, d, run = cfg0
+    p = wl.params[:8].copy()
+    r0 = run(p, d)
+    p2 = p.copy(); p2[:, 4] *= 3.0
+    r2 = run(p2, d)
+    np.testing.assert_allclose(r2["d_h"], 3.0 * r0["d_h"], rtol=1e-13)
+    np.testing.assert_allclose(r2["h_h"], 9.0 * r0["h_h"], rtol=1e-13)
+    # overlap O = sum W conj(d) h ; h(phi_c + delta) = e^{+i delta} h  => Re part rotates
+    delta = 0.7
+    p3 = p.copy(); p3[:, 3] += delta
+    p4 = p.copy(); p4[:, 3] += math.pi / 2
+    r3, r4 = run(p3, d), run(p4, d)
+    re, im = r0["d_h"], r4["d_h"]               # Re O and Re(i O) = -Im O
+    np.testing.assert_allclose(r3["d_h"], re * math.cos(delta) + im * math.sin(delta), rtol=1e-9, atol=1e-7)
+    np.testing.assert_allclose(r3["h_h"], r0["h_h"], rtol=1e-13)
+    # maximising over 1/D analytically: max_D log L = d_h^2/(2 h_h) - dd/2 >= log L
+    dd = -2.0 * r0["logL"] + 2.0 * r0["d_h"] - r0["h_h"]
+    assert np.all(0.5 * r0["d_h"] ** 2 / r0["h_h"] - 0.5 * dd >= r0["logL"] - 1e-9)
+
+
+# --------------------------------------------------------------------------- brute force, tiny inputs
+@pytest.mark.parametrize("n_m,n_nodes,n_f,banded", [(1, 4, 16, False), (1, 8, 64, True), (3, 6, 33, True)])
+def test_full_path_brute_force_tiny(orc, n_m, n_nodes, n_f, banded):
+    rng = np.random.default_rng(100 + n_nodes)
+    k_min, df = 5, 1.0 / 4096.0
+    f_lo, f_hi = k_min * df, (k_min + n_f - 1) * df
+    f_nodes = wlm.geomspace_exact(f_lo * 0.9, f_hi * 1.05, n_nodes)
+    amp, ph = _rand_smooth_nodes(rng, 3, n_m, f_nodes)
+    tf = _unit_tf(rng, 3, n_m) * rng.uniform(0.5, 1.5, (3, n_m, 2, 1))
+    W = rng.uniform(0.5, 2.0, n_f)
+    d = rng.standard_normal((2, n_f, 2))
+    band = None
+    if banded:
+        band = np.array([[f_lo, f_hi], [f_lo + 3.2 * df, f_hi - 5.5 * df], [f_hi * 2, f_hi * 3]])
+    o = orc.full_batch(f_nodes, amp, ph, tf, band, k_min, df, d, W)
+    b = _brute_full(f_nodes, amp, ph, tf, band, k_min, df, d, W)
+    for k in ("logL", "d_h", "h_h"):
+        np.testing.assert_allclose(o[k], b[k], rtol=1e-11, atol=1e-11)
+    if banded:      # a band that misses the grid gives log L = -<d|d>/2 (include/ll.h)
+        assert o["h_h"][2] == 0.0 and o["d_h"][2] == 0.0
+        assert o["logL"][2] == pytest.approx(-0.5 * orc.dd(d, W), rel=1e-15)
+
+
+def test_full_path_mpmath_one_walker(orc):
+    """One (walker, 2 modes) case summed with 40-digit arithmetic on top of SciPy spline values."""
+    rng = np.random.default_rng(7)
+    k_min, df, n_f = 3, 1.0 / 512.0, 12
+    f = np.arange(k_min, k_min + n_f) * df
+    f_nodes = wlm.geomspace_exact(f[0], f[-1], 5)
+    amp, ph = _rand_smooth_nodes(rng, 1, 2, f_nodes)
+    ph *= 0.01                                     # keep the phase small so the SciPy (fp64) spline values are exact enough
+    tf = _unit_tf(rng, 1, 2)
+    W = rng.uniform(0.5, 2.0, n_f)
+    d = rng.standard_normal((2, n_f, 2))
+    o = orc.full_batch(f_nodes, amp, ph, tf, None, k_min, df, d, W)
+    mpmath.mp.dps = 40
+    dh = hh = dd = mpmath.mpf(0)
+    for c in range(2):
+        for i in range(n_f):
+            h = mpmath.mpc(0)
+            for m in range(2):
+                A = mpmath.mpf(float(CubicSpline(f_nodes, amp[0, m], bc_type="natural")(f[i])))
+                P = mpmath.mpf(float(CubicSpline(f_nodes, ph[0, m], bc_type="natural")(f[i])))
+                h += mpmath.mpc(*map(float, tf[0, m, c])) * A * mpmath.expj(-P)
+            dc = mpmath.mpc(*map(float, d[c, i]))
+            dh += mpmath.mpf(float(W[i])) * (mpmath.conj(dc) * h).real
+            hh += mpmath.mpf(float(W[i])) * abs(h) ** 2
+            dd += mpmath.mpf(float(W[i])) * abs(dc) ** 2
+    assert o["d_h"][0] == pytest.approx(float(dh), rel=1e-12, abs=1e-12)
+    assert o["h_h"][0] == pytest.approx(float(hh), rel=1e-12)
+    assert o["logL"][0] == pytest.approx(float(dh - hh / 2 - dd / 2), rel=1e-12)
+
+
+def test_interval_lookup_on_node_and_empty_intervals(orc):
+    """R21: a bin that lands exactly on a node; intervals narrower than a bin (cfg-0 has 47 of them)."""
+    k_min, df, n_f = 8, 1.0 / 64.0, 20
+    f = np.arange(k_min, k_min + n_f) * df
+    f_nodes = np.array([f[0], f[0] + 0.2 * df, f[0] + 0.3 * df, f[3], f[3] + 0.5 * df, f[10], f[-1]])
+    rng = np.random.default_rng(3)
+    amp, ph = _rand_smooth_nodes(rng, 2, 1, f_nodes)
+    tf = _unit_tf(rng, 2, 1)
+    W, d = rng.uniform(0.5, 2, n_f), rng.standard_normal((2, n_f, 2))
+    o = orc.full_batch(f_nodes, amp, ph, tf, None, k_min, df, d, W)
+    b = _brute_full(f_nodes, amp, ph, tf, None, k_min, df, d, W)
+    np.testing.assert_allclose(o["logL"], b["logL"], rtol=1e-11)
+
+
+# --------------------------------------------------------------------------- heterodyne (Eq. 10-19)
+@pytest.fixture(scope="module")
+def het_small(orc):
+    """cfg-1 recipe on a 2^17 s grid (3.3k bins inside the band), 24 bins, 32 walkers."""
+    wl = wlm.make_workload(1, n_w=32, t_obs=2.0 ** 17, n_knots=24)
+    g = wl.grid
+    f = g.freqs()
+    lo, hi = f[0], f[-1]
+    direct = lambda p, ff: orc.standin_direct(p, wl.modes_m, wl.c_lm, wl.kappa, ff, lo, hi)
+    h1 = direct(wl.inj, f)
+    wl.finish_distance(orc.inner(h1, h1, wl.W).real)
+    h0 = direct(wl.inj, f)
+    d = wl.make_data(h0)
+    h0e = direct(wl.inj, wl.f_edges)
+    summ = orc.het_prepare(g.k_min, g.df, d, wl.W, h0, wl.f_edges)
+    return wl, f, d, h0, h0e, summ, direct
+
+
+def _band_mask(f, e):
+    return (f >= e[0]) & (f <= e[-1])
+
+
+def test_summary_data_partition_exactness(orc, het_small):
+    """sum_b A0(b) = sum_k W d conj(h0) and sum_b B0(b) = <h0|h0> over the het band; A1, B1 vs numpy."""
+    wl, f, d, h0, h0e, s, _ = het_small
+    m = _band_mask(f, wl.f_edges)
+    dc, hc, W = _c(d), _c(h0), wl.W
+    np.testing.assert_allclose(_c(s["A0"]).sum(axis=1), (W * dc * np.conj(hc))[:, m].sum(axis=1), rtol=1e-12)
+    np.testing.assert_allclose(s["B0"].sum(), (W * np.abs(hc) ** 2)[:, m].sum(), rtol=1e-12)
+    assert s["dd_band"] == pytest.approx((W * np.abs(dc) ** 2)[:, m].sum(), rel=1e-12)
+    e = wl.f_edges
+    idx = np.clip(np.searchsorted(e, f, side="right") - 1, 0, len(e) - 2)     # half-open bins, last closed (R13)
+    fb = 0.5 * (e[:-1] + e[1:])
+    for b in (0, 5, len(e) - 2):
+        sel = m & (idx == b)
+        assert sel.sum() > 0
+        t = f[sel] - fb[b]
+        np.testing.assert_allclose(_c(s["A1"])[:, b], (W[sel] * dc[:, sel] * np.conj(hc[:, sel]) * t).sum(axis=1),
+                                   rtol=1e-10, atol=1e-12 * np.abs(_c(s["A0"])[:, b]).max())
+        np.testing.assert_allclose(s["B1"][:, b], (W[sel] * np.abs(hc[:, sel]) ** 2 * t).sum(axis=1), rtol=1e-10,
+                                   atol=1e-12 * s["B0"][:, b].max() * (e[b + 1] - e[b]))
+
+
+def test_het_equals_full_at_reference(orc, het_small):
+    """north_star invariant: h = h0 => r = 1 => het log L = -1/2 <d-h0|d-h0>_band to rounding."""
+    wl, f, d, h0, h0e, s, _ = het_small
+    amp, ph, tf, _ = orc.standin_nodes(wl.inj[None], wl.modes_m, wl.c_lm, wl.kappa, wl.f_edges, f[0], f[-1])
+    r = orc.het_batch(wl.f_edges, amp, ph, tf, h0e, s)
+    m = _band_mask(f, wl.f_edges)
+    res = _c(d)[:, m] - _c(h0)[:, m]
+    direct = -0.5 * (wl.W[m] * np.abs(res) ** 2).sum()
+    assert r["logL"][0] == pytest.approx(direct, rel=1e-10)
+    assert r["h_h"][0] == pytest.approx(s["B0"].sum(), rel=1e-13)
+    assert r["d_h"][0] == pytest.approx(_c(s["A0"]).sum().real, rel=1e-13)
+
+
+def test_het_exact_for_linear_ratio_and_known_deficit(orc, het_small):
+    """h = (alpha + beta f) h0 => r exactly linear: Z[d,h] equals the dense <d|h>_band to rounding (Eq. 10-16),
+    and Z[h,h] falls short of the dense <h|h>_band by exactly sum |r1|^2 B2 (the O(f^2) term Eq. 17 drops)."""
+    wl, f, d, h0, h0e, s, _ = het_small
+    alpha, beta = 0.8 - 0.3j, (25.0 + 40.0j)
+    e = wl.f_edges
+    he = (alpha + beta * e)[None, :] * _c(h0e)                     # template at the edges, per channel
+    # feed it through the array entry: one "mode" per channel is not possible, so use tf = 1 and two calls
+    m = _band_mask(f, e)
+    hd = (alpha + beta * f)[None, :] * _c(h0)
+    dense_dh = (wl.W[m] * (np.conj(_c(d)[:, m]) * hd[:, m]).real).sum(axis=1)
+    dense_hh = (wl.W[m] * np.abs(hd[:, m]) ** 2).sum(axis=1)
+    for c in range(2):
+        amp = np.abs(he[c])[None, None, :]
+        ph = -np.unwrap(np.angle(he[c]))[None, None, :]            # h = A e^{-i Psi}  (Eq. 7, R6)
+        tf = np.zeros((1, 1, 2, 2)); tf[0, 0, c, 0] = 1.0
+        h0e_c = h0e.copy()
+        r = orc.het_batch(e, amp, ph, tf, h0e_c, s)
+        r1 = beta
+        deficit = abs(r1) ** 2 * s["B2"][c].sum()
+        # the other channel contributes h = 0 => r = 0 => nothing
+        assert r["d_h"][0] == pytest.approx(dense_dh[c], rel=1e-10)
+        assert r["h_h"][0] == pytest.approx(dense_hh[c] - deficit, rel=1e-10)
+        assert deficit / dense_hh[c] > 1e-9                        # the dropped term is visible, not rounding
+
+
+def test_het_brute_force_tiny(orc):
+    """2-4 bins x a few dozen dense points, everything random, numpy restatement of Eq. 11-19."""
+    rng = np.random.default_rng(11)
+    for n_b, n_f, n_m in ((2, 16, 1), (4, 40, 2), (3, 25, 3)):
+        k_min, df = 10, 1.0 / 1024.0
+        f = np.arange(k_min, k_min + n_f) * df
+        e = np.sort(np.concatenate([[f[1] - 0.3 * df, f[-2] + 0.1 * df], rng.uniform(f[3], f[-4], n_b - 1)]))
+        d, h0 = rng.standard_normal((2, n_f, 2)), rng.standard_normal((2, n_f, 2)) + 2.0
+        W = rng.uniform(0.5, 2.0, n_f)
+        h0e = rng.standard_normal((2, n_b + 1, 2)) + 2.0
+        s = orc.het_prepare(k_min, df, d, W, h0, e)
+        n_w = 3
+        amp = rng.uniform(0.5, 2.0, (n_w, n_m, n_b + 1))
+        ph = rng.uniform(-20, 20, (n_w, n_m, n_b + 1))
+        tf = _unit_tf(rng, n_w, n_m)
+        o = orc.het_batch(e, amp, ph, tf, h0e, s)
+        # numpy restatement
+        dc, hc = _c(d), _c(h0)
+        idx = np.searchsorted(e, f, side="right") - 1
+        idx[f == e[-1]] = n_b - 1
+        inside = (f >= e[0]) & (f <= e[-1])
+        fb = 0.5 * (e[:-1] + e[1:])
+        A0 = np.zeros((2, n_b), complex); A1 = A0.copy(); B0 = np.zeros((2, n_b)); B1 = B0.copy()
+        for i in np.nonzero(inside)[0]:
+            b = idx[i]
+            A0[:, b] += W[i] * dc[:, i] * np.conj(hc[:, i]); A1[:, b] += W[i] * dc[:, i] * np.conj(hc[:, i]) * (f[i] - fb[b])
+            B0[:, b] += W[i] * abs(hc[:, i]) ** 2; B1[:, b] += W[i] * abs(hc[:, i]) ** 2 * (f[i] - fb[b])
+        np.testing.assert_allclose(_c(s["A0"]), A0, rtol=1e-12, atol=1e-13)
+        np.testing.assert_allclose(s["B1"], B1, rtol=1e-10, atol=1e-13)
+        ddb = (W[inside] * np.abs(dc[:, inside]) ** 2).sum()
+        for w in range(n_w):
+            h = np.einsum("mc,me->ce", _c(tf[w]), amp[w] * np.exp(-1j * ph[w]))
+            r = h / _c(h0e)
+            r0, r1 = 0.5 * (r[:, :-1] + r[:, 1:]), (r[:, 1:] - r[:, :-1]) / np.diff(e)
+            dh = (A0 * np.conj(r0) + A1 * np.conj(r1)).real.sum()
+            hh = (B0 * np.abs(r0) ** 2 + 2 * B1 * (r0 * np.conj(r1)).real).sum()
+            assert o["d_h"][w] == pytest.approx(dh, rel=1e-11, abs=1e-11)
+            assert o["h_h"][w] == pytest.approx(hh, rel=1e-11)
+            assert o["logL"][w] == pytest.approx(dh - hh / 2 - ddb / 2, rel=1e-11)
+
+
+def test_het_reference_zero_is_an_error(orc, het_small):
+    wl, f, d, h0, h0e, s, _ = het_small
+    bad = h0e.copy(); bad[1, 3] = 0.0
+    amp, ph, tf, _ = orc.standin_nodes(wl.inj[None], wl.modes_m, wl.c_lm, wl.kappa, wl.f_edges, f[0], f[-1])
+    with pytest.raises(RuntimeError, match="-6"):
+        orc.het_batch(wl.f_edges, amp, ph, tf, bad, s)
+
+
+def test_het_tracks_dense_likelihood_near_reference(orc, het_small):
+    """the brute-force likelihood verifies the heterodyned one.  Accuracy of the METHOD
+    (not parity): for the 1e-3 Gaussian ball (|log L| of a few 1e3 at SNR 500) the heterodyned value tracks the
+    dense one to < 1 % with only 24 bins (measured 0.2-0.6 %; 1e-4 with 128 bins)."""
+    wl, f, d, h0, h0e, s, direct = het_small
+    r = orc.het_batch_standin(wl.modes_m, wl.c_lm, wl.kappa, wl.params, wl.f_edges, h0e, s)
+    m = _band_mask(f, wl.f_edges)
+    for w in range(8):
+        h = _c(direct(wl.params[w], f))
+        dense = -0.5 * (wl.W[m] * np.abs(_c(d)[:, m] - h[:, m]) ** 2).sum()
+        assert abs(dense - r["logL"][w]) < 0.01 * abs(dense)
+        assert dense < -100.0                                       # the ball really is off the peak
+
+
+# --------------------------------------------------------------------------- noise normalisation
+def test_noise_normalisation_statistic(orc):
+    """<n n'> = S_n delta / 2  =>  (d_h - h_h)/sqrt(h_h) at Theta_true is N(0,1) over noise seeds (R16)."""
+    wl = wlm.make_workload(1, n_w=1, t_obs=2.0 ** 15, n_knots=8)
+    g = wl.grid
+    f = g.freqs()
+    h = orc.standin_direct(wl.inj, wl.modes_m, wl.c_lm, wl.kappa, f, f[0], f[-1])
+    hh = orc.inner(h, h, wl.W).real
+    z = []
+    for s in range(200):
+        n = wlm._draw_noise(90000 + s, g, 2)
+        z.append(orc.inner(n, h, wl.W).real / math.sqrt(hh))
+    z = np.array(z)
+    assert abs(z.mean()) < 0.2
+    assert 0.7 < z.var() < 1.4
+    # E<n|n> = 2 n_f per channel
+    nn = np.mean([orc.dd(wlm._draw_noise(91000 + s, g, 2), wl.W) for s in range(20)])
+    assert nn == pytest.approx(4.0 * g.n_f, rel=0.05)
