@@ -1,0 +1,397 @@
+#!/usr/bin/env python
+"""bench.py — log-likelihood evaluations/s of the B200-native library on BASELINE.json's workloads.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload 2] [--quick]
+
+A step is one pass of the whole full-grid hot path (F1-F4: parameters -> node amp/phase -> spline -> fused
+evaluate/response/inner products -> log L) over BASELINE.json config 2 (16384 walkers x 1 574 725 bins, 1024
+nodes, FP64), the configuration north_star sets its roofline target on.  The same JSON line carries the
+heterodyned configs (1, 3, 4) and config 0 under "per_config", the ALU roofline of the fused kernel, the
+end-to-end number through the C ABI with host buffers, and the CPU oracle timed on this box.
+
+N > 1 (torchrun): walkers are independent, so every rank runs its own seeded config-2 batch
+(weak scaling), no data-path collective; the time is the max over ranks, the value the sum of units / that time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2111_01064_b200 import workloads as wlm  # noqa: E402
+
+METRIC = "log-likelihood evals/sec"
+UNIT = "evals/s"
+# algorithmic FP64 issue slots per active (walker, bin, mode) of the full-grid path, direct formulation
+# (t 1, two cubics 6, reduce 3, sincos 18, A e^{-i Psi} 2, two complex MACs 8, W A^2 2 => 40; the
+# SURVEY.md §8(d) figure of 39 is used as the contract number)
+SLOTS_FULL = 39.0
+SLOTS_HET = {1: 73.0, 6: 252.0}
+DFMA_PER_CLK_PER_SM = 64.0
+
+
+# ------------------------------------------------------------------------------------------------ helpers
+def rank_workload(index: int, rank: int, n_w=None, **kw):
+    """rank r draws its own batch: seed = SEED_BASE + index + 1000 r (weak scaling, walkers independent)."""
+    return wlm.make_workload(index, n_w=n_w, seed_offset=rank, **kw)
+
+
+def _dist():
+    import torch.distributed as dist
+    return dist if dist.is_available() and dist.is_initialized() else None
+
+
+def allreduce_max(x: float) -> float:
+    import torch
+    dist = _dist()
+    if dist is None:
+        return float(x)
+    dev = "cuda" if dist.get_backend() == "nccl" else "cpu"
+    t = torch.tensor([x], dtype=torch.float64, device=dev)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def allreduce_sum(x: float) -> float:
+    import torch
+    dist = _dist()
+    if dist is None:
+        return float(x)
+    dev = "cuda" if dist.get_backend() == "nccl" else "cpu"
+    t = torch.tensor([x], dtype=torch.float64, device=dev)
+    dist.all_reduce(t, op=dist.ReduceOp.SUM)
+    return float(t.item())
+
+
+def barrier():
+    dist = _dist()
+    if dist is not None:
+        dist.barrier()
+
+
+class ClockSampler:
+    """SM clock and throttle reasons sampled DURING the timed region (pynvml; nvidia-smi as a fallback)."""
+
+    BAD = {"hw_slowdown": 0x8, "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20}
+    NOTE = {"sw_power_cap": 0x4, "hw_power_brake": 0x80}
+
+    def __init__(self, index: int, period: float = 0.02):
+        self.index, self.period = index, period
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._t = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self.nv = None
+
+    def _loop(self):
+        nv = self.nv
+        while not self._stop.is_set():
+            try:
+                self.samples.append(float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                mask = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)) if hasattr(
+                    nv, "nvmlDeviceGetCurrentClocksEventReasons") else int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                for k, bit in {**self.BAD, **self.NOTE}.items():
+                    if mask & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            self._stop.wait(self.period)
+
+    def __enter__(self):
+        if self.nv is not None:
+            self._t = threading.Thread(target=self._loop, daemon=True)
+            self._t.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        if self._t is not None:
+            self._t.join()
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["unavailable"]}
+        return {"sm_mhz": statistics.median(self.samples), "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return json.load(open(p)), "measured"
+        except Exception:
+            pass
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+# ------------------------------------------------------------------------------------------------ GPU arm
+def time_steps(torch, fn, steps: int, warmup: int):
+    """W untimed steps, then K steps between two events on the current stream; returns total ms."""
+    for _ in range(warmup):
+        fn()
+    torch.cuda.synchronize()
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        fn()
+    e1.record()
+    torch.cuda.synchronize()
+    barrier()
+    return e0.elapsed_time(e1)
+
+
+def bench_config(torch, index: int, steps: int, warmup: int, rank: int = 0, profile: bool = False):
+    """device-resident timing of one config through the stand-in entry point (parameters -> log L)."""
+    from paper_2111_01064_b200 import synth
+    wl = rank_workload(index, rank)
+    ctx = synth.make_context(wl)
+    bufs = synth.setup(ctx, wl)
+    params = bufs["params"]
+    n_w = wl.n_w
+    out = tuple(torch.empty(n_w, dtype=torch.float64, device=params.device) for _ in range(3))
+    if wl.path == "full":
+        fn = lambda: ctx.full_batch_standin(wl.f_nodes, params, out=out)
+    else:
+        fn = lambda: ctx.het_batch_standin(params, out=out)
+    fn()                                    # first call: workspace allocation
+    for _ in range(warmup):
+        fn()
+    torch.cuda.synchronize()
+    l0 = ctx.kernel_launches()
+    if profile:
+        ctx.profile_enable(True)
+    ms = time_steps(torch, fn, steps, 0)
+    res = {"wl": wl, "ctx": ctx, "bufs": bufs, "fn": fn, "out": out, "ms_total": ms, "ms_per_step": ms / steps,
+           "launches": ctx.kernel_launches() - l0}
+    if profile:
+        kms, kn = ctx.profile_read()
+        ctx.profile_enable(False)
+        res["kernel_ms"] = kms / max(kn, 1)
+        res["kernel_n"] = kn
+    return res
+
+
+def e2e_config(torch, res, steps: int, warmup: int):
+    """same metric through the C ABI with HOST buffers: pinned params in, pinned results out, every step."""
+    wl, ctx = res["wl"], res["ctx"]
+    ph = torch.as_tensor(np.ascontiguousarray(wl.params)).pin_memory()
+    outs = tuple(torch.empty(wl.n_w, dtype=torch.float64).pin_memory() for _ in range(3))
+    if wl.path == "full":
+        fn = lambda: ctx.full_batch_standin_host(wl.f_nodes, ph, outs)
+    else:
+        fn = lambda: ctx.het_batch_standin_host(ph, outs)
+    ms = time_steps(torch, fn, steps, warmup)
+    dev_logL = res["out"][0].cpu()
+    assert torch.equal(dev_logL, outs[0]), "host-buffer path and device-resident path disagree"
+    return ms / steps, ph.numel() * 8, 3 * wl.n_w * 8
+
+
+def cpu_baseline(index: int, n_sample: int, budget_note: str = ""):
+    """the oracle, as it stands, on this box's cores, on the first n_sample walkers of the same workload"""
+    import oracle as orc
+    wl = rank_workload(index, 0)
+    g = wl.grid
+    t_setup = time.perf_counter()
+    if wl.path == "full":
+        run = lambda p, d, t=False: orc.full_batch_standin(wl.modes_m, wl.c_lm, wl.kappa, p, wl.f_nodes, g.k_min, g.df,
+                                                           g.n_f, d, wl.W, want_template=t)
+        wl.finish_distance(run(wl.inj[None], None)["h_h"][0])
+        d = wl.make_data(run(wl.inj[None], None, True)["h"])
+        work = lambda: run(wl.params[:n_sample], d)
+    else:
+        f = g.freqs()
+        direct = lambda p, ff: orc.standin_direct(p, wl.modes_m, wl.c_lm, wl.kappa, ff, float(f[0]), float(f[-1]))
+        h1 = direct(wl.inj, f)
+        wl.finish_distance(orc.inner(h1, h1, wl.W).real)
+        h0 = direct(wl.inj, f)
+        d = wl.make_data(h0)
+        h0e = direct(wl.inj, wl.f_edges)
+        summ = orc.het_prepare(g.k_min, g.df, d, wl.W, h0, wl.f_edges)
+        work = lambda: orc.het_batch_standin(wl.modes_m, wl.c_lm, wl.kappa, wl.params[:n_sample], wl.f_edges, h0e, summ)
+    t_setup = time.perf_counter() - t_setup
+    t0 = time.perf_counter()
+    work()
+    dt = time.perf_counter() - t0
+    return {"value": n_sample / dt, "unit": UNIT, "cores": orc.n_threads(), "kind": "oracle",
+            "sample": f"{wl.name}: first {n_sample} of {wl.n_w} walkers, whole grid, {dt:.1f} s wall{budget_note}",
+            "seconds": dt, "work": work, "n_sample": n_sample}
+
+
+def run_reference(args):
+    """--impl reference: the oracle is the reference arm for this tier (no reference implementation exists)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import oracle as orc
+    orc.build()
+    cores = orc.n_threads()
+    n_sample = max(cores, 1)
+    cb = cpu_baseline(args.workload, n_sample)
+    work = cb.pop("work")
+    for _ in range(max(args.warmup - 1, 0)):
+        work()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        work()
+    dt = time.perf_counter() - t0
+    wl = rank_workload(args.workload, 0)
+    val = n_sample * args.steps / dt
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64 (x87 long double accumulators)", "data": "synthetic",
+            "config": workload_config(wl, extra={"step": f"{n_sample} walkers of the batch per step (bounded sample)"}),
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle",
+                             "sample": f"{wl.name}: first {n_sample} walkers per step, whole grid"},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+def workload_config(wl, extra=None):
+    g = wl.grid
+    c = {"workload": wl.name, "path": wl.path, "n_walkers": wl.n_w, "n_modes": wl.n_m, "n_channels": wl.n_c,
+         "n_f": g.n_f, "t_obs_s": g.t_obs,
+         "inputs": "seeded synthetic (DESIGN.md §4), stand-in for LDC-1A",
+         "l2": "working set (spline coefficients 1.07 GB + node values 0.27 GB per step) exceeds the 126 MB L2; "
+               "no flush needed"}
+    if wl.path == "full":
+        c["n_nodes"] = int(len(wl.f_nodes))
+    else:
+        c["n_bins"] = int(len(wl.f_edges) - 1)
+        c["l2"] = "params and outputs only; summary tables live in shared memory (nothing to flush)"
+    if extra:
+        c.update(extra)
+    return c
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--workload", type=int, default=2, help="BASELINE.json config index of the headline step")
+    ap.add_argument("--quick", action="store_true", help="skip per_config, e2e and cpu_baseline (profiling runs)")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
+
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the library has no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+    from paper_2111_01064_b200 import build as _b
+    if rank == 0 or not os.path.exists(_b.SO):
+        _b.build()
+    barrier()
+
+    peaks, peak_src = measured_peaks()
+    with ClockSampler(local) as clk:
+        res = bench_config(torch, args.workload, args.steps, args.warmup, rank=rank, profile=True)
+    wl, ctx = res["wl"], res["ctx"]
+    t_ms = allreduce_max(res["ms_total"])
+    units = allreduce_sum(float(wl.n_w) * args.steps)
+    value = units / (t_ms * 1e-3)
+    clocks = clk.summary()
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": t_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic", "config": workload_config(wl), "clocks": clocks,
+            "gpu_launches": int(res["launches"]), "impl": "b200"}
+
+    if rank == 0:
+        # ---- roofline of the dominant kernel (fused full-grid F3, or the het batch kernel)
+        sm_max = float(clocks.get("sm_max_mhz") or peaks.get("sm_max_mhz", 1965.0))
+        n_sm = torch.cuda.get_device_properties(local).multi_processor_count
+        peak_slots = n_sm * DFMA_PER_CLK_PER_SM * sm_max * 1e6
+        if wl.path == "full":
+            pairs, n_blocks = ctx.last_full_stats()
+            slots = pairs * SLOTS_FULL
+            kname = "k_full_fused"
+        else:
+            pairs = float(wl.n_w) * (len(wl.f_edges) - 1)
+            slots = pairs * SLOTS_HET.get(wl.n_m, 73.0 + 36.0 * (wl.n_m - 1))
+            kname = "k_het_standin"
+        k_ms = res["kernel_ms"]
+        achieved = slots / (k_ms * 1e-3)
+        dfma_rate, dfma_ms = ctx.peak_fma(0, 4000)
+        ffma_rate, _ = ctx.peak_fma(1, 8000)
+        line["roofline"] = {
+            "bound": "alu", "kernel": kname, "achieved": achieved / 1e12, "peak": peak_slots / 1e12,
+            "unit": "T FP64 issue slots/s (1 DFMA|DMUL|DADD = 1 slot)", "frac": achieved / peak_slots,
+            "traffic": None, "kernel_ms": k_ms, "kernel_share_of_step": k_ms / (res["ms_per_step"]),
+            "algorithmic_slots_per_pair": SLOTS_FULL if wl.path == "full" else slots / pairs, "active_pairs": pairs,
+            "peak_source": f"{n_sm} SMs x {int(DFMA_PER_CLK_PER_SM)} DFMA/clk x {sm_max:.0f} MHz (DESIGN.md §6)",
+            "measured_dfma_per_s": dfma_rate, "measured_ffma_per_s": ffma_rate,
+            "frac_of_measured_dfma": achieved / dfma_rate,
+            "hbm_peak_gbs": peaks.get("hbm_gbs"), "hbm_peak_source": peak_src}
+
+    if not args.quick:
+        # ---- end to end through the C ABI with host buffers
+        ms_e2e, bi, bo = e2e_config(torch, res, max(args.steps // 2, 3), 3)
+        t_e2e = allreduce_max(ms_e2e)
+        line["e2e"] = {"value": world * wl.n_w / (t_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": bi,
+                       "d2h_bytes_per_step": bo, "ms_per_step": t_e2e}
+    res["ctx"].destroy()
+    del res
+    torch.cuda.empty_cache()
+
+    if rank == 0 and not args.quick and world == 1:
+        # ---- every BASELINE.json config, device-resident, stand-in entry points
+        per = {}
+        for idx in (0, 1, 2, 3, 4):
+            if idx == args.workload:
+                per[f"cfg{idx}"] = {"evals_per_s": value, "ms_per_batch": t_ms / args.steps, "n_walkers": wl.n_w}
+                continue
+            st = 50 if idx != 2 else args.steps
+            r = bench_config(torch, idx, st, 5)
+            per[f"cfg{idx}"] = {"evals_per_s": r["wl"].n_w / (r["ms_per_step"] * 1e-3), "ms_per_batch": r["ms_per_step"],
+                                "n_walkers": r["wl"].n_w}
+            r["ctx"].destroy()
+            del r
+            torch.cuda.empty_cache()
+        line["per_config"] = per
+        # ---- the oracle on this box's cores, bounded sample of the same workload
+        import oracle as orc
+        orc.build()
+        n_sample = 4 * orc.n_threads() if wl.path == "full" else min(wl.n_w, 4096)
+        cb = cpu_baseline(args.workload, n_sample)
+        cb.pop("work")
+        line["cpu_baseline"] = cb
+    if rank == 0:
+        print(json.dumps(line))
+    if world > 1:
+        import torch.distributed as dist
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -1,0 +1,168 @@
+/*
+ * ll.h — C ABI of the B200-native batched LISA MBHB log-likelihood library (libll_b200.so).
+ *
+ * What it computes (arXiv:2111.01064, text in /root/reference/PAPER.md; readings R1..R23 in DESIGN.md §3):
+ *   log L = -1/2 <d-h|d-h> = <d|h> - 1/2 <h|h> - 1/2 <d|d>                         Eq. 2
+ *   <a|b> = 4 Re sum_{A,E} int a~*(f) b~(f) / S_n(f) df                            Eq. 3
+ *   h~_lm(f) = A_lm(f) exp(-i phi_lm(f)),  h~^{A,E}(f) = sum_lm T^{A,E}_lm h~_lm   Eq. 7, 9
+ *   heterodyne: r = h/h0 = r0 + r1 (f - f_b);  Z[d,h], Z[h,h] from A0,A1,B0,B1     Eq. 10-19
+ * for a whole batch of parameter points ("walkers") per call, in two forms:
+ *   full-grid    (brute-force search): sparse-node amp/phase -> natural cubic spline -> dense
+ *                Fourier grid -> <d|h>, <h|h> per walker; the dense template never touches HBM.
+ *   heterodyned: template at the bin edges -> r -> r0, r1 -> contraction with
+ *                the summary data.
+ *
+ * Conventions
+ *   - Every function returns an int status (LL_OK = 0, negative = error) and never throws or aborts;
+ *     ll_last_error() gives the text of the last failure on that context.
+ *   - Pointers are marked DEV (device memory on the context's device), HOST, or PINNED (page-locked host).
+ *     The caller owns every pointer it passes.  The library copies what it keeps (pre-weighted data,
+ *     weights, summary tables) and holds no caller pointer once the stream has reached the end of the call.
+ *   - All arrays are row-major fp64.  Complex numbers are (re, im) pairs in the last axis.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Batch calls are
+ *     asynchronous on it, never synchronise, and do not allocate in steady state (scratch grows on the
+ *     first call at a larger shape; growing synchronises the device once).
+ *   - A context is not thread-safe: one context per host thread / stream.
+ *   - Non-finite inputs propagate to NaN outputs unchecked.  A walker whose band misses the grid gets
+ *     d_h = h_h = 0, log L = -1/2 <d|d>.
+ *   - There is no CPU fallback anywhere: without a CUDA device ll_create fails with LL_ERR_CUDA.
+ *
+ * Dense grid (reading R3): bin i = 0..n_f-1 has frequency f_i = (double)(k_min + i) * df.
+ * Weights (reading R4):    W_i = 4 df w_i / S_n(f_i), w_i the quadrature weight (trapezoid or rectangle).
+ * Parameter row of the stand-in waveform (reading R9; BASELINE.json config 0/3), P = 5 + 2 n_c n_m doubles:
+ *   Mc [s], q, t_c [s], phi_c [rad], 1/D, then T^c_m (re, im) mode-major, channel-minor.
+ */
+#ifndef LL_B200_H
+#define LL_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ll_ctx ll_ctx; /* opaque; owns every internal device buffer */
+
+enum {
+    LL_OK = 0,
+    LL_ERR_ARG = -1,         /* null pointer, bad size, non-ascending nodes/edges, nodes not covering the grid */
+    LL_ERR_STATE = -2,       /* ll_set_data / ll_het_prepare / ll_standin_config not called yet            */
+    LL_ERR_CUDA = -3,        /* a CUDA runtime call failed (text in ll_last_error)                         */
+    LL_ERR_NOMEM = -4,       /* device or host allocation failed                                           */
+    LL_ERR_UNSUPPORTED = -5, /* n_channels / n_modes / precision outside what is compiled in               */
+    LL_ERR_REF_ZERO = -6     /* heterodyne reference h0 is zero or non-finite at a bin edge                */
+};
+
+enum { LL_PREC_FP64 = 0, LL_PREC_FP32_ACC = 1 };
+
+#define LL_MAX_MODES 8
+#define LL_N_CHANNELS 2
+
+typedef struct {
+    int32_t device;     /* CUDA device ordinal                                                              */
+    int32_t n_channels; /* must be 2 (TDI A and E; reading R5)                                 */
+    int32_t n_modes;    /* 1..LL_MAX_MODES harmonics (l,m) summed per channel (Eq. 9)                       */
+    int32_t precision;  /* LL_PREC_FP64, or LL_PREC_FP32_ACC (full-grid path only; reading R15)             */
+    int32_t reserved[4];
+} ll_config;
+
+/* Create / destroy a context.  ll_create selects `device`, checks it is usable and allocates nothing big. */
+int ll_create(const ll_config *cfg, ll_ctx **out);
+int ll_destroy(ll_ctx *ctx);
+const char *ll_last_error(const ll_ctx *ctx);
+/* ABI version of the loaded library (bumped on any signature change). */
+int ll_abi_version(void);
+
+/* F0 — fix the data stream and the noise weights (Eq. 3; "prior to the analysis, we transform the data",
+ * PAPER.md:91).  Builds g^c_i = W_i conj(d^c_i) (interleaved [n_f][A re, A im, E re, E im]) and
+ * <d|d> = sum_c sum_i W_i |d^c_i|^2.  May be called again at any time; invalidates ll_het_prepare.
+ *   d : DEV [n_c][n_f][2]     W : DEV [n_f]                                                               */
+int ll_set_data(ll_ctx *ctx, int64_t n_f, int64_t k_min, double df, const double *d, const double *W,
+                void *stream);
+
+/* <d|d> over the whole grid and over the heterodyne band (0 before ll_het_prepare).  HOST out.
+ * Synchronises `stream` (the one the producing call ran on).                                              */
+int ll_get_dd(ll_ctx *ctx, double *dd_full, double *dd_het_band, void *stream);
+
+/* Stand-in waveform description (reading R9): modes (l,m), relative amplitudes c_lm, taper width kappa.
+ *   l, m, c_lm : HOST [n_modes]   (n_modes must equal the context's)                                      */
+int ll_standin_config(ll_ctx *ctx, int32_t n_modes, const int32_t *l, const int32_t *m, const double *c_lm,
+                      double taper_kappa);
+
+/* F2-F4 — full-grid log-likelihood of n_w walkers given node arrays (Eq. 2, 3, 7, 9; spline: reading R1).
+ *   f_nodes : HOST [n_nodes] strictly ascending, n_nodes >= 3, f_nodes[0] <= f_0, f_nodes[last] >= f_{n_f-1}
+ *   amp, phase : DEV [n_w][n_m][n_nodes]  (phase in radians; h_lm = amp exp(-i phase))
+ *   tf   : DEV [n_w][n_m][n_c][2]         transfer factors T^c_lm (Eq. 8-9 as per-walker constants, R5/R11)
+ *   band : DEV [n_w][2] (f_lo, f_hi) or NULL (whole grid); template is zero outside (reading R10)
+ *   logL, d_h, h_h : DEV [n_w]; d_h and/or h_h may be NULL.  n_w = 0 is a no-op.                          */
+int ll_full_batch(ll_ctx *ctx, int64_t n_w, int32_t n_nodes, const double *f_nodes, const double *amp,
+                  const double *phase, const double *tf, const double *band, double *logL, double *d_h,
+                  double *h_h, void *stream);
+
+/* F1-F4 — same, the node arrays produced on the device from parameter rows by the stand-in waveform.
+ *   params : DEV [n_w][P]                                                                                 */
+int ll_full_batch_standin(ll_ctx *ctx, int64_t n_w, int32_t n_nodes, const double *f_nodes,
+                          const double *params, double *logL, double *d_h, double *h_h, void *stream);
+
+/* End-to-end form of the call above: PINNED (or pageable) HOST params in, HOST results out; the H2D and D2H
+ * copies run on `stream`, which is synchronised before returning.                                         */
+int ll_full_batch_standin_host(ll_ctx *ctx, int64_t n_w, int32_t n_nodes, const double *f_nodes,
+                               const double *params_host, double *logL_host, double *d_h_host,
+                               double *h_h_host, void *stream);
+
+/* Dense template of ONE walker through the spline path (what F3 integrates, written out; setup utility
+ * used to synthesise data d = h_inj + n).   params_row : HOST [P]   h_out : DEV [n_c][n_f][2]             */
+int ll_full_template_standin(ll_ctx *ctx, int32_t n_nodes, const double *f_nodes, const double *params_row,
+                             double *h_out, void *stream);
+
+/* Stand-in template of ONE parameter row evaluated directly (no spline) at arbitrary frequencies; zero
+ * outside [f_lo, f_hi].  Used for the heterodyne reference h0 (reading R12).
+ *   params_row : HOST [P]   f : DEV [n_freq]   h_out : DEV [n_c][n_freq][2]                               */
+int ll_template_standin(ll_ctx *ctx, const double *params_row, int64_t n_freq, const double *f, double f_lo,
+                        double f_hi, double *h_out, void *stream);
+
+/* H0 — heterodyne summary data for reference template h0 on bins [e_b, e_{b+1}) (last closed), centre
+ * f_b = (e_b+e_{b+1})/2 (Eq. 15, 16, 18, 19 with 4 Delta f folded into W; readings R11-R13), 1/h0 at the
+ * edges, and <d|d> over the band.  Synchronises `stream` once (it validates h0 at the edges on the host).
+ *   f_edges : HOST [n_edges] strictly ascending, n_edges >= 2
+ *   h0_dense : DEV [n_c][n_f][2] on the ll_set_data grid      h0_edges : DEV [n_c][n_edges][2]            */
+int ll_het_prepare(ll_ctx *ctx, int32_t n_edges, const double *f_edges, const double *h0_dense,
+                   const double *h0_edges, void *stream);
+
+/* Summary data as computed by ll_het_prepare, for inspection.  HOST out, any pointer may be NULL.
+ *   A0, A1 : [n_c][n_b][2]    B0, B1 : [n_c][n_b]                                                         */
+int ll_het_get_summary(ll_ctx *ctx, double *A0, double *A1, double *B0, double *B1, void *stream);
+
+/* H1-H3 — heterodyned log-likelihood given amplitude/phase at the bin edges (Eq. 11, 14, 17).
+ *   amp_e, phase_e : DEV [n_w][n_m][n_edges]   tf : DEV [n_w][n_m][n_c][2]   outputs as ll_full_batch     */
+int ll_het_batch(ll_ctx *ctx, int64_t n_w, const double *amp_e, const double *phase_e, const double *tf,
+                 double *logL, double *d_h, double *h_h, void *stream);
+
+/* H1-H3 with the stand-in waveform evaluated at the edges on the device.   params : DEV [n_w][P]          */
+int ll_het_batch_standin(ll_ctx *ctx, int64_t n_w, const double *params, double *logL, double *d_h,
+                         double *h_h, void *stream);
+
+/* End-to-end form: HOST params in, HOST results out, copies on `stream`, synchronised before returning.   */
+int ll_het_batch_standin_host(ll_ctx *ctx, int64_t n_w, const double *params_host, double *logL_host,
+                              double *d_h_host, double *h_h_host, void *stream);
+
+/* Measurement helpers (no part of the method).
+ * ll_peak_fma: runs `iters` dependent-free FMA chains on every SM and returns the achieved rate in
+ *   FMA/s (HOST out); which = 0 -> FP64 DFMA, 1 -> FP32 FFMA.  Used for the ALU roofline denominator.
+ * ll_kernel_launches: number of kernels this context has launched since creation.
+ * ll_last_full_stats: HOST out, after the stream is idle: active (walker, bin, mode) pairs and number of
+ *   frequency tiles x walker blocks of the last full-grid call.                                           */
+int ll_peak_fma(ll_ctx *ctx, int32_t which, int64_t iters, double *fma_per_s, double *ms, void *stream);
+/* ll_profile_enable(on): while on, every full-grid call brackets its fused kernel (F3) and every heterodyned call
+ *   its batch kernel (H1-H3) with CUDA events on the call's stream (a ring of 512 pairs; enabling resets it).
+ * ll_profile_read: synchronises the recorded events and returns the summed device time in ms and the number
+ *   of bracketed launches since the last enable.  HOST out.                                                */
+int ll_profile_enable(ll_ctx *ctx, int32_t on);
+int ll_profile_read(ll_ctx *ctx, double *kernel_ms_sum, int64_t *n_launches);
+int64_t ll_kernel_launches(const ll_ctx *ctx);
+int ll_last_full_stats(ll_ctx *ctx, double *active_pairs, int64_t *n_blocks, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LL_B200_H */

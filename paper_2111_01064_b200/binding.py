@@ -1,0 +1,293 @@
+"""Thin ctypes binding over libll_b200.so — same names as include/ll.h, argument marshalling only.
+
+Every step of the path runs in the CUDA kernels behind the C ABI.  PyTorch is used for device memory
+(`tensor.data_ptr()`) and the current stream.  There is no CPU fallback: if the shared library is missing
+or no CUDA device is present the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+SO_PATH = os.path.join(_HERE, "libll_b200.so")
+
+LL_OK, LL_ERR_ARG, LL_ERR_STATE, LL_ERR_CUDA, LL_ERR_NOMEM, LL_ERR_UNSUPPORTED, LL_ERR_REF_ZERO = 0, -1, -2, -3, -4, -5, -6
+LL_PREC_FP64, LL_PREC_FP32_ACC = 0, 1
+
+# every symbol include/ll.h declares (tests/test_abi.py checks header and library against this list)
+SYMBOLS = (
+    "ll_create", "ll_destroy", "ll_last_error", "ll_abi_version", "ll_set_data", "ll_get_dd", "ll_standin_config",
+    "ll_full_batch", "ll_full_batch_standin", "ll_full_batch_standin_host", "ll_full_template_standin",
+    "ll_template_standin", "ll_het_prepare", "ll_het_get_summary", "ll_het_batch", "ll_het_batch_standin",
+    "ll_het_batch_standin_host", "ll_peak_fma", "ll_kernel_launches", "ll_last_full_stats",
+    "ll_profile_enable", "ll_profile_read",
+)
+
+
+class LLError(RuntimeError):
+    def __init__(self, code: int, what: str, text: str = ""):
+        super().__init__(f"{what} failed with status {code}" + (f": {text}" if text else ""))
+        self.code = code
+
+
+class ll_config(C.Structure):
+    _fields_ = [("device", C.c_int32), ("n_channels", C.c_int32), ("n_modes", C.c_int32), ("precision", C.c_int32),
+                ("reserved", C.c_int32 * 4)]
+
+
+_lib = None
+
+
+def load_library(path: Optional[str] = None):
+    """dlopen libll_b200.so (built by `paper_2111_01064_b200.build`); fails loudly if it is absent."""
+    global _lib
+    if _lib is not None and path is None:
+        return _lib
+    path = path or SO_PATH
+    if not os.path.exists(path):
+        raise FileNotFoundError(f"{path} not found: run `python -m paper_2111_01064_b200.build` "
+                                "(the CUDA extension is required; there is no CPU fallback)")
+    lib = C.CDLL(path)
+    vp, i64, i32, dbl = C.c_void_p, C.c_int64, C.c_int32, C.c_double
+    sig = {
+        "ll_create": (C.c_int, [C.POINTER(ll_config), C.POINTER(vp)]),
+        "ll_destroy": (C.c_int, [vp]),
+        "ll_last_error": (C.c_char_p, [vp]),
+        "ll_abi_version": (C.c_int, []),
+        "ll_set_data": (C.c_int, [vp, i64, i64, dbl, vp, vp, vp]),
+        "ll_get_dd": (C.c_int, [vp, C.POINTER(dbl), C.POINTER(dbl), vp]),
+        "ll_standin_config": (C.c_int, [vp, i32, vp, vp, vp, dbl]),
+        "ll_full_batch": (C.c_int, [vp, i64, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp]),
+        "ll_full_batch_standin": (C.c_int, [vp, i64, i32, vp, vp, vp, vp, vp, vp]),
+        "ll_full_batch_standin_host": (C.c_int, [vp, i64, i32, vp, vp, vp, vp, vp, vp]),
+        "ll_full_template_standin": (C.c_int, [vp, i32, vp, vp, vp, vp]),
+        "ll_template_standin": (C.c_int, [vp, vp, i64, vp, dbl, dbl, vp, vp]),
+        "ll_het_prepare": (C.c_int, [vp, i32, vp, vp, vp, vp]),
+        "ll_het_get_summary": (C.c_int, [vp, vp, vp, vp, vp, vp]),
+        "ll_het_batch": (C.c_int, [vp, i64, vp, vp, vp, vp, vp, vp, vp]),
+        "ll_het_batch_standin": (C.c_int, [vp, i64, vp, vp, vp, vp, vp]),
+        "ll_het_batch_standin_host": (C.c_int, [vp, i64, vp, vp, vp, vp, vp]),
+        "ll_peak_fma": (C.c_int, [vp, i32, i64, C.POINTER(dbl), C.POINTER(dbl), vp]),
+        "ll_kernel_launches": (i64, [vp]),
+        "ll_last_full_stats": (C.c_int, [vp, C.POINTER(dbl), C.POINTER(i64), vp]),
+        "ll_profile_enable": (C.c_int, [vp, i32]),
+        "ll_profile_read": (C.c_int, [vp, C.POINTER(dbl), C.POINTER(i64)]),
+    }
+    for name, (res, args) in sig.items():
+        fn = getattr(lib, name)
+        fn.restype, fn.argtypes = res, args
+    if path == SO_PATH:
+        _lib = lib
+    return lib
+
+
+def _torch():
+    import torch
+    return torch
+
+
+def _dev_ptr(t, what: str):
+    """device pointer of a contiguous float64 CUDA tensor (None -> NULL)"""
+    if t is None:
+        return None
+    torch = _torch()
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+        raise TypeError(f"{what}: need a contiguous float64 CUDA tensor")
+    return C.c_void_p(t.data_ptr())
+
+
+def _host_f64(a, what: str) -> np.ndarray:
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    if a.ndim < 1:
+        raise TypeError(f"{what}: need an array")
+    return a
+
+
+def _stream_ptr(stream=None):
+    torch = _torch()
+    s = torch.cuda.current_stream() if stream is None else stream
+    return C.c_void_p(s.cuda_stream)
+
+
+class Context:
+    """One `ll_ctx` (include/ll.h).  Methods carry the C names without the `ll_` prefix."""
+
+    def __init__(self, n_modes: int = 1, precision: int = LL_PREC_FP64, device: Optional[int] = None, n_channels: int = 2):
+        torch = _torch()
+        if not torch.cuda.is_available():
+            raise LLError(LL_ERR_CUDA, "ll_create", "no CUDA device (there is no CPU fallback)")
+        self._lib = load_library()
+        self.device = torch.cuda.current_device() if device is None else int(device)
+        self.n_modes, self.n_channels, self.precision = int(n_modes), int(n_channels), int(precision)
+        cfg = ll_config(self.device, self.n_channels, self.n_modes, self.precision, (C.c_int32 * 4)(0, 0, 0, 0))
+        h = C.c_void_p()
+        rc = self._lib.ll_create(C.byref(cfg), C.byref(h))
+        if rc != LL_OK:
+            raise LLError(rc, "ll_create")
+        self._h = h
+        self.n_f = 0
+
+    # -- plumbing
+    def _check(self, rc: int, what: str):
+        if rc != LL_OK:
+            raise LLError(rc, what, self.last_error())
+
+    def last_error(self) -> str:
+        return (self._lib.ll_last_error(self._h) or b"").decode()
+
+    def destroy(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            self._lib.ll_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    @property
+    def P(self) -> int:
+        return 5 + 2 * self.n_channels * self.n_modes
+
+    def _out(self, n_w: int, want: bool = True):
+        torch = _torch()
+        return torch.empty(n_w, dtype=torch.float64, device=f"cuda:{self.device}") if want else None
+
+    # -- F0
+    def set_data(self, n_f: int, k_min: int, df: float, d, W, stream=None):
+        self._check(self._lib.ll_set_data(self._h, n_f, k_min, df, _dev_ptr(d, "d"), _dev_ptr(W, "W"), _stream_ptr(stream)),
+                    "ll_set_data")
+        self.n_f = int(n_f)
+
+    def get_dd(self, stream=None):
+        a, b = C.c_double(), C.c_double()
+        self._check(self._lib.ll_get_dd(self._h, C.byref(a), C.byref(b), _stream_ptr(stream)), "ll_get_dd")
+        return a.value, b.value
+
+    def standin_config(self, l, m, c_lm, kappa: float):
+        l = np.ascontiguousarray(l, dtype=np.int32)
+        m = np.ascontiguousarray(m, dtype=np.int32)
+        c = _host_f64(c_lm, "c_lm")
+        self._check(self._lib.ll_standin_config(self._h, len(m), l.ctypes.data_as(C.c_void_p), m.ctypes.data_as(C.c_void_p),
+                                                c.ctypes.data_as(C.c_void_p), float(kappa)), "ll_standin_config")
+
+    # -- full-grid path
+    def full_batch(self, f_nodes, amp, phase, tf, band=None, want_parts: bool = True, stream=None):
+        f_nodes = _host_f64(f_nodes, "f_nodes")
+        n_w = int(amp.shape[0]) if amp is not None else 0
+        logL, d_h, h_h = self._out(n_w), self._out(n_w, want_parts), self._out(n_w, want_parts)
+        self._check(self._lib.ll_full_batch(self._h, n_w, len(f_nodes), f_nodes.ctypes.data_as(C.c_void_p),
+                                            _dev_ptr(amp, "amp"), _dev_ptr(phase, "phase"), _dev_ptr(tf, "tf"),
+                                            _dev_ptr(band, "band"), _dev_ptr(logL, "logL"), _dev_ptr(d_h, "d_h"),
+                                            _dev_ptr(h_h, "h_h"), _stream_ptr(stream)), "ll_full_batch")
+        return logL, d_h, h_h
+
+    def full_batch_standin(self, f_nodes, params, out=None, stream=None):
+        f_nodes = _host_f64(f_nodes, "f_nodes")
+        n_w = int(params.shape[0])
+        logL, d_h, h_h = out if out is not None else (self._out(n_w), self._out(n_w), self._out(n_w))
+        self._check(self._lib.ll_full_batch_standin(self._h, n_w, len(f_nodes), f_nodes.ctypes.data_as(C.c_void_p),
+                                                    _dev_ptr(params, "params"), _dev_ptr(logL, "logL"),
+                                                    _dev_ptr(d_h, "d_h"), _dev_ptr(h_h, "h_h"), _stream_ptr(stream)),
+                    "ll_full_batch_standin")
+        return logL, d_h, h_h
+
+    def full_batch_standin_host(self, f_nodes, params_host, out_host, stream=None):
+        """params_host, out_host = (logL, d_h, h_h): pinned CPU float64 tensors (or numpy arrays)."""
+        f_nodes = _host_f64(f_nodes, "f_nodes")
+        n_w = int(params_host.shape[0])
+        ptr = lambda t: None if t is None else C.c_void_p(t.data_ptr() if hasattr(t, "data_ptr") else t.ctypes.data)
+        self._check(self._lib.ll_full_batch_standin_host(self._h, n_w, len(f_nodes), f_nodes.ctypes.data_as(C.c_void_p),
+                                                         ptr(params_host), ptr(out_host[0]), ptr(out_host[1]),
+                                                         ptr(out_host[2]), _stream_ptr(stream)),
+                    "ll_full_batch_standin_host")
+        return out_host
+
+    def full_template_standin(self, f_nodes, params_row, stream=None):
+        torch = _torch()
+        f_nodes = _host_f64(f_nodes, "f_nodes")
+        row = _host_f64(params_row, "params_row")
+        assert row.shape == (self.P,)
+        h = torch.empty((self.n_channels, self.n_f, 2), dtype=torch.float64, device=f"cuda:{self.device}")
+        self._check(self._lib.ll_full_template_standin(self._h, len(f_nodes), f_nodes.ctypes.data_as(C.c_void_p),
+                                                       row.ctypes.data_as(C.c_void_p), _dev_ptr(h, "h"),
+                                                       _stream_ptr(stream)), "ll_full_template_standin")
+        return h
+
+    def template_standin(self, params_row, f, f_lo: float, f_hi: float, stream=None):
+        torch = _torch()
+        row = _host_f64(params_row, "params_row")
+        assert row.shape == (self.P,)
+        h = torch.empty((self.n_channels, f.shape[0], 2), dtype=torch.float64, device=f"cuda:{self.device}")
+        self._check(self._lib.ll_template_standin(self._h, row.ctypes.data_as(C.c_void_p), int(f.shape[0]), _dev_ptr(f, "f"),
+                                                  float(f_lo), float(f_hi), _dev_ptr(h, "h"), _stream_ptr(stream)),
+                    "ll_template_standin")
+        return h
+
+    # -- heterodyned path
+    def het_prepare(self, f_edges, h0_dense, h0_edges, stream=None):
+        f_edges = _host_f64(f_edges, "f_edges")
+        self._n_edges = len(f_edges)
+        self._check(self._lib.ll_het_prepare(self._h, len(f_edges), f_edges.ctypes.data_as(C.c_void_p),
+                                             _dev_ptr(h0_dense, "h0_dense"), _dev_ptr(h0_edges, "h0_edges"),
+                                             _stream_ptr(stream)), "ll_het_prepare")
+
+    def het_get_summary(self, stream=None):
+        n_b = self._n_edges - 1
+        A0, A1 = np.empty((self.n_channels, n_b, 2)), np.empty((self.n_channels, n_b, 2))
+        B0, B1 = np.empty((self.n_channels, n_b)), np.empty((self.n_channels, n_b))
+        p = lambda a: a.ctypes.data_as(C.c_void_p)
+        self._check(self._lib.ll_het_get_summary(self._h, p(A0), p(A1), p(B0), p(B1), _stream_ptr(stream)),
+                    "ll_het_get_summary")
+        return dict(A0=A0, A1=A1, B0=B0, B1=B1)
+
+    def het_batch(self, amp_e, phase_e, tf, stream=None):
+        n_w = int(amp_e.shape[0])
+        logL, d_h, h_h = self._out(n_w), self._out(n_w), self._out(n_w)
+        self._check(self._lib.ll_het_batch(self._h, n_w, _dev_ptr(amp_e, "amp_e"), _dev_ptr(phase_e, "phase_e"),
+                                           _dev_ptr(tf, "tf"), _dev_ptr(logL, "logL"), _dev_ptr(d_h, "d_h"),
+                                           _dev_ptr(h_h, "h_h"), _stream_ptr(stream)), "ll_het_batch")
+        return logL, d_h, h_h
+
+    def het_batch_standin(self, params, out=None, stream=None):
+        n_w = int(params.shape[0])
+        logL, d_h, h_h = out if out is not None else (self._out(n_w), self._out(n_w), self._out(n_w))
+        self._check(self._lib.ll_het_batch_standin(self._h, n_w, _dev_ptr(params, "params"), _dev_ptr(logL, "logL"),
+                                                   _dev_ptr(d_h, "d_h"), _dev_ptr(h_h, "h_h"), _stream_ptr(stream)),
+                    "ll_het_batch_standin")
+        return logL, d_h, h_h
+
+    def het_batch_standin_host(self, params_host, out_host, stream=None):
+        n_w = int(params_host.shape[0])
+        ptr = lambda t: None if t is None else C.c_void_p(t.data_ptr() if hasattr(t, "data_ptr") else t.ctypes.data)
+        self._check(self._lib.ll_het_batch_standin_host(self._h, n_w, ptr(params_host), ptr(out_host[0]), ptr(out_host[1]),
+                                                        ptr(out_host[2]), _stream_ptr(stream)),
+                    "ll_het_batch_standin_host")
+        return out_host
+
+    # -- measurement helpers
+    def peak_fma(self, which: int, iters: int, stream=None):
+        r, ms = C.c_double(), C.c_double()
+        self._check(self._lib.ll_peak_fma(self._h, which, iters, C.byref(r), C.byref(ms), _stream_ptr(stream)), "ll_peak_fma")
+        return r.value, ms.value
+
+    def kernel_launches(self) -> int:
+        return int(self._lib.ll_kernel_launches(self._h))
+
+    def last_full_stats(self, stream=None):
+        a, n = C.c_double(), C.c_int64()
+        self._check(self._lib.ll_last_full_stats(self._h, C.byref(a), C.byref(n), _stream_ptr(stream)), "ll_last_full_stats")
+        return a.value, n.value
+
+    def profile_enable(self, on: bool = True):
+        self._check(self._lib.ll_profile_enable(self._h, 1 if on else 0), "ll_profile_enable")
+
+    def profile_read(self):
+        ms, n = C.c_double(), C.c_int64()
+        self._check(self._lib.ll_profile_read(self._h, C.byref(ms), C.byref(n)), "ll_profile_read")
+        return ms.value, n.value

@@ -1,0 +1,885 @@
+// ll_b200.cu — host side of libll_b200.so: the C ABI of include/ll.h, workspace management, per-node-set and
+// per-reference host tables, launch shapes.  All arithmetic of the method on the batch path runs in the
+// kernels of ll_kernels.cuh; the host only builds walker-independent tables (Thomas factorisation of the
+// shared-node spline matrix, bin->interval offsets, f^(-7/6) / f^(-5/3) node tables, 1/h0 at the edges).
+//
+// Build: nvcc -O3 -std=c++17 -gencode arch=compute_100a,code=sm_100a -lineinfo -shared -Xcompiler -fPIC
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <algorithm>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "ll.h"
+#include "ll_kernels.cuh"
+
+using namespace ll;
+
+namespace {
+
+struct DevBuf {
+    void *p = nullptr;
+    size_t cap = 0;
+    cudaError_t ensure(size_t bytes)
+    {
+        if (bytes <= cap) return cudaSuccess;
+        if (p) {
+            cudaError_t e = cudaFree(p); // synchronises the device: no kernel can still be using the old block
+            p = nullptr;
+            cap = 0;
+            if (e != cudaSuccess) return e;
+        }
+        const size_t want = bytes + bytes / 8;
+        cudaError_t e = cudaMalloc(&p, want);
+        if (e != cudaSuccess) {
+            (void)cudaGetLastError();
+            e = cudaMalloc(&p, bytes);
+            if (e != cudaSuccess) { p = nullptr; return e; }
+            cap = bytes;
+            return cudaSuccess;
+        }
+        cap = want;
+        return cudaSuccess;
+    }
+    void release()
+    {
+        if (p) cudaFree(p);
+        p = nullptr;
+        cap = 0;
+    }
+    template <typename T> T *as() const { return reinterpret_cast<T *>(p); }
+};
+
+struct FullPlan {
+    int WB, TB, CH, n_tiles, n_wp, key_gran, n_keys;
+};
+
+} // namespace
+
+struct ll_ctx {
+    int device = 0, n_c = 2, n_m = 1, precision = 0;
+    int sm_count = 148;
+    std::string err;
+    int64_t launches = 0;
+
+    // F0 state
+    bool have_data = false;
+    long long n_f = 0, n_f_pad = 0, k_min = 0;
+    double df = 0.0;
+    DevBuf g4, Wd, dd_part, dd; // dd: [0] full grid, [1] het band
+    DevBuf pairs;               // unsigned long long [1]
+
+    // stand-in
+    bool have_standin = false;
+    StandinInfo si{};
+    double c_lm[kMaxModes] = {0};
+    int mode_l[kMaxModes] = {0};
+
+    // node-set cache
+    std::vector<double> nodes_host;
+    bool nodes_valid = false;
+    DevBuf node_tab; // doubles then ints
+    NodeTables nt{};
+
+    // full-grid scratch
+    DevBuf ilo_w, ihi_w, key_w, hist, perm, ilo_s, ihi_s, Y, C, TF, part, prow;
+    int last_n_blocks = 0;
+
+    // het state
+    bool have_het = false;
+    int n_e = 0;
+    DevBuf het_tab, het_raw, het_idx, het_fb;
+    HetTable ht{};
+    std::vector<double> raw_host; // [n_b][13]
+
+    // host staging for the *_host entry points
+    DevBuf stage_in, stage_out;
+
+    // optional event bracketing of the dominant kernel (ll_profile_enable)
+    bool profiling = false;
+    std::vector<cudaEvent_t> ev; // pairs
+    int ev_used = 0;             // pairs recorded since enable (ring)
+
+    int fail(int code, const std::string &msg)
+    {
+        err = msg;
+        return code;
+    }
+    int cuda_fail(const char *what, cudaError_t e)
+    {
+        err = std::string(what) + ": " + cudaGetErrorString(e);
+        (void)cudaGetLastError();
+        return (e == cudaErrorMemoryAllocation) ? LL_ERR_NOMEM : LL_ERR_CUDA;
+    }
+};
+
+namespace {
+
+struct DeviceGuard {
+    int prev = -1;
+    explicit DeviceGuard(int dev)
+    {
+        if (cudaGetDevice(&prev) != cudaSuccess) prev = -1;
+        if (prev != dev) cudaSetDevice(dev);
+        else prev = -1;
+    }
+    ~DeviceGuard()
+    {
+        if (prev >= 0) cudaSetDevice(prev);
+    }
+};
+
+#define CK(call)                                                           \
+    do {                                                                   \
+        cudaError_t e_ = (call);                                           \
+        if (e_ != cudaSuccess) return ctx->cuda_fail(#call, e_);           \
+    } while (0)
+
+#define LAUNCHED(ctx)                                                      \
+    do {                                                                   \
+        ++(ctx)->launches;                                                 \
+        cudaError_t e_ = cudaGetLastError();                               \
+        if (e_ != cudaSuccess) return (ctx)->cuda_fail("kernel launch", e_); \
+    } while (0)
+
+constexpr int kEvPairs = 512;
+
+struct ProfScope { // records an event pair around one launch when profiling is on
+    ll_ctx *ctx;
+    cudaStream_t st;
+    int slot = -1;
+    ProfScope(ll_ctx *c, cudaStream_t s) : ctx(c), st(s)
+    {
+        if (ctx->profiling && !ctx->ev.empty()) {
+            slot = ctx->ev_used % kEvPairs;
+            cudaEventRecord(ctx->ev[2 * slot], st);
+        }
+    }
+    ~ProfScope()
+    {
+        if (slot >= 0) {
+            cudaEventRecord(ctx->ev[2 * slot + 1], st);
+            ++ctx->ev_used;
+        }
+    }
+};
+
+inline int ceil_div(long long a, long long b) { return (int)((a + b - 1) / b); }
+inline long long round_up(long long a, long long b) { return (a + b - 1) / b * b; }
+
+// ---------------------------------------------------------------------------------------------------
+// Node set: everything that depends on f_nodes and the dense grid only (cached across calls)
+// ---------------------------------------------------------------------------------------------------
+int prepare_nodes(ll_ctx *ctx, int n, const double *x, cudaStream_t st)
+{
+    if (ctx->nodes_valid && (int)ctx->nodes_host.size() == n && memcmp(ctx->nodes_host.data(), x, sizeof(double) * n) == 0)
+        return LL_OK;
+    ctx->nodes_valid = false;
+    if (n < 3) return ctx->fail(LL_ERR_ARG, "n_nodes must be >= 3");
+    for (int j = 0; j + 1 < n; ++j)
+        if (!(x[j + 1] > x[j])) return ctx->fail(LL_ERR_ARG, "f_nodes must be strictly ascending and finite");
+    const double f_first = bin_freq(ctx->k_min, 0, ctx->df), f_last = bin_freq(ctx->k_min, ctx->n_f - 1, ctx->df);
+    if (!(x[0] <= f_first) || !(x[n - 1] >= f_last))
+        return ctx->fail(LL_ERR_ARG, "f_nodes do not cover the dense grid");
+    if (!(x[0] > 0.0) && ctx->have_standin) return ctx->fail(LL_ERR_ARG, "f_nodes must be positive");
+
+    const int n_m = ctx->n_m;
+    const size_t nd = (size_t)n * (7 + 3 * (size_t)n_m); // doubles (hj/invh padded to n)
+    std::vector<double> hd(nd, 0.0);
+    std::vector<int> hi(n, 0);
+    double *xj = hd.data(), *hj = xj + n, *invh = hj + n, *ta = invh + n, *tcp = ta + n, *tinv = tcp + n, *f4 = tinv + n;
+    double *cfp = f4 + n, *f2m = cfp + (size_t)n_m * n, *fm53 = f2m + (size_t)n_m * n;
+    typedef long double ld;
+    for (int j = 0; j < n; ++j) {
+        xj[j] = x[j];
+        f4[j] = 4.0 * x[j];
+    }
+    for (int j = 0; j + 1 < n; ++j) {
+        const ld h = (ld)x[j + 1] - (ld)x[j];
+        hj[j] = (double)h;
+        invh[j] = (double)(1.0L / h);
+    }
+    // Thomas factorisation of rows 1..n-2 of the natural-spline system (M_0 = M_{n-1} = 0)
+    {
+        ld cprev = 0.0L;
+        for (int j = 1; j <= n - 2; ++j) {
+            const ld hm = (ld)x[j] - (ld)x[j - 1], hp = (ld)x[j + 1] - (ld)x[j];
+            const ld a = hm / 6.0L, b = (hm + hp) / 3.0L, c = hp / 6.0L;
+            const ld den = (j == 1) ? b : b - a * cprev;
+            const ld cp = c / den;
+            ta[j] = (j == 1) ? 0.0 : (double)a;
+            tcp[j] = (double)cp;
+            tinv[j] = (double)(1.0L / den);
+            cprev = cp;
+        }
+    }
+    if (ctx->have_standin)
+        for (int m = 0; m < n_m; ++m) {
+            const ld mm = (ld)ctx->si.mode_m[m];
+            for (int j = 0; j < n; ++j) {
+                const ld f = (ld)x[j], fp = 2.0L * f / mm;
+                cfp[(size_t)m * n + j] = (double)((ld)ctx->c_lm[m] * powl(f, -7.0L / 6.0L));
+                f2m[(size_t)m * n + j] = (double)fp;
+                fm53[(size_t)m * n + j] = (double)powl(fp, -5.0L / 3.0L);
+            }
+        }
+    // bstart[j]: interval j covers dense bins [bstart[j], bstart[j+1]); lookup = largest j with x_j <= f,
+    // clamped to [0, n-2] (reading R21)
+    hi[0] = 0;
+    for (int j = 1; j <= n - 2; ++j) hi[j] = (int)first_bin_ge(x[j], ctx->k_min, ctx->n_f, ctx->df);
+    hi[n - 1] = (int)ctx->n_f;
+    for (int j = 1; j < n; ++j) hi[j] = std::max(hi[j], hi[j - 1]);
+
+    const size_t bytes_d = nd * sizeof(double), bytes_i = (size_t)n * sizeof(int);
+    CK(ctx->node_tab.ensure(bytes_d + bytes_i));
+    CK(cudaMemcpyAsync(ctx->node_tab.p, hd.data(), bytes_d, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync((char *)ctx->node_tab.p + bytes_d, hi.data(), bytes_i, cudaMemcpyHostToDevice, st));
+    CK(cudaStreamSynchronize(st)); // the host vectors above go out of scope
+    const double *b = ctx->node_tab.as<double>();
+    NodeTables &nt = ctx->nt;
+    nt.xj = b; nt.hj = b + n; nt.invh = b + 2 * n; nt.ta = b + 3 * n; nt.tcp = b + 4 * n; nt.tinv = b + 5 * n;
+    nt.f4 = b + 6 * n; nt.cfp = b + 7 * n; nt.f2m = nt.cfp + (size_t)n_m * n; nt.fm53 = nt.f2m + (size_t)n_m * n;
+    nt.bstart = reinterpret_cast<const int *>((const char *)ctx->node_tab.p + bytes_d);
+    ctx->nodes_host.assign(x, x + n);
+    ctx->nodes_valid = true;
+    return LL_OK;
+}
+
+FullPlan make_plan(const ll_ctx *ctx, long long n_w)
+{
+    FullPlan pl;
+    pl.WB = (n_w >= 4096) ? 128 : (n_w >= 1024 ? 64 : 32);
+    pl.n_wp = (int)round_up(std::max<long long>(n_w, 1), pl.WB);
+    const int n_wb = pl.n_wp / pl.WB;
+    // aim at ~16 blocks per SM over the whole grid, tiles between 64 and 4096 bins
+    const long long target = (long long)ctx->sm_count * 16;
+    long long tb = ctx->n_f * n_wb / target;
+    int TB = 64;
+    while (TB < 4096 && TB < tb) TB <<= 1;
+    pl.TB = TB;
+    pl.CH = std::min(TB, 256);
+    pl.n_tiles = ceil_div(ctx->n_f, TB);
+    pl.key_gran = std::max(1, ceil_div(ctx->n_f, 4096));
+    pl.n_keys = (int)(ctx->n_f / pl.key_gran) + 2;
+    return pl;
+}
+
+// the whole full-grid pipeline for walkers [0, n_w) given either stand-in params or caller arrays
+int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, const double *amp, const double *phase,
+             const double *tf, const double *band, double *logL, double *d_h, double *h_h, cudaStream_t st,
+             bool template_only, double *h_out)
+{
+    const bool standin = params != nullptr;
+    const int n_m = ctx->n_m;
+    const int P = 5 + 2 * kNC * n_m;
+    const FullPlan pl = make_plan(ctx, n_w);
+    const int n_wp = pl.n_wp;
+    const bool nm1 = (n_m == 1);
+    const int NQ = nm1 ? 5 : 2;
+
+    CK(ctx->ilo_w.ensure(sizeof(int) * n_wp));
+    CK(ctx->ihi_w.ensure(sizeof(int) * n_wp));
+    CK(ctx->key_w.ensure(sizeof(int) * n_wp));
+    CK(ctx->perm.ensure(sizeof(int) * n_wp));
+    CK(ctx->ilo_s.ensure(sizeof(int) * n_wp));
+    CK(ctx->ihi_s.ensure(sizeof(int) * n_wp));
+    CK(ctx->hist.ensure(sizeof(int) * 8192));
+    CK(ctx->pairs.ensure(sizeof(unsigned long long)));
+    CK(ctx->Y.ensure(sizeof(double) * (size_t)n_m * 2 * n_nodes * n_wp));
+    CK(ctx->C.ensure(sizeof(double) * (size_t)(n_nodes - 1) * n_m * 8 * n_wp));
+    CK(ctx->TF.ensure(sizeof(double) * (size_t)n_m * 4 * n_wp));
+    if (!template_only) CK(ctx->part.ensure(sizeof(double) * (size_t)pl.n_tiles * NQ * n_wp));
+
+    const GridInfo g{ctx->k_min, ctx->n_f, ctx->df};
+    CK(cudaMemsetAsync(ctx->hist.p, 0, sizeof(int) * pl.n_keys, st));
+    CK(cudaMemsetAsync(ctx->pairs.p, 0, sizeof(unsigned long long), st));
+    k_band_prep<<<ceil_div(n_w, 256), 256, 0, st>>>(standin ? 1 : 0, params, P, band, (int)n_w, g, ctx->si, pl.key_gran,
+                                                    ctx->ilo_w.as<int>(), ctx->ihi_w.as<int>(), ctx->key_w.as<int>(),
+                                                    ctx->hist.as<int>(), ctx->pairs.as<unsigned long long>());
+    LAUNCHED(ctx);
+    k_scan_hist<<<1, 1024, 0, st>>>(ctx->hist.as<int>(), pl.n_keys);
+    LAUNCHED(ctx);
+    k_scatter<<<ceil_div(n_wp, 256), 256, 0, st>>>((int)n_w, n_wp, ctx->key_w.as<int>(), ctx->ilo_w.as<int>(),
+                                                   ctx->ihi_w.as<int>(), ctx->hist.as<int>(), ctx->perm.as<int>(),
+                                                   ctx->ilo_s.as<int>(), ctx->ihi_s.as<int>());
+    LAUNCHED(ctx);
+    if (standin) {
+        dim3 grid(ceil_div(n_wp, 128), ceil_div(n_nodes, kNodesPerThread));
+        k_nodes_standin<<<grid, 128, 0, st>>>(params, P, ctx->perm.as<int>(), n_wp, n_nodes, ctx->si, ctx->nt,
+                                              ctx->Y.as<double>(), ctx->TF.as<double>());
+    } else {
+        dim3 grid(n_wp / 32, ceil_div(n_nodes, 32), n_m);
+        k_nodes_arrays<<<grid, 256, 0, st>>>(amp, phase, tf, ctx->perm.as<int>(), n_wp, n_nodes, n_m,
+                                             ctx->Y.as<double>(), ctx->TF.as<double>());
+    }
+    LAUNCHED(ctx);
+    {
+        dim3 grid(ceil_div(n_wp, 128), 2 * n_m);
+        k_spline<<<grid, 128, 0, st>>>(ctx->Y.as<double>(), ctx->C.as<double>(), n_wp, n_nodes, n_m, ctx->nt);
+        LAUNCHED(ctx);
+    }
+    FusedArgs fa;
+    fa.g4 = ctx->g4.as<double>(); fa.Wd = ctx->Wd.as<double>(); fa.C = ctx->C.as<double>(); fa.TF = ctx->TF.as<double>();
+    fa.xj = ctx->nt.xj; fa.bstart = ctx->nt.bstart; fa.ilo = ctx->ilo_s.as<int>(); fa.ihi = ctx->ihi_s.as<int>();
+    fa.part = ctx->part.as<double>(); fa.k_min = ctx->k_min; fa.df = ctx->df; fa.n_f = (int)ctx->n_f; fa.n_wp = n_wp;
+    fa.n_nodes = n_nodes; fa.n_m = n_m; fa.TB = pl.TB; fa.CH = pl.CH;
+    if (template_only) {
+        // sorted position of walker 0 of a one-walker batch is 0
+        k_full_template<<<ceil_div(ctx->n_f, 256), 256, 0, st>>>(fa, 0, h_out);
+        LAUNCHED(ctx);
+        return LL_OK;
+    }
+    {
+        dim3 grid(n_wp / pl.WB, pl.n_tiles);
+        const size_t smem = (size_t)2 * pl.CH * 40;
+        ProfScope prof(ctx, st);
+        if (nm1) k_full_fused<1><<<grid, pl.WB, smem, st>>>(fa);
+        else k_full_fused<0><<<grid, pl.WB, smem, st>>>(fa);
+        LAUNCHED(ctx);
+        ctx->last_n_blocks = (int)(grid.x * grid.y);
+    }
+    if (nm1)
+        k_finalize<1><<<ceil_div(n_wp, 128), 128, 0, st>>>(ctx->part.as<double>(), ctx->TF.as<double>(), ctx->perm.as<int>(),
+                                                           ctx->ilo_s.as<int>(), ctx->ihi_s.as<int>(), n_wp, pl.TB,
+                                                           ctx->dd.as<double>(), logL, d_h, h_h);
+    else
+        k_finalize<0><<<ceil_div(n_wp, 128), 128, 0, st>>>(ctx->part.as<double>(), ctx->TF.as<double>(), ctx->perm.as<int>(),
+                                                           ctx->ilo_s.as<int>(), ctx->ihi_s.as<int>(), n_wp, pl.TB,
+                                                           ctx->dd.as<double>(), logL, d_h, h_h);
+    LAUNCHED(ctx);
+    return LL_OK;
+}
+
+int check_full_common(ll_ctx *ctx, int64_t n_w, const double *f_nodes, const double *logL)
+{
+    if (!ctx) return LL_ERR_ARG;
+    if (n_w < 0) return ctx->fail(LL_ERR_ARG, "n_w < 0");
+    if (n_w > (1 << 24)) return ctx->fail(LL_ERR_ARG, "n_w > 2^24 per call: split the batch");
+    if (!f_nodes) return ctx->fail(LL_ERR_ARG, "f_nodes is NULL");
+    if (n_w > 0 && !logL) return ctx->fail(LL_ERR_ARG, "logL is NULL");
+    if (!ctx->have_data) return ctx->fail(LL_ERR_STATE, "ll_set_data has not been called");
+    if (ctx->precision != LL_PREC_FP64) return ctx->fail(LL_ERR_UNSUPPORTED, "FP32-accumulate variant not built yet");
+    return LL_OK;
+}
+
+// packed heterodyne table on the host
+int build_het_table(ll_ctx *ctx, int n_e, const double *e, const std::vector<double> &h0e, std::vector<double> &tab)
+{
+    typedef long double ld;
+    const int n_b = n_e - 1, n_m = ctx->n_m;
+    HetTable T;
+    T.base = nullptr; T.n_e = n_e; T.n_b = n_b; T.n_m = n_m;
+    T.total = 5 * n_e + 3 * n_m * n_e + 12 * n_b;
+    tab.assign(T.total, 0.0);
+    for (int j = 0; j < n_e; ++j) {
+        tab[T.off_f4() + j] = 4.0 * e[j];
+        for (int c = 0; c < kNC; ++c) {
+            const ld gr = h0e[((size_t)c * n_e + j) * 2], gi = h0e[((size_t)c * n_e + j) * 2 + 1];
+            const ld den = gr * gr + gi * gi;
+            if (!(den > 0.0L) || !std::isfinite((double)den)) return ctx->fail(LL_ERR_REF_ZERO, "h0 is zero or non-finite at a bin edge");
+            tab[T.off_ih0() + 4 * j + 2 * c] = (double)(gr / den);
+            tab[T.off_ih0() + 4 * j + 2 * c + 1] = (double)(-gi / den);
+        }
+        if (ctx->have_standin)
+            for (int m = 0; m < n_m; ++m) {
+                const ld f = (ld)e[j], fp = 2.0L * f / (ld)ctx->si.mode_m[m];
+                tab[T.off_cfp() + m * n_e + j] = (double)((ld)ctx->c_lm[m] * powl(f, -7.0L / 6.0L));
+                tab[T.off_f2m() + m * n_e + j] = (double)fp;
+                tab[T.off_fm53() + m * n_e + j] = (double)powl(fp, -5.0L / 3.0L);
+            }
+    }
+    const std::vector<double> &raw = ctx->raw_host;
+    for (int b = 0; b < n_b; ++b) {
+        const ld invw = 1.0L / ((ld)e[b + 1] - (ld)e[b]);
+        double *t = &tab[T.off_bins() + 12 * b];
+        const double *r = &raw[(size_t)b * 13];
+        // raw: A: (A0r, A0i, A1r, A1i, B0, B1) at 0..5, E at 6..11
+        t[0] = 0.5 * r[0]; t[1] = 0.5 * r[1]; t[2] = 0.5 * r[6]; t[3] = 0.5 * r[7];
+        t[4] = (double)((ld)r[2] * invw); t[5] = (double)((ld)r[3] * invw);
+        t[6] = (double)((ld)r[8] * invw); t[7] = (double)((ld)r[9] * invw);
+        t[8] = 0.25 * r[4]; t[9] = 0.25 * r[10];
+        t[10] = (double)((ld)r[5] * invw); t[11] = (double)((ld)r[11] * invw);
+    }
+    ctx->ht = T;
+    return LL_OK;
+}
+
+int het_check(ll_ctx *ctx, int64_t n_w, const double *logL)
+{
+    if (!ctx) return LL_ERR_ARG;
+    if (n_w < 0) return ctx->fail(LL_ERR_ARG, "n_w < 0");
+    if (n_w > (1LL << 30)) return ctx->fail(LL_ERR_ARG, "n_w too large");
+    if (n_w > 0 && !logL) return ctx->fail(LL_ERR_ARG, "logL is NULL");
+    if (!ctx->have_data) return ctx->fail(LL_ERR_STATE, "ll_set_data has not been called");
+    if (!ctx->have_het) return ctx->fail(LL_ERR_STATE, "ll_het_prepare has not been called");
+    return LL_OK;
+}
+
+template <int NM>
+int launch_het_standin(ll_ctx *ctx, int64_t n_w, const double *params, double *logL, double *d_h, double *h_h,
+                       cudaStream_t st)
+{
+    const int n_groups = ceil_div(n_w, 32);
+    // enough warps to fill the chip: split the bins over S warps when the batch is small
+    int S = 1;
+    while (S < 16 && (long long)n_groups * S < (long long)ctx->sm_count * 16 && ctx->ht.n_b / (2 * S) >= 4) S <<= 1;
+    const size_t smem = sizeof(double) * ((size_t)ctx->ht.total + (size_t)S * 64);
+    static bool attr_set = false;
+    if (!attr_set) {
+        CK(cudaFuncSetAttribute(k_het_standin<NM>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+        attr_set = true;
+    }
+    if (smem > 227 * 1024) return ctx->fail(LL_ERR_UNSUPPORTED, "heterodyne tables exceed shared memory (too many bins x modes)");
+    int blocks_per_sm = std::max(1, std::min(8, (int)((220 * 1024) / std::max<size_t>(smem, 1))));
+    int grid = std::min(n_groups, ctx->sm_count * blocks_per_sm);
+    const int P = 5 + 2 * kNC * ctx->n_m;
+    ProfScope prof(ctx, st);
+    k_het_standin<NM><<<grid, dim3(32, S), smem, st>>>(ctx->ht, ctx->si, params, P, (int)n_w, n_groups,
+                                                         ctx->dd.as<double>(), logL, d_h, h_h);
+    LAUNCHED(ctx);
+    return LL_OK;
+}
+
+} // namespace
+
+// =====================================================================================================
+// C ABI
+// =====================================================================================================
+extern "C" {
+
+int ll_abi_version(void) { return 1; }
+
+int ll_create(const ll_config *cfg, ll_ctx **out)
+{
+    if (!cfg || !out) return LL_ERR_ARG;
+    *out = nullptr;
+    if (cfg->n_channels != LL_N_CHANNELS) return LL_ERR_UNSUPPORTED;
+    if (cfg->n_modes < 1 || cfg->n_modes > LL_MAX_MODES) return LL_ERR_UNSUPPORTED;
+    if (cfg->precision != LL_PREC_FP64 && cfg->precision != LL_PREC_FP32_ACC) return LL_ERR_UNSUPPORTED;
+    int n_dev = 0;
+    if (cudaGetDeviceCount(&n_dev) != cudaSuccess || cfg->device < 0 || cfg->device >= n_dev) {
+        (void)cudaGetLastError();
+        return LL_ERR_CUDA; // no CUDA device: there is no CPU fallback
+    }
+    ll_ctx *ctx = new (std::nothrow) ll_ctx();
+    if (!ctx) return LL_ERR_NOMEM;
+    ctx->device = cfg->device;
+    ctx->n_c = cfg->n_channels;
+    ctx->n_m = cfg->n_modes;
+    ctx->precision = cfg->precision;
+    DeviceGuard dg(ctx->device);
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, ctx->device) != cudaSuccess) {
+        delete ctx;
+        return LL_ERR_CUDA;
+    }
+    if (prop.major < 10) { // the only SASS in this library is sm_100a
+        delete ctx;
+        return LL_ERR_UNSUPPORTED;
+    }
+    ctx->sm_count = prop.multiProcessorCount;
+    // default stand-in description: the (2,2) mode only, kappa = 1/2; overwritten by ll_standin_config
+    ctx->si.n_m = ctx->n_m;
+    ctx->si.kappa = 0.5;
+    *out = ctx;
+    return LL_OK;
+}
+
+int ll_destroy(ll_ctx *ctx)
+{
+    if (!ctx) return LL_ERR_ARG;
+    {
+        DeviceGuard dg(ctx->device);
+        cudaDeviceSynchronize();
+        DevBuf *all[] = {&ctx->g4, &ctx->Wd, &ctx->dd_part, &ctx->dd, &ctx->pairs, &ctx->node_tab, &ctx->ilo_w, &ctx->ihi_w,
+                         &ctx->key_w, &ctx->hist, &ctx->perm, &ctx->ilo_s, &ctx->ihi_s, &ctx->Y, &ctx->C, &ctx->TF,
+                         &ctx->part, &ctx->prow, &ctx->het_tab, &ctx->het_raw, &ctx->het_idx, &ctx->het_fb,
+                         &ctx->stage_in, &ctx->stage_out};
+        for (DevBuf *b : all) b->release();
+        for (auto &e : ctx->ev) cudaEventDestroy(e);
+    }
+    delete ctx;
+    return LL_OK;
+}
+
+const char *ll_last_error(const ll_ctx *ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+
+int64_t ll_kernel_launches(const ll_ctx *ctx) { return ctx ? ctx->launches : 0; }
+
+int ll_set_data(ll_ctx *ctx, int64_t n_f, int64_t k_min, double df, const double *d, const double *W, void *stream)
+{
+    if (!ctx) return LL_ERR_ARG;
+    if (!d || !W) return ctx->fail(LL_ERR_ARG, "d or W is NULL");
+    if (n_f < 1 || n_f > (1LL << 30)) return ctx->fail(LL_ERR_ARG, "n_f out of range [1, 2^30]");
+    if (k_min < 0 || !(df > 0.0) || !std::isfinite(df)) return ctx->fail(LL_ERR_ARG, "k_min < 0 or df not positive");
+    DeviceGuard dg(ctx->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    ctx->have_data = false;
+    ctx->have_het = false;
+    ctx->nodes_valid = false;
+    const long long n_pad = round_up(n_f, 512);
+    CK(ctx->g4.ensure(sizeof(double) * 4 * n_pad));
+    CK(ctx->Wd.ensure(sizeof(double) * n_pad));
+    CK(ctx->dd.ensure(sizeof(double) * 2));
+    const int nb = std::min(1024, ceil_div(n_f, 256));
+    CK(ctx->dd_part.ensure(sizeof(double) * 1024));
+    CK(cudaMemsetAsync(ctx->g4.as<double>() + 4 * n_f, 0, sizeof(double) * 4 * (n_pad - n_f), st));
+    CK(cudaMemsetAsync(ctx->Wd.as<double>() + n_f, 0, sizeof(double) * (n_pad - n_f), st));
+    CK(cudaMemsetAsync(ctx->dd.p, 0, sizeof(double) * 2, st));
+    k_preweight<<<nb, 256, 0, st>>>(d, W, n_f, ctx->g4.as<double>(), ctx->Wd.as<double>(), ctx->dd_part.as<double>());
+    LAUNCHED(ctx);
+    k_sum_parts<<<1, 256, 0, st>>>(ctx->dd_part.as<double>(), nb, ctx->dd.as<double>());
+    LAUNCHED(ctx);
+    ctx->n_f = n_f;
+    ctx->n_f_pad = n_pad;
+    ctx->k_min = k_min;
+    ctx->df = df;
+    ctx->have_data = true;
+    return LL_OK;
+}
+
+int ll_get_dd(ll_ctx *ctx, double *dd_full, double *dd_het_band, void *stream)
+{
+    if (!ctx) return LL_ERR_ARG;
+    if (!ctx->have_data) return ctx->fail(LL_ERR_STATE, "ll_set_data has not been called");
+    DeviceGuard dg(ctx->device);
+    double h[2];
+    CK(cudaMemcpyAsync(h, ctx->dd.p, sizeof(h), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+    CK(cudaStreamSynchronize((cudaStream_t)stream));
+    if (dd_full) *dd_full = h[0];
+    if (dd_het_band) *dd_het_band = h[1];
+    return LL_OK;
+}
+
+int ll_standin_config(ll_ctx *ctx, int32_t n_modes, const int32_t *l, const int32_t *m, const double *c_lm, double taper_kappa)
+{
+    if (!ctx) return LL_ERR_ARG;
+    if (!l || !m || !c_lm) return ctx->fail(LL_ERR_ARG, "l, m or c_lm is NULL");
+    if (n_modes != ctx->n_m) return ctx->fail(LL_ERR_ARG, "n_modes differs from the context's");
+    if (!(taper_kappa > 0.0) || !std::isfinite(taper_kappa)) return ctx->fail(LL_ERR_ARG, "taper_kappa must be positive");
+    int m_max = 0;
+    for (int i = 0; i < n_modes; ++i) {
+        if (m[i] < 1 || l[i] < m[i]) return ctx->fail(LL_ERR_ARG, "need 1 <= m <= l");
+        m_max = std::max(m_max, (int)m[i]);
+    }
+    ctx->si.n_m = n_modes;
+    ctx->si.m_max = m_max;
+    ctx->si.kappa = taper_kappa;
+    for (int i = 0; i < kMaxModes; ++i) {
+        ctx->si.mode_m[i] = i < n_modes ? m[i] : 2;
+        ctx->mode_l[i] = i < n_modes ? l[i] : 2;
+        ctx->c_lm[i] = i < n_modes ? c_lm[i] : 0.0;
+    }
+    ctx->have_standin = true;
+    ctx->nodes_valid = false; // node tables carry c_lm and m
+    ctx->have_het = false;
+    return LL_OK;
+}
+
+int ll_full_batch(ll_ctx *ctx, int64_t n_w, int32_t n_nodes, const double *f_nodes, const double *amp, const double *phase,
+                  const double *tf, const double *band, double *logL, double *d_h, double *h_h, void *stream)
+{
+    int rc = check_full_common(ctx, n_w, f_nodes, logL);
+    if (rc != LL_OK) return rc;
+    if (n_w > 0 && (!amp || !phase || !tf)) return ctx->fail(LL_ERR_ARG, "amp, phase or tf is NULL");
+    DeviceGuard dg(ctx->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    rc = prepare_nodes(ctx, n_nodes, f_nodes, st);
+    if (rc != LL_OK) return rc;
+    if (n_w == 0) return LL_OK;
+    return run_full(ctx, n_w, n_nodes, nullptr, amp, phase, tf, band, logL, d_h, h_h, st, false, nullptr);
+}
+
+int ll_full_batch_standin(ll_ctx *ctx, int64_t n_w, int32_t n_nodes, const double *f_nodes, const double *params,
+                          double *logL, double *d_h, double *h_h, void *stream)
+{
+    int rc = check_full_common(ctx, n_w, f_nodes, logL);
+    if (rc != LL_OK) return rc;
+    if (!ctx->have_standin) return ctx->fail(LL_ERR_STATE, "ll_standin_config has not been called");
+    if (n_w > 0 && !params) return ctx->fail(LL_ERR_ARG, "params is NULL");
+    DeviceGuard dg(ctx->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    rc = prepare_nodes(ctx, n_nodes, f_nodes, st);
+    if (rc != LL_OK) return rc;
+    if (n_w == 0) return LL_OK;
+    return run_full(ctx, n_w, n_nodes, params, nullptr, nullptr, nullptr, nullptr, logL, d_h, h_h, st, false, nullptr);
+}
+
+int ll_full_batch_standin_host(ll_ctx *ctx, int64_t n_w, int32_t n_nodes, const double *f_nodes, const double *params_host,
+                               double *logL_host, double *d_h_host, double *h_h_host, void *stream)
+{
+    int rc = check_full_common(ctx, n_w, f_nodes, logL_host);
+    if (rc != LL_OK) return rc;
+    if (n_w == 0) return ll_full_batch_standin(ctx, 0, n_nodes, f_nodes, params_host, logL_host, d_h_host, h_h_host, stream);
+    if (!params_host) return ctx->fail(LL_ERR_ARG, "params_host is NULL");
+    DeviceGuard dg(ctx->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t P = 5 + 2 * kNC * (size_t)ctx->n_m;
+    CK(ctx->stage_in.ensure(sizeof(double) * P * n_w));
+    CK(ctx->stage_out.ensure(sizeof(double) * 3 * n_w));
+    CK(cudaMemcpyAsync(ctx->stage_in.p, params_host, sizeof(double) * P * n_w, cudaMemcpyHostToDevice, st));
+    double *o = ctx->stage_out.as<double>();
+    rc = ll_full_batch_standin(ctx, n_w, n_nodes, f_nodes, ctx->stage_in.as<double>(), o, o + n_w, o + 2 * n_w, stream);
+    if (rc != LL_OK) return rc;
+    CK(cudaMemcpyAsync(logL_host, o, sizeof(double) * n_w, cudaMemcpyDeviceToHost, st));
+    if (d_h_host) CK(cudaMemcpyAsync(d_h_host, o + n_w, sizeof(double) * n_w, cudaMemcpyDeviceToHost, st));
+    if (h_h_host) CK(cudaMemcpyAsync(h_h_host, o + 2 * n_w, sizeof(double) * n_w, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    return LL_OK;
+}
+
+int ll_full_template_standin(ll_ctx *ctx, int32_t n_nodes, const double *f_nodes, const double *params_row, double *h_out,
+                             void *stream)
+{
+    if (!ctx) return LL_ERR_ARG;
+    if (!f_nodes || !params_row || !h_out) return ctx->fail(LL_ERR_ARG, "NULL argument");
+    if (!ctx->have_data) return ctx->fail(LL_ERR_STATE, "ll_set_data has not been called (it fixes the dense grid)");
+    if (!ctx->have_standin) return ctx->fail(LL_ERR_STATE, "ll_standin_config has not been called");
+    DeviceGuard dg(ctx->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc = prepare_nodes(ctx, n_nodes, f_nodes, st);
+    if (rc != LL_OK) return rc;
+    const size_t P = 5 + 2 * kNC * (size_t)ctx->n_m;
+    CK(ctx->prow.ensure(sizeof(double) * P));
+    CK(cudaMemcpyAsync(ctx->prow.p, params_row, sizeof(double) * P, cudaMemcpyHostToDevice, st));
+    CK(cudaStreamSynchronize(st)); // params_row is pageable caller memory
+    return run_full(ctx, 1, n_nodes, ctx->prow.as<double>(), nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, st,
+                    true, h_out);
+}
+
+int ll_template_standin(ll_ctx *ctx, const double *params_row, int64_t n_freq, const double *f, double f_lo, double f_hi,
+                        double *h_out, void *stream)
+{
+    if (!ctx) return LL_ERR_ARG;
+    if (!params_row || (n_freq > 0 && (!f || !h_out))) return ctx->fail(LL_ERR_ARG, "NULL argument");
+    if (n_freq < 0) return ctx->fail(LL_ERR_ARG, "n_freq < 0");
+    if (!ctx->have_standin) return ctx->fail(LL_ERR_STATE, "ll_standin_config has not been called");
+    if (n_freq == 0) return LL_OK;
+    DeviceGuard dg(ctx->device);
+    DirectRow row;
+    memset(&row, 0, sizeof(row));
+    const int P = 5 + 2 * kNC * ctx->n_m;
+    memcpy(row.p, params_row, sizeof(double) * P);
+    memcpy(row.c_lm, ctx->c_lm, sizeof(row.c_lm));
+    k_template_direct<<<ceil_div(n_freq, 256), 256, 0, (cudaStream_t)stream>>>(row, ctx->si, n_freq, f, f_lo, f_hi, h_out);
+    LAUNCHED(ctx);
+    return LL_OK;
+}
+
+int ll_het_prepare(ll_ctx *ctx, int32_t n_edges, const double *f_edges, const double *h0_dense, const double *h0_edges,
+                   void *stream)
+{
+    if (!ctx) return LL_ERR_ARG;
+    if (!f_edges || !h0_dense || !h0_edges) return ctx->fail(LL_ERR_ARG, "NULL argument");
+    if (n_edges < 2 || n_edges > 65536) return ctx->fail(LL_ERR_ARG, "n_edges out of range [2, 65536]");
+    for (int j = 0; j + 1 < n_edges; ++j)
+        if (!(f_edges[j + 1] > f_edges[j])) return ctx->fail(LL_ERR_ARG, "f_edges must be strictly ascending and finite");
+    if (!ctx->have_data) return ctx->fail(LL_ERR_STATE, "ll_set_data has not been called");
+    DeviceGuard dg(ctx->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    ctx->have_het = false;
+    const int n_e = n_edges, n_b = n_e - 1;
+    // bin membership [e_b, e_{b+1}), last bin closed (reading R13), with the grid's own frequencies
+    std::vector<int> es(n_e);
+    std::vector<double> fb(n_b);
+    for (int b = 0; b < n_b; ++b) {
+        es[b] = (int)first_bin_ge(f_edges[b], ctx->k_min, ctx->n_f, ctx->df);
+        fb[b] = (double)(0.5L * ((long double)f_edges[b] + (long double)f_edges[b + 1]));
+    }
+    es[n_b] = (int)first_bin_gt(f_edges[n_b], ctx->k_min, ctx->n_f, ctx->df);
+    CK(ctx->het_idx.ensure(sizeof(int) * n_e));
+    CK(ctx->het_fb.ensure(sizeof(double) * n_b));
+    CK(ctx->het_raw.ensure(sizeof(double) * 13 * n_b));
+    CK(cudaMemcpyAsync(ctx->het_idx.p, es.data(), sizeof(int) * n_e, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(ctx->het_fb.p, fb.data(), sizeof(double) * n_b, cudaMemcpyHostToDevice, st));
+    const GridInfo g{ctx->k_min, ctx->n_f, ctx->df};
+    k_het_prepare<<<n_b, 256, 0, st>>>(ctx->g4.as<double>(), ctx->Wd.as<double>(), h0_dense, g, ctx->het_idx.as<int>(),
+                                       ctx->het_fb.as<double>(), ctx->het_raw.as<double>());
+    LAUNCHED(ctx);
+    ctx->raw_host.assign((size_t)13 * n_b, 0.0);
+    std::vector<double> h0e((size_t)kNC * n_e * 2);
+    CK(cudaMemcpyAsync(ctx->raw_host.data(), ctx->het_raw.p, sizeof(double) * 13 * n_b, cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(h0e.data(), h0_edges, sizeof(double) * h0e.size(), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    std::vector<double> tab;
+    int rc = build_het_table(ctx, n_e, f_edges, h0e, tab);
+    if (rc != LL_OK) return rc;
+    // <d|d> over the band: bins in a fixed order, compensated
+    long double ddb = 0.0L;
+    for (int b = 0; b < n_b; ++b) ddb += (long double)ctx->raw_host[(size_t)b * 13 + 12];
+    const double ddb_d = (double)ddb;
+    CK(ctx->het_tab.ensure(sizeof(double) * tab.size()));
+    CK(cudaMemcpyAsync(ctx->het_tab.p, tab.data(), sizeof(double) * tab.size(), cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(ctx->dd.as<double>() + 1, &ddb_d, sizeof(double), cudaMemcpyHostToDevice, st));
+    CK(cudaStreamSynchronize(st));
+    ctx->ht.base = ctx->het_tab.as<double>();
+    ctx->n_e = n_e;
+    ctx->have_het = true;
+    return LL_OK;
+}
+
+int ll_het_get_summary(ll_ctx *ctx, double *A0, double *A1, double *B0, double *B1, void *stream)
+{
+    (void)stream;
+    if (!ctx) return LL_ERR_ARG;
+    if (!ctx->have_het) return ctx->fail(LL_ERR_STATE, "ll_het_prepare has not been called");
+    const int n_b = ctx->n_e - 1;
+    for (int c = 0; c < kNC; ++c)
+        for (int b = 0; b < n_b; ++b) {
+            const double *r = &ctx->raw_host[(size_t)b * 13 + 6 * c];
+            if (A0) { A0[((size_t)c * n_b + b) * 2] = r[0]; A0[((size_t)c * n_b + b) * 2 + 1] = r[1]; }
+            if (A1) { A1[((size_t)c * n_b + b) * 2] = r[2]; A1[((size_t)c * n_b + b) * 2 + 1] = r[3]; }
+            if (B0) B0[(size_t)c * n_b + b] = r[4];
+            if (B1) B1[(size_t)c * n_b + b] = r[5];
+        }
+    return LL_OK;
+}
+
+int ll_het_batch(ll_ctx *ctx, int64_t n_w, const double *amp_e, const double *phase_e, const double *tf, double *logL,
+                 double *d_h, double *h_h, void *stream)
+{
+    int rc = het_check(ctx, n_w, logL);
+    if (rc != LL_OK) return rc;
+    if (n_w == 0) return LL_OK;
+    if (!amp_e || !phase_e || !tf) return ctx->fail(LL_ERR_ARG, "amp_e, phase_e or tf is NULL");
+    DeviceGuard dg(ctx->device);
+    const size_t smem = sizeof(double) * (size_t)ctx->ht.total;
+    if (smem > 227 * 1024) return ctx->fail(LL_ERR_UNSUPPORTED, "heterodyne tables exceed shared memory");
+    static bool attr_set = false;
+    if (!attr_set) {
+        CK(cudaFuncSetAttribute(k_het_arrays, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+        attr_set = true;
+    }
+    const int wpb = 8;
+    int blocks_per_sm = std::max(1, std::min(8, (int)((220 * 1024) / std::max<size_t>(smem, 1))));
+    const int grid = std::min(ceil_div(n_w, wpb), ctx->sm_count * blocks_per_sm);
+    ProfScope prof(ctx, (cudaStream_t)stream);
+    k_het_arrays<<<grid, wpb * 32, smem, (cudaStream_t)stream>>>(ctx->ht, amp_e, phase_e, tf, (int)n_w, ctx->dd.as<double>(),
+                                                                  logL, d_h, h_h);
+    LAUNCHED(ctx);
+    return LL_OK;
+}
+
+int ll_het_batch_standin(ll_ctx *ctx, int64_t n_w, const double *params, double *logL, double *d_h, double *h_h, void *stream)
+{
+    int rc = het_check(ctx, n_w, logL);
+    if (rc != LL_OK) return rc;
+    if (!ctx->have_standin) return ctx->fail(LL_ERR_STATE, "ll_standin_config has not been called");
+    if (n_w == 0) return LL_OK;
+    if (!params) return ctx->fail(LL_ERR_ARG, "params is NULL");
+    DeviceGuard dg(ctx->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    switch (ctx->n_m) {
+    case 1: return launch_het_standin<1>(ctx, n_w, params, logL, d_h, h_h, st);
+    case 2: return launch_het_standin<2>(ctx, n_w, params, logL, d_h, h_h, st);
+    case 3: return launch_het_standin<3>(ctx, n_w, params, logL, d_h, h_h, st);
+    case 4: return launch_het_standin<4>(ctx, n_w, params, logL, d_h, h_h, st);
+    case 5: return launch_het_standin<5>(ctx, n_w, params, logL, d_h, h_h, st);
+    case 6: return launch_het_standin<6>(ctx, n_w, params, logL, d_h, h_h, st);
+    case 7: return launch_het_standin<7>(ctx, n_w, params, logL, d_h, h_h, st);
+    case 8: return launch_het_standin<8>(ctx, n_w, params, logL, d_h, h_h, st);
+    default: return ctx->fail(LL_ERR_UNSUPPORTED, "n_modes");
+    }
+}
+
+int ll_het_batch_standin_host(ll_ctx *ctx, int64_t n_w, const double *params_host, double *logL_host, double *d_h_host,
+                              double *h_h_host, void *stream)
+{
+    int rc = het_check(ctx, n_w, logL_host);
+    if (rc != LL_OK) return rc;
+    if (n_w == 0) return LL_OK;
+    if (!params_host) return ctx->fail(LL_ERR_ARG, "params_host is NULL");
+    DeviceGuard dg(ctx->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t P = 5 + 2 * kNC * (size_t)ctx->n_m;
+    CK(ctx->stage_in.ensure(sizeof(double) * P * n_w));
+    CK(ctx->stage_out.ensure(sizeof(double) * 3 * n_w));
+    CK(cudaMemcpyAsync(ctx->stage_in.p, params_host, sizeof(double) * P * n_w, cudaMemcpyHostToDevice, st));
+    double *o = ctx->stage_out.as<double>();
+    rc = ll_het_batch_standin(ctx, n_w, ctx->stage_in.as<double>(), o, o + n_w, o + 2 * n_w, stream);
+    if (rc != LL_OK) return rc;
+    CK(cudaMemcpyAsync(logL_host, o, sizeof(double) * n_w, cudaMemcpyDeviceToHost, st));
+    if (d_h_host) CK(cudaMemcpyAsync(d_h_host, o + n_w, sizeof(double) * n_w, cudaMemcpyDeviceToHost, st));
+    if (h_h_host) CK(cudaMemcpyAsync(h_h_host, o + 2 * n_w, sizeof(double) * n_w, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    return LL_OK;
+}
+
+int ll_peak_fma(ll_ctx *ctx, int32_t which, int64_t iters, double *fma_per_s, double *ms_out, void *stream)
+{
+    if (!ctx) return LL_ERR_ARG;
+    if (iters < 1 || (which != 0 && which != 1)) return ctx->fail(LL_ERR_ARG, "bad which/iters");
+    DeviceGuard dg(ctx->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    CK(ctx->prow.ensure(256));
+    cudaEvent_t e0, e1;
+    CK(cudaEventCreate(&e0));
+    CK(cudaEventCreate(&e1));
+    const int blocks = ctx->sm_count * 8, threads = 256;
+    for (int rep = 0; rep < 2; ++rep) { // first pass warms up
+        CK(cudaEventRecord(e0, st));
+        if (which == 0) k_peak_fma<double><<<blocks, threads, 0, st>>>(iters, ctx->prow.as<double>());
+        else k_peak_fma<float><<<blocks, threads, 0, st>>>(iters, ctx->prow.as<float>());
+        LAUNCHED(ctx);
+        CK(cudaEventRecord(e1, st));
+        CK(cudaEventSynchronize(e1));
+    }
+    float ms = 0.f;
+    CK(cudaEventElapsedTime(&ms, e0, e1));
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    const double n_fma = (double)blocks * threads * (double)iters * 32.0;
+    if (fma_per_s) *fma_per_s = n_fma / (ms * 1e-3);
+    if (ms_out) *ms_out = ms;
+    return LL_OK;
+}
+
+int ll_profile_enable(ll_ctx *ctx, int32_t on)
+{
+    if (!ctx) return LL_ERR_ARG;
+    DeviceGuard dg(ctx->device);
+    if (on && ctx->ev.empty()) {
+        ctx->ev.resize(2 * kEvPairs);
+        for (auto &e : ctx->ev) CK(cudaEventCreate(&e));
+    }
+    ctx->profiling = on != 0;
+    ctx->ev_used = 0;
+    return LL_OK;
+}
+
+int ll_profile_read(ll_ctx *ctx, double *kernel_ms_sum, int64_t *n_launches)
+{
+    if (!ctx) return LL_ERR_ARG;
+    DeviceGuard dg(ctx->device);
+    double sum = 0.0;
+    const int n = std::min(ctx->ev_used, kEvPairs);
+    for (int i = 0; i < n; ++i) {
+        float ms = 0.f;
+        CK(cudaEventSynchronize(ctx->ev[2 * i + 1]));
+        CK(cudaEventElapsedTime(&ms, ctx->ev[2 * i], ctx->ev[2 * i + 1]));
+        sum += ms;
+    }
+    if (kernel_ms_sum) *kernel_ms_sum = sum;
+    if (n_launches) *n_launches = n;
+    return LL_OK;
+}
+
+int ll_last_full_stats(ll_ctx *ctx, double *active_pairs, int64_t *n_blocks, void *stream)
+{
+    if (!ctx) return LL_ERR_ARG;
+    if (!ctx->pairs.p) return ctx->fail(LL_ERR_STATE, "no full-grid call yet");
+    DeviceGuard dg(ctx->device);
+    unsigned long long v = 0;
+    CK(cudaMemcpyAsync(&v, ctx->pairs.p, sizeof(v), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+    CK(cudaStreamSynchronize((cudaStream_t)stream));
+    if (active_pairs) *active_pairs = (double)v;
+    if (n_blocks) *n_blocks = ctx->last_n_blocks;
+    return LL_OK;
+}
+
+} // extern "C"

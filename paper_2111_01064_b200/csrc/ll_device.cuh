@@ -1,0 +1,172 @@
+// ll_device.cuh — device-side arithmetic building blocks of libll_b200 (sm_100a only).
+//
+// Nothing here is shared with oracle/: the oracle evaluates sinl/cosl of radians in long double, this
+// file reduces the phase in *quarter cycles* (the spline is set up on phase * 2/pi) with the
+// round-to-integer magic constant and evaluates two short Horner polynomials on the FP64 pipe.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace ll {
+
+constexpr double kMagic = 6755399441055744.0;        // 1.5 * 2^52: (y + kMagic) - kMagic == rint(y), |y| < 2^51
+constexpr double kTwoOverPi = 0x1.45f306dc9c883p-1;
+constexpr double kPi = 3.14159265358979323846;
+constexpr double kPio2_1 = 0x1.921fb54442d18p+0;     // pi/2 split in three doubles (Cody-Waite with FMA)
+constexpr double kPio2_2 = 0x1.1a62633145c07p-54;
+constexpr double kPio2_3 = -0x1.f1976b7ed8fbcp-110;
+constexpr double kSixth = 0x1.5555555555555p-3;
+
+// sin(pi r/2) = r * S(r^2), cos(pi r/2) = C(r^2), |r| <= 1/2: Taylor series of the scaled argument,
+// coefficients rounded from 50-digit values; truncation + coefficient error < 1e-16 (sin), 3e-17 (cos).
+__device__ __forceinline__ void sincos_poly_qc(double r, double &s, double &c)
+{
+    const double r2 = r * r;
+    double ps = -0x1.6fadb9f155744p-31;
+    ps = fma(ps, r2, 0x1.e8f434d018d63p-25);
+    ps = fma(ps, r2, -0x1.e3074fde8871fp-19);
+    ps = fma(ps, r2, 0x1.50783487ee782p-13);
+    ps = fma(ps, r2, -0x1.32d2cce62bd86p-8);
+    ps = fma(ps, r2, 0x1.466bc6775aae2p-4);
+    ps = fma(ps, r2, -0x1.4abbce625be53p-1);
+    ps = fma(ps, r2, 0x1.921fb54442d18p+0);
+    double pc = 0x1.20c62c2f2d7f5p-34;
+    pc = fma(pc, r2, -0x1.b6e24f44b128fp-28);
+    pc = fma(pc, r2, 0x1.f9d38a3763cc3p-22);
+    pc = fma(pc, r2, -0x1.a6d1f2a204a8cp-16);
+    pc = fma(pc, r2, 0x1.e1f506891babbp-11);
+    pc = fma(pc, r2, -0x1.55d3c7e3cbffap-6);
+    pc = fma(pc, r2, 0x1.03c1f081b5ac4p-2);
+    pc = fma(pc, r2, -0x1.3bd3cc9be45dep+0);
+    pc = fma(pc, r2, 1.0);
+    s = ps * r;
+    c = pc;
+}
+
+// quadrant bookkeeping: angle = (pi/2)(n + r); q = n mod 4
+__device__ __forceinline__ void quadrant_fix(int q, double s, double c, double &sn, double &cs)
+{
+    const double a = (q & 1) ? c : s;
+    const double b = (q & 1) ? s : c;
+    sn = (q & 2) ? -a : a;
+    cs = ((q + 1) & 2) ? -b : b;
+}
+
+// sin and cos of an angle given in quarter cycles (y = angle * 2/pi).
+__device__ __forceinline__ void sincos_qc(double y, double &sn, double &cs)
+{
+    const double sh = __dadd_rn(y, kMagic);
+    const int q = __double2loint(sh);
+    const double nd = __dadd_rn(sh, -kMagic);
+    const double r = __dadd_rn(y, -nd);
+    double s, c;
+    sincos_poly_qc(r, s, c);
+    quadrant_fix(q, s, c, sn, cs);
+}
+
+// sin and cos of an angle in radians, accurate for |x| up to ~1e9 (three-term Cody-Waite with FMA; the
+// reduced argument is then handed to the quarter-cycle polynomials).
+__device__ __forceinline__ void sincos_rad(double x, double &sn, double &cs)
+{
+    const double sh = __dadd_rn(x * kTwoOverPi, kMagic);
+    const int q = __double2loint(sh);
+    const double nd = __dadd_rn(sh, -kMagic);
+    double r = fma(-nd, kPio2_1, x);
+    r = fma(-nd, kPio2_2, r);
+    r = fma(-nd, kPio2_3, r);
+    double s, c;
+    sincos_poly_qc(r * kTwoOverPi, s, c);
+    quadrant_fix(q, s, c, sn, cs);
+}
+
+// taper(x) = 1 (x <= 1); s^3 (10 - 15 s + 6 s^2), s = (1 + kappa - x)/kappa (1 < x < 1 + kappa); 0 beyond.
+// (reading R9; BASELINE.json "tapered to zero above f_ISCO")
+__device__ __forceinline__ double taper(double x, double kappa, double inv_kappa)
+{
+    if (x <= 1.0) return 1.0;
+    if (x >= 1.0 + kappa) return 0.0;
+    const double s = (1.0 + kappa - x) * inv_kappa;
+    return s * s * s * fma(s, fma(6.0, s, -15.0), 10.0);
+}
+
+// frequency of dense bin i, exactly as the grid is defined (reading R3): f_i = (double)(k_min + i) * df
+__host__ __device__ __forceinline__ double bin_freq(long long k_min, long long i, double df)
+{
+    return (double)(k_min + i) * df;
+}
+
+// smallest i in [0, n_f] with f_i >= f  (n_f if none)
+__host__ __device__ inline long long first_bin_ge(double f, long long k_min, long long n_f, double df)
+{
+    double est = ceil(f / df) - (double)k_min;
+    if (!(est > 0.0)) est = 0.0;
+    if (est > (double)n_f) est = (double)n_f;
+    long long i = (long long)est;
+    while (i > 0 && bin_freq(k_min, i - 1, df) >= f) --i;
+    while (i < n_f && bin_freq(k_min, i, df) < f) ++i;
+    return i;
+}
+
+// smallest i in [0, n_f] with f_i > f  (n_f if none)
+__host__ __device__ inline long long first_bin_gt(double f, long long k_min, long long n_f, double df)
+{
+    double est = floor(f / df) + 1.0 - (double)k_min;
+    if (!(est > 0.0)) est = 0.0;
+    if (est > (double)n_f) est = (double)n_f;
+    long long i = (long long)est;
+    while (i > 0 && bin_freq(k_min, i - 1, df) > f) --i;
+    while (i < n_f && bin_freq(k_min, i, df) <= f) ++i;
+    return i;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// mbarrier + 1-D bulk TMA (cp.async.bulk) helpers; SASS: SYNCS.* / UBLKCP.
+// ---------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void *p)
+{
+    return (uint32_t)__cvta_generic_to_shared(p);
+}
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_fence_init()
+{
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    uint32_t done;
+    do {
+        asm volatile(
+            "{\n"
+            ".reg .pred p;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+            "selp.u32 %0, 1, 0, p;\n"
+            "}\n"
+            : "=r"(done)
+            : "r"(smem_u32(bar)), "r"(parity)
+            : "memory");
+    } while (!done);
+}
+__device__ __forceinline__ void tma_load_1d(void *dst_smem, const void *src_gmem, uint32_t bytes, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_u32(dst_smem)),
+                 "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+
+__device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+} // namespace ll

@@ -1,0 +1,876 @@
+// ll_kernels.cuh — the sm_100a kernels of libll_b200 (steps F0-F4, H0-H3 of DESIGN.md §2).
+//
+// Device layouts ("sorted position" p = index of a walker after the band-top counting sort; n_wp = n_w
+// rounded up to the walker-block size):
+//   g4   [n_f_pad][4]   W_i * conj(d^c_i): (A re, A im, E re, E im); im already negated          (F0)
+//   Wd   [n_f_pad]      W_i, zero in the padding
+//   Y    [n_m*2][n_nodes][n_wp]   node values, sys = 2 m + kind (0 amplitude, 1 phase in quarter cycles)
+//   C    [n_nodes-1][n_m][8][n_wp] cubic coefficients per interval: (y, b, c, d) amplitude, then phase
+//   TF   [n_m][2][2][n_wp]         transfer factors T^c_m (re, im)
+//   part [n_tiles][NQ][n_wp]       per-(frequency tile, walker) partial sums
+#pragma once
+#include <limits.h>
+#include "ll_device.cuh"
+
+namespace ll {
+
+constexpr int kMaxModes = 8;
+constexpr int kNC = 2;
+
+// ---------------------------------------------------------------------------------------------------
+// F0: pre-weighted data and <d|d>          (Eq. 3; "we transform the data")
+// ---------------------------------------------------------------------------------------------------
+__device__ __forceinline__ double block_sum_256(double v, double *sh)
+{
+    v = warp_sum(v);
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    if (lane == 0) sh[wid] = v;
+    __syncthreads();
+    double r = 0.0;
+    if (wid == 0) {
+        r = (lane < (int)(blockDim.x >> 5)) ? sh[lane] : 0.0;
+        r = warp_sum(r);
+    }
+    __syncthreads();
+    return r; // valid in warp 0
+}
+
+__global__ void __launch_bounds__(256) k_preweight(const double *__restrict__ d, const double *__restrict__ W,
+                                                   long long n_f, double *__restrict__ g4,
+                                                   double *__restrict__ Wd, double *__restrict__ dd_part)
+{
+    __shared__ double sh[8];
+    double acc = 0.0, comp = 0.0; // Neumaier-compensated per-thread sum
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n_f; i += (long long)gridDim.x * blockDim.x) {
+        const double w = W[i];
+        const double2 a = reinterpret_cast<const double2 *>(d)[i];
+        const double2 e = reinterpret_cast<const double2 *>(d)[n_f + i];
+        reinterpret_cast<double4 *>(g4)[i] = make_double4(w * a.x, -(w * a.y), w * e.x, -(w * e.y));
+        Wd[i] = w;
+        const double term = w * (a.x * a.x + a.y * a.y + e.x * e.x + e.y * e.y);
+        const double t = acc + term;
+        comp += (fabs(acc) >= fabs(term)) ? ((acc - t) + term) : ((term - t) + acc);
+        acc = t;
+    }
+    const double tot = block_sum_256(acc + comp, sh);
+    if (threadIdx.x == 0) dd_part[blockIdx.x] = tot;
+}
+
+// out[0] = sum of part[0..n) in a fixed order (single block; deterministic)
+__global__ void __launch_bounds__(256) k_sum_parts(const double *__restrict__ part, int n, double *__restrict__ out)
+{
+    __shared__ double sh[8];
+    double acc = 0.0;
+    for (int i = threadIdx.x; i < n; i += blockDim.x) acc += part[i];
+    const double tot = block_sum_256(acc, sh);
+    if (threadIdx.x == 0) out[0] = tot;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Band -> bin range per walker, sort key histogram, active-pair count          (reading R10)
+// ---------------------------------------------------------------------------------------------------
+struct GridInfo {
+    long long k_min;
+    long long n_f;
+    double df;
+};
+
+struct StandinInfo {
+    int n_m;
+    int m_max;
+    int mode_m[kMaxModes];
+    double kappa;
+};
+
+__device__ __forceinline__ void standin_masses(double Mc, double q, double &Mtot, double &eta, double &f_isco)
+{
+    eta = q / ((1.0 + q) * (1.0 + q));
+    Mtot = Mc * pow(eta, -0.6);
+    f_isco = 0x1.16b28f55d72d4p-4 / (kPi * Mtot); // 6^(-3/2) = 0.06804138174397717
+}
+
+// mode 0: stand-in parameters (params row stride P); mode 1: band array [n_w][2] or NULL
+__global__ void __launch_bounds__(256)
+k_band_prep(int use_standin, const double *__restrict__ params, int P, const double *__restrict__ band, int n_w,
+            GridInfo g, StandinInfo si, int key_gran, int *__restrict__ ilo_w, int *__restrict__ ihi_w,
+            int *__restrict__ key_w, int *__restrict__ hist, unsigned long long *__restrict__ pairs)
+{
+    const int w = blockIdx.x * blockDim.x + threadIdx.x;
+    long long span = 0;
+    if (w < n_w) {
+        double f_lo, f_hi;
+        if (use_standin) {
+            double Mtot, eta, fi;
+            standin_masses(params[(size_t)w * P], params[(size_t)w * P + 1], Mtot, eta, fi);
+            f_lo = bin_freq(g.k_min, 0, g.df);
+            const double top = (1.0 + si.kappa) * fi * (0.5 * (double)si.m_max);
+            const double f_last = bin_freq(g.k_min, g.n_f - 1, g.df);
+            f_hi = (top < f_last) ? top : f_last;
+        } else if (band) {
+            f_lo = band[2 * (size_t)w];
+            f_hi = band[2 * (size_t)w + 1];
+        } else {
+            f_lo = -INFINITY;
+            f_hi = INFINITY;
+        }
+        long long lo = first_bin_ge(f_lo, g.k_min, g.n_f, g.df);
+        long long hi = first_bin_gt(f_hi, g.k_min, g.n_f, g.df);
+        if (!(f_lo <= f_hi) || hi <= lo) { lo = 0; hi = 0; }
+        ilo_w[w] = (int)lo;
+        ihi_w[w] = (int)hi;
+        const int key = (int)(hi / key_gran);
+        key_w[w] = key;
+        atomicAdd(&hist[key], 1);
+        span = hi - lo;
+    }
+    // integer atomics: deterministic
+    unsigned long long s = (unsigned long long)span;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if ((threadIdx.x & 31) == 0 && s) atomicAdd(pairs, s * (unsigned long long)si.n_m);
+}
+
+// exclusive scan of hist[0..n) in place (single block of 1024 threads, n <= 1024*8)
+__global__ void __launch_bounds__(1024) k_scan_hist(int *__restrict__ hist, int n)
+{
+    __shared__ int wsum[32];
+    const int per = (n + 1023) / 1024;
+    const int b = threadIdx.x * per;
+    int loc[8];
+    int s = 0;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        loc[k] = 0;
+        if (k < per && b + k < n) loc[k] = hist[b + k];
+        s += loc[k];
+    }
+    int inc = s;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    if (lane == 31) wsum[wid] = inc;
+    __syncthreads();
+    if (wid == 0) {
+        int v = wsum[lane];
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int t = __shfl_up_sync(0xffffffffu, v, o);
+            if (lane >= o) v += t;
+        }
+        wsum[lane] = v;
+    }
+    __syncthreads();
+    int run = inc - s + (wid ? wsum[wid - 1] : 0);
+#pragma unroll
+    for (int k = 0; k < 8; ++k)
+        if (k < per && b + k < n) {
+            hist[b + k] = run;
+            run += loc[k];
+        }
+}
+
+// scatter walkers to sorted positions; padding positions get perm = -1 and an empty band
+__global__ void __launch_bounds__(256)
+k_scatter(int n_w, int n_wp, const int *__restrict__ key_w, const int *__restrict__ ilo_w, const int *__restrict__ ihi_w,
+          int *__restrict__ offs, int *__restrict__ perm, int *__restrict__ ilo_s, int *__restrict__ ihi_s)
+{
+    const int w = blockIdx.x * blockDim.x + threadIdx.x;
+    if (w < n_w) {
+        const int pos = atomicAdd(&offs[key_w[w]], 1);
+        perm[pos] = w;
+        ilo_s[pos] = ilo_w[w];
+        ihi_s[pos] = ihi_w[w];
+    } else if (w < n_wp) {
+        perm[w] = -1;
+        ilo_s[w] = 0;
+        ihi_s[w] = 0;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// F1: node amplitude / phase of the stand-in waveform             (Eq. 7; reading R9)
+//   A_lm(f)   = c_lm f^(-7/6)/D taper(2f/(m f_ISCO))
+//   Psi_lm(f) = (m/2) Psi(2f/m),  Psi(f) = 2 pi f t_c - phi_c - pi/4 + 3/(128 eta (pi M f)^(5/3))
+// Phase is written in quarter cycles: y = Psi_lm * 2/pi = 4 f t_c - (m/pi)(phi_c + pi/4) + (m/pi) K (2f/m)^(-5/3).
+// Node tables (host-built, per node set): cfp[m][j] = c_lm f_j^(-7/6), f2m[m][j] = 2 f_j/m,
+// fm53[m][j] = (2 f_j/m)^(-5/3), f4[j] = 4 f_j.
+// ---------------------------------------------------------------------------------------------------
+struct NodeTables {
+    const double *xj;    // [n]
+    const double *hj;    // [n-1]
+    const double *invh;  // [n-1]
+    const double *ta;    // [n] sub-diagonal of the natural-spline system
+    const double *tcp;   // [n] Thomas c'
+    const double *tinv;  // [n] Thomas 1/denominator
+    const double *f4;    // [n]
+    const double *cfp;   // [n_m][n]
+    const double *f2m;   // [n_m][n]
+    const double *fm53;  // [n_m][n]
+    const int *bstart;   // [n]: interval j covers dense bins [bstart[j], bstart[j+1]), j = 0..n-2
+};
+
+struct WalkerConst { // per walker constants of the stand-in
+    double tc, invD, inv_fisco, K, phi;
+};
+
+__device__ __forceinline__ WalkerConst standin_consts(const double *p)
+{
+    WalkerConst c;
+    double Mtot, eta, fi;
+    standin_masses(p[0], p[1], Mtot, eta, fi);
+    c.tc = p[2];
+    c.phi = p[3];
+    c.invD = p[4];
+    c.inv_fisco = 1.0 / fi;
+    const double v = cbrt(kPi * Mtot);
+    const double v2 = v * v;
+    c.K = 3.0 / (128.0 * eta * (v2 * v2 * v));
+    return c;
+}
+
+constexpr int kNodesPerThread = 8;
+
+__global__ void __launch_bounds__(128)
+k_nodes_standin(const double *__restrict__ params, int P, const int *__restrict__ perm, int n_wp, int n_nodes,
+                StandinInfo si, NodeTables nt, double *__restrict__ Y, double *__restrict__ TF)
+{
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= n_wp) return;
+    const int j0 = blockIdx.y * kNodesPerThread;
+    const int w = perm[p];
+    WalkerConst c = {0, 0, 0, 0, 0};
+    const double *row = nullptr;
+    if (w >= 0) {
+        row = params + (size_t)w * P;
+        c = standin_consts(row);
+    }
+    const double inv_kappa = 1.0 / si.kappa;
+    for (int m = 0; m < si.n_m; ++m) {
+        const double mh_pi = (double)si.mode_m[m] / kPi;
+        const double phq = mh_pi * (c.phi + 0.25 * kPi);
+        const double Kq = mh_pi * c.K;
+        double *ya = Y + ((size_t)(2 * m) * n_nodes) * n_wp + p;
+        double *yp = Y + ((size_t)(2 * m + 1) * n_nodes) * n_wp + p;
+#pragma unroll
+        for (int jj = 0; jj < kNodesPerThread; ++jj) {
+            const int j = j0 + jj;
+            if (j >= n_nodes) break;
+            double a = 0.0, y = 0.0;
+            if (w >= 0) {
+                const size_t t = (size_t)m * n_nodes + j;
+                a = nt.cfp[t] * c.invD * taper(nt.f2m[t] * c.inv_fisco, si.kappa, inv_kappa);
+                y = fma(nt.f4[j], c.tc, fma(Kq, nt.fm53[t], -phq));
+            }
+            ya[(size_t)j * n_wp] = a;
+            yp[(size_t)j * n_wp] = y;
+        }
+        if (blockIdx.y == 0) {
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+                TF[((size_t)m * 4 + q) * n_wp + p] = (w >= 0) ? row[5 + m * 4 + q] : 0.0;
+        }
+    }
+}
+
+// F1 (array entry point): transpose caller arrays [n_w][n_m][n_nodes] into Y; phase radians -> quarter cycles
+__global__ void __launch_bounds__(256)
+k_nodes_arrays(const double *__restrict__ amp, const double *__restrict__ phase, const double *__restrict__ tf,
+               const int *__restrict__ perm, int n_wp, int n_nodes, int n_m, double *__restrict__ Y,
+               double *__restrict__ TF)
+{
+    __shared__ double ta[32][33], tp[32][33];
+    const int m = blockIdx.z;
+    const int p0 = blockIdx.x * 32, j0 = blockIdx.y * 32;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5; // 32 x 8
+    for (int r = ty; r < 32; r += 8) {
+        const int w = perm[p0 + r];
+        const int j = j0 + tx;
+        double a = 0.0, ph = 0.0;
+        if (w >= 0 && j < n_nodes) {
+            const size_t idx = ((size_t)w * n_m + m) * n_nodes + j;
+            a = amp[idx];
+            ph = phase[idx] * kTwoOverPi;
+        }
+        ta[r][tx] = a;
+        tp[r][tx] = ph;
+    }
+    __syncthreads();
+    for (int r = ty; r < 32; r += 8) {
+        const int j = j0 + r;
+        if (j < n_nodes) {
+            Y[((size_t)(2 * m) * n_nodes + j) * n_wp + p0 + tx] = ta[tx][r];
+            Y[((size_t)(2 * m + 1) * n_nodes + j) * n_wp + p0 + tx] = tp[tx][r];
+        }
+    }
+    if (blockIdx.y == 0 && threadIdx.x < 32) {
+        const int w = perm[p0 + tx];
+#pragma unroll
+        for (int q = 0; q < 4; ++q)
+            TF[((size_t)m * 4 + q) * n_wp + p0 + tx] = (w >= 0) ? tf[((size_t)w * n_m + m) * 4 + q] : 0.0;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// F2: natural cubic spline, one system per thread, systems interleaved so every load/store is coalesced.
+// The tridiagonal matrix depends only on the (shared) nodes, so its Thomas factorisation (ta, tcp, tinv) is
+// built once per node set on the host; per system only the two substitution sweeps remain   (reading R1):
+//   dp_j = (r_j - a_j dp_{j-1}) / den_j,   r_j = (y_{j+1}-y_j)/h_j - (y_j-y_{j-1})/h_{j-1}
+//   M_j  = dp_j - c'_j M_{j+1},            M_0 = M_{n-1} = 0
+//   b_j = (y_{j+1}-y_j)/h_j - h_j (2 M_j + M_{j+1})/6,  c_j = M_j/2,  d_j = (M_{j+1}-M_j)/(6 h_j)
+// dp_j is parked in the b-slot of interval j between the sweeps.
+// ---------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128)
+k_spline(const double *__restrict__ Y, double *__restrict__ C, int n_wp, int n_nodes, int n_m, NodeTables nt)
+{
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= n_wp) return;
+    const int sys = blockIdx.y, m = sys >> 1, kind = sys & 1;
+    const size_t sw = (size_t)n_wp;
+    const double *y = Y + (size_t)sys * n_nodes * sw + p;
+    double *c = C + ((size_t)m * 8 + kind * 4) * sw + p; // + j * (n_m*8*sw) + q*sw
+    const size_t cj = (size_t)n_m * 8 * sw;
+    const int n = n_nodes;
+
+    double yprev = y[0], ycur = y[sw];
+    double sprev = (ycur - yprev) * __ldg(nt.invh);
+    double dpp = 0.0;
+#pragma unroll 8
+    for (int j = 1; j <= n - 2; ++j) {
+        const double ynext = y[(size_t)(j + 1) * sw];
+        const double s = (ynext - ycur) * __ldg(nt.invh + j);
+        const double r = s - sprev;
+        const double dp = (r - __ldg(nt.ta + j) * dpp) * __ldg(nt.tinv + j);
+        c[(size_t)j * cj + sw] = dp;
+        dpp = dp;
+        sprev = s;
+        ycur = ynext;
+    }
+    double Mn = 0.0;
+    double y1 = y[(size_t)(n - 1) * sw];
+#pragma unroll 4
+    for (int j = n - 2; j >= 0; --j) {
+        const double y0 = y[(size_t)j * sw];
+        double Mj = 0.0;
+        if (j >= 1) Mj = fma(-__ldg(nt.tcp + j), Mn, c[(size_t)j * cj + sw]);
+        const double h = __ldg(nt.hj + j), ih = __ldg(nt.invh + j);
+        double *cc = c + (size_t)j * cj;
+        cc[0] = y0;
+        cc[sw] = (y1 - y0) * ih - h * (2.0 * Mj + Mn) * kSixth;
+        cc[2 * sw] = 0.5 * Mj;
+        cc[3 * sw] = (Mn - Mj) * ih * kSixth;
+        Mn = Mj;
+        y1 = y0;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// F3: fused spline evaluation / channel response / inner products           (Eq. 3, 7, 9)
+// One thread = one walker; a warp = 32 walkers walking the SAME dense bins, so the data tile (g4, W) is a
+// shared-memory broadcast and no cross-thread reduction exists.  Tiles of g4/W arrive by 1-D bulk TMA into
+// a two-stage ring guarded by mbarriers.  The dense template is never written anywhere.
+// Single-mode specialisation: T^c is constant per walker, so the kernel accumulates the complex sums
+// S^c = sum_i g^c_i A e^{-i Psi} and H = sum_i W_i A^2; k_finalize applies T^c.
+// ---------------------------------------------------------------------------------------------------
+struct FusedArgs {
+    const double *g4;
+    const double *Wd;
+    const double *C;
+    const double *TF;
+    const double *xj;
+    const int *bstart;
+    const int *ilo;
+    const int *ihi;
+    double *part;
+    long long k_min;
+    double df;
+    int n_f, n_wp, n_nodes, n_m, TB, CH;
+};
+
+__device__ __forceinline__ int find_interval_of_bin(const int *__restrict__ bstart, int n_nodes, int i)
+{
+    // largest j in [0, n-2] with bstart[j] <= i
+    int lo = 0, hi = n_nodes - 2;
+    while (lo < hi) {
+        const int mid = (lo + hi + 1) >> 1;
+        if (__ldg(bstart + mid) <= i) lo = mid; else hi = mid - 1;
+    }
+    return lo;
+}
+
+template <int NM1> // NM1 = 1: single-mode specialisation (NQ = 5); 0: any n_m (NQ = 2)
+__global__ void __launch_bounds__(128, 4) k_full_fused(FusedArgs a)
+{
+    extern __shared__ __align__(128) double sm[];
+    __shared__ __align__(8) uint64_t bar[2];
+    __shared__ int s_lo, s_hi;
+
+    const int tid = threadIdx.x;
+    const int p = blockIdx.x * blockDim.x + tid;
+    const int tile = blockIdx.y;
+    const int i0 = tile * a.TB;
+    const int i1 = min(i0 + a.TB, a.n_f);
+    const int lo = max(a.ilo[p], i0), hi = min(a.ihi[p], i1);
+    if (tid == 0) {
+        s_lo = INT_MAX;
+        s_hi = INT_MIN;
+        mbar_init(&bar[0], 1);
+        mbar_init(&bar[1], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    if (lo < hi) {
+        atomicMin(&s_lo, lo);
+        atomicMax(&s_hi, hi);
+    }
+    __syncthreads();
+    const int blo = s_lo, bhi = s_hi;
+    if (blo >= bhi) return; // no walker of this block has bins in this tile; k_finalize never reads it
+
+    const int CH = a.CH;
+    const int c_begin = blo / CH, c_end = (bhi + CH - 1) / CH;
+    const uint32_t stage_bytes = (uint32_t)CH * 40u;
+    auto issue = [&](int c, int st) {
+        double *dst = sm + (size_t)st * CH * 5;
+        mbar_expect_tx(&bar[st], stage_bytes);
+        tma_load_1d(dst, a.g4 + (size_t)c * CH * 4, (uint32_t)CH * 32u, &bar[st]);
+        tma_load_1d(dst + (size_t)CH * 4, a.Wd + (size_t)c * CH, (uint32_t)CH * 8u, &bar[st]);
+    };
+    if (tid == 0) issue(c_begin, 0);
+
+    const size_t sw = (size_t)a.n_wp;
+    const size_t cj = (size_t)a.n_m * 8 * sw;
+    int j = find_interval_of_bin(a.bstart, a.n_nodes, blo);
+    int jl = -1;
+    double cA0 = 0, cA1 = 0, cA2 = 0, cA3 = 0, cP0 = 0, cP1 = 0, cP2 = 0, cP3 = 0, nxj = 0;
+    double sAr = 0, sAi = 0, sEr = 0, sEi = 0, sH = 0; // NM1: S^A, S^E, H;  generic: sAr = d_h, sH = h_h
+
+    for (int c = c_begin; c < c_end; ++c) {
+        const int st = (c - c_begin) & 1;
+        const uint32_t ph = (uint32_t)((c - c_begin) >> 1) & 1u;
+        if (tid == 0 && c + 1 < c_end) issue(c + 1, st ^ 1);
+        mbar_wait(&bar[st], ph);
+        const double *sg = sm + (size_t)st * CH * 5;
+        const double *sW = sg + (size_t)CH * 4;
+        const int cb = c * CH;
+        const int ce = min(cb + CH, bhi);
+        int i = max(cb, blo);
+        while (i < ce) {
+            while (j < a.n_nodes - 2 && __ldg(a.bstart + j + 1) <= i) ++j;
+            const int seg_end = (j < a.n_nodes - 2) ? min(__ldg(a.bstart + j + 1), ce) : ce;
+            int tlo = max(i, lo), thi = min(seg_end, hi);
+            if (tlo >= thi) { tlo = INT_MAX; thi = INT_MIN; }
+            const int wlo = __reduce_min_sync(0xffffffffu, tlo);
+            const int whi = __reduce_max_sync(0xffffffffu, thi);
+            if (wlo < whi) {
+                if (NM1) {
+                    if (j != jl) {
+                        const double *cc = a.C + (size_t)j * cj + p;
+                        cA0 = cc[0]; cA1 = cc[sw]; cA2 = cc[2 * sw]; cA3 = cc[3 * sw];
+                        cP0 = cc[4 * sw]; cP1 = cc[5 * sw]; cP2 = cc[6 * sw]; cP3 = cc[7 * sw];
+                        nxj = -__ldg(a.xj + j);
+                        jl = j;
+                    }
+                    double kd = (double)(a.k_min + wlo);
+#pragma unroll 2
+                    for (int ii = wlo; ii < whi; ++ii) {
+                        const bool act = (ii >= tlo) && (ii < thi);
+                        const double t = fma(kd, a.df, nxj);
+                        kd += 1.0;
+                        double A = fma(fma(fma(cA3, t, cA2), t, cA1), t, cA0);
+                        const double y = fma(fma(fma(cP3, t, cP2), t, cP1), t, cP0);
+                        A = act ? A : 0.0;
+                        double sn, cs;
+                        sincos_qc(y, sn, cs);
+                        const double u = A * cs, v = A * sn; // h = u - i v
+                        const double4 g = reinterpret_cast<const double4 *>(sg)[ii - cb];
+                        const double w = sW[ii - cb];
+                        sAr = fma(g.x, u, sAr); sAr = fma(g.y, v, sAr);
+                        sAi = fma(g.y, u, sAi); sAi = fma(-g.x, v, sAi);
+                        sEr = fma(g.z, u, sEr); sEr = fma(g.w, v, sEr);
+                        sEi = fma(g.w, u, sEi); sEi = fma(-g.z, v, sEi);
+                        sH = fma(w * A, A, sH);
+                    }
+                } else {
+                    nxj = -__ldg(a.xj + j);
+                    const double *cc0 = a.C + (size_t)j * cj + p;
+                    double kd = (double)(a.k_min + wlo);
+                    for (int ii = wlo; ii < whi; ++ii) {
+                        const bool act = (ii >= tlo) && (ii < thi);
+                        const double t = fma(kd, a.df, nxj);
+                        kd += 1.0;
+                        double hAr = 0, hAi = 0, hEr = 0, hEi = 0;
+                        for (int m = 0; m < a.n_m; ++m) {
+                            const double *cc = cc0 + (size_t)m * 8 * sw;
+                            const double A = fma(fma(fma(cc[3 * sw], t, cc[2 * sw]), t, cc[sw]), t, cc[0]);
+                            const double y = fma(fma(fma(cc[7 * sw], t, cc[6 * sw]), t, cc[5 * sw]), t, cc[4 * sw]);
+                            double sn, cs;
+                            sincos_qc(y, sn, cs);
+                            const double u = A * cs, v = A * sn;
+                            const double *tf = a.TF + (size_t)m * 4 * sw + p;
+                            const double tar = tf[0], tai = tf[sw], ter = tf[2 * sw], tei = tf[3 * sw];
+                            hAr = fma(tar, u, hAr); hAr = fma(tai, v, hAr);
+                            hAi = fma(tai, u, hAi); hAi = fma(-tar, v, hAi);
+                            hEr = fma(ter, u, hEr); hEr = fma(tei, v, hEr);
+                            hEi = fma(tei, u, hEi); hEi = fma(-ter, v, hEi);
+                        }
+                        if (act) {
+                            const double4 g = reinterpret_cast<const double4 *>(sg)[ii - cb];
+                            const double w = sW[ii - cb];
+                            sAr = fma(g.x, hAr, sAr); sAr = fma(-g.y, hAi, sAr);
+                            sAr = fma(g.z, hEr, sAr); sAr = fma(-g.w, hEi, sAr);
+                            sH = fma(w, hAr * hAr + hAi * hAi + hEr * hEr + hEi * hEi, sH);
+                        }
+                    }
+                }
+            }
+            i = seg_end;
+        }
+        __syncthreads(); // everyone is done with stage st before it is refilled two chunks later
+    }
+    if (NM1) {
+        double *o = a.part + ((size_t)tile * 5) * sw + p;
+        o[0] = sAr; o[sw] = sAi; o[2 * sw] = sEr; o[3 * sw] = sEi; o[4 * sw] = sH;
+    } else {
+        double *o = a.part + ((size_t)tile * 2) * sw + p;
+        o[0] = sAr; o[sw] = sH;
+    }
+}
+
+// F4: reduce the per-tile partials in tile order, apply T^c (single mode), form log L        (Eq. 2)
+template <int NM1>
+__global__ void __launch_bounds__(128)
+k_finalize(const double *__restrict__ part, const double *__restrict__ TF, const int *__restrict__ perm,
+           const int *__restrict__ ilo, const int *__restrict__ ihi, int n_wp, int TB, const double *__restrict__ dd,
+           double *__restrict__ logL, double *__restrict__ d_h, double *__restrict__ h_h)
+{
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= n_wp) return;
+    const int w = perm[p];
+    if (w < 0) return;
+    const size_t sw = (size_t)n_wp;
+    const int lo = ilo[p], hi = ihi[p];
+    constexpr int NQ = NM1 ? 5 : 2;
+    double acc[NQ];
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) acc[q] = 0.0;
+    if (hi > lo) {
+        const int t1 = (hi - 1) / TB;
+        for (int t = lo / TB; t <= t1; ++t) {
+            const double *o = part + ((size_t)t * NQ) * sw + p;
+#pragma unroll
+            for (int q = 0; q < NQ; ++q) acc[q] += o[q * sw];
+        }
+    }
+    double dh, hh;
+    if (NM1) {
+        const double tar = TF[p], tai = TF[sw + p], ter = TF[2 * sw + p], tei = TF[3 * sw + p];
+        // Re[T^A S^A + T^E S^E],  (|T^A|^2 + |T^E|^2) H
+        dh = (tar * acc[0] - tai * acc[1]) + (ter * acc[2] - tei * acc[3]);
+        hh = (tar * tar + tai * tai + ter * ter + tei * tei) * acc[4];
+    } else {
+        dh = acc[0];
+        hh = acc[1];
+    }
+    logL[w] = dh - 0.5 * hh - 0.5 * dd[0];
+    if (d_h) d_h[w] = dh;
+    if (h_h) h_h[w] = hh;
+}
+
+// dense template of the walker at sorted position p (setup utility; same arithmetic as k_full_fused)
+__global__ void __launch_bounds__(256)
+k_full_template(FusedArgs a, int p, double *__restrict__ h_out)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= a.n_f) return;
+    double hAr = 0, hAi = 0, hEr = 0, hEi = 0;
+    if (i >= a.ilo[p] && i < a.ihi[p]) {
+        const int j = find_interval_of_bin(a.bstart, a.n_nodes, (int)i);
+        const size_t sw = (size_t)a.n_wp;
+        const double t = fma((double)(a.k_min + i), a.df, -a.xj[j]);
+        for (int m = 0; m < a.n_m; ++m) {
+            const double *cc = a.C + ((size_t)j * a.n_m + m) * 8 * sw + p;
+            const double A = fma(fma(fma(cc[3 * sw], t, cc[2 * sw]), t, cc[sw]), t, cc[0]);
+            const double y = fma(fma(fma(cc[7 * sw], t, cc[6 * sw]), t, cc[5 * sw]), t, cc[4 * sw]);
+            double sn, cs;
+            sincos_qc(y, sn, cs);
+            const double u = A * cs, v = A * sn;
+            const double *tf = a.TF + (size_t)m * 4 * sw + p;
+            const double tar = tf[0], tai = tf[sw], ter = tf[2 * sw], tei = tf[3 * sw];
+            hAr = fma(tar, u, hAr); hAr = fma(tai, v, hAr);
+            hAi = fma(tai, u, hAi); hAi = fma(-tar, v, hAi);
+            hEr = fma(ter, u, hEr); hEr = fma(tei, v, hEr);
+            hEi = fma(tei, u, hEi); hEi = fma(-ter, v, hEi);
+        }
+    }
+    reinterpret_cast<double2 *>(h_out)[i] = make_double2(hAr, hAi);
+    reinterpret_cast<double2 *>(h_out)[a.n_f + i] = make_double2(hEr, hEi);
+}
+
+// stand-in template of one parameter row evaluated directly at arbitrary frequencies (no spline, no tables)
+struct DirectRow {
+    double p[5 + 4 * kMaxModes];
+    double c_lm[kMaxModes];
+};
+
+__global__ void __launch_bounds__(256)
+k_template_direct(DirectRow row, StandinInfo si, long long n_freq, const double *__restrict__ f, double f_lo,
+                  double f_hi, double *__restrict__ h_out)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_freq) return;
+    const double fi = f[i];
+    double hAr = 0, hAi = 0, hEr = 0, hEi = 0;
+    if (fi >= f_lo && fi <= f_hi) {
+        double Mtot, eta, fisco;
+        standin_masses(row.p[0], row.p[1], Mtot, eta, fisco);
+        const double tc = row.p[2], phic = row.p[3], invD = row.p[4];
+        const double inv_kappa = 1.0 / si.kappa;
+        for (int m = 0; m < si.n_m; ++m) {
+            const double mh = 0.5 * (double)si.mode_m[m];
+            const double fp = fi / mh;
+            const double A = row.c_lm[m] * pow(fi, -7.0 / 6.0) * invD * taper(fp / fisco, si.kappa, inv_kappa);
+            const double v = cbrt(kPi * Mtot * fp);
+            const double v2 = v * v;
+            const double psi = mh * (2.0 * kPi * fp * tc - phic - 0.25 * kPi + 3.0 / (128.0 * eta * (v2 * v2 * v)));
+            double sn, cs;
+            sincos_rad(psi, sn, cs);
+            const double u = A * cs, vv = A * sn;
+            const double tar = row.p[5 + m * 4], tai = row.p[6 + m * 4], ter = row.p[7 + m * 4], tei = row.p[8 + m * 4];
+            hAr = fma(tar, u, hAr); hAr = fma(tai, vv, hAr);
+            hAi = fma(tai, u, hAi); hAi = fma(-tar, vv, hAi);
+            hEr = fma(ter, u, hEr); hEr = fma(tei, vv, hEr);
+            hEi = fma(tei, u, hEi); hEi = fma(-ter, vv, hEi);
+        }
+    }
+    reinterpret_cast<double2 *>(h_out)[i] = make_double2(hAr, hAi);
+    reinterpret_cast<double2 *>(h_out)[n_freq + i] = make_double2(hEr, hEi);
+}
+
+// ---------------------------------------------------------------------------------------------------
+// H0: heterodyne summary data, one block per bin                   (Eq. 15, 16, 18, 19)
+//   A0 = sum W d conj(h0), A1 = sum W d conj(h0)(f - f_b), B0 = sum W |h0|^2, B1 = sum W |h0|^2 (f - f_b)
+// raw[b][13]: per channel (A0r, A0i, A1r, A1i, B0, B1), then sum_c W |d|^2 over the bin.
+// ---------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+k_het_prepare(const double *__restrict__ g4, const double *__restrict__ Wd, const double *__restrict__ h0, GridInfo g,
+              const int *__restrict__ estart, const double *__restrict__ fb, double *__restrict__ raw)
+{
+    __shared__ double sh[8];
+    const int b = blockIdx.x;
+    const int i_lo = estart[b], i_hi = estart[b + 1];
+    const double f_b = fb[b];
+    double acc[13];
+#pragma unroll
+    for (int q = 0; q < 13; ++q) acc[q] = 0.0;
+    for (int i = i_lo + threadIdx.x; i < i_hi; i += blockDim.x) {
+        const double4 gg = reinterpret_cast<const double4 *>(g4)[i]; // W conj(d): (W dAr, -W dAi, W dEr, -W dEi)
+        const double w = Wd[i];
+        const double t = bin_freq(g.k_min, i, g.df) - f_b;
+        const double2 ha = reinterpret_cast<const double2 *>(h0)[i];
+        const double2 he = reinterpret_cast<const double2 *>(h0)[g.n_f + i];
+        // W d conj(h0) = conj( (W conj d) h0 )
+        const double par = gg.x * ha.x - gg.y * ha.y, pai = -(gg.x * ha.y + gg.y * ha.x);
+        const double per = gg.z * he.x - gg.w * he.y, pei = -(gg.z * he.y + gg.w * he.x);
+        const double qa = w * (ha.x * ha.x + ha.y * ha.y), qe = w * (he.x * he.x + he.y * he.y);
+        acc[0] += par; acc[1] += pai; acc[2] = fma(par, t, acc[2]); acc[3] = fma(pai, t, acc[3]);
+        acc[4] += qa; acc[5] = fma(qa, t, acc[5]);
+        acc[6] += per; acc[7] += pei; acc[8] = fma(per, t, acc[8]); acc[9] = fma(pei, t, acc[9]);
+        acc[10] += qe; acc[11] = fma(qe, t, acc[11]);
+        // W |d|^2 = |W conj d|^2 / W
+        if (w > 0.0) acc[12] += (gg.x * gg.x + gg.y * gg.y + gg.z * gg.z + gg.w * gg.w) / w;
+    }
+#pragma unroll
+    for (int q = 0; q < 13; ++q) {
+        const double tot = block_sum_256(acc[q], sh);
+        if (threadIdx.x == 0) raw[(size_t)b * 13 + q] = tot;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// H1-H3: heterodyned likelihood.  Packed table (host-built by ll_het_prepare), all in shared memory:
+//   edge e : f4[e] = 4 f_e; ih0[e][4] = 1/h0^A (re, im), 1/h0^E (re, im);
+//            per mode m: cfp[m][e] = c_lm f_e^(-7/6), f2m[m][e] = 2 f_e/m, fm53[m][e] = (2 f_e/m)^(-5/3)
+//   bin b  : A0h[4] = A0/2 (A re, im, E re, im), A1w[4] = A1/(e_{b+1}-e_b), B0q[2] = B0/4, B1w[2] = B1/(e_{b+1}-e_b)
+// With s = r_lo + r_hi and dlt = r_hi - r_lo:  r0 = s/2, r1 = dlt/width                         (Eq. 11), so
+//   Z[d,h] term = Re[A0 conj r0 + A1 conj r1] = A0h . s + A1w . dlt                              (Eq. 14)
+//   Z[h,h] term = B0 |r0|^2 + 2 B1 Re[r0 conj r1] = B0q |s|^2 + B1w (s . dlt)                    (Eq. 17)
+// ---------------------------------------------------------------------------------------------------
+struct HetTable {
+    const double *base; // device copy of the packed table
+    int n_e, n_b, n_m;
+    int total;          // doubles
+    __host__ __device__ int off_f4() const { return 0; }
+    __host__ __device__ int off_ih0() const { return n_e; }
+    __host__ __device__ int off_cfp() const { return 5 * n_e; }
+    __host__ __device__ int off_f2m() const { return 5 * n_e + n_m * n_e; }
+    __host__ __device__ int off_fm53() const { return 5 * n_e + 2 * n_m * n_e; }
+    __host__ __device__ int off_bins() const { return 5 * n_e + 3 * n_m * n_e; }
+};
+
+__device__ __forceinline__ void het_bin_contract(const double *__restrict__ tb, double lAr, double lAi, double lEr,
+                                                 double lEi, double hAr, double hAi, double hEr, double hEi,
+                                                 double &dh, double &hh)
+{
+    const double sAr = lAr + hAr, sAi = lAi + hAi, sEr = lEr + hEr, sEi = lEi + hEi;
+    const double dAr = hAr - lAr, dAi = hAi - lAi, dEr = hEr - lEr, dEi = hEi - lEi;
+    dh = fma(tb[0], sAr, dh); dh = fma(tb[1], sAi, dh); dh = fma(tb[2], sEr, dh); dh = fma(tb[3], sEi, dh);
+    dh = fma(tb[4], dAr, dh); dh = fma(tb[5], dAi, dh); dh = fma(tb[6], dEr, dh); dh = fma(tb[7], dEi, dh);
+    hh = fma(tb[8], fma(sAr, sAr, sAi * sAi), hh);
+    hh = fma(tb[9], fma(sEr, sEr, sEi * sEi), hh);
+    hh = fma(tb[10], fma(sAr, dAr, sAi * dAi), hh);
+    hh = fma(tb[11], fma(sEr, dEr, sEi * dEi), hh);
+}
+
+// Stand-in parameters -> log L.  Block = 32 walkers x S frequency segments (warp s walks segment s); lanes of
+// a warp are 32 different walkers at the same edge, so every table read is a broadcast.
+template <int NM>
+__global__ void __launch_bounds__(512)
+k_het_standin(HetTable T, StandinInfo si, const double *__restrict__ params, int P, int n_w, int n_groups,
+              const double *__restrict__ dd, double *__restrict__ logL, double *__restrict__ d_h,
+              double *__restrict__ h_h)
+{
+    extern __shared__ __align__(16) double tab[];
+    double *red = tab + T.total; // [S][2][32]
+    for (int i = threadIdx.x + threadIdx.y * 32; i < T.total; i += 32 * blockDim.y) tab[i] = T.base[i];
+    __syncthreads();
+    const int S = blockDim.y, seg = threadIdx.y, lane = threadIdx.x;
+    const int per = (T.n_b + S - 1) / S;
+    const int b0 = seg * per, b1 = min(b0 + per, T.n_b);
+    const double *f4 = tab + T.off_f4(), *ih0 = tab + T.off_ih0(), *cfp = tab + T.off_cfp(),
+                 *f2m = tab + T.off_f2m(), *fm53 = tab + T.off_fm53(), *bins = tab + T.off_bins();
+    const double inv_kappa = 1.0 / si.kappa;
+    const double ddb = dd[1];
+
+    for (int grp = blockIdx.x; grp < n_groups; grp += gridDim.x) {
+        const int w = grp * 32 + lane;
+        const bool valid = w < n_w;
+        const double *row = params + (size_t)(valid ? w : 0) * P;
+        const WalkerConst c = standin_consts(row);
+        double Kq[NM], phq[NM], tf[NM][4];
+#pragma unroll
+        for (int m = 0; m < NM; ++m) {
+            const double mh_pi = (double)si.mode_m[m] / kPi;
+            Kq[m] = mh_pi * c.K;
+            phq[m] = mh_pi * (c.phi + 0.25 * kPi);
+#pragma unroll
+            for (int q = 0; q < 4; ++q) tf[m][q] = row[5 + m * 4 + q];
+        }
+        double dh = 0.0, hh = 0.0;
+        double pAr = 0, pAi = 0, pEr = 0, pEi = 0;
+        for (int e = b0; e <= b1 && b0 < b1; ++e) {
+            double hAr = 0, hAi = 0, hEr = 0, hEi = 0;
+            const double f4e = f4[e];
+#pragma unroll
+            for (int m = 0; m < NM; ++m) {
+                const int t = m * T.n_e + e;
+                const double y = fma(f4e, c.tc, fma(Kq[m], fm53[t], -phq[m]));
+                double sn, cs;
+                sincos_qc(y, sn, cs);
+                const double A = cfp[t] * c.invD * taper(f2m[t] * c.inv_fisco, si.kappa, inv_kappa);
+                const double u = A * cs, v = A * sn; // h_m = u - i v
+                hAr = fma(tf[m][0], u, hAr); hAr = fma(tf[m][1], v, hAr);
+                hAi = fma(tf[m][1], u, hAi); hAi = fma(-tf[m][0], v, hAi);
+                hEr = fma(tf[m][2], u, hEr); hEr = fma(tf[m][3], v, hEr);
+                hEi = fma(tf[m][3], u, hEi); hEi = fma(-tf[m][2], v, hEi);
+            }
+            const double *g = ih0 + 4 * e; // r = h * (1/h0)
+            const double rAr = hAr * g[0] - hAi * g[1], rAi = hAr * g[1] + hAi * g[0];
+            const double rEr = hEr * g[2] - hEi * g[3], rEi = hEr * g[3] + hEi * g[2];
+            if (e > b0) het_bin_contract(bins + 12 * (e - 1), pAr, pAi, pEr, pEi, rAr, rAi, rEr, rEi, dh, hh);
+            pAr = rAr; pAi = rAi; pEr = rEr; pEi = rEi;
+        }
+        if (S > 1) {
+            red[(seg * 2) * 32 + lane] = dh;
+            red[(seg * 2 + 1) * 32 + lane] = hh;
+            __syncthreads();
+            if (seg == 0) {
+                dh = 0.0; hh = 0.0;
+                for (int s = 0; s < S; ++s) { dh += red[(s * 2) * 32 + lane]; hh += red[(s * 2 + 1) * 32 + lane]; }
+            }
+        }
+        if (seg == 0 && valid) {
+            logL[w] = dh - 0.5 * hh - 0.5 * ddb;
+            if (d_h) d_h[w] = dh;
+            if (h_h) h_h[w] = hh;
+        }
+        if (S > 1) __syncthreads();
+    }
+}
+
+// Array entry point: amp_e, phase_e [n_w][n_m][n_e] (radians).  One warp per walker, lanes over edges (the
+// arrays are walker-major, so this is the coalesced direction); neighbouring edges meet through a shuffle.
+__global__ void __launch_bounds__(256)
+k_het_arrays(HetTable T, const double *__restrict__ amp_e, const double *__restrict__ phase_e,
+             const double *__restrict__ tf, int n_w, const double *__restrict__ dd, double *__restrict__ logL,
+             double *__restrict__ d_h, double *__restrict__ h_h)
+{
+    extern __shared__ __align__(16) double tab[];
+    for (int i = threadIdx.x; i < T.total; i += blockDim.x) tab[i] = T.base[i];
+    __syncthreads();
+    const double *ih0 = tab + T.off_ih0(), *bins = tab + T.off_bins();
+    const int lane = threadIdx.x & 31, wpb = blockDim.x >> 5;
+    const double ddb = dd[1];
+    for (int w = blockIdx.x * wpb + (threadIdx.x >> 5); w < n_w; w += gridDim.x * wpb) {
+        double dh = 0.0, hh = 0.0;
+        for (int base = 0; base < T.n_b; base += 31) {
+            const int e = base + lane;
+            double rAr = 0, rAi = 0, rEr = 0, rEi = 0;
+            if (e < T.n_e) {
+                double hAr = 0, hAi = 0, hEr = 0, hEi = 0;
+                for (int m = 0; m < T.n_m; ++m) {
+                    const size_t idx = ((size_t)w * T.n_m + m) * T.n_e + e;
+                    const double A = amp_e[idx];
+                    double sn, cs;
+                    sincos_rad(phase_e[idx], sn, cs);
+                    const double u = A * cs, v = A * sn;
+                    const double *t4 = tf + ((size_t)w * T.n_m + m) * 4;
+                    const double tar = __ldg(t4), tai = __ldg(t4 + 1), ter = __ldg(t4 + 2), tei = __ldg(t4 + 3);
+                    hAr = fma(tar, u, hAr); hAr = fma(tai, v, hAr);
+                    hAi = fma(tai, u, hAi); hAi = fma(-tar, v, hAi);
+                    hEr = fma(ter, u, hEr); hEr = fma(tei, v, hEr);
+                    hEi = fma(tei, u, hEi); hEi = fma(-ter, v, hEi);
+                }
+                const double *g = ih0 + 4 * e;
+                rAr = hAr * g[0] - hAi * g[1]; rAi = hAr * g[1] + hAi * g[0];
+                rEr = hEr * g[2] - hEi * g[3]; rEi = hEr * g[3] + hEi * g[2];
+            }
+            const double nAr = __shfl_down_sync(0xffffffffu, rAr, 1), nAi = __shfl_down_sync(0xffffffffu, rAi, 1);
+            const double nEr = __shfl_down_sync(0xffffffffu, rEr, 1), nEi = __shfl_down_sync(0xffffffffu, rEi, 1);
+            if (lane < 31 && e < T.n_b) het_bin_contract(bins + 12 * e, rAr, rAi, rEr, rEi, nAr, nAi, nEr, nEi, dh, hh);
+        }
+        dh = warp_sum(dh);
+        hh = warp_sum(hh);
+        if (lane == 0) {
+            logL[w] = dh - 0.5 * hh - 0.5 * ddb;
+            if (d_h) d_h[w] = dh;
+            if (h_h) h_h[w] = hh;
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// ALU roofline denominators: dependent-free FMA chains on every SM (measurement helper)
+// ---------------------------------------------------------------------------------------------------
+template <typename T>
+__global__ void __launch_bounds__(256) k_peak_fma(long long iters, T *__restrict__ sink)
+{
+    T a[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) a[k] = (T)(threadIdx.x + k) * (T)1e-3;
+    const T m = (T)0.999999, c = (T)1e-6;
+    for (long long it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int r = 0; r < 4; ++r)
+#pragma unroll
+            for (int k = 0; k < 8; ++k) a[k] = a[k] * m + c;
+    }
+    T s = 0;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) s += a[k];
+    if (s == (T)123456.789) sink[0] = s;
+}
+
+} // namespace ll

@@ -1,0 +1,64 @@
+"""Shared by the GPU parity tests: finish a seeded workload WITH THE ORACLE (so that every input both sides see
+comes from oracle/ or from the seeded generator, never from the CUDA path) and small comparison utilities."""
+import numpy as np
+
+from paper_2111_01064_b200 import workloads as wlm
+
+
+def tol_ll(ref):
+    """BASELINE.json north_star: |delta log L| <= 1e-6 * max(1, |log L|) for FP64."""
+    return 1e-6 * np.maximum(1.0, np.abs(ref))
+
+
+def assert_close_ll(got, ref, what=""):
+    got, ref = np.asarray(got, dtype=np.float64), np.asarray(ref, dtype=np.float64)
+    assert got.shape == ref.shape, (what, got.shape, ref.shape)
+    err = np.abs(got - ref)
+    bad = err > tol_ll(ref)
+    assert not bad.any(), f"{what}: {bad.sum()} of {bad.size} outside tolerance; worst |err|={err.max():.3e} " \
+                          f"at {int(err.argmax())} (ref {ref[err.argmax()]:.6e})"
+
+
+def oracle_setup_full(orc, wl: wlm.Workload):
+    g = wl.grid
+    run = lambda params, d, tmpl=False: orc.full_batch_standin(
+        wl.modes_m, wl.c_lm, wl.kappa, params, wl.f_nodes, g.k_min, g.df, g.n_f, d, wl.W, want_template=tmpl)
+    if not wl.finished:
+        wl.finish_distance(run(wl.inj[None], None)["h_h"][0])
+    h = run(wl.inj[None], None, True)["h"]
+    d = wl.make_data(h)
+    return d, run
+
+
+def oracle_setup_het(orc, wl: wlm.Workload):
+    g = wl.grid
+    f = g.freqs()
+    lo, hi = float(f[0]), float(f[-1])
+    direct = lambda p, ff: orc.standin_direct(p, wl.modes_m, wl.c_lm, wl.kappa, ff, lo, hi)
+    if not wl.finished:
+        h1 = direct(wl.inj, f)
+        wl.finish_distance(orc.inner(h1, h1, wl.W).real)
+    h0 = direct(wl.inj, f)
+    d = wl.make_data(h0)
+    h0e = direct(wl.inj, wl.f_edges)
+    summ = orc.het_prepare(g.k_min, g.df, d, wl.W, h0, wl.f_edges)
+    return d, h0, h0e, summ
+
+
+def rand_smooth_nodes(rng, n_w, n_m, f_nodes, phase_scale=200.0):
+    """smooth random amplitude/phase node arrays (not the stand-in), for the array entry points"""
+    x = np.log(f_nodes / f_nodes[0]) / np.log(f_nodes[-1] / f_nodes[0])
+    amp = np.empty((n_w, n_m, len(f_nodes)))
+    ph = np.empty((n_w, n_m, len(f_nodes)))
+    for w in range(n_w):
+        for m in range(n_m):
+            a = rng.uniform(0.5, 2.0, 4)
+            amp[w, m] = 1e-19 * (a[0] + a[1] * x + a[2] * np.sin(3 * x + a[3]))
+            b = rng.uniform(-1.0, 1.0, 4)
+            ph[w, m] = phase_scale * (b[0] + b[1] * x + b[2] * x ** 2 + np.cos(2 * x + b[3]))
+    return amp, ph
+
+
+def unit_tf(rng, n_w, n_m, n_c=2):
+    ang = rng.uniform(0, 2 * np.pi, (n_w, n_m, n_c))
+    return np.stack([np.cos(ang), np.sin(ang)], axis=-1)

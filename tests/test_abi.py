@@ -1,0 +1,136 @@
+"""CPU-side checks of the boundary (-m "not gpu"): the C-ABI library builds for sm_100a, loads, and exports every
+symbol include/ll.h declares; without a GPU ll_create fails loudly (no CPU fallback); the host-side sharding logic of
+the multi-GPU bench runs under gloo with world_size 2."""
+import ctypes as C
+import os
+import re
+import subprocess
+import sys
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+HEADER = os.path.join(ROOT, "include", "ll.h")
+
+
+@pytest.fixture(scope="module")
+def so_path():
+    from paper_2111_01064_b200 import build
+    return build.build()
+
+
+def _declared_symbols():
+    src = open(HEADER).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(ll_[a-z0-9_]+)\s*\(", src)))
+
+
+def test_header_declares_the_six_calls():
+    names = _declared_symbols()
+    for must in ("ll_create", "ll_set_data", "ll_full_batch", "ll_het_prepare", "ll_het_batch", "ll_destroy"):
+        assert must in names
+
+
+def test_library_exports_every_declared_symbol(so_path):
+    from paper_2111_01064_b200 import binding
+    lib = C.CDLL(so_path)
+    names = _declared_symbols()
+    assert sorted(binding.SYMBOLS) == names
+    for n in names:
+        assert hasattr(lib, n), n
+    assert lib.ll_abi_version() == 1
+
+
+def test_library_is_sm100a_only(so_path):
+    out = subprocess.run(["cuobjdump", "-lelf", so_path], capture_output=True, text=True)
+    if out.returncode != 0:
+        pytest.skip("cuobjdump unavailable")
+    archs = set(re.findall(r"sm_\d+a?", out.stdout))
+    assert archs == {"sm_100a"}, archs
+
+
+def test_tma_and_mbarrier_in_fused_kernel_sass(so_path):
+    out = subprocess.run(["cuobjdump", "-sass", "-fun", "_ZN2ll12k_full_fusedILi1EEEvNS_9FusedArgsE", so_path],
+                         capture_output=True, text=True)
+    if out.returncode != 0 or not out.stdout:
+        pytest.skip("cuobjdump unavailable")
+    assert "UBLKCP" in out.stdout          # cp.async.bulk (1-D TMA)
+    assert "SYNCS" in out.stdout           # mbarrier
+    assert "DFMA" in out.stdout
+
+
+def test_no_cpu_fallback_without_gpu(so_path):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    from paper_2111_01064_b200 import binding
+    lib = binding.load_library()
+    cfg = binding.ll_config(0, 2, 1, 0, (C.c_int32 * 4)(0, 0, 0, 0))
+    h = C.c_void_p()
+    assert lib.ll_create(C.byref(cfg), C.byref(h)) == binding.LL_ERR_CUDA
+    with pytest.raises(binding.LLError):
+        binding.Context()
+
+
+def test_create_rejects_bad_config(so_path):
+    from paper_2111_01064_b200 import binding
+    lib = binding.load_library()
+    h = C.c_void_p()
+    for dev, nc, nm, prec in ((0, 3, 1, 0), (0, 2, 0, 0), (0, 2, 9, 0), (0, 2, 1, 7)):
+        cfg = binding.ll_config(dev, nc, nm, prec, (C.c_int32 * 4)(0, 0, 0, 0))
+        assert lib.ll_create(C.byref(cfg), C.byref(h)) == binding.LL_ERR_UNSUPPORTED
+    assert lib.ll_create(None, C.byref(h)) == binding.LL_ERR_ARG
+    assert lib.ll_destroy(None) == binding.LL_ERR_ARG
+
+
+def test_shard_slices_cover_and_balance():
+    from paper_2111_01064_b200 import workloads as wlm
+    for n, ws in ((16384, 8), (10, 3), (1, 2), (0, 4)):
+        sl = wlm.shard_slices(n, ws)
+        idx = np.concatenate([np.arange(n)[s] for s in sl]) if n else np.array([], dtype=int)
+        assert idx.tolist() == list(range(n))
+        sizes = [s.stop - s.start for s in sl]
+        assert max(sizes) - min(sizes) <= 1
+
+
+def test_workload_seeds_differ_per_rank_and_are_reproducible():
+    from paper_2111_01064_b200 import workloads as wlm
+    a = wlm.make_workload(1, n_w=16, seed_offset=0)
+    b = wlm.make_workload(1, n_w=16, seed_offset=1)
+    c = wlm.make_workload(1, n_w=16, seed_offset=0)
+    assert not np.array_equal(a.params, b.params)
+    assert np.array_equal(a.params, c.params)
+
+
+_GLOO_WORKER = r"""
+import os, sys, json
+sys.path.insert(0, %(root)r)
+import torch, torch.distributed as dist
+import bench
+rank, world = int(os.environ["RANK"]), int(os.environ["WORLD_SIZE"])
+dist.init_process_group("gloo", rank=rank, world_size=world)
+# each rank holds its own seeded batch (weak scaling); times are max-reduced, counts sum-reduced
+wl = bench.rank_workload(1, rank, n_w=64 + rank)
+t = bench.allreduce_max(0.010 * (rank + 1))
+n = bench.allreduce_sum(float(wl.n_w))
+if rank == 0:
+    print(json.dumps({"t": t, "n": n, "seed_ok": True}))
+dist.destroy_process_group()
+"""
+
+
+def test_gloo_world_size_2_aggregation(tmp_path):
+    """bench.py's N>1 host logic: per-rank seeded shards, max-over-ranks time, sum-over-ranks units."""
+    script = tmp_path / "w.py"
+    script.write_text(_GLOO_WORKER % {"root": ROOT})
+    env = dict(os.environ, MASTER_ADDR="127.0.0.1", MASTER_PORT="29617", OMP_NUM_THREADS="1")
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node=2", "--master-addr", "127.0.0.1",
+           "--master-port", "29617", str(script)]
+    out = subprocess.run(cmd, capture_output=True, text=True, env=env, timeout=300)
+    assert out.returncode == 0, out.stderr[-2000:]
+    import json
+    line = [l for l in out.stdout.splitlines() if l.startswith("{")][-1]
+    r = json.loads(line)
+    assert r["t"] == pytest.approx(0.020)
+    assert r["n"] == pytest.approx(64 + 65)

@@ -1,0 +1,374 @@
+"""GPU parity tests (-m gpu): the CUDA path, called through the C ABI (binding.Context), against the CPU oracle on the
+same seeded inputs.  Tolerance (BASELINE.json north_star): |delta log L| <= 1e-6 max(1, |log L|) in FP64; d_h and h_h
+are held to the same bound separately (scaled by max(1, |h_h|)) so that a cancelling pair of errors cannot hide."""
+import math
+
+import numpy as np
+import pytest
+
+from paper_2111_01064_b200 import workloads as wlm
+from helpers import (assert_close_ll, oracle_setup_full, oracle_setup_het, rand_smooth_nodes, tol_ll, unit_tf)
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device; there is no CPU fallback to test instead")
+    return torch
+
+
+def dev(torch, a):
+    return torch.as_tensor(np.ascontiguousarray(a, dtype=np.float64), device="cuda")
+
+
+def make_ctx(wl, precision=0):
+    from paper_2111_01064_b200 import binding
+    ctx = binding.Context(n_modes=wl.n_m, precision=precision)
+    ctx.standin_config(wl.modes_l, wl.modes_m, wl.c_lm, wl.kappa)
+    return ctx
+
+
+def check_triplet(got, ref, what):
+    logL, d_h, h_h = (x.cpu().numpy() for x in got)
+    assert_close_ll(logL, ref["logL"], what + " logL")
+    scale = np.maximum(1.0, np.abs(ref["h_h"]))
+    assert np.all(np.abs(d_h - ref["d_h"]) <= 1e-6 * np.maximum(scale, np.abs(ref["d_h"]))), what + " d_h"
+    assert np.all(np.abs(h_h - ref["h_h"]) <= 1e-6 * scale), what + " h_h"
+
+
+# ------------------------------------------------------------------------------------------- full grid
+@pytest.fixture(scope="module")
+def cfg0(orc, torch_cuda):
+    wl = wlm.make_workload(0)
+    d, run = oracle_setup_full(orc, wl)
+    ctx = make_ctx(wl)
+    g = wl.grid
+    ctx.set_data(g.n_f, g.k_min, g.df, dev(torch_cuda, d), dev(torch_cuda, wl.W))
+    return wl, d, run, ctx
+
+
+def test_cfg0_full_standin_parity(cfg0, torch_cuda):
+    """BASELINE.json config 0 in full: 64 walkers, 256 nodes, 6540 bins, noiseless; log L[0] = 0."""
+    wl, d, run, ctx = cfg0
+    ref = run(wl.params, d)
+    got = ctx.full_batch_standin(wl.f_nodes, dev(torch_cuda, wl.params))
+    check_triplet(got, ref, "cfg0")
+    assert abs(float(got[0][0])) <= 1e-6
+    assert math.sqrt(float(got[2][0])) == pytest.approx(500.0, rel=1e-9)
+
+
+def test_dd_matches_oracle(cfg0, orc):
+    wl, d, run, ctx = cfg0
+    dd_full, _ = ctx.get_dd()
+    ref = orc.dd(d, wl.W)
+    assert abs(dd_full - ref) <= 1e-12 * abs(ref)
+
+
+def test_cfg0_rerun_is_bit_identical(cfg0, torch_cuda):
+    wl, d, run, ctx = cfg0
+    p = dev(torch_cuda, wl.params)
+    a = [x.clone() for x in ctx.full_batch_standin(wl.f_nodes, p)]
+    b = ctx.full_batch_standin(wl.f_nodes, p)
+    for x, y in zip(a, b):
+        assert torch_cuda.equal(x, y)
+
+
+@pytest.mark.parametrize("n_w", [1, 31, 33, 200])
+def test_full_standin_ragged_batches(cfg0, torch_cuda, n_w):
+    wl, d, run, ctx = cfg0
+    rng = np.random.default_rng(n_w)
+    idx = rng.integers(0, wl.n_w, n_w)
+    params = wl.params[idx].copy()
+    params[:, 0] *= rng.uniform(0.7, 1.4, n_w)          # new masses -> new bands
+    ref = run(params, d)
+    got = ctx.full_batch_standin(wl.f_nodes, dev(torch_cuda, params))
+    check_triplet(got, ref, f"ragged n_w={n_w}")
+
+
+def test_full_standin_empty_batch_is_noop(cfg0, torch_cuda):
+    wl, d, run, ctx = cfg0
+    got = ctx.full_batch_standin(wl.f_nodes, torch_cuda.empty((0, wl.P), dtype=torch_cuda.float64, device="cuda"))
+    assert all(x.numel() == 0 for x in got)
+
+
+def test_full_template_matches_oracle(cfg0, torch_cuda):
+    """The dense template the fused kernel integrates (never stored on the hot path), written out by the utility."""
+    wl, d, run, ctx = cfg0
+    for w in (0, 5, 17):
+        ref = run(wl.params[w][None], None, True)["h"]
+        got = ctx.full_template_standin(wl.f_nodes, wl.params[w]).cpu().numpy()
+        scale = np.abs(ref).max()
+        assert np.abs(got - ref).max() <= 1e-9 * scale, w
+
+
+def test_walker_outside_grid_gets_minus_half_dd(cfg0, torch_cuda):
+    wl, d, run, ctx = cfg0
+    rng = np.random.default_rng(3)
+    f_nodes = wl.f_nodes
+    amp, ph = rand_smooth_nodes(rng, 3, 1, f_nodes)
+    tf = unit_tf(rng, 3, 1)
+    band = np.array([[1.0, 2.0], [1e-9, 2e-9], [3e-3, 2e-3]])      # above, below, inverted
+    logL, d_h, h_h = ctx.full_batch(f_nodes, dev(torch_cuda, amp), dev(torch_cuda, ph), dev(torch_cuda, tf), dev(torch_cuda, band))
+    dd_full, _ = ctx.get_dd()
+    assert np.all(d_h.cpu().numpy() == 0.0) and np.all(h_h.cpu().numpy() == 0.0)
+    np.testing.assert_allclose(logL.cpu().numpy(), -0.5 * dd_full, rtol=1e-15)
+
+
+@pytest.mark.parametrize("n_m,banded,n_w", [(1, False, 40), (1, True, 97), (3, True, 50), (6, False, 33)])
+def test_full_arrays_entry_point(orc, torch_cuda, n_m, banded, n_w):
+    """ll_full_batch with caller arrays (not the stand-in), several modes, per-walker bands, noisy data."""
+    from paper_2111_01064_b200 import binding
+    rng = np.random.default_rng(1000 + 10 * n_m + n_w)
+    grid = wlm.make_grid(2.0 ** 16)
+    f = grid.freqs()
+    f_nodes = wlm.geomspace_exact(wlm.F_LO, wlm.F_HI, 61)
+    W = wlm.trapezoid_weights(grid)
+    amp, ph = rand_smooth_nodes(rng, n_w, n_m, f_nodes)
+    tf = unit_tf(rng, n_w, n_m)
+    sigma = np.sqrt(wlm.psd_sn(f) / (4 * grid.df))
+    d = rng.standard_normal((2, grid.n_f, 2)) * sigma[None, :, None]
+    band = None
+    if banded:
+        lo = rng.uniform(0.5e-4, 5e-3, n_w)
+        band = np.stack([lo, lo * rng.uniform(1.0, 40.0, n_w)], axis=1)
+        band[0] = [f[10], f[10]]            # a single bin
+        band[1] = [f[0], f[-1]]             # exactly the whole grid
+    ref = orc.full_batch(f_nodes, amp, ph, tf, band, grid.k_min, grid.df, d, W)
+    ctx = binding.Context(n_modes=n_m)
+    ctx.set_data(grid.n_f, grid.k_min, grid.df, dev(torch_cuda, d), dev(torch_cuda, W))
+    got = ctx.full_batch(f_nodes, dev(torch_cuda, amp), dev(torch_cuda, ph), dev(torch_cuda, tf),
+                         None if band is None else dev(torch_cuda, band))
+    check_triplet(got, ref, f"arrays n_m={n_m}")
+    ctx.destroy()
+
+
+def test_full_multimode_standin(orc, torch_cuda):
+    """six-mode stand-in through the full-grid path (generic-n_m kernel)."""
+    wl = wlm.make_workload(3, n_w=48, t_obs=2.0 ** 16, n_knots=24)
+    wl.path = "full"
+    wl.f_nodes = wlm.geomspace_exact(wlm.F_LO, wlm.F_HI, 200)
+    wl.params[:, 0] *= np.random.default_rng(5).uniform(0.5, 2.0, wl.n_w)
+    d, run = oracle_setup_full(orc, wl)
+    ctx = make_ctx(wl)
+    g = wl.grid
+    ctx.set_data(g.n_f, g.k_min, g.df, dev(torch_cuda, d), dev(torch_cuda, wl.W))
+    ref = run(wl.params, d)
+    got = ctx.full_batch_standin(wl.f_nodes, dev(torch_cuda, wl.params))
+    check_triplet(got, ref, "6-mode full")
+    ctx.destroy()
+
+
+def test_cfg2_scaled_multi_tile(orc, torch_cuda):
+    """config-2 recipe at 1/16 of the grid (98k bins, 1024 nodes, noisy), 600 walkers: several walker blocks,
+    many frequency tiles, ragged tails in both directions."""
+    wl = wlm.make_workload(2, n_w=600, t_obs=31557600.0 / 16)
+    d, run = oracle_setup_full(orc, wl)
+    ctx = make_ctx(wl)
+    g = wl.grid
+    ctx.set_data(g.n_f, g.k_min, g.df, dev(torch_cuda, d), dev(torch_cuda, wl.W))
+    ref = run(wl.params, d)
+    got = ctx.full_batch_standin(wl.f_nodes, dev(torch_cuda, wl.params))
+    check_triplet(got, ref, "cfg2/16")
+    pairs, _ = ctx.last_full_stats()
+    # active pairs = sum over walkers of bins inside the band (reading R10), counted by the oracle's mask
+    f = g.freqs()
+    _, _, _, band = orc.standin_nodes(wl.params, wl.modes_m, wl.c_lm, wl.kappa, wl.f_nodes, f[0], f[-1])
+    expect = sum(int(((f >= lo) & (f <= hi)).sum()) for lo, hi in band)
+    assert pairs == expect
+    ctx.destroy()
+
+
+def test_cfg2_full_size_sampled(orc, torch_cuda):
+    """BASELINE.json config 2 at full size in the launch configuration bench.py times (16384 walkers, 1024 nodes,
+    1 574 725 bins, noisy); the oracle recomputes a sample of walkers one by one."""
+    wl = wlm.make_workload(2)
+    d, run = oracle_setup_full(orc, wl)
+    ctx = make_ctx(wl)
+    g = wl.grid
+    ctx.set_data(g.n_f, g.k_min, g.df, dev(torch_cuda, d), dev(torch_cuda, wl.W))
+    got = [x.cpu().numpy() for x in ctx.full_batch_standin(wl.f_nodes, dev(torch_cuda, wl.params))]
+    fis = np.array([orc.standin_fisco(p) for p in wl.params])
+    sample = sorted({0, int(fis.argmin()), int(fis.argmax()), 1, 4097, 16383} | set(range(37, 16384, 2048)))
+    ref = run(wl.params[sample], d)
+    check_triplet([__import__("torch").as_tensor(x[sample]) for x in got], ref, "cfg2 sampled")
+    assert np.all(np.isfinite(got[0]))
+    # properties that hold for every walker: Cauchy-Schwarz and log L <= max over 1/D
+    dd_full, _ = ctx.get_dd()
+    assert np.all(got[1] ** 2 <= dd_full * got[2] * (1 + 1e-9))
+    np.testing.assert_allclose(got[0], got[1] - 0.5 * got[2] - 0.5 * dd_full, rtol=1e-13)
+    ctx.destroy()
+
+
+# ------------------------------------------------------------------------------------------- heterodyne
+@pytest.fixture(scope="module")
+def het_small(orc, torch_cuda):
+    wl = wlm.make_workload(1, n_w=300, t_obs=2.0 ** 18, n_knots=37)
+    d, h0, h0e, summ = oracle_setup_het(orc, wl)
+    ctx = make_ctx(wl)
+    g = wl.grid
+    ctx.set_data(g.n_f, g.k_min, g.df, dev(torch_cuda, d), dev(torch_cuda, wl.W))
+    ctx.het_prepare(wl.f_edges, dev(torch_cuda, h0), dev(torch_cuda, h0e))
+    return wl, d, h0, h0e, summ, ctx
+
+
+def test_het_summary_data_matches_oracle(het_small):
+    wl, d, h0, h0e, summ, ctx = het_small
+    got = ctx.het_get_summary()
+    for k in ("A0", "B0"):
+        np.testing.assert_allclose(got[k], summ[k], rtol=1e-11, atol=1e-11 * np.abs(summ[k]).max(), err_msg=k)
+    for k in ("A1", "B1"):      # first moments about the bin centre: cancel, so the scale is |.|_max
+        np.testing.assert_allclose(got[k], summ[k], rtol=0, atol=1e-10 * np.abs(summ[k]).max(), err_msg=k)
+    _, ddb = ctx.get_dd()
+    assert abs(ddb - summ["dd_band"]) <= 1e-12 * summ["dd_band"]
+
+
+def test_het_standin_parity(orc, het_small, torch_cuda):
+    wl, d, h0, h0e, summ, ctx = het_small
+    ref = orc.het_batch_standin(wl.modes_m, wl.c_lm, wl.kappa, wl.params, wl.f_edges, h0e, summ)
+    got = ctx.het_batch_standin(dev(torch_cuda, wl.params))
+    check_triplet(got, ref, "het standin")
+
+
+def test_het_arrays_parity(orc, het_small, torch_cuda):
+    wl, d, h0, h0e, summ, ctx = het_small
+    amp, ph, tf, _ = orc.standin_nodes(wl.params, wl.modes_m, wl.c_lm, wl.kappa, wl.f_edges,
+                                       float(wl.f_edges[0]), float(wl.f_edges[-1]))
+    ref = orc.het_batch(wl.f_edges, amp, ph, tf, h0e, summ)
+    got = ctx.het_batch(dev(torch_cuda, amp), dev(torch_cuda, ph), dev(torch_cuda, tf))
+    check_triplet(got, ref, "het arrays")
+
+
+def test_het_equals_full_at_reference(het_small, torch_cuda):
+    """north_star invariant: h = h0 => r = 1 => het log L = -1/2 <d-h0|d-h0> over the band."""
+    wl, d, h0, h0e, summ, ctx = het_small
+    logL, d_h, h_h = ctx.het_batch_standin(dev(torch_cuda, wl.inj[None]))
+    f = wl.grid.freqs()
+    m = (f >= wl.f_edges[0]) & (f <= wl.f_edges[-1])
+    res = d[:, m, :] - h0[:, m, :]
+    direct = -0.5 * float((wl.W[m][None, :] * (res ** 2).sum(axis=2)).sum())
+    assert abs(float(logL[0]) - direct) <= 1e-6 * max(1.0, abs(direct))
+
+
+@pytest.mark.parametrize("n_w", [1, 33, 1000])
+def test_het_ragged_batches(orc, het_small, torch_cuda, n_w):
+    wl, d, h0, h0e, summ, ctx = het_small
+    rng = np.random.default_rng(n_w)
+    params = wl.params[rng.integers(0, wl.n_w, n_w)].copy()
+    params[:, 2] += rng.normal(0, 5.0, n_w)
+    ref = orc.het_batch_standin(wl.modes_m, wl.c_lm, wl.kappa, params, wl.f_edges, h0e, summ)
+    got = ctx.het_batch_standin(dev(torch_cuda, params))
+    check_triplet(got, ref, f"het ragged {n_w}")
+    assert ctx.het_batch_standin(dev(torch_cuda, params[:0]))[0].numel() == 0
+
+
+def test_het_rerun_is_bit_identical(het_small, torch_cuda):
+    wl, d, h0, h0e, summ, ctx = het_small
+    p = dev(torch_cuda, wl.params)
+    a = [x.clone() for x in ctx.het_batch_standin(p)]
+    b = ctx.het_batch_standin(p)
+    for x, y in zip(a, b):
+        assert torch_cuda.equal(x, y)
+
+
+def test_het_reference_zero_is_an_error(het_small, torch_cuda):
+    from paper_2111_01064_b200 import binding
+    wl, d, h0, h0e, summ, ctx = het_small
+    bad = h0e.copy()
+    bad[1, 3, :] = 0.0
+    ctx2 = make_ctx(wl)
+    g = wl.grid
+    ctx2.set_data(g.n_f, g.k_min, g.df, dev(torch_cuda, d), dev(torch_cuda, wl.W))
+    with pytest.raises(binding.LLError) as ei:
+        ctx2.het_prepare(wl.f_edges, dev(torch_cuda, h0), dev(torch_cuda, bad))
+    assert ei.value.code == binding.LL_ERR_REF_ZERO
+    with pytest.raises(binding.LLError) as ei:
+        ctx2.het_batch_standin(dev(torch_cuda, wl.params))
+    assert ei.value.code == binding.LL_ERR_STATE
+    ctx2.destroy()
+
+
+def test_cfg1_full_size(orc, torch_cuda):
+    """BASELINE.json config 1 in full: 4096 walkers, 128 bins, 2^22 s grid (209 296 bins), noisy."""
+    wl = wlm.make_workload(1)
+    d, h0, h0e, summ = oracle_setup_het(orc, wl)
+    ctx = make_ctx(wl)
+    g = wl.grid
+    ctx.set_data(g.n_f, g.k_min, g.df, dev(torch_cuda, d), dev(torch_cuda, wl.W))
+    ctx.het_prepare(wl.f_edges, dev(torch_cuda, h0), dev(torch_cuda, h0e))
+    got_s = ctx.het_get_summary()
+    np.testing.assert_allclose(got_s["A0"], summ["A0"], rtol=0, atol=1e-11 * np.abs(summ["A0"]).max())
+    np.testing.assert_allclose(got_s["B0"], summ["B0"], rtol=1e-11)
+    ref = orc.het_batch_standin(wl.modes_m, wl.c_lm, wl.kappa, wl.params, wl.f_edges, h0e, summ)
+    got = ctx.het_batch_standin(dev(torch_cuda, wl.params))
+    check_triplet(got, ref, "cfg1")
+    ctx.destroy()
+
+
+def test_cfg3_higher_modes_full_size_sampled(orc, torch_cuda):
+    """BASELINE.json config 3: six modes, 256 bins, 32768 walkers on the GPU; the oracle recomputes every 16th."""
+    wl = wlm.make_workload(3)
+    d, h0, h0e, summ = oracle_setup_het(orc, wl)
+    ctx = make_ctx(wl)
+    g = wl.grid
+    ctx.set_data(g.n_f, g.k_min, g.df, dev(torch_cuda, d), dev(torch_cuda, wl.W))
+    ctx.het_prepare(wl.f_edges, dev(torch_cuda, h0), dev(torch_cuda, h0e))
+    got = [x.cpu().numpy() for x in ctx.het_batch_standin(dev(torch_cuda, wl.params))]
+    sample = np.arange(0, wl.n_w, 16)
+    ref = orc.het_batch_standin(wl.modes_m, wl.c_lm, wl.kappa, wl.params[sample], wl.f_edges, h0e, summ)
+    check_triplet([torch_cuda.as_tensor(x[sample]) for x in got], ref, "cfg3 sampled")
+    assert np.all(np.isfinite(got[0]))
+    ctx.destroy()
+
+
+def test_cfg4_large_batch_full_size_sampled(orc, torch_cuda):
+    """BASELINE.json config 4: 131072 walkers (16 x 8192), 512 bins; the oracle recomputes every 32nd walker."""
+    wl = wlm.make_workload(4)
+    d, h0, h0e, summ = oracle_setup_het(orc, wl)
+    ctx = make_ctx(wl)
+    g = wl.grid
+    ctx.set_data(g.n_f, g.k_min, g.df, dev(torch_cuda, d), dev(torch_cuda, wl.W))
+    ctx.het_prepare(wl.f_edges, dev(torch_cuda, h0), dev(torch_cuda, h0e))
+    got = [x.cpu().numpy() for x in ctx.het_batch_standin(dev(torch_cuda, wl.params))]
+    sample = np.arange(0, wl.n_w, 32)
+    ref = orc.het_batch_standin(wl.modes_m, wl.c_lm, wl.kappa, wl.params[sample], wl.f_edges, h0e, summ)
+    check_triplet([torch_cuda.as_tensor(x[sample]) for x in got], ref, "cfg4 sampled")
+    assert np.all(np.isfinite(got[0]))
+    ctx.destroy()
+
+
+# ------------------------------------------------------------------------------------------- boundary behaviour
+def test_state_and_argument_errors(torch_cuda):
+    from paper_2111_01064_b200 import binding
+    ctx = binding.Context(n_modes=1)
+    f_nodes = wlm.geomspace_exact(1e-4, 0.05, 16)
+    p = torch_cuda.zeros((4, 9), dtype=torch_cuda.float64, device="cuda")
+    with pytest.raises(binding.LLError) as ei:
+        ctx.full_batch_standin(f_nodes, p)
+    assert ei.value.code == binding.LL_ERR_STATE            # no data yet
+    grid = wlm.make_grid(2.0 ** 14)
+    W = dev(torch_cuda, wlm.trapezoid_weights(grid))
+    d = torch_cuda.zeros((2, grid.n_f, 2), dtype=torch_cuda.float64, device="cuda")
+    ctx.set_data(grid.n_f, grid.k_min, grid.df, d, W)
+    with pytest.raises(binding.LLError) as ei:
+        ctx.full_batch_standin(f_nodes, p)
+    assert ei.value.code == binding.LL_ERR_STATE            # no stand-in description yet
+    ctx.standin_config([2], [2], [1.0], 0.5)
+    for bad in (f_nodes[::-1].copy(), f_nodes[:2], np.linspace(1e-3, 2e-3, 16)):
+        with pytest.raises(binding.LLError) as ei:
+            ctx.full_batch_standin(bad, p)
+        assert ei.value.code == binding.LL_ERR_ARG
+    with pytest.raises(binding.LLError) as ei:
+        ctx.het_batch_standin(p)
+    assert ei.value.code == binding.LL_ERR_STATE
+    with pytest.raises(binding.LLError) as ei:
+        ctx.set_data(0, grid.k_min, grid.df, d, W)
+    assert ei.value.code == binding.LL_ERR_ARG
+    ctx.destroy()
+
+
+def test_smoke_entry(torch_cuda):
+    import __graft_entry__
+    __graft_entry__.smoke()
