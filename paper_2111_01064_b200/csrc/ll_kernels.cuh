@@ -724,19 +724,21 @@ __device__ __forceinline__ void het_bin_contract(const double *__restrict__ tb, 
     hh = fma(tb[11], fma(sEr, dEr, sEi * dEi), hh);
 }
 
-// Stand-in parameters -> log L.  Block = 32 walkers x S frequency segments (warp s walks segment s); lanes of
-// a warp are 32 different walkers at the same edge, so every table read is a broadcast.
+// Stand-in parameters -> log L.  Block = 32 lanes x (G walker groups x S frequency segments) warps sharing ONE
+// copy of the table: warp (g, s) walks segment s of the bins for the 32 walkers of group g.  Lanes of a warp
+// are 32 different walkers at the same edge, so every table read is a broadcast.  Blocks stride over passes of
+// G groups; the S partial sums of a group meet in shared memory in segment order (deterministic).
 template <int NM>
 __global__ void __launch_bounds__(512)
-k_het_standin(HetTable T, StandinInfo si, const double *__restrict__ params, int P, int n_w, int n_groups,
+k_het_standin(HetTable T, StandinInfo si, const double *__restrict__ params, int P, int n_w, int n_groups, int S,
               const double *__restrict__ dd, double *__restrict__ logL, double *__restrict__ d_h,
               double *__restrict__ h_h)
 {
     extern __shared__ __align__(16) double tab[];
-    double *red = tab + T.total; // [S][2][32]
+    double *red = tab + T.total; // [G][S][2][32]
     for (int i = threadIdx.x + threadIdx.y * 32; i < T.total; i += 32 * blockDim.y) tab[i] = T.base[i];
     __syncthreads();
-    const int S = blockDim.y, seg = threadIdx.y, lane = threadIdx.x;
+    const int G = blockDim.y / S, seg = threadIdx.y % S, gslot = threadIdx.y / S, lane = threadIdx.x;
     const int per = (T.n_b + S - 1) / S;
     const int b0 = seg * per, b1 = min(b0 + per, T.n_b);
     const double *f4 = tab + T.off_f4(), *ih0 = tab + T.off_ih0(), *cfp = tab + T.off_cfp(),
@@ -744,9 +746,10 @@ k_het_standin(HetTable T, StandinInfo si, const double *__restrict__ params, int
     const double inv_kappa = 1.0 / si.kappa;
     const double ddb = dd[1];
 
-    for (int grp = blockIdx.x; grp < n_groups; grp += gridDim.x) {
+    for (int base = blockIdx.x * G; base < n_groups; base += gridDim.x * G) {
+        const int grp = base + gslot;
         const int w = grp * 32 + lane;
-        const bool valid = w < n_w;
+        const bool valid = grp < n_groups && w < n_w;
         const double *row = params + (size_t)(valid ? w : 0) * P;
         const WalkerConst c = standin_consts(row);
         double Kq[NM], phq[NM], tf[NM][4];
@@ -760,6 +763,7 @@ k_het_standin(HetTable T, StandinInfo si, const double *__restrict__ params, int
         }
         double dh = 0.0, hh = 0.0;
         double pAr = 0, pAi = 0, pEr = 0, pEi = 0;
+        if (grp < n_groups)
         for (int e = b0; e <= b1 && b0 < b1; ++e) {
             double hAr = 0, hAi = 0, hEr = 0, hEi = 0;
             const double f4e = f4[e];
@@ -783,12 +787,13 @@ k_het_standin(HetTable T, StandinInfo si, const double *__restrict__ params, int
             pAr = rAr; pAi = rAi; pEr = rEr; pEi = rEi;
         }
         if (S > 1) {
-            red[(seg * 2) * 32 + lane] = dh;
-            red[(seg * 2 + 1) * 32 + lane] = hh;
+            double *rg = red + (size_t)gslot * S * 64;
+            rg[(seg * 2) * 32 + lane] = dh;
+            rg[(seg * 2 + 1) * 32 + lane] = hh;
             __syncthreads();
             if (seg == 0) {
                 dh = 0.0; hh = 0.0;
-                for (int s = 0; s < S; ++s) { dh += red[(s * 2) * 32 + lane]; hh += red[(s * 2 + 1) * 32 + lane]; }
+                for (int s = 0; s < S; ++s) { dh += rg[(s * 2) * 32 + lane]; hh += rg[(s * 2 + 1) * 32 + lane]; }
             }
         }
         if (seg == 0 && valid) {
