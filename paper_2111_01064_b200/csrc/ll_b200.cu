@@ -533,6 +533,7 @@ int ll_set_data(ll_ctx *ctx, int64_t n_f, int64_t k_min, double df, const double
     if (!d || !W) return ctx->fail(LL_ERR_ARG, "d or W is NULL");
     if (n_f < 1 || n_f > (1LL << 30)) return ctx->fail(LL_ERR_ARG, "n_f out of range [1, 2^30]");
     if (k_min < 0 || !(df > 0.0) || !std::isfinite(df)) return ctx->fail(LL_ERR_ARG, "k_min < 0 or df not positive");
+    if (k_min + n_f >= (1LL << 31)) return ctx->fail(LL_ERR_ARG, "k_min + n_f must stay below 2^31 (bin numbers are int32 on the device)");
     DeviceGuard dg(ctx->device);
     cudaStream_t st = (cudaStream_t)stream;
     ctx->have_data = false;

@@ -17,39 +17,59 @@ constexpr double kPio2_2 = 0x1.1a62633145c07p-54;
 constexpr double kPio2_3 = -0x1.f1976b7ed8fbcp-110;
 constexpr double kSixth = 0x1.5555555555555p-3;
 
-// sin(pi r/2) = r * S(r^2), cos(pi r/2) = C(r^2), |r| <= 1/2: Taylor series of the scaled argument,
-// coefficients rounded from 50-digit values; truncation + coefficient error < 1e-16 (sin), 3e-17 (cos).
+// sin(pi r/2) = r * S(r^2), cos(pi r/2) = C(r^2), |r| <= 1/2.  S and C are degree-6 polynomials in r^2
+// interpolated at the Chebyshev nodes of [0, 1/4] (gen_sincos_coeffs.py; max error 2.6e-17 (sin), 1.0e-16
+// (cos) before evaluation rounding).  The coefficients live in constant memory so that every Horner step is
+// one DFMA with a constant-bank operand (no UMOV/IMAD.MOV literal rebuilds inside the hot loop).
+__constant__ double kSinC[7] = {0x1.921fb54442d18p+0,  -0x1.4abbce625be41p-1, 0x1.466bc677587f8p-4, -0x1.32d2cce2e5b19p-8,
+                                0x1.50782fda12d96p-13, -0x1.e30071afc3e59p-19, 0x1.e3f38399551bfp-25};
+__constant__ double kCosC[7] = {0x1.0000000000000p+0,  -0x1.3bd3cc9be458bp+0, 0x1.03c1f081b0780p-2, -0x1.55d3c7dbfd139p-6,
+                                0x1.e1f4fb60281f6p-11, -0x1.a6c9c1be9eb49p-16, 0x1.f3dbcea61b1a4p-22};
+
 __device__ __forceinline__ void sincos_poly_qc(double r, double &s, double &c)
 {
     const double r2 = r * r;
-    double ps = -0x1.6fadb9f155744p-31;
-    ps = fma(ps, r2, 0x1.e8f434d018d63p-25);
-    ps = fma(ps, r2, -0x1.e3074fde8871fp-19);
-    ps = fma(ps, r2, 0x1.50783487ee782p-13);
-    ps = fma(ps, r2, -0x1.32d2cce62bd86p-8);
-    ps = fma(ps, r2, 0x1.466bc6775aae2p-4);
-    ps = fma(ps, r2, -0x1.4abbce625be53p-1);
-    ps = fma(ps, r2, 0x1.921fb54442d18p+0);
-    double pc = 0x1.20c62c2f2d7f5p-34;
-    pc = fma(pc, r2, -0x1.b6e24f44b128fp-28);
-    pc = fma(pc, r2, 0x1.f9d38a3763cc3p-22);
-    pc = fma(pc, r2, -0x1.a6d1f2a204a8cp-16);
-    pc = fma(pc, r2, 0x1.e1f506891babbp-11);
-    pc = fma(pc, r2, -0x1.55d3c7e3cbffap-6);
-    pc = fma(pc, r2, 0x1.03c1f081b5ac4p-2);
-    pc = fma(pc, r2, -0x1.3bd3cc9be45dep+0);
-    pc = fma(pc, r2, 1.0);
+    double ps = fma(kSinC[6], r2, kSinC[5]);
+    double pc = fma(kCosC[6], r2, kCosC[5]);
+    ps = fma(ps, r2, kSinC[4]);
+    pc = fma(pc, r2, kCosC[4]);
+    ps = fma(ps, r2, kSinC[3]);
+    pc = fma(pc, r2, kCosC[3]);
+    ps = fma(ps, r2, kSinC[2]);
+    pc = fma(pc, r2, kCosC[2]);
+    ps = fma(ps, r2, kSinC[1]);
+    pc = fma(pc, r2, kCosC[1]);
+    ps = fma(ps, r2, kSinC[0]);
+    pc = fma(pc, r2, kCosC[0]);
     s = ps * r;
     c = pc;
 }
 
-// quadrant bookkeeping: angle = (pi/2)(n + r); q = n mod 4
+// quadrant bookkeeping: angle = (pi/2)(n + r); q = n mod 4.  Integer-pipe only (selects and sign-bit XORs on
+// the high words), so it costs no FP64 issue slot.
+__device__ __forceinline__ double flip_sign_if(double x, unsigned mask /* 0 or 0x80000000 */)
+{
+    return __hiloint2double(__double2hiint(x) ^ (int)mask, __double2loint(x));
+}
 __device__ __forceinline__ void quadrant_fix(int q, double s, double c, double &sn, double &cs)
 {
-    const double a = (q & 1) ? c : s;
-    const double b = (q & 1) ? s : c;
-    sn = (q & 2) ? -a : a;
-    cs = ((q + 1) & 2) ? -b : b;
+    const bool sw = q & 1;
+    const double a = sw ? c : s;
+    const double b = sw ? s : c;
+    sn = flip_sign_if(a, ((unsigned)q << 30) & 0x80000000u);
+    cs = flip_sign_if(b, ((unsigned)(q + 1) << 30) & 0x80000000u);
+}
+// as quadrant_fix, but returns e = amp * (cos, sin) with the signs folded into amp and the swap
+__device__ __forceinline__ void quadrant_apply(int q, double amp, double s, double c, double &u, double &v)
+{
+    // sn = sg * a, cs = sg * (sw ? -s : c), sg = (q & 2) ? -1 : 1, a = sw ? c : s
+    const bool sw = q & 1;
+    const double ms = flip_sign_if(s, 0x80000000u);
+    const double a = sw ? c : s;
+    const double b = sw ? ms : c;
+    const double as = flip_sign_if(amp, ((unsigned)q << 30) & 0x80000000u);
+    u = as * b;
+    v = as * a;
 }
 
 // sin and cos of an angle given in quarter cycles (y = angle * 2/pi).
@@ -62,6 +82,17 @@ __device__ __forceinline__ void sincos_qc(double y, double &sn, double &cs)
     double s, c;
     sincos_poly_qc(r, s, c);
     quadrant_fix(q, s, c, sn, cs);
+}
+// u - i v = amp * exp(-i (pi/2) y)
+__device__ __forceinline__ void amp_expi_qc(double amp, double y, double &u, double &v)
+{
+    const double sh = __dadd_rn(y, kMagic);
+    const int q = __double2loint(sh);
+    const double nd = __dadd_rn(sh, -kMagic);
+    const double r = __dadd_rn(y, -nd);
+    double s, c;
+    sincos_poly_qc(r, s, c);
+    quadrant_apply(q, amp, s, c, u, v);
 }
 
 // sin and cos of an angle in radians, accurate for |x| up to ~1e9 (three-term Cody-Waite with FMA; the

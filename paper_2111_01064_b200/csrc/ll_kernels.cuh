@@ -400,6 +400,33 @@ __device__ __forceinline__ int find_interval_of_bin(const int *__restrict__ bsta
     return lo;
 }
 
+// bins [b0, b1) of one spline interval for the single-mode kernel: t, the two cubics, A e^{-i Psi}, the two
+// complex MACs with g^A, g^E and W A^2.  MASK = per-lane band test (only at the ragged ends of a warp's band).
+template <bool MASK>
+__device__ __forceinline__ void fused_bins_nm1(int b0, int b1, int tlo, int thi, int kbase, double df, double nxj,
+                                               double cA0, double cA1, double cA2, double cA3, double cP0, double cP1,
+                                               double cP2, double cP3, const double4 *__restrict__ sg4,
+                                               const double *__restrict__ sWc, double &sAr, double &sAi, double &sEr,
+                                               double &sEi, double &sH)
+{
+#pragma unroll 2
+    for (int ii = b0; ii < b1; ++ii) {
+        const double t = fma((double)(kbase + ii), df, nxj);
+        double A = fma(fma(fma(cA3, t, cA2), t, cA1), t, cA0);
+        const double y = fma(fma(fma(cP3, t, cP2), t, cP1), t, cP0);
+        if (MASK) A = ((ii >= tlo) && (ii < thi)) ? A : 0.0;
+        double u, v; // h = u - i v
+        amp_expi_qc(A, y, u, v);
+        const double4 g = sg4[ii];
+        const double w = sWc[ii];
+        sAr = fma(g.x, u, sAr); sAr = fma(g.y, v, sAr);
+        sAi = fma(g.y, u, sAi); sAi = fma(-g.x, v, sAi);
+        sEr = fma(g.z, u, sEr); sEr = fma(g.w, v, sEr);
+        sEi = fma(g.w, u, sEi); sEi = fma(-g.z, v, sEi);
+        sH = fma(w * A, A, sH);
+    }
+}
+
 template <int NM1> // NM1 = 1: single-mode specialisation (NQ = 5); 0: any n_m (NQ = 2)
 __global__ void __launch_bounds__(128, 4) k_full_fused(FusedArgs a)
 {
@@ -445,6 +472,7 @@ __global__ void __launch_bounds__(128, 4) k_full_fused(FusedArgs a)
     int j = find_interval_of_bin(a.bstart, a.n_nodes, blo);
     int jl = -1;
     double cA0 = 0, cA1 = 0, cA2 = 0, cA3 = 0, cP0 = 0, cP1 = 0, cP2 = 0, cP3 = 0, nxj = 0;
+    const int kbase = (int)a.k_min; // k_min + n_f < 2^31 is checked on the host
     double sAr = 0, sAi = 0, sEr = 0, sEi = 0, sH = 0; // NM1: S^A, S^E, H;  generic: sAr = d_h, sH = h_h
 
     for (int c = c_begin; c < c_end; ++c) {
@@ -473,25 +501,21 @@ __global__ void __launch_bounds__(128, 4) k_full_fused(FusedArgs a)
                         nxj = -__ldg(a.xj + j);
                         jl = j;
                     }
-                    double kd = (double)(a.k_min + wlo);
-#pragma unroll 2
-                    for (int ii = wlo; ii < whi; ++ii) {
-                        const bool act = (ii >= tlo) && (ii < thi);
-                        const double t = fma(kd, a.df, nxj);
-                        kd += 1.0;
-                        double A = fma(fma(fma(cA3, t, cA2), t, cA1), t, cA0);
-                        const double y = fma(fma(fma(cP3, t, cP2), t, cP1), t, cP0);
-                        A = act ? A : 0.0;
-                        double sn, cs;
-                        sincos_qc(y, sn, cs);
-                        const double u = A * cs, v = A * sn; // h = u - i v
-                        const double4 g = reinterpret_cast<const double4 *>(sg)[ii - cb];
-                        const double w = sW[ii - cb];
-                        sAr = fma(g.x, u, sAr); sAr = fma(g.y, v, sAr);
-                        sAi = fma(g.y, u, sAi); sAi = fma(-g.x, v, sAi);
-                        sEr = fma(g.z, u, sEr); sEr = fma(g.w, v, sEr);
-                        sEi = fma(g.w, u, sEi); sEi = fma(-g.z, v, sEi);
-                        sH = fma(w * A, A, sH);
+                    // bins every lane of the warp has inside its band run without the per-lane mask
+                    const int flo = __reduce_max_sync(0xffffffffu, max(lo, i));
+                    const int fhi = __reduce_min_sync(0xffffffffu, min(hi, seg_end));
+                    const double4 *sg4 = reinterpret_cast<const double4 *>(sg) - cb;
+                    const double *sWc = sW - cb;
+                    if (flo < fhi) {
+                        fused_bins_nm1<true>(wlo, flo, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1, cP2, cP3,
+                                             sg4, sWc, sAr, sAi, sEr, sEi, sH);
+                        fused_bins_nm1<false>(flo, fhi, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1, cP2, cP3,
+                                              sg4, sWc, sAr, sAi, sEr, sEi, sH);
+                        fused_bins_nm1<true>(fhi, whi, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1, cP2, cP3,
+                                             sg4, sWc, sAr, sAi, sEr, sEi, sH);
+                    } else {
+                        fused_bins_nm1<true>(wlo, whi, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1, cP2, cP3,
+                                             sg4, sWc, sAr, sAi, sEr, sEi, sH);
                     }
                 } else {
                     nxj = -__ldg(a.xj + j);
