@@ -38,6 +38,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     cmd = [nvcc_path(), "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
            "-Xcompiler", "-fPIC", "-shared", "-I", os.path.join(ROOT, "include"), "-I", CSRC,
            "-o", SO] + SOURCES
+    cmd[1:1] = os.environ.get("LL_NVCC_FLAGS", "").split()  # e.g. -DLL_FUSED_UNROLL=4 for tuning sweeps
     if verbose:
         cmd.insert(1, "-Xptxas=-v")
         print(" ".join(cmd), file=sys.stderr)

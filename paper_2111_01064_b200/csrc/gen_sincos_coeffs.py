@@ -26,6 +26,7 @@ def C(u):
 
 
 def cheb_fit(F, n):
+    global A, B
     xs = [(A + B) / 2 + (B - A) / 2 * mp.cos(mp.pi * (2 * k + 1) / (2 * (n + 1))) for k in range(n + 1)]
     M = mp.matrix(n + 1, n + 1)
     y = mp.matrix(n + 1, 1)
@@ -58,8 +59,49 @@ def emit(name, F, n, dtype, weight):
     print("    " + ", ".join(lits))
 
 
+# FP32-accumulate variant (reading R15): argument in radians, |x| <= pi/4, leading terms exact in binary
+# (sin x = x + x^3 S1(x^2), cos x = 1 - x^2/2 + x^4 C2(x^2)) so that no coefficient rounding is coherent at
+# the 1e-8 level.
+def S1(u):
+    if u == 0:
+        return -mp.mpf(1) / 6
+    x = mp.sqrt(u)
+    return (mp.sin(x) / x - 1) / u
+
+
+def C2(u):
+    if u == 0:
+        return mp.mpf(1) / 24
+    return (mp.cos(mp.sqrt(u)) - 1 + u / 2) / (u * u)
+
+
+def emit_f32_sequential(name, F, n, weight):
+    """float-aware fit: weighted least squares on 200 Chebyshev points; round the lowest free coefficient to
+    binary32, freeze it, refit the remaining ones to what is left, repeat"""
+    us = [(A + B) / 2 + (B - A) / 2 * mp.cos(mp.pi * (2 * k + 1) / 400) for k in range(200)]
+    fs = [F(u) for u in us]
+    ws = [weight(u) for u in us]
+    fixed = []
+    for k in range(n + 1):
+        free = list(range(k, n + 1))
+        M = mp.matrix(len(us), len(free))
+        y = mp.matrix(len(us), 1)
+        for i, u in enumerate(us):
+            for jj, pw in enumerate(free):
+                M[i, jj] = ws[i] * u ** pw
+            y[i] = ws[i] * (fs[i] - sum(c * u ** q for q, c in enumerate(fixed)))
+        c = mp.lu_solve(M.T * M, M.T * y)
+        fixed.append(mp.mpf(float(np.float32(float(c[0])))))
+    out = [float(x) for x in fixed]
+    print(f"// {name}: {n + 1} coefficients (f32, sequentially rounded), low order first; "
+          f"max |error| {mp.nstr(max_err(F, out, weight), 3)}")
+    print("    " + ", ".join(float.hex(x) + "f" for x in out))
+
+
 if __name__ == "__main__":
     emit("S (sin(pi r/2)/r), error weighted by r", S, 6, "f64", lambda u: mp.sqrt(u))
     emit("C (cos(pi r/2))", C, 6, "f64", lambda u: 1)
-    emit("S32", S, 4, "f32", lambda u: mp.sqrt(u))
-    emit("C32", C, 4, "f32", lambda u: 1)
+    B = (mp.pi / 4) ** 2
+    emit_f32_sequential("S1 (sin x = x + x^3 S1(x^2)), error weighted by x^3", S1, 3, lambda u: mp.sqrt(u) ** 3)
+    emit_f32_sequential("C2 (cos x = 1 - x^2/2 + x^4 C2(x^2)), error weighted by x^4", C2, 2, lambda u: u * u)
+    emit_f32_sequential("C2, 4 coefficients", C2, 3, lambda u: u * u)

@@ -72,6 +72,7 @@ struct ll_ctx {
     long long n_f = 0, n_f_pad = 0, k_min = 0;
     double df = 0.0;
     DevBuf g4, Wd, dd_part, dd; // dd: [0] full grid, [1] het band
+    DevBuf g4f, Wf, scale, wmax; // FP32-accumulate variant: g/sigma in binary32, W/sigma^2 in FP64, (sigma, 1/sigma, 1/sigma^2)
     DevBuf pairs;               // unsigned long long [1]
 
     // stand-in
@@ -336,9 +337,13 @@ int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, cons
     }
     {
         dim3 grid(n_wp / pl.WB, pl.n_tiles);
-        const size_t smem = (size_t)2 * pl.CH * 40;
+        const bool mixed = ctx->precision == LL_PREC_FP32_ACC;
+        const size_t smem = (size_t)2 * pl.CH * (mixed ? 24 : 40);
         ProfScope prof(ctx, st);
-        if (nm1) k_full_fused<1><<<grid, pl.WB, smem, st>>>(fa);
+        if (mixed) {
+            const FusedArgsF32 fm{ctx->g4f.as<float>(), ctx->Wf.as<double>(), ctx->scale.as<double>()};
+            k_full_fused_mixed<<<grid, pl.WB, smem, st>>>(fa, fm);
+        } else if (nm1) k_full_fused<1><<<grid, pl.WB, smem, st>>>(fa);
         else k_full_fused<0><<<grid, pl.WB, smem, st>>>(fa);
         LAUNCHED(ctx);
         ctx->last_n_blocks = (int)(grid.x * grid.y);
@@ -363,7 +368,8 @@ int check_full_common(ll_ctx *ctx, int64_t n_w, const double *f_nodes, const dou
     if (!f_nodes) return ctx->fail(LL_ERR_ARG, "f_nodes is NULL");
     if (n_w > 0 && !logL) return ctx->fail(LL_ERR_ARG, "logL is NULL");
     if (!ctx->have_data) return ctx->fail(LL_ERR_STATE, "ll_set_data has not been called");
-    if (ctx->precision != LL_PREC_FP64) return ctx->fail(LL_ERR_UNSUPPORTED, "FP32-accumulate variant not built yet");
+    if (ctx->precision == LL_PREC_FP32_ACC && ctx->n_m != 1)
+        return ctx->fail(LL_ERR_UNSUPPORTED, "the FP32-accumulate variant is built for n_modes = 1 only");
     return LL_OK;
 }
 
@@ -515,7 +521,7 @@ int ll_destroy(ll_ctx *ctx)
         DevBuf *all[] = {&ctx->g4, &ctx->Wd, &ctx->dd_part, &ctx->dd, &ctx->pairs, &ctx->node_tab, &ctx->ilo_w, &ctx->ihi_w,
                          &ctx->key_w, &ctx->hist, &ctx->perm, &ctx->ilo_s, &ctx->ihi_s, &ctx->Y, &ctx->C, &ctx->TF,
                          &ctx->part, &ctx->prow, &ctx->het_tab, &ctx->het_raw, &ctx->het_idx, &ctx->het_fb,
-                         &ctx->stage_in, &ctx->stage_out};
+                         &ctx->stage_in, &ctx->stage_out, &ctx->g4f, &ctx->Wf, &ctx->scale, &ctx->wmax};
         for (DevBuf *b : all) b->release();
         for (auto &e : ctx->ev) cudaEventDestroy(e);
     }
@@ -552,6 +558,20 @@ int ll_set_data(ll_ctx *ctx, int64_t n_f, int64_t k_min, double df, const double
     LAUNCHED(ctx);
     k_sum_parts<<<1, 256, 0, st>>>(ctx->dd_part.as<double>(), nb, ctx->dd.as<double>());
     LAUNCHED(ctx);
+    if (ctx->precision == LL_PREC_FP32_ACC) {
+        CK(ctx->g4f.ensure(sizeof(float) * 4 * n_pad));
+        CK(ctx->Wf.ensure(sizeof(double) * n_pad));
+        CK(ctx->scale.ensure(sizeof(double) * 4));
+        CK(ctx->wmax.ensure(sizeof(unsigned long long)));
+        CK(cudaMemsetAsync(ctx->wmax.p, 0, sizeof(unsigned long long), st));
+        k_wmax<<<nb, 256, 0, st>>>(W, n_f, ctx->wmax.as<unsigned long long>());
+        LAUNCHED(ctx);
+        k_scale_from_wmax<<<1, 1, 0, st>>>(ctx->wmax.as<unsigned long long>(), ctx->scale.as<double>());
+        LAUNCHED(ctx);
+        k_prescale_f32<<<ceil_div(n_pad, 256), 256, 0, st>>>(ctx->g4.as<double>(), ctx->Wd.as<double>(), n_pad,
+                                                             ctx->scale.as<double>(), ctx->g4f.as<float>(), ctx->Wf.as<double>());
+        LAUNCHED(ctx);
+    }
     ctx->n_f = n_f;
     ctx->n_f_pad = n_pad;
     ctx->k_min = k_min;

@@ -95,6 +95,46 @@ __device__ __forceinline__ void amp_expi_qc(double amp, double y, double &u, dou
     quadrant_apply(q, amp, s, c, u, v);
 }
 
+// ---- FP32-accumulate variant (reading R15) --------------------------------------------------------
+// sin x = x + x^3 S1(x^2), cos x = 1 - x^2/2 + x^4 C2(x^2), |x| <= pi/4, binary32.  The leading terms are exact
+// in binary and the remaining coefficients were fitted after rounding their predecessors
+// (gen_sincos_coeffs.py: max polynomial error 7.0e-11 (sin), 1.1e-10 (cos)), so the only error left at the
+// 1e-8 level is the evaluation rounding, which is incoherent from bin to bin.
+__device__ __forceinline__ void sincos_poly_f32(float x, float &s, float &c)
+{
+    const float x2 = x * x;
+    float ps = fmaf(0x1.7658e0p-19f, x2, -0x1.a0423ap-13f);
+    float pc = fmaf(0x1.99ead0p-16f, x2, -0x1.6c0c2ep-10f);
+    ps = fmaf(ps, x2, 0x1.11115ep-7f);
+    pc = fmaf(pc, x2, 0x1.55554ap-5f);
+    ps = fmaf(ps, x2, -0x1.555556p-3f);
+    pc = fmaf(pc, x2, -0.5f);
+    s = fmaf(x * x2, ps, x);
+    c = fmaf(pc, x2, 1.0f);
+}
+__device__ __forceinline__ float flip_sign_if_f32(float x, unsigned mask /* 0 or 0x80000000 */)
+{
+    return __uint_as_float(__float_as_uint(x) ^ mask);
+}
+// u - i v = amp * exp(-i (pi/2) y): the phase y (quarter cycles) is reduced to [-1/2, 1/2] in FP64, scaled to
+// radians in FP64 (so that the pi/2 factor is not rounded to binary32), then everything else is binary32.
+__device__ __forceinline__ void amp_expi_qc_f32(float amp, double y, float &u, float &v)
+{
+    const double sh = __dadd_rn(y, kMagic);
+    const int q = __double2loint(sh);
+    const double nd = __dadd_rn(sh, -kMagic);
+    const double r = __dadd_rn(y, -nd);
+    const float x = __double2float_rn(r * kPio2_1);
+    float s, c;
+    sincos_poly_f32(x, s, c);
+    const bool sw = q & 1;
+    const float a = sw ? c : s;
+    const float b = sw ? -s : c;
+    const float as = flip_sign_if_f32(amp, ((unsigned)q << 30) & 0x80000000u);
+    u = as * b;
+    v = as * a;
+}
+
 // sin and cos of an angle in radians, accurate for |x| up to ~1e9 (three-term Cody-Waite with FMA; the
 // reduced argument is then handed to the quarter-cycle polynomials).
 __device__ __forceinline__ void sincos_rad(double x, double &sn, double &cs)

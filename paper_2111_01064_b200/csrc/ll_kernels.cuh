@@ -400,6 +400,13 @@ __device__ __forceinline__ int find_interval_of_bin(const int *__restrict__ bsta
     return lo;
 }
 
+#ifndef LL_FUSED_UNROLL
+#define LL_FUSED_UNROLL 4 // bins in flight per thread in the hot loop (tuned on B200, profiles/)
+#endif
+#ifndef LL_FUSED_MINB
+#define LL_FUSED_MINB 4 // resident 128-thread blocks per SM the register budget is held to
+#endif
+constexpr int kFusedUnroll = LL_FUSED_UNROLL;
 // bins [b0, b1) of one spline interval for the single-mode kernel: t, the two cubics, A e^{-i Psi}, the two
 // complex MACs with g^A, g^E and W A^2.  MASK = per-lane band test (only at the ragged ends of a warp's band).
 template <bool MASK>
@@ -409,7 +416,7 @@ __device__ __forceinline__ void fused_bins_nm1(int b0, int b1, int tlo, int thi,
                                                const double *__restrict__ sWc, double &sAr, double &sAi, double &sEr,
                                                double &sEi, double &sH)
 {
-#pragma unroll 2
+#pragma unroll kFusedUnroll
     for (int ii = b0; ii < b1; ++ii) {
         const double t = fma((double)(kbase + ii), df, nxj);
         double A = fma(fma(fma(cA3, t, cA2), t, cA1), t, cA0);
@@ -428,7 +435,7 @@ __device__ __forceinline__ void fused_bins_nm1(int b0, int b1, int tlo, int thi,
 }
 
 template <int NM1> // NM1 = 1: single-mode specialisation (NQ = 5); 0: any n_m (NQ = 2)
-__global__ void __launch_bounds__(128, 4) k_full_fused(FusedArgs a)
+__global__ void __launch_bounds__(128, LL_FUSED_MINB) k_full_fused(FusedArgs a)
 {
     extern __shared__ __align__(128) double sm[];
     __shared__ __align__(8) uint64_t bar[2];
@@ -561,6 +568,190 @@ __global__ void __launch_bounds__(128, 4) k_full_fused(FusedArgs a)
         double *o = a.part + ((size_t)tile * 2) * sw + p;
         o[0] = sAr; o[sw] = sH;
     }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// F3, FP32-accumulate variant (BASELINE.json config 2; reading R15), single mode.
+// FP64: bin frequency offset t, phase and amplitude cubics, reduction of the phase to [-1/2, 1/2] quarter
+// cycles and its scaling to radians, <h|h> = sum W A^2 (all terms positive: binary32 partial sums would lose
+// ~1e-7 of it), every sum longer than kMixedChain terms.  binary32: sin/cos polynomials, A e^{-i Psi}, the
+// products with the pre-scaled binary32 data tile and <d|h> partial sums of <= kMixedChain terms.
+// The data are pre-scaled by a power of two sigma (g/sigma in binary32, W/sigma^2 in FP64; amplitudes * sigma)
+// so that every binary32 quantity is O(1): k_prescale_f32.
+// ---------------------------------------------------------------------------------------------------
+constexpr int kMixedChain = 8;
+
+// scale[0] = sigma = 2^ceil(log2(max W)/2), scale[1] = 1/sigma, scale[2] = 1/sigma^2 (exact powers of two)
+__global__ void __launch_bounds__(256) k_wmax(const double *__restrict__ W, long long n_f, unsigned long long *__restrict__ wmax_bits)
+{
+    double m = 0.0;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n_f; i += (long long)gridDim.x * blockDim.x) {
+        const double w = fabs(W[i]);
+        if (w > m && w < INFINITY) m = w;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if ((threadIdx.x & 31) == 0) atomicMax(wmax_bits, (unsigned long long)__double_as_longlong(m)); // m >= 0: order-preserving
+}
+__global__ void k_scale_from_wmax(const unsigned long long *__restrict__ wmax_bits, double *__restrict__ scale)
+{
+    const double m = __longlong_as_double((long long)wmax_bits[0]);
+    int e = 0;
+    if (m > 0.0) {
+        (void)frexp(m, &e); // m = f 2^e, f in [1/2, 1)
+        e = (e + 1) >> 1;   // sigma^2 = 2^(2e) >= m
+    }
+    scale[0] = ldexp(1.0, e);
+    scale[1] = ldexp(1.0, -e);
+    scale[2] = ldexp(1.0, -2 * e);
+}
+__global__ void __launch_bounds__(256) k_prescale_f32(const double *__restrict__ g4, const double *__restrict__ Wd,
+                                                      long long n_pad, const double *__restrict__ scale,
+                                                      float *__restrict__ g4f, double *__restrict__ Wds)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_pad) return;
+    const double is = scale[1], is2 = scale[2];
+    const double4 g = reinterpret_cast<const double4 *>(g4)[i];
+    reinterpret_cast<float4 *>(g4f)[i] = make_float4((float)(g.x * is), (float)(g.y * is), (float)(g.z * is), (float)(g.w * is));
+    Wds[i] = Wd[i] * is2;
+}
+
+struct MixedAcc { // FP64 accumulators of one walker
+    double sAr, sAi, sEr, sEi, sH;
+};
+
+// bins [b0, b1) of one spline interval, in chains of <= kMixedChain bins flushed into the FP64 accumulators
+template <bool MASK>
+__device__ __forceinline__ void fused_bins_mixed(int b0, int b1, int tlo, int thi, int kbase, double df, double nxj,
+                                                 double cA0, double cA1, double cA2, double cA3, double cP0, double cP1,
+                                                 double cP2, double cP3, const float4 *__restrict__ sg4,
+                                                 const double *__restrict__ sWc, MixedAcc &acc)
+{
+    for (int base = b0; base < b1; base += kMixedChain) {
+        const int end = min(base + kMixedChain, b1);
+        float fAr = 0.f, fAi = 0.f, fEr = 0.f, fEi = 0.f;
+#pragma unroll 4
+        for (int ii = base; ii < end; ++ii) {
+            const double t = fma((double)(kbase + ii), df, nxj);
+            double A = fma(fma(fma(cA3, t, cA2), t, cA1), t, cA0);
+            const double y = fma(fma(fma(cP3, t, cP2), t, cP1), t, cP0);
+            if (MASK) A = ((ii >= tlo) && (ii < thi)) ? A : 0.0;
+            acc.sH = fma(sWc[ii] * A, A, acc.sH);
+            float u, v; // h = u - i v
+            amp_expi_qc_f32(__double2float_rn(A), y, u, v);
+            const float4 g = sg4[ii];
+            fAr = fmaf(g.x, u, fAr); fAr = fmaf(g.y, v, fAr);
+            fAi = fmaf(g.y, u, fAi); fAi = fmaf(-g.x, v, fAi);
+            fEr = fmaf(g.z, u, fEr); fEr = fmaf(g.w, v, fEr);
+            fEi = fmaf(g.w, u, fEi); fEi = fmaf(-g.z, v, fEi);
+        }
+        acc.sAr += (double)fAr; acc.sAi += (double)fAi; acc.sEr += (double)fEr; acc.sEi += (double)fEi;
+    }
+}
+
+struct FusedArgsF32 {
+    const float *g4f;   // [n_f_pad][4] binary32, g / sigma
+    const double *Wds;  // [n_f_pad] FP64, W / sigma^2
+    const double *scale;
+};
+
+__global__ void __launch_bounds__(128, 4) k_full_fused_mixed(FusedArgs a, FusedArgsF32 m)
+{
+    extern __shared__ __align__(128) double sm[];
+    __shared__ __align__(8) uint64_t bar[2];
+    __shared__ int s_lo, s_hi;
+
+    const int tid = threadIdx.x;
+    const int p = blockIdx.x * blockDim.x + tid;
+    const int tile = blockIdx.y;
+    const int i0 = tile * a.TB;
+    const int i1 = min(i0 + a.TB, a.n_f);
+    const int lo = max(a.ilo[p], i0), hi = min(a.ihi[p], i1);
+    if (tid == 0) {
+        s_lo = INT_MAX;
+        s_hi = INT_MIN;
+        mbar_init(&bar[0], 1);
+        mbar_init(&bar[1], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    if (lo < hi) {
+        atomicMin(&s_lo, lo);
+        atomicMax(&s_hi, hi);
+    }
+    __syncthreads();
+    const int blo = s_lo, bhi = s_hi;
+    if (blo >= bhi) return;
+
+    const int CH = a.CH;
+    const int c_begin = blo / CH, c_end = (bhi + CH - 1) / CH;
+    // stage = CH float4 (g) + CH double (W) = 24 B per bin = 3 doubles
+    const uint32_t stage_bytes = (uint32_t)CH * 24u;
+    auto issue = [&](int c, int st) {
+        double *dst = sm + (size_t)st * CH * 3;
+        mbar_expect_tx(&bar[st], stage_bytes);
+        tma_load_1d(dst, m.g4f + (size_t)c * CH * 4, (uint32_t)CH * 16u, &bar[st]);
+        tma_load_1d(dst + (size_t)CH * 2, m.Wds + (size_t)c * CH, (uint32_t)CH * 8u, &bar[st]);
+    };
+    if (tid == 0) issue(c_begin, 0);
+
+    const size_t sw = (size_t)a.n_wp;
+    const size_t cj = (size_t)8 * sw;
+    const double sigma = m.scale[0];
+    const int kbase = (int)a.k_min;
+    int j = find_interval_of_bin(a.bstart, a.n_nodes, blo);
+    int jl = -1;
+    double cA0 = 0, cA1 = 0, cA2 = 0, cA3 = 0, cP0 = 0, cP1 = 0, cP2 = 0, cP3 = 0, nxj = 0;
+    MixedAcc acc{0, 0, 0, 0, 0};
+
+    for (int c = c_begin; c < c_end; ++c) {
+        const int st = (c - c_begin) & 1;
+        const uint32_t ph = (uint32_t)((c - c_begin) >> 1) & 1u;
+        if (tid == 0 && c + 1 < c_end) issue(c + 1, st ^ 1);
+        mbar_wait(&bar[st], ph);
+        const double *sg = sm + (size_t)st * CH * 3;
+        const double *sW = sg + (size_t)CH * 2;
+        const int cb = c * CH;
+        const int ce = min(cb + CH, bhi);
+        int i = max(cb, blo);
+        while (i < ce) {
+            while (j < a.n_nodes - 2 && __ldg(a.bstart + j + 1) <= i) ++j;
+            const int seg_end = (j < a.n_nodes - 2) ? min(__ldg(a.bstart + j + 1), ce) : ce;
+            int tlo = max(i, lo), thi = min(seg_end, hi);
+            if (tlo >= thi) { tlo = INT_MAX; thi = INT_MIN; }
+            const int wlo = __reduce_min_sync(0xffffffffu, tlo);
+            const int whi = __reduce_max_sync(0xffffffffu, thi);
+            if (wlo < whi) {
+                if (j != jl) {
+                    const double *cc = a.C + (size_t)j * cj + p;
+                    cA0 = cc[0] * sigma; cA1 = cc[sw] * sigma; cA2 = cc[2 * sw] * sigma; cA3 = cc[3 * sw] * sigma;
+                    cP0 = cc[4 * sw]; cP1 = cc[5 * sw]; cP2 = cc[6 * sw]; cP3 = cc[7 * sw];
+                    nxj = -__ldg(a.xj + j);
+                    jl = j;
+                }
+                const int flo = __reduce_max_sync(0xffffffffu, max(lo, i));
+                const int fhi = __reduce_min_sync(0xffffffffu, min(hi, seg_end));
+                const float4 *sg4 = reinterpret_cast<const float4 *>(sg) - cb;
+                const double *sWc = sW - cb;
+                if (flo < fhi) {
+                    fused_bins_mixed<true>(wlo, flo, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1,
+                                           cP2, cP3, sg4, sWc, acc);
+                    fused_bins_mixed<false>(flo, fhi, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1,
+                                            cP2, cP3, sg4, sWc, acc);
+                    fused_bins_mixed<true>(fhi, whi, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1,
+                                           cP2, cP3, sg4, sWc, acc);
+                } else {
+                    fused_bins_mixed<true>(wlo, whi, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1,
+                                           cP2, cP3, sg4, sWc, acc);
+                }
+            }
+            i = seg_end;
+        }
+        __syncthreads();
+    }
+    double *o = a.part + ((size_t)tile * 5) * sw + p;
+    o[0] = acc.sAr; o[sw] = acc.sAi; o[2 * sw] = acc.sEr; o[3 * sw] = acc.sEi; o[4 * sw] = acc.sH;
 }
 
 // F4: reduce the per-tile partials in tile order, apply T^c (single mode), form log L        (Eq. 2)

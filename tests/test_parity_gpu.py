@@ -202,6 +202,80 @@ def test_cfg2_full_size_sampled(orc, torch_cuda):
     ctx.destroy()
 
 
+# ------------------------------------------------------------------ full grid, FP32-accumulate variant
+MIXED_ABS_TOL = 1e-3  # BASELINE.json north_star: "<= 1e-3 absolute for any mixed-precision variant"
+
+
+def check_mixed(got, ref, what, tol=MIXED_ABS_TOL):
+    logL, d_h, h_h = (np.asarray(x.cpu().numpy() if hasattr(x, "cpu") else x) for x in got)
+    for name, a, b in (("logL", logL, ref["logL"]), ("d_h", d_h, ref["d_h"])):
+        err = np.abs(a - b)
+        assert err.max() <= tol, f"{what} {name}: worst |err| {err.max():.3e} at {int(err.argmax())}"
+    # <h|h> stays in FP64 in this variant (reading R15): FP64 bar
+    assert np.all(np.abs(h_h - ref["h_h"]) <= 1e-6 * np.maximum(1.0, np.abs(ref["h_h"]))), what + " h_h"
+    return float(np.abs(logL - ref["logL"]).max())
+
+
+def test_cfg0_mixed_precision_parity(cfg0, torch_cuda):
+    """FP32-accumulate variant (reading R15) on config 0: a logic / ragged-shape check, not a BASELINE case for
+    this variant (config 2 is).  Noiseless SNR 500-1000 on only 6.5k bins makes the per-bin terms of <d|h> ~240x
+    larger than config 2's; binary32 rounding is relative to each term, so the absolute error grows like
+    <d|h>/sqrt(n_bins): 2^-24 * 1e6 / sqrt(3e3) * (a few roundings) ~ 2e-3.  Bound used here: 5e-3."""
+    wl, d, run, _ = cfg0
+    ctx = make_ctx(wl, precision=1)
+    g = wl.grid
+    ctx.set_data(g.n_f, g.k_min, g.df, dev(torch_cuda, d), dev(torch_cuda, wl.W))
+    ref = run(wl.params, d)
+    got = ctx.full_batch_standin(wl.f_nodes, dev(torch_cuda, wl.params))
+    check_mixed(got, ref, "cfg0 mixed", tol=5e-3)
+    again = ctx.full_batch_standin(wl.f_nodes, dev(torch_cuda, wl.params))
+    assert all(torch_cuda.equal(a, b) for a, b in zip(got, again))
+    ctx.destroy()
+
+
+def test_cfg2_scaled_mixed_precision_parity(orc, torch_cuda):
+    """config-2 recipe at 1/16 of the grid, noisy data, 600 walkers, FP32-accumulate variant."""
+    wl = wlm.make_workload(2, n_w=600, t_obs=31557600.0 / 16)
+    d, run = oracle_setup_full(orc, wl)
+    ctx = make_ctx(wl, precision=1)
+    g = wl.grid
+    ctx.set_data(g.n_f, g.k_min, g.df, dev(torch_cuda, d), dev(torch_cuda, wl.W))
+    ref = run(wl.params, d)
+    got = ctx.full_batch_standin(wl.f_nodes, dev(torch_cuda, wl.params))
+    check_mixed(got, ref, "cfg2/16 mixed")
+    ctx.destroy()
+
+
+def test_cfg2_full_size_sampled_mixed(orc, torch_cuda):
+    """BASELINE.json config 2 at full size, FP32-accumulate variant, sampled walkers against the oracle."""
+    wl = wlm.make_workload(2)
+    d, run = oracle_setup_full(orc, wl)
+    ctx = make_ctx(wl, precision=1)
+    g = wl.grid
+    ctx.set_data(g.n_f, g.k_min, g.df, dev(torch_cuda, d), dev(torch_cuda, wl.W))
+    got = [x.cpu().numpy() for x in ctx.full_batch_standin(wl.f_nodes, dev(torch_cuda, wl.params))]
+    fis = np.array([orc.standin_fisco(p) for p in wl.params])
+    sample = sorted({0, int(fis.argmin()), int(fis.argmax()), 1, 4097, 16383} | set(range(37, 16384, 2048)))
+    ref = run(wl.params[sample], d)
+    check_mixed([x[sample] for x in got], ref, "cfg2 mixed sampled")
+    assert np.all(np.isfinite(got[0]))
+    ctx.destroy()
+
+
+def test_mixed_precision_multimode_is_unsupported(torch_cuda):
+    from paper_2111_01064_b200 import binding
+    wl = wlm.make_workload(3, n_w=8, t_obs=2.0 ** 16, n_knots=24)
+    wl.f_nodes = wlm.geomspace_exact(wlm.F_LO, wlm.F_HI, 64)
+    ctx = make_ctx(wl, precision=1)
+    g = wl.grid
+    z = torch_cuda.zeros(2 * g.n_f * 2, dtype=torch_cuda.float64, device="cuda")
+    ctx.set_data(g.n_f, g.k_min, g.df, z, dev(torch_cuda, wl.W))
+    with pytest.raises(binding.LLError) as ei:
+        ctx.full_batch_standin(wl.f_nodes, dev(torch_cuda, wl.params))
+    assert ei.value.code == binding.LL_ERR_UNSUPPORTED
+    ctx.destroy()
+
+
 # ------------------------------------------------------------------------------------------- heterodyne
 @pytest.fixture(scope="module")
 def het_small(orc, torch_cuda):
