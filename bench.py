@@ -37,6 +37,14 @@ UNIT = "evals/s"
 # SURVEY.md §8(d) figure of 39 is used as the contract number)
 SLOTS_FULL = 39.0
 SLOTS_HET = {1: 73.0, 6: 252.0}
+# FP32-accumulate variant: bound by instruction issue (one warp instruction per scheduler per
+# clock = 4 x 32 lane-instructions/clk/SM).  Algorithmic instructions per active pair: 13 FP64 (t, two cubics,
+# reduce 3, scale 1, W A^2 2) + 3 conversions + 20 binary32 (sincos 10, A e^{-i Psi} 2, MACs 8) + 6 quadrant
+# + 2 shared loads + 1 loop = 45
+INSTR_FULL_FP32ACC = 45.0
+ISSUE_LANES_PER_CLK_PER_SM = 128.0
+# DRAM traffic per launch of the dominant kernel, from the committed `ncu --set full` captures (profiles/)
+NCU_TRAFFIC_BYTES = {("k_full_fused", 2): 803.1e6 + 39.2e6, ("k_full_fused_mixed", 2): 787.9e6 + 37.3e6}
 DFMA_PER_CLK_PER_SM = 64.0
 
 
@@ -158,12 +166,19 @@ def time_steps(torch, fn, steps: int, warmup: int):
     return e0.elapsed_time(e1)
 
 
-def bench_config(torch, index: int, steps: int, warmup: int, rank: int = 0, profile: bool = False):
-    """device-resident timing of one config through the stand-in entry point (parameters -> log L)."""
+def bench_config(torch, index: int, steps: int, warmup: int, rank: int = 0, profile: bool = False, precision: int = 0):
+    """device-resident timing of one config through the stand-in entry point (parameters -> log L).
+    precision = 1: the FP32-accumulate variant of the full-grid path on the SAME data (the data stream is built
+    by an FP64 context first, so the two variants can be compared output by output)."""
     from paper_2111_01064_b200 import synth
     wl = rank_workload(index, rank)
     ctx = synth.make_context(wl)
     bufs = synth.setup(ctx, wl)
+    if precision:
+        ctx.destroy()
+        ctx = synth.make_context(wl, precision=precision)
+        g = wl.grid
+        ctx.set_data(g.n_f, g.k_min, g.df, bufs["d"], bufs["W"])
     params = bufs["params"]
     n_w = wl.n_w
     out = tuple(torch.empty(n_w, dtype=torch.float64, device=params.device) for _ in range(3))
@@ -291,6 +306,8 @@ def main():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--workload", type=int, default=2, help="BASELINE.json config index of the headline step")
     ap.add_argument("--quick", action="store_true", help="skip per_config, e2e and cpu_baseline (profiling runs)")
+    ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32acc"],
+                    help="fp32acc: time the FP32-accumulate variant of the full-grid path as the headline step")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
 
@@ -314,8 +331,10 @@ def main():
 
     peaks, peak_src = measured_peaks()
     with ClockSampler(local) as clk:
-        res = bench_config(torch, args.workload, args.steps, args.warmup, rank=rank, profile=True)
+        res = bench_config(torch, args.workload, args.steps, args.warmup, rank=rank, profile=True,
+                           precision=1 if args.precision == "fp32acc" else 0)
     wl, ctx = res["wl"], res["ctx"]
+    headline_logL = res["out"][0].clone()
     t_ms = allreduce_max(res["ms_total"])
     units = allreduce_sum(float(wl.n_w) * args.steps)
     value = units / (t_ms * 1e-3)
@@ -323,7 +342,8 @@ def main():
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": t_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f64", "data": "synthetic", "config": workload_config(wl), "clocks": clocks,
+            "dtype": "f64" if args.precision == "fp64" else "f64 phase/amplitude/<h|h> + f32 trig/products (reading R15)",
+            "data": "synthetic", "config": workload_config(wl), "clocks": clocks,
             "gpu_launches": int(res["launches"]), "impl": "b200"}
 
     if rank == 0:
@@ -334,24 +354,39 @@ def main():
         if wl.path == "full":
             pairs, n_blocks = ctx.last_full_stats()
             slots = pairs * SLOTS_FULL
-            kname = "k_full_fused"
+            kname = "k_full_fused" if args.precision == "fp64" else "k_full_fused_mixed"
         else:
             pairs = float(wl.n_w) * (len(wl.f_edges) - 1)
             slots = pairs * SLOTS_HET.get(wl.n_m, 73.0 + 36.0 * (wl.n_m - 1))
             kname = "k_het_standin"
         k_ms = res["kernel_ms"]
-        achieved = slots / (k_ms * 1e-3)
         dfma_rate, dfma_ms = ctx.peak_fma(0, 4000)
         ffma_rate, _ = ctx.peak_fma(1, 8000)
-        line["roofline"] = {
-            "bound": "alu", "kernel": kname, "achieved": achieved / 1e12, "peak": peak_slots / 1e12,
-            "unit": "T FP64 issue slots/s (1 DFMA|DMUL|DADD = 1 slot)", "frac": achieved / peak_slots,
-            "traffic": None, "kernel_ms": k_ms, "kernel_share_of_step": k_ms / (res["ms_per_step"]),
-            "algorithmic_slots_per_pair": SLOTS_FULL if wl.path == "full" else slots / pairs, "active_pairs": pairs,
-            "peak_source": f"{n_sm} SMs x {int(DFMA_PER_CLK_PER_SM)} DFMA/clk x {sm_max:.0f} MHz (DESIGN.md §6)",
-            "measured_dfma_per_s": dfma_rate, "measured_ffma_per_s": ffma_rate,
-            "frac_of_measured_dfma": achieved / dfma_rate,
-            "hbm_peak_gbs": peaks.get("hbm_gbs"), "hbm_peak_source": peak_src}
+        traffic = NCU_TRAFFIC_BYTES.get((kname, args.workload))
+        if kname == "k_full_fused_mixed":
+            peak_issue = n_sm * ISSUE_LANES_PER_CLK_PER_SM * sm_max * 1e6
+            achieved = pairs * INSTR_FULL_FP32ACC / (k_ms * 1e-3)
+            line["roofline"] = {
+                "bound": "alu", "kernel": kname, "achieved": achieved / 1e12, "peak": peak_issue / 1e12,
+                "unit": "T lane-instructions/s (instruction issue: 1 warp instruction/scheduler/clk)",
+                "frac": achieved / peak_issue, "traffic": traffic, "kernel_ms": k_ms,
+                "kernel_share_of_step": k_ms / (res["ms_per_step"]),
+                "algorithmic_instructions_per_pair": INSTR_FULL_FP32ACC, "active_pairs": pairs,
+                "peak_source": f"{n_sm} SMs x 4 schedulers x 32 lanes x {sm_max:.0f} MHz (DESIGN.md §6)",
+                "fp64_slots_per_pair": 13.0, "fp64_pipe_frac": pairs * 13.0 / (k_ms * 1e-3) / peak_slots,
+                "measured_dfma_per_s": dfma_rate, "measured_ffma_per_s": ffma_rate,
+                "hbm_peak_gbs": peaks.get("hbm_gbs"), "hbm_peak_source": peak_src}
+        else:
+            achieved = slots / (k_ms * 1e-3)
+            line["roofline"] = {
+                "bound": "alu", "kernel": kname, "achieved": achieved / 1e12, "peak": peak_slots / 1e12,
+                "unit": "T FP64 issue slots/s (1 DFMA|DMUL|DADD = 1 slot)", "frac": achieved / peak_slots,
+                "traffic": traffic, "kernel_ms": k_ms, "kernel_share_of_step": k_ms / (res["ms_per_step"]),
+                "algorithmic_slots_per_pair": SLOTS_FULL if wl.path == "full" else slots / pairs, "active_pairs": pairs,
+                "peak_source": f"{n_sm} SMs x {int(DFMA_PER_CLK_PER_SM)} DFMA/clk x {sm_max:.0f} MHz (DESIGN.md §6)",
+                "measured_dfma_per_s": dfma_rate, "measured_ffma_per_s": ffma_rate,
+                "frac_of_measured_dfma": achieved / dfma_rate,
+                "hbm_peak_gbs": peaks.get("hbm_gbs"), "hbm_peak_source": peak_src}
 
     if not args.quick:
         # ---- end to end through the C ABI with host buffers
@@ -374,6 +409,16 @@ def main():
             r = bench_config(torch, idx, st, 5)
             per[f"cfg{idx}"] = {"evals_per_s": r["wl"].n_w / (r["ms_per_step"] * 1e-3), "ms_per_batch": r["ms_per_step"],
                                 "n_walkers": r["wl"].n_w}
+            r["ctx"].destroy()
+            del r
+            torch.cuda.empty_cache()
+        if args.workload == 2 and args.precision == "fp64":
+            # ---- config 2's FP32-accumulate variant on the same data: throughput and its distance from FP64
+            r = bench_config(torch, 2, args.steps, 5, profile=True, precision=1)
+            dl = (r["out"][0] - headline_logL).abs()
+            per["cfg2_fp32acc"] = {"evals_per_s": r["wl"].n_w / (r["ms_per_step"] * 1e-3), "ms_per_batch": r["ms_per_step"],
+                                   "n_walkers": r["wl"].n_w, "kernel": "k_full_fused_mixed", "kernel_ms": r["kernel_ms"],
+                                   "max_abs_dlogL_vs_fp64": float(dl.max()), "rms_dlogL_vs_fp64": float(dl.pow(2).mean().sqrt())}
             r["ctx"].destroy()
             del r
             torch.cuda.empty_cache()
