@@ -94,8 +94,9 @@ struct ll_ctx {
     // het state
     bool have_het = false;
     int n_e = 0;
-    DevBuf het_tab, het_raw, het_idx, het_fb;
+    DevBuf het_tab, het_raw, het_idx, het_fb, het_tab1;
     HetTable ht{};
+    Het1Table ht1{}; // single-mode regrouped table (k_het_standin1); base == nullptr when not built
     std::vector<double> raw_host; // [n_b][13]
 
     // host staging for the *_host entry points
@@ -396,7 +397,9 @@ int build_het_table(ll_ctx *ctx, int n_e, const double *e, const std::vector<dou
                 const ld f = (ld)e[j], fp = 2.0L * f / (ld)ctx->si.mode_m[m];
                 tab[T.off_cfp() + m * n_e + j] = (double)((ld)ctx->c_lm[m] * powl(f, -7.0L / 6.0L));
                 tab[T.off_f2m() + m * n_e + j] = (double)fp;
-                tab[T.off_fm53() + m * n_e + j] = (double)powl(fp, -5.0L / 3.0L);
+                // (m / pi) (2f/m)^(-5/3): the mode's phase factor m/2 and the radians -> quarter cycles 2/pi folded in
+                tab[T.off_fm53() + m * n_e + j] = (double)((ld)ctx->si.mode_m[m] / 3.14159265358979323846264338327950288L *
+                                                           powl(fp, -5.0L / 3.0L));
             }
     }
     const std::vector<double> &raw = ctx->raw_host;
@@ -415,6 +418,57 @@ int build_het_table(ll_ctx *ctx, int n_e, const double *e, const std::vector<dou
     return LL_OK;
 }
 
+// single-mode regrouped table (k_het_standin1): 14 doubles per edge, see ll_kernels.cuh
+void build_het1_table(ll_ctx *ctx, int n_e, const double *e, const std::vector<double> &h0e, std::vector<double> &tab)
+{
+    typedef long double ld;
+    const int n_b = n_e - 1;
+    const std::vector<double> &raw = ctx->raw_host; // [n_b][13]: per channel (A0r, A0i, A1r, A1i, B0, B1), then dd
+    tab.assign((size_t)n_e * kHet1Stride, 0.0);
+    std::vector<ld> ihr((size_t)kNC * n_e), ihi((size_t)kNC * n_e);
+    for (int c = 0; c < kNC; ++c)
+        for (int j = 0; j < n_e; ++j) {
+            const ld gr = h0e[((size_t)c * n_e + j) * 2], gi = h0e[((size_t)c * n_e + j) * 2 + 1];
+            const ld den = gr * gr + gi * gi;
+            ihr[(size_t)c * n_e + j] = gr / den;
+            ihi[(size_t)c * n_e + j] = -gi / den;
+        }
+    for (int j = 0; j < n_e; ++j) {
+        double *t = &tab[(size_t)j * kHet1Stride];
+        const ld f = (ld)e[j], fp = 2.0L * f / (ld)ctx->si.mode_m[0];
+        t[0] = 4.0 * e[j];
+        t[1] = (double)powl(fp, -5.0L / 3.0L);
+        t[2] = (double)((ld)ctx->c_lm[0] * powl(f, -7.0L / 6.0L));
+        t[3] = (double)fp;
+        for (int c = 0; c < kNC; ++c) {
+            ld Gr = 0, Gi = 0, Pc = 0;
+            if (j >= 1) { // bin j - 1 ends at this edge
+                const double *r = &raw[(size_t)(j - 1) * 13 + 6 * c];
+                const ld invw = 1.0L / ((ld)e[j] - (ld)e[j - 1]);
+                Gr += 0.5L * r[0] + r[2] * invw; Gi += 0.5L * r[1] + r[3] * invw;
+                Pc += 0.25L * r[4] + r[5] * invw;
+            }
+            if (j < n_b) { // bin j starts at this edge
+                const double *r = &raw[(size_t)j * 13 + 6 * c];
+                const ld invw = 1.0L / ((ld)e[j + 1] - (ld)e[j]);
+                Gr += 0.5L * r[0] - r[2] * invw; Gi += 0.5L * r[1] - r[3] * invw;
+                Pc += 0.25L * r[4] - r[5] * invw;
+            }
+            const ld ar = ihr[(size_t)c * n_e + j], ai = ihi[(size_t)c * n_e + j];
+            // Q = G conj(1/h0)
+            t[4 + 2 * c] = (double)(Gr * ar + Gi * ai);
+            t[5 + 2 * c] = (double)(Gi * ar - Gr * ai);
+            t[8 + c] = (double)(Pc * (ar * ar + ai * ai));
+            if (j < n_b) { // X = (B0/2) (1/h0_j) conj(1/h0_{j+1})
+                const ld br = ihr[(size_t)c * n_e + j + 1], bi = ihi[(size_t)c * n_e + j + 1];
+                const ld hb = 0.5L * raw[(size_t)j * 13 + 6 * c + 4];
+                t[10 + 2 * c] = (double)(hb * (ar * br + ai * bi));
+                t[11 + 2 * c] = (double)(hb * (ai * br - ar * bi));
+            }
+        }
+    }
+}
+
 int het_check(ll_ctx *ctx, int64_t n_w, const double *logL)
 {
     if (!ctx) return LL_ERR_ARG;
@@ -423,6 +477,45 @@ int het_check(ll_ctx *ctx, int64_t n_w, const double *logL)
     if (n_w > 0 && !logL) return ctx->fail(LL_ERR_ARG, "logL is NULL");
     if (!ctx->have_data) return ctx->fail(LL_ERR_STATE, "ll_set_data has not been called");
     if (!ctx->have_het) return ctx->fail(LL_ERR_STATE, "ll_het_prepare has not been called");
+    return LL_OK;
+}
+
+// single mode: the regrouped kernel (one table copy per block, WY warps = G walker groups x S edge segments)
+int launch_het_standin1(ll_ctx *ctx, int64_t n_w, const double *params, double *logL, double *d_h, double *h_h,
+                        cudaStream_t st)
+{
+    const int n_groups = ceil_div(n_w, 32), n_e = ctx->ht1.n_e;
+    constexpr int WY = 16;
+    const size_t smem = sizeof(double) * ((size_t)n_e * kHet1Stride + (size_t)WY * 192);
+    static bool attr_set = false;
+    if (!attr_set) {
+        CK(cudaFuncSetAttribute(k_het_standin1, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+        attr_set = true;
+    }
+    if (smem > 227 * 1024) return ctx->fail(LL_ERR_UNSUPPORTED, "heterodyne tables exceed shared memory (too many bins)");
+    static size_t bps_smem = 0;
+    static int bps = 0;
+    if (bps == 0 || bps_smem != smem) {
+        CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, k_het_standin1, 32 * WY, smem));
+        bps = std::max(1, bps);
+        bps_smem = smem;
+    }
+    const int max_blocks = ctx->sm_count * bps;
+    int S = 1, grid = 1;
+    double best = 1e300;
+    for (int s = 1; s <= WY; s <<= 1) {
+        if (s > 1 && n_e / s < 8) break;
+        const int G = WY / s;
+        const long long passes = ceil_div(n_groups, G);
+        const int gr = (int)std::min<long long>(passes, max_blocks);
+        const double work = (double)ceil_div(gr, ctx->sm_count) * (double)ceil_div(passes, gr) * WY * (ceil_div(n_e, s) + 1.0);
+        if (work < best * 0.999) { best = work; S = s; grid = gr; }
+    }
+    const int P = 5 + 2 * kNC;
+    ProfScope prof(ctx, st);
+    k_het_standin1<<<grid, dim3(32, WY), smem, st>>>(ctx->ht1, ctx->si, params, P, (int)n_w, n_groups, S,
+                                                     ctx->dd.as<double>(), logL, d_h, h_h);
+    LAUNCHED(ctx);
     return LL_OK;
 }
 
@@ -520,7 +613,7 @@ int ll_destroy(ll_ctx *ctx)
         cudaDeviceSynchronize();
         DevBuf *all[] = {&ctx->g4, &ctx->Wd, &ctx->dd_part, &ctx->dd, &ctx->pairs, &ctx->node_tab, &ctx->ilo_w, &ctx->ihi_w,
                          &ctx->key_w, &ctx->hist, &ctx->perm, &ctx->ilo_s, &ctx->ihi_s, &ctx->Y, &ctx->C, &ctx->TF,
-                         &ctx->part, &ctx->prow, &ctx->het_tab, &ctx->het_raw, &ctx->het_idx, &ctx->het_fb,
+                         &ctx->part, &ctx->prow, &ctx->het_tab, &ctx->het_tab1, &ctx->het_raw, &ctx->het_idx, &ctx->het_fb,
                          &ctx->stage_in, &ctx->stage_out, &ctx->g4f, &ctx->Wf, &ctx->scale, &ctx->wmax};
         for (DevBuf *b : all) b->release();
         for (auto &e : ctx->ev) cudaEventDestroy(e);
@@ -752,6 +845,14 @@ int ll_het_prepare(ll_ctx *ctx, int32_t n_edges, const double *f_edges, const do
     const double ddb_d = (double)ddb;
     CK(ctx->het_tab.ensure(sizeof(double) * tab.size()));
     CK(cudaMemcpyAsync(ctx->het_tab.p, tab.data(), sizeof(double) * tab.size(), cudaMemcpyHostToDevice, st));
+    std::vector<double> tab1;
+    ctx->ht1 = Het1Table{nullptr, n_e, n_b};
+    if (ctx->n_m == 1 && ctx->have_standin) {
+        build_het1_table(ctx, n_e, f_edges, h0e, tab1);
+        CK(ctx->het_tab1.ensure(sizeof(double) * tab1.size()));
+        CK(cudaMemcpyAsync(ctx->het_tab1.p, tab1.data(), sizeof(double) * tab1.size(), cudaMemcpyHostToDevice, st));
+        ctx->ht1.base = ctx->het_tab1.as<double>();
+    }
     CK(cudaMemcpyAsync(ctx->dd.as<double>() + 1, &ddb_d, sizeof(double), cudaMemcpyHostToDevice, st));
     CK(cudaStreamSynchronize(st));
     ctx->ht.base = ctx->het_tab.as<double>();
@@ -812,7 +913,9 @@ int ll_het_batch_standin(ll_ctx *ctx, int64_t n_w, const double *params, double 
     DeviceGuard dg(ctx->device);
     cudaStream_t st = (cudaStream_t)stream;
     switch (ctx->n_m) {
-    case 1: return launch_het_standin<1>(ctx, n_w, params, logL, d_h, h_h, st);
+    case 1:
+        if (ctx->ht1.base) return launch_het_standin1(ctx, n_w, params, logL, d_h, h_h, st);
+        return launch_het_standin<1>(ctx, n_w, params, logL, d_h, h_h, st);
     case 2: return launch_het_standin<2>(ctx, n_w, params, logL, d_h, h_h, st);
     case 3: return launch_het_standin<3>(ctx, n_w, params, logL, d_h, h_h, st);
     case 4: return launch_het_standin<4>(ctx, n_w, params, logL, d_h, h_h, st);

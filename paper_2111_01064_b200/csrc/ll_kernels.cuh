@@ -967,29 +967,27 @@ k_het_standin(HetTable T, StandinInfo si, const double *__restrict__ params, int
         const bool valid = grp < n_groups && w < n_w;
         const double *row = params + (size_t)(valid ? w : 0) * P;
         const WalkerConst c = standin_consts(row);
-        double Kq[NM], phq[NM], tf[NM][4];
+        double tf[NM][4];
 #pragma unroll
         for (int m = 0; m < NM; ++m) {
-            const double mh_pi = (double)si.mode_m[m] / kPi;
-            Kq[m] = mh_pi * c.K;
-            phq[m] = mh_pi * (c.phi + 0.25 * kPi);
 #pragma unroll
             for (int q = 0; q < 4; ++q) tf[m][q] = row[5 + m * 4 + q];
         }
+        const double phi0 = c.phi + 0.25 * kPi;
         double dh = 0.0, hh = 0.0;
         double pAr = 0, pAi = 0, pEr = 0, pEi = 0;
         if (grp < n_groups)
         for (int e = b0; e <= b1 && b0 < b1; ++e) {
             double hAr = 0, hAi = 0, hEr = 0, hEi = 0;
-            const double f4e = f4[e];
+            const double ftc = f4[e] * c.tc;
 #pragma unroll
             for (int m = 0; m < NM; ++m) {
                 const int t = m * T.n_e + e;
-                const double y = fma(f4e, c.tc, fma(Kq[m], fm53[t], -phq[m]));
-                double sn, cs;
-                sincos_qc(y, sn, cs);
+                // quarter cycles: 4 f t_c + (m/2pi) K (2f/m)^(-5/3) - (m/2pi)(phi_c + pi/4); fm53 carries m/(2 pi) ... m/pi
+                const double y = fma(c.K, fm53[t], fma(-((double)si.mode_m[m] / kPi), phi0, ftc));
                 const double A = cfp[t] * c.invD * taper(f2m[t] * c.inv_fisco, si.kappa, inv_kappa);
-                const double u = A * cs, v = A * sn; // h_m = u - i v
+                double u, v; // h_m = u - i v
+                amp_expi_qc(A, y, u, v);
                 hAr = fma(tf[m][0], u, hAr); hAr = fma(tf[m][1], v, hAr);
                 hAi = fma(tf[m][1], u, hAi); hAi = fma(-tf[m][0], v, hAi);
                 hEr = fma(tf[m][2], u, hEr); hEr = fma(tf[m][3], v, hEr);
@@ -1012,6 +1010,110 @@ k_het_standin(HetTable T, StandinInfo si, const double *__restrict__ params, int
             }
         }
         if (seg == 0 && valid) {
+            logL[w] = dh - 0.5 * hh - 0.5 * ddb;
+            if (d_h) d_h[w] = dh;
+            if (h_h) h_h[w] = hh;
+        }
+        if (S > 1) __syncthreads();
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// H1-H3, single mode, regrouped by edge.  With one mode and constant T^c, r^c_e = T^c z_e / h0^c_e with
+// z_e = A(f_e) e^{-i Psi(f_e)} common to both channels, and Eq. 14 / Eq. 17 regroup exactly into sums over edges:
+//   Z[d,h] = Re sum_c conj(T^c) sum_e conj(z_e) Q^c_e,
+//            Q^c_e = conj(1/h0^c_e) (A0_{e-1}/2 + A1_{e-1}/D_{e-1} + A0_e/2 - A1_e/D_e)            (Eq. 11, 14)
+//   Z[h,h] = sum_c |T^c|^2 ( sum_e |z_e|^2 P^c_e + sum_b Re[z_b conj(z_{b+1}) X^c_b] ),
+//            P^c_e = |1/h0^c_e|^2 (B0_{e-1}/4 + B1_{e-1}/D_{e-1} + B0_e/4 - B1_e/D_e),
+//            X^c_b = (B0_b/2) (1/h0^c_b) conj(1/h0^c_{b+1})                                         (Eq. 11, 17)
+// (D_b = f_{b+1} - f_b; terms whose bin index falls outside [0, n_b) are absent; 2 Re[r0 conj r1] =
+// (|r_hi|^2 - |r_lo|^2)/D.)  Same arithmetic as the bin-by-bin form up to rounding; 48 instead of 73 FP64 slots
+// per (walker, bin).  Table: 14 doubles per edge, resident in shared memory, every read a broadcast.
+// ---------------------------------------------------------------------------------------------------
+constexpr int kHet1Stride = 14; // f4, fm53, cfp, f2m, QAr, QAi, QEr, QEi, PA, PE, XAr, XAi, XEr, XEi
+
+struct Het1Table {
+    const double *base;
+    int n_e, n_b;
+};
+
+__global__ void __launch_bounds__(512)
+k_het_standin1(Het1Table T, StandinInfo si, const double *__restrict__ params, int P, int n_w, int n_groups, int S,
+               const double *__restrict__ dd, double *__restrict__ logL, double *__restrict__ d_h,
+               double *__restrict__ h_h)
+{
+    extern __shared__ __align__(16) double tab[];
+    const int total = T.n_e * kHet1Stride;
+    double *red = tab + total; // [G][S][6][32]
+    {
+        const double2 *src = reinterpret_cast<const double2 *>(T.base);
+        double2 *dst = reinterpret_cast<double2 *>(tab);
+        for (int i = threadIdx.x + threadIdx.y * 32; i < total / 2; i += 32 * blockDim.y) dst[i] = src[i];
+    }
+    __syncthreads();
+    const int G = blockDim.y / S, seg = threadIdx.y % S, gslot = threadIdx.y / S, lane = threadIdx.x;
+    const int per = (T.n_e + S - 1) / S;
+    const int e0 = seg * per, e1 = min(e0 + per, T.n_e); // this segment owns edges [e0, e1) and bins [e0, min(e1, n_b))
+    const double inv_kappa = 1.0 / si.kappa;
+    const double ddb = dd[1];
+    const double mh_pi = (double)si.mode_m[0] / kPi;
+
+    for (int base = blockIdx.x * G; base < n_groups; base += gridDim.x * G) {
+        const int grp = base + gslot;
+        const int w = grp * 32 + lane;
+        const bool valid = grp < n_groups && w < n_w;
+        const double *row = params + (size_t)(valid ? w : 0) * P;
+        const WalkerConst c = standin_consts(row);
+        const double Kq = mh_pi * c.K, nphq = -mh_pi * (c.phi + 0.25 * kPi);
+        double DAr = 0, DAi = 0, DEr = 0, DEi = 0, HA = 0, HE = 0;
+        if (grp < n_groups && e0 < e1) {
+            auto edge = [&](const double *t, double &u, double &v, double &amp) {
+                const double y = fma(t[0], c.tc, fma(Kq, t[1], nphq));
+                amp = t[2] * c.invD * taper(t[3] * c.inv_fisco, si.kappa, inv_kappa);
+                amp_expi_qc(amp, y, u, v); // z = u - i v
+            };
+            const double *t = tab + (size_t)e0 * kHet1Stride;
+            double up, vp, ap;
+            edge(t, up, vp, ap);
+            const int last = min(e1, T.n_b); // one past the last bin whose cross term this segment owns
+#pragma unroll 2
+            for (int e = e0; e < e1; ++e, t += kHet1Stride) {
+                // edge terms of e: conj(z) Q and |z|^2 P
+                DAr = fma(up, t[4], DAr); DAr = fma(-vp, t[5], DAr);
+                DAi = fma(up, t[5], DAi); DAi = fma(vp, t[4], DAi);
+                DEr = fma(up, t[6], DEr); DEr = fma(-vp, t[7], DEr);
+                DEi = fma(up, t[7], DEi); DEi = fma(vp, t[6], DEi);
+                const double a2 = ap * ap;
+                HA = fma(a2, t[8], HA);
+                HE = fma(a2, t[9], HE);
+                if (e < last) { // bin e = [e, e + 1]: needs z at e + 1 (the next segment's first edge at the boundary)
+                    double un, vn, an;
+                    edge(t + kHet1Stride, un, vn, an);
+                    const double wr = fma(up, un, vp * vn), wi = fma(up, vn, -(vp * un)); // z_e conj(z_{e+1})
+                    HA = fma(wr, t[10], HA); HA = fma(-wi, t[11], HA);
+                    HE = fma(wr, t[12], HE); HE = fma(-wi, t[13], HE);
+                    up = un; vp = vn; ap = an;
+                }
+            }
+        }
+        if (S > 1) {
+            double *rg = red + (size_t)gslot * S * 192;
+            double *q = rg + seg * 192 + lane;
+            q[0] = DAr; q[32] = DAi; q[64] = DEr; q[96] = DEi; q[128] = HA; q[160] = HE;
+            __syncthreads();
+            if (seg == 0) {
+                DAr = DAi = DEr = DEi = HA = HE = 0.0;
+                for (int s = 0; s < S; ++s) {
+                    const double *r = rg + s * 192 + lane;
+                    DAr += r[0]; DAi += r[32]; DEr += r[64]; DEi += r[96]; HA += r[128]; HE += r[160];
+                }
+            }
+        }
+        if (seg == 0 && valid) {
+            const double tar = row[5], tai = row[6], ter = row[7], tei = row[8];
+            // Re[conj(T^A) D^A + conj(T^E) D^E],  |T^A|^2 H^A + |T^E|^2 H^E
+            const double dh = (tar * DAr + tai * DAi) + (ter * DEr + tei * DEi);
+            const double hh = (tar * tar + tai * tai) * HA + (ter * ter + tei * tei) * HE;
             logL[w] = dh - 0.5 * hh - 0.5 * ddb;
             if (d_h) d_h[w] = dh;
             if (h_h) h_h[w] = hh;
