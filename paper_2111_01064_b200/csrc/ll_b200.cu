@@ -350,11 +350,11 @@ int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, cons
         ctx->last_n_blocks = (int)(grid.x * grid.y);
     }
     if (nm1)
-        k_finalize<1><<<ceil_div(n_wp, 128), 128, 0, st>>>(ctx->part.as<double>(), ctx->TF.as<double>(), ctx->perm.as<int>(),
+        k_finalize<1><<<ceil_div(n_wp, 32), dim3(32, kFinY), 0, st>>>(ctx->part.as<double>(), ctx->TF.as<double>(), ctx->perm.as<int>(),
                                                            ctx->ilo_s.as<int>(), ctx->ihi_s.as<int>(), n_wp, pl.TB,
                                                            ctx->dd.as<double>(), logL, d_h, h_h);
     else
-        k_finalize<0><<<ceil_div(n_wp, 128), 128, 0, st>>>(ctx->part.as<double>(), ctx->TF.as<double>(), ctx->perm.as<int>(),
+        k_finalize<0><<<ceil_div(n_wp, 32), dim3(32, kFinY), 0, st>>>(ctx->part.as<double>(), ctx->TF.as<double>(), ctx->perm.as<int>(),
                                                            ctx->ilo_s.as<int>(), ctx->ihi_s.as<int>(), n_wp, pl.TB,
                                                            ctx->dd.as<double>(), logL, d_h, h_h);
     LAUNCHED(ctx);

@@ -322,6 +322,7 @@ k_nodes_arrays(const double *__restrict__ amp, const double *__restrict__ phase,
 //   b_j = (y_{j+1}-y_j)/h_j - h_j (2 M_j + M_{j+1})/6,  c_j = M_j/2,  d_j = (M_{j+1}-M_j)/(6 h_j)
 // dp_j is parked in the b-slot of interval j between the sweeps.
 // ---------------------------------------------------------------------------------------------------
+constexpr int kSplineBlk = 16;
 __global__ void __launch_bounds__(128)
 k_spline(const double *__restrict__ Y, double *__restrict__ C, int n_wp, int n_nodes, int n_m, NodeTables nt)
 {
@@ -334,12 +335,14 @@ k_spline(const double *__restrict__ Y, double *__restrict__ C, int n_wp, int n_n
     const size_t cj = (size_t)n_m * 8 * sw;
     const int n = n_nodes;
 
-    double yprev = y[0], ycur = y[sw];
+    double yprev = __ldg(y), ycur = __ldg(y + sw);
     double sprev = (ycur - yprev) * __ldg(nt.invh);
     double dpp = 0.0;
-#pragma unroll 8
+    // node values are read through the read-only path (__ldg): the compiler may then hoist the loads of an
+    // unrolled group above the stores of the parked dp values instead of paying one memory latency per row
+#pragma unroll 16
     for (int j = 1; j <= n - 2; ++j) {
-        const double ynext = y[(size_t)(j + 1) * sw];
+        const double ynext = __ldg(y + (size_t)(j + 1) * sw);
         const double s = (ynext - ycur) * __ldg(nt.invh + j);
         const double r = s - sprev;
         const double dp = (r - __ldg(nt.ta + j) * dpp) * __ldg(nt.tinv + j);
@@ -348,21 +351,36 @@ k_spline(const double *__restrict__ Y, double *__restrict__ C, int n_wp, int n_n
         sprev = s;
         ycur = ynext;
     }
+    // backward sweep in register blocks of kSplineBlk intervals: the parked dp values and node values of a
+    // block are loaded first (independent loads, all in flight together), then the recurrence runs on
+    // registers, then the coefficients are stored.  (A load of dp_j issued between the stores of interval
+    // j + 1 could not be hoisted by the compiler: same base pointer, so each step paid a full memory latency.)
     double Mn = 0.0;
-    double y1 = y[(size_t)(n - 1) * sw];
-#pragma unroll 4
-    for (int j = n - 2; j >= 0; --j) {
-        const double y0 = y[(size_t)j * sw];
-        double Mj = 0.0;
-        if (j >= 1) Mj = fma(-__ldg(nt.tcp + j), Mn, c[(size_t)j * cj + sw]);
-        const double h = __ldg(nt.hj + j), ih = __ldg(nt.invh + j);
-        double *cc = c + (size_t)j * cj;
-        cc[0] = y0;
-        cc[sw] = (y1 - y0) * ih - h * (2.0 * Mj + Mn) * kSixth;
-        cc[2 * sw] = 0.5 * Mj;
-        cc[3 * sw] = (Mn - Mj) * ih * kSixth;
-        Mn = Mj;
-        y1 = y0;
+    double y1 = __ldg(y + (size_t)(n - 1) * sw);
+    for (int jt = n - 2; jt >= 0; jt -= kSplineBlk) {
+        double dpv[kSplineBlk], yv[kSplineBlk];
+#pragma unroll
+        for (int k = 0; k < kSplineBlk; ++k) {
+            const int j = jt - k;
+            dpv[k] = (j >= 1) ? c[(size_t)j * cj + sw] : 0.0;
+            yv[k] = (j >= 0) ? __ldg(y + (size_t)j * sw) : 0.0;
+        }
+#pragma unroll
+        for (int k = 0; k < kSplineBlk; ++k) {
+            const int j = jt - k;
+            if (j >= 0) {
+                const double y0 = yv[k];
+                const double Mj = (j >= 1) ? fma(-__ldg(nt.tcp + j), Mn, dpv[k]) : 0.0;
+                const double h = __ldg(nt.hj + j), ih = __ldg(nt.invh + j);
+                double *cc = c + (size_t)j * cj;
+                cc[0] = y0;
+                cc[sw] = (y1 - y0) * ih - h * (2.0 * Mj + Mn) * kSixth;
+                cc[2 * sw] = 0.5 * Mj;
+                cc[3 * sw] = (Mn - Mj) * ih * kSixth;
+                Mn = Mj;
+                y1 = y0;
+            }
+        }
     }
 }
 
@@ -754,30 +772,45 @@ __global__ void __launch_bounds__(128, 4) k_full_fused_mixed(FusedArgs a, FusedA
     o[0] = acc.sAr; o[sw] = acc.sAi; o[2 * sw] = acc.sEr; o[3 * sw] = acc.sEi; o[4 * sw] = acc.sH;
 }
 
-// F4: reduce the per-tile partials in tile order, apply T^c (single mode), form log L        (Eq. 2)
+// F4: reduce the per-tile partials in a fixed order, apply T^c (single mode), form log L        (Eq. 2)
+// Block = 32 walkers x kFinY tile slices: slice ty sums tiles t0 + ty, t0 + ty + kFinY, ... of its walker, the
+// slices meet in shared memory and are added in slice order (deterministic: reruns are bit-identical).
+constexpr int kFinY = 8;
 template <int NM1>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(32 * kFinY)
 k_finalize(const double *__restrict__ part, const double *__restrict__ TF, const int *__restrict__ perm,
            const int *__restrict__ ilo, const int *__restrict__ ihi, int n_wp, int TB, const double *__restrict__ dd,
            double *__restrict__ logL, double *__restrict__ d_h, double *__restrict__ h_h)
 {
-    const int p = blockIdx.x * blockDim.x + threadIdx.x;
-    if (p >= n_wp) return;
-    const int w = perm[p];
-    if (w < 0) return;
-    const size_t sw = (size_t)n_wp;
-    const int lo = ilo[p], hi = ihi[p];
     constexpr int NQ = NM1 ? 5 : 2;
+    __shared__ double red[kFinY][NQ][32];
+    const int p = blockIdx.x * 32 + threadIdx.x, ty = threadIdx.y;
+    const bool in = p < n_wp;
+    const size_t sw = (size_t)n_wp;
+    const int lo = in ? ilo[p] : 0, hi = in ? ihi[p] : 0;
     double acc[NQ];
 #pragma unroll
     for (int q = 0; q < NQ; ++q) acc[q] = 0.0;
     if (hi > lo) {
         const int t1 = (hi - 1) / TB;
-        for (int t = lo / TB; t <= t1; ++t) {
+        for (int t = lo / TB + ty; t <= t1; t += kFinY) {
             const double *o = part + ((size_t)t * NQ) * sw + p;
 #pragma unroll
             for (int q = 0; q < NQ; ++q) acc[q] += o[q * sw];
         }
+    }
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) red[ty][q][threadIdx.x] = acc[q];
+    __syncthreads();
+    if (ty != 0 || !in) return;
+    const int w = perm[p];
+    if (w < 0) return;
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) {
+        double v = red[0][q][threadIdx.x];
+#pragma unroll
+        for (int k = 1; k < kFinY; ++k) v += red[k][q][threadIdx.x];
+        acc[q] = v;
     }
     double dh, hh;
     if (NM1) {
