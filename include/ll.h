@@ -148,7 +148,9 @@ int ll_het_batch_standin_host(ll_ctx *ctx, int64_t n_w, const double *params_hos
 
 /* Measurement helpers (no part of the method).
  * ll_peak_fma: runs `iters` dependent-free FMA chains on every SM and returns the achieved rate in
- *   FMA/s (HOST out); which = 0 -> FP64 DFMA, 1 -> FP32 FFMA.  Used for the ALU roofline denominator.
+ *   FMA/s (HOST out); which = 0 -> FP64 DFMA (two loop-invariant register operands), 1 -> FP32 FFMA,
+ *   2 -> DFMA with three distinct register operands, 3 -> DFMA with one constant-bank operand.
+ *   Used for the ALU roofline denominator and for the operand-pattern note under profiles/.
  * ll_kernel_launches: number of kernels this context has launched since creation.
  * ll_last_full_stats: HOST out, after the stream is idle: active (walker, bin, mode) pairs and number of
  *   frequency tiles x walker blocks of the last full-grid call.                                           */

@@ -953,10 +953,11 @@ int ll_het_batch_standin_host(ll_ctx *ctx, int64_t n_w, const double *params_hos
 int ll_peak_fma(ll_ctx *ctx, int32_t which, int64_t iters, double *fma_per_s, double *ms_out, void *stream)
 {
     if (!ctx) return LL_ERR_ARG;
-    if (iters < 1 || (which != 0 && which != 1)) return ctx->fail(LL_ERR_ARG, "bad which/iters");
+    if (iters < 1 || which < 0 || which > 3) return ctx->fail(LL_ERR_ARG, "bad which/iters");
     DeviceGuard dg(ctx->device);
     cudaStream_t st = (cudaStream_t)stream;
     CK(ctx->prow.ensure(256));
+    CK(cudaMemsetAsync(ctx->prow.p, 0, 256, st));
     cudaEvent_t e0, e1;
     CK(cudaEventCreate(&e0));
     CK(cudaEventCreate(&e1));
@@ -964,7 +965,9 @@ int ll_peak_fma(ll_ctx *ctx, int32_t which, int64_t iters, double *fma_per_s, do
     for (int rep = 0; rep < 2; ++rep) { // first pass warms up
         CK(cudaEventRecord(e0, st));
         if (which == 0) k_peak_fma<double><<<blocks, threads, 0, st>>>(iters, ctx->prow.as<double>());
-        else k_peak_fma<float><<<blocks, threads, 0, st>>>(iters, ctx->prow.as<float>());
+        else if (which == 1) k_peak_fma<float><<<blocks, threads, 0, st>>>(iters, ctx->prow.as<float>());
+        else if (which == 2) k_peak_dfma_pattern<0><<<blocks, threads, 0, st>>>(iters, ctx->prow.as<double>());
+        else k_peak_dfma_pattern<1><<<blocks, threads, 0, st>>>(iters, ctx->prow.as<double>());
         LAUNCHED(ctx);
         CK(cudaEventRecord(e1, st));
         CK(cudaEventSynchronize(e1));

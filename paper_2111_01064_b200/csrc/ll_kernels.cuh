@@ -1228,4 +1228,29 @@ __global__ void __launch_bounds__(256) k_peak_fma(long long iters, T *__restrict
     if (s == (T)123456.789) sink[0] = s;
 }
 
+
+// operand-pattern variants of the FP64 peak kernel (profiles/: why k_full_fused tops out below 64 DFMA/clk/SM):
+//   PAT 0: three distinct, rotating register operands;  PAT 1: one operand from the constant bank
+__constant__ double kPeakC[4] = {0.999999, 1e-6, 0.5, 0.25};
+template <int PAT>
+__global__ void __launch_bounds__(256) k_peak_dfma_pattern(long long iters, double *__restrict__ sink)
+{
+    double a[8], b[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        a[k] = (double)(threadIdx.x + k) * 1e-3;
+        b[k] = 0.9999 + 1e-5 * k + sink[1];
+    }
+    for (long long it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int r = 0; r < 4; ++r)
+#pragma unroll
+            for (int k = 0; k < 8; ++k) a[k] = PAT == 0 ? fma(a[k], b[k], a[(k + 3) & 7]) : fma(a[k], b[k], kPeakC[r]);
+    }
+    double s = 0;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) s += a[k];
+    if (s == 123456.789) sink[0] = s;
+}
+
 } // namespace ll
