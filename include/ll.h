@@ -149,7 +149,9 @@ int ll_het_batch_standin_host(ll_ctx *ctx, int64_t n_w, const double *params_hos
 /* Measurement helpers (no part of the method).
  * ll_peak_fma: runs `iters` dependent-free FMA chains on every SM and returns the achieved rate in
  *   FMA/s (HOST out); which = 0 -> FP64 DFMA (two loop-invariant register operands), 1 -> FP32 FFMA,
- *   2 -> DFMA with three distinct register operands, 3 -> DFMA with one constant-bank operand.
+ *   2 -> DFMA with three distinct register operands, 3 -> DFMA with one constant-bank operand,
+ *   4 / 5 -> pattern 3 plus 1 integer add per 2 / per 1 DFMA, 6 / 7 -> pattern 3 plus 1 FFMA per 2 / per 1 DFMA
+ *   (the rate returned always counts the DFMAs only).
  *   Used for the ALU roofline denominator and for the operand-pattern note under profiles/.
  * ll_kernel_launches: number of kernels this context has launched since creation.
  * ll_last_full_stats: HOST out, after the stream is idle: active (walker, bin, mode) pairs and number of

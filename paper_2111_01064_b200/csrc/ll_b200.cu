@@ -953,7 +953,7 @@ int ll_het_batch_standin_host(ll_ctx *ctx, int64_t n_w, const double *params_hos
 int ll_peak_fma(ll_ctx *ctx, int32_t which, int64_t iters, double *fma_per_s, double *ms_out, void *stream)
 {
     if (!ctx) return LL_ERR_ARG;
-    if (iters < 1 || which < 0 || which > 3) return ctx->fail(LL_ERR_ARG, "bad which/iters");
+    if (iters < 1 || which < 0 || which > 7) return ctx->fail(LL_ERR_ARG, "bad which/iters");
     DeviceGuard dg(ctx->device);
     cudaStream_t st = (cudaStream_t)stream;
     CK(ctx->prow.ensure(256));
@@ -967,7 +967,11 @@ int ll_peak_fma(ll_ctx *ctx, int32_t which, int64_t iters, double *fma_per_s, do
         if (which == 0) k_peak_fma<double><<<blocks, threads, 0, st>>>(iters, ctx->prow.as<double>());
         else if (which == 1) k_peak_fma<float><<<blocks, threads, 0, st>>>(iters, ctx->prow.as<float>());
         else if (which == 2) k_peak_dfma_pattern<0><<<blocks, threads, 0, st>>>(iters, ctx->prow.as<double>());
-        else k_peak_dfma_pattern<1><<<blocks, threads, 0, st>>>(iters, ctx->prow.as<double>());
+        else if (which == 3) k_peak_dfma_pattern<1><<<blocks, threads, 0, st>>>(iters, ctx->prow.as<double>());
+        else if (which == 4) k_peak_dfma_mix<0, 16><<<blocks, threads, 0, st>>>(iters, ctx->prow.as<double>());
+        else if (which == 5) k_peak_dfma_mix<0, 32><<<blocks, threads, 0, st>>>(iters, ctx->prow.as<double>());
+        else if (which == 6) k_peak_dfma_mix<1, 16><<<blocks, threads, 0, st>>>(iters, ctx->prow.as<double>());
+        else k_peak_dfma_mix<1, 32><<<blocks, threads, 0, st>>>(iters, ctx->prow.as<double>());
         LAUNCHED(ctx);
         CK(cudaEventRecord(e1, st));
         CK(cudaEventSynchronize(e1));

@@ -135,6 +135,61 @@ __device__ __forceinline__ void amp_expi_qc_f32(float amp, double y, float &u, f
     v = as * a;
 }
 
+// packed binary32 pairs (sm_100 f32x2 instructions: one instruction for two bins' worth of FMA)
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pack2(float lo, float hi)
+{
+    f32x2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void unpack2(f32x2 v, float &lo, float &hi)
+{
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c)
+{
+    f32x2 r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+    return r;
+}
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b)
+{
+    f32x2 r;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+// both lanes: sin x = x + x^3 S1(x^2), cos x = 1 - x^2/2 + x^4 C2(x^2)   (same coefficients as sincos_poly_f32)
+__device__ __forceinline__ void sincos_poly_f32x2(f32x2 x, f32x2 &s, f32x2 &c)
+{
+    const f32x2 x2 = mul2(x, x);
+    f32x2 ps = fma2(pack2(0x1.7658e0p-19f, 0x1.7658e0p-19f), x2, pack2(-0x1.a0423ap-13f, -0x1.a0423ap-13f));
+    f32x2 pc = fma2(pack2(0x1.99ead0p-16f, 0x1.99ead0p-16f), x2, pack2(-0x1.6c0c2ep-10f, -0x1.6c0c2ep-10f));
+    ps = fma2(ps, x2, pack2(0x1.11115ep-7f, 0x1.11115ep-7f));
+    pc = fma2(pc, x2, pack2(0x1.55554ap-5f, 0x1.55554ap-5f));
+    ps = fma2(ps, x2, pack2(-0x1.555556p-3f, -0x1.555556p-3f));
+    pc = fma2(pc, x2, pack2(-0.5f, -0.5f));
+    s = fma2(mul2(x, x2), ps, x);
+    c = fma2(pc, x2, pack2(1.0f, 1.0f));
+}
+// FP64 part of amp_expi_qc_f32: quadrant number and reduced angle in radians (binary32)
+__device__ __forceinline__ float reduce_qc_to_rad_f32(double y, int &q)
+{
+    const double sh = __dadd_rn(y, kMagic);
+    q = __double2loint(sh);
+    const double nd = __dadd_rn(sh, -kMagic);
+    const double r = __dadd_rn(y, -nd);
+    return __double2float_rn(r * kPio2_1);
+}
+// quadrant bookkeeping on binary32: amp e^{-i angle} = u - i v with u = as * b, v = as * a
+__device__ __forceinline__ void quadrant_f32(int q, float amp, float s, float c, float &as, float &a, float &b)
+{
+    const bool sw = q & 1;
+    a = sw ? c : s;
+    b = sw ? -s : c;
+    as = flip_sign_if_f32(amp, ((unsigned)q << 30) & 0x80000000u);
+}
+
 // sin and cos of an angle in radians, accurate for |x| up to ~1e9 (three-term Cody-Waite with FMA; the
 // reduced argument is then handed to the quarter-cycle polynomials).
 __device__ __forceinline__ void sincos_rad(double x, double &sn, double &cs)

@@ -631,7 +631,9 @@ __global__ void __launch_bounds__(256) k_prescale_f32(const double *__restrict__
     if (i >= n_pad) return;
     const double is = scale[1], is2 = scale[2];
     const double4 g = reinterpret_cast<const double4 *>(g4)[i];
-    reinterpret_cast<float4 *>(g4f)[i] = make_float4((float)(g.x * is), (float)(g.y * is), (float)(g.z * is), (float)(g.w * is));
+    // pair-interleaved: bins (2p, 2p+1) -> [Ar Ar' Ai Ai' Er Er' Ei Ei'], so that one LDS.128 pair feeds f32x2 MACs
+    float *o = g4f + (i >> 1) * 8 + (i & 1);
+    o[0] = (float)(g.x * is); o[2] = (float)(g.y * is); o[4] = (float)(g.z * is); o[6] = (float)(g.w * is);
     Wds[i] = Wd[i] * is2;
 }
 
@@ -643,9 +645,10 @@ struct MixedAcc { // FP64 accumulators of one walker
 template <bool MASK>
 __device__ __forceinline__ void fused_bins_mixed(int b0, int b1, int tlo, int thi, int kbase, double df, double nxj,
                                                  double cA0, double cA1, double cA2, double cA3, double cP0, double cP1,
-                                                 double cP2, double cP3, const float4 *__restrict__ sg4,
+                                                 double cP2, double cP3, const float *__restrict__ sgp,
                                                  const double *__restrict__ sWc, MixedAcc &acc)
 {
+    // sgp: pair-interleaved data tile addressed by global bin (see k_prescale_f32)
     for (int base = b0; base < b1; base += kMixedChain) {
         const int end = min(base + kMixedChain, b1);
         float fAr = 0.f, fAi = 0.f, fEr = 0.f, fEi = 0.f;
@@ -658,13 +661,62 @@ __device__ __forceinline__ void fused_bins_mixed(int b0, int b1, int tlo, int th
             acc.sH = fma(sWc[ii] * A, A, acc.sH);
             float u, v; // h = u - i v
             amp_expi_qc_f32(__double2float_rn(A), y, u, v);
-            const float4 g = sg4[ii];
-            fAr = fmaf(g.x, u, fAr); fAr = fmaf(g.y, v, fAr);
-            fAi = fmaf(g.y, u, fAi); fAi = fmaf(-g.x, v, fAi);
-            fEr = fmaf(g.z, u, fEr); fEr = fmaf(g.w, v, fEr);
-            fEi = fmaf(g.w, u, fEi); fEi = fmaf(-g.z, v, fEi);
+            const float *gp = sgp + (ii >> 1) * 8 + (ii & 1);
+            const float gx = gp[0], gy = gp[2], gz = gp[4], gw = gp[6];
+            fAr = fmaf(gx, u, fAr); fAr = fmaf(gy, v, fAr);
+            fAi = fmaf(gy, u, fAi); fAi = fmaf(-gx, v, fAi);
+            fEr = fmaf(gz, u, fEr); fEr = fmaf(gw, v, fEr);
+            fEi = fmaf(gw, u, fEi); fEi = fmaf(-gz, v, fEi);
         }
         acc.sAr += (double)fAr; acc.sAi += (double)fAi; acc.sEr += (double)fEr; acc.sEi += (double)fEi;
+    }
+}
+
+// unmasked bins [b0, b1), b0 and b1 even: pairs of bins (2p, 2p+1) ride in the two lanes of f32x2 instructions
+// (sin/cos polynomials, A e^{-i Psi}, MACs): fewer instructions, and none of the select / add bookkeeping of two
+// scalar passes.  Each accumulator lane sums every other bin, so a flush every 2 kMixedChain bins keeps the chains
+// at kMixedChain terms.  The four products g_re u, g_im v, g_im u, g_re v are summed separately (f32x2 FMA has no
+// operand negation) and combined at the flush.
+__device__ __forceinline__ void fused_pairs_mixed(int b0, int b1, int kbase, double df, double nxj, double cA0, double cA1,
+                                                  double cA2, double cA3, double cP0, double cP1, double cP2, double cP3,
+                                                  const float *__restrict__ sgp, const double *__restrict__ sWc,
+                                                  MixedAcc &acc)
+{
+    for (int base = b0; base < b1; base += 2 * kMixedChain) {
+        const int end = min(base + 2 * kMixedChain, b1);
+        f32x2 aXU = 0, aYV = 0, aYU = 0, aXV = 0, eXU = 0, eYV = 0, eYU = 0, eXV = 0; // +0.0f in both lanes
+#pragma unroll 2
+        for (int ii = base; ii < end; ii += 2) {
+            const double t0 = fma((double)(kbase + ii), df, nxj), t1 = fma((double)(kbase + ii + 1), df, nxj);
+            const double A0 = fma(fma(fma(cA3, t0, cA2), t0, cA1), t0, cA0);
+            const double A1 = fma(fma(fma(cA3, t1, cA2), t1, cA1), t1, cA0);
+            const double y0 = fma(fma(fma(cP3, t0, cP2), t0, cP1), t0, cP0);
+            const double y1 = fma(fma(fma(cP3, t1, cP2), t1, cP1), t1, cP0);
+            const double2 w = *reinterpret_cast<const double2 *>(sWc + ii);
+            acc.sH = fma(w.x * A0, A0, acc.sH);
+            acc.sH = fma(w.y * A1, A1, acc.sH);
+            int q0, q1;
+            const float x0 = reduce_qc_to_rad_f32(y0, q0), x1 = reduce_qc_to_rad_f32(y1, q1);
+            f32x2 S, C;
+            sincos_poly_f32x2(pack2(x0, x1), S, C);
+            float s0, s1, c0, c1, as0, as1, a0, a1, bb0, bb1;
+            unpack2(S, s0, s1);
+            unpack2(C, c0, c1);
+            quadrant_f32(q0, __double2float_rn(A0), s0, c0, as0, a0, bb0);
+            quadrant_f32(q1, __double2float_rn(A1), s1, c1, as1, a1, bb1);
+            const f32x2 AS = pack2(as0, as1);
+            const f32x2 U = mul2(AS, pack2(bb0, bb1)), V = mul2(AS, pack2(a0, a1)); // h = u - i v per lane
+            const ulonglong2 gA = *reinterpret_cast<const ulonglong2 *>(sgp + (ii >> 1) * 8);
+            const ulonglong2 gE = *reinterpret_cast<const ulonglong2 *>(sgp + (ii >> 1) * 8 + 4);
+            aXU = fma2(gA.x, U, aXU); aYV = fma2(gA.y, V, aYV); aYU = fma2(gA.y, U, aYU); aXV = fma2(gA.x, V, aXV);
+            eXU = fma2(gE.x, U, eXU); eYV = fma2(gE.y, V, eYV); eYU = fma2(gE.y, U, eYU); eXV = fma2(gE.x, V, eXV);
+        }
+        float l0, h0, l1, h1;
+        // S^A_re = sum g_re u + g_im v,  S^A_im = sum g_im u - g_re v   (g already holds W conj(d))
+        unpack2(aXU, l0, h0); unpack2(aYV, l1, h1); acc.sAr += (double)((l0 + h0) + (l1 + h1));
+        unpack2(aYU, l0, h0); unpack2(aXV, l1, h1); acc.sAi += (double)((l0 + h0) - (l1 + h1));
+        unpack2(eXU, l0, h0); unpack2(eYV, l1, h1); acc.sEr += (double)((l0 + h0) + (l1 + h1));
+        unpack2(eYU, l0, h0); unpack2(eXV, l1, h1); acc.sEi += (double)((l0 + h0) - (l1 + h1));
     }
 }
 
@@ -750,18 +802,19 @@ __global__ void __launch_bounds__(128, 4) k_full_fused_mixed(FusedArgs a, FusedA
                 }
                 const int flo = __reduce_max_sync(0xffffffffu, max(lo, i));
                 const int fhi = __reduce_min_sync(0xffffffffu, min(hi, seg_end));
-                const float4 *sg4 = reinterpret_cast<const float4 *>(sg) - cb;
+                const float *sgp = reinterpret_cast<const float *>(sg) - (size_t)cb * 4; // cb is even
                 const double *sWc = sW - cb;
-                if (flo < fhi) {
-                    fused_bins_mixed<true>(wlo, flo, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1,
-                                           cP2, cP3, sg4, sWc, acc);
-                    fused_bins_mixed<false>(flo, fhi, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1,
-                                            cP2, cP3, sg4, sWc, acc);
-                    fused_bins_mixed<true>(fhi, whi, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1,
-                                           cP2, cP3, sg4, sWc, acc);
+                // masked bins up to the first even bin every lane has, packed pairs, masked rest
+                const int plo = (flo + 1) & ~1, phi = fhi & ~1;
+                if (plo < phi) {
+                    fused_bins_mixed<true>(wlo, plo, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1,
+                                           cP2, cP3, sgp, sWc, acc);
+                    fused_pairs_mixed(plo, phi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1, cP2, cP3, sgp, sWc, acc);
+                    fused_bins_mixed<true>(phi, whi, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1,
+                                           cP2, cP3, sgp, sWc, acc);
                 } else {
                     fused_bins_mixed<true>(wlo, whi, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1,
-                                           cP2, cP3, sg4, sWc, acc);
+                                           cP2, cP3, sgp, sWc, acc);
                 }
             }
             i = seg_end;
@@ -1251,6 +1304,45 @@ __global__ void __launch_bounds__(256) k_peak_dfma_pattern(long long iters, doub
 #pragma unroll
     for (int k = 0; k < 8; ++k) s += a[k];
     if (s == 123456.789) sink[0] = s;
+}
+
+
+// issue-mix variants: 32 constant-bank DFMA per iteration plus NI independent integer adds (MIX 0) or binary32
+// FMAs (MIX 1) per iteration, in separate dependency chains.  Shows whether instructions for other pipes ride
+// along for free while the FP64 pipe is saturated (they do not: profiles/).
+template <int MIX, int NI>
+__global__ void __launch_bounds__(256) k_peak_dfma_mix(long long iters, double *__restrict__ sink)
+{
+    double a[8], b[8];
+    int q[8];
+    float f[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        a[k] = (double)(threadIdx.x + k) * 1e-3;
+        b[k] = 0.9999 + 1e-5 * k + sink[1];
+        q[k] = threadIdx.x + k;
+        f[k] = (float)(threadIdx.x + k) * 1e-3f;
+    }
+    const int inc = (int)sink[2] + 3;
+    const float fm = (float)sink[3] + 0.999f;
+    for (long long it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int r = 0; r < 4; ++r)
+#pragma unroll
+            for (int k = 0; k < 8; ++k) {
+                a[k] = fma(a[k], b[k], kPeakC[r]);
+                if ((r * 8 + k) < NI) {
+                    if (MIX == 0) asm volatile("add.s32 %0, %0, %1;" : "+r"(q[k]) : "r"(inc));
+                    else asm volatile("fma.rn.f32 %0, %0, %1, %1;" : "+f"(f[k]) : "f"(fm));
+                }
+            }
+    }
+    double s = 0;
+    int t = 0;
+    float g = 0.f;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) { s += a[k]; t += q[k]; g += f[k]; }
+    if (s == 123456.789 || t == 123456789 || g == 1234.5f) sink[0] = s;
 }
 
 } // namespace ll

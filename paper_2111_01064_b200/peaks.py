@@ -15,6 +15,10 @@ from .binding import Context
 PATTERNS = ((0, "DFMA  a = fma(a, m, c), m and c loop-invariant registers", 4000),
             (2, "DFMA  three distinct register operands", 4000),
             (3, "DFMA  one operand from the constant bank", 4000),
+            (4, "DFMA  constant bank + 1 integer add per 2 DFMA", 4000),
+            (5, "DFMA  constant bank + 1 integer add per DFMA", 4000),
+            (6, "DFMA  constant bank + 1 FFMA per 2 DFMA", 4000),
+            (7, "DFMA  constant bank + 1 FFMA per DFMA", 4000),
             (1, "FFMA  a = fma(a, m, c)", 8000))
 
 
