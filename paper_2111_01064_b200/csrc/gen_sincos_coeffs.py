@@ -99,8 +99,8 @@ def emit_f32_sequential(name, F, n, weight):
 
 
 if __name__ == "__main__":
-    emit("S (sin(pi r/2)/r), error weighted by r", S, 6, "f64", lambda u: mp.sqrt(u))
-    emit("C (cos(pi r/2))", C, 6, "f64", lambda u: 1)
+    emit("S (sin(pi r/2)/r), error weighted by r", S, 5, "f64", lambda u: mp.sqrt(u))
+    emit("C (cos(pi r/2))", C, 5, "f64", lambda u: 1)
     B = (mp.pi / 4) ** 2
     emit_f32_sequential("S1 (sin x = x + x^3 S1(x^2)), error weighted by x^3", S1, 3, lambda u: mp.sqrt(u) ** 3)
     emit_f32_sequential("C2 (cos x = 1 - x^2/2 + x^4 C2(x^2)), error weighted by x^4", C2, 2, lambda u: u * u)

@@ -252,6 +252,9 @@ int prepare_nodes(ll_ctx *ctx, int n, const double *x, cudaStream_t st)
     return LL_OK;
 }
 
+#ifndef LL_FUSED_CH
+#define LL_FUSED_CH 256 // bins per TMA stage of the fused kernel (two stages per block)
+#endif
 FullPlan make_plan(const ll_ctx *ctx, long long n_w)
 {
     FullPlan pl;
@@ -264,7 +267,7 @@ FullPlan make_plan(const ll_ctx *ctx, long long n_w)
     int TB = 64;
     while (TB < 4096 && TB < tb) TB <<= 1;
     pl.TB = TB;
-    pl.CH = std::min(TB, 256);
+    pl.CH = std::min(TB, LL_FUSED_CH);
     pl.n_tiles = ceil_div(ctx->n_f, TB);
     pl.key_gran = std::max(1, ceil_div(ctx->n_f, 4096));
     pl.n_keys = (int)(ctx->n_f / pl.key_gran) + 2;

@@ -17,22 +17,22 @@ constexpr double kPio2_2 = 0x1.1a62633145c07p-54;
 constexpr double kPio2_3 = -0x1.f1976b7ed8fbcp-110;
 constexpr double kSixth = 0x1.5555555555555p-3;
 
-// sin(pi r/2) = r * S(r^2), cos(pi r/2) = C(r^2), |r| <= 1/2.  S and C are degree-6 polynomials in r^2
-// interpolated at the Chebyshev nodes of [0, 1/4] (gen_sincos_coeffs.py; max error 2.6e-17 (sin), 1.0e-16
-// (cos) before evaluation rounding).  The coefficients live in constant memory so that every Horner step is
-// one DFMA with a constant-bank operand (no UMOV/IMAD.MOV literal rebuilds inside the hot loop).
-__constant__ double kSinC[7] = {0x1.921fb54442d18p+0,  -0x1.4abbce625be41p-1, 0x1.466bc677587f8p-4, -0x1.32d2cce2e5b19p-8,
-                                0x1.50782fda12d96p-13, -0x1.e30071afc3e59p-19, 0x1.e3f38399551bfp-25};
-__constant__ double kCosC[7] = {0x1.0000000000000p+0,  -0x1.3bd3cc9be458bp+0, 0x1.03c1f081b0780p-2, -0x1.55d3c7dbfd139p-6,
-                                0x1.e1f4fb60281f6p-11, -0x1.a6c9c1be9eb49p-16, 0x1.f3dbcea61b1a4p-22};
+// sin(pi r/2) = r * S(r^2), cos(pi r/2) = C(r^2), |r| <= 1/2.  S and C are degree-5 polynomials in r^2
+// interpolated at the Chebyshev nodes of [0, 1/4] (gen_sincos_coeffs.py; max error 3.4e-15 (sin), 5.6e-14 (cos)).
+// That is far below the rounding of the argument itself (a phase of 1e6-1e7 quarter cycles carries 1e-10-1e-9 of
+// absolute error in FP64) and 20x below what the 1e-6 bar on log L needs at <d|h> = 1e6; one more term each would
+// cost two FP64 issue slots per bin for nothing measurable.  The coefficients live in constant memory so that every
+// Horner step is one DFMA with a constant-bank operand (no UMOV/IMAD.MOV literal rebuilds inside the hot loop).
+__constant__ double kSinC[6] = {0x1.921fb54442cfap+0, -0x1.4abbce6257a2ap-1, 0x1.466bc67123fa1p-4,
+                                -0x1.32d2c644adc0bp-8, 0x1.5071ce4b47930p-13, -0x1.dd54805f3f706p-19};
+__constant__ double kCosC[6] = {0x1.ffffffffffe0bp-1, -0x1.3bd3cc9bd2c35p+0, 0x1.03c1f074ded21p-2,
+                                -0x1.55d3ba300cd50p-6, 0x1.e1e7ccccb387ap-11, -0x1.a0ee132c60c1fp-16};
 
 __device__ __forceinline__ void sincos_poly_qc(double r, double &s, double &c)
 {
     const double r2 = r * r;
-    double ps = fma(kSinC[6], r2, kSinC[5]);
-    double pc = fma(kCosC[6], r2, kCosC[5]);
-    ps = fma(ps, r2, kSinC[4]);
-    pc = fma(pc, r2, kCosC[4]);
+    double ps = fma(kSinC[5], r2, kSinC[4]);
+    double pc = fma(kCosC[5], r2, kCosC[4]);
     ps = fma(ps, r2, kSinC[3]);
     pc = fma(pc, r2, kCosC[3]);
     ps = fma(ps, r2, kSinC[2]);
@@ -64,9 +64,10 @@ __device__ __forceinline__ void quadrant_apply(int q, double amp, double s, doub
 {
     // sn = sg * a, cs = sg * (sw ? -s : c), sg = (q & 2) ? -1 : 1, a = sw ? c : s
     const bool sw = q & 1;
-    const double ms = flip_sign_if(s, 0x80000000u);
     const double a = sw ? c : s;
-    const double b = sw ? ms : c;
+    // b = sw ? -s : c, written on the words so that the negation folds into the select of the high word
+    const float bh = sw ? -__int_as_float(__double2hiint(s)) : __int_as_float(__double2hiint(c));
+    const double b = __hiloint2double(__float_as_int(bh), sw ? __double2loint(s) : __double2loint(c));
     const double as = flip_sign_if(amp, ((unsigned)q << 30) & 0x80000000u);
     u = as * b;
     v = as * a;

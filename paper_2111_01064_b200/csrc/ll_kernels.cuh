@@ -419,7 +419,7 @@ __device__ __forceinline__ int find_interval_of_bin(const int *__restrict__ bsta
 }
 
 #ifndef LL_FUSED_UNROLL
-#define LL_FUSED_UNROLL 4 // bins in flight per thread in the hot loop (tuned on B200, profiles/)
+#define LL_FUSED_UNROLL 3 // bins in flight per thread in the hot loop (tuned on B200, profiles/)
 #endif
 #ifndef LL_FUSED_MINB
 #define LL_FUSED_MINB 4 // resident 128-thread blocks per SM the register budget is held to
