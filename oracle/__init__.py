@@ -151,6 +151,36 @@ def full_batch(f_nodes, amp, phase, tf, band, k_min, df, d, W, want_template=Fal
     return out
 
 
+def full_batch_tf(f_nodes, amp, phase, tf_nodes, band, k_min, df, d, W, want_template=False):
+    """frequency-dependent transfer function T [n_w][n_m][n_c][n_nodes][2] splined alongside amp/phase (Eq. 8-9)."""
+    f_nodes, amp, phase, tf_nodes, W = _f64(f_nodes), _f64(amp), _f64(phase), _f64(tf_nodes), _f64(W)
+    n_w, n_m, n_nodes = amp.shape
+    n_c = tf_nodes.shape[2]
+    assert tf_nodes.shape == (n_w, n_m, n_c, n_nodes, 2)
+    n_f = W.shape[0]
+    band = None if band is None else _f64(band)
+    d = None if d is None else _f64(d)
+    out = {k: np.empty(n_w) for k in ("logL", "d_h", "h_h", "logL_direct")}
+    h = np.empty((n_c, n_f, 2)) if want_template else None
+    _check(lib().orc_full_batch_tf(C.c_int64(n_w), C.c_int(n_m), C.c_int(n_c), C.c_int(n_nodes), _p(f_nodes),
+                                   _p(amp), _p(phase), _p(tf_nodes), _p(band), C.c_int64(n_f), C.c_int64(k_min),
+                                   C.c_double(df), _p(d), _p(W), _p(out["logL"]), _p(out["d_h"]), _p(out["h_h"]),
+                                   _p(out["logL_direct"]), _p(h)), "full_batch_tf")
+    if want_template:
+        out["h"] = h
+    return out
+
+
+def tlm_nodes(f_nodes, phase, t_ref) -> np.ndarray:
+    """t_lm(f_j) = t_ref - (1/2pi) dphi/df from the natural spline of the node phases (Eq. 8)."""
+    f_nodes, phase = _f64(f_nodes), _f64(phase)
+    n_w, n_m, n_nodes = phase.shape
+    out = np.empty_like(phase)
+    _check(lib().orc_tlm_nodes(C.c_int64(n_w), C.c_int(n_m), C.c_int(n_nodes), _p(f_nodes), _p(phase),
+                               C.c_double(t_ref), _p(out)), "tlm_nodes")
+    return out
+
+
 def full_batch_standin(wl_modes_m, c_lm, kappa, params, f_nodes, k_min, df, n_f, d, W, want_template=False):
     """parameters -> node arrays (stand-in, rounded to fp64) -> full_batch."""
     f_lo, f_hi = float(k_min) * df, float(k_min + n_f - 1) * df

@@ -29,13 +29,16 @@
  * elimination, linear/cubic reproduction; closed-form <h|h> under a flat PSD (+ Euler-Maclaurin term)
  * and mpmath sums; log L = 0 at d = h; 1/D, phi_c scalings; brute-force numpy/mpmath sums on tiny
  * inputs; summary-data partition exactness; het exactness for r linear in f and its known B2
- * deficit; het == full at h = h0.  No function here is "parity unpinned".
+ * deficit; het == full at h = h0; the frequency-dependent-T path against the constant-T path, a template
+ * whose T is linear in f against direct numpy evaluation, SciPy on tiny inputs; t_lm against SciPy's spline
+ * derivative and the stand-in's analytic d Psi/df.  No function here is "parity unpinned".
  *
  * Layouts (all row-major, fp64):
  *   d, h, h0_dense, noise : [n_c][n_f][2]  (re, im)
  *   W                     : [n_f]          W_k = 4 df w_k / S_n(f_k)
  *   amp, phase            : [n_w][n_m][n_nodes]   (phase in radians)
  *   tf                    : [n_w][n_m][n_c][2]
+ *   tf_nodes              : [n_w][n_m][n_c][n_nodes][2]   (frequency-dependent transfer function, Eq. 8-9)
  *   band                  : [n_w][2] (f_lo, f_hi) or NULL
  *   params                : [n_w][P], P = 5 + 2 n_c n_m:
  *                           Mc[s], q, t_c[s], phi_c[rad], 1/D, then T^c_m (re, im), m-major, c-minor
@@ -307,6 +310,115 @@ int orc_full_batch(int64_t n_w, int n_m, int n_c, int n_nodes, const double *f_n
         if (h_h) h_h[w] = (double)s_hh;
         if (logL_direct) logL_direct[w] = (double)(-0.5L * s_res);
         free(yA); free(MA); free(yP); free(MP);
+    }
+    return fail ? -4 : 0;
+}
+
+/* ---------------------------------------------------------------------------------------------
+ * Full-grid path with a frequency-dependent transfer function.
+ *   h~^{A,E}(f) = sum_lm T^{A,E}(f, t_lm(f)) h~_lm(f)                          Eq. 9
+ * The transfer function's formula is in the paper's ref. [44], not in PAPER.md, so T arrives as caller
+ * arrays at the spline nodes, T_nodes [n_w][n_m][n_c][n_nodes][2] (re, im); its real and imaginary parts
+ * are splined exactly like amplitude and phase (natural cubic in f, reading R1) and evaluated per bin.
+ * Everything else is orc_full_batch.
+ * ------------------------------------------------------------------------------------------- */
+int orc_full_batch_tf(int64_t n_w, int n_m, int n_c, int n_nodes, const double *f_nodes,
+                      const double *amp, const double *phase, const double *tf_nodes, const double *band,
+                      int64_t n_f, int64_t k_min, double df, const double *d, const double *W,
+                      double *logL, double *d_h, double *h_h, double *logL_direct, double *h_out)
+{
+    if (n_nodes < 3 || n_m < 1 || n_c < 1 || n_c > 3) return -1;
+    if (h_out && n_w != 1) return -1;
+    const ld dd = d ? inner_dd(n_c, n_f, d, W, 0, n_f) : 0.0L;
+    int fail = 0;
+    #pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t w = 0; w < n_w; ++w) {
+        const size_t nn = (size_t)n_nodes;
+        const size_t ns = (size_t)n_m * (2 + 2 * (size_t)n_c);      /* splines per walker */
+        ld *y = (ld *)malloc(sizeof(ld) * nn * ns), *M = (ld *)malloc(sizeof(ld) * nn * ns);
+        if (!y || !M) { fail = 1; free(y); free(M); continue; }
+        /* spline s of mode m: 0 amplitude, 1 phase, 2 + 2c Re T^c, 3 + 2c Im T^c */
+        for (int m = 0; m < n_m; ++m) {
+            ld *ym = y + (size_t)m * (2 + 2 * n_c) * nn, *Mm = M + (size_t)m * (2 + 2 * n_c) * nn;
+            for (int j = 0; j < n_nodes; ++j) {
+                ym[0 * nn + j] = (ld)amp[(w * n_m + m) * nn + j];
+                ym[1 * nn + j] = (ld)phase[(w * n_m + m) * nn + j];
+                for (int c = 0; c < n_c; ++c) {
+                    const double *t = tf_nodes + ((((size_t)w * n_m + m) * n_c + c) * nn + j) * 2;
+                    ym[(2 + 2 * c) * nn + j] = (ld)t[0];
+                    ym[(3 + 2 * c) * nn + j] = (ld)t[1];
+                }
+            }
+            for (int s = 0; s < 2 + 2 * n_c; ++s) spline_natural_ld(n_nodes, f_nodes, ym + s * nn, Mm + s * nn);
+        }
+        const double f_lo = band ? band[2 * w] : -HUGE_VAL, f_hi = band ? band[2 * w + 1] : HUGE_VAL;
+        ld s_dh = 0.0L, s_hh = 0.0L, s_res = 0.0L;
+        for (int c = 0; c < n_c; ++c)
+            for (int64_t i = 0; i < n_f; ++i) {
+                const double f = (double)(k_min + i) * df;
+                ld hr = 0.0L, hi = 0.0L;
+                if (f >= f_lo && f <= f_hi) {
+                    const int j = find_interval(n_nodes, f_nodes, f);
+                    for (int m = 0; m < n_m; ++m) {
+                        const ld *ym = y + (size_t)m * (2 + 2 * n_c) * nn, *Mm = M + (size_t)m * (2 + 2 * n_c) * nn;
+                        ld A = spline_eval_ld(f_nodes, ym, Mm, j, f);
+                        ld Psi = spline_eval_ld(f_nodes, ym + nn, Mm + nn, j, f);
+                        ld tr = spline_eval_ld(f_nodes, ym + (2 + 2 * c) * nn, Mm + (2 + 2 * c) * nn, j, f);
+                        ld ti = spline_eval_ld(f_nodes, ym + (3 + 2 * c) * nn, Mm + (3 + 2 * c) * nn, j, f);
+                        ld mr = A * cosl(Psi), mi = -A * sinl(Psi);          /* Eq. 7: A e^{-i Psi} */
+                        hr += tr * mr - ti * mi;                             /* Eq. 9 */
+                        hi += tr * mi + ti * mr;
+                    }
+                }
+                if (h_out) { h_out[(c * n_f + i) * 2] = (double)hr; h_out[(c * n_f + i) * 2 + 1] = (double)hi; }
+                if (d) {
+                    ld dr = d[(c * n_f + i) * 2], di = d[(c * n_f + i) * 2 + 1];
+                    s_dh += (ld)W[i] * (dr * hr + di * hi);
+                    s_res += (ld)W[i] * ((dr - hr) * (dr - hr) + (di - hi) * (di - hi));
+                }
+                s_hh += (ld)W[i] * (hr * hr + hi * hi);
+            }
+        if (logL) logL[w] = (double)(s_dh - 0.5L * s_hh - 0.5L * dd);
+        if (d_h) d_h[w] = (double)s_dh;
+        if (h_h) h_h[w] = (double)s_hh;
+        if (logL_direct) logL_direct[w] = (double)(-0.5L * s_res);
+        free(y); free(M);
+    }
+    return fail ? -4 : 0;
+}
+
+/* ---------------------------------------------------------------------------------------------
+ * Time-frequency correspondence at the spline nodes                              Eq. 8
+ *   t_lm(f) = t_ref - (1/2pi) d phi_lm / df
+ * with d phi/df the first derivative of the natural cubic spline of the node phases (reading R1):
+ *   y'(x_j)     = (y_{j+1}-y_j)/h_j - h_j (2 M_j + M_{j+1})/6          j < n-1  (left end of interval j)
+ *   y'(x_{n-1}) = (y_{n-1}-y_{n-2})/h + h (M_{n-2} + 2 M_{n-1})/6      (right end of the last interval)
+ * phase [n_w][n_m][n_nodes] radians -> t_lm [n_w][n_m][n_nodes] seconds.
+ * ------------------------------------------------------------------------------------------- */
+int orc_tlm_nodes(int64_t n_w, int n_m, int n_nodes, const double *f_nodes, const double *phase, double t_ref,
+                  double *t_lm)
+{
+    if (n_nodes < 3 || n_m < 1) return -1;
+    int fail = 0;
+    #pragma omp parallel for schedule(static)
+    for (int64_t s = 0; s < n_w * n_m; ++s) {
+        const size_t nn = (size_t)n_nodes;
+        ld *y = (ld *)malloc(sizeof(ld) * nn), *M = (ld *)malloc(sizeof(ld) * nn);
+        if (!y || !M) { fail = 1; free(y); free(M); continue; }
+        for (int j = 0; j < n_nodes; ++j) y[j] = (ld)phase[(size_t)s * nn + j];
+        spline_natural_ld(n_nodes, f_nodes, y, M);
+        for (int j = 0; j < n_nodes; ++j) {
+            ld dy;
+            if (j < n_nodes - 1) {
+                const ld h = (ld)f_nodes[j + 1] - (ld)f_nodes[j];
+                dy = (y[j + 1] - y[j]) / h - h * (2.0L * M[j] + M[j + 1]) / 6.0L;
+            } else {
+                const ld h = (ld)f_nodes[j] - (ld)f_nodes[j - 1];
+                dy = (y[j] - y[j - 1]) / h + h * (M[j - 1] + 2.0L * M[j]) / 6.0L;
+            }
+            t_lm[(size_t)s * nn + j] = (double)((ld)t_ref - dy / (2.0L * PI_L));
+        }
+        free(y); free(M);
     }
     return fail ? -4 : 0;
 }

@@ -534,3 +534,116 @@ def test_noise_normalisation_statistic(orc):
     # E<n|n> = 2 n_f per channel
     nn = np.mean([orc.dd(wlm._draw_noise(91000 + s, g, 2), wl.W) for s in range(20)])
     assert nn == pytest.approx(4.0 * g.n_f, rel=0.05)
+
+
+# ------------------------------------------- frequency-dependent transfer function (Eq. 8-9), SURVEY §8(f) item 1
+def _rand_tf_nodes(rng, n_w, n_m, n_c, f_nodes):
+    """smooth complex T^c_m at the nodes: (a + b x + c sin(2x + p)) e^{i(q + r x)}, x = normalised log f"""
+    x = np.log(f_nodes / f_nodes[0]) / np.log(f_nodes[-1] / f_nodes[0])
+    t = np.empty((n_w, n_m, n_c, len(f_nodes), 2))
+    for idx in np.ndindex(n_w, n_m, n_c):
+        a = rng.uniform(-1.0, 1.0, 6)
+        mod = 1.0 + 0.3 * a[0] * x + 0.2 * a[1] * np.sin(2 * x + a[2])
+        ang = 3.0 * a[3] + 2.0 * a[4] * x
+        t[idx][:, 0], t[idx][:, 1] = mod * np.cos(ang), mod * np.sin(ang)
+    return t
+
+
+def test_tf_path_reduces_to_constant_tf_path(orc):
+    """T constant over the nodes: its spline is that constant, so the result is orc_full_batch's (pinned above).
+    Fails on a wrong Re/Im slot, a channel/mode index swap or a conjugation in the new path."""
+    rng = np.random.default_rng(41)
+    k_min, df, n_f, n_w, n_m = 7, 1.0 / 2048.0, 90, 4, 3
+    f_lo, f_hi = k_min * df, (k_min + n_f - 1) * df
+    f_nodes = wlm.geomspace_exact(f_lo * 0.95, f_hi * 1.02, 12)
+    amp, ph = _rand_smooth_nodes(rng, n_w, n_m, f_nodes)
+    tf = _unit_tf(rng, n_w, n_m) * rng.uniform(0.5, 1.5, (n_w, n_m, 2, 1))
+    tfn = np.repeat(tf[:, :, :, None, :], len(f_nodes), axis=3)
+    W = rng.uniform(0.5, 2.0, n_f)
+    d = rng.standard_normal((2, n_f, 2))
+    band = np.array([[f_lo, f_hi], [f_lo + 2.5 * df, f_hi - 7.1 * df], [f_lo, f_lo + 20 * df], [f_hi * 2, f_hi * 3]])
+    a = orc.full_batch(f_nodes, amp, ph, tf, band, k_min, df, d, W)
+    b = orc.full_batch_tf(f_nodes, amp, ph, tfn, band, k_min, df, d, W)
+    for k in ("logL", "d_h", "h_h", "logL_direct"):
+        np.testing.assert_allclose(b[k], a[k], rtol=1e-14, atol=1e-13)
+
+
+def test_tf_path_linear_T_against_direct_numpy(orc):
+    """Re T and Im T linear in f are reproduced exactly by any cubic spline, so the dense template must equal
+    (alpha + beta f) x (the constant-T template with T = 1) bin by bin, computed here in numpy.
+    Fails if T is evaluated at the wrong frequency / interval or multiplied in the wrong order."""
+    rng = np.random.default_rng(43)
+    k_min, df, n_f, n_m = 11, 1.0 / 1024.0, 70, 2
+    f = np.arange(k_min, k_min + n_f) * df
+    f_nodes = wlm.geomspace_exact(f[0] * 0.9, f[-1] * 1.1, 9)
+    amp, ph = _rand_smooth_nodes(rng, 1, n_m, f_nodes)
+    W = rng.uniform(0.5, 2.0, n_f)
+    d = rng.standard_normal((2, n_f, 2))
+    alpha = rng.standard_normal((n_m, 2)) + 1j * rng.standard_normal((n_m, 2))
+    beta = (rng.standard_normal((n_m, 2)) + 1j * rng.standard_normal((n_m, 2))) / f[-1]
+    tfn = np.empty((1, n_m, 2, len(f_nodes), 2))
+    h_expect = np.zeros((2, n_f), dtype=complex)
+    for m in range(n_m):
+        one = np.zeros((1, 1, 2, 2)); one[..., 0] = 1.0
+        hm = orc.full_batch(f_nodes, amp[:, m:m + 1], ph[:, m:m + 1], one, None, k_min, df, None, W, want_template=True)["h"]
+        hm = hm[..., 0] + 1j * hm[..., 1]                          # [n_c][n_f], identical channels (T = 1)
+        for c in range(2):
+            tn = alpha[m, c] + beta[m, c] * f_nodes
+            tfn[0, m, c, :, 0], tfn[0, m, c, :, 1] = tn.real, tn.imag
+            h_expect[c] += (alpha[m, c] + beta[m, c] * f) * hm[c]
+    o = orc.full_batch_tf(f_nodes, amp, ph, tfn, None, k_min, df, d, W, want_template=True)
+    h = o["h"][..., 0] + 1j * o["h"][..., 1]
+    np.testing.assert_allclose(h, h_expect, rtol=1e-12, atol=1e-30)
+    dc = d[..., 0] + 1j * d[..., 1]
+    assert o["d_h"][0] == pytest.approx(float(np.sum(W * (np.conj(dc) * h_expect).real)), rel=1e-11)
+    assert o["h_h"][0] == pytest.approx(float(np.sum(W * np.abs(h_expect) ** 2)), rel=1e-12)
+
+
+def test_tf_path_brute_force_scipy(orc):
+    """tiny case, every spline by SciPy, sums by numpy complex arithmetic"""
+    rng = np.random.default_rng(47)
+    k_min, df, n_f, n_w, n_m = 4, 1.0 / 512.0, 40, 3, 2
+    f = np.arange(k_min, k_min + n_f) * df
+    f_nodes = wlm.geomspace_exact(f[0], f[-1], 7)
+    amp, ph = _rand_smooth_nodes(rng, n_w, n_m, f_nodes)
+    tfn = _rand_tf_nodes(rng, n_w, n_m, 2, f_nodes)
+    W = rng.uniform(0.5, 2.0, n_f)
+    d = rng.standard_normal((2, n_f, 2))
+    dc = d[..., 0] + 1j * d[..., 1]
+    band = np.array([[f[0], f[-1]], [f[3] + 0.2 * df, f[-4] - 0.3 * df], [f[0], f[10]]])
+    o = orc.full_batch_tf(f_nodes, amp, ph, tfn, band, k_min, df, d, W)
+    sp = lambda y: CubicSpline(f_nodes, y, bc_type="natural")(f)
+    for w in range(n_w):
+        mask = (f >= band[w, 0]) & (f <= band[w, 1])
+        h = np.zeros((2, n_f), dtype=complex)
+        for m in range(n_m):
+            z = sp(amp[w, m]) * np.exp(-1j * sp(ph[w, m]))
+            for c in range(2):
+                h[c] += (sp(tfn[w, m, c, :, 0]) + 1j * sp(tfn[w, m, c, :, 1])) * z
+        h *= mask
+        dh = float(np.sum(W * (np.conj(dc) * h).real)); hh = float(np.sum(W * np.abs(h) ** 2))
+        assert o["d_h"][w] == pytest.approx(dh, rel=1e-10, abs=1e-10)
+        assert o["h_h"][w] == pytest.approx(hh, rel=1e-10)
+        assert o["logL"][w] == pytest.approx(dh - 0.5 * hh - 0.5 * orc.dd(d, W), rel=1e-10)
+        assert o["logL_direct"][w] == pytest.approx(-0.5 * float(np.sum(W * np.abs(dc - h) ** 2)), rel=1e-10)
+
+
+def test_tlm_nodes_matches_scipy_derivative_and_chirp_time(orc):
+    """Eq. 8: t_lm = t_ref - (1/2pi) dphi/df.  (i) the spline derivative at every node equals SciPy's;
+    (ii) for the stand-in phase, whose 2 pi f t_c term is inside phi, t_ref = 0 gives -(t_c - tau(f)) up to the
+    spline's own error (interior nodes of a 256-node grid): fails on a sign, a 2 pi, or an off-by-one node."""
+    rng = np.random.default_rng(53)
+    f_nodes = wlm.geomspace_exact(1e-4, 5e-2, 40)
+    _, ph = _rand_smooth_nodes(rng, 2, 3, f_nodes)
+    t = orc.tlm_nodes(f_nodes, ph, 123.0)
+    for w in range(2):
+        for m in range(3):
+            dy = CubicSpline(f_nodes, ph[w, m], bc_type="natural")(f_nodes, 1)
+            np.testing.assert_allclose(t[w, m], 123.0 - dy / TWO_PI, rtol=1e-9, atol=1e-9 * np.abs(dy).max() / TWO_PI)
+    p = _row(mc_msun=4e5, q=0.3, t_c=9.0e4)
+    fn = wlm.geomspace_exact(1e-4, 5e-2, 256)
+    _, php, _, _ = orc.standin_nodes(p[None], mode_m=[2], c_lm=[1.0], kappa=0.5, f=fn, f_grid_lo=0.0, f_grid_hi=1.0)
+    tl = orc.tlm_nodes(fn, php, 0.0)[0, 0]
+    tau = 5.0 / 256.0 * p[0] ** (-5.0 / 3.0) * (math.pi * fn) ** (-8.0 / 3.0)
+    sl = slice(20, 236)
+    np.testing.assert_allclose(tl[sl], -(p[2] - tau[sl]), rtol=2e-6, atol=0.1)   # seconds; values 1e3 .. 4e6
