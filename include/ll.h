@@ -99,6 +99,21 @@ int ll_full_batch(ll_ctx *ctx, int64_t n_w, int32_t n_nodes, const double *f_nod
                   const double *phase, const double *tf, const double *band, double *logL, double *d_h,
                   double *h_h, void *stream);
 
+/* F2-F4 with a frequency-dependent transfer function — h^c(f) = sum_lm T^c_lm(f, t_lm(f)) h_lm(f) (Eq. 8-9,
+ * PAPER.md:100-110).  The transfer function's formula is in the paper's ref. [44], so T arrives at the nodes:
+ *   tf_nodes : DEV [n_w][n_m][n_c][n_nodes][2]  (re, im); Re T and Im T are splined exactly like amp and phase
+ *              (natural cubic in f) and evaluated at every dense bin.  Other arguments as ll_full_batch.
+ * FP64 contexts only (LL_ERR_UNSUPPORTED otherwise).                                                        */
+int ll_full_batch_tf(ll_ctx *ctx, int64_t n_w, int32_t n_nodes, const double *f_nodes, const double *amp,
+                     const double *phase, const double *tf_nodes, const double *band, double *logL, double *d_h,
+                     double *h_h, void *stream);
+
+/* Eq. 8 utility — t_lm(f_j) = t_ref - (1/2pi) dphi_lm/df at the nodes, dphi/df being the first derivative of the
+ * natural cubic spline of the node phases (what a caller needs to evaluate T(f, t_lm(f)) at the nodes).
+ *   phase : DEV [n_w][n_m][n_nodes] radians;  t_lm : DEV out, same shape, seconds.  Needs ll_set_data first.   */
+int ll_tlm_nodes(ll_ctx *ctx, int64_t n_w, int32_t n_nodes, const double *f_nodes, const double *phase,
+                 double t_ref, double *t_lm, void *stream);
+
 /* F1-F4 — same, the node arrays produced on the device from parameter rows by the stand-in waveform.
  *   params : DEV [n_w][P]                                                                                 */
 int ll_full_batch_standin(ll_ctx *ctx, int64_t n_w, int32_t n_nodes, const double *f_nodes,

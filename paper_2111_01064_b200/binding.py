@@ -21,7 +21,8 @@ LL_PREC_FP64, LL_PREC_FP32_ACC = 0, 1
 # every symbol include/ll.h declares (tests/test_abi.py checks header and library against this list)
 SYMBOLS = (
     "ll_create", "ll_destroy", "ll_last_error", "ll_abi_version", "ll_set_data", "ll_get_dd", "ll_standin_config",
-    "ll_full_batch", "ll_full_batch_standin", "ll_full_batch_standin_host", "ll_full_template_standin",
+    "ll_full_batch", "ll_full_batch_tf", "ll_tlm_nodes", "ll_full_batch_standin", "ll_full_batch_standin_host",
+    "ll_full_template_standin",
     "ll_template_standin", "ll_het_prepare", "ll_het_get_summary", "ll_het_batch", "ll_het_batch_standin",
     "ll_het_batch_standin_host", "ll_peak_fma", "ll_kernel_launches", "ll_last_full_stats",
     "ll_profile_enable", "ll_profile_read",
@@ -62,6 +63,8 @@ def load_library(path: Optional[str] = None):
         "ll_get_dd": (C.c_int, [vp, C.POINTER(dbl), C.POINTER(dbl), vp]),
         "ll_standin_config": (C.c_int, [vp, i32, vp, vp, vp, dbl]),
         "ll_full_batch": (C.c_int, [vp, i64, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp]),
+        "ll_full_batch_tf": (C.c_int, [vp, i64, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp]),
+        "ll_tlm_nodes": (C.c_int, [vp, i64, i32, vp, vp, dbl, vp, vp]),
         "ll_full_batch_standin": (C.c_int, [vp, i64, i32, vp, vp, vp, vp, vp, vp]),
         "ll_full_batch_standin_host": (C.c_int, [vp, i64, i32, vp, vp, vp, vp, vp, vp]),
         "ll_full_template_standin": (C.c_int, [vp, i32, vp, vp, vp, vp]),
@@ -186,6 +189,28 @@ class Context:
                                             _dev_ptr(band, "band"), _dev_ptr(logL, "logL"), _dev_ptr(d_h, "d_h"),
                                             _dev_ptr(h_h, "h_h"), _stream_ptr(stream)), "ll_full_batch")
         return logL, d_h, h_h
+
+    def full_batch_tf(self, f_nodes, amp, phase, tf_nodes, band=None, want_parts: bool = True, out=None, stream=None):
+        """frequency-dependent transfer function: tf_nodes [n_w][n_m][n_c][n_nodes][2] (Eq. 8-9)"""
+        f_nodes = _host_f64(f_nodes, "f_nodes")
+        n_w = int(amp.shape[0]) if amp is not None else 0
+        logL, d_h, h_h = out if out is not None else (self._out(n_w), self._out(n_w, want_parts), self._out(n_w, want_parts))
+        self._check(self._lib.ll_full_batch_tf(self._h, n_w, len(f_nodes), f_nodes.ctypes.data_as(C.c_void_p),
+                                               _dev_ptr(amp, "amp"), _dev_ptr(phase, "phase"),
+                                               _dev_ptr(tf_nodes, "tf_nodes"), _dev_ptr(band, "band"),
+                                               _dev_ptr(logL, "logL"), _dev_ptr(d_h, "d_h"), _dev_ptr(h_h, "h_h"),
+                                               _stream_ptr(stream)), "ll_full_batch_tf")
+        return logL, d_h, h_h
+
+    def tlm_nodes(self, f_nodes, phase, t_ref: float, stream=None):
+        """t_lm(f_j) = t_ref - (1/2pi) dphi/df at the nodes (Eq. 8); phase [n_w][n_m][n_nodes] radians"""
+        f_nodes = _host_f64(f_nodes, "f_nodes")
+        torch = _torch()
+        out = torch.empty_like(phase)
+        self._check(self._lib.ll_tlm_nodes(self._h, int(phase.shape[0]), len(f_nodes), f_nodes.ctypes.data_as(C.c_void_p),
+                                           _dev_ptr(phase, "phase"), float(t_ref), _dev_ptr(out, "t_lm"),
+                                           _stream_ptr(stream)), "ll_tlm_nodes")
+        return out
 
     def full_batch_standin(self, f_nodes, params, out=None, stream=None):
         f_nodes = _host_f64(f_nodes, "f_nodes")

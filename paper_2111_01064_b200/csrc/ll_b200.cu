@@ -277,15 +277,17 @@ FullPlan make_plan(const ll_ctx *ctx, long long n_w)
 // the whole full-grid pipeline for walkers [0, n_w) given either stand-in params or caller arrays
 int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, const double *amp, const double *phase,
              const double *tf, const double *band, double *logL, double *d_h, double *h_h, cudaStream_t st,
-             bool template_only, double *h_out)
+             bool template_only, double *h_out, const double *tf_nodes = nullptr)
 {
     const bool standin = params != nullptr;
+    const bool tfp = tf_nodes != nullptr; // frequency-dependent transfer function: 6 splines per mode
+    const int ns = tfp ? 6 : 2;
     const int n_m = ctx->n_m;
     const int P = 5 + 2 * kNC * n_m;
     const FullPlan pl = make_plan(ctx, n_w);
     const int n_wp = pl.n_wp;
     const bool nm1 = (n_m == 1);
-    const int NQ = nm1 ? 5 : 2;
+    const int NQ = (nm1 && !tfp) ? 5 : 2;
 
     CK(ctx->ilo_w.ensure(sizeof(int) * n_wp));
     CK(ctx->ihi_w.ensure(sizeof(int) * n_wp));
@@ -295,8 +297,8 @@ int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, cons
     CK(ctx->ihi_s.ensure(sizeof(int) * n_wp));
     CK(ctx->hist.ensure(sizeof(int) * 8192));
     CK(ctx->pairs.ensure(sizeof(unsigned long long)));
-    CK(ctx->Y.ensure(sizeof(double) * (size_t)n_m * 2 * n_nodes * n_wp));
-    CK(ctx->C.ensure(sizeof(double) * (size_t)(n_nodes - 1) * n_m * 8 * n_wp));
+    CK(ctx->Y.ensure(sizeof(double) * (size_t)n_m * ns * n_nodes * n_wp));
+    CK(ctx->C.ensure(sizeof(double) * (size_t)(n_nodes - 1) * n_m * ns * 4 * n_wp));
     CK(ctx->TF.ensure(sizeof(double) * (size_t)n_m * 4 * n_wp));
     if (!template_only) CK(ctx->part.ensure(sizeof(double) * (size_t)pl.n_tiles * NQ * n_wp));
 
@@ -317,6 +319,10 @@ int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, cons
         dim3 grid(ceil_div(n_wp, 128), ceil_div(n_nodes, kNodesPerThread));
         k_nodes_standin<<<grid, 128, 0, st>>>(params, P, ctx->perm.as<int>(), n_wp, n_nodes, ctx->si, ctx->nt,
                                               ctx->Y.as<double>(), ctx->TF.as<double>());
+    } else if (tfp) {
+        dim3 grid(n_wp / 32, ceil_div(n_nodes, 32), n_m * 6);
+        k_nodes_arrays_tf<<<grid, 256, 0, st>>>(amp, phase, tf_nodes, ctx->perm.as<int>(), n_wp, n_nodes, n_m,
+                                                ctx->Y.as<double>());
     } else {
         dim3 grid(n_wp / 32, ceil_div(n_nodes, 32), n_m);
         k_nodes_arrays<<<grid, 256, 0, st>>>(amp, phase, tf, ctx->perm.as<int>(), n_wp, n_nodes, n_m,
@@ -324,8 +330,8 @@ int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, cons
     }
     LAUNCHED(ctx);
     {
-        dim3 grid(ceil_div(n_wp, 128), 2 * n_m);
-        k_spline<<<grid, 128, 0, st>>>(ctx->Y.as<double>(), ctx->C.as<double>(), n_wp, n_nodes, n_m, ctx->nt);
+        dim3 grid(ceil_div(n_wp, 128), ns * n_m);
+        k_spline<<<grid, 128, 0, st>>>(ctx->Y.as<double>(), ctx->C.as<double>(), n_wp, n_nodes, n_m, ns, ctx->nt);
         LAUNCHED(ctx);
     }
     FusedArgs fa;
@@ -341,10 +347,13 @@ int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, cons
     }
     {
         dim3 grid(n_wp / pl.WB, pl.n_tiles);
-        const bool mixed = ctx->precision == LL_PREC_FP32_ACC;
+        const bool mixed = ctx->precision == LL_PREC_FP32_ACC && !tfp;
         const size_t smem = (size_t)2 * pl.CH * (mixed ? 24 : 40);
         ProfScope prof(ctx, st);
-        if (mixed) {
+        if (tfp) {
+            if (nm1) k_full_fused_tf<1><<<grid, pl.WB, smem, st>>>(fa);
+            else k_full_fused_tf<0><<<grid, pl.WB, smem, st>>>(fa);
+        } else if (mixed) {
             const FusedArgsF32 fm{ctx->g4f.as<float>(), ctx->Wf.as<double>(), ctx->scale.as<double>()};
             k_full_fused_mixed<<<grid, pl.WB, smem, st>>>(fa, fm);
         } else if (nm1) k_full_fused<1><<<grid, pl.WB, smem, st>>>(fa);
@@ -352,7 +361,7 @@ int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, cons
         LAUNCHED(ctx);
         ctx->last_n_blocks = (int)(grid.x * grid.y);
     }
-    if (nm1)
+    if (nm1 && !tfp)
         k_finalize<1><<<ceil_div(n_wp, 32), dim3(32, kFinY), 0, st>>>(ctx->part.as<double>(), ctx->TF.as<double>(), ctx->perm.as<int>(),
                                                            ctx->ilo_s.as<int>(), ctx->ihi_s.as<int>(), n_wp, pl.TB,
                                                            ctx->dd.as<double>(), logL, d_h, h_h);
@@ -726,6 +735,43 @@ int ll_full_batch(ll_ctx *ctx, int64_t n_w, int32_t n_nodes, const double *f_nod
     if (rc != LL_OK) return rc;
     if (n_w == 0) return LL_OK;
     return run_full(ctx, n_w, n_nodes, nullptr, amp, phase, tf, band, logL, d_h, h_h, st, false, nullptr);
+}
+
+int ll_full_batch_tf(ll_ctx *ctx, int64_t n_w, int32_t n_nodes, const double *f_nodes, const double *amp,
+                     const double *phase, const double *tf_nodes, const double *band, double *logL, double *d_h,
+                     double *h_h, void *stream)
+{
+    int rc = check_full_common(ctx, n_w, f_nodes, logL);
+    if (rc != LL_OK) return rc;
+    if (ctx->precision != LL_PREC_FP64) return ctx->fail(LL_ERR_UNSUPPORTED, "ll_full_batch_tf is FP64 only");
+    if (n_w > 0 && (!amp || !phase || !tf_nodes)) return ctx->fail(LL_ERR_ARG, "amp, phase or tf_nodes is NULL");
+    DeviceGuard dg(ctx->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    rc = prepare_nodes(ctx, n_nodes, f_nodes, st);
+    if (rc != LL_OK) return rc;
+    if (n_w == 0) return LL_OK;
+    return run_full(ctx, n_w, n_nodes, nullptr, amp, phase, nullptr, band, logL, d_h, h_h, st, false, nullptr, tf_nodes);
+}
+
+int ll_tlm_nodes(ll_ctx *ctx, int64_t n_w, int32_t n_nodes, const double *f_nodes, const double *phase, double t_ref,
+                 double *t_lm, void *stream)
+{
+    if (!ctx) return LL_ERR_ARG;
+    if (n_w < 0) return ctx->fail(LL_ERR_ARG, "n_w < 0");
+    if (!f_nodes) return ctx->fail(LL_ERR_ARG, "f_nodes is NULL");
+    if (n_w > 0 && (!phase || !t_lm)) return ctx->fail(LL_ERR_ARG, "phase or t_lm is NULL");
+    if (!ctx->have_data) return ctx->fail(LL_ERR_STATE, "ll_set_data has not been called (the node tables are tied to the grid)");
+    DeviceGuard dg(ctx->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc = prepare_nodes(ctx, n_nodes, f_nodes, st);
+    if (rc != LL_OK) return rc;
+    if (n_w == 0) return LL_OK;
+    const long long n_sys = n_w * ctx->n_m;
+    if (n_sys > (1LL << 30)) return ctx->fail(LL_ERR_ARG, "n_w x n_modes too large");
+    CK(ctx->Y.ensure(sizeof(double) * (size_t)n_sys * n_nodes));
+    k_tlm_nodes<<<ceil_div(n_sys, 128), 128, 0, st>>>(phase, (int)n_sys, n_nodes, t_ref, ctx->nt, ctx->Y.as<double>(), t_lm);
+    LAUNCHED(ctx);
+    return LL_OK;
 }
 
 int ll_full_batch_standin(ll_ctx *ctx, int64_t n_w, int32_t n_nodes, const double *f_nodes, const double *params,

@@ -313,6 +313,36 @@ k_nodes_arrays(const double *__restrict__ amp, const double *__restrict__ phase,
     }
 }
 
+// F1 (array entry point with a frequency-dependent transfer function, Eq. 8-9): six splines per mode,
+// sys = 6 m + s with s = 0 amplitude, 1 phase (radians -> quarter cycles), 2 + 2c Re T^c, 3 + 2c Im T^c;
+// tf_nodes is [n_w][n_m][n_c][n_nodes][2].  One 32 x 32 transpose tile per block, blockIdx.z = sys.
+__global__ void __launch_bounds__(256)
+k_nodes_arrays_tf(const double *__restrict__ amp, const double *__restrict__ phase, const double *__restrict__ tf_nodes,
+                  const int *__restrict__ perm, int n_wp, int n_nodes, int n_m, double *__restrict__ Y)
+{
+    __shared__ double tt[32][33];
+    const int sys = blockIdx.z, m = sys / 6, s = sys % 6;
+    const int p0 = blockIdx.x * 32, j0 = blockIdx.y * 32;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5; // 32 x 8
+    for (int r = ty; r < 32; r += 8) {
+        const int w = perm[p0 + r];
+        const int j = j0 + tx;
+        double v = 0.0;
+        if (w >= 0 && j < n_nodes) {
+            const size_t wm = (size_t)w * n_m + m;
+            if (s == 0) v = amp[wm * n_nodes + j];
+            else if (s == 1) v = phase[wm * n_nodes + j] * kTwoOverPi;
+            else v = tf_nodes[((wm * kNC + ((s - 2) >> 1)) * n_nodes + j) * 2 + ((s - 2) & 1)];
+        }
+        tt[r][tx] = v;
+    }
+    __syncthreads();
+    for (int r = ty; r < 32; r += 8) {
+        const int j = j0 + r;
+        if (j < n_nodes) Y[((size_t)sys * n_nodes + j) * n_wp + p0 + tx] = tt[tx][r];
+    }
+}
+
 // ---------------------------------------------------------------------------------------------------
 // F2: natural cubic spline, one system per thread, systems interleaved so every load/store is coalesced.
 // The tridiagonal matrix depends only on the (shared) nodes, so its Thomas factorisation (ta, tcp, tinv) is
@@ -324,15 +354,16 @@ k_nodes_arrays(const double *__restrict__ amp, const double *__restrict__ phase,
 // ---------------------------------------------------------------------------------------------------
 constexpr int kSplineBlk = 16;
 __global__ void __launch_bounds__(128)
-k_spline(const double *__restrict__ Y, double *__restrict__ C, int n_wp, int n_nodes, int n_m, NodeTables nt)
+k_spline(const double *__restrict__ Y, double *__restrict__ C, int n_wp, int n_nodes, int n_m, int ns, NodeTables nt)
 {
+    // ns = splines per mode: 2 (amplitude, phase) or 6 (+ Re/Im of T^A, T^E: frequency-dependent transfer function)
     const int p = blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= n_wp) return;
-    const int sys = blockIdx.y, m = sys >> 1, kind = sys & 1;
+    const int sys = blockIdx.y, m = sys / ns, kind = sys % ns;
     const size_t sw = (size_t)n_wp;
     const double *y = Y + (size_t)sys * n_nodes * sw + p;
-    double *c = C + ((size_t)m * 8 + kind * 4) * sw + p; // + j * (n_m*8*sw) + q*sw
-    const size_t cj = (size_t)n_m * 8 * sw;
+    double *c = C + ((size_t)m * ns * 4 + kind * 4) * sw + p; // + j * (n_m*ns*4*sw) + q*sw
+    const size_t cj = (size_t)n_m * ns * 4 * sw;
     const int n = n_nodes;
 
     double yprev = __ldg(y), ycur = __ldg(y + sw);
@@ -823,6 +854,171 @@ __global__ void __launch_bounds__(128, 4) k_full_fused_mixed(FusedArgs a, FusedA
     }
     double *o = a.part + ((size_t)tile * 5) * sw + p;
     o[0] = acc.sAr; o[sw] = acc.sAi; o[2 * sw] = acc.sEr; o[3 * sw] = acc.sEi; o[4 * sw] = acc.sH;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// F3 with a frequency-dependent transfer function (Eq. 8-9).  Same mapping, staging and
+// band logic as k_full_fused; per (walker, bin, mode) six cubics (amplitude, phase, Re/Im of T^A and T^E), then
+// h^c += T^c(f) A e^{-i Psi}.  Coefficient block per (interval, mode): 24 doubles, walker fastest.
+// NM1 = 1: the 24 coefficients of the current interval live in registers; 0: any n_m, coefficients re-read per
+// bin through L1 (they would not fit in registers for several modes).
+// ---------------------------------------------------------------------------------------------------
+__device__ __forceinline__ double cubic4(const double *c4, double t)
+{
+    return fma(fma(fma(c4[3], t, c4[2]), t, c4[1]), t, c4[0]);
+}
+
+template <int NM1>
+__global__ void __launch_bounds__(128, 3) k_full_fused_tf(FusedArgs a)
+{
+    extern __shared__ __align__(128) double sm[];
+    __shared__ __align__(8) uint64_t bar[2];
+    __shared__ int s_lo, s_hi;
+
+    const int tid = threadIdx.x;
+    const int p = blockIdx.x * blockDim.x + tid;
+    const int tile = blockIdx.y;
+    const int i0 = tile * a.TB;
+    const int i1 = min(i0 + a.TB, a.n_f);
+    const int lo = max(a.ilo[p], i0), hi = min(a.ihi[p], i1);
+    if (tid == 0) {
+        s_lo = INT_MAX;
+        s_hi = INT_MIN;
+        mbar_init(&bar[0], 1);
+        mbar_init(&bar[1], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    if (lo < hi) {
+        atomicMin(&s_lo, lo);
+        atomicMax(&s_hi, hi);
+    }
+    __syncthreads();
+    const int blo = s_lo, bhi = s_hi;
+    if (blo >= bhi) return;
+
+    const int CH = a.CH;
+    const int c_begin = blo / CH, c_end = (bhi + CH - 1) / CH;
+    const uint32_t stage_bytes = (uint32_t)CH * 40u;
+    auto issue = [&](int c, int st) {
+        double *dst = sm + (size_t)st * CH * 5;
+        mbar_expect_tx(&bar[st], stage_bytes);
+        tma_load_1d(dst, a.g4 + (size_t)c * CH * 4, (uint32_t)CH * 32u, &bar[st]);
+        tma_load_1d(dst + (size_t)CH * 4, a.Wd + (size_t)c * CH, (uint32_t)CH * 8u, &bar[st]);
+    };
+    if (tid == 0) issue(c_begin, 0);
+
+    const size_t sw = (size_t)a.n_wp;
+    const size_t cm = (size_t)24 * sw;          // one mode's block
+    const size_t cj = (size_t)a.n_m * cm;       // one interval's block
+    const int kbase = (int)a.k_min;
+    int j = find_interval_of_bin(a.bstart, a.n_nodes, blo);
+    int jl = -1;
+    double co[24];
+    double nxj = 0.0, s_dh = 0.0, s_hh = 0.0;
+
+    for (int c = c_begin; c < c_end; ++c) {
+        const int st = (c - c_begin) & 1;
+        const uint32_t ph = (uint32_t)((c - c_begin) >> 1) & 1u;
+        if (tid == 0 && c + 1 < c_end) issue(c + 1, st ^ 1);
+        mbar_wait(&bar[st], ph);
+        const double *sg = sm + (size_t)st * CH * 5;
+        const double *sW = sg + (size_t)CH * 4;
+        const int cb = c * CH;
+        const int ce = min(cb + CH, bhi);
+        int i = max(cb, blo);
+        while (i < ce) {
+            while (j < a.n_nodes - 2 && __ldg(a.bstart + j + 1) <= i) ++j;
+            const int seg_end = (j < a.n_nodes - 2) ? min(__ldg(a.bstart + j + 1), ce) : ce;
+            int tlo = max(i, lo), thi = min(seg_end, hi);
+            if (tlo >= thi) { tlo = INT_MAX; thi = INT_MIN; }
+            const int wlo = __reduce_min_sync(0xffffffffu, tlo);
+            const int whi = __reduce_max_sync(0xffffffffu, thi);
+            if (wlo < whi) {
+                const double *cc0 = a.C + (size_t)j * cj + p;
+                if (j != jl) {
+                    nxj = -__ldg(a.xj + j);
+                    if (NM1) {
+#pragma unroll
+                        for (int q = 0; q < 24; ++q) co[q] = cc0[(size_t)q * sw];
+                    }
+                    jl = j;
+                }
+                const double4 *sg4 = reinterpret_cast<const double4 *>(sg) - cb;
+                const double *sWc = sW - cb;
+#pragma unroll 2
+                for (int ii = wlo; ii < whi; ++ii) {
+                    const bool act = (ii >= tlo) && (ii < thi);
+                    const double t = fma((double)(kbase + ii), a.df, nxj);
+                    double hAr = 0, hAi = 0, hEr = 0, hEi = 0;
+                    const int n_m = NM1 ? 1 : a.n_m;
+                    for (int m = 0; m < n_m; ++m) {
+                        if (!NM1) {
+                            const double *cc = cc0 + (size_t)m * cm;
+#pragma unroll
+                            for (int q = 0; q < 24; ++q) co[q] = cc[(size_t)q * sw];
+                        }
+                        const double A = cubic4(co, t), y = cubic4(co + 4, t);
+                        const double tar = cubic4(co + 8, t), tai = cubic4(co + 12, t);
+                        const double ter = cubic4(co + 16, t), tei = cubic4(co + 20, t);
+                        double u, v; // h_m = u - i v
+                        amp_expi_qc(A, y, u, v);
+                        hAr = fma(tar, u, hAr); hAr = fma(tai, v, hAr);
+                        hAi = fma(tai, u, hAi); hAi = fma(-tar, v, hAi);
+                        hEr = fma(ter, u, hEr); hEr = fma(tei, v, hEr);
+                        hEi = fma(tei, u, hEi); hEi = fma(-ter, v, hEi);
+                    }
+                    if (act) {
+                        const double4 g = sg4[ii];
+                        const double w = sWc[ii];
+                        s_dh = fma(g.x, hAr, s_dh); s_dh = fma(-g.y, hAi, s_dh);
+                        s_dh = fma(g.z, hEr, s_dh); s_dh = fma(-g.w, hEi, s_dh);
+                        s_hh = fma(w, fma(hAr, hAr, hAi * hAi) + fma(hEr, hEr, hEi * hEi), s_hh);
+                    }
+                }
+            }
+            i = seg_end;
+        }
+        __syncthreads();
+    }
+    double *o = a.part + ((size_t)tile * 2) * sw + p;
+    o[0] = s_dh; o[sw] = s_hh;
+}
+
+// Eq. 8 utility: t_lm(f_j) = t_ref - (1/2pi) dphi/df at the nodes, dphi/df from the natural spline of the caller's
+// node phases [n_sys][n_nodes] (radians).  One thread per system (off the hot path: the caller needs t_lm to build
+// T(f, t_lm(f)) at the nodes).  scratch [n_nodes][n_sys] holds the forward-sweep values.
+__global__ void __launch_bounds__(128)
+k_tlm_nodes(const double *__restrict__ phase, int n_sys, int n_nodes, double t_ref, NodeTables nt,
+            double *__restrict__ scratch, double *__restrict__ t_lm)
+{
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= n_sys) return;
+    const double *y = phase + (size_t)s * n_nodes;
+    double *out = t_lm + (size_t)s * n_nodes;
+    const int n = n_nodes;
+    double ycur = y[1], sprev = (y[1] - y[0]) * __ldg(nt.invh), dpp = 0.0;
+    for (int j = 1; j <= n - 2; ++j) {
+        const double ynext = y[j + 1];
+        const double sl = (ynext - ycur) * __ldg(nt.invh + j);
+        const double dp = ((sl - sprev) - __ldg(nt.ta + j) * dpp) * __ldg(nt.tinv + j);
+        scratch[(size_t)j * n_sys + s] = dp;
+        dpp = dp;
+        sprev = sl;
+        ycur = ynext;
+    }
+    const double inv2pi = 0.5 / kPi;
+    double Mn = 0.0, y1 = y[n - 1];
+    for (int j = n - 2; j >= 0; --j) {
+        const double y0 = y[j];
+        const double Mj = (j >= 1) ? fma(-__ldg(nt.tcp + j), Mn, scratch[(size_t)j * n_sys + s]) : 0.0;
+        const double h = __ldg(nt.hj + j), ih = __ldg(nt.invh + j);
+        const double sl = (y1 - y0) * ih;
+        if (j == n - 2) out[n - 1] = t_ref - (sl + h * (Mj + 2.0 * Mn) * kSixth) * inv2pi; // right end of the last interval
+        out[j] = t_ref - (sl - h * (2.0 * Mj + Mn) * kSixth) * inv2pi;
+        Mn = Mj;
+        y1 = y0;
+    }
 }
 
 // F4: reduce the per-tile partials in a fixed order, apply T^c (single mode), form log L        (Eq. 2)

@@ -202,6 +202,72 @@ def test_cfg2_full_size_sampled(orc, torch_cuda):
     ctx.destroy()
 
 
+# ------------------------------------------- full grid, frequency-dependent transfer function (Eq. 8-9)
+def _smooth_tf_nodes(rng, n_w, n_m, f_nodes, n_c=2):
+    """smooth complex T^c_m at the nodes (not a physical response: its formula is in the paper's ref. [44])"""
+    x = np.log(f_nodes / f_nodes[0]) / np.log(f_nodes[-1] / f_nodes[0])
+    a = rng.uniform(-1.0, 1.0, (n_w, n_m, n_c, 6, 1))
+    mod = 1.0 + 0.3 * a[..., 0, :] * x + 0.2 * a[..., 1, :] * np.sin(2 * x + a[..., 2, :])
+    ang = 3.0 * a[..., 3, :] + 2.0 * a[..., 4, :] * x
+    return np.ascontiguousarray(np.stack([mod * np.cos(ang), mod * np.sin(ang)], axis=-1))
+
+
+@pytest.mark.parametrize("n_m,banded,n_w", [(1, False, 40), (1, True, 97), (3, True, 50)])
+def test_full_tf_entry_point(orc, torch_cuda, n_m, banded, n_w):
+    """ll_full_batch_tf against the oracle: several walker blocks and tiles, ragged bands, 1 and 3 modes."""
+    rng = np.random.default_rng(900 + n_m + n_w)
+    grid = wlm.make_grid(2.0 ** 15)
+    f = grid.freqs()
+    f_nodes = wlm.geomspace_exact(wlm.F_LO, wlm.F_HI, 96)
+    amp, ph = rand_smooth_nodes(rng, n_w, n_m, f_nodes)
+    amp *= 1e19 * 0.05                                     # O(1) templates against O(1) data
+    tfn = _smooth_tf_nodes(rng, n_w, n_m, f_nodes)
+    W = rng.uniform(0.5, 2.0, grid.n_f)
+    d = rng.standard_normal((2, grid.n_f, 2))
+    band = None
+    if banded:
+        lo = rng.uniform(f[0], f[grid.n_f // 3], n_w)
+        hi = rng.uniform(f[grid.n_f // 2], f[-1], n_w)
+        band = np.stack([lo, hi], axis=1)
+        band[0] = [f[-1] * 2, f[-1] * 3]                   # misses the grid
+        band[1] = [f[5], f[5]]                             # a single bin
+    ref = orc.full_batch_tf(f_nodes, amp, ph, tfn, band, grid.k_min, grid.df, d, W)
+    from paper_2111_01064_b200 import binding
+    ctx = binding.Context(n_modes=n_m)
+    ctx.set_data(grid.n_f, grid.k_min, grid.df, dev(torch_cuda, d), dev(torch_cuda, W))
+    got = ctx.full_batch_tf(f_nodes, dev(torch_cuda, amp), dev(torch_cuda, ph), dev(torch_cuda, tfn),
+                            None if band is None else dev(torch_cuda, band))
+    check_triplet(got, ref, f"tf n_m={n_m}")
+    again = ctx.full_batch_tf(f_nodes, dev(torch_cuda, amp), dev(torch_cuda, ph), dev(torch_cuda, tfn),
+                              None if band is None else dev(torch_cuda, band))
+    assert all(torch_cuda.equal(a, b) for a, b in zip(got, again))
+    # a transfer function that is constant over the nodes must give what ll_full_batch gives (same library)
+    tf_const = np.ascontiguousarray(tfn[:, :, :, 0, :])
+    tfn_c = np.ascontiguousarray(np.repeat(tf_const[:, :, :, None, :], len(f_nodes), axis=3))
+    a = ctx.full_batch(f_nodes, dev(torch_cuda, amp), dev(torch_cuda, ph), dev(torch_cuda, tf_const),
+                       None if band is None else dev(torch_cuda, band))
+    b = ctx.full_batch_tf(f_nodes, dev(torch_cuda, amp), dev(torch_cuda, ph), dev(torch_cuda, tfn_c),
+                          None if band is None else dev(torch_cuda, band))
+    check_triplet(b, {k: v.cpu().numpy() for k, v in zip(("logL", "d_h", "h_h"), a)}, "tf const vs constant-T path")
+    ctx.destroy()
+
+
+def test_tlm_nodes_parity(orc, torch_cuda):
+    """Eq. 8 utility against the oracle (spline derivative at the nodes)."""
+    rng = np.random.default_rng(77)
+    wl = wlm.make_workload(0)
+    d, run = oracle_setup_full(orc, wl)
+    ctx = make_ctx(wl)
+    g = wl.grid
+    ctx.set_data(g.n_f, g.k_min, g.df, dev(torch_cuda, d), dev(torch_cuda, wl.W))
+    f = g.freqs()
+    _, ph, _, _ = orc.standin_nodes(wl.params[:37], wl.modes_m, wl.c_lm, wl.kappa, wl.f_nodes, f[0], f[-1])
+    ref = orc.tlm_nodes(wl.f_nodes, ph, 1000.0)
+    got = ctx.tlm_nodes(wl.f_nodes, dev(torch_cuda, ph), 1000.0).cpu().numpy()
+    np.testing.assert_allclose(got, ref, rtol=1e-9, atol=1e-9 * np.abs(ref).max())
+    ctx.destroy()
+
+
 # ------------------------------------------------------------------ full grid, FP32-accumulate variant
 MIXED_ABS_TOL = 1e-3  # BASELINE.json north_star: "<= 1e-3 absolute for any mixed-precision variant"
 
