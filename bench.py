@@ -422,6 +422,29 @@ def main():
             r["ctx"].destroy()
             del r
             torch.cuda.empty_cache()
+        if args.workload == 2 and args.precision == "fp64":
+            # ---- frequency-dependent transfer function (six splines per mode) at config-2
+            # size through the array entry point; node arrays from ll_standin_nodes, a smooth T(f) at the nodes
+            from paper_2111_01064_b200 import synth
+            wl2 = rank_workload(2, 0)
+            c2 = synth.make_context(wl2)
+            b2 = synth.setup(c2, wl2)
+            amp, ph = c2.standin_nodes(wl2.f_nodes, b2["params"])
+            tfn = synth.smooth_tf_nodes(b2["params"], wl2.f_nodes)
+            o2 = tuple(torch.empty(wl2.n_w, dtype=torch.float64, device=amp.device) for _ in range(3))
+            fn2 = lambda: c2.full_batch_tf(wl2.f_nodes, amp, ph, tfn, out=o2)
+            fn2()
+            c2.profile_enable(True)
+            ms2 = time_steps(torch, fn2, max(args.steps // 2, 3), 3)
+            kms, kn = c2.profile_read()
+            c2.profile_enable(False)
+            nst = max(args.steps // 2, 3)
+            per["cfg2_tf"] = {"evals_per_s": wl2.n_w / (ms2 / nst * 1e-3), "ms_per_batch": ms2 / nst, "n_walkers": wl2.n_w,
+                              "kernel": "k_full_fused_tf", "kernel_ms": kms / max(kn, 1),
+                              "entry": "ll_full_batch_tf (amp, phase, T at 1024 nodes as device arrays; whole grid band)"}
+            c2.destroy()
+            del amp, ph, tfn, b2
+            torch.cuda.empty_cache()
         line["per_config"] = per
         # ---- the oracle on this box's cores, bounded sample of the same workload
         import oracle as orc

@@ -21,7 +21,7 @@ LL_PREC_FP64, LL_PREC_FP32_ACC = 0, 1
 # every symbol include/ll.h declares (tests/test_abi.py checks header and library against this list)
 SYMBOLS = (
     "ll_create", "ll_destroy", "ll_last_error", "ll_abi_version", "ll_set_data", "ll_get_dd", "ll_standin_config",
-    "ll_full_batch", "ll_full_batch_tf", "ll_tlm_nodes", "ll_full_batch_standin", "ll_full_batch_standin_host",
+    "ll_full_batch", "ll_full_batch_tf", "ll_tlm_nodes", "ll_standin_nodes", "ll_full_batch_standin", "ll_full_batch_standin_host",
     "ll_full_template_standin",
     "ll_template_standin", "ll_het_prepare", "ll_het_get_summary", "ll_het_batch", "ll_het_batch_standin",
     "ll_het_batch_standin_host", "ll_peak_fma", "ll_kernel_launches", "ll_last_full_stats",
@@ -65,6 +65,7 @@ def load_library(path: Optional[str] = None):
         "ll_full_batch": (C.c_int, [vp, i64, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp]),
         "ll_full_batch_tf": (C.c_int, [vp, i64, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp]),
         "ll_tlm_nodes": (C.c_int, [vp, i64, i32, vp, vp, dbl, vp, vp]),
+        "ll_standin_nodes": (C.c_int, [vp, i64, i32, vp, vp, vp, vp, vp]),
         "ll_full_batch_standin": (C.c_int, [vp, i64, i32, vp, vp, vp, vp, vp, vp]),
         "ll_full_batch_standin_host": (C.c_int, [vp, i64, i32, vp, vp, vp, vp, vp, vp]),
         "ll_full_template_standin": (C.c_int, [vp, i32, vp, vp, vp, vp]),
@@ -201,6 +202,18 @@ class Context:
                                                _dev_ptr(logL, "logL"), _dev_ptr(d_h, "d_h"), _dev_ptr(h_h, "h_h"),
                                                _stream_ptr(stream)), "ll_full_batch_tf")
         return logL, d_h, h_h
+
+    def standin_nodes(self, f_nodes, params, stream=None):
+        """stand-in node arrays in the caller layout: amp, phase [n_w][n_m][n_nodes] (radians)"""
+        f_nodes = _host_f64(f_nodes, "f_nodes")
+        torch = _torch()
+        n_w = int(params.shape[0])
+        amp = torch.empty((n_w, self.n_modes, len(f_nodes)), dtype=torch.float64, device=params.device)
+        phase = torch.empty_like(amp)
+        self._check(self._lib.ll_standin_nodes(self._h, n_w, len(f_nodes), f_nodes.ctypes.data_as(C.c_void_p),
+                                               _dev_ptr(params, "params"), _dev_ptr(amp, "amp"), _dev_ptr(phase, "phase"),
+                                               _stream_ptr(stream)), "ll_standin_nodes")
+        return amp, phase
 
     def tlm_nodes(self, f_nodes, phase, t_ref: float, stream=None):
         """t_lm(f_j) = t_ref - (1/2pi) dphi/df at the nodes (Eq. 8); phase [n_w][n_m][n_nodes] radians"""

@@ -753,6 +753,25 @@ int ll_full_batch_tf(ll_ctx *ctx, int64_t n_w, int32_t n_nodes, const double *f_
     return run_full(ctx, n_w, n_nodes, nullptr, amp, phase, nullptr, band, logL, d_h, h_h, st, false, nullptr, tf_nodes);
 }
 
+int ll_standin_nodes(ll_ctx *ctx, int64_t n_w, int32_t n_nodes, const double *f_nodes, const double *params,
+                     double *amp, double *phase, void *stream)
+{
+    if (!ctx) return LL_ERR_ARG;
+    if (n_w < 0 || n_w > (1LL << 30)) return ctx->fail(LL_ERR_ARG, "n_w out of range");
+    if (!f_nodes) return ctx->fail(LL_ERR_ARG, "f_nodes is NULL");
+    if (n_w > 0 && (!params || !amp || !phase)) return ctx->fail(LL_ERR_ARG, "params, amp or phase is NULL");
+    if (!ctx->have_standin) return ctx->fail(LL_ERR_STATE, "ll_standin_config has not been called");
+    if (!ctx->have_data) return ctx->fail(LL_ERR_STATE, "ll_set_data has not been called (the node tables are tied to the grid)");
+    DeviceGuard dg(ctx->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc = prepare_nodes(ctx, n_nodes, f_nodes, st);
+    if (rc != LL_OK) return rc;
+    if (n_w == 0) return LL_OK;
+    k_standin_nodes_out<<<(unsigned)n_w, 128, 0, st>>>(params, 5 + 2 * kNC * ctx->n_m, n_nodes, ctx->si, ctx->nt, amp, phase);
+    LAUNCHED(ctx);
+    return LL_OK;
+}
+
 int ll_tlm_nodes(ll_ctx *ctx, int64_t n_w, int32_t n_nodes, const double *f_nodes, const double *phase, double t_ref,
                  double *t_lm, void *stream)
 {

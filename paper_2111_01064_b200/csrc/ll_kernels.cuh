@@ -275,6 +275,28 @@ k_nodes_standin(const double *__restrict__ params, int P, const int *__restrict_
     }
 }
 
+// F1 utility: the stand-in's node arrays in the CALLER layout amp, phase [n_w][n_m][n_nodes] (phase in radians),
+// e.g. to feed ll_full_batch / ll_full_batch_tf or ll_tlm_nodes.  One block per walker.
+__global__ void __launch_bounds__(128)
+k_standin_nodes_out(const double *__restrict__ params, int P, int n_nodes, StandinInfo si, NodeTables nt,
+                    double *__restrict__ amp, double *__restrict__ phase)
+{
+    const size_t w = blockIdx.x;
+    const WalkerConst c = standin_consts(params + w * P);
+    const double inv_kappa = 1.0 / si.kappa;
+    for (int m = 0; m < si.n_m; ++m) {
+        const double mh_pi = (double)si.mode_m[m] / kPi;
+        const double phq = mh_pi * (c.phi + 0.25 * kPi);
+        const double Kq = mh_pi * c.K;
+        for (int j = threadIdx.x; j < n_nodes; j += blockDim.x) {
+            const size_t t = (size_t)m * n_nodes + j;
+            const size_t o = (w * si.n_m + m) * n_nodes + j;
+            amp[o] = nt.cfp[t] * c.invD * taper(nt.f2m[t] * c.inv_fisco, si.kappa, inv_kappa);
+            phase[o] = fma(nt.f4[j], c.tc, fma(Kq, nt.fm53[t], -phq)) * kPio2_1; // quarter cycles -> radians
+        }
+    }
+}
+
 // F1 (array entry point): transpose caller arrays [n_w][n_m][n_nodes] into Y; phase radians -> quarter cycles
 __global__ void __launch_bounds__(256)
 k_nodes_arrays(const double *__restrict__ amp, const double *__restrict__ phase, const double *__restrict__ tf,

@@ -68,3 +68,19 @@ def setup_het(ctx: Context, wl: wlm.Workload):
 
 def setup(ctx: Context, wl: wlm.Workload):
     return setup_full(ctx, wl) if wl.path == "full" else setup_het(ctx, wl)
+
+
+def smooth_tf_nodes(params, f_nodes, n_m: int = 1, n_c: int = 2):
+    """A smooth frequency-dependent transfer function at the nodes for timing / demonstration runs of
+    ll_full_batch_tf: T^c_m(f_j) = T^c_m(params) * (1 + 0.2 x_j) e^{2 i x_j}, x = log(f/f_0)/log(f_last/f_0).
+    (The physical response's formula is in the paper's ref. [44], not in PAPER.md; any smooth T exercises the
+    same six-spline path.)  Returns a device tensor [n_w][n_m][n_c][n_nodes][2]."""
+    dev = params.device
+    f = torch.as_tensor(np.asarray(f_nodes, dtype=np.float64), device=dev)
+    x = torch.log(f / f[0]) / math.log(float(f_nodes[-1]) / float(f_nodes[0]))
+    mod = (1.0 + 0.2 * x)
+    cr, ci = mod * torch.cos(2.0 * x), mod * torch.sin(2.0 * x)
+    t = params[:, 5:5 + 2 * n_c * n_m].reshape(-1, n_m, n_c, 1, 2)
+    tr, ti = t[..., 0], t[..., 1]
+    out = torch.stack([tr * cr - ti * ci, tr * ci + ti * cr], dim=-1)
+    return out.contiguous()
