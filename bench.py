@@ -44,7 +44,7 @@ SLOTS_HET = {1: 73.0, 6: 252.0}
 INSTR_FULL_FP32ACC = 45.0
 ISSUE_LANES_PER_CLK_PER_SM = 128.0
 # DRAM traffic per launch of the dominant kernel, from the committed `ncu --set full` captures (profiles/)
-NCU_TRAFFIC_BYTES = {("k_full_fused", 2): 803.1e6 + 39.2e6, ("k_full_fused_mixed", 2): 787.9e6 + 37.3e6}
+NCU_TRAFFIC_BYTES = {("k_full_fused", 2): 804.4e6 + 41.2e6, ("k_full_fused_mixed", 2): 786.4e6 + 37.0e6}
 DFMA_PER_CLK_PER_SM = 64.0
 
 
