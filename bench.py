@@ -42,6 +42,9 @@ SLOTS_HET = {1: 73.0, 6: 252.0}
 # reduce 3, scale 1, W A^2 2) + 3 conversions + 20 binary32 (sincos 10, A e^{-i Psi} 2, MACs 8) + 6 quadrant
 # + 2 shared loads + 1 loop = 45
 INSTR_FULL_FP32ACC = 45.0
+# frequency-dependent transfer function (Eq. 8-9): t 1, six cubics 18, reduce 3, sincos 18, A e^{-i Psi} 2, T^c h 8,
+# Re g h 4, W |h|^2 5 = 59
+SLOTS_FULL_TF = 59.0
 ISSUE_LANES_PER_CLK_PER_SM = 128.0
 # DRAM traffic per launch of the dominant kernel, from the committed `ncu --set full` captures (profiles/)
 NCU_TRAFFIC_BYTES = {("k_full_fused", 2): 804.4e6 + 41.2e6, ("k_full_fused_mixed", 2): 786.4e6 + 37.0e6}
@@ -429,19 +432,22 @@ def main():
             wl2 = rank_workload(2, 0)
             c2 = synth.make_context(wl2)
             b2 = synth.setup(c2, wl2)
-            amp, ph = c2.standin_nodes(wl2.f_nodes, b2["params"])
+            amp, ph, bnd = c2.standin_nodes(wl2.f_nodes, b2["params"], with_band=True)
             tfn = synth.smooth_tf_nodes(b2["params"], wl2.f_nodes)
             o2 = tuple(torch.empty(wl2.n_w, dtype=torch.float64, device=amp.device) for _ in range(3))
-            fn2 = lambda: c2.full_batch_tf(wl2.f_nodes, amp, ph, tfn, out=o2)
+            fn2 = lambda: c2.full_batch_tf(wl2.f_nodes, amp, ph, tfn, band=bnd, out=o2)
             fn2()
             c2.profile_enable(True)
             ms2 = time_steps(torch, fn2, max(args.steps // 2, 3), 3)
             kms, kn = c2.profile_read()
             c2.profile_enable(False)
             nst = max(args.steps // 2, 3)
+            pairs2 = c2.last_full_stats()[0]
             per["cfg2_tf"] = {"evals_per_s": wl2.n_w / (ms2 / nst * 1e-3), "ms_per_batch": ms2 / nst, "n_walkers": wl2.n_w,
-                              "kernel": "k_full_fused_tf", "kernel_ms": kms / max(kn, 1),
-                              "entry": "ll_full_batch_tf (amp, phase, T at 1024 nodes as device arrays; whole grid band)"}
+                              "kernel": "k_full_fused_tf", "kernel_ms": kms / max(kn, 1), "active_pairs": pairs2,
+                              "algorithmic_slots_per_pair": SLOTS_FULL_TF,
+                              "frac": pairs2 * SLOTS_FULL_TF / (kms / max(kn, 1) * 1e-3) / peak_slots,
+                              "entry": "ll_full_batch_tf (amp, phase, T at 1024 nodes as device arrays; the walkers' own bands)"}
             c2.destroy()
             del amp, ph, tfn, b2
             torch.cuda.empty_cache()

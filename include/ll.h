@@ -109,10 +109,11 @@ int ll_full_batch_tf(ll_ctx *ctx, int64_t n_w, int32_t n_nodes, const double *f_
                      double *h_h, void *stream);
 
 /* F1 utility — the stand-in's node arrays in the caller layout (what ll_full_batch_standin builds internally):
- *   params : DEV [n_w][P];  amp, phase : DEV out [n_w][n_m][n_nodes] (phase in radians).
+ *   params : DEV [n_w][P];  amp, phase : DEV out [n_w][n_m][n_nodes] (phase in radians);
+ *   band   : DEV out [n_w][2] = (f_0, min(f_last, (1+kappa) f_ISCO max_m(m/2))) (reading R10), or NULL.
  * Needs ll_standin_config and ll_set_data first.                                                            */
 int ll_standin_nodes(ll_ctx *ctx, int64_t n_w, int32_t n_nodes, const double *f_nodes, const double *params,
-                     double *amp, double *phase, void *stream);
+                     double *amp, double *phase, double *band, void *stream);
 
 /* Eq. 8 utility — t_lm(f_j) = t_ref - (1/2pi) dphi_lm/df at the nodes, dphi/df being the first derivative of the
  * natural cubic spline of the node phases (what a caller needs to evaluate T(f, t_lm(f)) at the nodes).

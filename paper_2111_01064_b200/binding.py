@@ -65,7 +65,7 @@ def load_library(path: Optional[str] = None):
         "ll_full_batch": (C.c_int, [vp, i64, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp]),
         "ll_full_batch_tf": (C.c_int, [vp, i64, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp]),
         "ll_tlm_nodes": (C.c_int, [vp, i64, i32, vp, vp, dbl, vp, vp]),
-        "ll_standin_nodes": (C.c_int, [vp, i64, i32, vp, vp, vp, vp, vp]),
+        "ll_standin_nodes": (C.c_int, [vp, i64, i32, vp, vp, vp, vp, vp, vp]),
         "ll_full_batch_standin": (C.c_int, [vp, i64, i32, vp, vp, vp, vp, vp, vp]),
         "ll_full_batch_standin_host": (C.c_int, [vp, i64, i32, vp, vp, vp, vp, vp, vp]),
         "ll_full_template_standin": (C.c_int, [vp, i32, vp, vp, vp, vp]),
@@ -203,17 +203,20 @@ class Context:
                                                _stream_ptr(stream)), "ll_full_batch_tf")
         return logL, d_h, h_h
 
-    def standin_nodes(self, f_nodes, params, stream=None):
-        """stand-in node arrays in the caller layout: amp, phase [n_w][n_m][n_nodes] (radians)"""
+    def standin_nodes(self, f_nodes, params, with_band=False, stream=None):
+        """stand-in node arrays in the caller layout: amp, phase [n_w][n_m][n_nodes] (radians); with_band: also the
+        walkers' bands [n_w][2] (reading R10)"""
         f_nodes = _host_f64(f_nodes, "f_nodes")
         torch = _torch()
         n_w = int(params.shape[0])
         amp = torch.empty((n_w, self.n_modes, len(f_nodes)), dtype=torch.float64, device=params.device)
         phase = torch.empty_like(amp)
+        band = torch.empty((n_w, 2), dtype=torch.float64, device=params.device) if with_band else None
         self._check(self._lib.ll_standin_nodes(self._h, n_w, len(f_nodes), f_nodes.ctypes.data_as(C.c_void_p),
                                                _dev_ptr(params, "params"), _dev_ptr(amp, "amp"), _dev_ptr(phase, "phase"),
+                                               _dev_ptr(band, "band") if with_band else None,
                                                _stream_ptr(stream)), "ll_standin_nodes")
-        return amp, phase
+        return (amp, phase, band) if with_band else (amp, phase)
 
     def tlm_nodes(self, f_nodes, phase, t_ref: float, stream=None):
         """t_lm(f_j) = t_ref - (1/2pi) dphi/df at the nodes (Eq. 8); phase [n_w][n_m][n_nodes] radians"""

@@ -754,7 +754,7 @@ int ll_full_batch_tf(ll_ctx *ctx, int64_t n_w, int32_t n_nodes, const double *f_
 }
 
 int ll_standin_nodes(ll_ctx *ctx, int64_t n_w, int32_t n_nodes, const double *f_nodes, const double *params,
-                     double *amp, double *phase, void *stream)
+                     double *amp, double *phase, double *band, void *stream)
 {
     if (!ctx) return LL_ERR_ARG;
     if (n_w < 0 || n_w > (1LL << 30)) return ctx->fail(LL_ERR_ARG, "n_w out of range");
@@ -767,7 +767,8 @@ int ll_standin_nodes(ll_ctx *ctx, int64_t n_w, int32_t n_nodes, const double *f_
     int rc = prepare_nodes(ctx, n_nodes, f_nodes, st);
     if (rc != LL_OK) return rc;
     if (n_w == 0) return LL_OK;
-    k_standin_nodes_out<<<(unsigned)n_w, 128, 0, st>>>(params, 5 + 2 * kNC * ctx->n_m, n_nodes, ctx->si, ctx->nt, amp, phase);
+    k_standin_nodes_out<<<(unsigned)n_w, 128, 0, st>>>(params, 5 + 2 * kNC * ctx->n_m, n_nodes, ctx->si, ctx->nt,
+                                                        GridInfo{ctx->k_min, ctx->n_f, ctx->df}, amp, phase, band);
     LAUNCHED(ctx);
     return LL_OK;
 }

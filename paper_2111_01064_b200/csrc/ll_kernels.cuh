@@ -278,11 +278,19 @@ k_nodes_standin(const double *__restrict__ params, int P, const int *__restrict_
 // F1 utility: the stand-in's node arrays in the CALLER layout amp, phase [n_w][n_m][n_nodes] (phase in radians),
 // e.g. to feed ll_full_batch / ll_full_batch_tf or ll_tlm_nodes.  One block per walker.
 __global__ void __launch_bounds__(128)
-k_standin_nodes_out(const double *__restrict__ params, int P, int n_nodes, StandinInfo si, NodeTables nt,
-                    double *__restrict__ amp, double *__restrict__ phase)
+k_standin_nodes_out(const double *__restrict__ params, int P, int n_nodes, StandinInfo si, NodeTables nt, GridInfo g,
+                    double *__restrict__ amp, double *__restrict__ phase, double *__restrict__ band)
 {
     const size_t w = blockIdx.x;
     const WalkerConst c = standin_consts(params + w * P);
+    if (band && threadIdx.x == 0) { // the walker's band exactly as k_band_prep takes it (reading R10)
+        double Mtot, eta, fi;
+        standin_masses(params[w * P], params[w * P + 1], Mtot, eta, fi);
+        const double top = (1.0 + si.kappa) * fi * (0.5 * (double)si.m_max);
+        const double f_last = bin_freq(g.k_min, g.n_f - 1, g.df);
+        band[2 * w] = bin_freq(g.k_min, 0, g.df);
+        band[2 * w + 1] = (top < f_last) ? top : f_last;
+    }
     const double inv_kappa = 1.0 / si.kappa;
     for (int m = 0; m < si.n_m; ++m) {
         const double mh_pi = (double)si.mode_m[m] / kPi;

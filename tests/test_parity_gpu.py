@@ -261,9 +261,11 @@ def test_tlm_nodes_parity(orc, torch_cuda):
     g = wl.grid
     ctx.set_data(g.n_f, g.k_min, g.df, dev(torch_cuda, d), dev(torch_cuda, wl.W))
     f = g.freqs()
-    am, ph, _, _ = orc.standin_nodes(wl.params[:37], wl.modes_m, wl.c_lm, wl.kappa, wl.f_nodes, f[0], f[-1])
+    am, ph, _, o_bd = orc.standin_nodes(wl.params[:37], wl.modes_m, wl.c_lm, wl.kappa, wl.f_nodes, f[0], f[-1])
     # ll_standin_nodes: the library's own node arrays in the caller layout against the oracle's
-    g_am, g_ph = (x.cpu().numpy() for x in ctx.standin_nodes(wl.f_nodes, dev(torch_cuda, wl.params[:37])))
+    g_am, g_ph, g_bd = (x.cpu().numpy() for x in ctx.standin_nodes(wl.f_nodes, dev(torch_cuda, wl.params[:37]),
+                                                                   with_band=True))
+    np.testing.assert_allclose(g_bd, o_bd, rtol=1e-14)
     # absolute term: the taper's s = (1+kappa-x)/kappa cancels near its zero, where the amplitude itself is ~1e-12 of its peak
     np.testing.assert_allclose(g_am, am, rtol=1e-13, atol=1e-15 * am.max())
     np.testing.assert_allclose(g_ph, ph, rtol=1e-14, atol=1e-9)
