@@ -647,3 +647,59 @@ def test_tlm_nodes_matches_scipy_derivative_and_chirp_time(orc):
     tau = 5.0 / 256.0 * p[0] ** (-5.0 / 3.0) * (math.pi * fn) ** (-8.0 / 3.0)
     sl = slice(20, 236)
     np.testing.assert_allclose(tl[sl], -(p[2] - tau[sl]), rtol=2e-6, atol=0.1)   # seconds; values 1e3 .. 4e6
+
+
+# --------------------------------------------------------------------------- reference update and audit
+def test_reference_update_picks_best_and_places_edges(orc, het_small):
+    """best walker = plain scan (ties -> lowest index, NaN/inf never win); edges = numpy geomspace with exact ends,
+    stopping at min(f_last, f_ISCO) with f_ISCO from the textbook formula (reading R12)."""
+    from oracle import reference_update as ru
+    assert ru.best_walker([1.0, 3.0, 3.0, -1.0]) == 1
+    assert ru.best_walker([np.nan, -5.0, np.inf, -7.0]) == 1
+    assert ru.best_walker([np.nan, np.inf]) == -1
+    wl, f, d, h0, h0e, s, _ = het_small
+    p = wl.params[3]
+    e = ru.reference_edges(p, f[0], f[-1], 25)
+    eta = p[1] / (1 + p[1]) ** 2
+    f_isco = 6.0 ** -1.5 / (math.pi * p[0] * eta ** -0.6)
+    assert e[0] == f[0] and e[-1] == pytest.approx(min(f[-1], f_isco), rel=1e-14)
+    np.testing.assert_allclose(np.diff(np.log(e)), np.log(e[-1] / e[0]) / 24, rtol=1e-10)
+    with pytest.raises(ValueError):
+        ru.reference_edges(np.r_[1e3, 1.0, p[2:]], f[0], f[-1], 25)      # f_ISCO ~ 3e-6 Hz, below the grid
+
+
+def test_audit_is_zero_at_d_equals_h_and_matches_numpy(orc, het_small):
+    """Noiseless d = h: direct residual form bitwise 0, three-term form |.| <= 1e-6; on noisy data the
+    three-term audit equals numpy complex arithmetic on the masked band."""
+    from oracle import reference_update as ru
+    wl, f, d, h0, h0e, s, _ = het_small
+    g = wl.grid
+    a = ru.audit(wl.inj[None], wl.modes_m, wl.c_lm, wl.kappa, g.k_min, g.df, g.n_f, h0, wl.W, wl.f_edges)
+    assert a["logL_direct"][0] == 0.0
+    assert abs(a["logL"][0]) <= 1e-6
+    b = ru.audit(wl.params[:3], wl.modes_m, wl.c_lm, wl.kappa, g.k_min, g.df, g.n_f, d, wl.W, wl.f_edges)
+    m = _band_mask(f, wl.f_edges)
+    for w in range(3):
+        hc = _c(orc.standin_direct(wl.params[w], wl.modes_m, wl.c_lm, wl.kappa, f, f[0], f[-1]))[:, m]
+        res = _c(d)[:, m] - hc
+        assert b["logL"][w] == pytest.approx(-0.5 * (wl.W[m] * np.abs(res) ** 2).sum(), rel=1e-9)
+        assert b["logL_direct"][w] == pytest.approx(b["logL"][w], rel=1e-9)
+        assert b["h_h"][w] == pytest.approx((wl.W[m] * np.abs(hc) ** 2).sum(), rel=1e-12)
+
+
+def test_reference_update_then_het_equals_audit_at_new_reference(orc, het_small):
+    """After the update the best walker IS the reference: r = 1, so its heterodyned log L equals its brute-force
+    log L over the new band to rounding (north_star invariant), and nearby walkers agree closely."""
+    from oracle import reference_update as ru
+    wl, f, d, h0, h0e, s, _ = het_small
+    g = wl.grid
+    old = orc.het_batch_standin(wl.modes_m, wl.c_lm, wl.kappa, wl.params, wl.f_edges, h0e, s)
+    up = ru.reference_update(wl.params, old["logL"], wl.modes_m, wl.c_lm, wl.kappa, g.k_min, g.df, g.n_f, d, wl.W, 25)
+    assert up["best"] == int(np.argmax(old["logL"]))
+    het = orc.het_batch_standin(wl.modes_m, wl.c_lm, wl.kappa, wl.params, up["f_edges"], up["h0_edges"], up["summ"])
+    aud = ru.audit(wl.params, wl.modes_m, wl.c_lm, wl.kappa, g.k_min, g.df, g.n_f, d, wl.W, up["f_edges"])
+    b = up["best"]
+    assert het["logL"][b] == pytest.approx(aud["logL"][b], rel=1e-10, abs=1e-8)
+    assert het["h_h"][b] == pytest.approx(aud["h_h"][b], rel=1e-12)
+    # the method's own accuracy with 24 bins on a 1e-3 ball (cf. test_het_tracks_dense_likelihood_near_reference)
+    assert np.all(np.abs(het["logL"] - aud["logL"]) < 0.01 * np.abs(aud["logL"]) + 1e-6)
