@@ -151,6 +151,25 @@ int ll_template_standin(ll_ctx *ctx, const double *params_row, int64_t n_freq, c
 int ll_het_prepare(ll_ctx *ctx, int32_t n_edges, const double *f_edges, const double *h0_dense,
                    const double *h0_edges, void *stream);
 
+/* H0 inside the sampling loop — "The reference template is updated every 5000 iterations of the sampler by
+ * replacing it with the highest Likelihood point in the population"; the band is where h0 != 0
+ * (PAPER.md:204-210).  Picks the walker with the largest finite log L (lowest index on ties), evaluates its
+ * stand-in template directly on the dense grid and at n_edges log-spaced edges
+ * f_edges = geomspace(f_0, min(f_{n_f-1}, f_ISCO(best)), n_edges) (reading R12) on the device, and runs H0 on
+ * them (everything ll_het_prepare does).  Synchronises `stream`.
+ *   params : DEV [n_w][P]   logL : DEV [n_w]   best_index : HOST out (may be NULL)
+ *   f_edges_out : HOST out [n_edges] (may be NULL).
+ * LL_ERR_ARG when no log L is finite; LL_ERR_REF_ZERO when the best walker's f_ISCO lies below the grid.     */
+int ll_het_refresh_standin(ll_ctx *ctx, int64_t n_w, const double *params, const double *logL, int32_t n_edges,
+                           int64_t *best_index, double *f_edges_out, void *stream);
+
+/* Audit — "the brute-force Likelihood can ... verify the Heterodyning results": log L, <d|h>, <h|h>
+ * of each walker summed bin by bin over the dense bins the heterodyne bins cover (three-term form, Eq. 2-3, with
+ * <d|d> over the same bins), the stand-in template evaluated directly at every bin — no spline, no heterodyne.
+ * Compare with ll_het_batch_standin on the same rows.   params : DEV [n_w][P]; outputs as ll_het_batch.      */
+int ll_het_audit_standin(ll_ctx *ctx, int64_t n_w, const double *params, double *logL, double *d_h, double *h_h,
+                         void *stream);
+
 /* Summary data as computed by ll_het_prepare, for inspection.  HOST out, any pointer may be NULL.
  *   A0, A1 : [n_c][n_b][2]    B0, B1 : [n_c][n_b]                                                         */
 int ll_het_get_summary(ll_ctx *ctx, double *A0, double *A1, double *B0, double *B1, void *stream);

@@ -23,7 +23,7 @@ SYMBOLS = (
     "ll_create", "ll_destroy", "ll_last_error", "ll_abi_version", "ll_set_data", "ll_get_dd", "ll_standin_config",
     "ll_full_batch", "ll_full_batch_tf", "ll_tlm_nodes", "ll_standin_nodes", "ll_full_batch_standin", "ll_full_batch_standin_host",
     "ll_full_template_standin",
-    "ll_template_standin", "ll_het_prepare", "ll_het_get_summary", "ll_het_batch", "ll_het_batch_standin",
+    "ll_template_standin", "ll_het_prepare", "ll_het_refresh_standin", "ll_het_audit_standin", "ll_het_get_summary", "ll_het_batch", "ll_het_batch_standin",
     "ll_het_batch_standin_host", "ll_peak_fma", "ll_kernel_launches", "ll_last_full_stats",
     "ll_profile_enable", "ll_profile_read",
 )
@@ -74,6 +74,8 @@ def load_library(path: Optional[str] = None):
         "ll_het_get_summary": (C.c_int, [vp, vp, vp, vp, vp, vp]),
         "ll_het_batch": (C.c_int, [vp, i64, vp, vp, vp, vp, vp, vp, vp]),
         "ll_het_batch_standin": (C.c_int, [vp, i64, vp, vp, vp, vp, vp]),
+        "ll_het_refresh_standin": (C.c_int, [vp, i64, vp, vp, i32, vp, vp, vp]),
+        "ll_het_audit_standin": (C.c_int, [vp, i64, vp, vp, vp, vp, vp]),
         "ll_het_batch_standin_host": (C.c_int, [vp, i64, vp, vp, vp, vp, vp]),
         "ll_peak_fma": (C.c_int, [vp, i32, i64, C.POINTER(dbl), C.POINTER(dbl), vp]),
         "ll_kernel_launches": (i64, [vp]),
@@ -301,6 +303,26 @@ class Context:
         self._check(self._lib.ll_het_batch_standin(self._h, n_w, _dev_ptr(params, "params"), _dev_ptr(logL, "logL"),
                                                    _dev_ptr(d_h, "d_h"), _dev_ptr(h_h, "h_h"), _stream_ptr(stream)),
                     "ll_het_batch_standin")
+        return logL, d_h, h_h
+
+    def het_refresh_standin(self, params, logL, n_edges: int, stream=None):
+        """reference update: best walker -> h0 -> summary data; returns (best_index, f_edges)"""
+        best = C.c_int64(-1)
+        f_edges = np.empty(int(n_edges), dtype=np.float64)
+        self._check(self._lib.ll_het_refresh_standin(self._h, int(params.shape[0]), _dev_ptr(params, "params"),
+                                                     _dev_ptr(logL, "logL"), int(n_edges), C.byref(best),
+                                                     f_edges.ctypes.data_as(C.c_void_p), _stream_ptr(stream)),
+                    "ll_het_refresh_standin")
+        self._n_edges = int(n_edges)
+        return best.value, f_edges
+
+    def het_audit_standin(self, params, out=None, stream=None):
+        """brute-force dense log L over the heterodyne band"""
+        n_w = int(params.shape[0])
+        logL, d_h, h_h = out if out is not None else (self._out(n_w), self._out(n_w), self._out(n_w))
+        self._check(self._lib.ll_het_audit_standin(self._h, n_w, _dev_ptr(params, "params"), _dev_ptr(logL, "logL"),
+                                                   _dev_ptr(d_h, "d_h"), _dev_ptr(h_h, "h_h"), _stream_ptr(stream)),
+                    "ll_het_audit_standin")
         return logL, d_h, h_h
 
     def het_batch_standin_host(self, params_host, out_host, stream=None):

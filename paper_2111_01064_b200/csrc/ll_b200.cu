@@ -95,6 +95,7 @@ struct ll_ctx {
     bool have_het = false;
     int n_e = 0;
     DevBuf het_tab, het_raw, het_idx, het_fb, het_tab1;
+    DevBuf ref_idx, ref_dense, ref_edges; // ll_het_refresh_standin: argmax slot, h0 on the grid, h0 and f at the edges
     HetTable ht{};
     Het1Table ht1{}; // single-mode regrouped table (k_het_standin1); base == nullptr when not built
     std::vector<double> raw_host; // [n_b][13]
@@ -865,7 +866,8 @@ int ll_template_standin(ll_ctx *ctx, const double *params_row, int64_t n_freq, c
     const int P = 5 + 2 * kNC * ctx->n_m;
     memcpy(row.p, params_row, sizeof(double) * P);
     memcpy(row.c_lm, ctx->c_lm, sizeof(row.c_lm));
-    k_template_direct<<<ceil_div(n_freq, 256), 256, 0, (cudaStream_t)stream>>>(row, ctx->si, n_freq, f, f_lo, f_hi, h_out);
+    k_template_direct<<<ceil_div(n_freq, 256), 256, 0, (cudaStream_t)stream>>>(row, ctx->si, n_freq, f, GridInfo{0, 0, 0.0},
+                                                                                f_lo, f_hi, h_out);
     LAUNCHED(ctx);
     return LL_OK;
 }
@@ -927,6 +929,83 @@ int ll_het_prepare(ll_ctx *ctx, int32_t n_edges, const double *f_edges, const do
     ctx->ht.base = ctx->het_tab.as<double>();
     ctx->n_e = n_e;
     ctx->have_het = true;
+    return LL_OK;
+}
+
+// H0 inside the sampling loop: the highest-likelihood walker becomes the reference; the band is where
+// h0 != 0 (reading R12: log-spaced edges from the grid's first frequency to min(f_last, f_ISCO)).
+int ll_het_refresh_standin(ll_ctx *ctx, int64_t n_w, const double *params, const double *logL, int32_t n_edges,
+                           int64_t *best_index, double *f_edges_out, void *stream)
+{
+    if (!ctx) return LL_ERR_ARG;
+    if (n_w <= 0 || n_w > (1LL << 30)) return ctx->fail(LL_ERR_ARG, "n_w out of range (needs at least one walker)");
+    if (!params || !logL) return ctx->fail(LL_ERR_ARG, "params or logL is NULL");
+    if (n_edges < 2 || n_edges > 65536) return ctx->fail(LL_ERR_ARG, "n_edges out of range [2, 65536]");
+    if (!ctx->have_data) return ctx->fail(LL_ERR_STATE, "ll_set_data has not been called");
+    if (!ctx->have_standin) return ctx->fail(LL_ERR_STATE, "ll_standin_config has not been called");
+    DeviceGuard dg(ctx->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    const int P = 5 + 2 * kNC * ctx->n_m;
+    CK(ctx->ref_idx.ensure(sizeof(long long)));
+    k_argmax<<<1, 1024, 0, st>>>(logL, (long long)n_w, ctx->ref_idx.as<long long>());
+    LAUNCHED(ctx);
+    long long best = -1;
+    CK(cudaMemcpyAsync(&best, ctx->ref_idx.p, sizeof(long long), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    if (best < 0) return ctx->fail(LL_ERR_ARG, "no finite log L in the population");
+    DirectRow row;
+    memset(&row, 0, sizeof(row));
+    CK(cudaMemcpyAsync(row.p, params + (size_t)best * P, sizeof(double) * P, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    memcpy(row.c_lm, ctx->c_lm, sizeof(row.c_lm));
+    // edges: geomspace(f_0, min(f_last, f_ISCO(best)), n_edges), end points exact
+    const double q = row.p[1];
+    const double eta = q / ((1.0 + q) * (1.0 + q));
+    const double f_isco = 0x1.16b28f55d72d4p-4 / (3.14159265358979323846 * row.p[0] * std::pow(eta, -0.6));
+    const double f_first = bin_freq(ctx->k_min, 0, ctx->df), f_last = bin_freq(ctx->k_min, ctx->n_f - 1, ctx->df);
+    const double f_top = std::min(f_last, f_isco);
+    if (!(f_top > f_first)) return ctx->fail(LL_ERR_REF_ZERO, "the best walker's f_ISCO lies below the grid: no heterodyne band");
+    std::vector<double> e((size_t)n_edges);
+    const long double l0 = std::log((long double)f_first), l1 = std::log((long double)f_top);
+    for (int j = 0; j < n_edges; ++j) e[j] = (double)std::exp(l0 + (l1 - l0) * (long double)j / (long double)(n_edges - 1));
+    e[0] = f_first;
+    e[n_edges - 1] = f_top;
+    CK(ctx->ref_dense.ensure(sizeof(double) * 2 * kNC * (size_t)ctx->n_f));
+    CK(ctx->ref_edges.ensure(sizeof(double) * (2 * kNC + 1) * (size_t)n_edges));
+    double *fe_dev = ctx->ref_edges.as<double>() + (size_t)2 * kNC * n_edges;
+    CK(cudaMemcpyAsync(fe_dev, e.data(), sizeof(double) * n_edges, cudaMemcpyHostToDevice, st));
+    const GridInfo g{ctx->k_min, ctx->n_f, ctx->df};
+    k_template_direct<<<ceil_div(ctx->n_f, 256), 256, 0, st>>>(row, ctx->si, ctx->n_f, nullptr, g, f_first, f_last,
+                                                               ctx->ref_dense.as<double>());
+    LAUNCHED(ctx);
+    k_template_direct<<<ceil_div(n_edges, 256), 256, 0, st>>>(row, ctx->si, n_edges, fe_dev, g, f_first, f_last,
+                                                              ctx->ref_edges.as<double>());
+    LAUNCHED(ctx);
+    int rc = ll_het_prepare(ctx, n_edges, e.data(), ctx->ref_dense.as<double>(), ctx->ref_edges.as<double>(), stream);
+    if (rc != LL_OK) return rc;
+    if (best_index) *best_index = best;
+    if (f_edges_out) memcpy(f_edges_out, e.data(), sizeof(double) * n_edges);
+    return LL_OK;
+}
+
+// brute-force dense log L over the heterodyne band, template evaluated directly at every dense bin
+int ll_het_audit_standin(ll_ctx *ctx, int64_t n_w, const double *params, double *logL, double *d_h, double *h_h,
+                         void *stream)
+{
+    int rc = het_check(ctx, n_w, logL);
+    if (rc != LL_OK) return rc;
+    if (!ctx->have_standin) return ctx->fail(LL_ERR_STATE, "ll_standin_config has not been called");
+    if (n_w == 0) return LL_OK;
+    if (!params) return ctx->fail(LL_ERR_ARG, "params is NULL");
+    DeviceGuard dg(ctx->device);
+    DirectClm cl;
+    memcpy(cl.c_lm, ctx->c_lm, sizeof(cl.c_lm));
+    const GridInfo g{ctx->k_min, ctx->n_f, ctx->df};
+    k_het_audit<<<(unsigned)n_w, 256, 0, (cudaStream_t)stream>>>(params, 5 + 2 * kNC * ctx->n_m, cl, ctx->si,
+                                                                 ctx->g4.as<double>(), ctx->Wd.as<double>(), g,
+                                                                 ctx->het_idx.as<int>(), ctx->n_e - 1, ctx->dd.as<double>(),
+                                                                 logL, d_h, h_h);
+    LAUNCHED(ctx);
     return LL_OK;
 }
 

@@ -1141,39 +1141,121 @@ struct DirectRow {
     double p[5 + 4 * kMaxModes];
     double c_lm[kMaxModes];
 };
+struct DirectClm {
+    double c_lm[kMaxModes];
+};
 
+// h^A, h^E of one stand-in parameter row at frequency fi, evaluated directly (Eq. 7, 9; reading R9)
+__device__ __forceinline__ void direct_template_at(const double *__restrict__ rp, const double *__restrict__ c_lm,
+                                                   const StandinInfo &si, double Mtot, double eta, double fisco,
+                                                   double fi, double &hAr, double &hAi, double &hEr, double &hEi)
+{
+    const double tc = rp[2], phic = rp[3], invD = rp[4];
+    const double inv_kappa = 1.0 / si.kappa;
+    hAr = hAi = hEr = hEi = 0.0;
+    for (int m = 0; m < si.n_m; ++m) {
+        const double mh = 0.5 * (double)si.mode_m[m];
+        const double fp = fi / mh;
+        const double A = c_lm[m] * pow(fi, -7.0 / 6.0) * invD * taper(fp / fisco, si.kappa, inv_kappa);
+        const double v = cbrt(kPi * Mtot * fp);
+        const double v2 = v * v;
+        const double psi = mh * (2.0 * kPi * fp * tc - phic - 0.25 * kPi + 3.0 / (128.0 * eta * (v2 * v2 * v)));
+        double sn, cs;
+        sincos_rad(psi, sn, cs);
+        const double u = A * cs, vv = A * sn;
+        const double tar = rp[5 + m * 4], tai = rp[6 + m * 4], ter = rp[7 + m * 4], tei = rp[8 + m * 4];
+        hAr = fma(tar, u, hAr); hAr = fma(tai, vv, hAr);
+        hAi = fma(tai, u, hAi); hAi = fma(-tar, vv, hAi);
+        hEr = fma(ter, u, hEr); hEr = fma(tei, vv, hEr);
+        hEi = fma(tei, u, hEi); hEi = fma(-ter, vv, hEi);
+    }
+}
+
+// f == NULL: the frequencies are the dense grid's own, f_i = (k_min + i) df
 __global__ void __launch_bounds__(256)
-k_template_direct(DirectRow row, StandinInfo si, long long n_freq, const double *__restrict__ f, double f_lo,
+k_template_direct(DirectRow row, StandinInfo si, long long n_freq, const double *__restrict__ f, GridInfo g, double f_lo,
                   double f_hi, double *__restrict__ h_out)
 {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n_freq) return;
-    const double fi = f[i];
+    const double fi = f ? f[i] : bin_freq(g.k_min, i, g.df);
     double hAr = 0, hAi = 0, hEr = 0, hEi = 0;
     if (fi >= f_lo && fi <= f_hi) {
         double Mtot, eta, fisco;
         standin_masses(row.p[0], row.p[1], Mtot, eta, fisco);
-        const double tc = row.p[2], phic = row.p[3], invD = row.p[4];
-        const double inv_kappa = 1.0 / si.kappa;
-        for (int m = 0; m < si.n_m; ++m) {
-            const double mh = 0.5 * (double)si.mode_m[m];
-            const double fp = fi / mh;
-            const double A = row.c_lm[m] * pow(fi, -7.0 / 6.0) * invD * taper(fp / fisco, si.kappa, inv_kappa);
-            const double v = cbrt(kPi * Mtot * fp);
-            const double v2 = v * v;
-            const double psi = mh * (2.0 * kPi * fp * tc - phic - 0.25 * kPi + 3.0 / (128.0 * eta * (v2 * v2 * v)));
-            double sn, cs;
-            sincos_rad(psi, sn, cs);
-            const double u = A * cs, vv = A * sn;
-            const double tar = row.p[5 + m * 4], tai = row.p[6 + m * 4], ter = row.p[7 + m * 4], tei = row.p[8 + m * 4];
-            hAr = fma(tar, u, hAr); hAr = fma(tai, vv, hAr);
-            hAi = fma(tai, u, hAi); hAi = fma(-tar, vv, hAi);
-            hEr = fma(ter, u, hEr); hEr = fma(tei, vv, hEr);
-            hEi = fma(tei, u, hEi); hEi = fma(-ter, vv, hEi);
-        }
+        direct_template_at(row.p, row.c_lm, si, Mtot, eta, fisco, fi, hAr, hAi, hEr, hEi);
     }
     reinterpret_cast<double2 *>(h_out)[i] = make_double2(hAr, hAi);
     reinterpret_cast<double2 *>(h_out)[n_freq + i] = make_double2(hEr, hEi);
+}
+
+// PAPER.md:210 "replacing it with the highest Likelihood point in the population": index of the largest finite
+// log L (lowest index on ties), one block; out_idx = -1 when no entry is finite.
+__global__ void __launch_bounds__(1024) k_argmax(const double *__restrict__ v, long long n, long long *__restrict__ out_idx)
+{
+    __shared__ double sv[32];
+    __shared__ long long si_[32];
+    double bv = -INFINITY;
+    long long bi = -1;
+    for (long long i = threadIdx.x; i < n; i += blockDim.x) {
+        const double x = v[i];
+        if (x == x && fabs(x) != INFINITY && (bi < 0 || x > bv)) { bv = x; bi = i; } // ascending i: ties keep the lowest
+    }
+    auto better = [](double xv, long long xi, double yv, long long yi) {
+        if (xi < 0) return false;
+        if (yi < 0) return true;
+        return xv > yv || (xv == yv && xi < yi);
+    };
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        const double ov = __shfl_xor_sync(0xffffffffu, bv, o);
+        const long long oi = __shfl_xor_sync(0xffffffffu, bi, o);
+        if (better(ov, oi, bv, bi)) { bv = ov; bi = oi; }
+    }
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    if (lane == 0) { sv[wid] = bv; si_[wid] = bi; }
+    __syncthreads();
+    if (wid == 0) {
+        bv = sv[lane]; bi = si_[lane];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            const double ov = __shfl_xor_sync(0xffffffffu, bv, o);
+            const long long oi = __shfl_xor_sync(0xffffffffu, bi, o);
+            if (better(ov, oi, bv, bi)) { bv = ov; bi = oi; }
+        }
+        if (lane == 0) out_idx[0] = bi;
+    }
+}
+
+// PAPER.md:276 "the brute-force Likelihood can ... verify the Heterodyning results": dense log L of each walker
+// over the dense bins [i_lo, i_hi) the heterodyne bins cover, template evaluated directly at every bin (no spline,
+// no heterodyne), three-term form (Eq. 2-3).  One block per walker; fixed-order reduction.
+__global__ void __launch_bounds__(256)
+k_het_audit(const double *__restrict__ params, int P, DirectClm cl, StandinInfo si, const double *__restrict__ g4,
+            const double *__restrict__ Wd, GridInfo g, const int *__restrict__ estart, int n_b,
+            const double *__restrict__ dd, double *__restrict__ logL, double *__restrict__ d_h, double *__restrict__ h_h)
+{
+    __shared__ double sh[8];
+    const size_t w = blockIdx.x;
+    const double *rp = params + w * P;
+    const int i_lo = estart[0], i_hi = estart[n_b];
+    double Mtot, eta, fisco;
+    standin_masses(rp[0], rp[1], Mtot, eta, fisco);
+    double a_dh = 0.0, a_hh = 0.0;
+    for (int i = i_lo + threadIdx.x; i < i_hi; i += blockDim.x) {
+        double hAr, hAi, hEr, hEi;
+        direct_template_at(rp, cl.c_lm, si, Mtot, eta, fisco, bin_freq(g.k_min, i, g.df), hAr, hAi, hEr, hEi);
+        const double4 gg = reinterpret_cast<const double4 *>(g4)[i]; // W conj(d)
+        a_dh += (gg.x * hAr - gg.y * hAi) + (gg.z * hEr - gg.w * hEi);
+        a_hh = fma(Wd[i], (hAr * hAr + hAi * hAi) + (hEr * hEr + hEi * hEi), a_hh);
+    }
+    const double t_dh = block_sum_256(a_dh, sh);
+    const double t_hh = block_sum_256(a_hh, sh);
+    if (threadIdx.x == 0) {
+        logL[w] = t_dh - 0.5 * t_hh - 0.5 * dd[1];
+        if (d_h) d_h[w] = t_dh;
+        if (h_h) h_h[w] = t_hh;
+    }
 }
 
 // ---------------------------------------------------------------------------------------------------

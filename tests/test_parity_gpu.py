@@ -519,3 +519,55 @@ def test_state_and_argument_errors(torch_cuda):
 def test_smoke_entry(torch_cuda):
     import __graft_entry__
     __graft_entry__.smoke()
+
+
+# ------------------------------------------------------------- reference update and audit
+def test_het_audit_parity(orc, het_small, torch_cuda):
+    """brute-force dense log L over the heterodyne band against the oracle's"""
+    from oracle import reference_update as ru
+    wl, d, h0, h0e, summ, ctx = het_small
+    g = wl.grid
+    ref = ru.audit(wl.params[:64], wl.modes_m, wl.c_lm, wl.kappa, g.k_min, g.df, g.n_f, d, wl.W, wl.f_edges)
+    got = ctx.het_audit_standin(dev(torch_cuda, wl.params[:64]))
+    check_triplet(got, ref, "het audit")
+    assert ctx.het_audit_standin(dev(torch_cuda, wl.params[:0]))[0].numel() == 0
+
+
+def test_het_refresh_parity(orc, torch_cuda):
+    """reference update on the device: same best walker, same edges, same summary data and the same log L for the
+    whole population afterwards as the oracle's step-by-step update; het = audit at the new reference."""
+    from oracle import reference_update as ru
+    wl = wlm.make_workload(1, n_w=300, t_obs=2.0 ** 18, n_knots=37)
+    d, h0, h0e, summ = oracle_setup_het(orc, wl)
+    ctx = make_ctx(wl)
+    g = wl.grid
+    ctx.set_data(g.n_f, g.k_min, g.df, dev(torch_cuda, d), dev(torch_cuda, wl.W))
+    ctx.het_prepare(wl.f_edges, dev(torch_cuda, h0), dev(torch_cuda, h0e))
+    p = dev(torch_cuda, wl.params)
+    logL0 = ctx.het_batch_standin(p)[0]
+    ref0 = orc.het_batch_standin(wl.modes_m, wl.c_lm, wl.kappa, wl.params, wl.f_edges, h0e, summ)
+    up = ru.reference_update(wl.params, ref0["logL"], wl.modes_m, wl.c_lm, wl.kappa, g.k_min, g.df, g.n_f, d, wl.W, 41)
+    best, f_edges = ctx.het_refresh_standin(p, logL0, 41)
+    assert best == up["best"]
+    # numpy.geomspace itself carries a few ulp of log10/pow rounding; the library forms the edges in long double
+    np.testing.assert_allclose(f_edges, up["f_edges"], rtol=4e-15)
+    assert f_edges[0] == up["f_edges"][0] and abs(f_edges[-1] / up["f_edges"][-1] - 1.0) <= 1e-15   # f_ISCO: pow(eta, -0.6) and the division, a few ulp
+    # summary data: the library's own edges differ from numpy's by <= 2 ulp, which can move a dense bin across an
+    # edge only if it sits on one; compare with the oracle run on the library's edges (edges are an input of H0)
+    f = g.freqs()
+    h0n = orc.standin_direct(wl.params[best], wl.modes_m, wl.c_lm, wl.kappa, f, float(f[0]), float(f[-1]))
+    h0en = orc.standin_direct(wl.params[best], wl.modes_m, wl.c_lm, wl.kappa, f_edges, float(f[0]), float(f[-1]))
+    summ_n = orc.het_prepare(g.k_min, g.df, d, wl.W, h0n, f_edges)
+    got_s = ctx.het_get_summary()
+    for k in ("A0", "B0"):
+        np.testing.assert_allclose(got_s[k], summ_n[k], rtol=1e-10, atol=1e-10 * np.abs(summ_n[k]).max(), err_msg=k)
+    ref = orc.het_batch_standin(wl.modes_m, wl.c_lm, wl.kappa, wl.params, f_edges, h0en, summ_n)
+    got = ctx.het_batch_standin(p)
+    check_triplet(got, ref, "het after refresh")
+    aud = ctx.het_audit_standin(p[best:best + 1])
+    assert abs(float(got[0][best]) - float(aud[0][0])) <= 1e-6 * max(1.0, abs(float(aud[0][0])))
+    # no finite log L -> error, state untouched
+    from paper_2111_01064_b200 import binding
+    with pytest.raises(binding.LLError):
+        ctx.het_refresh_standin(p, torch_cuda.full_like(logL0, float("nan")), 41)
+    ctx.destroy()
