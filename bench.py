@@ -412,6 +412,22 @@ def main():
             r = bench_config(torch, idx, st, 5)
             per[f"cfg{idx}"] = {"evals_per_s": r["wl"].n_w / (r["ms_per_step"] * 1e-3), "ms_per_batch": r["ms_per_step"],
                                 "n_walkers": r["wl"].n_w}
+            if idx == 1:
+                # ---- the reference update inside the loop (every 5000 iterations)
+                # and the brute-force audit of the heterodyned values, config-1 size
+                c1, p1, n_e = r["ctx"], r["bufs"]["params"], len(r["wl"].f_edges)
+                t0 = time.perf_counter()
+                for _ in range(5):
+                    c1.het_refresh_standin(p1, r["out"][0], n_e)          # synchronises the stream itself
+                ms_ref = (time.perf_counter() - t0) / 5 * 1e3
+                het = [x.clone() for x in c1.het_batch_standin(p1)]
+                o1 = tuple(torch.empty_like(het[0]) for _ in range(3))
+                ms_a = time_steps(torch, lambda: c1.het_audit_standin(p1, out=o1), 5, 2) / 5
+                per["cfg1_refresh"] = {"ms_per_update": ms_ref, "n_edges": n_e, "n_f": r["wl"].grid.n_f,
+                                       "entry": "ll_het_refresh_standin (argmax, h0 on the grid and at the edges, H0; host wall time, the call synchronises)"}
+                per["cfg1_audit"] = {"evals_per_s": r["wl"].n_w / (ms_a * 1e-3), "ms_per_batch": ms_a, "n_walkers": r["wl"].n_w,
+                                     "max_abs_het_minus_dense_logL": float((het[0] - o1[0]).abs().max()),
+                                     "entry": "ll_het_audit_standin (direct template at every dense bin of the band)"}
             r["ctx"].destroy()
             del r
             torch.cuda.empty_cache()

@@ -538,33 +538,37 @@ int launch_het_standin(ll_ctx *ctx, int64_t n_w, const double *params, double *l
 {
     const int n_groups = ceil_div(n_w, 32), n_b = ctx->ht.n_b;
     constexpr int WY = 16; // warps per block, all sharing one table copy
-    const size_t smem = sizeof(double) * ((size_t)ctx->ht.total + (size_t)WY * 64);
+    // table + [WY][2][32] segment partials + -(m/pi) + lane-major transfer factors of the G = WY/S walker groups
+    auto smem_of = [&](int s) { return sizeof(double) * ((size_t)ctx->ht.total + (size_t)WY * 64 + 8 + (size_t)(WY / s) * NM * 128); };
     static bool attr_set = false;
     if (!attr_set) {
         CK(cudaFuncSetAttribute(k_het_standin<NM>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
         attr_set = true;
     }
-    if (smem > 227 * 1024) return ctx->fail(LL_ERR_UNSUPPORTED, "heterodyne tables exceed shared memory (too many bins x modes)");
-    static size_t bps_smem = 0; // resident blocks per SM (registers, threads, shared memory), cached per table size
-    static int bps = 0;
-    if (bps == 0 || bps_smem != smem) {
-        CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, k_het_standin<NM>, 32 * WY, smem));
-        bps = std::max(1, bps);
-        bps_smem = smem;
-    }
-    const int max_blocks = ctx->sm_count * bps;
+    if (smem_of(WY) > 227 * 1024) return ctx->fail(LL_ERR_UNSUPPORTED, "heterodyne tables exceed shared memory (too many bins x modes)");
     // S = frequency segments per walker group (G = WY/S groups per block pass): pick the split whose busiest SM
     // has the least work, work = resident blocks x passes per block x warp-edges per pass
-    int S = 1, grid = 1;
-    double best = 1e300;
-    for (int s = 1; s <= WY; s <<= 1) {
-        if (s > 1 && n_b / s < 8) break;
-        const int G = WY / s;
-        const long long passes = ceil_div(n_groups, G);
-        const int gr = (int)std::min<long long>(passes, max_blocks);
-        const double work = (double)ceil_div(gr, ctx->sm_count) * (double)ceil_div(passes, gr) * WY * (ceil_div(n_b, s) + 1.0);
-        if (work < best * 0.999) { best = work; S = s; grid = gr; }
+    static long long key_groups = -1; // decision cached per (batch size, table size)
+    static int key_total = -1, S = 1, grid = 1;
+    if (key_groups != n_groups || key_total != ctx->ht.total) {
+        double best = 1e300;
+        for (int s = 1; s <= WY; s <<= 1) {
+            if (s > 1 && n_b / s < 8) break;
+            if (smem_of(s) > 227 * 1024) continue;
+            int bps = 0;
+            CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, k_het_standin<NM>, 32 * WY, smem_of(s)));
+            bps = std::max(1, bps);
+            const int G = WY / s;
+            const long long passes = ceil_div(n_groups, G);
+            const int gr = (int)std::min<long long>(passes, (long long)ctx->sm_count * bps);
+            const double work = (double)ceil_div(gr, ctx->sm_count) * (double)ceil_div(passes, gr) * WY * (ceil_div(n_b, s) + 1.0);
+            if (work < best * 0.999) { best = work; S = s; grid = gr; }
+        }
+        if (best == 1e300) { S = WY; grid = (int)std::min<long long>(n_groups, ctx->sm_count); }
+        key_groups = n_groups;
+        key_total = ctx->ht.total;
     }
+    const size_t smem = smem_of(S);
     const int P = 5 + 2 * kNC * ctx->n_m;
     ProfScope prof(ctx, st);
     k_het_standin<NM><<<grid, dim3(32, WY), smem, st>>>(ctx->ht, ctx->si, params, P, (int)n_w, n_groups, S,

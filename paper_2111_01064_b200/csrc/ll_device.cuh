@@ -216,6 +216,13 @@ __device__ __forceinline__ double taper(double x, double kappa, double inv_kappa
     return s * s * s * fma(s, fma(6.0, s, -15.0), 10.0);
 }
 
+// the same function without branches: s clamped to [0, 1] gives exactly 1 at s = 1 (1 * (6 - 15 + 10)) and 0 at s = 0
+__device__ __forceinline__ double taper_nobranch(double x, double kappa, double inv_kappa)
+{
+    const double s = fmin(fmax((1.0 + kappa - x) * inv_kappa, 0.0), 1.0);
+    return s * s * s * fma(s, fma(6.0, s, -15.0), 10.0);
+}
+
 // frequency of dense bin i, exactly as the grid is defined (reading R3): f_i = (double)(k_min + i) * df
 __host__ __device__ __forceinline__ double bin_freq(long long k_min, long long i, double df)
 {

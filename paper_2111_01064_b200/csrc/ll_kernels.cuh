@@ -1337,23 +1337,88 @@ __device__ __forceinline__ void het_bin_contract(const double *__restrict__ tb, 
 // copy of the table: warp (g, s) walks segment s of the bins for the 32 walkers of group g.  Lanes of a warp
 // are 32 different walkers at the same edge, so every table read is a broadcast.  Blocks stride over passes of
 // G groups; the S partial sums of a group meet in shared memory in segment order (deterministic).
+//
+// Inside a segment the edges go in chunks of E = 4 with the MODE loop outside the edge loop: the transfer factors
+// of a mode are read once per chunk (from a lane-major shared copy, so they do not occupy 4 n_m registers for
+// the whole kernel), and the four edges of a chunk are four independent phase -> sincos -> T^c h chains in
+// flight per thread (with 16 warps per SM the FP64 pipe needs that instruction-level parallelism).  Whether any
+// lane needs the taper polynomial is decided once per chunk (warp-uniform), below f_ISCO m_min/2 it is 1.
+struct HetEdgeCtx {
+    const double *f4, *ih0, *cfp, *f2m, *fm53;
+    const double *tfs; // shared, [n_m][4][32] + lane
+    const double *nmq; // shared, [n_m]: -(m/pi)
+    int n_e;
+    double tc, invD, inv_fisco, K, phi0, kappa, inv_kappa;
+};
+
+template <int NM, int E, bool TAPER>
+__device__ __forceinline__ void het_eval_edges(const HetEdgeCtx &x, const StandinInfo &si, int e, double (&r)[E][4])
+{
+    double h[E][4], ftc[E];
+#pragma unroll
+    for (int k = 0; k < E; ++k) {
+        h[k][0] = h[k][1] = h[k][2] = h[k][3] = 0.0;
+        ftc[k] = x.f4[e + k] * x.tc;
+    }
+#pragma unroll 1
+    for (int m = 0; m < NM; ++m) {
+        const double nmq = x.nmq[m]; // -(m/pi), shared
+        const double *tq = x.tfs + m * 128;
+        const double t0 = tq[0], t1 = tq[32], t2 = tq[64], t3 = tq[96];
+        const int t = m * x.n_e + e;
+#pragma unroll
+        for (int k = 0; k < E; ++k) {
+            // quarter cycles: 4 f t_c + (m/pi) K (2f/m)^(-5/3) - (m/pi)(phi_c + pi/4)
+            const double y = fma(x.K, x.fm53[t + k], fma(nmq, x.phi0, ftc[k]));
+            double A = x.cfp[t + k] * x.invD;
+            if (TAPER) A *= taper_nobranch(x.f2m[t + k] * x.inv_fisco, x.kappa, x.inv_kappa);
+            double u, v; // h_m = u - i v
+            amp_expi_qc(A, y, u, v);
+            h[k][0] = fma(t0, u, h[k][0]); h[k][0] = fma(t1, v, h[k][0]);
+            h[k][1] = fma(t1, u, h[k][1]); h[k][1] = fma(-t0, v, h[k][1]);
+            h[k][2] = fma(t2, u, h[k][2]); h[k][2] = fma(t3, v, h[k][2]);
+            h[k][3] = fma(t3, u, h[k][3]); h[k][3] = fma(-t2, v, h[k][3]);
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < E; ++k) { // r = h * (1/h0)
+        const double *g = x.ih0 + 4 * (e + k);
+        r[k][0] = h[k][0] * g[0] - h[k][1] * g[1];
+        r[k][1] = h[k][0] * g[1] + h[k][1] * g[0];
+        r[k][2] = h[k][2] * g[2] - h[k][3] * g[3];
+        r[k][3] = h[k][2] * g[3] + h[k][3] * g[2];
+    }
+}
+
 template <int NM>
 __global__ void __launch_bounds__(512)
 k_het_standin(HetTable T, StandinInfo si, const double *__restrict__ params, int P, int n_w, int n_groups, int S,
               const double *__restrict__ dd, double *__restrict__ logL, double *__restrict__ d_h,
               double *__restrict__ h_h)
 {
+    constexpr int E = 4;
     extern __shared__ __align__(16) double tab[];
-    double *red = tab + T.total; // [G][S][2][32]
-    for (int i = threadIdx.x + threadIdx.y * 32; i < T.total; i += 32 * blockDim.y) tab[i] = T.base[i];
-    __syncthreads();
     const int G = blockDim.y / S, seg = threadIdx.y % S, gslot = threadIdx.y / S, lane = threadIdx.x;
+    double *red = tab + T.total;                 // [G][S][2][32]
+    double *nmq_s = red + (size_t)blockDim.y * 64;   // [8]
+    double *tfs_all = nmq_s + 8;                     // [G][NM][4][32]
+    for (int i = threadIdx.x + threadIdx.y * 32; i < T.total; i += 32 * blockDim.y) tab[i] = T.base[i];
+    if (threadIdx.y == 0 && lane < NM) nmq_s[lane] = -((double)si.mode_m[lane] / kPi);
     const int per = (T.n_b + S - 1) / S;
     const int b0 = seg * per, b1 = min(b0 + per, T.n_b);
-    const double *f4 = tab + T.off_f4(), *ih0 = tab + T.off_ih0(), *cfp = tab + T.off_cfp(),
-                 *f2m = tab + T.off_f2m(), *fm53 = tab + T.off_fm53(), *bins = tab + T.off_bins();
-    const double inv_kappa = 1.0 / si.kappa;
+    HetEdgeCtx x;
+    x.f4 = tab + T.off_f4(); x.ih0 = tab + T.off_ih0(); x.cfp = tab + T.off_cfp();
+    x.f2m = tab + T.off_f2m(); x.fm53 = tab + T.off_fm53();
+    x.tfs = tfs_all + (size_t)gslot * NM * 128 + lane;
+    x.nmq = nmq_s;
+    x.n_e = T.n_e;
+    x.kappa = si.kappa;
+    x.inv_kappa = 1.0 / si.kappa;
+    const double *bins = tab + T.off_bins();
     const double ddb = dd[1];
+    int m_min = si.mode_m[0];
+#pragma unroll
+    for (int m = 1; m < NM; ++m) m_min = min(m_min, si.mode_m[m]);
 
     for (int base = blockIdx.x * G; base < n_groups; base += gridDim.x * G) {
         const int grp = base + gslot;
@@ -1361,37 +1426,41 @@ k_het_standin(HetTable T, StandinInfo si, const double *__restrict__ params, int
         const bool valid = grp < n_groups && w < n_w;
         const double *row = params + (size_t)(valid ? w : 0) * P;
         const WalkerConst c = standin_consts(row);
-        double tf[NM][4];
+        x.tc = c.tc; x.invD = c.invD; x.inv_fisco = c.inv_fisco; x.K = c.K;
+        x.phi0 = c.phi + 0.25 * kPi;
+        __syncthreads(); // table staged (first pass) / previous pass done with tfs and red
+        if (seg == 0) {
+            double *tw = tfs_all + (size_t)gslot * NM * 128 + lane;
 #pragma unroll
-        for (int m = 0; m < NM; ++m) {
-#pragma unroll
-            for (int q = 0; q < 4; ++q) tf[m][q] = row[5 + m * 4 + q];
+            for (int q = 0; q < 4 * NM; ++q) tw[q * 32] = row[5 + q];
         }
-        const double phi0 = c.phi + 0.25 * kPi;
+        __syncthreads();
+        // x of the lowest-m mode = 2 f/(m_min f_ISCO) = 4 f * x_scale: above 1 somewhere in the warp -> taper needed
+        const double x_scale = c.inv_fisco * (0.5 / (double)m_min);
         double dh = 0.0, hh = 0.0;
-        double pAr = 0, pAi = 0, pEr = 0, pEi = 0;
-        if (grp < n_groups)
-        for (int e = b0; e <= b1 && b0 < b1; ++e) {
-            double hAr = 0, hAi = 0, hEr = 0, hEi = 0;
-            const double ftc = f4[e] * c.tc;
+        if (grp < n_groups && b0 < b1) {
+            double pr[1][4];
+            if (__any_sync(0xffffffffu, x.f4[b0] * x_scale > 1.0)) het_eval_edges<NM, 1, true>(x, si, b0, pr);
+            else het_eval_edges<NM, 1, false>(x, si, b0, pr);
+            double pAr = pr[0][0], pAi = pr[0][1], pEr = pr[0][2], pEi = pr[0][3];
+            int e = b0 + 1;
+            for (; e + E <= b1 + 1; e += E) {
+                double r[E][4];
+                if (__any_sync(0xffffffffu, x.f4[e + E - 1] * x_scale > 1.0)) het_eval_edges<NM, E, true>(x, si, e, r);
+                else het_eval_edges<NM, E, false>(x, si, e, r);
 #pragma unroll
-            for (int m = 0; m < NM; ++m) {
-                const int t = m * T.n_e + e;
-                // quarter cycles: 4 f t_c + (m/2pi) K (2f/m)^(-5/3) - (m/2pi)(phi_c + pi/4); fm53 carries m/(2 pi) ... m/pi
-                const double y = fma(c.K, fm53[t], fma(-((double)si.mode_m[m] / kPi), phi0, ftc));
-                const double A = cfp[t] * c.invD * taper(f2m[t] * c.inv_fisco, si.kappa, inv_kappa);
-                double u, v; // h_m = u - i v
-                amp_expi_qc(A, y, u, v);
-                hAr = fma(tf[m][0], u, hAr); hAr = fma(tf[m][1], v, hAr);
-                hAi = fma(tf[m][1], u, hAi); hAi = fma(-tf[m][0], v, hAi);
-                hEr = fma(tf[m][2], u, hEr); hEr = fma(tf[m][3], v, hEr);
-                hEi = fma(tf[m][3], u, hEi); hEi = fma(-tf[m][2], v, hEi);
+                for (int k = 0; k < E; ++k) {
+                    het_bin_contract(bins + 12 * (e + k - 1), pAr, pAi, pEr, pEi, r[k][0], r[k][1], r[k][2], r[k][3], dh, hh);
+                    pAr = r[k][0]; pAi = r[k][1]; pEr = r[k][2]; pEi = r[k][3];
+                }
             }
-            const double *g = ih0 + 4 * e; // r = h * (1/h0)
-            const double rAr = hAr * g[0] - hAi * g[1], rAi = hAr * g[1] + hAi * g[0];
-            const double rEr = hEr * g[2] - hEi * g[3], rEi = hEr * g[3] + hEi * g[2];
-            if (e > b0) het_bin_contract(bins + 12 * (e - 1), pAr, pAi, pEr, pEi, rAr, rAi, rEr, rEi, dh, hh);
-            pAr = rAr; pAi = rAi; pEr = rEr; pEi = rEi;
+            for (; e <= b1; ++e) {
+                double r[1][4];
+                if (__any_sync(0xffffffffu, x.f4[e] * x_scale > 1.0)) het_eval_edges<NM, 1, true>(x, si, e, r);
+                else het_eval_edges<NM, 1, false>(x, si, e, r);
+                het_bin_contract(bins + 12 * (e - 1), pAr, pAi, pEr, pEi, r[0][0], r[0][1], r[0][2], r[0][3], dh, hh);
+                pAr = r[0][0]; pAi = r[0][1]; pEr = r[0][2]; pEi = r[0][3];
+            }
         }
         if (S > 1) {
             double *rg = red + (size_t)gslot * S * 64;
@@ -1408,7 +1477,6 @@ k_het_standin(HetTable T, StandinInfo si, const double *__restrict__ params, int
             if (d_h) d_h[w] = dh;
             if (h_h) h_h[w] = hh;
         }
-        if (S > 1) __syncthreads();
     }
 }
 
