@@ -537,7 +537,7 @@ int launch_het_standin(ll_ctx *ctx, int64_t n_w, const double *params, double *l
                        cudaStream_t st)
 {
     const int n_groups = ceil_div(n_w, 32), n_b = ctx->ht.n_b;
-    constexpr int WY = 16; // warps per block, all sharing one table copy
+    constexpr int WY = LL_HET_WY; // warps per block, all sharing one table copy
     // table + [WY][2][32] segment partials + -(m/pi) + lane-major transfer factors of the G = WY/S walker groups
     auto smem_of = [&](int s) { return sizeof(double) * ((size_t)ctx->ht.total + (size_t)WY * 64 + 8 + (size_t)(WY / s) * NM * 128); };
     static bool attr_set = false;
@@ -552,7 +552,8 @@ int launch_het_standin(ll_ctx *ctx, int64_t n_w, const double *params, double *l
     static int key_total = -1, S = 1, grid = 1;
     if (key_groups != n_groups || key_total != ctx->ht.total) {
         double best = 1e300;
-        for (int s = 1; s <= WY; s <<= 1) {
+        for (int s = 1; s <= WY; ++s) {
+            if (WY % s) continue;
             if (s > 1 && n_b / s < 8) break;
             if (smem_of(s) > 227 * 1024) continue;
             int bps = 0;

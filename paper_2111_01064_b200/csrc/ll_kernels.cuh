@@ -1390,13 +1390,19 @@ __device__ __forceinline__ void het_eval_edges(const HetEdgeCtx &x, const Standi
     }
 }
 
+#ifndef LL_HET_E
+#define LL_HET_E 4   // edges per chunk (independent chains per thread)
+#endif
+#ifndef LL_HET_WY
+#define LL_HET_WY 16 // warps per block (one block per SM: the table copy is shared by all of them)
+#endif
 template <int NM>
-__global__ void __launch_bounds__(512)
+__global__ void __launch_bounds__(32 * LL_HET_WY)
 k_het_standin(HetTable T, StandinInfo si, const double *__restrict__ params, int P, int n_w, int n_groups, int S,
               const double *__restrict__ dd, double *__restrict__ logL, double *__restrict__ d_h,
               double *__restrict__ h_h)
 {
-    constexpr int E = 4;
+    constexpr int E = LL_HET_E;
     extern __shared__ __align__(16) double tab[];
     const int G = blockDim.y / S, seg = threadIdx.y % S, gslot = threadIdx.y / S, lane = threadIdx.x;
     double *red = tab + T.total;                 // [G][S][2][32]
@@ -1404,8 +1410,7 @@ k_het_standin(HetTable T, StandinInfo si, const double *__restrict__ params, int
     double *tfs_all = nmq_s + 8;                     // [G][NM][4][32]
     for (int i = threadIdx.x + threadIdx.y * 32; i < T.total; i += 32 * blockDim.y) tab[i] = T.base[i];
     if (threadIdx.y == 0 && lane < NM) nmq_s[lane] = -((double)si.mode_m[lane] / kPi);
-    const int per = (T.n_b + S - 1) / S;
-    const int b0 = seg * per, b1 = min(b0 + per, T.n_b);
+    const int b0 = (int)((long long)seg * T.n_b / S), b1 = (int)((long long)(seg + 1) * T.n_b / S); // balanced to +-1 bin
     HetEdgeCtx x;
     x.f4 = tab + T.off_f4(); x.ih0 = tab + T.off_ih0(); x.cfp = tab + T.off_cfp();
     x.f2m = tab + T.off_f2m(); x.fm53 = tab + T.off_fm53();
