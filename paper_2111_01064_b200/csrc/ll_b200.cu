@@ -632,7 +632,8 @@ int ll_destroy(ll_ctx *ctx)
         DevBuf *all[] = {&ctx->g4, &ctx->Wd, &ctx->dd_part, &ctx->dd, &ctx->pairs, &ctx->node_tab, &ctx->ilo_w, &ctx->ihi_w,
                          &ctx->key_w, &ctx->hist, &ctx->perm, &ctx->ilo_s, &ctx->ihi_s, &ctx->Y, &ctx->C, &ctx->TF,
                          &ctx->part, &ctx->prow, &ctx->het_tab, &ctx->het_tab1, &ctx->het_raw, &ctx->het_idx, &ctx->het_fb,
-                         &ctx->stage_in, &ctx->stage_out, &ctx->g4f, &ctx->Wf, &ctx->scale, &ctx->wmax};
+                         &ctx->stage_in, &ctx->stage_out, &ctx->g4f, &ctx->Wf, &ctx->scale, &ctx->wmax, &ctx->ref_idx,
+                         &ctx->ref_dense, &ctx->ref_edges};
         for (DevBuf *b : all) b->release();
         for (auto &e : ctx->ev) cudaEventDestroy(e);
     }
