@@ -703,3 +703,93 @@ def test_reference_update_then_het_equals_audit_at_new_reference(orc, het_small)
     assert het["h_h"][b] == pytest.approx(aud["h_h"][b], rel=1e-12)
     # the method's own accuracy with 24 bins on a 1e-3 ball (cf. test_het_tracks_dense_likelihood_near_reference)
     assert np.all(np.abs(het["logL"] - aud["logL"]) < 0.01 * np.abs(aud["logL"]) + 1e-6)
+
+
+# --------------------------------------------------------------------------- sampler step
+def test_stretch_z_is_inverse_cdf_of_g():
+    """g(z) ~ 1/sqrt(z) on [1/a, a]: CDF F(z) = (sqrt(a z) - 1)/(a - 1), so z(u) = ((a-1)u + 1)^2/a (R25)."""
+    from oracle import sampler as sm
+    u = np.linspace(0.0, 1.0, 11, endpoint=False)
+    for a in (2.0, 3.5):
+        z = sm.stretch_z(u, a)
+        np.testing.assert_allclose((np.sqrt(a * z) - 1.0) / (a - 1.0), u, atol=1e-15)
+        assert z[0] == pytest.approx(1.0 / a) and np.all((z >= 1.0 / a) & (z < a))
+
+
+def _gauss_loglike(prec):
+    def f(rows):
+        return -0.5 * np.einsum("ni,ij,nj->n", rows, prec, rows), {}
+    return f
+
+
+@pytest.mark.parametrize("beta", [1.0, 0.25])
+def test_stretch_move_keeps_gaussian_target(beta):
+    """Invariance of the target under the move: a d = 3 correlated Gaussian sampled at inverse temperature beta has
+    covariance C/beta.  Dropping z^(d-1), or using z^d, shifts the variance by tens of per cent."""
+    from oracle import sampler as sm
+    rng = np.random.default_rng(5)
+    C = np.array([[1.0, 0.6, 0.0], [0.6, 2.0, -0.3], [0.0, -0.3, 0.5]])
+    ll = _gauss_loglike(np.linalg.inv(C))
+    n_w, d = 64, 3
+    x = rng.normal(size=(1, n_w, d))
+    logL = ll(x[0])[0][None, :].copy()
+    lo, hi = np.full(d, -np.inf), np.full(d, np.inf)
+    keep = []
+    for it in range(1500):
+        for half in (0, 1):
+            sm.stretch_half(x, logL, half, [beta], lo, hi, d, 2.0, rng.random((1, n_w // 2)), rng.random((1, n_w // 2)),
+                            rng.random((1, n_w // 2)), ll)
+        if it >= 300:
+            keep.append(x[0].copy())
+    s = np.concatenate(keep)
+    np.testing.assert_allclose(logL[0], ll(x[0])[0], rtol=1e-12)          # bookkeeping of the stored log L
+    np.testing.assert_allclose(s.mean(axis=0), 0.0, atol=0.06 / np.sqrt(beta))
+    np.testing.assert_allclose(np.cov(s.T), C / beta, rtol=0.08, atol=0.05 / beta)
+
+
+def test_stretch_move_respects_prior_box_and_frozen_coordinates():
+    from oracle import sampler as sm
+    rng = np.random.default_rng(6)
+    ll = _gauss_loglike(np.eye(3))
+    x = rng.uniform(-1, 1, size=(2, 16, 3))
+    x[..., 2] = 0.7                                                        # frozen: identical in every walker
+    logL = np.stack([ll(x[t])[0] for t in range(2)])
+    lo, hi = np.array([-1.0, -1.0, -np.inf]), np.array([1.0, 1.0, np.inf])
+    for it in range(50):
+        for half in (0, 1):
+            sm.stretch_half(x, logL, half, [1.0, 0.1], lo, hi, 2, 2.0, rng.random((2, 8)), rng.random((2, 8)),
+                            rng.random((2, 8)), ll)
+    assert np.all(x[..., 2] == 0.7) and np.all(np.abs(x[..., :2]) <= 1.0)
+
+
+def test_temperature_swaps_textbook_cases():
+    """Equal betas: ln u < 0 always, every pair swaps.  Two temperatures: probability min(1, e^{dbeta dL}) (R27)."""
+    from oracle import sampler as sm
+    x = np.arange(2 * 4 * 1, dtype=float).reshape(2, 4, 1)
+    logL = np.array([[0.0, -1.0, -2.0, -3.0], [-5.0, -0.5, -2.0, 1.0]])
+    x0, l0 = x.copy(), logL.copy()
+    done = sm.temperature_swaps(x, logL, [1.0, 1.0], np.full((1, 4), 0.999))
+    assert done.all() and np.array_equal(x[0], x0[1]) and np.array_equal(logL[1], l0[0])
+    x, logL = x0.copy(), l0.copy()
+    # beta = (1, 0.5): ln q = (0.5 - 1)(L_cold - L_hot) = 0.5 (L_hot - L_cold) -> (-2.5, 0.25, 0, 2)
+    u = np.exp(np.array([[-2.4, 0.1, -1e-9, 1.9]]))                         # just above / below each threshold
+    u = np.minimum(u, 0.999999)
+    done = sm.temperature_swaps(x, logL, [1.0, 0.5], u)
+    assert done[0].tolist() == [False, True, True, True]
+    # a three-rung sweep lets the best hot walker climb to the cold chain in one sweep
+    x = np.array([[[0.0]], [[1.0]], [[2.0]]]); logL = np.array([[-9.0], [-5.0], [0.0]])
+    sm.temperature_swaps(x, logL, [1.0, 0.5, 0.1], np.full((2, 1), 0.5))
+    assert x[0, 0, 0] == 2.0 and logL[0, 0] == 0.0
+
+
+def test_stopping_functions():
+    """Module 1: extracted SNR against the limit.  Module 2: max log L unchanged (within 1) for 30
+    consecutive checks."""
+    from oracle import sampler as sm
+    best, bi, snr = sm.population_stats([-3.0, np.nan, -1.0, -1.0], [3.0, 1.0, 8.0, 1.0], [1.0, 1.0, 4.0, 0.0])
+    assert (best, bi, snr) == (-1.0, 2, 4.0)
+    s1 = sm.StopSNR(20.0)
+    assert not s1.check(19.9) and s1.check(20.0)
+    s2 = sm.StopConverged(n_checks=3, tol=1.0)
+    seq = [-10.0, -5.0, -4.5, -4.2, -3.9, -2.0, -1.9, -1.8, -1.7]
+    assert [s2.check(v) for v in seq] == [False, False, False, False, False, False, False, False, True]
