@@ -187,6 +187,49 @@ int ll_het_batch_standin(ll_ctx *ctx, int64_t n_w, const double *params, double 
 int ll_het_batch_standin_host(ll_ctx *ctx, int64_t n_w, const double *params_host, double *logL_host,
                               double *d_h_host, double *h_h_host, void *stream);
 
+/* ---- Sampler step around the likelihood ------------------------------------------------
+ * "This sampler is based on the overall structure of emcee with the parallel tempering scheme from ptemcee ...
+ * the typical 'stretch' proposal".  The formulas are in the paper's refs [72]-[74]; readings
+ * R25-R28.  The random numbers are INPUTS (uniform on [0,1)), so a step is a deterministic function.
+ * A position is a stand-in parameter row [P]; temperatures and walkers are laid out [n_temps][n_walkers].
+ *
+ * ll_pt_stretch_half_*: update half `half` (0: walkers [0, n/2); 1: [n/2, n)) of every temperature in place.
+ *   Walker k draws partner j = floor(u_partner n/2) from the other half and z = ((a-1) u_z + 1)^2 / a;
+ *   Y = X_j + z (X_k - X_j); accepted when ln u_accept < (n_dim-1) ln z + beta_t (ln L(Y) - ln L(X_k)), Y inside
+ *   [lo, hi] (uniform priors, Table I) and ln L(Y) finite.  ln L(Y) comes from the heterodyned (_het) or the
+ *   full-grid (_full) stand-in path of this context: three launches (propose, likelihood, accept), no host sync.
+ *   x : DEV [n_temps][n_walkers][P] in/out    logL : DEV [n_temps][n_walkers] in/out (must hold ln L(x) on entry)
+ *   d_h, h_h : DEV, same shape, in/out, or NULL    betas : DEV [n_temps]    lo, hi : DEV [P] (+-inf allowed)
+ *   n_dim : number of sampled (non-frozen) coordinates    a : stretch scale (2)
+ *   u_z, u_partner, u_accept : DEV [n_temps][n_walkers/2]    accepted : DEV out [n_temps][n_walkers/2] or NULL
+ * ll_pt_swap: for t = n_temps-1 .. 1, walker i of temperature t and walker i of t-1 exchange (x, ln L, d_h, h_h)
+ *   when ln u_swap[t-1][i] < (beta_t - beta_{t-1}) (ln L_{t-1,i} - ln L_{t,i}).   u_swap : DEV [n_temps-1][n_walkers]
+ * ll_pt_stats: out3 (DEV [3]) = max finite ln L, its index (as a double; lowest on ties, -1 if none), max
+ *   extracted SNR <d|h>/sqrt(<h|h>) — what the two stopping tests look at.
+ * ll_stop_snr / ll_stop_converged: the stopping functions themselves (host): 1 = stop. */
+int ll_pt_stretch_half_het(ll_ctx *ctx, int32_t n_temps, int32_t n_walkers, int32_t half, double *x, double *logL,
+                           double *d_h, double *h_h, const double *betas, const double *lo, const double *hi,
+                           int32_t n_dim, double a, const double *u_z, const double *u_partner, const double *u_accept,
+                           int32_t *accepted, void *stream);
+int ll_pt_stretch_half_full(ll_ctx *ctx, int32_t n_nodes, const double *f_nodes, int32_t n_temps, int32_t n_walkers,
+                            int32_t half, double *x, double *logL, double *d_h, double *h_h, const double *betas,
+                            const double *lo, const double *hi, int32_t n_dim, double a, const double *u_z,
+                            const double *u_partner, const double *u_accept, int32_t *accepted, void *stream);
+int ll_pt_swap(ll_ctx *ctx, int32_t n_temps, int32_t n_walkers, double *x, double *logL, double *d_h, double *h_h,
+               const double *betas, const double *u_swap, int32_t *swapped, void *stream);
+int ll_pt_stats(ll_ctx *ctx, int64_t n, const double *logL, const double *d_h, const double *h_h, double *out3,
+                void *stream);
+typedef struct {
+    int32_t n_checks; /* consecutive unchanged checks needed to stop (30 in the paper)   */
+    int32_t count;    /* consecutive unchanged checks so far                             */
+    int32_t has_ref;  /* 0 before the first check                                        */
+    int32_t reserved;
+    double tol;       /* "does not change its value by 1": 1.0                           */
+    double ref;       /* the value the current run of unchanged checks started from      */
+} ll_stop_state;
+int ll_stop_snr(double extracted_snr, double limit);
+int ll_stop_converged(ll_stop_state *s, double max_logL);
+
 /* Measurement helpers (no part of the method).
  * ll_peak_fma: runs `iters` dependent-free FMA chains on every SM and returns the achieved rate in
  *   FMA/s (HOST out); which = 0 -> FP64 DFMA (two loop-invariant register operands), 1 -> FP32 FFMA,

@@ -23,7 +23,8 @@ SYMBOLS = (
     "ll_create", "ll_destroy", "ll_last_error", "ll_abi_version", "ll_set_data", "ll_get_dd", "ll_standin_config",
     "ll_full_batch", "ll_full_batch_tf", "ll_tlm_nodes", "ll_standin_nodes", "ll_full_batch_standin", "ll_full_batch_standin_host",
     "ll_full_template_standin",
-    "ll_template_standin", "ll_het_prepare", "ll_het_refresh_standin", "ll_het_audit_standin", "ll_het_get_summary", "ll_het_batch", "ll_het_batch_standin",
+    "ll_template_standin", "ll_het_prepare", "ll_het_refresh_standin", "ll_het_audit_standin",
+    "ll_pt_stretch_half_het", "ll_pt_stretch_half_full", "ll_pt_swap", "ll_pt_stats", "ll_stop_snr", "ll_stop_converged", "ll_het_get_summary", "ll_het_batch", "ll_het_batch_standin",
     "ll_het_batch_standin_host", "ll_peak_fma", "ll_kernel_launches", "ll_last_full_stats",
     "ll_profile_enable", "ll_profile_read",
 )
@@ -76,6 +77,13 @@ def load_library(path: Optional[str] = None):
         "ll_het_batch_standin": (C.c_int, [vp, i64, vp, vp, vp, vp, vp]),
         "ll_het_refresh_standin": (C.c_int, [vp, i64, vp, vp, i32, vp, vp, vp]),
         "ll_het_audit_standin": (C.c_int, [vp, i64, vp, vp, vp, vp, vp]),
+        "ll_pt_stretch_half_het": (C.c_int, [vp, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp, i32, dbl, vp, vp, vp, vp, vp]),
+        "ll_pt_stretch_half_full": (C.c_int, [vp, i32, vp, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp, i32, dbl, vp, vp, vp,
+                                              vp, vp]),
+        "ll_pt_swap": (C.c_int, [vp, i32, i32, vp, vp, vp, vp, vp, vp, vp, vp]),
+        "ll_pt_stats": (C.c_int, [vp, i64, vp, vp, vp, vp, vp]),
+        "ll_stop_snr": (C.c_int, [dbl, dbl]),
+        "ll_stop_converged": (C.c_int, [vp, dbl]),
         "ll_het_batch_standin_host": (C.c_int, [vp, i64, vp, vp, vp, vp, vp]),
         "ll_peak_fma": (C.c_int, [vp, i32, i64, C.POINTER(dbl), C.POINTER(dbl), vp]),
         "ll_kernel_launches": (i64, [vp]),
@@ -94,6 +102,16 @@ def load_library(path: Optional[str] = None):
 def _torch():
     import torch
     return torch
+
+
+def _dev_ptr_i32(t, what: str):
+    """device pointer of a contiguous int32 CUDA tensor (None -> NULL)"""
+    if t is None:
+        return None
+    torch = _torch()
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.int32 and t.is_contiguous()):
+        raise TypeError(f"{what}: need a contiguous int32 CUDA tensor")
+    return C.c_void_p(t.data_ptr())
 
 
 def _dev_ptr(t, what: str):
@@ -117,6 +135,20 @@ def _stream_ptr(stream=None):
     torch = _torch()
     s = torch.cuda.current_stream() if stream is None else stream
     return C.c_void_p(s.cuda_stream)
+
+
+class StopState(C.Structure):
+    """ll_stop_state (include/ll.h): Module-2 stopping function state"""
+    _fields_ = [("n_checks", C.c_int32), ("count", C.c_int32), ("has_ref", C.c_int32), ("reserved", C.c_int32),
+                ("tol", C.c_double), ("ref", C.c_double)]
+
+
+def stop_snr(extracted_snr: float, limit: float) -> bool:
+    return bool(load_library().ll_stop_snr(float(extracted_snr), float(limit)))
+
+
+def stop_converged(state: StopState, max_logL: float) -> bool:
+    return bool(load_library().ll_stop_converged(C.byref(state), float(max_logL)))
 
 
 class Context:
@@ -324,6 +356,36 @@ class Context:
                                                    _dev_ptr(d_h, "d_h"), _dev_ptr(h_h, "h_h"), _stream_ptr(stream)),
                     "ll_het_audit_standin")
         return logL, d_h, h_h
+
+    # -- sampler step (readings R25-R28): x [n_temps][n_walkers][P], everything on the device
+    def pt_stretch_half(self, half, x, logL, d_h, h_h, betas, lo, hi, n_dim, u_z, u_partner, u_accept, a=2.0,
+                        accepted=None, f_nodes=None, stream=None):
+        """stretch move on one half of every temperature, in place; f_nodes given -> full-grid likelihood, else het"""
+        n_t, n_w = int(x.shape[0]), int(x.shape[1])
+        tail = (n_t, n_w, int(half), _dev_ptr(x, "x"), _dev_ptr(logL, "logL"), _dev_ptr(d_h, "d_h"), _dev_ptr(h_h, "h_h"),
+                _dev_ptr(betas, "betas"), _dev_ptr(lo, "lo"), _dev_ptr(hi, "hi"), int(n_dim), float(a), _dev_ptr(u_z, "u_z"),
+                _dev_ptr(u_partner, "u_partner"), _dev_ptr(u_accept, "u_accept"), _dev_ptr_i32(accepted, "accepted"),
+                _stream_ptr(stream))
+        if f_nodes is None:
+            self._check(self._lib.ll_pt_stretch_half_het(self._h, *tail), "ll_pt_stretch_half_het")
+        else:
+            f_nodes = _host_f64(f_nodes, "f_nodes")
+            self._check(self._lib.ll_pt_stretch_half_full(self._h, len(f_nodes), f_nodes.ctypes.data_as(C.c_void_p), *tail),
+                        "ll_pt_stretch_half_full")
+
+    def pt_swap(self, x, logL, d_h, h_h, betas, u_swap, swapped=None, stream=None):
+        self._check(self._lib.ll_pt_swap(self._h, int(x.shape[0]), int(x.shape[1]), _dev_ptr(x, "x"), _dev_ptr(logL, "logL"),
+                                         _dev_ptr(d_h, "d_h"), _dev_ptr(h_h, "h_h"), _dev_ptr(betas, "betas"),
+                                         _dev_ptr(u_swap, "u_swap"), _dev_ptr_i32(swapped, "swapped"), _stream_ptr(stream)),
+                    "ll_pt_swap")
+
+    def pt_stats(self, logL, d_h, h_h, out3=None, stream=None):
+        """-> device tensor [3]: max log L, its index, max extracted SNR"""
+        if out3 is None:
+            out3 = _torch().empty(3, dtype=_torch().float64, device=logL.device)
+        self._check(self._lib.ll_pt_stats(self._h, int(logL.numel()), _dev_ptr(logL, "logL"), _dev_ptr(d_h, "d_h"),
+                                          _dev_ptr(h_h, "h_h"), _dev_ptr(out3, "out3"), _stream_ptr(stream)), "ll_pt_stats")
+        return out3
 
     def het_batch_standin_host(self, params_host, out_host, stream=None):
         n_w = int(params_host.shape[0])

@@ -95,6 +95,7 @@ struct ll_ctx {
     bool have_het = false;
     int n_e = 0;
     DevBuf het_tab, het_raw, het_idx, het_fb, het_tab1;
+    DevBuf pt_y, pt_out, pt_in; // sampler step: proposals [n][P], (log L, <d|h>, <h|h>, (d-1) ln z) [4][n], inside flags
     DevBuf ref_idx, ref_dense, ref_edges; // ll_het_refresh_standin: argmax slot, h0 on the grid, h0 and f at the edges
     HetTable ht{};
     Het1Table ht1{}; // single-mode regrouped table (k_het_standin1); base == nullptr when not built
@@ -633,7 +634,7 @@ int ll_destroy(ll_ctx *ctx)
                          &ctx->key_w, &ctx->hist, &ctx->perm, &ctx->ilo_s, &ctx->ihi_s, &ctx->Y, &ctx->C, &ctx->TF,
                          &ctx->part, &ctx->prow, &ctx->het_tab, &ctx->het_tab1, &ctx->het_raw, &ctx->het_idx, &ctx->het_fb,
                          &ctx->stage_in, &ctx->stage_out, &ctx->g4f, &ctx->Wf, &ctx->scale, &ctx->wmax, &ctx->ref_idx,
-                         &ctx->ref_dense, &ctx->ref_edges};
+                         &ctx->ref_dense, &ctx->ref_edges, &ctx->pt_y, &ctx->pt_out, &ctx->pt_in};
         for (DevBuf *b : all) b->release();
         for (auto &e : ctx->ev) cudaEventDestroy(e);
     }
@@ -1102,6 +1103,98 @@ int ll_het_batch_standin_host(ll_ctx *ctx, int64_t n_w, const double *params_hos
     if (h_h_host) CK(cudaMemcpyAsync(h_h_host, o + 2 * n_w, sizeof(double) * n_w, cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
     return LL_OK;
+}
+
+// ---- sampler step around the likelihood (readings R25-R28) ----------------
+namespace {
+int pt_half(ll_ctx *ctx, bool full, int32_t n_nodes, const double *f_nodes, int32_t n_t, int32_t n_w, int32_t half,
+            double *x, double *logL, double *d_h, double *h_h, const double *betas, const double *lo, const double *hi,
+            int32_t n_dim, double a, const double *u_z, const double *u_partner, const double *u_accept,
+            int32_t *accepted, void *stream)
+{
+    if (!ctx) return LL_ERR_ARG;
+    if (n_t < 1 || n_w < 2 || (n_w & 1)) return ctx->fail(LL_ERR_ARG, "n_temps >= 1 and an even n_walkers >= 2 are required");
+    if ((int64_t)n_t * n_w > (1LL << 30)) return ctx->fail(LL_ERR_ARG, "n_temps * n_walkers too large");
+    if (half != 0 && half != 1) return ctx->fail(LL_ERR_ARG, "half must be 0 or 1");
+    if (!x || !logL || !betas || !lo || !hi || !u_z || !u_partner || !u_accept) return ctx->fail(LL_ERR_ARG, "NULL argument");
+    if (n_dim < 1 || !(a > 1.0)) return ctx->fail(LL_ERR_ARG, "n_dim >= 1 and a > 1 are required");
+    if (!ctx->have_standin) return ctx->fail(LL_ERR_STATE, "ll_standin_config has not been called");
+    DeviceGuard dg(ctx->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    const int P = 5 + 2 * kNC * ctx->n_m;
+    const int64_t np = (int64_t)n_t * (n_w / 2);
+    CK(ctx->pt_y.ensure(sizeof(double) * (size_t)np * P));
+    CK(ctx->pt_out.ensure(sizeof(double) * (size_t)np * 4));
+    CK(ctx->pt_in.ensure(sizeof(int) * (size_t)np));
+    double *y = ctx->pt_y.as<double>(), *ly = ctx->pt_out.as<double>(), *ydh = ly + np, *yhh = ly + 2 * np, *lnz = ly + 3 * np;
+    const int grid = (int)ceil_div(np, 128);
+    k_pt_propose<<<grid, 128, 0, st>>>(x, n_t, n_w, P, half, a, n_dim, lo, hi, u_z, u_partner, y, lnz, ctx->pt_in.as<int>());
+    LAUNCHED(ctx);
+    int rc = full ? ll_full_batch_standin(ctx, np, n_nodes, f_nodes, y, ly, ydh, yhh, stream)
+                  : ll_het_batch_standin(ctx, np, y, ly, ydh, yhh, stream);
+    if (rc != LL_OK) return rc;
+    k_pt_accept<<<grid, 128, 0, st>>>(x, logL, d_h, h_h, n_t, n_w, P, half, betas, u_accept, y, ly, ydh, yhh, lnz,
+                                      ctx->pt_in.as<int>(), accepted);
+    LAUNCHED(ctx);
+    return LL_OK;
+}
+} // namespace
+
+int ll_pt_stretch_half_het(ll_ctx *ctx, int32_t n_temps, int32_t n_walkers, int32_t half, double *x, double *logL,
+                           double *d_h, double *h_h, const double *betas, const double *lo, const double *hi,
+                           int32_t n_dim, double a, const double *u_z, const double *u_partner, const double *u_accept,
+                           int32_t *accepted, void *stream)
+{
+    return pt_half(ctx, false, 0, nullptr, n_temps, n_walkers, half, x, logL, d_h, h_h, betas, lo, hi, n_dim, a, u_z,
+                   u_partner, u_accept, accepted, stream);
+}
+
+int ll_pt_stretch_half_full(ll_ctx *ctx, int32_t n_nodes, const double *f_nodes, int32_t n_temps, int32_t n_walkers,
+                            int32_t half, double *x, double *logL, double *d_h, double *h_h, const double *betas,
+                            const double *lo, const double *hi, int32_t n_dim, double a, const double *u_z,
+                            const double *u_partner, const double *u_accept, int32_t *accepted, void *stream)
+{
+    return pt_half(ctx, true, n_nodes, f_nodes, n_temps, n_walkers, half, x, logL, d_h, h_h, betas, lo, hi, n_dim, a, u_z,
+                   u_partner, u_accept, accepted, stream);
+}
+
+int ll_pt_swap(ll_ctx *ctx, int32_t n_temps, int32_t n_walkers, double *x, double *logL, double *d_h, double *h_h,
+               const double *betas, const double *u_swap, int32_t *swapped, void *stream)
+{
+    if (!ctx) return LL_ERR_ARG;
+    if (n_temps < 1 || n_walkers < 1) return ctx->fail(LL_ERR_ARG, "n_temps, n_walkers >= 1 are required");
+    if (!x || !logL || !betas || (n_temps > 1 && !u_swap)) return ctx->fail(LL_ERR_ARG, "NULL argument");
+    if (n_temps == 1) return LL_OK;
+    DeviceGuard dg(ctx->device);
+    k_pt_swap<<<(int)ceil_div(n_walkers, 128), 128, 0, (cudaStream_t)stream>>>(x, logL, d_h, h_h, n_temps, n_walkers,
+                                                                              5 + 2 * kNC * ctx->n_m, betas, u_swap, swapped);
+    LAUNCHED(ctx);
+    return LL_OK;
+}
+
+int ll_pt_stats(ll_ctx *ctx, int64_t n, const double *logL, const double *d_h, const double *h_h, double *out3, void *stream)
+{
+    if (!ctx) return LL_ERR_ARG;
+    if (n < 1 || !logL || !out3) return ctx->fail(LL_ERR_ARG, "n >= 1, logL and out3 are required");
+    DeviceGuard dg(ctx->device);
+    k_pt_stats<<<1, 1024, 0, (cudaStream_t)stream>>>(logL, d_h, h_h, (long long)n, out3);
+    LAUNCHED(ctx);
+    return LL_OK;
+}
+
+int ll_stop_snr(double extracted_snr, double limit) { return extracted_snr >= limit ? 1 : 0; }
+
+int ll_stop_converged(ll_stop_state *s, double max_logL)
+{
+    if (!s) return LL_ERR_ARG;
+    if (!s->has_ref || !(fabs(max_logL - s->ref) < s->tol)) {
+        s->ref = max_logL;
+        s->count = 0;
+        s->has_ref = 1;
+    } else {
+        s->count += 1;
+    }
+    return s->count >= s->n_checks ? 1 : 0;
 }
 
 int ll_peak_fma(ll_ctx *ctx, int32_t which, int64_t iters, double *fma_per_s, double *ms_out, void *stream)

@@ -1641,6 +1641,144 @@ k_het_arrays(HetTable T, const double *__restrict__ amp_e, const double *__restr
 }
 
 // ---------------------------------------------------------------------------------------------------
+// Sampler step around the likelihood (emcee structure, ptemcee tempering, stretch proposal [74];
+// readings R25-R28).  The random numbers are inputs.  Proposal arithmetic is written with explicit _rn
+// operations (no FMA contraction) so that it is the plain IEEE expression Y = X_j + z (X_k - X_j).
+// ---------------------------------------------------------------------------------------------------
+// one thread per proposal (t, k): partner j from the other half, z = ((a-1)u+1)^2/a, Y, prior-box test.
+// A proposal outside the box is replaced by the walker's own position (so the likelihood kernel sees a valid
+// row) and flagged; lnz = (d-1) ln z.
+__global__ void __launch_bounds__(128)
+k_pt_propose(const double *__restrict__ x, int n_t, int n_w, int P, int half, double a, int n_dim,
+             const double *__restrict__ lo, const double *__restrict__ hi, const double *__restrict__ u_z,
+             const double *__restrict__ u_partner, double *__restrict__ y, double *__restrict__ lnz,
+             int *__restrict__ inside)
+{
+    const int nh = n_w / 2;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_t * nh) return;
+    const int t = i / nh, k = i - t * nh;
+    const int k0 = half == 0 ? 0 : nh, j0 = half == 0 ? nh : 0;
+    const double tt = __dadd_rn(__dmul_rn(a - 1.0, u_z[i]), 1.0);
+    const double z = __ddiv_rn(__dmul_rn(tt, tt), a);
+    int j = (int)(u_partner[i] * (double)nh);
+    j = min(max(j, 0), nh - 1);
+    const double *xk = x + ((size_t)t * n_w + k0 + k) * P;
+    const double *xj = x + ((size_t)t * n_w + j0 + j) * P;
+    double *yo = y + (size_t)i * P;
+    bool in = true;
+    for (int q = 0; q < P; ++q) {
+        const double v = __dadd_rn(xj[q], __dmul_rn(z, __dadd_rn(xk[q], -xj[q])));
+        in = in && (v >= lo[q]) && (v <= hi[q]);
+        yo[q] = v;
+    }
+    if (!in)
+        for (int q = 0; q < P; ++q) yo[q] = xk[q];
+    inside[i] = in ? 1 : 0;
+    lnz[i] = (double)(n_dim - 1) * log(z);
+}
+
+// accept when ln u' < (d-1) ln z + beta_t (ln L(Y) - ln L(X_k)), Y inside the box and ln L(Y) finite (R25, R26)
+__global__ void __launch_bounds__(128)
+k_pt_accept(double *__restrict__ x, double *__restrict__ logL, double *__restrict__ d_h, double *__restrict__ h_h,
+            int n_t, int n_w, int P, int half, const double *__restrict__ betas, const double *__restrict__ u_accept,
+            const double *__restrict__ y, const double *__restrict__ ly, const double *__restrict__ ydh,
+            const double *__restrict__ yhh, const double *__restrict__ lnz, const int *__restrict__ inside,
+            int *__restrict__ accepted)
+{
+    const int nh = n_w / 2;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_t * nh) return;
+    const int t = i / nh, k = i - t * nh;
+    const size_t wk = (size_t)t * n_w + (half == 0 ? 0 : nh) + k;
+    const double l_new = ly[i];
+    bool acc = false;
+    if (inside[i] && l_new == l_new && fabs(l_new) != INFINITY) {
+        const double lnq = __dadd_rn(lnz[i], __dmul_rn(betas[t], __dadd_rn(l_new, -logL[wk])));
+        acc = log(u_accept[i]) < lnq;
+    }
+    if (acc) {
+        const double *yo = y + (size_t)i * P;
+        double *xo = x + wk * P;
+        for (int q = 0; q < P; ++q) xo[q] = yo[q];
+        logL[wk] = l_new;
+        if (d_h) d_h[wk] = ydh[i];
+        if (h_h) h_h[wk] = yhh[i];
+    }
+    if (accepted) accepted[i] = acc ? 1 : 0;
+}
+
+// temperature swaps (R27): one thread per walker column i, rungs swept from the hottest down, sequential in t
+__global__ void __launch_bounds__(128)
+k_pt_swap(double *__restrict__ x, double *__restrict__ logL, double *__restrict__ d_h, double *__restrict__ h_h,
+          int n_t, int n_w, int P, const double *__restrict__ betas, const double *__restrict__ u_swap,
+          int *__restrict__ swapped)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_w) return;
+    for (int t = n_t - 1; t >= 1; --t) {
+        const size_t hi_ = (size_t)t * n_w + i, lo_ = (size_t)(t - 1) * n_w + i;
+        const double lh = logL[hi_], lc = logL[lo_];
+        const double lnq = __dmul_rn(__dadd_rn(betas[t], -betas[t - 1]), __dadd_rn(lc, -lh));
+        const bool sw = log(u_swap[(size_t)(t - 1) * n_w + i]) < lnq;
+        if (sw) {
+            double *a = x + hi_ * P, *b = x + lo_ * P;
+            for (int q = 0; q < P; ++q) { const double v = a[q]; a[q] = b[q]; b[q] = v; }
+            logL[hi_] = lc; logL[lo_] = lh;
+            if (d_h) { const double v = d_h[hi_]; d_h[hi_] = d_h[lo_]; d_h[lo_] = v; }
+            if (h_h) { const double v = h_h[hi_]; h_h[hi_] = h_h[lo_]; h_h[lo_] = v; }
+        }
+        if (swapped) swapped[(size_t)(t - 1) * n_w + i] = sw ? 1 : 0;
+    }
+}
+
+// what the stopping tests look at: out[0] = max finite log L, out[1] = its index (lowest on
+// ties, -1 if none), out[2] = max extracted SNR <d|h>/sqrt(<h|h>) over entries with <h|h> > 0.  One block.
+__global__ void __launch_bounds__(1024)
+k_pt_stats(const double *__restrict__ logL, const double *__restrict__ d_h, const double *__restrict__ h_h, long long n,
+           double *__restrict__ out)
+{
+    __shared__ double sv[32], ss[32];
+    __shared__ long long si_[32];
+    double bv = -INFINITY, bs = -INFINITY;
+    long long bi = -1;
+    for (long long i = threadIdx.x; i < n; i += blockDim.x) {
+        const double v = logL[i];
+        if (v == v && fabs(v) != INFINITY && (bi < 0 || v > bv)) { bv = v; bi = i; }
+        if (d_h && h_h) {
+            const double hh = h_h[i], dh = d_h[i];
+            if (hh > 0.0 && dh == dh && fabs(dh) != INFINITY) bs = fmax(bs, dh / sqrt(hh));
+        }
+    }
+    auto better = [](double xv, long long xi, double yv, long long yi) {
+        if (xi < 0) return false;
+        if (yi < 0) return true;
+        return xv > yv || (xv == yv && xi < yi);
+    };
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        const double ov = __shfl_xor_sync(0xffffffffu, bv, o);
+        const long long oi = __shfl_xor_sync(0xffffffffu, bi, o);
+        if (better(ov, oi, bv, bi)) { bv = ov; bi = oi; }
+        bs = fmax(bs, __shfl_xor_sync(0xffffffffu, bs, o));
+    }
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    if (lane == 0) { sv[wid] = bv; si_[wid] = bi; ss[wid] = bs; }
+    __syncthreads();
+    if (wid == 0) {
+        bv = sv[lane]; bi = si_[lane]; bs = ss[lane];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            const double ov = __shfl_xor_sync(0xffffffffu, bv, o);
+            const long long oi = __shfl_xor_sync(0xffffffffu, bi, o);
+            if (better(ov, oi, bv, bi)) { bv = ov; bi = oi; }
+            bs = fmax(bs, __shfl_xor_sync(0xffffffffu, bs, o));
+        }
+        if (lane == 0) { out[0] = bv; out[1] = (double)bi; out[2] = bs; }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
 // ALU roofline denominators: dependent-free FMA chains on every SM (measurement helper)
 // ---------------------------------------------------------------------------------------------------
 template <typename T>

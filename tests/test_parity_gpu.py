@@ -571,3 +571,116 @@ def test_het_refresh_parity(orc, torch_cuda):
     with pytest.raises(binding.LLError):
         ctx.het_refresh_standin(p, torch_cuda.full_like(logL0, float("nan")), 41)
     ctx.destroy()
+
+
+# ------------------------------------------------------------------- sampler step (R25-R28)
+def _oracle_loglike_het(orc, wl, h0e, summ):
+    def f(rows):
+        r = orc.het_batch_standin(wl.modes_m, wl.c_lm, wl.kappa, rows, wl.f_edges, h0e, summ)
+        return r["logL"], {"d_h": r["d_h"], "h_h": r["h_h"]}
+    return f
+
+
+def _prior_box(wl, params, widen):
+    """uniform box around the population (Table I priors are uniform); the transfer factors are frozen"""
+    P = params.shape[1]
+    lo, hi = np.full(P, -np.inf), np.full(P, np.inf)
+    c, w = params[:, :5].mean(axis=0), widen * np.ptp(params[:, :5], axis=0)
+    lo[:5], hi[:5] = c - w, c + w
+    return lo, hi
+
+
+def test_pt_step_parity_het(orc, het_small, torch_cuda):
+    """three iterations (two half updates + a swap sweep each) of 3 temperatures x 64 walkers on the heterodyned
+    likelihood: same accept/swap decisions, same positions bit for bit, same log L within the FP64 bar."""
+    from oracle import sampler as sm
+    wl, d, h0, h0e, summ, ctx = het_small
+    tc = torch_cuda
+    rng = np.random.default_rng(190)
+    n_t, n_w = 3, 64
+    x = wl.params[:n_t * n_w].reshape(n_t, n_w, -1).copy()
+    x[:, :, 5:] = wl.inj[5:]                                   # frozen coordinates: identical in every walker
+    betas = np.array([1.0, 0.3, 0.05])
+    lo, hi = _prior_box(wl, wl.params, 0.35)                   # tight enough that some proposals leave the box
+    ll = _oracle_loglike_het(orc, wl, h0e, summ)
+    l0, ex = ll(x.reshape(n_t * n_w, -1))
+    logL, d_h, h_h = (v.reshape(n_t, n_w).copy() for v in (l0, ex["d_h"], ex["h_h"]))
+    gx, gl, gd, gh = dev(tc, x), dev(tc, logL), dev(tc, d_h), dev(tc, h_h)
+    gb, glo, ghi = dev(tc, betas), dev(tc, lo), dev(tc, hi)
+    acc_g = tc.empty((n_t, n_w // 2), dtype=tc.int32, device="cuda")
+    sw_g = tc.empty((n_t - 1, n_w), dtype=tc.int32, device="cuda")
+    n_acc = n_out = n_sw = 0
+    for it in range(3):
+        for half in (0, 1):
+            u = rng.random((3, n_t, n_w // 2))
+            acc, y, ly, extra = sm.stretch_half(x, logL, half, betas, lo, hi, 5, 2.0, u[0], u[1], u[2], ll)
+            k0 = 0 if half == 0 else n_w // 2                  # the oracle keeps d_h, h_h of accepted proposals too
+            for t in range(n_t):
+                sel = np.nonzero(acc[t])[0]
+                d_h[t, k0 + sel] = extra["d_h"].reshape(n_t, -1)[t, sel]
+                h_h[t, k0 + sel] = extra["h_h"].reshape(n_t, -1)[t, sel]
+            ctx.pt_stretch_half(half, gx, gl, gd, gh, gb, glo, ghi, 5, dev(tc, u[0]), dev(tc, u[1]), dev(tc, u[2]),
+                                accepted=acc_g)
+            assert np.array_equal(acc_g.cpu().numpy().astype(bool), acc), f"accept decisions, it {it} half {half}"
+            n_acc += int(acc.sum())
+            n_out += int((~np.all((y >= lo) & (y <= hi), axis=2)).sum())
+        us = rng.random((n_t - 1, n_w))
+        done = sm.temperature_swaps(x, logL, betas, us)
+        for t in range(n_t - 1, 0, -1):                          # d_h, h_h travel with the walker
+            for i in np.nonzero(done[t - 1])[0]:
+                d_h[t, i], d_h[t - 1, i] = d_h[t - 1, i], d_h[t, i]
+                h_h[t, i], h_h[t - 1, i] = h_h[t - 1, i], h_h[t, i]
+        ctx.pt_swap(gx, gl, gd, gh, gb, dev(tc, us), swapped=sw_g)
+        assert np.array_equal(sw_g.cpu().numpy().astype(bool), done)
+        n_sw += int(done.sum())
+        assert np.array_equal(gx.cpu().numpy(), x), "positions are the same IEEE expression on both sides"
+        check_triplet((gl.reshape(-1), gd.reshape(-1), gh.reshape(-1)),
+                      {"logL": logL.reshape(-1), "d_h": d_h.reshape(-1), "h_h": h_h.reshape(-1)}, f"pt state it {it}")
+    assert n_acc > 50 and n_out > 5 and n_sw > 5                # every branch was exercised
+    best, bi, snr = sm.population_stats(logL, d_h, h_h)
+    got = ctx.pt_stats(gl, gd, gh).cpu().numpy()
+    assert int(got[1]) == bi and abs(got[0] - best) <= 1e-6 * max(1.0, abs(best)) and abs(got[2] - snr) <= 1e-9 * snr
+
+
+def test_pt_step_parity_full(orc, torch_cuda):
+    """the same move on the full-grid likelihood (Module 1): one iteration, 2 temperatures x 32 walkers"""
+    from oracle import sampler as sm
+    tc = torch_cuda
+    wl = wlm.make_workload(0)
+    d, run = oracle_setup_full(orc, wl)
+    ctx = make_ctx(wl)
+    g = wl.grid
+    ctx.set_data(g.n_f, g.k_min, g.df, dev(tc, d), dev(tc, wl.W))
+    rng = np.random.default_rng(194)
+    n_t, n_w = 2, 32
+    x = wl.params[:n_t * n_w].reshape(n_t, n_w, -1).copy()
+    x[:, :, 5:] = wl.params[0, 5:]
+
+    def ll(rows):
+        r = run(rows, d)
+        return r["logL"], {"d_h": r["d_h"], "h_h": r["h_h"]}
+    betas = np.array([1.0, 0.01])
+    lo, hi = _prior_box(wl, wl.params, 0.6)
+    l0, _ = ll(x.reshape(n_t * n_w, -1))
+    logL = l0.reshape(n_t, n_w).copy()
+    gx, gl = dev(tc, x), dev(tc, logL)
+    acc_g = tc.empty((n_t, n_w // 2), dtype=tc.int32, device="cuda")
+    for half in (0, 1):
+        u = rng.random((3, n_t, n_w // 2))
+        acc, _, _, _ = sm.stretch_half(x, logL, half, betas, lo, hi, 5, 2.0, u[0], u[1], u[2], ll)
+        ctx.pt_stretch_half(half, gx, gl, None, None, dev(tc, betas), dev(tc, lo), dev(tc, hi), 5, dev(tc, u[0]),
+                            dev(tc, u[1]), dev(tc, u[2]), accepted=acc_g, f_nodes=wl.f_nodes)
+        assert np.array_equal(acc_g.cpu().numpy().astype(bool), acc)
+    assert np.array_equal(gx.cpu().numpy(), x)
+    err = np.abs(gl.cpu().numpy() - logL) / np.maximum(1.0, np.abs(logL))
+    assert err.max() <= 1e-6
+    ctx.destroy()
+
+
+def test_stop_functions_match_oracle():
+    from oracle import sampler as sm
+    from paper_2111_01064_b200 import binding
+    assert binding.stop_snr(20.0, 20.0) and not binding.stop_snr(19.99, 20.0)
+    st, ref = binding.StopState(n_checks=3, tol=1.0), sm.StopConverged(3, 1.0)
+    for v in [-10.0, -5.0, -4.5, -4.2, -3.9, -2.0, -1.9, -1.8, -1.7, -1.65]:
+        assert binding.stop_converged(st, v) == ref.check(v)
