@@ -207,6 +207,58 @@ def bench_config(torch, index: int, steps: int, warmup: int, rank: int = 0, prof
     return res
 
 
+def bench_sampler_iteration(torch, ctx, wl, params, n_t: int = 10, n_w: int = 400, iters: int = 50):
+    """one sampler iteration at Module-2 size (10 temperatures x 400 walkers) on the
+    heterodyned likelihood: two half updates (propose, likelihood, accept), a temperature-swap sweep and the stopping
+    statistics — 8 launches of this library plus torch's uniform draws — timed eagerly and as a CUDA-graph replay
+    (the iteration never returns to the host)."""
+    P = params.shape[1]
+    x = params[: n_t * n_w].reshape(n_t, n_w, P).clone()
+    x[:, :, 5:] = params[0, 5:]                      # transfer factors frozen: 5 sampled coordinates
+    flat = x.reshape(-1, P)
+    c = flat[:, :5].mean(dim=0)
+    w = 3.0 * (flat[:, :5].max(dim=0).values - flat[:, :5].min(dim=0).values)
+    lo = torch.full((P,), -float("inf"), dtype=torch.float64, device=x.device)
+    hi = torch.full((P,), float("inf"), dtype=torch.float64, device=x.device)
+    lo[:5], hi[:5] = c - w, c + w
+    betas = torch.tensor([0.5 ** t for t in range(n_t - 1)] + [0.0], dtype=torch.float64, device=x.device)
+    logL, d_h, h_h = (v.reshape(n_t, n_w).clone() for v in ctx.het_batch_standin(flat.contiguous()))
+    out3 = torch.empty(3, dtype=torch.float64, device=x.device)
+    acc = torch.zeros((n_t, n_w // 2), dtype=torch.int32, device=x.device)
+    n_acc = torch.zeros((), dtype=torch.int64, device=x.device)
+
+    def iteration():
+        for half in (0, 1):
+            u = torch.rand((3, n_t, n_w // 2), dtype=torch.float64, device=x.device)
+            ctx.pt_stretch_half(half, x, logL, d_h, h_h, betas, lo, hi, 5, u[0], u[1], u[2], accepted=acc)
+            n_acc.add_(acc.sum())
+        ctx.pt_swap(x, logL, d_h, h_h, betas, torch.rand((n_t - 1, n_w), dtype=torch.float64, device=x.device))
+        ctx.pt_stats(logL[0], d_h[0], h_h[0], out3=out3)
+
+    for _ in range(5):
+        iteration()
+    ms_eager = time_steps(torch, iteration, iters, 0) / iters
+    res = {"n_temps": n_t, "n_walkers": n_w, "likelihood": "heterodyned, %d bins" % (len(wl.f_edges) - 1),
+           "ms_per_iteration_eager": ms_eager, "evals_per_s_eager": n_t * n_w / (ms_eager * 1e-3)}
+    try:
+        s = torch.cuda.Stream()
+        s.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(s):
+            iteration()
+            graph = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(graph, stream=s):
+                iteration()
+        torch.cuda.current_stream().wait_stream(s)
+        n_acc.zero_()
+        ms_graph = time_steps(torch, graph.replay, iters, 3) / iters
+        res.update({"ms_per_iteration_graph": ms_graph, "evals_per_s_graph": n_t * n_w / (ms_graph * 1e-3),
+                    "acceptance_fraction": float(n_acc) / ((iters + 3) * n_t * n_w),
+                    "max_logL_cold_chain": float(out3[0]), "extracted_snr_cold_chain": float(out3[2])})
+    except Exception as e:  # capture is a convenience of the harness, not part of the library
+        res["graph_error"] = repr(e)[:200]
+    return res
+
+
 def e2e_config(torch, res, steps: int, warmup: int):
     """same metric through the C ABI with HOST buffers: pinned params in, pinned results out, every step."""
     wl, ctx = res["wl"], res["ctx"]
@@ -428,6 +480,7 @@ def main():
                 per["cfg1_audit"] = {"evals_per_s": r["wl"].n_w / (ms_a * 1e-3), "ms_per_batch": ms_a, "n_walkers": r["wl"].n_w,
                                      "max_abs_het_minus_dense_logL": float((het[0] - o1[0]).abs().max()),
                                      "entry": "ll_het_audit_standin (direct template at every dense bin of the band)"}
+                per["module2_iteration"] = bench_sampler_iteration(torch, c1, r["wl"], p1)
             r["ctx"].destroy()
             del r
             torch.cuda.empty_cache()
