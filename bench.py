@@ -464,6 +464,22 @@ def main():
             r = bench_config(torch, idx, st, 5)
             per[f"cfg{idx}"] = {"evals_per_s": r["wl"].n_w / (r["ms_per_step"] * 1e-3), "ms_per_batch": r["ms_per_step"],
                                 "n_walkers": r["wl"].n_w}
+            if idx in (0, 1):
+                # ---- launch-bound configs: the same call replayed as a CUDA graph
+                try:
+                    sg = torch.cuda.Stream()
+                    sg.wait_stream(torch.cuda.current_stream())
+                    with torch.cuda.stream(sg):
+                        r["fn"]()
+                        gr = torch.cuda.CUDAGraph()
+                        with torch.cuda.graph(gr, stream=sg):
+                            r["fn"]()
+                    torch.cuda.current_stream().wait_stream(sg)
+                    ms_g = time_steps(torch, gr.replay, 200, 5) / 200
+                    per[f"cfg{idx}"].update({"ms_per_batch_graph": ms_g, "evals_per_s_graph": r["wl"].n_w / (ms_g * 1e-3)})
+                    del gr
+                except Exception as e:
+                    per[f"cfg{idx}"]["graph_error"] = repr(e)[:200]
             if idx == 1:
                 # ---- the reference update inside the loop (every 5000 iterations)
                 # and the brute-force audit of the heterodyned values, config-1 size
