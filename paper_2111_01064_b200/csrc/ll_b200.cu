@@ -332,8 +332,16 @@ int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, cons
     }
     LAUNCHED(ctx);
     {
-        dim3 grid(ceil_div(n_wp, 128), ns * n_m);
-        k_spline<<<grid, 128, 0, st>>>(ctx->Y.as<double>(), ctx->C.as<double>(), n_wp, n_nodes, n_m, ns, ctx->nt);
+        // few systems (Module-1 sized batches): one warp per system, scan-based sweeps; else one thread per system
+        const long long n_sys = (long long)n_wp * ns * n_m;
+        const size_t smem_w = sizeof(double) * 2 * (size_t)n_nodes * kSplineWarpsPerBlock;
+        if (n_sys <= (long long)ctx->sm_count * 32 && smem_w <= 48 * 1024) {
+            k_spline_warp<<<(unsigned)ceil_div(n_sys, kSplineWarpsPerBlock), 32 * kSplineWarpsPerBlock, smem_w, st>>>(
+                ctx->Y.as<double>(), ctx->C.as<double>(), n_wp, n_nodes, n_m, ns, ctx->nt);
+        } else {
+            dim3 grid(ceil_div(n_wp, 128), ns * n_m);
+            k_spline<<<grid, 128, 0, st>>>(ctx->Y.as<double>(), ctx->C.as<double>(), n_wp, n_nodes, n_m, ns, ctx->nt);
+        }
         LAUNCHED(ctx);
     }
     FusedArgs fa;

@@ -446,6 +446,89 @@ k_spline(const double *__restrict__ Y, double *__restrict__ C, int n_wp, int n_n
 }
 
 // ---------------------------------------------------------------------------------------------------
+// F2 for small batches (Module-1 sized: tens to hundreds of walkers): one WARP per system.  With
+// few systems the thread-per-system kernel above is a chain of 2 (n-2) dependent steps on a nearly empty GPU.
+// Both Thomas sweeps are first-order linear recurrences x_j = alpha_j + beta_j x_{j-1}, i.e. compositions of
+// affine maps, which are associative: each lane composes the maps of its ceil(n/32) consecutive rows, a warp
+// scan composes across lanes, and each lane then re-runs its rows from the right start value.  Dependent chain:
+// 2 ceil(n/32) + 5 steps instead of n.  Same factorisation tables; results differ from the sequential sweep
+// by rounding only.  Shared memory per warp: node values and dp / M, 2 n doubles.
+// ---------------------------------------------------------------------------------------------------
+constexpr int kSplineWarpsPerBlock = 2;
+__global__ void __launch_bounds__(32 * kSplineWarpsPerBlock)
+k_spline_warp(const double *__restrict__ Y, double *__restrict__ C, int n_wp, int n_nodes, int n_m, int ns, NodeTables nt)
+{
+    extern __shared__ double ssm[];
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    const long long gsys = (long long)blockIdx.x * kSplineWarpsPerBlock + wib;
+    if (gsys >= (long long)n_m * ns * n_wp) return; // whole warp
+    const int sys = (int)(gsys / n_wp), p = (int)(gsys - (long long)sys * n_wp);
+    const int m = sys / ns, kind = sys % ns;
+    const int n = n_nodes;
+    const size_t sw = (size_t)n_wp;
+    double *ys = ssm + (size_t)wib * 2 * n, *ds = ys + n;
+    for (int j = lane; j < n; j += 32) ys[j] = __ldg(Y + ((size_t)sys * n + j) * sw + p);
+    __syncwarp();
+    const int L = (n + 31) / 32;
+    const int j0 = lane * L, j1 = min(j0 + L, n);
+    auto rhs = [&](int j) { return (ys[j + 1] - ys[j]) * __ldg(nt.invh + j) - (ys[j] - ys[j - 1]) * __ldg(nt.invh + j - 1); };
+    // ---- forward sweep: dp_j = (r_j - a_j dp_{j-1}) / den_j for j = 1..n-2, dp_0 = 0
+    double A = 0.0, B = 1.0; // dp at the end of this lane's rows = A + B * dp before them
+    for (int j = j0; j < j1; ++j)
+        if (j >= 1 && j <= n - 2) {
+            const double ti = __ldg(nt.tinv + j), be = -__ldg(nt.ta + j) * ti;
+            A = fma(be, A, rhs(j) * ti);
+            B *= be;
+        }
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { // inclusive scan: this lane's map after the maps of the lanes below
+        const double Ap = __shfl_up_sync(0xffffffffu, A, o), Bp = __shfl_up_sync(0xffffffffu, B, o);
+        if (lane >= o) { A = fma(B, Ap, A); B *= Bp; }
+    }
+    double start = __shfl_up_sync(0xffffffffu, A, 1); // the maps below applied to dp_0 = 0
+    if (lane == 0) start = 0.0;
+    for (int j = j0; j < j1; ++j) {
+        if (j >= 1 && j <= n - 2) start = (rhs(j) - __ldg(nt.ta + j) * start) * __ldg(nt.tinv + j);
+        ds[j] = (j >= 1 && j <= n - 2) ? start : 0.0;
+    }
+    __syncwarp();
+    // ---- backward sweep: M_j = dp_j - c'_j M_{j+1} for j = n-2..1, M_0 = M_{n-1} = 0
+    A = 0.0; B = 1.0; // M at this lane's first row = A + B * M just above its last row
+    for (int j = j1 - 1; j >= j0; --j) {
+        if (j >= 1 && j <= n - 2) {
+            const double be = -__ldg(nt.tcp + j);
+            A = fma(be, A, ds[j]);
+            B *= be;
+        } else { A = 0.0; B = 0.0; }
+    }
+    if (j0 >= j1) { A = 0.0; B = 1.0; } // a lane without rows is the identity
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const double Ap = __shfl_down_sync(0xffffffffu, A, o), Bp = __shfl_down_sync(0xffffffffu, B, o);
+        if (lane + o < 32) { A = fma(B, Ap, A); B *= Bp; }
+    }
+    double Mn = __shfl_down_sync(0xffffffffu, A, 1); // the maps above applied to M = 0 beyond the last node
+    if (lane == 31) Mn = 0.0;
+    for (int j = j1 - 1; j >= j0; --j) {
+        Mn = (j >= 1 && j <= n - 2) ? fma(-__ldg(nt.tcp + j), Mn, ds[j]) : 0.0;
+        ds[j] = Mn;
+    }
+    __syncwarp();
+    // ---- coefficients of interval j (same formulas as k_spline)
+    double *c = C + ((size_t)m * ns * 4 + kind * 4) * sw + p;
+    const size_t cj = (size_t)n_m * ns * 4 * sw;
+    for (int j = lane; j < n - 1; j += 32) {
+        const double y0 = ys[j], y1 = ys[j + 1], Mj = ds[j], Mn1 = ds[j + 1];
+        const double h = __ldg(nt.hj + j), ih = __ldg(nt.invh + j);
+        double *cc = c + (size_t)j * cj;
+        cc[0] = y0;
+        cc[sw] = (y1 - y0) * ih - h * (2.0 * Mj + Mn1) * kSixth;
+        cc[2 * sw] = 0.5 * Mj;
+        cc[3 * sw] = (Mn1 - Mj) * ih * kSixth;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
 // F3: fused spline evaluation / channel response / inner products           (Eq. 3, 7, 9)
 // One thread = one walker; a warp = 32 walkers walking the SAME dense bins, so the data tile (g4, W) is a
 // shared-memory broadcast and no cross-thread reduction exists.  Tiles of g4/W arrive by 1-D bulk TMA into
