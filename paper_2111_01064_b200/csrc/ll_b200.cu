@@ -84,6 +84,11 @@ struct ll_ctx {
     // node-set cache
     std::vector<double> nodes_host;
     bool nodes_valid = false;
+    std::vector<int> bstart_host;  // bin -> interval table of the current node set (host copy)
+    long long nodes_version = 0;   // bumped whenever the node tables are rebuilt
+    DevBuf tile_tab;               // frequency-tile boundaries of the fused kernel [n_tiles + 1]
+    long long tile_key_version = -1;
+    int tile_key_TB = -1, tile_key_small = -1, tile_n = 0;
     DevBuf node_tab; // doubles then ints
     NodeTables nt{};
 
@@ -250,6 +255,8 @@ int prepare_nodes(ll_ctx *ctx, int n, const double *x, cudaStream_t st)
     nt.f4 = b + 6 * n; nt.cfp = b + 7 * n; nt.f2m = nt.cfp + (size_t)n_m * n; nt.fm53 = nt.f2m + (size_t)n_m * n;
     nt.bstart = reinterpret_cast<const int *>((const char *)ctx->node_tab.p + bytes_d);
     ctx->nodes_host.assign(x, x + n);
+    ctx->bstart_host = hi;
+    ctx->nodes_version += 1;
     ctx->nodes_valid = true;
     return LL_OK;
 }
@@ -276,6 +283,53 @@ FullPlan make_plan(const ll_ctx *ctx, long long n_w)
     return pl;
 }
 
+// Frequency tiles of the fused kernel.  Large batches: uniform tiles of TB bins.  Small batches (latency matters:
+// Module-1 sized): a tile is also limited by the spline intervals it crosses, since every interval
+// change costs one dependent global load of the coefficients (~14 bins' worth of arithmetic) and log-spaced nodes
+// put dozens of intervals into the first tiles of the grid; cost = bins + 14 per interval <= TB.
+int ensure_tiles(ll_ctx *ctx, FullPlan &pl, cudaStream_t st)
+{
+    const int small = pl.n_wp <= 1024 ? 1 : 0;
+    if (ctx->tile_key_version == ctx->nodes_version && ctx->tile_key_TB == pl.TB && ctx->tile_key_small == small) {
+        pl.n_tiles = ctx->tile_n;
+        return LL_OK;
+    }
+    const int n_f = (int)ctx->n_f, n = (int)ctx->bstart_host.size();
+    std::vector<int> ts;
+    ts.push_back(0);
+    if (!small) {
+        for (int i = pl.TB; i < n_f; i += pl.TB) ts.push_back(i);
+    } else {
+        const int kIntervalCost = 14;
+        int end = 0, j = 0;
+        while (end < n_f) {
+            int cost = 0;
+            const int start = end;
+            while (end < n_f) {
+                while (j < n - 2 && ctx->bstart_host[j + 1] <= end) ++j;
+                const int seg_end = (j < n - 2) ? ctx->bstart_host[j + 1] : n_f;
+                const int room = pl.TB - cost - kIntervalCost;
+                if (room <= 0 && end > start) break;
+                const int take = std::min(seg_end - end, std::max(room, 1));
+                end += take;
+                cost += take + kIntervalCost;
+            }
+            ts.push_back(end);
+        }
+        ts.pop_back();
+    }
+    ts.push_back(n_f);
+    pl.n_tiles = (int)ts.size() - 1;
+    CK(ctx->tile_tab.ensure(sizeof(int) * ts.size()));
+    CK(cudaMemcpyAsync(ctx->tile_tab.p, ts.data(), sizeof(int) * ts.size(), cudaMemcpyHostToDevice, st));
+    CK(cudaStreamSynchronize(st)); // ts goes out of scope
+    ctx->tile_key_version = ctx->nodes_version;
+    ctx->tile_key_TB = pl.TB;
+    ctx->tile_key_small = small;
+    ctx->tile_n = pl.n_tiles;
+    return LL_OK;
+}
+
 // the whole full-grid pipeline for walkers [0, n_w) given either stand-in params or caller arrays
 int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, const double *amp, const double *phase,
              const double *tf, const double *band, double *logL, double *d_h, double *h_h, cudaStream_t st,
@@ -286,7 +340,11 @@ int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, cons
     const int ns = tfp ? 6 : 2;
     const int n_m = ctx->n_m;
     const int P = 5 + 2 * kNC * n_m;
-    const FullPlan pl = make_plan(ctx, n_w);
+    FullPlan pl = make_plan(ctx, n_w);
+    {
+        const int rc_t = ensure_tiles(ctx, pl, st);
+        if (rc_t != LL_OK) return rc_t;
+    }
     const int n_wp = pl.n_wp;
     const bool nm1 = (n_m == 1);
     const int NQ = (nm1 && !tfp) ? 5 : 2;
@@ -349,6 +407,7 @@ int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, cons
     fa.xj = ctx->nt.xj; fa.bstart = ctx->nt.bstart; fa.ilo = ctx->ilo_s.as<int>(); fa.ihi = ctx->ihi_s.as<int>();
     fa.part = ctx->part.as<double>(); fa.k_min = ctx->k_min; fa.df = ctx->df; fa.n_f = (int)ctx->n_f; fa.n_wp = n_wp;
     fa.n_nodes = n_nodes; fa.n_m = n_m; fa.TB = pl.TB; fa.CH = pl.CH;
+    fa.tile_start = ctx->tile_tab.as<int>();
     if (template_only) {
         // sorted position of walker 0 of a one-walker batch is 0
         k_full_template<<<ceil_div(ctx->n_f, 256), 256, 0, st>>>(fa, 0, h_out);
@@ -373,11 +432,11 @@ int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, cons
     }
     if (nm1 && !tfp)
         k_finalize<1><<<ceil_div(n_wp, 32), dim3(32, kFinY), 0, st>>>(ctx->part.as<double>(), ctx->TF.as<double>(), ctx->perm.as<int>(),
-                                                           ctx->ilo_s.as<int>(), ctx->ihi_s.as<int>(), n_wp, pl.TB,
+                                                           ctx->ilo_s.as<int>(), ctx->ihi_s.as<int>(), n_wp, ctx->tile_tab.as<int>(), pl.n_tiles,
                                                            ctx->dd.as<double>(), logL, d_h, h_h);
     else
         k_finalize<0><<<ceil_div(n_wp, 32), dim3(32, kFinY), 0, st>>>(ctx->part.as<double>(), ctx->TF.as<double>(), ctx->perm.as<int>(),
-                                                           ctx->ilo_s.as<int>(), ctx->ihi_s.as<int>(), n_wp, pl.TB,
+                                                           ctx->ilo_s.as<int>(), ctx->ihi_s.as<int>(), n_wp, ctx->tile_tab.as<int>(), pl.n_tiles,
                                                            ctx->dd.as<double>(), logL, d_h, h_h);
     LAUNCHED(ctx);
     return LL_OK;
@@ -642,7 +701,7 @@ int ll_destroy(ll_ctx *ctx)
                          &ctx->key_w, &ctx->hist, &ctx->perm, &ctx->ilo_s, &ctx->ihi_s, &ctx->Y, &ctx->C, &ctx->TF,
                          &ctx->part, &ctx->prow, &ctx->het_tab, &ctx->het_tab1, &ctx->het_raw, &ctx->het_idx, &ctx->het_fb,
                          &ctx->stage_in, &ctx->stage_out, &ctx->g4f, &ctx->Wf, &ctx->scale, &ctx->wmax, &ctx->ref_idx,
-                         &ctx->ref_dense, &ctx->ref_edges, &ctx->pt_y, &ctx->pt_out, &ctx->pt_in};
+                         &ctx->ref_dense, &ctx->ref_edges, &ctx->tile_tab, &ctx->pt_y, &ctx->pt_out, &ctx->pt_in};
         for (DevBuf *b : all) b->release();
         for (auto &e : ctx->ev) cudaEventDestroy(e);
     }

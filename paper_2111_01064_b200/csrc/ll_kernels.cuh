@@ -548,8 +548,20 @@ struct FusedArgs {
     double *part;
     long long k_min;
     double df;
+    const int *tile_start; // [n_tiles + 1]: frequency tile t covers dense bins [tile_start[t], tile_start[t+1])
     int n_f, n_wp, n_nodes, n_m, TB, CH;
 };
+
+// largest t in [0, n_tiles-1] with tile_start[t] <= i
+__device__ __forceinline__ int tile_of_bin(const int *__restrict__ tile_start, int n_tiles, int i)
+{
+    int lo = 0, hi = n_tiles - 1;
+    while (lo < hi) {
+        const int mid = (lo + hi + 1) >> 1;
+        if (__ldg(tile_start + mid) <= i) lo = mid; else hi = mid - 1;
+    }
+    return lo;
+}
 
 __device__ __forceinline__ int find_interval_of_bin(const int *__restrict__ bstart, int n_nodes, int i)
 {
@@ -606,8 +618,7 @@ __global__ void __launch_bounds__(128, LL_FUSED_MINB) k_full_fused(FusedArgs a)
     const int tid = threadIdx.x;
     const int p = blockIdx.x * blockDim.x + tid;
     const int tile = blockIdx.y;
-    const int i0 = tile * a.TB;
-    const int i1 = min(i0 + a.TB, a.n_f);
+    const int i0 = __ldg(a.tile_start + tile), i1 = __ldg(a.tile_start + tile + 1); // tile = dense bins [i0, i1)
     const int lo = max(a.ilo[p], i0), hi = min(a.ihi[p], i1);
     if (tid == 0) {
         s_lo = INT_MAX;
@@ -879,8 +890,7 @@ __global__ void __launch_bounds__(128, 4) k_full_fused_mixed(FusedArgs a, FusedA
     const int tid = threadIdx.x;
     const int p = blockIdx.x * blockDim.x + tid;
     const int tile = blockIdx.y;
-    const int i0 = tile * a.TB;
-    const int i1 = min(i0 + a.TB, a.n_f);
+    const int i0 = __ldg(a.tile_start + tile), i1 = __ldg(a.tile_start + tile + 1); // tile = dense bins [i0, i1)
     const int lo = max(a.ilo[p], i0), hi = min(a.ihi[p], i1);
     if (tid == 0) {
         s_lo = INT_MAX;
@@ -991,8 +1001,7 @@ __global__ void __launch_bounds__(128, 3) k_full_fused_tf(FusedArgs a)
     const int tid = threadIdx.x;
     const int p = blockIdx.x * blockDim.x + tid;
     const int tile = blockIdx.y;
-    const int i0 = tile * a.TB;
-    const int i1 = min(i0 + a.TB, a.n_f);
+    const int i0 = __ldg(a.tile_start + tile), i1 = __ldg(a.tile_start + tile + 1); // tile = dense bins [i0, i1)
     const int lo = max(a.ilo[p], i0), hi = min(a.ihi[p], i1);
     if (tid == 0) {
         s_lo = INT_MAX;
@@ -1141,8 +1150,9 @@ constexpr int kFinY = 8;
 template <int NM1>
 __global__ void __launch_bounds__(32 * kFinY)
 k_finalize(const double *__restrict__ part, const double *__restrict__ TF, const int *__restrict__ perm,
-           const int *__restrict__ ilo, const int *__restrict__ ihi, int n_wp, int TB, const double *__restrict__ dd,
-           double *__restrict__ logL, double *__restrict__ d_h, double *__restrict__ h_h)
+           const int *__restrict__ ilo, const int *__restrict__ ihi, int n_wp, const int *__restrict__ tile_start,
+           int n_tiles, const double *__restrict__ dd, double *__restrict__ logL, double *__restrict__ d_h,
+           double *__restrict__ h_h)
 {
     constexpr int NQ = NM1 ? 5 : 2;
     __shared__ double red[kFinY][NQ][32];
@@ -1154,8 +1164,8 @@ k_finalize(const double *__restrict__ part, const double *__restrict__ TF, const
 #pragma unroll
     for (int q = 0; q < NQ; ++q) acc[q] = 0.0;
     if (hi > lo) {
-        const int t1 = (hi - 1) / TB;
-        for (int t = lo / TB + ty; t <= t1; t += kFinY) {
+        const int t0 = tile_of_bin(tile_start, n_tiles, lo), t1 = tile_of_bin(tile_start, n_tiles, hi - 1);
+        for (int t = t0 + ty; t <= t1; t += kFinY) {
             const double *o = part + ((size_t)t * NQ) * sw + p;
 #pragma unroll
             for (int q = 0; q < NQ; ++q) acc[q] += o[q * sw];
