@@ -363,18 +363,24 @@ int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, cons
     if (!template_only) CK(ctx->part.ensure(sizeof(double) * (size_t)pl.n_tiles * NQ * n_wp));
 
     const GridInfo g{ctx->k_min, ctx->n_f, ctx->df};
-    CK(cudaMemsetAsync(ctx->hist.p, 0, sizeof(int) * pl.n_keys, st));
-    CK(cudaMemsetAsync(ctx->pairs.p, 0, sizeof(unsigned long long), st));
-    k_band_prep<<<ceil_div(n_w, 256), 256, 0, st>>>(standin ? 1 : 0, params, P, band, (int)n_w, g, ctx->si, pl.key_gran,
-                                                    ctx->ilo_w.as<int>(), ctx->ihi_w.as<int>(), ctx->key_w.as<int>(),
-                                                    ctx->hist.as<int>(), ctx->pairs.as<unsigned long long>());
-    LAUNCHED(ctx);
-    k_scan_hist<<<1, 1024, 0, st>>>(ctx->hist.as<int>(), pl.n_keys);
-    LAUNCHED(ctx);
-    k_scatter<<<ceil_div(n_wp, 256), 256, 0, st>>>((int)n_w, n_wp, ctx->key_w.as<int>(), ctx->ilo_w.as<int>(),
-                                                   ctx->ihi_w.as<int>(), ctx->hist.as<int>(), ctx->perm.as<int>(),
-                                                   ctx->ilo_s.as<int>(), ctx->ihi_s.as<int>());
-    LAUNCHED(ctx);
+    if (n_w <= 1024 && n_wp <= 1024) {
+        k_band_sort_small<<<1, 1024, 0, st>>>(standin ? 1 : 0, params, P, band, (int)n_w, n_wp, g, ctx->si, ctx->perm.as<int>(),
+                                              ctx->ilo_s.as<int>(), ctx->ihi_s.as<int>(), ctx->pairs.as<unsigned long long>());
+        LAUNCHED(ctx);
+    } else {
+        CK(cudaMemsetAsync(ctx->hist.p, 0, sizeof(int) * pl.n_keys, st));
+        CK(cudaMemsetAsync(ctx->pairs.p, 0, sizeof(unsigned long long), st));
+        k_band_prep<<<ceil_div(n_w, 256), 256, 0, st>>>(standin ? 1 : 0, params, P, band, (int)n_w, g, ctx->si, pl.key_gran,
+                                                        ctx->ilo_w.as<int>(), ctx->ihi_w.as<int>(), ctx->key_w.as<int>(),
+                                                        ctx->hist.as<int>(), ctx->pairs.as<unsigned long long>());
+        LAUNCHED(ctx);
+        k_scan_hist<<<1, 1024, 0, st>>>(ctx->hist.as<int>(), pl.n_keys);
+        LAUNCHED(ctx);
+        k_scatter<<<ceil_div(n_wp, 256), 256, 0, st>>>((int)n_w, n_wp, ctx->key_w.as<int>(), ctx->ilo_w.as<int>(),
+                                                       ctx->ihi_w.as<int>(), ctx->hist.as<int>(), ctx->perm.as<int>(),
+                                                       ctx->ilo_s.as<int>(), ctx->ihi_s.as<int>());
+        LAUNCHED(ctx);
+    }
     if (standin) {
         dim3 grid(ceil_div(n_wp, 128), ceil_div(n_nodes, kNodesPerThread));
         k_nodes_standin<<<grid, 128, 0, st>>>(params, P, ctx->perm.as<int>(), n_wp, n_nodes, ctx->si, ctx->nt,

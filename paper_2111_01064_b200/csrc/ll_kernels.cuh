@@ -89,7 +89,31 @@ __device__ __forceinline__ void standin_masses(double Mc, double q, double &Mtot
     f_isco = 0x1.16b28f55d72d4p-4 / (kPi * Mtot); // 6^(-3/2) = 0.06804138174397717
 }
 
-// mode 0: stand-in parameters (params row stride P); mode 1: band array [n_w][2] or NULL
+// bin range [lo, hi) of walker w's band: stand-in parameters (reading R10), a caller band [n_w][2], or the whole grid
+__device__ __forceinline__ void band_bins(int use_standin, const double *__restrict__ params, int P,
+                                          const double *__restrict__ band, int w, const GridInfo &g, const StandinInfo &si,
+                                          long long &lo, long long &hi)
+{
+    double f_lo, f_hi;
+    if (use_standin) {
+        double Mtot, eta, fi;
+        standin_masses(params[(size_t)w * P], params[(size_t)w * P + 1], Mtot, eta, fi);
+        f_lo = bin_freq(g.k_min, 0, g.df);
+        const double top = (1.0 + si.kappa) * fi * (0.5 * (double)si.m_max);
+        const double f_last = bin_freq(g.k_min, g.n_f - 1, g.df);
+        f_hi = (top < f_last) ? top : f_last;
+    } else if (band) {
+        f_lo = band[2 * (size_t)w];
+        f_hi = band[2 * (size_t)w + 1];
+    } else {
+        f_lo = -INFINITY;
+        f_hi = INFINITY;
+    }
+    lo = first_bin_ge(f_lo, g.k_min, g.n_f, g.df);
+    hi = first_bin_gt(f_hi, g.k_min, g.n_f, g.df);
+    if (!(f_lo <= f_hi) || hi <= lo) { lo = 0; hi = 0; }
+}
+
 __global__ void __launch_bounds__(256)
 k_band_prep(int use_standin, const double *__restrict__ params, int P, const double *__restrict__ band, int n_w,
             GridInfo g, StandinInfo si, int key_gran, int *__restrict__ ilo_w, int *__restrict__ ihi_w,
@@ -98,24 +122,8 @@ k_band_prep(int use_standin, const double *__restrict__ params, int P, const dou
     const int w = blockIdx.x * blockDim.x + threadIdx.x;
     long long span = 0;
     if (w < n_w) {
-        double f_lo, f_hi;
-        if (use_standin) {
-            double Mtot, eta, fi;
-            standin_masses(params[(size_t)w * P], params[(size_t)w * P + 1], Mtot, eta, fi);
-            f_lo = bin_freq(g.k_min, 0, g.df);
-            const double top = (1.0 + si.kappa) * fi * (0.5 * (double)si.m_max);
-            const double f_last = bin_freq(g.k_min, g.n_f - 1, g.df);
-            f_hi = (top < f_last) ? top : f_last;
-        } else if (band) {
-            f_lo = band[2 * (size_t)w];
-            f_hi = band[2 * (size_t)w + 1];
-        } else {
-            f_lo = -INFINITY;
-            f_hi = INFINITY;
-        }
-        long long lo = first_bin_ge(f_lo, g.k_min, g.n_f, g.df);
-        long long hi = first_bin_gt(f_hi, g.k_min, g.n_f, g.df);
-        if (!(f_lo <= f_hi) || hi <= lo) { lo = 0; hi = 0; }
+        long long lo, hi;
+        band_bins(use_standin, params, P, band, w, g, si, lo, hi);
         ilo_w[w] = (int)lo;
         ihi_w[w] = (int)hi;
         const int key = (int)(hi / key_gran);
@@ -128,6 +136,47 @@ k_band_prep(int use_standin, const double *__restrict__ params, int P, const dou
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
     if ((threadIdx.x & 31) == 0 && s) atomicAdd(pairs, s * (unsigned long long)si.n_m);
+}
+
+// The same three steps (band -> bin range, sort by band top, scatter) for batches of up to 1024 walkers in ONE
+// block (Module-1 sized batches are latency-bound: one launch instead of three plus two memsets).  Rank of a walker
+// = number of walkers with a smaller (top bin, index): an O(n^2) count over shared memory, n <= 1024.
+__global__ void __launch_bounds__(1024)
+k_band_sort_small(int use_standin, const double *__restrict__ params, int P, const double *__restrict__ band, int n_w,
+                  int n_wp, GridInfo g, StandinInfo si, int *__restrict__ perm, int *__restrict__ ilo_s,
+                  int *__restrict__ ihi_s, unsigned long long *__restrict__ pairs)
+{
+    __shared__ int s_hi[1024];
+    __shared__ unsigned long long s_span[32];
+    const int w = threadIdx.x;
+    long long lo = 0, hi = 0;
+    if (w < n_w) band_bins(use_standin, params, P, band, w, g, si, lo, hi);
+    s_hi[w] = (w < n_w) ? (int)hi : INT_MAX;
+    unsigned long long s = (unsigned long long)(hi - lo);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if ((w & 31) == 0) s_span[w >> 5] = s;
+    __syncthreads();
+    if (w == 0) {
+        unsigned long long t = 0;
+        for (int k = 0; k < 32; ++k) t += s_span[k];
+        pairs[0] = t * (unsigned long long)si.n_m;
+    }
+    if (w < n_w) {
+        const int mine = (int)hi;
+        int rank = 0;
+        for (int k = 0; k < n_w; ++k) {
+            const int other = s_hi[k];
+            rank += (other < mine) || (other == mine && k < w);
+        }
+        perm[rank] = w;
+        ilo_s[rank] = (int)lo;
+        ihi_s[rank] = (int)hi;
+    } else if (w < n_wp) {
+        perm[w] = -1;
+        ilo_s[w] = 0;
+        ihi_s[w] = 0;
+    }
 }
 
 // exclusive scan of hist[0..n) in place (single block of 1024 threads, n <= 1024*8)
@@ -1146,7 +1195,7 @@ k_tlm_nodes(const double *__restrict__ phase, int n_sys, int n_nodes, double t_r
 // F4: reduce the per-tile partials in a fixed order, apply T^c (single mode), form log L        (Eq. 2)
 // Block = 32 walkers x kFinY tile slices: slice ty sums tiles t0 + ty, t0 + ty + kFinY, ... of its walker, the
 // slices meet in shared memory and are added in slice order (deterministic: reruns are bit-identical).
-constexpr int kFinY = 8;
+constexpr int kFinY = 32;
 template <int NM1>
 __global__ void __launch_bounds__(32 * kFinY)
 k_finalize(const double *__restrict__ part, const double *__restrict__ TF, const int *__restrict__ perm,
@@ -1165,6 +1214,7 @@ k_finalize(const double *__restrict__ part, const double *__restrict__ TF, const
     for (int q = 0; q < NQ; ++q) acc[q] = 0.0;
     if (hi > lo) {
         const int t0 = tile_of_bin(tile_start, n_tiles, lo), t1 = tile_of_bin(tile_start, n_tiles, hi - 1);
+#pragma unroll 4
         for (int t = t0 + ty; t <= t1; t += kFinY) {
             const double *o = part + ((size_t)t * NQ) * sw + p;
 #pragma unroll
