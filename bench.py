@@ -207,11 +207,11 @@ def bench_config(torch, index: int, steps: int, warmup: int, rank: int = 0, prof
     return res
 
 
-def bench_sampler_iteration(torch, ctx, wl, params, n_t: int = 10, n_w: int = 400, iters: int = 50):
-    """one sampler iteration at Module-2 size (10 temperatures x 400 walkers) on the
-    heterodyned likelihood: two half updates (propose, likelihood, accept), a temperature-swap sweep and the stopping
-    statistics — 8 launches of this library plus torch's uniform draws — timed eagerly and as a CUDA-graph replay
-    (the iteration never returns to the host)."""
+def bench_sampler_iteration(torch, ctx, wl, params, n_t: int = 10, n_w: int = 400, iters: int = 50, f_nodes=None):
+    """one sampler iteration — two half updates (propose, likelihood, accept), a temperature-swap
+    sweep and the stopping statistics — timed eagerly and as a CUDA-graph replay (the iteration never returns to the
+    host).  Default: Module-2 size (10 temperatures x 400 walkers, PAPER.md:212) on the heterodyned likelihood;
+    with f_nodes: the full-grid likelihood (Module 1: 4 temperatures x 80 walkers)."""
     P = params.shape[1]
     x = params[: n_t * n_w].reshape(n_t, n_w, P).clone()
     x[:, :, 5:] = params[0, 5:]                      # transfer factors frozen: 5 sampled coordinates
@@ -222,7 +222,8 @@ def bench_sampler_iteration(torch, ctx, wl, params, n_t: int = 10, n_w: int = 40
     hi = torch.full((P,), float("inf"), dtype=torch.float64, device=x.device)
     lo[:5], hi[:5] = c - w, c + w
     betas = torch.tensor([0.5 ** t for t in range(n_t - 1)] + [0.0], dtype=torch.float64, device=x.device)
-    logL, d_h, h_h = (v.reshape(n_t, n_w).clone() for v in ctx.het_batch_standin(flat.contiguous()))
+    first = ctx.het_batch_standin(flat.contiguous()) if f_nodes is None else ctx.full_batch_standin(f_nodes, flat.contiguous())
+    logL, d_h, h_h = (v.reshape(n_t, n_w).clone() for v in first)
     out3 = torch.empty(3, dtype=torch.float64, device=x.device)
     acc = torch.zeros((n_t, n_w // 2), dtype=torch.int32, device=x.device)
     n_acc = torch.zeros((), dtype=torch.int64, device=x.device)
@@ -230,7 +231,7 @@ def bench_sampler_iteration(torch, ctx, wl, params, n_t: int = 10, n_w: int = 40
     def iteration():
         for half in (0, 1):
             u = torch.rand((3, n_t, n_w // 2), dtype=torch.float64, device=x.device)
-            ctx.pt_stretch_half(half, x, logL, d_h, h_h, betas, lo, hi, 5, u[0], u[1], u[2], accepted=acc)
+            ctx.pt_stretch_half(half, x, logL, d_h, h_h, betas, lo, hi, 5, u[0], u[1], u[2], accepted=acc, f_nodes=f_nodes)
             n_acc.add_(acc.sum())
         ctx.pt_swap(x, logL, d_h, h_h, betas, torch.rand((n_t - 1, n_w), dtype=torch.float64, device=x.device))
         ctx.pt_stats(logL[0], d_h[0], h_h[0], out3=out3)
@@ -238,7 +239,9 @@ def bench_sampler_iteration(torch, ctx, wl, params, n_t: int = 10, n_w: int = 40
     for _ in range(5):
         iteration()
     ms_eager = time_steps(torch, iteration, iters, 0) / iters
-    res = {"n_temps": n_t, "n_walkers": n_w, "likelihood": "heterodyned, %d bins" % (len(wl.f_edges) - 1),
+    res = {"n_temps": n_t, "n_walkers": n_w,
+           "likelihood": ("heterodyned, %d bins" % (len(wl.f_edges) - 1)) if f_nodes is None else
+                         ("full grid, %d bins, %d nodes" % (wl.grid.n_f, len(f_nodes))),
            "ms_per_iteration_eager": ms_eager, "evals_per_s_eager": n_t * n_w / (ms_eager * 1e-3)}
     try:
         s = torch.cuda.Stream()
@@ -533,6 +536,9 @@ def main():
                               "algorithmic_slots_per_pair": SLOTS_FULL_TF,
                               "frac": pairs2 * SLOTS_FULL_TF / (kms / max(kn, 1) * 1e-3) / peak_slots,
                               "entry": "ll_full_batch_tf (amp, phase, T at 1024 nodes as device arrays; the walkers' own bands)"}
+            # ---- Module-1 sized sampler iteration on the full-grid likelihood of the same one-year data stream
+            per["module1_iteration"] = bench_sampler_iteration(torch, c2, wl2, b2["params"], n_t=4, n_w=80, iters=20,
+                                                               f_nodes=wl2.f_nodes)
             c2.destroy()
             del amp, ph, tfn, b2
             torch.cuda.empty_cache()

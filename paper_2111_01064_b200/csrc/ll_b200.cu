@@ -270,8 +270,10 @@ FullPlan make_plan(const ll_ctx *ctx, long long n_w)
     pl.WB = (n_w >= 4096) ? 128 : (n_w >= 1024 ? 64 : 32);
     pl.n_wp = (int)round_up(std::max<long long>(n_w, 1), pl.WB);
     const int n_wb = pl.n_wp / pl.WB;
-    // aim at ~16 blocks per SM over the whole grid, tiles between 64 and 4096 bins
-    const long long target = (long long)ctx->sm_count * 16;
+    // aim at ~16 blocks per SM over the whole grid, tiles between 64 and 4096 bins.  Small batches (blocks of one
+    // warp, most tiles beyond the walkers' bands and exiting at once): 8x as many, smaller tiles, so that the active
+    // ones still fill the SMs (measured on 160 walkers x 1.57e6 bins: TB 4096 -> 512 halves the fused kernel's time)
+    const long long target = (long long)ctx->sm_count * (pl.n_wp <= 1024 ? 128 : 16);
     long long tb = ctx->n_f * n_wb / target;
     int TB = 64;
     while (TB < 4096 && TB < tb) TB <<= 1;
@@ -398,10 +400,12 @@ int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, cons
     {
         // few systems (Module-1 sized batches): one warp per system, scan-based sweeps; else one thread per system
         const long long n_sys = (long long)n_wp * ns * n_m;
-        const size_t smem_w = sizeof(double) * 2 * (size_t)n_nodes * kSplineWarpsPerBlock;
+        int T = 32;
+        while (T < 256 && T * 4 < n_nodes) T <<= 1; // ~4 rows per thread
+        const size_t smem_w = sizeof(double) * (2 * (size_t)n_nodes + T);
         if (n_sys <= (long long)ctx->sm_count * 32 && smem_w <= 48 * 1024) {
-            k_spline_warp<<<(unsigned)ceil_div(n_sys, kSplineWarpsPerBlock), 32 * kSplineWarpsPerBlock, smem_w, st>>>(
-                ctx->Y.as<double>(), ctx->C.as<double>(), n_wp, n_nodes, n_m, ns, ctx->nt);
+            k_spline_block<<<(unsigned)n_sys, T, smem_w, st>>>(ctx->Y.as<double>(), ctx->C.as<double>(), n_wp, n_nodes, n_m, ns,
+                                                             ctx->nt);
         } else {
             dim3 grid(ceil_div(n_wp, 128), ns * n_m);
             k_spline<<<grid, 128, 0, st>>>(ctx->Y.as<double>(), ctx->C.as<double>(), n_wp, n_nodes, n_m, ns, ctx->nt);

@@ -495,54 +495,88 @@ k_spline(const double *__restrict__ Y, double *__restrict__ C, int n_wp, int n_n
 }
 
 // ---------------------------------------------------------------------------------------------------
-// F2 for small batches (Module-1 sized: tens to hundreds of walkers): one WARP per system.  With
+// F2 for small batches (Module-1 sized: tens to hundreds of walkers): one warp or block per system.  With
 // few systems the thread-per-system kernel above is a chain of 2 (n-2) dependent steps on a nearly empty GPU.
 // Both Thomas sweeps are first-order linear recurrences x_j = alpha_j + beta_j x_{j-1}, i.e. compositions of
-// affine maps, which are associative: each lane composes the maps of its ceil(n/32) consecutive rows, a warp
-// scan composes across lanes, and each lane then re-runs its rows from the right start value.  Dependent chain:
-// 2 ceil(n/32) + 5 steps instead of n.  Same factorisation tables; results differ from the sequential sweep
+// affine maps, which are associative: each thread composes the maps of its ceil(n/T) consecutive rows, a scan
+// composes across threads, and each thread then re-runs its rows from the right start value.  Dependent chain:
+// 2 ceil(n/T) + scan steps instead of n.  Same factorisation tables; results differ from the sequential sweep
 // by rounding only.  Shared memory per warp: node values and dp / M, 2 n doubles.
 // ---------------------------------------------------------------------------------------------------
-constexpr int kSplineWarpsPerBlock = 2;
-__global__ void __launch_bounds__(32 * kSplineWarpsPerBlock)
-k_spline_warp(const double *__restrict__ Y, double *__restrict__ C, int n_wp, int n_nodes, int n_m, int ns, NodeTables nt)
+// Generalised to one BLOCK of T = 32..256 threads per system (T ~ n/4): the scan runs inside each warp and then
+// across the warps' totals, so 1024 nodes are a chain of 2 x 4 rows + two block scans instead of 2 x 32 rows.
+__device__ __forceinline__ void affine_block_scan_up(double &A, double &B, double *sA, double *sB, int lane, int wid, int nwarp)
 {
-    extern __shared__ double ssm[];
-    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
-    const long long gsys = (long long)blockIdx.x * kSplineWarpsPerBlock + wib;
-    if (gsys >= (long long)n_m * ns * n_wp) return; // whole warp
-    const int sys = (int)(gsys / n_wp), p = (int)(gsys - (long long)sys * n_wp);
+    // inclusive scan of maps x -> A + B x in thread order (thread t's map applied after those of threads < t)
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const double Ap = __shfl_up_sync(0xffffffffu, A, o), Bp = __shfl_up_sync(0xffffffffu, B, o);
+        if (lane >= o) { A = fma(B, Ap, A); B *= Bp; }
+    }
+    if (nwarp > 1) {
+        if (lane == 31) { sA[wid] = A; sB[wid] = B; }
+        __syncthreads();
+        double pa = 0.0, pb = 1.0; // composition of the warps below, in order
+        for (int k = 0; k < wid; ++k) { pa = fma(sB[k], pa, sA[k]); pb *= sB[k]; }
+        A = fma(B, pa, A);
+        B *= pb;
+        __syncthreads();
+    }
+}
+__device__ __forceinline__ void affine_block_scan_down(double &A, double &B, double *sA, double *sB, int lane, int wid, int nwarp)
+{
+    // the mirror image: thread t's map applied after those of threads > t
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const double Ap = __shfl_down_sync(0xffffffffu, A, o), Bp = __shfl_down_sync(0xffffffffu, B, o);
+        if (lane + o < 32) { A = fma(B, Ap, A); B *= Bp; }
+    }
+    if (nwarp > 1) {
+        if (lane == 0) { sA[wid] = A; sB[wid] = B; }
+        __syncthreads();
+        double pa = 0.0, pb = 1.0;
+        for (int k = nwarp - 1; k > wid; --k) { pa = fma(sB[k], pa, sA[k]); pb *= sB[k]; }
+        A = fma(B, pa, A);
+        B *= pb;
+        __syncthreads();
+    }
+}
+
+__global__ void __launch_bounds__(256)
+k_spline_block(const double *__restrict__ Y, double *__restrict__ C, int n_wp, int n_nodes, int n_m, int ns, NodeTables nt)
+{
+    extern __shared__ double ssm[]; // ys[n], ds[n], then the exchange slots
+    __shared__ double sA[8], sB[8];
+    const int tid = threadIdx.x, T = blockDim.x, lane = tid & 31, wid = tid >> 5, nwarp = T >> 5;
+    const int sys = blockIdx.x / n_wp, p = blockIdx.x - sys * n_wp;
     const int m = sys / ns, kind = sys % ns;
     const int n = n_nodes;
     const size_t sw = (size_t)n_wp;
-    double *ys = ssm + (size_t)wib * 2 * n, *ds = ys + n;
-    for (int j = lane; j < n; j += 32) ys[j] = __ldg(Y + ((size_t)sys * n + j) * sw + p);
-    __syncwarp();
-    const int L = (n + 31) / 32;
-    const int j0 = lane * L, j1 = min(j0 + L, n);
+    double *ys = ssm, *ds = ys + n, *xch = ds + n; // xch[T]: value handed to the neighbouring thread
+    for (int j = tid; j < n; j += T) ys[j] = __ldg(Y + ((size_t)sys * n + j) * sw + p);
+    __syncthreads();
+    const int L = (n + T - 1) / T;
+    const int j0 = min(tid * L, n), j1 = min(j0 + L, n);
     auto rhs = [&](int j) { return (ys[j + 1] - ys[j]) * __ldg(nt.invh + j) - (ys[j] - ys[j - 1]) * __ldg(nt.invh + j - 1); };
     // ---- forward sweep: dp_j = (r_j - a_j dp_{j-1}) / den_j for j = 1..n-2, dp_0 = 0
-    double A = 0.0, B = 1.0; // dp at the end of this lane's rows = A + B * dp before them
+    double A = 0.0, B = 1.0;
     for (int j = j0; j < j1; ++j)
         if (j >= 1 && j <= n - 2) {
             const double ti = __ldg(nt.tinv + j), be = -__ldg(nt.ta + j) * ti;
             A = fma(be, A, rhs(j) * ti);
             B *= be;
         }
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) { // inclusive scan: this lane's map after the maps of the lanes below
-        const double Ap = __shfl_up_sync(0xffffffffu, A, o), Bp = __shfl_up_sync(0xffffffffu, B, o);
-        if (lane >= o) { A = fma(B, Ap, A); B *= Bp; }
-    }
-    double start = __shfl_up_sync(0xffffffffu, A, 1); // the maps below applied to dp_0 = 0
-    if (lane == 0) start = 0.0;
+    affine_block_scan_up(A, B, sA, sB, lane, wid, nwarp);
+    xch[tid] = A; // all maps up to and including this thread applied to dp_0 = 0
+    __syncthreads();
+    double start = tid ? xch[tid - 1] : 0.0;
     for (int j = j0; j < j1; ++j) {
         if (j >= 1 && j <= n - 2) start = (rhs(j) - __ldg(nt.ta + j) * start) * __ldg(nt.tinv + j);
         ds[j] = (j >= 1 && j <= n - 2) ? start : 0.0;
     }
-    __syncwarp();
+    __syncthreads();
     // ---- backward sweep: M_j = dp_j - c'_j M_{j+1} for j = n-2..1, M_0 = M_{n-1} = 0
-    A = 0.0; B = 1.0; // M at this lane's first row = A + B * M just above its last row
+    A = 0.0; B = 1.0;
     for (int j = j1 - 1; j >= j0; --j) {
         if (j >= 1 && j <= n - 2) {
             const double be = -__ldg(nt.tcp + j);
@@ -550,23 +584,19 @@ k_spline_warp(const double *__restrict__ Y, double *__restrict__ C, int n_wp, in
             B *= be;
         } else { A = 0.0; B = 0.0; }
     }
-    if (j0 >= j1) { A = 0.0; B = 1.0; } // a lane without rows is the identity
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        const double Ap = __shfl_down_sync(0xffffffffu, A, o), Bp = __shfl_down_sync(0xffffffffu, B, o);
-        if (lane + o < 32) { A = fma(B, Ap, A); B *= Bp; }
-    }
-    double Mn = __shfl_down_sync(0xffffffffu, A, 1); // the maps above applied to M = 0 beyond the last node
-    if (lane == 31) Mn = 0.0;
+    affine_block_scan_down(A, B, sA, sB, lane, wid, nwarp);
+    xch[tid] = A;
+    __syncthreads();
+    double Mn = (tid + 1 < T) ? xch[tid + 1] : 0.0;
     for (int j = j1 - 1; j >= j0; --j) {
         Mn = (j >= 1 && j <= n - 2) ? fma(-__ldg(nt.tcp + j), Mn, ds[j]) : 0.0;
         ds[j] = Mn;
     }
-    __syncwarp();
+    __syncthreads();
     // ---- coefficients of interval j (same formulas as k_spline)
     double *c = C + ((size_t)m * ns * 4 + kind * 4) * sw + p;
     const size_t cj = (size_t)n_m * ns * 4 * sw;
-    for (int j = lane; j < n - 1; j += 32) {
+    for (int j = tid; j < n - 1; j += T) {
         const double y0 = ys[j], y1 = ys[j + 1], Mj = ds[j], Mn1 = ds[j + 1];
         const double h = __ldg(nt.hj + j), ih = __ldg(nt.invh + j);
         double *cc = c + (size_t)j * cj;
