@@ -88,7 +88,8 @@ struct ll_ctx {
     long long nodes_version = 0;   // bumped whenever the node tables are rebuilt
     DevBuf tile_tab;               // frequency-tile boundaries of the fused kernel [n_tiles + 1]
     long long tile_key_version = -1;
-    int tile_key_TB = -1, tile_key_small = -1, tile_n = 0;
+    int tile_key_TB = -1, tile_key_small = -1, tile_n = 0, tile2_off = 0, tile2_n = 0;
+    DevBuf part2;                  // chunk partials of the two-stage finalize
     DevBuf node_tab; // doubles then ints
     NodeTables nt{};
 
@@ -289,6 +290,7 @@ FullPlan make_plan(const ll_ctx *ctx, long long n_w)
 // Module-1 sized): a tile is also limited by the spline intervals it crosses, since every interval
 // change costs one dependent global load of the coefficients (~14 bins' worth of arithmetic) and log-spaced nodes
 // put dozens of intervals into the first tiles of the grid; cost = bins + 14 per interval <= TB.
+constexpr int kTileChunk = 64;
 int ensure_tiles(ll_ctx *ctx, FullPlan &pl, cudaStream_t st)
 {
     const int small = pl.n_wp <= 1024 ? 1 : 0;
@@ -322,6 +324,11 @@ int ensure_tiles(ll_ctx *ctx, FullPlan &pl, cudaStream_t st)
     }
     ts.push_back(n_f);
     pl.n_tiles = (int)ts.size() - 1;
+    // chunk boundaries for the two-stage finalize of small batches: tile_start2[z] = tile_start[z * kTileChunk]
+    ctx->tile2_off = (int)ts.size();
+    ctx->tile2_n = ceil_div(pl.n_tiles, kTileChunk);
+    for (int z = 0; z < ctx->tile2_n; ++z) ts.push_back(ts[(size_t)z * kTileChunk]);
+    ts.push_back(n_f);
     CK(ctx->tile_tab.ensure(sizeof(int) * ts.size()));
     CK(cudaMemcpyAsync(ctx->tile_tab.p, ts.data(), sizeof(int) * ts.size(), cudaMemcpyHostToDevice, st));
     CK(cudaStreamSynchronize(st)); // ts goes out of scope
@@ -440,13 +447,30 @@ int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, cons
         LAUNCHED(ctx);
         ctx->last_n_blocks = (int)(grid.x * grid.y);
     }
+    const double *fin_part = ctx->part.as<double>();
+    const int *fin_tiles = ctx->tile_tab.as<int>();
+    int fin_n = pl.n_tiles;
+    if (n_wp <= 1024 && pl.n_tiles >= 8 * kTileChunk) { // thousands of tiles, a handful of walker blocks: two stages
+        CK(ctx->part2.ensure(sizeof(double) * (size_t)ctx->tile2_n * NQ * n_wp));
+        dim3 grid(ceil_div(n_wp, 32), ctx->tile2_n);
+        if (NQ == 5)
+            k_reduce_tiles<5><<<grid, dim3(32, 32), 0, st>>>(fin_part, ctx->ilo_s.as<int>(), ctx->ihi_s.as<int>(), n_wp, fin_tiles,
+                                                            fin_n, kTileChunk, ctx->part2.as<double>());
+        else
+            k_reduce_tiles<2><<<grid, dim3(32, 32), 0, st>>>(fin_part, ctx->ilo_s.as<int>(), ctx->ihi_s.as<int>(), n_wp, fin_tiles,
+                                                            fin_n, kTileChunk, ctx->part2.as<double>());
+        LAUNCHED(ctx);
+        fin_part = ctx->part2.as<double>();
+        fin_tiles = ctx->tile_tab.as<int>() + ctx->tile2_off;
+        fin_n = ctx->tile2_n;
+    }
     if (nm1 && !tfp)
-        k_finalize<1><<<ceil_div(n_wp, 32), dim3(32, kFinY), 0, st>>>(ctx->part.as<double>(), ctx->TF.as<double>(), ctx->perm.as<int>(),
-                                                           ctx->ilo_s.as<int>(), ctx->ihi_s.as<int>(), n_wp, ctx->tile_tab.as<int>(), pl.n_tiles,
+        k_finalize<1><<<ceil_div(n_wp, 32), dim3(32, kFinY), 0, st>>>(fin_part, ctx->TF.as<double>(), ctx->perm.as<int>(),
+                                                           ctx->ilo_s.as<int>(), ctx->ihi_s.as<int>(), n_wp, fin_tiles, fin_n,
                                                            ctx->dd.as<double>(), logL, d_h, h_h);
     else
-        k_finalize<0><<<ceil_div(n_wp, 32), dim3(32, kFinY), 0, st>>>(ctx->part.as<double>(), ctx->TF.as<double>(), ctx->perm.as<int>(),
-                                                           ctx->ilo_s.as<int>(), ctx->ihi_s.as<int>(), n_wp, ctx->tile_tab.as<int>(), pl.n_tiles,
+        k_finalize<0><<<ceil_div(n_wp, 32), dim3(32, kFinY), 0, st>>>(fin_part, ctx->TF.as<double>(), ctx->perm.as<int>(),
+                                                           ctx->ilo_s.as<int>(), ctx->ihi_s.as<int>(), n_wp, fin_tiles, fin_n,
                                                            ctx->dd.as<double>(), logL, d_h, h_h);
     LAUNCHED(ctx);
     return LL_OK;
@@ -711,7 +735,7 @@ int ll_destroy(ll_ctx *ctx)
                          &ctx->key_w, &ctx->hist, &ctx->perm, &ctx->ilo_s, &ctx->ihi_s, &ctx->Y, &ctx->C, &ctx->TF,
                          &ctx->part, &ctx->prow, &ctx->het_tab, &ctx->het_tab1, &ctx->het_raw, &ctx->het_idx, &ctx->het_fb,
                          &ctx->stage_in, &ctx->stage_out, &ctx->g4f, &ctx->Wf, &ctx->scale, &ctx->wmax, &ctx->ref_idx,
-                         &ctx->ref_dense, &ctx->ref_edges, &ctx->tile_tab, &ctx->pt_y, &ctx->pt_out, &ctx->pt_in};
+                         &ctx->ref_dense, &ctx->ref_edges, &ctx->tile_tab, &ctx->part2, &ctx->pt_y, &ctx->pt_out, &ctx->pt_in};
         for (DevBuf *b : all) b->release();
         for (auto &e : ctx->ev) cudaEventDestroy(e);
     }

@@ -1222,6 +1222,46 @@ k_tlm_nodes(const double *__restrict__ phase, int n_sys, int n_nodes, double t_r
     }
 }
 
+// F4, first stage for small batches with thousands of tiles: block (x, z) adds, for its 32 walkers, the partials of
+// the tiles of chunk z = [z cs, (z+1) cs) that lie in the walker's band, in a fixed order, into part2[z][NQ][n_wp];
+// k_finalize then runs over the chunks as if they were tiles (tile_start2[z] = tile_start[z cs]).
+template <int NQ>
+__global__ void __launch_bounds__(32 * 32)
+k_reduce_tiles(const double *__restrict__ part, const int *__restrict__ ilo, const int *__restrict__ ihi, int n_wp,
+               const int *__restrict__ tile_start, int n_tiles, int cs, double *__restrict__ part2)
+{
+    __shared__ double red[32][NQ][32];
+    const int p = blockIdx.x * 32 + threadIdx.x, ty = threadIdx.y, z = blockIdx.y;
+    const bool in = p < n_wp;
+    const size_t sw = (size_t)n_wp;
+    const int lo = in ? ilo[p] : 0, hi = in ? ihi[p] : 0;
+    double acc[NQ];
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) acc[q] = 0.0;
+    bool any = false;
+    if (hi > lo) {
+        const int t0 = max(tile_of_bin(tile_start, n_tiles, lo), z * cs);
+        const int t1 = min(tile_of_bin(tile_start, n_tiles, hi - 1), min((z + 1) * cs, n_tiles) - 1);
+        any = t0 <= t1;
+        for (int t = t0 + ty; t <= t1; t += 32) {
+            const double *o = part + ((size_t)t * NQ) * sw + p;
+#pragma unroll
+            for (int q = 0; q < NQ; ++q) acc[q] += o[q * sw];
+        }
+    }
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) red[ty][q][threadIdx.x] = acc[q];
+    __syncthreads();
+    if (ty != 0 || !in || !any) return;
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) {
+        double v = red[0][q][threadIdx.x];
+#pragma unroll
+        for (int k = 1; k < 32; ++k) v += red[k][q][threadIdx.x];
+        part2[((size_t)z * NQ + q) * sw + p] = v;
+    }
+}
+
 // F4: reduce the per-tile partials in a fixed order, apply T^c (single mode), form log L        (Eq. 2)
 // Block = 32 walkers x kFinY tile slices: slice ty sums tiles t0 + ty, t0 + ty + kFinY, ... of its walker, the
 // slices meet in shared memory and are added in slice order (deterministic: reruns are bit-identical).
