@@ -36,7 +36,10 @@ UNIT = "evals/s"
 # (t 1, two cubics 6, reduce 3, sincos 18, A e^{-i Psi} 2, two complex MACs 8, W A^2 2 => 40; the
 # SURVEY.md §8(d) figure of 39 is used as the contract number)
 SLOTS_FULL = 39.0
-SLOTS_HET = {1: 73.0, 6: 252.0}
+# single mode: the kernel regroups Eq. 14/17 by edge, whose own count is 48 slots per (walker, bin): phase 2,
+# reduce 3, sincos 18, taper and amplitude 4, z conj(Q) 8, |z|^2 P 3, z_b conj(z_{b+1}) X 10; the bin-by-bin form needs 73
+SLOTS_HET = {1: 48.0, 6: 252.0}
+SLOTS_HET_DIRECT_FORM = {1: 73.0}
 # FP32-accumulate variant: bound by instruction issue (one warp instruction per scheduler per
 # clock = 4 x 32 lane-instructions/clk/SM).  Algorithmic instructions per active pair: 13 FP64 (t, two cubics,
 # reduce 3, scale 1, W A^2 2) + 3 conversions + 20 binary32 (sincos 10, A e^{-i Psi} 2, MACs 8) + 6 quadrant
@@ -445,6 +448,9 @@ def main():
                 "measured_dfma_per_s": dfma_rate, "measured_ffma_per_s": ffma_rate,
                 "frac_of_measured_dfma": achieved / dfma_rate,
                 "hbm_peak_gbs": peaks.get("hbm_gbs"), "hbm_peak_source": peak_src}
+            if wl.path != "full" and wl.n_m in SLOTS_HET_DIRECT_FORM:
+                line["roofline"]["formulation"] = "regrouped by edge (DESIGN.md §5); the bin-by-bin form of Eq. 14/17 needs %g" \
+                                                  % SLOTS_HET_DIRECT_FORM[wl.n_m]
 
     if not args.quick:
         # ---- end to end through the C ABI with host buffers

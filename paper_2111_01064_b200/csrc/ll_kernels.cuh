@@ -1756,22 +1756,51 @@ k_het_standin1(Het1Table T, StandinInfo si, const double *__restrict__ params, i
             double up, vp, ap;
             edge(t, up, vp, ap);
             const int last = min(e1, T.n_b); // one past the last bin whose cross term this segment owns
-#pragma unroll 2
-            for (int e = e0; e < e1; ++e, t += kHet1Stride) {
-                // edge terms of e: conj(z) Q and |z|^2 P
-                DAr = fma(up, t[4], DAr); DAr = fma(-vp, t[5], DAr);
-                DAi = fma(up, t[5], DAi); DAi = fma(vp, t[4], DAi);
-                DEr = fma(up, t[6], DEr); DEr = fma(-vp, t[7], DEr);
-                DEi = fma(up, t[7], DEi); DEi = fma(vp, t[6], DEi);
-                const double a2 = ap * ap;
-                HA = fma(a2, t[8], HA);
-                HE = fma(a2, t[9], HE);
+            auto edge_terms = [&](const double *tt, double u, double v, double a) { // conj(z) Q and |z|^2 P of one edge
+                DAr = fma(u, tt[4], DAr); DAr = fma(-v, tt[5], DAr);
+                DAi = fma(u, tt[5], DAi); DAi = fma(v, tt[4], DAi);
+                DEr = fma(u, tt[6], DEr); DEr = fma(-v, tt[7], DEr);
+                DEi = fma(u, tt[7], DEi); DEi = fma(v, tt[6], DEi);
+                const double a2 = a * a;
+                HA = fma(a2, tt[8], HA);
+                HE = fma(a2, tt[9], HE);
+            };
+            auto cross_terms = [&](const double *tt, double u0, double v0, double u1, double v1) { // z_e conj(z_{e+1}) X
+                const double wr = fma(u0, u1, v0 * v1), wi = fma(u0, v1, -(v0 * u1));
+                HA = fma(wr, tt[10], HA); HA = fma(-wi, tt[11], HA);
+                HE = fma(wr, tt[12], HE); HE = fma(-wi, tt[13], HE);
+            };
+            int e = e0;
+            // chunks of kE bins: the kE next edges are kE independent phase -> sincos chains in flight per thread;
+            // the taper polynomial is needed only where some lane is above its f_ISCO (one warp-uniform test per chunk)
+            constexpr int kE = 4;
+            for (; e + kE <= last; e += kE, t += kE * kHet1Stride) {
+                double un[kE], vn[kE], an[kE];
+                const bool tapered = __any_sync(0xffffffffu, t[kE * kHet1Stride + 3] * c.inv_fisco > 1.0);
+#pragma unroll
+                for (int k = 0; k < kE; ++k) {
+                    const double *tn = t + (k + 1) * kHet1Stride;
+                    const double y = fma(tn[0], c.tc, fma(Kq, tn[1], nphq));
+                    double a = tn[2] * c.invD;
+                    if (tapered) a *= taper_nobranch(tn[3] * c.inv_fisco, si.kappa, inv_kappa);
+                    an[k] = a;
+                    amp_expi_qc(a, y, un[k], vn[k]);
+                }
+#pragma unroll
+                for (int k = 0; k < kE; ++k) {
+                    const double *tt = t + k * kHet1Stride;
+                    const double u0 = k ? un[k - 1] : up, v0 = k ? vn[k - 1] : vp, a0 = k ? an[k - 1] : ap;
+                    edge_terms(tt, u0, v0, a0);
+                    cross_terms(tt, u0, v0, un[k], vn[k]);
+                }
+                up = un[kE - 1]; vp = vn[kE - 1]; ap = an[kE - 1];
+            }
+            for (; e < e1; ++e, t += kHet1Stride) {
+                edge_terms(t, up, vp, ap);
                 if (e < last) { // bin e = [e, e + 1]: needs z at e + 1 (the next segment's first edge at the boundary)
                     double un, vn, an;
                     edge(t + kHet1Stride, un, vn, an);
-                    const double wr = fma(up, un, vp * vn), wi = fma(up, vn, -(vp * un)); // z_e conj(z_{e+1})
-                    HA = fma(wr, t[10], HA); HA = fma(-wi, t[11], HA);
-                    HE = fma(wr, t[12], HE); HE = fma(-wi, t[13], HE);
+                    cross_terms(t, up, vp, un, vn);
                     up = un; vp = vn; ap = an;
                 }
             }
