@@ -793,3 +793,68 @@ def test_stopping_functions():
     s2 = sm.StopConverged(n_checks=3, tol=1.0)
     seq = [-10.0, -5.0, -4.5, -4.2, -3.9, -2.0, -1.9, -1.8, -1.7]
     assert [s2.check(v) for v in seq] == [False, False, False, False, False, False, False, False, True]
+
+
+# --------------------------------------------------------------------------- per-walker node grids
+def _pw_case(rng, n_w, n_m, n_nodes, n_f, k_min, df):
+    f = (k_min + np.arange(n_f)) * df
+    x = np.empty((n_w, n_nodes))
+    for w in range(n_w):
+        lo = f[0] * rng.uniform(0.8, 1.5)
+        hi = f[-1] * rng.uniform(0.5, 1.1)
+        x[w] = np.geomspace(lo, hi, n_nodes)
+    xn = np.log(x / x[:, :1]) / np.log(x[:, -1:] / x[:, :1])
+    amp = 1e-19 * (1.0 + rng.uniform(0.2, 1.0, (n_w, n_m, 1)) * xn[:, None, :] ** 2)
+    ph = 40.0 * rng.uniform(-1, 1, (n_w, n_m, 1)) * xn[:, None, :] + 25.0 * np.cos(3 * xn[:, None, :] + rng.uniform(0, 6, (n_w, n_m, 1)))
+    ang = rng.uniform(0, 2 * np.pi, (n_w, n_m, 2))
+    tf = np.stack([np.cos(ang), np.sin(ang)], axis=-1)
+    W = rng.uniform(0.5, 2.0, n_f) * 1e37
+    d = rng.normal(size=(2, n_f, 2)) * 1e-19
+    return f, x, amp, ph, tf, W, d
+
+
+def test_per_walker_nodes_reduce_to_shared_nodes(orc):
+    from oracle import per_walker as pw
+    rng = np.random.default_rng(82)
+    f, x, amp, ph, tf, W, d = _pw_case(rng, 5, 2, 12, 90, 40, 1e-5)
+    x[:] = x[0]
+    band = np.tile([[x[0, 0], x[0, -1]]], (5, 1))
+    a = pw.full_batch_pw(x, amp, ph, tf, None, 40, 1e-5, d, W)
+    b = orc.full_batch(x[0], amp, ph, tf, band, 40, 1e-5, d, W)
+    for k in ("logL", "d_h", "h_h"):
+        assert np.array_equal(a[k], b[k]), k
+
+
+def test_per_walker_nodes_brute_force_scipy(orc):
+    """different nodes per walker, zero outside each walker's own node span (R30): SciPy + numpy, one walker at a time"""
+    from oracle import per_walker as pw
+    rng = np.random.default_rng(83)
+    f, x, amp, ph, tf, W, d = _pw_case(rng, 4, 2, 9, 70, 30, 2e-5)
+    band = np.stack([x[:, 0] * 1.05, x[:, -1] * rng.uniform(0.7, 1.2, 4)], axis=1)
+    for bnd in (None, band):
+        got = pw.full_batch_pw(x, amp, ph, tf, bnd, 30, 2e-5, d, W)
+        for w in range(4):
+            b = np.array([[x[w, 0], x[w, -1]]]) if bnd is None else np.array([[max(x[w, 0], bnd[w, 0]), min(x[w, -1], bnd[w, 1])]])
+            ref = _brute_full(x[w], amp[w:w + 1], ph[w:w + 1], tf[w:w + 1], b, 30, 2e-5, d, W)
+            assert (f < x[w, 0]).any() or (f > x[w, -1]).any()                # some bins really are outside
+            for k in ("logL", "d_h", "h_h"):
+                assert got[k][w] == pytest.approx(ref[k][0], rel=1e-9, abs=1e-9 * abs(ref["logL"][0])), (k, w)
+
+
+def test_per_walker_nodes_do_not_matter_for_a_spline_reproducible_template(orc):
+    """Amplitude and phase linear in f are reproduced exactly by any natural spline, so two different node sets over
+    the same span give the same likelihood."""
+    from oracle import per_walker as pw
+    rng = np.random.default_rng(84)
+    n_f, k_min, df = 80, 25, 1e-5
+    f = (k_min + np.arange(n_f)) * df
+    xa = np.geomspace(f[3], f[-4], 7)
+    xb = np.sort(np.r_[xa[0], rng.uniform(xa[0], xa[-1], 9), xa[-1]])
+    W = rng.uniform(0.5, 2.0, n_f) * 1e37
+    d = rng.normal(size=(2, n_f, 2)) * 1e-19
+    tf = np.array([[[[0.6, 0.8], [1.0, 0.0]]]])
+    lin = lambda x: (1e-19 * (1 + 300.0 * x)[None, None, :], (5.0 + 9e4 * x)[None, None, :])
+    ra = pw.full_batch_pw(xa[None], *lin(xa), tf, None, k_min, df, d, W)
+    rb = pw.full_batch_pw(xb[None], *lin(xb), tf, None, k_min, df, d, W)
+    for k in ("logL", "d_h", "h_h"):
+        assert ra[k][0] == pytest.approx(rb[k][0], rel=1e-11)
