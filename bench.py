@@ -542,6 +542,25 @@ def main():
                               "algorithmic_slots_per_pair": SLOTS_FULL_TF,
                               "frac": pairs2 * SLOTS_FULL_TF / (kms / max(kn, 1) * 1e-3) / peak_slots,
                               "entry": "ll_full_batch_tf (amp, phase, T at 1024 nodes as device arrays; the walkers' own bands)"}
+            # ---- per-walker node grids at config-2 size.  Every walker gets its own copy of the
+            # 1024 nodes (so the numbers can be compared with the shared-node path output by output); what is timed is
+            # the per-walker machinery: one tridiagonal factorisation per system, one bin -> interval map per lane
+            tfc = b2["params"][:, 5:9].reshape(-1, 1, 2, 2).contiguous()
+            xw = torch.as_tensor(np.ascontiguousarray(wl2.f_nodes), device=amp.device).repeat(wl2.n_w, 1).contiguous()
+            o3 = tuple(torch.empty(wl2.n_w, dtype=torch.float64, device=amp.device) for _ in range(3))
+            fn3 = lambda: c2.full_batch_pw(xw, amp, ph, tfc, band=bnd, out=o3)
+            fn3()
+            sh = c2.full_batch(wl2.f_nodes, amp, ph, tfc, band=bnd)
+            c2.profile_enable(True)
+            ms3 = time_steps(torch, fn3, nst, 2)
+            kms3, kn3 = c2.profile_read()
+            c2.profile_enable(False)
+            per["cfg2_pw"] = {"evals_per_s": wl2.n_w / (ms3 / nst * 1e-3), "ms_per_batch": ms3 / nst, "n_walkers": wl2.n_w,
+                              "kernel": "k_full_fused_pw", "kernel_ms": kms3 / max(kn3, 1),
+                              "frac": pairs2 * SLOTS_FULL / (kms3 / max(kn3, 1) * 1e-3) / peak_slots,
+                              "max_abs_dlogL_vs_shared_nodes": float((o3[0] - sh[0]).abs().max()),
+                              "entry": "ll_full_batch_pw (f_nodes_w [n_w][1024] on the device; the walkers' own bands)"}
+            del xw, sh, tfc
             # ---- Module-1 sized sampler iteration on the full-grid likelihood of the same one-year data stream
             per["module1_iteration"] = bench_sampler_iteration(torch, c2, wl2, b2["params"], n_t=4, n_w=80, iters=20,
                                                                f_nodes=wl2.f_nodes)

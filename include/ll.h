@@ -108,6 +108,16 @@ int ll_full_batch_tf(ll_ctx *ctx, int64_t n_w, int32_t n_nodes, const double *f_
                      const double *phase, const double *tf_nodes, const double *band, double *logL, double *d_h,
                      double *h_h, void *stream);
 
+/* F2-F4 with PER-WALKER node grids: every walker brings its own nodes, spanning its own band,
+ * so each walker has its own tridiagonal system (a true batched solve) and its own bin -> interval map.
+ *   f_nodes_w : DEV [n_w][n_nodes], strictly ascending per walker (not checked: the array lives on the device)
+ *   amp, phase, tf, band, outputs: as ll_full_batch.  A spline is not extrapolated: the template of walker w is
+ *   zero outside [f_nodes_w[w][0], f_nodes_w[w][n_nodes-1]] (intersected with `band` when given; reading R30).
+ * FP64 contexts only.                                                                                        */
+int ll_full_batch_pw(ll_ctx *ctx, int64_t n_w, int32_t n_nodes, const double *f_nodes_w, const double *amp,
+                     const double *phase, const double *tf, const double *band, double *logL, double *d_h, double *h_h,
+                     void *stream);
+
 /* F1 utility — the stand-in's node arrays in the caller layout (what ll_full_batch_standin builds internally):
  *   params : DEV [n_w][P];  amp, phase : DEV out [n_w][n_m][n_nodes] (phase in radians);
  *   band   : DEV out [n_w][2] = (f_0, min(f_last, (1+kappa) f_ISCO max_m(m/2))) (reading R10), or NULL.

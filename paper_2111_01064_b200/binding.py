@@ -21,7 +21,7 @@ LL_PREC_FP64, LL_PREC_FP32_ACC = 0, 1
 # every symbol include/ll.h declares (tests/test_abi.py checks header and library against this list)
 SYMBOLS = (
     "ll_create", "ll_destroy", "ll_last_error", "ll_abi_version", "ll_set_data", "ll_get_dd", "ll_standin_config",
-    "ll_full_batch", "ll_full_batch_tf", "ll_tlm_nodes", "ll_standin_nodes", "ll_full_batch_standin", "ll_full_batch_standin_host",
+    "ll_full_batch", "ll_full_batch_pw", "ll_full_batch_tf", "ll_tlm_nodes", "ll_standin_nodes", "ll_full_batch_standin", "ll_full_batch_standin_host",
     "ll_full_template_standin",
     "ll_template_standin", "ll_het_prepare", "ll_het_refresh_standin", "ll_het_audit_standin",
     "ll_pt_stretch_half_het", "ll_pt_stretch_half_full", "ll_pt_swap", "ll_pt_stats", "ll_stop_snr", "ll_stop_converged", "ll_het_get_summary", "ll_het_batch", "ll_het_batch_standin",
@@ -65,6 +65,7 @@ def load_library(path: Optional[str] = None):
         "ll_standin_config": (C.c_int, [vp, i32, vp, vp, vp, dbl]),
         "ll_full_batch": (C.c_int, [vp, i64, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp]),
         "ll_full_batch_tf": (C.c_int, [vp, i64, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp]),
+        "ll_full_batch_pw": (C.c_int, [vp, i64, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp]),
         "ll_tlm_nodes": (C.c_int, [vp, i64, i32, vp, vp, dbl, vp, vp]),
         "ll_standin_nodes": (C.c_int, [vp, i64, i32, vp, vp, vp, vp, vp, vp]),
         "ll_full_batch_standin": (C.c_int, [vp, i64, i32, vp, vp, vp, vp, vp, vp]),
@@ -223,6 +224,16 @@ class Context:
                                             _dev_ptr(amp, "amp"), _dev_ptr(phase, "phase"), _dev_ptr(tf, "tf"),
                                             _dev_ptr(band, "band"), _dev_ptr(logL, "logL"), _dev_ptr(d_h, "d_h"),
                                             _dev_ptr(h_h, "h_h"), _stream_ptr(stream)), "ll_full_batch")
+        return logL, d_h, h_h
+
+    def full_batch_pw(self, f_nodes_w, amp, phase, tf, band=None, want_parts: bool = True, out=None, stream=None):
+        """per-walker node grids: f_nodes_w [n_w][n_nodes] on the device (reading R30)"""
+        n_w, n_nodes = int(f_nodes_w.shape[0]), int(f_nodes_w.shape[1])
+        logL, d_h, h_h = out if out is not None else (self._out(n_w), self._out(n_w, want_parts), self._out(n_w, want_parts))
+        self._check(self._lib.ll_full_batch_pw(self._h, n_w, n_nodes, _dev_ptr(f_nodes_w, "f_nodes_w"), _dev_ptr(amp, "amp"),
+                                               _dev_ptr(phase, "phase"), _dev_ptr(tf, "tf"), _dev_ptr(band, "band"),
+                                               _dev_ptr(logL, "logL"), _dev_ptr(d_h, "d_h"), _dev_ptr(h_h, "h_h"),
+                                               _stream_ptr(stream)), "ll_full_batch_pw")
         return logL, d_h, h_h
 
     def full_batch_tf(self, f_nodes, amp, phase, tf_nodes, band=None, want_parts: bool = True, out=None, stream=None):

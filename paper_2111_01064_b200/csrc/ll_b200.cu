@@ -90,6 +90,7 @@ struct ll_ctx {
     long long tile_key_version = -1;
     int tile_key_TB = -1, tile_key_small = -1, tile_n = 0, tile2_off = 0, tile2_n = 0;
     DevBuf part2;                  // chunk partials of the two-stage finalize
+    DevBuf pw_x;                   // per-walker node grids: X [n_nodes][n_wp], then the effective bands [n_w][2]
     DevBuf node_tab; // doubles then ints
     NodeTables nt{};
 
@@ -291,9 +292,9 @@ FullPlan make_plan(const ll_ctx *ctx, long long n_w)
 // change costs one dependent global load of the coefficients (~14 bins' worth of arithmetic) and log-spaced nodes
 // put dozens of intervals into the first tiles of the grid; cost = bins + 14 per interval <= TB.
 constexpr int kTileChunk = 64;
-int ensure_tiles(ll_ctx *ctx, FullPlan &pl, cudaStream_t st)
+int ensure_tiles(ll_ctx *ctx, FullPlan &pl, cudaStream_t st, bool uniform = false)
 {
-    const int small = pl.n_wp <= 1024 ? 1 : 0;
+    const int small = uniform ? 2 : (pl.n_wp <= 1024 ? 1 : 0); // 2: per-walker node grids, no shared interval table
     if (ctx->tile_key_version == ctx->nodes_version && ctx->tile_key_TB == pl.TB && ctx->tile_key_small == small) {
         pl.n_tiles = ctx->tile_n;
         return LL_OK;
@@ -301,7 +302,7 @@ int ensure_tiles(ll_ctx *ctx, FullPlan &pl, cudaStream_t st)
     const int n_f = (int)ctx->n_f, n = (int)ctx->bstart_host.size();
     std::vector<int> ts;
     ts.push_back(0);
-    if (!small) {
+    if (small != 1) {
         for (int i = pl.TB; i < n_f; i += pl.TB) ts.push_back(i);
     } else {
         const int kIntervalCost = 14;
@@ -472,6 +473,89 @@ int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, cons
         k_finalize<0><<<ceil_div(n_wp, 32), dim3(32, kFinY), 0, st>>>(fin_part, ctx->TF.as<double>(), ctx->perm.as<int>(),
                                                            ctx->ilo_s.as<int>(), ctx->ihi_s.as<int>(), n_wp, fin_tiles, fin_n,
                                                            ctx->dd.as<double>(), logL, d_h, h_h);
+    LAUNCHED(ctx);
+    return LL_OK;
+}
+
+// full-grid pipeline with per-walker node grids (reading R30)
+int run_full_pw(ll_ctx *ctx, long long n_w, int n_nodes, const double *f_nodes_w, const double *amp, const double *phase,
+                const double *tf, const double *band, double *logL, double *d_h, double *h_h, cudaStream_t st)
+{
+    const int n_m = ctx->n_m;
+    FullPlan pl = make_plan(ctx, n_w);
+    {
+        const int rc_t = ensure_tiles(ctx, pl, st, true);
+        if (rc_t != LL_OK) return rc_t;
+    }
+    const int n_wp = pl.n_wp;
+    const int NQ = 2;
+    CK(ctx->ilo_w.ensure(sizeof(int) * n_wp));
+    CK(ctx->ihi_w.ensure(sizeof(int) * n_wp));
+    CK(ctx->key_w.ensure(sizeof(int) * n_wp));
+    CK(ctx->perm.ensure(sizeof(int) * n_wp));
+    CK(ctx->ilo_s.ensure(sizeof(int) * n_wp));
+    CK(ctx->ihi_s.ensure(sizeof(int) * n_wp));
+    CK(ctx->hist.ensure(sizeof(int) * 8192));
+    CK(ctx->pairs.ensure(sizeof(unsigned long long)));
+    CK(ctx->Y.ensure(sizeof(double) * (size_t)n_m * 2 * n_nodes * n_wp));
+    CK(ctx->C.ensure(sizeof(double) * (size_t)(n_nodes - 1) * n_m * 8 * n_wp));
+    CK(ctx->TF.ensure(sizeof(double) * (size_t)n_m * 4 * n_wp));
+    CK(ctx->part.ensure(sizeof(double) * (size_t)pl.n_tiles * NQ * n_wp));
+    CK(ctx->pw_x.ensure(sizeof(double) * ((size_t)n_nodes * n_wp + 2 * (size_t)n_w)));
+    double *X = ctx->pw_x.as<double>(), *band_w = X + (size_t)n_nodes * n_wp;
+
+    const GridInfo g{ctx->k_min, ctx->n_f, ctx->df};
+    k_pw_band<<<ceil_div(n_w, 256), 256, 0, st>>>(f_nodes_w, band, (int)n_w, n_nodes, band_w);
+    LAUNCHED(ctx);
+    if (n_w <= 1024 && n_wp <= 1024) {
+        k_band_sort_small<<<1, 1024, 0, st>>>(0, nullptr, 0, band_w, (int)n_w, n_wp, g, ctx->si, ctx->perm.as<int>(),
+                                              ctx->ilo_s.as<int>(), ctx->ihi_s.as<int>(), ctx->pairs.as<unsigned long long>());
+        LAUNCHED(ctx);
+    } else {
+        CK(cudaMemsetAsync(ctx->hist.p, 0, sizeof(int) * pl.n_keys, st));
+        CK(cudaMemsetAsync(ctx->pairs.p, 0, sizeof(unsigned long long), st));
+        k_band_prep<<<ceil_div(n_w, 256), 256, 0, st>>>(0, nullptr, 0, band_w, (int)n_w, g, ctx->si, pl.key_gran,
+                                                        ctx->ilo_w.as<int>(), ctx->ihi_w.as<int>(), ctx->key_w.as<int>(),
+                                                        ctx->hist.as<int>(), ctx->pairs.as<unsigned long long>());
+        LAUNCHED(ctx);
+        k_scan_hist<<<1, 1024, 0, st>>>(ctx->hist.as<int>(), pl.n_keys);
+        LAUNCHED(ctx);
+        k_scatter<<<ceil_div(n_wp, 256), 256, 0, st>>>((int)n_w, n_wp, ctx->key_w.as<int>(), ctx->ilo_w.as<int>(),
+                                                       ctx->ihi_w.as<int>(), ctx->hist.as<int>(), ctx->perm.as<int>(),
+                                                       ctx->ilo_s.as<int>(), ctx->ihi_s.as<int>());
+        LAUNCHED(ctx);
+    }
+    {
+        dim3 grid(n_wp / 32, ceil_div(n_nodes, 32), n_m);
+        k_nodes_arrays<<<grid, 256, 0, st>>>(amp, phase, tf, ctx->perm.as<int>(), n_wp, n_nodes, n_m, ctx->Y.as<double>(),
+                                             ctx->TF.as<double>());
+        LAUNCHED(ctx);
+        dim3 gx(n_wp / 32, ceil_div(n_nodes, 32));
+        k_pw_nodes_x<<<gx, 256, 0, st>>>(f_nodes_w, ctx->perm.as<int>(), n_wp, n_nodes, X);
+        LAUNCHED(ctx);
+        dim3 gs(ceil_div(n_wp, 128), 2 * n_m);
+        k_spline_pw<<<gs, 128, 0, st>>>(ctx->Y.as<double>(), X, ctx->C.as<double>(), n_wp, n_nodes, n_m);
+        LAUNCHED(ctx);
+    }
+    FusedArgs fa;
+    fa.g4 = ctx->g4.as<double>(); fa.Wd = ctx->Wd.as<double>(); fa.C = ctx->C.as<double>(); fa.TF = ctx->TF.as<double>();
+    fa.xj = nullptr; fa.bstart = nullptr; fa.ilo = ctx->ilo_s.as<int>(); fa.ihi = ctx->ihi_s.as<int>();
+    fa.part = ctx->part.as<double>(); fa.k_min = ctx->k_min; fa.df = ctx->df; fa.n_f = (int)ctx->n_f; fa.n_wp = n_wp;
+    fa.n_nodes = n_nodes; fa.n_m = n_m; fa.TB = pl.TB; fa.CH = pl.CH;
+    fa.tile_start = ctx->tile_tab.as<int>();
+    {
+        dim3 grid(n_wp / pl.WB, pl.n_tiles);
+        const size_t smem = (size_t)2 * pl.CH * 40;
+        ProfScope prof(ctx, st);
+        if (n_m == 1) k_full_fused_pw<1><<<grid, pl.WB, smem, st>>>(fa, X);
+        else k_full_fused_pw<0><<<grid, pl.WB, smem, st>>>(fa, X);
+        LAUNCHED(ctx);
+        ctx->last_n_blocks = (int)(grid.x * grid.y);
+    }
+    k_finalize<0><<<ceil_div(n_wp, 32), dim3(32, kFinY), 0, st>>>(ctx->part.as<double>(), ctx->TF.as<double>(), ctx->perm.as<int>(),
+                                                                 ctx->ilo_s.as<int>(), ctx->ihi_s.as<int>(), n_wp,
+                                                                 ctx->tile_tab.as<int>(), pl.n_tiles, ctx->dd.as<double>(), logL,
+                                                                 d_h, h_h);
     LAUNCHED(ctx);
     return LL_OK;
 }
@@ -735,7 +819,7 @@ int ll_destroy(ll_ctx *ctx)
                          &ctx->key_w, &ctx->hist, &ctx->perm, &ctx->ilo_s, &ctx->ihi_s, &ctx->Y, &ctx->C, &ctx->TF,
                          &ctx->part, &ctx->prow, &ctx->het_tab, &ctx->het_tab1, &ctx->het_raw, &ctx->het_idx, &ctx->het_fb,
                          &ctx->stage_in, &ctx->stage_out, &ctx->g4f, &ctx->Wf, &ctx->scale, &ctx->wmax, &ctx->ref_idx,
-                         &ctx->ref_dense, &ctx->ref_edges, &ctx->tile_tab, &ctx->part2, &ctx->pt_y, &ctx->pt_out, &ctx->pt_in};
+                         &ctx->ref_dense, &ctx->ref_edges, &ctx->tile_tab, &ctx->part2, &ctx->pw_x, &ctx->pt_y, &ctx->pt_out, &ctx->pt_in};
         for (DevBuf *b : all) b->release();
         for (auto &e : ctx->ev) cudaEventDestroy(e);
     }
@@ -844,6 +928,22 @@ int ll_full_batch(ll_ctx *ctx, int64_t n_w, int32_t n_nodes, const double *f_nod
     if (rc != LL_OK) return rc;
     if (n_w == 0) return LL_OK;
     return run_full(ctx, n_w, n_nodes, nullptr, amp, phase, tf, band, logL, d_h, h_h, st, false, nullptr);
+}
+
+int ll_full_batch_pw(ll_ctx *ctx, int64_t n_w, int32_t n_nodes, const double *f_nodes_w, const double *amp,
+                     const double *phase, const double *tf, const double *band, double *logL, double *d_h, double *h_h,
+                     void *stream)
+{
+    if (!ctx) return LL_ERR_ARG;
+    if (n_w < 0) return ctx->fail(LL_ERR_ARG, "n_w < 0");
+    if (n_w > (1 << 24)) return ctx->fail(LL_ERR_ARG, "n_w > 2^24 per call: split the batch");
+    if (n_nodes < 3 || n_nodes > (1 << 20)) return ctx->fail(LL_ERR_ARG, "n_nodes out of range [3, 2^20]");
+    if (n_w > 0 && (!f_nodes_w || !amp || !phase || !tf || !logL)) return ctx->fail(LL_ERR_ARG, "NULL argument");
+    if (!ctx->have_data) return ctx->fail(LL_ERR_STATE, "ll_set_data has not been called");
+    if (ctx->precision != LL_PREC_FP64) return ctx->fail(LL_ERR_UNSUPPORTED, "ll_full_batch_pw is FP64 only");
+    if (n_w == 0) return LL_OK;
+    DeviceGuard dg(ctx->device);
+    return run_full_pw(ctx, n_w, n_nodes, f_nodes_w, amp, phase, tf, band, logL, d_h, h_h, (cudaStream_t)stream);
 }
 
 int ll_full_batch_tf(ll_ctx *ctx, int64_t n_w, int32_t n_nodes, const double *f_nodes, const double *amp,

@@ -1186,6 +1186,203 @@ __global__ void __launch_bounds__(128, 3) k_full_fused_tf(FusedArgs a)
     o[0] = s_dh; o[sw] = s_hh;
 }
 
+// ---------------------------------------------------------------------------------------------------
+// Per-walker node grids (reading R30): every walker has its own nodes x_{w,j}, hence its own
+// tridiagonal matrix (a true batched solve) and its own bin -> interval map.
+// ---------------------------------------------------------------------------------------------------
+// X[j][p] = f_nodes_w[perm[p]][j] (walker fastest); padding positions get an ascending dummy grid.
+// band_w[w] = [max(band_lo, x_0), min(band_hi, x_last)]: a spline is not extrapolated beyond its own nodes.
+__global__ void __launch_bounds__(256)
+k_pw_band(const double *__restrict__ f_nodes_w, const double *__restrict__ band, int n_w, int n_nodes,
+          double *__restrict__ band_w)
+{
+    const int w = blockIdx.x * blockDim.x + threadIdx.x;
+    if (w >= n_w) return;
+    double lo = f_nodes_w[(size_t)w * n_nodes], hi = f_nodes_w[(size_t)w * n_nodes + n_nodes - 1];
+    if (band) { lo = fmax(lo, band[2 * (size_t)w]); hi = fmin(hi, band[2 * (size_t)w + 1]); }
+    band_w[2 * (size_t)w] = lo;
+    band_w[2 * (size_t)w + 1] = hi;
+}
+
+__global__ void __launch_bounds__(256)
+k_pw_nodes_x(const double *__restrict__ f_nodes_w, const int *__restrict__ perm, int n_wp, int n_nodes, double *__restrict__ X)
+{
+    __shared__ double tt[32][33];
+    const int p0 = blockIdx.x * 32, j0 = blockIdx.y * 32;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5; // 32 x 8
+    for (int r = ty; r < 32; r += 8) {
+        const int w = perm[p0 + r];
+        const int j = j0 + tx;
+        tt[r][tx] = (j < n_nodes) ? (w >= 0 ? f_nodes_w[(size_t)w * n_nodes + j] : (double)(j + 1)) : 0.0;
+    }
+    __syncthreads();
+    for (int r = ty; r < 32; r += 8) {
+        const int j = j0 + r;
+        if (j < n_nodes) X[(size_t)j * n_wp + p0 + tx] = tt[tx][r];
+    }
+}
+
+// F2, one thread per system, full Thomas elimination with the walker's own nodes (reading R1: natural BC).
+// c'_j and dp_j are parked in the c- and b-slots of interval j between the sweeps.
+__global__ void __launch_bounds__(128)
+k_spline_pw(const double *__restrict__ Y, const double *__restrict__ X, double *__restrict__ C, int n_wp, int n_nodes, int n_m)
+{
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= n_wp) return;
+    const int sys = blockIdx.y, m = sys >> 1, kind = sys & 1;
+    const size_t sw = (size_t)n_wp;
+    const double *y = Y + (size_t)sys * n_nodes * sw + p;
+    const double *x = X + p;
+    double *c = C + ((size_t)m * 8 + kind * 4) * sw + p;
+    const size_t cj = (size_t)n_m * 8 * sw;
+    const int n = n_nodes;
+    double x0 = __ldg(x), x1 = __ldg(x + sw), y0 = __ldg(y), y1 = __ldg(y + sw);
+    double hm = x1 - x0, sprev = (y1 - y0) / hm;
+    double cpp = 0.0, dpp = 0.0;
+#pragma unroll 4
+    for (int j = 1; j <= n - 2; ++j) {
+        const double x2 = __ldg(x + (size_t)(j + 1) * sw), y2 = __ldg(y + (size_t)(j + 1) * sw);
+        const double hp = x2 - x1;
+        const double s = (y2 - y1) / hp;
+        const double a = (j == 1) ? 0.0 : hm * kSixth, b = (hm + hp) * (1.0 / 3.0), cc = hp * kSixth;
+        const double inv = 1.0 / (b - a * cpp);
+        const double cp = cc * inv, dp = ((s - sprev) - a * dpp) * inv;
+        c[(size_t)j * cj + sw] = dp;
+        c[(size_t)j * cj + 2 * sw] = cp;
+        cpp = cp; dpp = dp; sprev = s; hm = hp; x1 = x2; y1 = y2;
+    }
+    double Mn = 0.0;
+    double xh = __ldg(x + (size_t)(n - 1) * sw), yh = __ldg(y + (size_t)(n - 1) * sw);
+    for (int j = n - 2; j >= 0; --j) {
+        const double xl = __ldg(x + (size_t)j * sw), yl = __ldg(y + (size_t)j * sw);
+        double *cc = c + (size_t)j * cj;
+        const double Mj = (j >= 1) ? fma(-cc[2 * sw], Mn, cc[sw]) : 0.0;
+        const double h = xh - xl, ih = 1.0 / h;
+        cc[0] = yl;
+        cc[sw] = (yh - yl) * ih - h * (2.0 * Mj + Mn) * kSixth;
+        cc[2 * sw] = 0.5 * Mj;
+        cc[3 * sw] = (Mn - Mj) * ih * kSixth;
+        Mn = Mj; xh = xl; yh = yl;
+    }
+}
+
+// F3 with per-walker intervals.  Same mapping and data staging as k_full_fused_tf (one thread = one walker, TMA-fed
+// g/W tiles broadcast from shared memory); every lane tracks its own interval: the bins go up, so the interval index
+// only moves forward, by a comparison with the lane's next node per bin.  NM1: the 8 coefficients of the lane's
+// current interval live in registers; otherwise they are re-read per bin through L1.
+template <int NM1>
+__global__ void __launch_bounds__(128, 3) k_full_fused_pw(FusedArgs a, const double *__restrict__ X)
+{
+    extern __shared__ __align__(128) double sm[];
+    __shared__ __align__(8) uint64_t bar[2];
+    __shared__ int s_lo, s_hi;
+
+    const int tid = threadIdx.x;
+    const int p = blockIdx.x * blockDim.x + tid;
+    const int tile = blockIdx.y;
+    const int i0 = __ldg(a.tile_start + tile), i1 = __ldg(a.tile_start + tile + 1);
+    const int lo = max(a.ilo[p], i0), hi = min(a.ihi[p], i1);
+    if (tid == 0) {
+        s_lo = INT_MAX;
+        s_hi = INT_MIN;
+        mbar_init(&bar[0], 1);
+        mbar_init(&bar[1], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    if (lo < hi) {
+        atomicMin(&s_lo, lo);
+        atomicMax(&s_hi, hi);
+    }
+    __syncthreads();
+    const int blo = s_lo, bhi = s_hi;
+    if (blo >= bhi) return;
+
+    const int CH = a.CH;
+    const int c_begin = blo / CH, c_end = (bhi + CH - 1) / CH;
+    const uint32_t stage_bytes = (uint32_t)CH * 40u;
+    auto issue = [&](int c, int st) {
+        double *dst = sm + (size_t)st * CH * 5;
+        mbar_expect_tx(&bar[st], stage_bytes);
+        tma_load_1d(dst, a.g4 + (size_t)c * CH * 4, (uint32_t)CH * 32u, &bar[st]);
+        tma_load_1d(dst + (size_t)CH * 4, a.Wd + (size_t)c * CH, (uint32_t)CH * 8u, &bar[st]);
+    };
+    if (tid == 0) issue(c_begin, 0);
+
+    const size_t sw = (size_t)a.n_wp;
+    const size_t cm = (size_t)8 * sw, cj = (size_t)a.n_m * cm;
+    const int n = a.n_nodes;
+    const double *x = X + p;
+    // this lane's interval at its first bin: largest j in [0, n-2] with x_j <= f
+    int j = 0;
+    double xj = 0.0, xnext = INFINITY;
+    double co[8];
+    auto load_interval = [&](int jj) {
+        xj = __ldg(x + (size_t)jj * sw);
+        xnext = (jj < n - 2) ? __ldg(x + (size_t)(jj + 1) * sw) : INFINITY;
+        if (NM1) {
+            const double *cc = a.C + (size_t)jj * cj + p;
+#pragma unroll
+            for (int q = 0; q < 8; ++q) co[q] = cc[(size_t)q * sw];
+        }
+    };
+    if (lo < hi) {
+        const double f0 = (double)(a.k_min + lo) * a.df;
+        int l = 0, h = n - 2;
+        while (l < h) {
+            const int mid = (l + h + 1) >> 1;
+            if (__ldg(x + (size_t)mid * sw) <= f0) l = mid; else h = mid - 1;
+        }
+        j = l;
+        load_interval(j);
+    }
+    double s_dh = 0.0, s_hh = 0.0;
+
+    for (int c = c_begin; c < c_end; ++c) {
+        const int st = (c - c_begin) & 1;
+        const uint32_t ph = (uint32_t)((c - c_begin) >> 1) & 1u;
+        if (tid == 0 && c + 1 < c_end) issue(c + 1, st ^ 1);
+        mbar_wait(&bar[st], ph);
+        const double *sg = sm + (size_t)st * CH * 5;
+        const double *sW = sg + (size_t)CH * 4;
+        const int cb = c * CH;
+        const int tlo = max(cb, lo), thi = min(cb + CH, hi);
+        const double4 *sg4 = reinterpret_cast<const double4 *>(sg) - cb;
+        const double *sWc = sW - cb;
+        for (int ii = tlo; ii < thi; ++ii) {
+            const double f = (double)(a.k_min + ii) * a.df;
+            while (f >= xnext) load_interval(++j);
+            const double t = f - xj;
+            double hAr = 0, hAi = 0, hEr = 0, hEi = 0;
+            const int n_m = NM1 ? 1 : a.n_m;
+            for (int m = 0; m < n_m; ++m) {
+                if (!NM1) {
+                    const double *cc = a.C + (size_t)j * cj + (size_t)m * cm + p;
+#pragma unroll
+                    for (int q = 0; q < 8; ++q) co[q] = cc[(size_t)q * sw];
+                }
+                const double A = cubic4(co, t), y = cubic4(co + 4, t);
+                double u, v; // h_m = u - i v
+                amp_expi_qc(A, y, u, v);
+                const double *tf = a.TF + (size_t)m * 4 * sw + p;
+                const double tar = tf[0], tai = tf[sw], ter = tf[2 * sw], tei = tf[3 * sw];
+                hAr = fma(tar, u, hAr); hAr = fma(tai, v, hAr);
+                hAi = fma(tai, u, hAi); hAi = fma(-tar, v, hAi);
+                hEr = fma(ter, u, hEr); hEr = fma(tei, v, hEr);
+                hEi = fma(tei, u, hEi); hEi = fma(-ter, v, hEi);
+            }
+            const double4 g = sg4[ii];
+            const double w = sWc[ii];
+            s_dh = fma(g.x, hAr, s_dh); s_dh = fma(-g.y, hAi, s_dh);
+            s_dh = fma(g.z, hEr, s_dh); s_dh = fma(-g.w, hEi, s_dh);
+            s_hh = fma(w, fma(hAr, hAr, hAi * hAi) + fma(hEr, hEr, hEi * hEi), s_hh);
+        }
+        __syncthreads();
+    }
+    double *o = a.part + ((size_t)tile * 2) * sw + p;
+    o[0] = s_dh; o[sw] = s_hh;
+}
+
 // Eq. 8 utility: t_lm(f_j) = t_ref - (1/2pi) dphi/df at the nodes, dphi/df from the natural spline of the caller's
 // node phases [n_sys][n_nodes] (radians).  One thread per system (off the hot path: the caller needs t_lm to build
 // T(f, t_lm(f)) at the nodes).  scratch [n_nodes][n_sys] holds the forward-sweep values.

@@ -62,3 +62,20 @@ def rand_smooth_nodes(rng, n_w, n_m, f_nodes, phase_scale=200.0):
 def unit_tf(rng, n_w, n_m, n_c=2):
     ang = rng.uniform(0, 2 * np.pi, (n_w, n_m, n_c))
     return np.stack([np.cos(ang), np.sin(ang)], axis=-1)
+
+
+def pw_case(rng, n_w, n_m, n_nodes, n_f, k_min, df):
+    """per-walker node grids: log-spaced nodes over each walker's own span (some start above the grid's first bin,
+    some end below its last), smooth amplitude / phase at the nodes, unit-modulus transfer factors, random data"""
+    f = (k_min + np.arange(n_f)) * df
+    x = np.empty((n_w, n_nodes))
+    for w in range(n_w):
+        x[w] = np.geomspace(f[0] * rng.uniform(0.8, 1.5), f[-1] * rng.uniform(0.4, 1.1), n_nodes)
+    xn = np.log(x / x[:, :1]) / np.log(x[:, -1:] / x[:, :1])
+    amp = 1e-19 * (1.0 + rng.uniform(0.2, 1.0, (n_w, n_m, 1)) * xn[:, None, :] ** 2)
+    ph = 4000.0 * rng.uniform(-1, 1, (n_w, n_m, 1)) * xn[:, None, :] + 25.0 * np.cos(3 * xn[:, None, :] + rng.uniform(0, 6, (n_w, n_m, 1)))
+    ang = rng.uniform(0, 2 * np.pi, (n_w, n_m, 2))
+    tf = np.ascontiguousarray(np.stack([np.cos(ang), np.sin(ang)], axis=-1))
+    W = rng.uniform(0.5, 2.0, n_f) * 1e37
+    d = rng.normal(size=(2, n_f, 2)) * 1e-19
+    return f, x, np.ascontiguousarray(amp), np.ascontiguousarray(ph), tf, W, d

@@ -692,3 +692,36 @@ def test_stop_functions_match_oracle():
     st, ref = binding.StopState(n_checks=3, tol=1.0), sm.StopConverged(3, 1.0)
     for v in [-10.0, -5.0, -4.5, -4.2, -3.9, -2.0, -1.9, -1.8, -1.7, -1.65]:
         assert binding.stop_converged(st, v) == ref.check(v)
+
+
+# ------------------------------------------------------------ per-walker node grids
+@pytest.mark.parametrize("n_m,banded,n_w,n_nodes", [(1, False, 40, 33), (1, True, 97, 64), (3, True, 50, 20), (1, False, 1500, 48)])
+def test_full_per_walker_nodes(orc, torch_cuda, n_m, banded, n_w, n_nodes):
+    from oracle import per_walker as pw
+    from paper_2111_01064_b200 import binding
+    from helpers import pw_case
+    tc = torch_cuda
+    rng = np.random.default_rng(1000 * n_m + n_w)
+    n_f, k_min, df = 5000, 40, 1e-5
+    f, x, amp, ph, tf, W, d = pw_case(rng, n_w, n_m, n_nodes, n_f, k_min, df)
+    band = np.stack([x[:, 0] * rng.uniform(0.9, 1.2, n_w), x[:, -1] * rng.uniform(0.6, 1.2, n_w)], axis=1) if banded else None
+    if banded:
+        band[3] = [f[-1] * 2, f[-1] * 3]                          # a walker whose band misses the grid
+    ctx = binding.Context(n_modes=n_m)
+    ctx.set_data(n_f, k_min, df, dev(tc, d), dev(tc, W))
+    got = ctx.full_batch_pw(dev(tc, x), dev(tc, amp), dev(tc, ph), dev(tc, tf), None if band is None else dev(tc, band))
+    sample = np.arange(n_w) if n_w <= 100 else np.r_[0, 1, 31, 32, 1023, 1024, n_w - 1, rng.integers(0, n_w, 20)]
+    ref = pw.full_batch_pw(x[sample], amp[sample], ph[sample], tf[sample], None if band is None else band[sample],
+                           k_min, df, d, W)
+    check_triplet([__import__("torch").as_tensor(v.cpu().numpy()[sample]) for v in got], ref, "per-walker nodes")
+    if banded:
+        dd_full, _ = ctx.get_dd()
+        assert float(got[0][3]) == -0.5 * dd_full and float(got[2][3]) == 0.0
+    # identical nodes for every walker: the per-walker path equals the shared-node path (needs nodes covering the grid)
+    xs = np.tile(np.geomspace(f[0] * 0.9, f[-1] * 1.05, n_nodes), (n_w, 1))
+    a = ctx.full_batch_pw(dev(tc, xs), dev(tc, amp), dev(tc, ph), dev(tc, tf))
+    b = ctx.full_batch(xs[0], dev(tc, amp), dev(tc, ph), dev(tc, tf))
+    for u, v in zip(a, b):
+        un, vn = u.cpu().numpy(), v.cpu().numpy()
+        assert np.all(np.abs(un - vn) <= 1e-9 * np.maximum(1.0, np.abs(vn)))
+    ctx.destroy()
