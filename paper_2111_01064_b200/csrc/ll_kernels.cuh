@@ -1336,6 +1336,8 @@ __global__ void __launch_bounds__(128, 3) k_full_fused_pw(FusedArgs a, const dou
         j = l;
         load_interval(j);
     }
+    double tf1[4] = {0, 0, 0, 0}; // single mode: the walker's transfer factors stay in registers
+    if (NM1) { tf1[0] = a.TF[p]; tf1[1] = a.TF[sw + p]; tf1[2] = a.TF[2 * sw + p]; tf1[3] = a.TF[3 * sw + p]; }
     double s_dh = 0.0, s_hh = 0.0;
 
     for (int c = c_begin; c < c_end; ++c) {
@@ -1349,9 +1351,7 @@ __global__ void __launch_bounds__(128, 3) k_full_fused_pw(FusedArgs a, const dou
         const int tlo = max(cb, lo), thi = min(cb + CH, hi);
         const double4 *sg4 = reinterpret_cast<const double4 *>(sg) - cb;
         const double *sWc = sW - cb;
-        for (int ii = tlo; ii < thi; ++ii) {
-            const double f = (double)(a.k_min + ii) * a.df;
-            while (f >= xnext) load_interval(++j);
+        auto one_bin = [&](int ii, double f) {
             const double t = f - xj;
             double hAr = 0, hAi = 0, hEr = 0, hEi = 0;
             const int n_m = NM1 ? 1 : a.n_m;
@@ -1364,8 +1364,11 @@ __global__ void __launch_bounds__(128, 3) k_full_fused_pw(FusedArgs a, const dou
                 const double A = cubic4(co, t), y = cubic4(co + 4, t);
                 double u, v; // h_m = u - i v
                 amp_expi_qc(A, y, u, v);
-                const double *tf = a.TF + (size_t)m * 4 * sw + p;
-                const double tar = tf[0], tai = tf[sw], ter = tf[2 * sw], tei = tf[3 * sw];
+                double tar = tf1[0], tai = tf1[1], ter = tf1[2], tei = tf1[3];
+                if (!NM1) {
+                    const double *tf = a.TF + (size_t)m * 4 * sw + p;
+                    tar = tf[0]; tai = tf[sw]; ter = tf[2 * sw]; tei = tf[3 * sw];
+                }
                 hAr = fma(tar, u, hAr); hAr = fma(tai, v, hAr);
                 hAi = fma(tai, u, hAi); hAi = fma(-tar, v, hAi);
                 hEr = fma(ter, u, hEr); hEr = fma(tei, v, hEr);
@@ -1376,6 +1379,21 @@ __global__ void __launch_bounds__(128, 3) k_full_fused_pw(FusedArgs a, const dou
             s_dh = fma(g.x, hAr, s_dh); s_dh = fma(-g.y, hAi, s_dh);
             s_dh = fma(g.z, hEr, s_dh); s_dh = fma(-g.w, hEi, s_dh);
             s_hh = fma(w, fma(hAr, hAr, hAi * hAi) + fma(hEr, hEr, hEi * hEi), s_hh);
+        };
+        int ii = tlo;
+        while (ii < thi) {
+            const double f = (double)(a.k_min + ii) * a.df;
+            while (f >= xnext) load_interval(++j);
+            // four bins at once while they stay inside this lane's interval (intervals are hundreds of bins wide
+            // almost everywhere): four independent chains, no interval test in between
+            if (NM1 && ii + 4 <= thi && (double)(a.k_min + ii + 3) * a.df < xnext) {
+#pragma unroll
+                for (int k = 0; k < 4; ++k) one_bin(ii + k, (double)(a.k_min + ii + k) * a.df);
+                ii += 4;
+            } else {
+                one_bin(ii, f);
+                ii += 1;
+            }
         }
         __syncthreads();
     }
