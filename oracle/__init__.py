@@ -71,6 +71,19 @@ def spline_natural(x, y) -> np.ndarray:
     return M
 
 
+def set_spline_bc(bc: int) -> None:
+    """0 natural (default, reading R1), 1 not-a-knot: process-wide switch of the C oracle (see ll_oracle.c)"""
+    _check(lib().orc_set_spline_bc(C.c_int(bc)), "set_spline_bc")
+
+
+def spline_second_derivatives(x, y) -> np.ndarray:
+    """M_j = y''(x_j) under the current boundary condition"""
+    x, y = _f64(x), _f64(y)
+    M = np.empty_like(x)
+    _check(lib().orc_spline_second_derivatives(C.c_int(len(x)), _p(x), _p(y), _p(M)), "spline_second_derivatives")
+    return M
+
+
 def spline_eval(x, y, f_q) -> np.ndarray:
     x, y, f_q = _f64(x), _f64(y), _f64(f_q)
     out = np.empty_like(f_q)

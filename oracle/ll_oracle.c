@@ -91,6 +91,68 @@ static int spline_natural_ld(int n, const double *x, const ld *y, ld *M)
     return 0;
 }
 
+/* ---------------------------------------------------------------------------------------------
+ * Not-a-knot cubic spline (R1 lists it as the optional boundary condition).
+ * The interior rows are those of the natural spline.  The two end conditions say that the third derivative is
+ * continuous across x_1 and across x_{n-2}:
+ *   (M_1 - M_0)/h_0 = (M_2 - M_1)/h_1              =>  M_0     = (1 + h_0/h_1) M_1 - (h_0/h_1) M_2
+ *   (M_{n-1} - M_{n-2})/h_{n-2} = (M_{n-2} - M_{n-3})/h_{n-3}
+ *                                                  =>  M_{n-1} = (1 + h_{n-2}/h_{n-3}) M_{n-2} - (h_{n-2}/h_{n-3}) M_{n-3}
+ * Substituting them into rows 1 and n-2 keeps the system tridiagonal in M_1..M_{n-2} (n >= 4):
+ *   row 1  : [ (h_0+h_1)/3 + (h_0/6)(1 + h_0/h_1) ] M_1 + [ h_1/6 - (h_0/6)(h_0/h_1) ] M_2 = r_1
+ *   row n-2: [ h_{n-3}/6 - (h_{n-2}/6)(h_{n-2}/h_{n-3}) ] M_{n-3}
+ *            + [ (h_{n-3}+h_{n-2})/3 + (h_{n-2}/6)(1 + h_{n-2}/h_{n-3}) ] M_{n-2} = r_{n-2}
+ * Naive Thomas elimination, then the two end values.
+ * ------------------------------------------------------------------------------------------- */
+static int spline_notaknot_ld(int n, const double *x, const ld *y, ld *M)
+{
+    if (n < 4) return -1;
+    ld *cp = (ld *)malloc(sizeof(ld) * (size_t)n);
+    ld *dp = (ld *)malloc(sizeof(ld) * (size_t)n);
+    if (!cp || !dp) { free(cp); free(dp); return -4; }
+    const ld h0 = (ld)x[1] - (ld)x[0], h1 = (ld)x[2] - (ld)x[1];
+    const ld hl = (ld)x[n - 1] - (ld)x[n - 2], hk = (ld)x[n - 2] - (ld)x[n - 3];
+    const ld rho0 = h0 / h1, rhon = hl / hk;
+    for (int j = 1; j <= n - 2; ++j) {
+        ld hm = (ld)x[j] - (ld)x[j - 1];
+        ld hp = (ld)x[j + 1] - (ld)x[j];
+        ld a = hm / 6.0L, b = (hm + hp) / 3.0L, c = hp / 6.0L;
+        ld r = (y[j + 1] - y[j]) / hp - (y[j] - y[j - 1]) / hm;
+        if (j == 1)     { b += a * (1.0L + rho0); c -= a * rho0; a = 0.0L; }
+        if (j == n - 2) { b += c * (1.0L + rhon); a -= c * rhon; c = 0.0L; }
+        if (j == 1) {
+            cp[j] = c / b;
+            dp[j] = r / b;
+        } else {
+            ld den = b - a * cp[j - 1];
+            cp[j] = c / den;
+            dp[j] = (r - a * dp[j - 1]) / den;
+        }
+    }
+    M[n - 2] = dp[n - 2];
+    for (int j = n - 3; j >= 1; --j)
+        M[j] = dp[j] - cp[j] * M[j + 1];
+    M[0] = (1.0L + rho0) * M[1] - rho0 * M[2];
+    M[n - 1] = (1.0L + rhon) * M[n - 2] - rhon * M[n - 3];
+    free(cp); free(dp);
+    return 0;
+}
+
+/* Which boundary condition the splines of this library use: 0 natural (the default, reading R1), 1 not-a-knot.
+ * One process-wide switch (set it before a call, not during one), so that every path that splines node arrays
+ * (amplitude, phase, transfer function) follows it without a second copy of each entry point. */
+static int g_spline_bc = 0;
+int orc_set_spline_bc(int bc)
+{
+    if (bc != 0 && bc != 1) return -1;
+    g_spline_bc = bc;
+    return 0;
+}
+static int spline_ld(int n, const double *x, const ld *y, ld *M)
+{
+    return g_spline_bc ? spline_notaknot_ld(n, x, y, M) : spline_natural_ld(n, x, y, M);
+}
+
 /* interval index: largest j with x_j <= f, clamped to [0, n-2] (R21) */
 static int find_interval(int n, const double *x, double f)
 {
@@ -124,12 +186,23 @@ int orc_spline_natural(int n, const double *x, const double *y, double *M_out)
     return rc;
 }
 
+int orc_spline_second_derivatives(int n, const double *x, const double *y, double *M_out)
+{
+    ld *yl = (ld *)malloc(sizeof(ld) * (size_t)n), *M = (ld *)malloc(sizeof(ld) * (size_t)n);
+    if (!yl || !M) { free(yl); free(M); return -4; }
+    for (int j = 0; j < n; ++j) yl[j] = (ld)y[j];
+    int rc = spline_ld(n, x, yl, M);
+    if (rc == 0) for (int j = 0; j < n; ++j) M_out[j] = (double)M[j];
+    free(yl); free(M);
+    return rc;
+}
+
 int orc_spline_eval(int n, const double *x, const double *y, int64_t n_q, const double *f_q, double *out)
 {
     ld *yl = (ld *)malloc(sizeof(ld) * (size_t)n), *M = (ld *)malloc(sizeof(ld) * (size_t)n);
     if (!yl || !M) { free(yl); free(M); return -4; }
     for (int j = 0; j < n; ++j) yl[j] = (ld)y[j];
-    int rc = spline_natural_ld(n, x, yl, M);
+    int rc = spline_ld(n, x, yl, M);
     if (rc == 0)
         for (int64_t i = 0; i < n_q; ++i)
             out[i] = (double)spline_eval_ld(x, yl, M, find_interval(n, x, f_q[i]), f_q[i]);
@@ -277,8 +350,8 @@ int orc_full_batch(int64_t n_w, int n_m, int n_c, int n_nodes, const double *f_n
                 yA[m * nn + j] = (ld)amp[(w * n_m + m) * nn + j];
                 yP[m * nn + j] = (ld)phase[(w * n_m + m) * nn + j];
             }
-            spline_natural_ld(n_nodes, f_nodes, yA + m * nn, MA + m * nn);
-            spline_natural_ld(n_nodes, f_nodes, yP + m * nn, MP + m * nn);
+            spline_ld(n_nodes, f_nodes, yA + m * nn, MA + m * nn);
+            spline_ld(n_nodes, f_nodes, yP + m * nn, MP + m * nn);
         }
         const double f_lo = band ? band[2 * w] : -HUGE_VAL, f_hi = band ? band[2 * w + 1] : HUGE_VAL;
         ld s_dh = 0.0L, s_hh = 0.0L, s_res = 0.0L;
@@ -349,7 +422,7 @@ int orc_full_batch_tf(int64_t n_w, int n_m, int n_c, int n_nodes, const double *
                     ym[(3 + 2 * c) * nn + j] = (ld)t[1];
                 }
             }
-            for (int s = 0; s < 2 + 2 * n_c; ++s) spline_natural_ld(n_nodes, f_nodes, ym + s * nn, Mm + s * nn);
+            for (int s = 0; s < 2 + 2 * n_c; ++s) spline_ld(n_nodes, f_nodes, ym + s * nn, Mm + s * nn);
         }
         const double f_lo = band ? band[2 * w] : -HUGE_VAL, f_hi = band ? band[2 * w + 1] : HUGE_VAL;
         ld s_dh = 0.0L, s_hh = 0.0L, s_res = 0.0L;

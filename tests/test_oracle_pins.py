@@ -858,3 +858,78 @@ def test_per_walker_nodes_do_not_matter_for_a_spline_reproducible_template(orc):
     rb = pw.full_batch_pw(xb[None], *lin(xb), tf, None, k_min, df, d, W)
     for k in ("logL", "d_h", "h_h"):
         assert ra[k][0] == pytest.approx(rb[k][0], rel=1e-11)
+
+
+# --------------------------------------------------------------------------- not-a-knot boundary condition
+@pytest.fixture
+def notaknot(orc):
+    orc.set_spline_bc(1)
+    yield orc
+    orc.set_spline_bc(0)
+
+
+@pytest.mark.parametrize("n", [4, 5, 16, 257])
+def test_notaknot_spline_matches_scipy(notaknot, n):
+    """SciPy's CubicSpline default IS not-a-knot: values, second derivatives at the nodes."""
+    orc = notaknot
+    rng = np.random.default_rng(n)
+    x = np.sort(rng.uniform(1e-4, 5e-2, n)) if n < 100 else np.geomspace(1e-4, 5e-2, n)
+    y = np.cumsum(rng.normal(size=n)) * 50.0
+    cs = CubicSpline(x, y)                                                       # bc_type='not-a-knot'
+    q = np.r_[x, rng.uniform(x[0], x[-1], 300)]
+    np.testing.assert_allclose(orc.spline_eval(x, y, q), cs(q), rtol=1e-10, atol=1e-9 * np.abs(y).max())
+    M = orc.spline_second_derivatives(x, y)
+    np.testing.assert_allclose(M, cs(x, 2), rtol=1e-7, atol=1e-8 * np.abs(cs(x, 2)).max())
+
+
+def test_notaknot_reproduces_a_single_cubic_and_differs_from_natural(notaknot):
+    """Not-a-knot reproduces any cubic exactly (natural does not: it forces y'' = 0 at the ends); the third
+    derivative is continuous across x_1 and x_{n-2}; dense elimination of the full (n x n) system agrees."""
+    orc = notaknot
+    rng = np.random.default_rng(9)
+    x = np.sort(rng.uniform(0.0, 2.0, 9))
+    cub = lambda t: 1.0 - 2.0 * t + 0.7 * t ** 2 + 3.0 * t ** 3
+    q = np.linspace(x[0], x[-1], 101)
+    np.testing.assert_allclose(orc.spline_eval(x, cub(x), q), cub(q), rtol=1e-12)
+    orc.set_spline_bc(0)
+    assert np.max(np.abs(orc.spline_eval(x, cub(x), q) - cub(q))) > 1e-3
+    orc.set_spline_bc(1)
+    y = rng.normal(size=9)
+    M = orc.spline_second_derivatives(x, y)
+    h = np.diff(x)
+    d3 = np.diff(M) / h
+    assert d3[0] == pytest.approx(d3[1], rel=1e-9) and d3[-1] == pytest.approx(d3[-2], rel=1e-9)
+    A = np.zeros((9, 9)); r = np.zeros(9)
+    for j in range(1, 8):
+        A[j, j - 1], A[j, j], A[j, j + 1] = h[j - 1] / 6, (h[j - 1] + h[j]) / 3, h[j] / 6
+        r[j] = (y[j + 1] - y[j]) / h[j] - (y[j] - y[j - 1]) / h[j - 1]
+    A[0, :3] = [-1 / h[0], 1 / h[0] + 1 / h[1], -1 / h[1]]
+    A[8, -3:] = [-1 / h[-2], 1 / h[-2] + 1 / h[-1], -1 / h[-1]]
+    np.testing.assert_allclose(M, np.linalg.solve(A, r), rtol=1e-9, atol=1e-10 * np.abs(M).max())
+
+
+def test_notaknot_full_path_brute_force(notaknot):
+    """the full-grid path under the switch against SciPy's not-a-knot spline + numpy complex sums"""
+    orc = notaknot
+    rng = np.random.default_rng(10)
+    n_w, n_m, n_nodes, n_f, k_min, df = 3, 2, 8, 48, 20, 1e-4
+    f = (k_min + np.arange(n_f)) * df
+    x = np.geomspace(f[0] * 0.9, f[-1] * 1.1, n_nodes)
+    amp = 1e-19 * rng.uniform(0.5, 2.0, (n_w, n_m, n_nodes))
+    ph = np.cumsum(rng.uniform(0.0, 3.0, (n_w, n_m, n_nodes)), axis=2)
+    ang = rng.uniform(0, 2 * np.pi, (n_w, n_m, 2))
+    tf = np.stack([np.cos(ang), np.sin(ang)], axis=-1)
+    W = rng.uniform(0.5, 2.0, n_f) * 1e37
+    d = rng.normal(size=(2, n_f, 2)) * 1e-19
+    got = orc.full_batch(x, amp, ph, tf, None, k_min, df, d, W)
+    dc = d[..., 0] + 1j * d[..., 1]
+    for w in range(n_w):
+        h = np.zeros((2, n_f), complex)
+        for m in range(n_m):
+            hm = CubicSpline(x, amp[w, m])(f) * np.exp(-1j * CubicSpline(x, ph[w, m])(f))
+            for c in range(2):
+                h[c] += (tf[w, m, c, 0] + 1j * tf[w, m, c, 1]) * hm
+        d_h = (W * (np.conj(dc) * h).real).sum()
+        h_h = (W * np.abs(h) ** 2).sum()
+        assert got["d_h"][w] == pytest.approx(d_h, rel=1e-9, abs=1e-9 * h_h)
+        assert got["h_h"][w] == pytest.approx(h_h, rel=1e-10)
