@@ -54,6 +54,7 @@ enum {
 };
 
 enum { LL_PREC_FP64 = 0, LL_PREC_FP32_ACC = 1 };
+enum { LL_BC_NATURAL = 0, LL_BC_NOT_A_KNOT = 1 }; /* not-a-knot needs n_nodes >= 4; ll_tlm_nodes is natural-only */
 
 #define LL_MAX_MODES 8
 #define LL_N_CHANNELS 2
@@ -63,7 +64,8 @@ typedef struct {
     int32_t n_channels; /* must be 2 (TDI A and E; reading R5)                                 */
     int32_t n_modes;    /* 1..LL_MAX_MODES harmonics (l,m) summed per channel (Eq. 9)                       */
     int32_t precision;  /* LL_PREC_FP64, or LL_PREC_FP32_ACC (full-grid path only; reading R15)             */
-    int32_t reserved[4];
+    int32_t spline_bc;  /* LL_BC_NATURAL (reading R1) or LL_BC_NOT_A_KNOT: boundary condition of every node spline   */
+    int32_t reserved[3];
 } ll_config;
 
 /* Create / destroy a context.  ll_create selects `device`, checks it is usable and allocates nothing big. */

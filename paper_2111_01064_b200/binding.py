@@ -17,6 +17,7 @@ SO_PATH = os.path.join(_HERE, "libll_b200.so")
 
 LL_OK, LL_ERR_ARG, LL_ERR_STATE, LL_ERR_CUDA, LL_ERR_NOMEM, LL_ERR_UNSUPPORTED, LL_ERR_REF_ZERO = 0, -1, -2, -3, -4, -5, -6
 LL_PREC_FP64, LL_PREC_FP32_ACC = 0, 1
+LL_BC_NATURAL, LL_BC_NOT_A_KNOT = 0, 1
 
 # every symbol include/ll.h declares (tests/test_abi.py checks header and library against this list)
 SYMBOLS = (
@@ -38,7 +39,7 @@ class LLError(RuntimeError):
 
 class ll_config(C.Structure):
     _fields_ = [("device", C.c_int32), ("n_channels", C.c_int32), ("n_modes", C.c_int32), ("precision", C.c_int32),
-                ("reserved", C.c_int32 * 4)]
+                ("spline_bc", C.c_int32), ("reserved", C.c_int32 * 3)]
 
 
 _lib = None
@@ -155,14 +156,15 @@ def stop_converged(state: StopState, max_logL: float) -> bool:
 class Context:
     """One `ll_ctx` (include/ll.h).  Methods carry the C names without the `ll_` prefix."""
 
-    def __init__(self, n_modes: int = 1, precision: int = LL_PREC_FP64, device: Optional[int] = None, n_channels: int = 2):
+    def __init__(self, n_modes: int = 1, precision: int = LL_PREC_FP64, device: Optional[int] = None, n_channels: int = 2,
+                 spline_bc: int = 0):
         torch = _torch()
         if not torch.cuda.is_available():
             raise LLError(LL_ERR_CUDA, "ll_create", "no CUDA device (there is no CPU fallback)")
         self._lib = load_library()
         self.device = torch.cuda.current_device() if device is None else int(device)
         self.n_modes, self.n_channels, self.precision = int(n_modes), int(n_channels), int(precision)
-        cfg = ll_config(self.device, self.n_channels, self.n_modes, self.precision, (C.c_int32 * 4)(0, 0, 0, 0))
+        cfg = ll_config(self.device, self.n_channels, self.n_modes, self.precision, int(spline_bc), (C.c_int32 * 3)(0, 0, 0))
         h = C.c_void_p()
         rc = self._lib.ll_create(C.byref(cfg), C.byref(h))
         if rc != LL_OK:

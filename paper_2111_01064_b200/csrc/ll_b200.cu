@@ -62,7 +62,7 @@ struct FullPlan {
 } // namespace
 
 struct ll_ctx {
-    int device = 0, n_c = 2, n_m = 1, precision = 0;
+    int device = 0, n_c = 2, n_m = 1, precision = 0, spline_bc = 0;
     int sm_count = 148;
     std::string err;
     int64_t launches = 0;
@@ -192,6 +192,7 @@ int prepare_nodes(ll_ctx *ctx, int n, const double *x, cudaStream_t st)
         return LL_OK;
     ctx->nodes_valid = false;
     if (n < 3) return ctx->fail(LL_ERR_ARG, "n_nodes must be >= 3");
+    if (n < 4 && ctx->spline_bc == LL_BC_NOT_A_KNOT) return ctx->fail(LL_ERR_ARG, "the not-a-knot boundary condition needs n_nodes >= 4");
     for (int j = 0; j + 1 < n; ++j)
         if (!(x[j + 1] > x[j])) return ctx->fail(LL_ERR_ARG, "f_nodes must be strictly ascending and finite");
     const double f_first = bin_freq(ctx->k_min, 0, ctx->df), f_last = bin_freq(ctx->k_min, ctx->n_f - 1, ctx->df);
@@ -215,12 +216,23 @@ int prepare_nodes(ll_ctx *ctx, int n, const double *x, cudaStream_t st)
         hj[j] = (double)h;
         invh[j] = (double)(1.0L / h);
     }
-    // Thomas factorisation of rows 1..n-2 of the natural-spline system (M_0 = M_{n-1} = 0)
+    // Thomas factorisation of rows 1..n-2 of the spline system.  Natural: M_0 = M_{n-1} = 0.  Not-a-knot: the end
+    // conditions M_0 = (1 + rho0) M_1 - rho0 M_2, M_{n-1} = (1 + rhon) M_{n-2} - rhon M_{n-3} (third derivative
+    // continuous across x_1 and x_{n-2}) substituted into rows 1 and n-2, which stay tridiagonal.
+    ld rho0 = 0.0L, rhon = 0.0L;
+    if (ctx->spline_bc == LL_BC_NOT_A_KNOT) {
+        rho0 = ((ld)x[1] - (ld)x[0]) / ((ld)x[2] - (ld)x[1]);
+        rhon = ((ld)x[n - 1] - (ld)x[n - 2]) / ((ld)x[n - 2] - (ld)x[n - 3]);
+    }
     {
         ld cprev = 0.0L;
         for (int j = 1; j <= n - 2; ++j) {
             const ld hm = (ld)x[j] - (ld)x[j - 1], hp = (ld)x[j + 1] - (ld)x[j];
-            const ld a = hm / 6.0L, b = (hm + hp) / 3.0L, c = hp / 6.0L;
+            ld a = hm / 6.0L, b = (hm + hp) / 3.0L, c = hp / 6.0L;
+            if (ctx->spline_bc == LL_BC_NOT_A_KNOT) {
+                if (j == 1)     { b += a * (1.0L + rho0); c -= a * rho0; }
+                if (j == n - 2) { b += c * (1.0L + rhon); a -= c * rhon; c = 0.0L; }
+            }
             const ld den = (j == 1) ? b : b - a * cprev;
             const ld cp = c / den;
             ta[j] = (j == 1) ? 0.0 : (double)a;
@@ -255,6 +267,7 @@ int prepare_nodes(ll_ctx *ctx, int n, const double *x, cudaStream_t st)
     NodeTables &nt = ctx->nt;
     nt.xj = b; nt.hj = b + n; nt.invh = b + 2 * n; nt.ta = b + 3 * n; nt.tcp = b + 4 * n; nt.tinv = b + 5 * n;
     nt.f4 = b + 6 * n; nt.cfp = b + 7 * n; nt.f2m = nt.cfp + (size_t)n_m * n; nt.fm53 = nt.f2m + (size_t)n_m * n;
+    nt.bc = ctx->spline_bc; nt.rho0 = (double)rho0; nt.rhon = (double)rhon;
     nt.bstart = reinterpret_cast<const int *>((const char *)ctx->node_tab.p + bytes_d);
     ctx->nodes_host.assign(x, x + n);
     ctx->bstart_host = hi;
@@ -534,7 +547,7 @@ int run_full_pw(ll_ctx *ctx, long long n_w, int n_nodes, const double *f_nodes_w
         k_pw_nodes_x<<<gx, 256, 0, st>>>(f_nodes_w, ctx->perm.as<int>(), n_wp, n_nodes, X);
         LAUNCHED(ctx);
         dim3 gs(ceil_div(n_wp, 128), 2 * n_m);
-        k_spline_pw<<<gs, 128, 0, st>>>(ctx->Y.as<double>(), X, ctx->C.as<double>(), n_wp, n_nodes, n_m);
+        k_spline_pw<<<gs, 128, 0, st>>>(ctx->Y.as<double>(), X, ctx->C.as<double>(), n_wp, n_nodes, n_m, ctx->spline_bc);
         LAUNCHED(ctx);
     }
     FusedArgs fa;
@@ -780,6 +793,7 @@ int ll_create(const ll_config *cfg, ll_ctx **out)
     if (cfg->n_channels != LL_N_CHANNELS) return LL_ERR_UNSUPPORTED;
     if (cfg->n_modes < 1 || cfg->n_modes > LL_MAX_MODES) return LL_ERR_UNSUPPORTED;
     if (cfg->precision != LL_PREC_FP64 && cfg->precision != LL_PREC_FP32_ACC) return LL_ERR_UNSUPPORTED;
+    if (cfg->spline_bc != LL_BC_NATURAL && cfg->spline_bc != LL_BC_NOT_A_KNOT) return LL_ERR_UNSUPPORTED;
     int n_dev = 0;
     if (cudaGetDeviceCount(&n_dev) != cudaSuccess || cfg->device < 0 || cfg->device >= n_dev) {
         (void)cudaGetLastError();
@@ -791,6 +805,7 @@ int ll_create(const ll_config *cfg, ll_ctx **out)
     ctx->n_c = cfg->n_channels;
     ctx->n_m = cfg->n_modes;
     ctx->precision = cfg->precision;
+    ctx->spline_bc = cfg->spline_bc;
     DeviceGuard dg(ctx->device);
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, ctx->device) != cudaSuccess) {
@@ -938,6 +953,7 @@ int ll_full_batch_pw(ll_ctx *ctx, int64_t n_w, int32_t n_nodes, const double *f_
     if (n_w < 0) return ctx->fail(LL_ERR_ARG, "n_w < 0");
     if (n_w > (1 << 24)) return ctx->fail(LL_ERR_ARG, "n_w > 2^24 per call: split the batch");
     if (n_nodes < 3 || n_nodes > (1 << 20)) return ctx->fail(LL_ERR_ARG, "n_nodes out of range [3, 2^20]");
+    if (n_nodes < 4 && ctx->spline_bc == LL_BC_NOT_A_KNOT) return ctx->fail(LL_ERR_ARG, "the not-a-knot boundary condition needs n_nodes >= 4");
     if (n_w > 0 && (!f_nodes_w || !amp || !phase || !tf || !logL)) return ctx->fail(LL_ERR_ARG, "NULL argument");
     if (!ctx->have_data) return ctx->fail(LL_ERR_STATE, "ll_set_data has not been called");
     if (ctx->precision != LL_PREC_FP64) return ctx->fail(LL_ERR_UNSUPPORTED, "ll_full_batch_pw is FP64 only");
@@ -990,6 +1006,7 @@ int ll_tlm_nodes(ll_ctx *ctx, int64_t n_w, int32_t n_nodes, const double *f_node
     if (!f_nodes) return ctx->fail(LL_ERR_ARG, "f_nodes is NULL");
     if (n_w > 0 && (!phase || !t_lm)) return ctx->fail(LL_ERR_ARG, "phase or t_lm is NULL");
     if (!ctx->have_data) return ctx->fail(LL_ERR_STATE, "ll_set_data has not been called (the node tables are tied to the grid)");
+    if (ctx->spline_bc != LL_BC_NATURAL) return ctx->fail(LL_ERR_UNSUPPORTED, "ll_tlm_nodes differentiates the natural spline only");
     DeviceGuard dg(ctx->device);
     cudaStream_t st = (cudaStream_t)stream;
     int rc = prepare_nodes(ctx, n_nodes, f_nodes, st);

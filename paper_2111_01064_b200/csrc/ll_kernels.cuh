@@ -259,6 +259,8 @@ struct NodeTables {
     const double *f2m;   // [n_m][n]
     const double *fm53;  // [n_m][n]
     const int *bstart;   // [n]: interval j covers dense bins [bstart[j], bstart[j+1]), j = 0..n-2
+    int bc;              // 0 natural, 1 not-a-knot (the tables above are then those of the substituted system)
+    double rho0, rhon;   // not-a-knot: M_0 = (1+rho0) M_1 - rho0 M_2,  M_{n-1} = (1+rhon) M_{n-2} - rhon M_{n-3}
 };
 
 struct WalkerConst { // per walker constants of the stand-in
@@ -465,7 +467,12 @@ k_spline(const double *__restrict__ Y, double *__restrict__ C, int n_wp, int n_n
     // block are loaded first (independent loads, all in flight together), then the recurrence runs on
     // registers, then the coefficients are stored.  (A load of dp_j issued between the stores of interval
     // j + 1 could not be hoisted by the compiler: same base pointer, so each step paid a full memory latency.)
-    double Mn = 0.0;
+    double Mn = 0.0, Mnn = 0.0; // M_{j+1}, M_{j+2}
+    if (nt.bc) { // not-a-knot: M_{n-1} from M_{n-2} = dp_{n-2} (its c' is 0) and M_{n-3}
+        const double M2 = c[(size_t)(n - 2) * cj + sw];
+        const double M3 = fma(-__ldg(nt.tcp + n - 3), M2, c[(size_t)(n - 3) * cj + sw]);
+        Mn = (1.0 + nt.rhon) * M2 - nt.rhon * M3;
+    }
     double y1 = __ldg(y + (size_t)(n - 1) * sw);
     for (int jt = n - 2; jt >= 0; jt -= kSplineBlk) {
         double dpv[kSplineBlk], yv[kSplineBlk];
@@ -480,13 +487,15 @@ k_spline(const double *__restrict__ Y, double *__restrict__ C, int n_wp, int n_n
             const int j = jt - k;
             if (j >= 0) {
                 const double y0 = yv[k];
-                const double Mj = (j >= 1) ? fma(-__ldg(nt.tcp + j), Mn, dpv[k]) : 0.0;
+                const double Mj = (j >= 1) ? fma(-__ldg(nt.tcp + j), Mn, dpv[k])
+                                           : (nt.bc ? (1.0 + nt.rho0) * Mn - nt.rho0 * Mnn : 0.0);
                 const double h = __ldg(nt.hj + j), ih = __ldg(nt.invh + j);
                 double *cc = c + (size_t)j * cj;
                 cc[0] = y0;
                 cc[sw] = (y1 - y0) * ih - h * (2.0 * Mj + Mn) * kSixth;
                 cc[2 * sw] = 0.5 * Mj;
                 cc[3 * sw] = (Mn - Mj) * ih * kSixth;
+                Mnn = Mn;
                 Mn = Mj;
                 y1 = y0;
             }
@@ -593,6 +602,13 @@ k_spline_block(const double *__restrict__ Y, double *__restrict__ C, int n_wp, i
         ds[j] = Mn;
     }
     __syncthreads();
+    if (nt.bc) { // not-a-knot end values from their neighbours
+        if (tid == 0) {
+            ds[0] = (1.0 + nt.rho0) * ds[1] - nt.rho0 * ds[2];
+            ds[n - 1] = (1.0 + nt.rhon) * ds[n - 2] - nt.rhon * ds[n - 3];
+        }
+        __syncthreads();
+    }
     // ---- coefficients of interval j (same formulas as k_spline)
     double *c = C + ((size_t)m * ns * 4 + kind * 4) * sw + p;
     const size_t cj = (size_t)n_m * ns * 4 * sw;
@@ -1225,7 +1241,8 @@ k_pw_nodes_x(const double *__restrict__ f_nodes_w, const int *__restrict__ perm,
 // F2, one thread per system, full Thomas elimination with the walker's own nodes (reading R1: natural BC).
 // c'_j and dp_j are parked in the c- and b-slots of interval j between the sweeps.
 __global__ void __launch_bounds__(128)
-k_spline_pw(const double *__restrict__ Y, const double *__restrict__ X, double *__restrict__ C, int n_wp, int n_nodes, int n_m)
+k_spline_pw(const double *__restrict__ Y, const double *__restrict__ X, double *__restrict__ C, int n_wp, int n_nodes, int n_m,
+            int bc)
 {
     const int p = blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= n_wp) return;
@@ -1238,31 +1255,41 @@ k_spline_pw(const double *__restrict__ Y, const double *__restrict__ X, double *
     const int n = n_nodes;
     double x0 = __ldg(x), x1 = __ldg(x + sw), y0 = __ldg(y), y1 = __ldg(y + sw);
     double hm = x1 - x0, sprev = (y1 - y0) / hm;
-    double cpp = 0.0, dpp = 0.0;
+    double cpp = 0.0, dpp = 0.0, rho0 = 0.0, rhon = 0.0;
 #pragma unroll 4
     for (int j = 1; j <= n - 2; ++j) {
         const double x2 = __ldg(x + (size_t)(j + 1) * sw), y2 = __ldg(y + (size_t)(j + 1) * sw);
         const double hp = x2 - x1;
         const double s = (y2 - y1) / hp;
-        const double a = (j == 1) ? 0.0 : hm * kSixth, b = (hm + hp) * (1.0 / 3.0), cc = hp * kSixth;
+        double a = hm * kSixth, b = (hm + hp) * (1.0 / 3.0), cc = hp * kSixth;
+        if (bc) { // not-a-knot: end conditions substituted into rows 1 and n-2
+            if (j == 1) { rho0 = hm / hp; b += a * (1.0 + rho0); cc -= a * rho0; }
+            if (j == n - 2) { rhon = hp / hm; b += cc * (1.0 + rhon); a -= cc * rhon; cc = 0.0; }
+        }
+        if (j == 1) a = 0.0;
         const double inv = 1.0 / (b - a * cpp);
         const double cp = cc * inv, dp = ((s - sprev) - a * dpp) * inv;
         c[(size_t)j * cj + sw] = dp;
         c[(size_t)j * cj + 2 * sw] = cp;
         cpp = cp; dpp = dp; sprev = s; hm = hp; x1 = x2; y1 = y2;
     }
-    double Mn = 0.0;
+    double Mn = 0.0, Mnn = 0.0;
+    if (bc) {
+        const double M2 = c[(size_t)(n - 2) * cj + sw];
+        const double M3 = fma(-c[(size_t)(n - 3) * cj + 2 * sw], M2, c[(size_t)(n - 3) * cj + sw]);
+        Mn = (1.0 + rhon) * M2 - rhon * M3;
+    }
     double xh = __ldg(x + (size_t)(n - 1) * sw), yh = __ldg(y + (size_t)(n - 1) * sw);
     for (int j = n - 2; j >= 0; --j) {
         const double xl = __ldg(x + (size_t)j * sw), yl = __ldg(y + (size_t)j * sw);
         double *cc = c + (size_t)j * cj;
-        const double Mj = (j >= 1) ? fma(-cc[2 * sw], Mn, cc[sw]) : 0.0;
+        const double Mj = (j >= 1) ? fma(-cc[2 * sw], Mn, cc[sw]) : (bc ? (1.0 + rho0) * Mn - rho0 * Mnn : 0.0);
         const double h = xh - xl, ih = 1.0 / h;
         cc[0] = yl;
         cc[sw] = (yh - yl) * ih - h * (2.0 * Mj + Mn) * kSixth;
         cc[2 * sw] = 0.5 * Mj;
         cc[3 * sw] = (Mn - Mj) * ih * kSixth;
-        Mn = Mj; xh = xl; yh = yl;
+        Mnn = Mn; Mn = Mj; xh = xl; yh = yl;
     }
 }
 

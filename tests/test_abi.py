@@ -66,7 +66,7 @@ def test_no_cpu_fallback_without_gpu(so_path):
         pytest.skip("GPU present")
     from paper_2111_01064_b200 import binding
     lib = binding.load_library()
-    cfg = binding.ll_config(0, 2, 1, 0, (C.c_int32 * 4)(0, 0, 0, 0))
+    cfg = binding.ll_config(0, 2, 1, 0, 0, (C.c_int32 * 3)(0, 0, 0))
     h = C.c_void_p()
     assert lib.ll_create(C.byref(cfg), C.byref(h)) == binding.LL_ERR_CUDA
     with pytest.raises(binding.LLError):
@@ -77,8 +77,8 @@ def test_create_rejects_bad_config(so_path):
     from paper_2111_01064_b200 import binding
     lib = binding.load_library()
     h = C.c_void_p()
-    for dev, nc, nm, prec in ((0, 3, 1, 0), (0, 2, 0, 0), (0, 2, 9, 0), (0, 2, 1, 7)):
-        cfg = binding.ll_config(dev, nc, nm, prec, (C.c_int32 * 4)(0, 0, 0, 0))
+    for dev, nc, nm, prec, bc in ((0, 3, 1, 0, 0), (0, 2, 0, 0, 0), (0, 2, 9, 0, 0), (0, 2, 1, 7, 0), (0, 2, 1, 0, 2)):
+        cfg = binding.ll_config(dev, nc, nm, prec, bc, (C.c_int32 * 3)(0, 0, 0))
         assert lib.ll_create(C.byref(cfg), C.byref(h)) == binding.LL_ERR_UNSUPPORTED
     assert lib.ll_create(None, C.byref(h)) == binding.LL_ERR_ARG
     assert lib.ll_destroy(None) == binding.LL_ERR_ARG

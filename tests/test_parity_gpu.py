@@ -725,3 +725,56 @@ def test_full_per_walker_nodes(orc, torch_cuda, n_m, banded, n_w, n_nodes):
         un, vn = u.cpu().numpy(), v.cpu().numpy()
         assert np.all(np.abs(un - vn) <= 1e-9 * np.maximum(1.0, np.abs(vn)))
     ctx.destroy()
+
+
+# ------------------------------------------------------- not-a-knot boundary condition
+@pytest.fixture
+def notaknot(orc):
+    orc.set_spline_bc(1)
+    yield orc
+    orc.set_spline_bc(0)
+
+
+def test_notaknot_all_spline_kernels(notaknot, torch_cuda):
+    """ll_config.spline_bc = LL_BC_NOT_A_KNOT through every spline kernel: block-per-system (small batch), thread-per-
+    system (large batch), six-spline transfer-function path, per-walker nodes; oracle under the same switch."""
+    from oracle import per_walker as pw
+    from paper_2111_01064_b200 import binding
+    from helpers import pw_case
+    orc, tc = notaknot, torch_cuda
+    # stand-in entry point, config-0 recipe (small batch -> k_spline_block)
+    wl = wlm.make_workload(0)
+    d, run = oracle_setup_full(orc, wl)                    # data = walker 0's NOT-A-KNOT spline template
+    ctx = binding.Context(n_modes=1, spline_bc=binding.LL_BC_NOT_A_KNOT)
+    ctx.standin_config(wl.modes_l, wl.modes_m, wl.c_lm, wl.kappa)
+    g = wl.grid
+    ctx.set_data(g.n_f, g.k_min, g.df, dev(tc, d), dev(tc, wl.W))
+    got = ctx.full_batch_standin(wl.f_nodes, dev(tc, wl.params))
+    check_triplet(got, run(wl.params, d), "not-a-knot cfg0")
+    assert abs(float(got[0][0])) <= 1e-6                   # log L = 0 at d = h (PAPER.md:59) under this BC too
+    with pytest.raises(binding.LLError):
+        ctx.tlm_nodes(wl.f_nodes, dev(tc, np.zeros((1, 1, len(wl.f_nodes)))), 0.0)
+    ctx.destroy()
+    # array entry points on a random grid: large batch (thread-per-system), transfer-function path, per-walker nodes
+    rng = np.random.default_rng(2)
+    n_f, k_min, df = 3000, 40, 1e-5
+    f, x, amp, ph, tf, W, dd_ = pw_case(rng, 5000, 1, 24, n_f, k_min, df)
+    xs = np.geomspace(f[0] * 0.95, f[-1] * 1.02, 24)
+    ctx = binding.Context(n_modes=1, spline_bc=binding.LL_BC_NOT_A_KNOT)
+    ctx.set_data(n_f, k_min, df, dev(tc, dd_), dev(tc, W))
+    got = ctx.full_batch(xs, dev(tc, amp), dev(tc, ph), dev(tc, tf))
+    sample = np.r_[0, 1, 4999, rng.integers(0, 5000, 30)]
+    ref = orc.full_batch(xs, amp[sample], ph[sample], tf[sample], None, k_min, df, dd_, W)
+    check_triplet([__import__("torch").as_tensor(v.cpu().numpy()[sample]) for v in got], ref, "not-a-knot large batch")
+    s2 = sample[:12]
+    tfn = _smooth_tf_nodes(rng, len(s2), 1, xs)
+    got = ctx.full_batch_tf(xs, dev(tc, amp[s2]), dev(tc, ph[s2]), dev(tc, tfn))
+    check_triplet(got, orc.full_batch_tf(xs, amp[s2], ph[s2], tfn, None, k_min, df, dd_, W), "not-a-knot tf")
+    got = ctx.full_batch_pw(dev(tc, x[:200]), dev(tc, amp[:200]), dev(tc, ph[:200]), dev(tc, tf[:200]))
+    check_triplet(got, pw.full_batch_pw(x[:200], amp[:200], ph[:200], tf[:200], None, k_min, df, dd_, W), "not-a-knot per-walker")
+    # and the boundary condition really changes the answer
+    ctx_n = binding.Context(n_modes=1)
+    ctx_n.set_data(n_f, k_min, df, dev(tc, dd_), dev(tc, W))
+    nat = ctx_n.full_batch_pw(dev(tc, x[:200]), dev(tc, amp[:200]), dev(tc, ph[:200]), dev(tc, tf[:200]))
+    assert float((nat[1] - got[1]).abs().max()) > 1e-6 * float(got[2].abs().max())
+    ctx.destroy(); ctx_n.destroy()
