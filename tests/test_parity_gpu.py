@@ -521,6 +521,25 @@ def test_state_and_argument_errors(torch_cuda):
     with pytest.raises(binding.LLError) as ei:
         ctx.set_data(0, grid.k_min, grid.df, d, W)
     assert ei.value.code == binding.LL_ERR_ARG
+    # the entry points added for the SURVEY 8(f) rows: state before ll_het_prepare, sizes, NULLs
+    tc = torch_cuda
+    z = lambda *sh: tc.zeros(sh, dtype=tc.float64, device="cuda")
+    for call in (lambda: ctx.het_audit_standin(p),
+                 lambda: ctx.pt_stretch_half(0, z(1, 4, 9), z(1, 4), None, None, z(1), z(9), z(9), 5, z(1, 2), z(1, 2), z(1, 2))):
+        with pytest.raises(binding.LLError) as ei:
+            call()
+        assert ei.value.code == binding.LL_ERR_STATE        # no heterodyne reference yet
+    for call in (lambda: ctx.pt_stretch_half(2, z(1, 4, 9), z(1, 4), None, None, z(1), z(9), z(9), 5, z(1, 2), z(1, 2), z(1, 2)),
+                 lambda: ctx.pt_stretch_half(0, z(1, 5, 9), z(1, 5), None, None, z(1), z(9), z(9), 5, z(1, 2), z(1, 2), z(1, 2)),
+                 lambda: ctx.pt_stretch_half(0, z(1, 4, 9), z(1, 4), None, None, z(1), z(9), z(9), 0, z(1, 2), z(1, 2), z(1, 2)),
+                 lambda: ctx.het_refresh_standin(p, z(4), 1),
+                 lambda: ctx.full_batch_pw(z(4, 2), z(4, 1, 2), z(4, 1, 2), z(4, 1, 2, 2)),
+                 lambda: ctx.pt_stats(z(0), None, None)):
+        with pytest.raises(binding.LLError) as ei:
+            call()
+        assert ei.value.code == binding.LL_ERR_ARG
+    assert ctx.full_batch_pw(z(0, 8), z(0, 1, 8), z(0, 1, 8), z(0, 1, 2, 2))[0].numel() == 0     # empty batch: no-op
+    ctx.pt_swap(z(1, 4, 9), z(1, 4), None, None, z(1), None)                                    # one temperature: no-op
     ctx.destroy()
 
 
