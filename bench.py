@@ -32,10 +32,13 @@ from paper_2111_01064_b200 import workloads as wlm  # noqa: E402
 
 METRIC = "log-likelihood evals/sec"
 UNIT = "evals/s"
-# algorithmic FP64 issue slots per active (walker, bin, mode) of the full-grid path, direct formulation
-# (t 1, two cubics 6, reduce 3, sincos 18, A e^{-i Psi} 2, two complex MACs 8, W A^2 2 => 40; the
-# SURVEY.md §8(d) figure of 39 is used as the contract number)
-SLOTS_FULL = 39.0
+# algorithmic FP64 issue slots per active (walker, bin, mode) of the full-grid path.  Direct formulation (DESIGN.md §6:
+# t 1, two cubics 6, reduce 3, sincos 18, A e^{-i Psi} 2, two complex MACs 8, W A^2 2 => 40; SURVEY.md §8(d) uses 39).
+# The single-mode FP64 kernel advances e^{-i Psi} and A by recurrence (three complex rotations and three additions per
+# bin, re-synchronised from the cubics every 32 bins), and SURVEY §8(d) asks that such a build quote ITS count:
+# 12 + 3 + 2 + 8 + 2 = 27 per bin plus (2 cubics 6 + differences 16 + 3 sincos 54 + 3 normalisations 15 + 1)/32 = 2.9 => 30
+SLOTS_FULL_DIRECT = 39.0
+SLOTS_FULL = 30.0
 # single mode: the kernel regroups Eq. 14/17 by edge, whose own count is 48 slots per (walker, bin): phase 2,
 # reduce 3, sincos 18, taper and amplitude 4, z conj(Q) 8, |z|^2 P 3, z_b conj(z_{b+1}) X 10; the bin-by-bin form needs 73
 SLOTS_HET = {1: 48.0, 6: 252.0}
@@ -448,6 +451,10 @@ def main():
                 "measured_dfma_per_s": dfma_rate, "measured_ffma_per_s": ffma_rate,
                 "frac_of_measured_dfma": achieved / dfma_rate,
                 "hbm_peak_gbs": peaks.get("hbm_gbs"), "hbm_peak_source": peak_src}
+            if wl.path == "full":
+                line["roofline"]["formulation"] = ("rotation recurrence, re-synchronised every 32 bins (DESIGN.md §5); the direct "
+                                                   "formulation needs %g slots per pair" % SLOTS_FULL_DIRECT)
+                line["roofline"]["frac_in_direct_form_slots"] = pairs * SLOTS_FULL_DIRECT / (k_ms * 1e-3) / peak_slots
             if wl.path != "full" and wl.n_m in SLOTS_HET_DIRECT_FORM:
                 line["roofline"]["formulation"] = "regrouped by edge (DESIGN.md §5); the bin-by-bin form of Eq. 14/17 needs %g" \
                                                   % SLOTS_HET_DIRECT_FORM[wl.n_m]
@@ -557,7 +564,8 @@ def main():
             c2.profile_enable(False)
             per["cfg2_pw"] = {"evals_per_s": wl2.n_w / (ms3 / nst * 1e-3), "ms_per_batch": ms3 / nst, "n_walkers": wl2.n_w,
                               "kernel": "k_full_fused_pw", "kernel_ms": kms3 / max(kn3, 1),
-                              "frac": pairs2 * SLOTS_FULL / (kms3 / max(kn3, 1) * 1e-3) / peak_slots,
+                              "frac": pairs2 * SLOTS_FULL_DIRECT / (kms3 / max(kn3, 1) * 1e-3) / peak_slots,
+                              "algorithmic_slots_per_pair": SLOTS_FULL_DIRECT,
                               "max_abs_dlogL_vs_shared_nodes": float((o3[0] - sh[0]).abs().max()),
                               "entry": "ll_full_batch_pw (f_nodes_w [n_w][1024] on the device; the walkers' own bands)"}
             del xw, sh, tfc

