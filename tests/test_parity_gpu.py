@@ -797,3 +797,29 @@ def test_notaknot_all_spline_kernels(notaknot, torch_cuda):
     nat = ctx_n.full_batch_pw(dev(tc, x[:200]), dev(tc, amp[:200]), dev(tc, ph[:200]), dev(tc, tf[:200]))
     assert float((nat[1] - got[1]).abs().max()) > 1e-6 * float(got[2].abs().max())
     ctx.destroy(); ctx_n.destroy()
+
+
+def test_one_year_noiseless_logL_is_zero_at_truth(orc, torch_cuda):
+    """The thinnest margin of the FP64 bar (SURVEY 8(c) probes): noiseless data on the one-year grid, log L = 0 at
+    the injection to 1e-6 ABSOLUTE while <d|h> = <h|h> = <d|d> = 2.5e5 — each of them is needed to
+    4e-12 relative.  Also a near walker and a far one against the oracle."""
+    wl = wlm.make_workload(2)
+    wl.noise = None
+    d, run = oracle_setup_full(orc, wl)
+    ctx = make_ctx(wl)
+    g = wl.grid
+    ctx.set_data(g.n_f, g.k_min, g.df, dev(torch_cuda, d), dev(torch_cuda, wl.W))
+    p = wl.params[:3].copy()
+    p[1] = wl.inj
+    p[1, 0] *= 1.0 + 3e-4                                   # near: log L of a few hundred
+    p[1, 2] += 3.0
+    ref = run(p, d)
+    got = ctx.full_batch_standin(wl.f_nodes, dev(torch_cuda, p))
+    check_triplet(got, ref, "one-year noiseless")
+    assert abs(ref["logL"][0]) <= 1e-6 and abs(float(got[0][0])) <= 1e-6
+    assert -1e4 < ref["logL"][1] < -10.0
+    # the same through a large batch (other tiles, thread-per-system spline)
+    big = np.tile(p, (2000, 1))
+    gb = ctx.full_batch_standin(wl.f_nodes, dev(torch_cuda, big))[0].cpu().numpy().reshape(2000, 3)
+    assert np.all(np.abs(gb - ref["logL"][None, :]) <= 1e-6 * np.maximum(1.0, np.abs(ref["logL"]))[None, :])
+    ctx.destroy()
