@@ -53,7 +53,7 @@ INSTR_FULL_FP32ACC = 45.0
 SLOTS_FULL_TF = 59.0
 ISSUE_LANES_PER_CLK_PER_SM = 128.0
 # DRAM traffic per launch of the dominant kernel, from the committed `ncu --set full` captures (profiles/)
-NCU_TRAFFIC_BYTES = {("k_full_fused", 2): 806.3e6 + 39.5e6, ("k_full_fused_mixed", 2): 786.4e6 + 37.0e6}
+NCU_TRAFFIC_BYTES = {("k_full_fused", 2): 806.3e6 + 39.9e6, ("k_full_fused_mixed", 2): 786.4e6 + 37.0e6}
 DFMA_PER_CLK_PER_SM = 64.0
 
 
