@@ -39,6 +39,9 @@ UNIT = "evals/s"
 # 12 + 3 + 2 + 8 + 2 = 27 per bin plus (2 cubics 6 + differences 16 + 3 sincos 54 + 3 normalisations 15 + 1)/32 = 2.9 => 30
 SLOTS_FULL_DIRECT = 39.0
 SLOTS_FULL = 30.0
+# per-walker node grids: the recurrence route with T^c applied per bin (it accumulates <d|h>, <h|h> directly):
+# 12 + 3 + 2 + T^c h 8 + Re g h 4 + W |h|^2 5 = 34 per bin + (6 + 16 + 4 sincos 72 + 20 + 1)/32 = 3.6 => 38
+SLOTS_FULL_PW = 38.0
 # single mode: the kernel regroups Eq. 14/17 by edge, whose own count is 48 slots per (walker, bin): phase 2,
 # reduce 3, sincos 18, taper and amplitude 4, z conj(Q) 8, |z|^2 P 3, z_b conj(z_{b+1}) X 10; the bin-by-bin form needs 73
 SLOTS_HET = {1: 48.0, 6: 252.0}
@@ -564,8 +567,8 @@ def main():
             c2.profile_enable(False)
             per["cfg2_pw"] = {"evals_per_s": wl2.n_w / (ms3 / nst * 1e-3), "ms_per_batch": ms3 / nst, "n_walkers": wl2.n_w,
                               "kernel": "k_full_fused_pw", "kernel_ms": kms3 / max(kn3, 1),
-                              "frac": pairs2 * SLOTS_FULL_DIRECT / (kms3 / max(kn3, 1) * 1e-3) / peak_slots,
-                              "algorithmic_slots_per_pair": SLOTS_FULL_DIRECT,
+                              "frac": pairs2 * SLOTS_FULL_PW / (kms3 / max(kn3, 1) * 1e-3) / peak_slots,
+                              "algorithmic_slots_per_pair": SLOTS_FULL_PW,
                               "max_abs_dlogL_vs_shared_nodes": float((o3[0] - sh[0]).abs().max()),
                               "entry": "ll_full_batch_pw (f_nodes_w [n_w][1024] on the device; the walkers' own bands)"}
             del xw, sh, tfc

@@ -719,7 +719,11 @@ __device__ __forceinline__ void fused_bins_nm1(int b0, int b1, int tlo, int thi,
 #define LL_ROT_SYNC 32 // measured at config 2 (max |error of <d|h>| over sampled walkers, kernel time): 32: 8e-8, 10.7 ms
                        // (the exact route: 7e-8, 13.0 ms); 64: 3e-7, 10.2 ms; 128: 2e-6, 10.0 ms; 256: 1.3e-5, 9.9 ms
 #endif
+#ifndef LL_ROT_UNROLL
+#define LL_ROT_UNROLL 2
+#endif
 constexpr int kRotSync = LL_ROT_SYNC;
+constexpr int kRotUnroll = LL_ROT_UNROLL;
 // The sin/cos polynomials are minimax fits: cos(0) comes out as 1 - 5.5e-14, so a rotation built from them has modulus
 // 1 - O(1e-14).  Harmless once, but u multiplies into v, v into w and w into z every bin, and the modulus of z would
 // decay like k^3/6 x 5.5e-14 (measured: 5e-10 relative on <d|h> at 64 bins between re-syncs).  One Newton step of
@@ -755,7 +759,7 @@ __device__ __forceinline__ void fused_bins_rot(int b0, int b1, int kbase, double
         unit_modulus(cz, sz);
         unit_modulus(cw, sw);
         unit_modulus(cv, sv);
-#pragma unroll 2
+#pragma unroll kRotUnroll
         for (int ii = k0; ii < k1; ++ii) {
             const double u = A * cz, v = A * sz; // h = u - i v
             const double4 g = sg4[ii];
@@ -1486,12 +1490,44 @@ __global__ void __launch_bounds__(128, 3) k_full_fused_pw(FusedArgs a, const dou
         while (ii < thi) {
             const double f = (double)(a.k_min + ii) * a.df;
             while (f >= xnext) load_interval(++j);
-            // four bins at once while they stay inside this lane's interval (intervals are hundreds of bins wide
-            // almost everywhere): four independent chains, no interval test in between
-            if (NM1 && ii + 4 <= thi && (double)(a.k_min + ii + 3) * a.df < xnext) {
-#pragma unroll
-                for (int k = 0; k < 4; ++k) one_bin(ii + k, (double)(a.k_min + ii + k) * a.df);
-                ii += 4;
+            // while the next bins stay inside this lane's interval (intervals are hundreds of bins wide almost
+            // everywhere) they go by the recurrence route of fused_bins_rot: up to kRotSync bins per re-sync
+            int m = 0;
+            if (NM1 && LL_FUSED_ROT) {
+                m = min(thi - ii, kRotSync);
+                const double room = (xnext - f) / a.df; // bins ii .. ii + ceil(room) - 1 lie below the next node
+                if (room < (double)m) m = (int)room;    // conservative: the bin at the boundary takes the exact route
+            }
+            if (m >= 8) {
+                const double df = a.df, df2 = df * df, df3 = df2 * df;
+                const double t = f - xj, tt = fma(2.0, t, df), q3 = fma(3.0 * t, t + df, df2), t1 = t + df;
+                double A = cubic4(co, t);
+                double d1A = df * fma(co[3], q3, fma(co[2], tt, co[1]));
+                double d2A = df2 * fma(6.0 * co[3], t1, 2.0 * co[2]);
+                const double d3A = 6.0 * co[3] * df3;
+                double sz, cz, sw_, cw, sv, cv, su, cu;
+                sincos_qc(cubic4(co + 4, t), sz, cz);
+                sincos_qc(df * fma(co[7], q3, fma(co[6], tt, co[5])), sw_, cw);
+                sincos_qc(df2 * fma(6.0 * co[7], t1, 2.0 * co[6]), sv, cv);
+                sincos_qc(6.0 * co[7] * df3, su, cu);
+                unit_modulus(cz, sz); unit_modulus(cw, sw_); unit_modulus(cv, sv); unit_modulus(cu, su);
+#pragma unroll 2
+                for (int k = 0; k < m; ++k) {
+                    const double u = A * cz, v = A * sz; // h = u - i v
+                    const double hAr = fma(tf1[0], u, tf1[1] * v), hAi = fma(tf1[1], u, -(tf1[0] * v));
+                    const double hEr = fma(tf1[2], u, tf1[3] * v), hEi = fma(tf1[3], u, -(tf1[2] * v));
+                    const double4 g = sg4[ii + k];
+                    const double w = sWc[ii + k];
+                    s_dh = fma(g.x, hAr, s_dh); s_dh = fma(-g.y, hAi, s_dh);
+                    s_dh = fma(g.z, hEr, s_dh); s_dh = fma(-g.w, hEi, s_dh);
+                    s_hh = fma(w, fma(hAr, hAr, hAi * hAi) + fma(hEr, hEr, hEi * hEi), s_hh);
+                    const double nzc = fma(cz, cw, -(sz * sw_)), nzs = fma(sz, cw, cz * sw_);
+                    const double nwc = fma(cw, cv, -(sw_ * sv)), nws = fma(sw_, cv, cw * sv);
+                    const double nvc = fma(cv, cu, -(sv * su)), nvs = fma(sv, cu, cv * su);
+                    cz = nzc; sz = nzs; cw = nwc; sw_ = nws; cv = nvc; sv = nvs;
+                    A += d1A; d1A += d2A; d2A += d3A;
+                }
+                ii += m;
             } else {
                 one_bin(ii, f);
                 ii += 1;
