@@ -51,9 +51,10 @@ SLOTS_HET_DIRECT_FORM = {1: 73.0}
 # reduce 3, scale 1, W A^2 2) + 3 conversions + 20 binary32 (sincos 10, A e^{-i Psi} 2, MACs 8) + 6 quadrant
 # + 2 shared loads + 1 loop = 45
 INSTR_FULL_FP32ACC = 45.0
-# frequency-dependent transfer function (Eq. 8-9): t 1, six cubics 18, reduce 3, sincos 18, A e^{-i Psi} 2, T^c h 8,
-# Re g h 4, W |h|^2 5 = 59
-SLOTS_FULL_TF = 59.0
+# frequency-dependent transfer function (Eq. 8-9), direct formulation: t 1, six cubics 18, reduce 3, sincos 18,
+# A e^{-i Psi} 2, T^c h 8, Re g h 4, W |h|^2 5 = 59.  The kernel advances A and e^{-i Psi} by the recurrence and keeps
+# Horner for the four T cubics: t 1 + 12 + rotations 12 + amplitude 3 + 2 + 8 + 4 + 5 = 47 per bin + re-sync 3 => 50
+SLOTS_FULL_TF = 50.0
 ISSUE_LANES_PER_CLK_PER_SM = 128.0
 # DRAM traffic per launch of the dominant kernel, from the committed `ncu --set full` captures (profiles/)
 NCU_TRAFFIC_BYTES = {("k_full_fused", 2): 806.3e6 + 39.9e6, ("k_full_fused_mixed", 2): 786.4e6 + 37.0e6}

@@ -1242,35 +1242,83 @@ __global__ void __launch_bounds__(128, 3) k_full_fused_tf(FusedArgs a)
                 }
                 const double4 *sg4 = reinterpret_cast<const double4 *>(sg) - cb;
                 const double *sWc = sW - cb;
+                auto direct_bins = [&](int b0, int b1) {
 #pragma unroll 2
-                for (int ii = wlo; ii < whi; ++ii) {
-                    const bool act = (ii >= tlo) && (ii < thi);
-                    const double t = fma((double)(kbase + ii), a.df, nxj);
-                    double hAr = 0, hAi = 0, hEr = 0, hEi = 0;
-                    const int n_m = NM1 ? 1 : a.n_m;
-                    for (int m = 0; m < n_m; ++m) {
-                        if (!NM1) {
-                            const double *cc = cc0 + (size_t)m * cm;
+                    for (int ii = b0; ii < b1; ++ii) {
+                        const bool act = (ii >= tlo) && (ii < thi);
+                        const double t = fma((double)(kbase + ii), a.df, nxj);
+                        double hAr = 0, hAi = 0, hEr = 0, hEi = 0;
+                        const int n_m = NM1 ? 1 : a.n_m;
+                        for (int m = 0; m < n_m; ++m) {
+                            if (!NM1) {
+                                const double *cc = cc0 + (size_t)m * cm;
 #pragma unroll
-                            for (int q = 0; q < 24; ++q) co[q] = cc[(size_t)q * sw];
+                                for (int q = 0; q < 24; ++q) co[q] = cc[(size_t)q * sw];
+                            }
+                            const double A = cubic4(co, t), y = cubic4(co + 4, t);
+                            const double tar = cubic4(co + 8, t), tai = cubic4(co + 12, t);
+                            const double ter = cubic4(co + 16, t), tei = cubic4(co + 20, t);
+                            double u, v; // h_m = u - i v
+                            amp_expi_qc(A, y, u, v);
+                            hAr = fma(tar, u, hAr); hAr = fma(tai, v, hAr);
+                            hAi = fma(tai, u, hAi); hAi = fma(-tar, v, hAi);
+                            hEr = fma(ter, u, hEr); hEr = fma(tei, v, hEr);
+                            hEi = fma(tei, u, hEi); hEi = fma(-ter, v, hEi);
                         }
-                        const double A = cubic4(co, t), y = cubic4(co + 4, t);
-                        const double tar = cubic4(co + 8, t), tai = cubic4(co + 12, t);
-                        const double ter = cubic4(co + 16, t), tei = cubic4(co + 20, t);
-                        double u, v; // h_m = u - i v
-                        amp_expi_qc(A, y, u, v);
-                        hAr = fma(tar, u, hAr); hAr = fma(tai, v, hAr);
-                        hAi = fma(tai, u, hAi); hAi = fma(-tar, v, hAi);
-                        hEr = fma(ter, u, hEr); hEr = fma(tei, v, hEr);
-                        hEi = fma(tei, u, hEi); hEi = fma(-ter, v, hEi);
+                        if (act) {
+                            const double4 g = sg4[ii];
+                            const double w = sWc[ii];
+                            s_dh = fma(g.x, hAr, s_dh); s_dh = fma(-g.y, hAi, s_dh);
+                            s_dh = fma(g.z, hEr, s_dh); s_dh = fma(-g.w, hEi, s_dh);
+                            s_hh = fma(w, fma(hAr, hAr, hAi * hAi) + fma(hEr, hEr, hEi * hEi), s_hh);
+                        }
                     }
-                    if (act) {
-                        const double4 g = sg4[ii];
-                        const double w = sWc[ii];
-                        s_dh = fma(g.x, hAr, s_dh); s_dh = fma(-g.y, hAi, s_dh);
-                        s_dh = fma(g.z, hEr, s_dh); s_dh = fma(-g.w, hEi, s_dh);
-                        s_hh = fma(w, fma(hAr, hAr, hAi * hAi) + fma(hEr, hEr, hEi * hEi), s_hh);
+                };
+                // bins inside every lane's band: e^{-i Psi} and A by the recurrence of fused_bins_rot, T^c(f) by Horner
+                const int flo = __reduce_max_sync(0xffffffffu, max(lo, i));
+                const int fhi = __reduce_min_sync(0xffffffffu, min(hi, seg_end));
+                if (NM1 && LL_FUSED_ROT && fhi - flo >= 8) {
+                    direct_bins(wlo, flo);
+                    const double df = a.df, df2 = df * df, df3 = df2 * df;
+                    const double d3A = 6.0 * co[3] * df3;
+                    double su, cu;
+                    sincos_qc(6.0 * co[7] * df3, su, cu);
+                    unit_modulus(cu, su);
+                    for (int k0 = flo; k0 < fhi; k0 += kRotSync) {
+                        const int k1 = min(k0 + kRotSync, fhi);
+                        const double t0 = fma((double)(kbase + k0), df, nxj);
+                        const double tt = fma(2.0, t0, df), q3 = fma(3.0 * t0, t0 + df, df2), t1 = t0 + df;
+                        double A = cubic4(co, t0);
+                        double d1A = df * fma(co[3], q3, fma(co[2], tt, co[1]));
+                        double d2A = df2 * fma(6.0 * co[3], t1, 2.0 * co[2]);
+                        double sz, cz, sw_, cw, sv, cv;
+                        sincos_qc(cubic4(co + 4, t0), sz, cz);
+                        sincos_qc(df * fma(co[7], q3, fma(co[6], tt, co[5])), sw_, cw);
+                        sincos_qc(df2 * fma(6.0 * co[7], t1, 2.0 * co[6]), sv, cv);
+                        unit_modulus(cz, sz); unit_modulus(cw, sw_); unit_modulus(cv, sv);
+#pragma unroll 2
+                        for (int ii = k0; ii < k1; ++ii) {
+                            const double t = fma((double)(kbase + ii), df, nxj);
+                            const double tar = cubic4(co + 8, t), tai = cubic4(co + 12, t);
+                            const double ter = cubic4(co + 16, t), tei = cubic4(co + 20, t);
+                            const double u = A * cz, v = A * sz; // h = u - i v
+                            const double hAr = fma(tar, u, tai * v), hAi = fma(tai, u, -(tar * v));
+                            const double hEr = fma(ter, u, tei * v), hEi = fma(tei, u, -(ter * v));
+                            const double4 g = sg4[ii];
+                            const double w = sWc[ii];
+                            s_dh = fma(g.x, hAr, s_dh); s_dh = fma(-g.y, hAi, s_dh);
+                            s_dh = fma(g.z, hEr, s_dh); s_dh = fma(-g.w, hEi, s_dh);
+                            s_hh = fma(w, fma(hAr, hAr, hAi * hAi) + fma(hEr, hEr, hEi * hEi), s_hh);
+                            const double nzc = fma(cz, cw, -(sz * sw_)), nzs = fma(sz, cw, cz * sw_);
+                            const double nwc = fma(cw, cv, -(sw_ * sv)), nws = fma(sw_, cv, cw * sv);
+                            const double nvc = fma(cv, cu, -(sv * su)), nvs = fma(sv, cu, cv * su);
+                            cz = nzc; sz = nzs; cw = nwc; sw_ = nws; cv = nvc; sv = nvs;
+                            A += d1A; d1A += d2A; d2A += d3A;
+                        }
                     }
+                    direct_bins(fhi, whi);
+                } else {
+                    direct_bins(wlo, whi);
                 }
             }
             i = seg_end;
