@@ -272,6 +272,36 @@ def bench_sampler_iteration(torch, ctx, wl, params, n_t: int = 10, n_w: int = 40
     return res
 
 
+def bench_full_hm(torch, steps: int = 5, n_w: int = 2048):
+    """The paper's higher-mode analysis ran the brute-force likelihood, not the heterodyned one: config 3's
+    six modes through the FULL-GRID path on config 2's one-year grid and 1024 nodes, prior-draw walkers with unit-modulus
+    transfer factors per mode, data = noise of the config-2 recipe (timing only; parity of this path is in the tests)."""
+    from paper_2111_01064_b200 import binding
+    wl6, wl2 = wlm.make_workload(3, n_w=8), wlm.make_workload(2, n_w=n_w)
+    rng = np.random.default_rng(wlm.SEED_BASE + 232)
+    params = np.empty((n_w, 5 + 4 * wl6.n_m))
+    params[:, :5] = wl2.params[:, :5]
+    ang = rng.uniform(0, 2 * np.pi, (n_w, 2 * wl6.n_m))
+    params[:, 5::2], params[:, 6::2] = np.cos(ang), np.sin(ang)
+    ctx = binding.Context(n_modes=wl6.n_m)
+    ctx.standin_config(wl6.modes_l, wl6.modes_m, wl6.c_lm, wl6.kappa)
+    g = wl2.grid
+    dev = lambda a: torch.as_tensor(np.ascontiguousarray(a, dtype=np.float64), device="cuda")
+    ctx.set_data(g.n_f, g.k_min, g.df, dev(wl2.noise), dev(wl2.W))
+    p = dev(params)
+    out = tuple(torch.empty(n_w, dtype=torch.float64, device="cuda") for _ in range(3))
+    fn = lambda: ctx.full_batch_standin(wl2.f_nodes, p, out=out)
+    fn()
+    ctx.profile_enable(True)
+    ms = time_steps(torch, fn, steps, 2) / steps
+    kms, kn = ctx.profile_read()
+    pairs = ctx.last_full_stats()[0]
+    ctx.destroy()
+    return {"evals_per_s": n_w / (ms * 1e-3), "ms_per_batch": ms, "n_walkers": n_w, "n_modes": int(wl6.n_m),
+            "kernel": "k_full_fused<0>", "kernel_ms": kms / max(kn, 1), "active_pair_modes": pairs,
+            "algorithmic_slots_per_pair_mode": SLOTS_FULL_DIRECT}
+
+
 def e2e_config(torch, res, steps: int, warmup: int):
     """same metric through the C ABI with HOST buffers: pinned params in, pinned results out, every step."""
     wl, ctx = res["wl"], res["ctx"]
@@ -573,6 +603,10 @@ def main():
                               "max_abs_dlogL_vs_shared_nodes": float((o3[0] - sh[0]).abs().max()),
                               "entry": "ll_full_batch_pw (f_nodes_w [n_w][1024] on the device; the walkers' own bands)"}
             del xw, sh, tfc
+            # ---- six modes through the full-grid path (the paper's higher-mode run used the brute-force likelihood)
+            hm = bench_full_hm(torch)
+            hm["frac"] = hm["active_pair_modes"] * SLOTS_FULL_DIRECT / (hm["kernel_ms"] * 1e-3) / peak_slots
+            per["cfg2_hm6"] = hm
             # ---- Module-1 sized sampler iteration on the full-grid likelihood of the same one-year data stream
             per["module1_iteration"] = bench_sampler_iteration(torch, c2, wl2, b2["params"], n_t=4, n_w=80, iters=20,
                                                                f_nodes=wl2.f_nodes)

@@ -872,34 +872,48 @@ __global__ void __launch_bounds__(128, LL_FUSED_MINB) k_full_fused(FusedArgs a)
                                              sg4, sWc, sAr, sAi, sEr, sEi, sH);
                     }
                 } else {
+                    // any number of modes: chunks of four bins with the MODE loop outside the bins, so that a mode's
+                    // 8 coefficients and 4 transfer factors are read once per chunk (not once per bin) and the four
+                    // bins are four independent cubic -> sincos -> T^c h chains in flight per thread
                     nxj = -__ldg(a.xj + j);
                     const double *cc0 = a.C + (size_t)j * cj + p;
-                    double kd = (double)(a.k_min + wlo);
-                    for (int ii = wlo; ii < whi; ++ii) {
-                        const bool act = (ii >= tlo) && (ii < thi);
-                        const double t = fma(kd, a.df, nxj);
-                        kd += 1.0;
-                        double hAr = 0, hAi = 0, hEr = 0, hEi = 0;
+                    for (int c4 = wlo; c4 < whi; c4 += 4) {
+                        double t4[4], h4[4][4];
+#pragma unroll
+                        for (int k = 0; k < 4; ++k) {
+                            t4[k] = fma((double)(kbase + c4 + k), a.df, nxj);
+                            h4[k][0] = h4[k][1] = h4[k][2] = h4[k][3] = 0.0;
+                        }
+#pragma unroll 1
                         for (int m = 0; m < a.n_m; ++m) {
                             const double *cc = cc0 + (size_t)m * 8 * sw;
-                            const double A = fma(fma(fma(cc[3 * sw], t, cc[2 * sw]), t, cc[sw]), t, cc[0]);
-                            const double y = fma(fma(fma(cc[7 * sw], t, cc[6 * sw]), t, cc[5 * sw]), t, cc[4 * sw]);
-                            double sn, cs;
-                            sincos_qc(y, sn, cs);
-                            const double u = A * cs, v = A * sn;
+                            double co[8];
+#pragma unroll
+                            for (int q = 0; q < 8; ++q) co[q] = cc[(size_t)q * sw];
                             const double *tf = a.TF + (size_t)m * 4 * sw + p;
                             const double tar = tf[0], tai = tf[sw], ter = tf[2 * sw], tei = tf[3 * sw];
-                            hAr = fma(tar, u, hAr); hAr = fma(tai, v, hAr);
-                            hAi = fma(tai, u, hAi); hAi = fma(-tar, v, hAi);
-                            hEr = fma(ter, u, hEr); hEr = fma(tei, v, hEr);
-                            hEi = fma(tei, u, hEi); hEi = fma(-ter, v, hEi);
+#pragma unroll
+                            for (int k = 0; k < 4; ++k) {
+                                const double A = fma(fma(fma(co[3], t4[k], co[2]), t4[k], co[1]), t4[k], co[0]);
+                                const double y = fma(fma(fma(co[7], t4[k], co[6]), t4[k], co[5]), t4[k], co[4]);
+                                double u, v; // h_m = u - i v
+                                amp_expi_qc(A, y, u, v);
+                                h4[k][0] = fma(tar, u, h4[k][0]); h4[k][0] = fma(tai, v, h4[k][0]);
+                                h4[k][1] = fma(tai, u, h4[k][1]); h4[k][1] = fma(-tar, v, h4[k][1]);
+                                h4[k][2] = fma(ter, u, h4[k][2]); h4[k][2] = fma(tei, v, h4[k][2]);
+                                h4[k][3] = fma(tei, u, h4[k][3]); h4[k][3] = fma(-ter, v, h4[k][3]);
+                            }
                         }
-                        if (act) {
-                            const double4 g = reinterpret_cast<const double4 *>(sg)[ii - cb];
-                            const double w = sW[ii - cb];
-                            sAr = fma(g.x, hAr, sAr); sAr = fma(-g.y, hAi, sAr);
-                            sAr = fma(g.z, hEr, sAr); sAr = fma(-g.w, hEi, sAr);
-                            sH = fma(w, hAr * hAr + hAi * hAi + hEr * hEr + hEi * hEi, sH);
+#pragma unroll
+                        for (int k = 0; k < 4; ++k) {
+                            const int ii = c4 + k;
+                            if (ii < whi && ii >= tlo && ii < thi) {
+                                const double4 g = reinterpret_cast<const double4 *>(sg)[ii - cb];
+                                const double w = sW[ii - cb];
+                                sAr = fma(g.x, h4[k][0], sAr); sAr = fma(-g.y, h4[k][1], sAr);
+                                sAr = fma(g.z, h4[k][2], sAr); sAr = fma(-g.w, h4[k][3], sAr);
+                                sH = fma(w, h4[k][0] * h4[k][0] + h4[k][1] * h4[k][1] + h4[k][2] * h4[k][2] + h4[k][3] * h4[k][3], sH);
+                            }
                         }
                     }
                 }
