@@ -1257,6 +1257,49 @@ __global__ void __launch_bounds__(128, 3) k_full_fused_tf(FusedArgs a)
                 const double4 *sg4 = reinterpret_cast<const double4 *>(sg) - cb;
                 const double *sWc = sW - cb;
                 auto direct_bins = [&](int b0, int b1) {
+                    if (!NM1) {
+                        // several modes: chunks of four bins, mode loop outside (24 coefficients read once per chunk)
+                        for (int c4 = b0; c4 < b1; c4 += 4) {
+                            double t4[4], h4[4][4];
+#pragma unroll
+                            for (int k = 0; k < 4; ++k) {
+                                t4[k] = fma((double)(kbase + c4 + k), a.df, nxj);
+                                h4[k][0] = h4[k][1] = h4[k][2] = h4[k][3] = 0.0;
+                            }
+#pragma unroll 1
+                            for (int m = 0; m < a.n_m; ++m) {
+                                const double *cc = cc0 + (size_t)m * cm;
+#pragma unroll
+                                for (int q = 0; q < 24; ++q) co[q] = cc[(size_t)q * sw];
+#pragma unroll
+                                for (int k = 0; k < 4; ++k) {
+                                    const double t = t4[k];
+                                    const double A = cubic4(co, t), y = cubic4(co + 4, t);
+                                    const double tar = cubic4(co + 8, t), tai = cubic4(co + 12, t);
+                                    const double ter = cubic4(co + 16, t), tei = cubic4(co + 20, t);
+                                    double u, v; // h_m = u - i v
+                                    amp_expi_qc(A, y, u, v);
+                                    h4[k][0] = fma(tar, u, h4[k][0]); h4[k][0] = fma(tai, v, h4[k][0]);
+                                    h4[k][1] = fma(tai, u, h4[k][1]); h4[k][1] = fma(-tar, v, h4[k][1]);
+                                    h4[k][2] = fma(ter, u, h4[k][2]); h4[k][2] = fma(tei, v, h4[k][2]);
+                                    h4[k][3] = fma(tei, u, h4[k][3]); h4[k][3] = fma(-ter, v, h4[k][3]);
+                                }
+                            }
+#pragma unroll
+                            for (int k = 0; k < 4; ++k) {
+                                const int ii = c4 + k;
+                                if (ii < b1 && ii >= tlo && ii < thi) {
+                                    const double4 g = sg4[ii];
+                                    const double w = sWc[ii];
+                                    s_dh = fma(g.x, h4[k][0], s_dh); s_dh = fma(-g.y, h4[k][1], s_dh);
+                                    s_dh = fma(g.z, h4[k][2], s_dh); s_dh = fma(-g.w, h4[k][3], s_dh);
+                                    s_hh = fma(w, fma(h4[k][0], h4[k][0], h4[k][1] * h4[k][1]) +
+                                                      fma(h4[k][2], h4[k][2], h4[k][3] * h4[k][3]), s_hh);
+                                }
+                            }
+                        }
+                        return;
+                    }
 #pragma unroll 2
                     for (int ii = b0; ii < b1; ++ii) {
                         const bool act = (ii >= tlo) && (ii < thi);
