@@ -1384,8 +1384,13 @@ int ll_pt_swap(ll_ctx *ctx, int32_t n_temps, int32_t n_walkers, double *x, doubl
     if (!x || !logL || !betas || (n_temps > 1 && !u_swap)) return ctx->fail(LL_ERR_ARG, "NULL argument");
     if (n_temps == 1) return LL_OK;
     DeviceGuard dg(ctx->device);
-    k_pt_swap<<<(int)ceil_div(n_walkers, 128), 128, 0, (cudaStream_t)stream>>>(x, logL, d_h, h_h, n_temps, n_walkers,
-                                                                              5 + 2 * kNC * ctx->n_m, betas, u_swap, swapped);
+    const int P = 5 + 2 * kNC * ctx->n_m;
+    if (n_temps <= 32 && P <= 64)
+        k_pt_swap_warp<<<(int)ceil_div(n_walkers, 4), 128, 0, (cudaStream_t)stream>>>(x, logL, d_h, h_h, n_temps, n_walkers, P,
+                                                                                     betas, u_swap, swapped);
+    else
+        k_pt_swap<<<(int)ceil_div(n_walkers, 128), 128, 0, (cudaStream_t)stream>>>(x, logL, d_h, h_h, n_temps, n_walkers, P,
+                                                                                  betas, u_swap, swapped);
     LAUNCHED(ctx);
     return LL_OK;
 }

@@ -2432,6 +2432,66 @@ k_pt_swap(double *__restrict__ x, double *__restrict__ logL, double *__restrict_
     }
 }
 
+// The same sweep with one WARP per walker column for n_t <= 32 and P <= 32 * kSwapRegs... (P <= 64): every row of the
+// column is loaded up front (lane q holds coordinate q of each rung; lane t holds ln L, <d|h>, <h|h> and ln u of rung
+// t), the cascade then runs on registers and shuffles, and the rows that changed are written back.  Same decisions
+// and results as k_pt_swap; the chain of dependent global loads (one per rung) is gone.
+__global__ void __launch_bounds__(128)
+k_pt_swap_warp(double *__restrict__ x, double *__restrict__ logL, double *__restrict__ d_h, double *__restrict__ h_h,
+               int n_t, int n_w, int P, const double *__restrict__ betas, const double *__restrict__ u_swap,
+               int *__restrict__ swapped)
+{
+    const int lane = threadIdx.x & 31;
+    const int i = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (i >= n_w) return; // whole warp
+    // rung data, one rung per lane
+    const bool has = lane < n_t;
+    const size_t col = (size_t)(has ? lane : 0) * n_w + i;
+    double l = has ? logL[col] : 0.0;
+    double dh = (has && d_h) ? d_h[col] : 0.0, hh = (has && h_h) ? h_h[col] : 0.0;
+    const double beta = has ? betas[lane] : 0.0;
+    const double lnu = (lane >= 1 && has) ? log(u_swap[(size_t)(lane - 1) * n_w + i]) : 0.0; // for the pair (lane, lane-1)
+    // coordinates: lane q (and q + 32) of every rung
+    double xa[32], xb[32];
+#pragma unroll
+    for (int t = 0; t < 32; ++t) {
+        xa[t] = (t < n_t && lane < P) ? x[((size_t)t * n_w + i) * P + lane] : 0.0;
+        xb[t] = (t < n_t && lane + 32 < P) ? x[((size_t)t * n_w + i) * P + lane + 32] : 0.0;
+    }
+    unsigned changed = 0u;
+#pragma unroll
+    for (int t = 31; t >= 1; --t) {
+        if (t < n_t) { // uniform
+            const double lh = __shfl_sync(0xffffffffu, l, t), lc = __shfl_sync(0xffffffffu, l, t - 1);
+            const double bh = __shfl_sync(0xffffffffu, beta, t), bc = __shfl_sync(0xffffffffu, beta, t - 1);
+            const double lu = __shfl_sync(0xffffffffu, lnu, t);
+            const bool sw = lu < __dmul_rn(__dadd_rn(bh, -bc), __dadd_rn(lc, -lh));
+            if (sw) {
+                const double ta = xa[t]; xa[t] = xa[t - 1]; xa[t - 1] = ta;
+                const double tb = xb[t]; xb[t] = xb[t - 1]; xb[t - 1] = tb;
+                // rung values live in lanes t and t-1: exchange them
+                const double dhh = __shfl_sync(0xffffffffu, dh, t), dhc = __shfl_sync(0xffffffffu, dh, t - 1);
+                const double hhh = __shfl_sync(0xffffffffu, hh, t), hhc = __shfl_sync(0xffffffffu, hh, t - 1);
+                if (lane == t) { l = lc; dh = dhc; hh = hhc; }
+                if (lane == t - 1) { l = lh; dh = dhh; hh = hhh; }
+                changed |= (1u << t) | (1u << (t - 1));
+            }
+            if (swapped && lane == 0) swapped[(size_t)(t - 1) * n_w + i] = sw ? 1 : 0;
+        }
+    }
+#pragma unroll
+    for (int t = 0; t < 32; ++t)
+        if (t < n_t && ((changed >> t) & 1u)) {
+            if (lane < P) x[((size_t)t * n_w + i) * P + lane] = xa[t];
+            if (lane + 32 < P) x[((size_t)t * n_w + i) * P + lane + 32] = xb[t];
+        }
+    if (has && ((changed >> lane) & 1u)) {
+        logL[col] = l;
+        if (d_h) d_h[col] = dh;
+        if (h_h) h_h[col] = hh;
+    }
+}
+
 // what the stopping tests look at: out[0] = max finite log L, out[1] = its index (lowest on
 // ties, -1 if none), out[2] = max extracted SNR <d|h>/sqrt(<h|h>) over entries with <h|h> > 0.  One block.
 __global__ void __launch_bounds__(1024)
