@@ -118,3 +118,46 @@ class StopConverged:
         else:
             self.count += 1
         return self.count >= self.n_checks
+
+
+# ------------------------------------------------------------------ counter-based uniforms and a whole run
+# R31: when the sampler runs by itself for many iterations (ll_pt_run_het) the uniforms come from a
+# counter-based generator that this oracle and the CUDA path each implement: SplitMix64 (Steele, Lea & Flood 2014).
+#   mix(z): z ^= z >> 30; z *= 0xBF58476D1CE4E5B9; z ^= z >> 27; z *= 0x94D049BB133111EB; z ^= z >> 31
+#   stream key   k = mix(seed + G (8 iter + kind + 1)),  G = 0x9E3779B97F4A7C15
+#   r(index)     = mix(k + G (index + 1))        (= the (index+1)-th output of SplitMix64 seeded with k)
+#   u            = (r >> 11) 2^-53  in [0, 1)
+# kinds: 0, 1, 2 = u_z, u_partner, u_accept of half 0; 3, 4, 5 = the same of half 1; 6 = u_swap.
+_G = 0x9E3779B97F4A7C15
+_M64 = (1 << 64) - 1
+
+
+def _mix(z: int) -> int:
+    z &= _M64
+    z = ((z ^ (z >> 30)) * 0xBF58476D1CE4E5B9) & _M64
+    z = ((z ^ (z >> 27)) * 0x94D049BB133111EB) & _M64
+    return z ^ (z >> 31)
+
+
+def stream_key(seed: int, it: int, kind: int) -> int:
+    return _mix(seed + _G * (8 * it + kind + 1))
+
+
+def uniforms(seed: int, it: int, kind: int, n: int) -> np.ndarray:
+    k = stream_key(seed, it, kind)
+    return np.array([(_mix(k + _G * (i + 1)) >> 11) * 2.0 ** -53 for i in range(n)])
+
+
+def run(x, logL, betas, lo, hi, n_dim, a, seed, iter0, n_iter, loglike):
+    """n_iter iterations (half 0, half 1, swap sweep) in place; returns accepted proposals per temperature."""
+    n_t, n_w, _ = x.shape
+    nh = n_w // 2
+    n_acc = np.zeros(n_t, dtype=np.int64)
+    for it in range(iter0, iter0 + n_iter):
+        for half in (0, 1):
+            u = [uniforms(seed, it, 3 * half + q, n_t * nh).reshape(n_t, nh) for q in range(3)]
+            acc, _, _, _ = stretch_half(x, logL, half, betas, lo, hi, n_dim, a, u[0], u[1], u[2], loglike)
+            n_acc += acc.sum(axis=1)
+        if n_t > 1:
+            temperature_swaps(x, logL, betas, uniforms(seed, it, 6, (n_t - 1) * n_w).reshape(n_t - 1, n_w))
+    return n_acc

@@ -933,3 +933,38 @@ def test_notaknot_full_path_brute_force(notaknot):
         h_h = (W * np.abs(h) ** 2).sum()
         assert got["d_h"][w] == pytest.approx(d_h, rel=1e-9, abs=1e-9 * h_h)
         assert got["h_h"][w] == pytest.approx(h_h, rel=1e-10)
+
+
+def test_counter_based_uniforms_are_splitmix64():
+    """Known answers of SplitMix64 (seed 1234567: the reference implementation's first outputs), range, and the plain
+    statistics of a uniform: mean 1/2, variance 1/12, no correlation between neighbouring streams or indices."""
+    from oracle import sampler as sm
+    kat = [6457827717110365317, 3203168211198807973, 9817491932198370423, 4593380528125082431, 16408922859458223821]
+    assert [sm._mix(1234567 + sm._G * (i + 1)) for i in range(5)] == kat
+    u = np.concatenate([sm.uniforms(99, it, kind, 500) for it in range(4) for kind in range(7)])
+    assert u.min() >= 0.0 and u.max() < 1.0
+    assert abs(u.mean() - 0.5) < 0.01 and abs(u.var() - 1.0 / 12.0) < 0.003
+    a, b = sm.uniforms(99, 0, 0, 4000), sm.uniforms(99, 0, 1, 4000)
+    assert abs(np.corrcoef(a, b)[0, 1]) < 0.05 and abs(np.corrcoef(a[:-1], a[1:])[0, 1]) < 0.05
+    assert not np.array_equal(sm.uniforms(99, 1, 0, 8), sm.uniforms(99, 0, 0, 8))
+    assert np.array_equal(sm.uniforms(99, 3, 2, 8), sm.uniforms(99, 3, 2, 8))        # a pure function of its counter
+
+
+def test_sampler_run_keeps_gaussian_target():
+    """the whole loop (halves + swaps, counter-based uniforms) on a 2-d Gaussian: cold chain keeps the target"""
+    from oracle import sampler as sm
+    C = np.array([[1.0, 0.5], [0.5, 2.0]])
+    ll = _gauss_loglike(np.linalg.inv(C))
+    rng = np.random.default_rng(3)
+    x = rng.normal(size=(3, 32, 2))
+    logL = np.stack([ll(x[t])[0] for t in range(3)])
+    betas = np.array([1.0, 0.5, 0.1])
+    keep = []
+    for blk in range(40):
+        n_acc = sm.run(x, logL, betas, np.full(2, -np.inf), np.full(2, np.inf), 2, 2.0, 7, 25 * blk, 25, ll)
+        if blk >= 8:
+            keep.append(x[0].copy())
+        assert np.all(n_acc > 0)
+    s = np.concatenate(keep)
+    np.testing.assert_allclose(np.cov(s.T), C, rtol=0.2, atol=0.15)
+    np.testing.assert_allclose(logL[0], ll(x[0])[0], rtol=1e-12)
