@@ -231,6 +231,19 @@ int ll_pt_swap(ll_ctx *ctx, int32_t n_temps, int32_t n_walkers, double *x, doubl
                const double *betas, const double *u_swap, int32_t *swapped, void *stream);
 int ll_pt_stats(ll_ctx *ctx, int64_t n, const double *logL, const double *d_h, const double *h_h, double *out3,
                 void *stream);
+/* ll_pt_run_*: n_iter whole iterations (half 0, half 1, swap sweep; iterations iter0 .. iter0 + n_iter - 1) with the
+ *   library's own counter-based uniforms (reading R31: SplitMix64; u[kind][index] of iteration it is
+ *   mix(mix(seed + G (8 it + kind + 1)) + G (index + 1)) >> 11, times 2^-53; kinds 0-2 = u_z, u_partner, u_accept of
+ *   half 0, 3-5 of half 1, 6 = u_swap; G = 0x9E3779B97F4A7C15), so a run is a pure function of (seed, iter0, state).
+ *   Everything is enqueued on `stream` (9 launches per iteration for the heterodyned likelihood) and nothing returns to
+ *   the host in between; call ll_pt_stats and the stopping functions between runs (every 150 iterations in the paper).
+ *   n_accepted : DEV [n_temps] uint64, accepted proposals are ADDED to it (zero it first), or NULL.            */
+int ll_pt_run_het(ll_ctx *ctx, int32_t n_temps, int32_t n_walkers, double *x, double *logL, double *d_h, double *h_h,
+                  const double *betas, const double *lo, const double *hi, int32_t n_dim, double a, uint64_t seed,
+                  int64_t iter0, int64_t n_iter, uint64_t *n_accepted, void *stream);
+int ll_pt_run_full(ll_ctx *ctx, int32_t n_nodes, const double *f_nodes, int32_t n_temps, int32_t n_walkers, double *x,
+                   double *logL, double *d_h, double *h_h, const double *betas, const double *lo, const double *hi,
+                   int32_t n_dim, double a, uint64_t seed, int64_t iter0, int64_t n_iter, uint64_t *n_accepted, void *stream);
 typedef struct {
     int32_t n_checks; /* consecutive unchanged checks needed to stop (30 in the paper)   */
     int32_t count;    /* consecutive unchanged checks so far                             */

@@ -25,7 +25,7 @@ SYMBOLS = (
     "ll_full_batch", "ll_full_batch_pw", "ll_full_batch_tf", "ll_tlm_nodes", "ll_standin_nodes", "ll_full_batch_standin", "ll_full_batch_standin_host",
     "ll_full_template_standin",
     "ll_template_standin", "ll_het_prepare", "ll_het_refresh_standin", "ll_het_audit_standin",
-    "ll_pt_stretch_half_het", "ll_pt_stretch_half_full", "ll_pt_swap", "ll_pt_stats", "ll_stop_snr", "ll_stop_converged", "ll_het_get_summary", "ll_het_batch", "ll_het_batch_standin",
+    "ll_pt_stretch_half_het", "ll_pt_stretch_half_full", "ll_pt_swap", "ll_pt_stats", "ll_pt_run_het", "ll_pt_run_full", "ll_stop_snr", "ll_stop_converged", "ll_het_get_summary", "ll_het_batch", "ll_het_batch_standin",
     "ll_het_batch_standin_host", "ll_peak_fma", "ll_kernel_launches", "ll_last_full_stats",
     "ll_profile_enable", "ll_profile_read",
 )
@@ -83,6 +83,9 @@ def load_library(path: Optional[str] = None):
         "ll_pt_stretch_half_full": (C.c_int, [vp, i32, vp, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp, i32, dbl, vp, vp, vp,
                                               vp, vp]),
         "ll_pt_swap": (C.c_int, [vp, i32, i32, vp, vp, vp, vp, vp, vp, vp, vp]),
+        "ll_pt_run_het": (C.c_int, [vp, i32, i32, vp, vp, vp, vp, vp, vp, vp, i32, dbl, C.c_uint64, i64, i64, vp, vp]),
+        "ll_pt_run_full": (C.c_int, [vp, i32, vp, i32, i32, vp, vp, vp, vp, vp, vp, vp, i32, dbl, C.c_uint64, i64, i64, vp,
+                                     vp]),
         "ll_pt_stats": (C.c_int, [vp, i64, vp, vp, vp, vp, vp]),
         "ll_stop_snr": (C.c_int, [dbl, dbl]),
         "ll_stop_converged": (C.c_int, [vp, dbl]),
@@ -385,6 +388,24 @@ class Context:
             f_nodes = _host_f64(f_nodes, "f_nodes")
             self._check(self._lib.ll_pt_stretch_half_full(self._h, len(f_nodes), f_nodes.ctypes.data_as(C.c_void_p), *tail),
                         "ll_pt_stretch_half_full")
+
+    def pt_run(self, x, logL, d_h, h_h, betas, lo, hi, n_dim, seed, iter0, n_iter, a=2.0, n_accepted=None, f_nodes=None,
+               stream=None):
+        """n_iter whole iterations with the library's counter-based uniforms (reading R31); n_accepted: int64 CUDA
+        tensor [n_temps] the accepted proposals are added to, or None"""
+        torch = _torch()
+        if n_accepted is not None and not (n_accepted.is_cuda and n_accepted.dtype == torch.int64 and n_accepted.is_contiguous()):
+            raise TypeError("n_accepted: need a contiguous int64 CUDA tensor")
+        acc = None if n_accepted is None else C.c_void_p(n_accepted.data_ptr())
+        tail = (int(x.shape[0]), int(x.shape[1]), _dev_ptr(x, "x"), _dev_ptr(logL, "logL"), _dev_ptr(d_h, "d_h"),
+                _dev_ptr(h_h, "h_h"), _dev_ptr(betas, "betas"), _dev_ptr(lo, "lo"), _dev_ptr(hi, "hi"), int(n_dim), float(a),
+                int(seed), int(iter0), int(n_iter), acc, _stream_ptr(stream))
+        if f_nodes is None:
+            self._check(self._lib.ll_pt_run_het(self._h, *tail), "ll_pt_run_het")
+        else:
+            f_nodes = _host_f64(f_nodes, "f_nodes")
+            self._check(self._lib.ll_pt_run_full(self._h, len(f_nodes), f_nodes.ctypes.data_as(C.c_void_p), *tail),
+                        "ll_pt_run_full")
 
     def pt_swap(self, x, logL, d_h, h_h, betas, u_swap, swapped=None, stream=None):
         self._check(self._lib.ll_pt_swap(self._h, int(x.shape[0]), int(x.shape[1]), _dev_ptr(x, "x"), _dev_ptr(logL, "logL"),

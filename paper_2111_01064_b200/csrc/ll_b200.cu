@@ -102,6 +102,7 @@ struct ll_ctx {
     bool have_het = false;
     int n_e = 0;
     DevBuf het_tab, het_raw, het_idx, het_fb, het_tab1;
+    DevBuf pt_u;                // ll_pt_run_*: the uniforms of one iteration
     DevBuf pt_y, pt_out, pt_in; // sampler step: proposals [n][P], (log L, <d|h>, <h|h>, (d-1) ln z) [4][n], inside flags
     DevBuf ref_idx, ref_dense, ref_edges; // ll_het_refresh_standin: argmax slot, h0 on the grid, h0 and f at the edges
     HetTable ht{};
@@ -834,7 +835,7 @@ int ll_destroy(ll_ctx *ctx)
                          &ctx->key_w, &ctx->hist, &ctx->perm, &ctx->ilo_s, &ctx->ihi_s, &ctx->Y, &ctx->C, &ctx->TF,
                          &ctx->part, &ctx->prow, &ctx->het_tab, &ctx->het_tab1, &ctx->het_raw, &ctx->het_idx, &ctx->het_fb,
                          &ctx->stage_in, &ctx->stage_out, &ctx->g4f, &ctx->Wf, &ctx->scale, &ctx->wmax, &ctx->ref_idx,
-                         &ctx->ref_dense, &ctx->ref_edges, &ctx->tile_tab, &ctx->part2, &ctx->pw_x, &ctx->pt_y, &ctx->pt_out, &ctx->pt_in};
+                         &ctx->ref_dense, &ctx->ref_edges, &ctx->tile_tab, &ctx->part2, &ctx->pw_x, &ctx->pt_y, &ctx->pt_out, &ctx->pt_in, &ctx->pt_u};
         for (DevBuf *b : all) b->release();
         for (auto &e : ctx->ev) cudaEventDestroy(e);
     }
@@ -1328,7 +1329,7 @@ namespace {
 int pt_half(ll_ctx *ctx, bool full, int32_t n_nodes, const double *f_nodes, int32_t n_t, int32_t n_w, int32_t half,
             double *x, double *logL, double *d_h, double *h_h, const double *betas, const double *lo, const double *hi,
             int32_t n_dim, double a, const double *u_z, const double *u_partner, const double *u_accept,
-            int32_t *accepted, void *stream)
+            int32_t *accepted, void *stream, unsigned long long *n_acc = nullptr)
 {
     if (!ctx) return LL_ERR_ARG;
     if (n_t < 1 || n_w < 2 || (n_w & 1)) return ctx->fail(LL_ERR_ARG, "n_temps >= 1 and an even n_walkers >= 2 are required");
@@ -1352,7 +1353,7 @@ int pt_half(ll_ctx *ctx, bool full, int32_t n_nodes, const double *f_nodes, int3
                   : ll_het_batch_standin(ctx, np, y, ly, ydh, yhh, stream);
     if (rc != LL_OK) return rc;
     k_pt_accept<<<grid, 128, 0, st>>>(x, logL, d_h, h_h, n_t, n_w, P, half, betas, u_accept, y, ly, ydh, yhh, lnz,
-                                      ctx->pt_in.as<int>(), accepted);
+                                      ctx->pt_in.as<int>(), accepted, n_acc);
     LAUNCHED(ctx);
     return LL_OK;
 }
@@ -1393,6 +1394,56 @@ int ll_pt_swap(ll_ctx *ctx, int32_t n_temps, int32_t n_walkers, double *x, doubl
                                                                                   betas, u_swap, swapped);
     LAUNCHED(ctx);
     return LL_OK;
+}
+
+// n_iter whole iterations (half 0, half 1, swap sweep) with the library's own counter-based uniforms (reading R31):
+// every launch is enqueued on `stream`, nothing returns to the host in between.
+namespace {
+int pt_run(ll_ctx *ctx, bool full, int32_t n_nodes, const double *f_nodes, int32_t n_t, int32_t n_w, double *x, double *logL,
+           double *d_h, double *h_h, const double *betas, const double *lo, const double *hi, int32_t n_dim, double a,
+           uint64_t seed, int64_t iter0, int64_t n_iter, uint64_t *n_accepted, void *stream)
+{
+    if (!ctx) return LL_ERR_ARG;
+    if (n_iter < 0 || iter0 < 0) return ctx->fail(LL_ERR_ARG, "iter0, n_iter >= 0 are required");
+    if (n_t < 1 || n_w < 2 || (n_w & 1)) return ctx->fail(LL_ERR_ARG, "n_temps >= 1 and an even n_walkers >= 2 are required");
+    if ((int64_t)n_t * n_w > (1LL << 28)) return ctx->fail(LL_ERR_ARG, "n_temps * n_walkers too large");
+    DeviceGuard dg(ctx->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    const int n_half = n_t * (n_w / 2), n_swap = (n_t - 1) * n_w;
+    CK(ctx->pt_u.ensure(sizeof(double) * (size_t)(6 * n_half + n_swap)));
+    double *u = ctx->pt_u.as<double>();
+    for (int64_t it = iter0; it < iter0 + n_iter; ++it) {
+        k_pt_uniforms<<<ceil_div(6 * n_half + n_swap, 256), 256, 0, st>>>(seed, it, n_half, n_swap, u);
+        LAUNCHED(ctx);
+        for (int half = 0; half < 2; ++half) {
+            const double *uh = u + (size_t)3 * half * n_half;
+            int rc = pt_half(ctx, full, n_nodes, f_nodes, n_t, n_w, half, x, logL, d_h, h_h, betas, lo, hi, n_dim, a, uh,
+                             uh + n_half, uh + 2 * (size_t)n_half, nullptr, stream, (unsigned long long *)n_accepted);
+            if (rc != LL_OK) return rc;
+        }
+        if (n_t > 1) {
+            int rc = ll_pt_swap(ctx, n_t, n_w, x, logL, d_h, h_h, betas, u + (size_t)6 * n_half, nullptr, stream);
+            if (rc != LL_OK) return rc;
+        }
+    }
+    return LL_OK;
+}
+} // namespace
+
+int ll_pt_run_het(ll_ctx *ctx, int32_t n_temps, int32_t n_walkers, double *x, double *logL, double *d_h, double *h_h,
+                  const double *betas, const double *lo, const double *hi, int32_t n_dim, double a, uint64_t seed,
+                  int64_t iter0, int64_t n_iter, uint64_t *n_accepted, void *stream)
+{
+    return pt_run(ctx, false, 0, nullptr, n_temps, n_walkers, x, logL, d_h, h_h, betas, lo, hi, n_dim, a, seed, iter0, n_iter,
+                  n_accepted, stream);
+}
+
+int ll_pt_run_full(ll_ctx *ctx, int32_t n_nodes, const double *f_nodes, int32_t n_temps, int32_t n_walkers, double *x,
+                   double *logL, double *d_h, double *h_h, const double *betas, const double *lo, const double *hi,
+                   int32_t n_dim, double a, uint64_t seed, int64_t iter0, int64_t n_iter, uint64_t *n_accepted, void *stream)
+{
+    return pt_run(ctx, true, n_nodes, f_nodes, n_temps, n_walkers, x, logL, d_h, h_h, betas, lo, hi, n_dim, a, seed, iter0,
+                  n_iter, n_accepted, stream);
 }
 
 int ll_pt_stats(ll_ctx *ctx, int64_t n, const double *logL, const double *d_h, const double *h_h, double *out3, void *stream)

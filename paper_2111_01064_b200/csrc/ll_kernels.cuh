@@ -2384,7 +2384,7 @@ k_pt_accept(double *__restrict__ x, double *__restrict__ logL, double *__restric
             int n_t, int n_w, int P, int half, const double *__restrict__ betas, const double *__restrict__ u_accept,
             const double *__restrict__ y, const double *__restrict__ ly, const double *__restrict__ ydh,
             const double *__restrict__ yhh, const double *__restrict__ lnz, const int *__restrict__ inside,
-            int *__restrict__ accepted)
+            int *__restrict__ accepted, unsigned long long *__restrict__ n_acc)
 {
     const int nh = n_w / 2;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -2406,6 +2406,7 @@ k_pt_accept(double *__restrict__ x, double *__restrict__ logL, double *__restric
         if (h_h) h_h[wk] = yhh[i];
     }
     if (accepted) accepted[i] = acc ? 1 : 0;
+    if (n_acc && acc) atomicAdd(n_acc + t, 1ull); // integer: order-independent
 }
 
 // temperature swaps (R27): one thread per walker column i, rungs swept from the hottest down, sequential in t
@@ -2490,6 +2491,29 @@ k_pt_swap_warp(double *__restrict__ x, double *__restrict__ logL, double *__rest
         if (d_h) d_h[col] = dh;
         if (h_h) h_h[col] = hh;
     }
+}
+
+// Counter-based uniforms for ll_pt_run_* (reading R31): SplitMix64.  u[kind][index] of iteration `it`:
+//   k = mix(seed + G (8 it + kind + 1)),  r = mix(k + G (index + 1)),  u = (r >> 11) 2^-53 in [0, 1)
+// kinds 0-2 = u_z, u_partner, u_accept of half 0; 3-5 = of half 1 (n_half = n_t n_w/2 each); 6 = u_swap ((n_t-1) n_w).
+__host__ __device__ __forceinline__ unsigned long long splitmix_mix(unsigned long long z)
+{
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+    z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+    return z ^ (z >> 31);
+}
+__global__ void __launch_bounds__(256)
+k_pt_uniforms(unsigned long long seed, long long it, int n_half, int n_swap, double *__restrict__ u)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int total = 6 * n_half + n_swap;
+    if (i >= total) return;
+    const int kind = (i < 6 * n_half) ? i / n_half : 6;
+    const int index = i - kind * n_half;
+    const unsigned long long G = 0x9E3779B97F4A7C15ull;
+    const unsigned long long k = splitmix_mix(seed + G * (unsigned long long)(8 * it + kind + 1));
+    const unsigned long long r = splitmix_mix(k + G * (unsigned long long)(index + 1));
+    u[i] = (double)(r >> 11) * 0x1.0p-53;
 }
 
 // what the stopping tests look at: out[0] = max finite log L, out[1] = its index (lowest on

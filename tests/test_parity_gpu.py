@@ -823,3 +823,32 @@ def test_one_year_noiseless_logL_is_zero_at_truth(orc, torch_cuda):
     gb = ctx.full_batch_standin(wl.f_nodes, dev(torch_cuda, big))[0].cpu().numpy().reshape(2000, 3)
     assert np.all(np.abs(gb - ref["logL"][None, :]) <= 1e-6 * np.maximum(1.0, np.abs(ref["logL"]))[None, :])
     ctx.destroy()
+
+
+def test_pt_run_parity_het(orc, het_small, torch_cuda):
+    """ll_pt_run_het: 12 whole iterations with the counter-based uniforms (reading R31) against the oracle's loop with
+    its own implementation of the same generator: identical positions, acceptance counts, log L at the FP64 bar;
+    two runs of 6 continue exactly like one run of 12."""
+    from oracle import sampler as sm
+    wl, d, h0, h0e, summ, ctx = het_small
+    tc = torch_cuda
+    n_t, n_w = 3, 64
+    x = wl.params[:n_t * n_w].reshape(n_t, n_w, -1).copy()
+    x[:, :, 5:] = wl.inj[5:]
+    betas = np.array([1.0, 0.3, 0.05])
+    lo, hi = _prior_box(wl, wl.params, 0.35)
+    ll = _oracle_loglike_het(orc, wl, h0e, summ)
+    logL = ll(x.reshape(n_t * n_w, -1))[0].reshape(n_t, n_w).copy()
+    gx, gl = dev(tc, x), dev(tc, logL)
+    gx2, gl2 = gx.clone(), gl.clone()
+    acc_g = tc.zeros(n_t, dtype=tc.int64, device="cuda")
+    seed = 2111_01064
+    n_acc = sm.run(x, logL, betas, lo, hi, 5, 2.0, seed, 100, 12, ll)
+    ctx.pt_run(gx, gl, None, None, dev(tc, betas), dev(tc, lo), dev(tc, hi), 5, seed, 100, 12, n_accepted=acc_g)
+    assert np.array_equal(gx.cpu().numpy(), x)
+    assert np.array_equal(acc_g.cpu().numpy(), n_acc) and n_acc.sum() > 200
+    err = np.abs(gl.cpu().numpy() - logL) / np.maximum(1.0, np.abs(logL))
+    assert err.max() <= 1e-6
+    ctx.pt_run(gx2, gl2, None, None, dev(tc, betas), dev(tc, lo), dev(tc, hi), 5, seed, 100, 6)
+    ctx.pt_run(gx2, gl2, None, None, dev(tc, betas), dev(tc, lo), dev(tc, hi), 5, seed, 106, 6)
+    assert tc.equal(gx2, gx) and tc.equal(gl2, gl)
