@@ -269,6 +269,24 @@ def bench_sampler_iteration(torch, ctx, wl, params, n_t: int = 10, n_w: int = 40
                     "max_logL_cold_chain": float(out3[0]), "extracted_snr_cold_chain": float(out3[2])})
     except Exception as e:  # capture is a convenience of the harness, not part of the library
         res["graph_error"] = repr(e)[:200]
+    # ---- the library's own loop: ll_pt_run_* (counter-based uniforms, nothing returns to the host), in blocks of 150
+    # iterations with the stopping statistics read back after each block, as the paper's modules do
+    from paper_2111_01064_b200 import binding
+    n_acc64 = torch.zeros(n_t, dtype=torch.int64, device=x.device)
+    stop = binding.StopState(n_checks=30, tol=1.0)
+    blocks, per_block = (4, 150) if f_nodes is None else (2, 20)
+    ctx.pt_run(x, logL, d_h, h_h, betas, lo, hi, 5, 2111, 0, 5, f_nodes=f_nodes)          # warm-up
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for b in range(blocks):
+        ctx.pt_run(x, logL, d_h, h_h, betas, lo, hi, 5, 2111, 5 + b * per_block, per_block, n_accepted=n_acc64, f_nodes=f_nodes)
+        st3 = ctx.pt_stats(logL[0], d_h[0], h_h[0], out3=out3).cpu()                        # synchronises
+        stopped = binding.stop_converged(stop, float(st3[0])) or binding.stop_snr(float(st3[2]), float("inf"))
+    ms_run = (time.perf_counter() - t0) * 1e3 / (blocks * per_block)
+    res.update({"ms_per_iteration_run": ms_run, "evals_per_s_run": n_t * n_w / (ms_run * 1e-3),
+                "run": "ll_pt_run_%s, %d blocks of %d iterations, stopping statistics read back after each (host wall time)"
+                       % ("het" if f_nodes is None else "full", blocks, per_block),
+                "acceptance_fraction_run": float(n_acc64.sum()) / (blocks * per_block * n_t * n_w), "stopped": bool(stopped)})
     return res
 
 
