@@ -852,3 +852,59 @@ def test_pt_run_parity_het(orc, het_small, torch_cuda):
     ctx.pt_run(gx2, gl2, None, None, dev(tc, betas), dev(tc, lo), dev(tc, hi), 5, seed, 100, 6)
     ctx.pt_run(gx2, gl2, None, None, dev(tc, betas), dev(tc, lo), dev(tc, hi), 5, seed, 106, 6)
     assert tc.equal(gx2, gx) and tc.equal(gl2, gl)
+
+
+def test_module2_loop_with_reference_update(orc, torch_cuda):
+    """The Module-2 loop in miniature: sample, update the reference to the best walker, re-evaluate
+    the population against the new reference, sample on, read the stopping statistics — library calls only on one
+    side, the oracle's step-by-step functions on the other; identical walker positions at the end."""
+    from oracle import sampler as sm
+    from paper_2111_01064_b200 import binding
+    tc = torch_cuda
+    wl = wlm.make_workload(1, n_w=128, t_obs=2.0 ** 18, n_knots=37)
+    d, h0, h0e, summ = oracle_setup_het(orc, wl)
+    ctx = make_ctx(wl)
+    g = wl.grid
+    f = g.freqs()
+    ctx.set_data(g.n_f, g.k_min, g.df, dev(tc, d), dev(tc, wl.W))
+    ctx.het_prepare(wl.f_edges, dev(tc, h0), dev(tc, h0e))
+    n_t, n_w = 2, 64
+    x = wl.params.reshape(n_t, n_w, -1).copy()
+    x[:, :, 5:] = wl.inj[5:]
+    betas = np.array([1.0, 0.2])
+    lo, hi = _prior_box(wl, wl.params, 0.5)
+    seed = 5000
+    # ---- oracle side
+    edges, he, sm_ = wl.f_edges, h0e, summ
+    ll = lambda rows: (orc.het_batch_standin(wl.modes_m, wl.c_lm, wl.kappa, rows, edges, he, sm_)["logL"], {})
+    xo = x.copy()
+    lo_ = ll(xo.reshape(n_t * n_w, -1))[0].reshape(n_t, n_w).copy()
+    sm.run(xo, lo_, betas, lo, hi, 5, 2.0, seed, 0, 10, ll)
+    # ---- library side, first block
+    gx = dev(tc, x)
+    out = ctx.het_batch_standin(gx.reshape(n_t * n_w, -1))
+    gl, gd, gh = (v.reshape(n_t, n_w).clone() for v in out)
+    gb, glo, ghi = dev(tc, betas), dev(tc, lo), dev(tc, hi)
+    ctx.pt_run(gx, gl, gd, gh, gb, glo, ghi, 5, seed, 0, 10)
+    assert np.array_equal(gx.cpu().numpy(), xo)
+    # ---- reference update on both sides (the library's edges are an input of the oracle's H0, cf. test_het_refresh_parity)
+    best, f_edges = ctx.het_refresh_standin(gx.reshape(n_t * n_w, -1), gl.reshape(-1), 38)
+    assert best == sm.population_stats(lo_, lo_, np.ones_like(lo_))[1]
+    pb = xo.reshape(n_t * n_w, -1)[best]
+    h0n = orc.standin_direct(pb, wl.modes_m, wl.c_lm, wl.kappa, f, float(f[0]), float(f[-1]))
+    he = orc.standin_direct(pb, wl.modes_m, wl.c_lm, wl.kappa, f_edges, float(f[0]), float(f[-1]))
+    sm_ = orc.het_prepare(g.k_min, g.df, d, wl.W, h0n, f_edges)
+    edges = f_edges
+    lo_ = ll(xo.reshape(n_t * n_w, -1))[0].reshape(n_t, n_w).copy()
+    out = ctx.het_batch_standin(gx.reshape(n_t * n_w, -1))
+    gl, gd, gh = (v.reshape(n_t, n_w).clone() for v in out)
+    # ---- second block and the stopping statistics
+    sm.run(xo, lo_, betas, lo, hi, 5, 2.0, seed, 10, 10, ll)
+    ctx.pt_run(gx, gl, gd, gh, gb, glo, ghi, 5, seed, 10, 10)
+    assert np.array_equal(gx.cpu().numpy(), xo)
+    st = ctx.pt_stats(gl[0], gd[0], gh[0]).cpu().numpy()
+    best_o, bi_o, _ = sm.population_stats(lo_[0], lo_[0], np.ones(n_w))
+    assert int(st[1]) == bi_o and abs(st[0] - best_o) <= 1e-6 * max(1.0, abs(best_o))
+    stop = binding.StopState(n_checks=30, tol=1.0)
+    assert not binding.stop_converged(stop, float(st[0]))
+    ctx.destroy()
