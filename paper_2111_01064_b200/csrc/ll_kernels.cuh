@@ -1464,16 +1464,34 @@ k_spline_pw(const double *__restrict__ Y, const double *__restrict__ X, double *
         Mn = (1.0 + rhon) * M2 - rhon * M3;
     }
     double xh = __ldg(x + (size_t)(n - 1) * sw), yh = __ldg(y + (size_t)(n - 1) * sw);
-    for (int j = n - 2; j >= 0; --j) {
-        const double xl = __ldg(x + (size_t)j * sw), yl = __ldg(y + (size_t)j * sw);
-        double *cc = c + (size_t)j * cj;
-        const double Mj = (j >= 1) ? fma(-cc[2 * sw], Mn, cc[sw]) : (bc ? (1.0 + rho0) * Mn - rho0 * Mnn : 0.0);
-        const double h = xh - xl, ih = 1.0 / h;
-        cc[0] = yl;
-        cc[sw] = (yh - yl) * ih - h * (2.0 * Mj + Mn) * kSixth;
-        cc[2 * sw] = 0.5 * Mj;
-        cc[3 * sw] = (Mn - Mj) * ih * kSixth;
-        Mnn = Mn; Mn = Mj; xh = xl; yh = yl;
+    // backward sweep in register blocks of 8 rows (loads first, then the recurrence, then the stores): a load of the
+    // parked c', dp of row j issued between the stores of row j + 1 could not be hoisted (same base pointer)
+    constexpr int kB = 8;
+    for (int jt = n - 2; jt >= 0; jt -= kB) {
+        double xv[kB], yv[kB], dpv[kB], cpv[kB];
+#pragma unroll
+        for (int k = 0; k < kB; ++k) {
+            const int j = jt - k;
+            xv[k] = (j >= 0) ? __ldg(x + (size_t)j * sw) : 0.0;
+            yv[k] = (j >= 0) ? __ldg(y + (size_t)j * sw) : 0.0;
+            dpv[k] = (j >= 1) ? c[(size_t)j * cj + sw] : 0.0;
+            cpv[k] = (j >= 1) ? c[(size_t)j * cj + 2 * sw] : 0.0;
+        }
+#pragma unroll
+        for (int k = 0; k < kB; ++k) {
+            const int j = jt - k;
+            if (j >= 0) {
+                const double xl = xv[k], yl = yv[k];
+                double *cc = c + (size_t)j * cj;
+                const double Mj = (j >= 1) ? fma(-cpv[k], Mn, dpv[k]) : (bc ? (1.0 + rho0) * Mn - rho0 * Mnn : 0.0);
+                const double h = xh - xl, ih = 1.0 / h;
+                cc[0] = yl;
+                cc[sw] = (yh - yl) * ih - h * (2.0 * Mj + Mn) * kSixth;
+                cc[2 * sw] = 0.5 * Mj;
+                cc[3 * sw] = (Mn - Mj) * ih * kSixth;
+                Mnn = Mn; Mn = Mj; xh = xl; yh = yl;
+            }
+        }
     }
 }
 
