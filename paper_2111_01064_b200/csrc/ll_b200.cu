@@ -738,8 +738,8 @@ int launch_het_standin(ll_ctx *ctx, int64_t n_w, const double *params, double *l
 {
     const int n_groups = ceil_div(n_w, 32), n_b = ctx->ht.n_b;
     constexpr int WY = LL_HET_WY; // warps per block, all sharing one table copy
-    // table + [WY][2][32] segment partials + -(m/pi) + lane-major transfer factors of the G = WY/S walker groups
-    auto smem_of = [&](int s) { return sizeof(double) * ((size_t)ctx->ht.total + (size_t)WY * 64 + 8 + (size_t)(WY / s) * NM * 128); };
+    // table + [WY][2][32] segment partials + -(m/pi) + the staged parameter rows of the G = WY/S walker groups
+    auto smem_of = [&](int s) { return sizeof(double) * ((size_t)ctx->ht.total + (size_t)WY * 64 + 8 + (size_t)(WY / s) * 32 * (5 + 4 * NM)); };
     static bool attr_set = false;
     if (!attr_set) {
         CK(cudaFuncSetAttribute(k_het_standin<NM>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));

@@ -2034,7 +2034,7 @@ __device__ __forceinline__ void het_bin_contract(const double *__restrict__ tb, 
 // lane needs the taper polynomial is decided once per chunk (warp-uniform), below f_ISCO m_min/2 it is 1.
 struct HetEdgeCtx {
     const double *f4, *ih0, *cfp, *f2m, *fm53;
-    const double *tfs; // shared, [n_m][4][32] + lane
+    const double *tfs; // shared: this lane's staged parameter row + 5, i.e. T^c_m (re, im) mode-major, [n_m][4]
     const double *nmq; // shared, [n_m]: -(m/pi)
     int n_e;
     double tc, invD, inv_fisco, K, phi0, kappa, inv_kappa;
@@ -2052,8 +2052,8 @@ __device__ __forceinline__ void het_eval_edges(const HetEdgeCtx &x, const Standi
 #pragma unroll 1
     for (int m = 0; m < NM; ++m) {
         const double nmq = x.nmq[m]; // -(m/pi), shared
-        const double *tq = x.tfs + m * 128;
-        const double t0 = tq[0], t1 = tq[32], t2 = tq[64], t3 = tq[96];
+        const double *tq = x.tfs + m * 4;
+        const double t0 = tq[0], t1 = tq[1], t2 = tq[2], t3 = tq[3];
         const int t = m * x.n_e + e;
 #pragma unroll
         for (int k = 0; k < E; ++k) {
@@ -2096,14 +2096,13 @@ k_het_standin(HetTable T, StandinInfo si, const double *__restrict__ params, int
     const int G = blockDim.y / S, seg = threadIdx.y % S, gslot = threadIdx.y / S, lane = threadIdx.x;
     double *red = tab + T.total;                 // [G][S][2][32]
     double *nmq_s = red + (size_t)blockDim.y * 64;   // [8]
-    double *tfs_all = nmq_s + 8;                     // [G][NM][4][32]
+    double *tfs_all = nmq_s + 8;                     // [G][32][P]: the parameter rows of the pass
     for (int i = threadIdx.x + threadIdx.y * 32; i < T.total; i += 32 * blockDim.y) tab[i] = T.base[i];
     if (threadIdx.y == 0 && lane < NM) nmq_s[lane] = -((double)si.mode_m[lane] / kPi);
     const int b0 = (int)((long long)seg * T.n_b / S), b1 = (int)((long long)(seg + 1) * T.n_b / S); // balanced to +-1 bin
     HetEdgeCtx x;
     x.f4 = tab + T.off_f4(); x.ih0 = tab + T.off_ih0(); x.cfp = tab + T.off_cfp();
     x.f2m = tab + T.off_f2m(); x.fm53 = tab + T.off_fm53();
-    x.tfs = tfs_all + (size_t)gslot * NM * 128 + lane;
     x.nmq = nmq_s;
     x.n_e = T.n_e;
     x.kappa = si.kappa;
@@ -2118,17 +2117,18 @@ k_het_standin(HetTable T, StandinInfo si, const double *__restrict__ params, int
         const int grp = base + gslot;
         const int w = grp * 32 + lane;
         const bool valid = grp < n_groups && w < n_w;
-        const double *row = params + (size_t)(valid ? w : 0) * P;
-        const WalkerConst c = standin_consts(row);
-        x.tc = c.tc; x.invD = c.invD; x.inv_fisco = c.inv_fisco; x.K = c.K;
-        x.phi0 = c.phi + 0.25 * kPi;
-        __syncthreads(); // table staged (first pass) / previous pass done with tfs and red
-        if (seg == 0) {
-            double *tw = tfs_all + (size_t)gslot * NM * 128 + lane;
-#pragma unroll
-            for (int q = 0; q < 4 * NM; ++q) tw[q * 32] = row[5 + q];
+        __syncthreads(); // table staged (first pass) / previous pass done with the staged rows and red
+        {   // the G x 32 parameter rows of this pass are contiguous in memory: the whole block stages them with
+            // coalesced loads (instead of one warp reading 4 n_m strided values per lane while the others wait)
+            const long long r0 = (long long)base * 32 * P, r1 = min((long long)(base + G) * 32, (long long)n_w) * P;
+            for (long long i = r0 + threadIdx.x + threadIdx.y * 32; i < r1; i += 32 * blockDim.y) tfs_all[i - r0] = params[i];
         }
         __syncthreads();
+        const double *row = tfs_all + ((size_t)gslot * 32 + (valid ? lane : 0)) * P; // rows of lanes past n_w: lane 0's
+        const WalkerConst c = standin_consts(valid ? row : tfs_all + (size_t)gslot * 32 * P);
+        x.tc = c.tc; x.invD = c.invD; x.inv_fisco = c.inv_fisco; x.K = c.K;
+        x.phi0 = c.phi + 0.25 * kPi;
+        x.tfs = (valid ? row : tfs_all + (size_t)gslot * 32 * P) + 5;
         // x of the lowest-m mode = 2 f/(m_min f_ISCO) = 4 f * x_scale: above 1 somewhere in the warp -> taper needed
         const double x_scale = c.inv_fisco * (0.5 / (double)m_min);
         double dh = 0.0, hh = 0.0;
