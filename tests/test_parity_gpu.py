@@ -908,3 +908,30 @@ def test_module2_loop_with_reference_update(orc, torch_cuda):
     stop = binding.StopState(n_checks=30, tol=1.0)
     assert not binding.stop_converged(stop, float(st[0]))
     ctx.destroy()
+
+
+def test_pt_run_parity_full(orc, torch_cuda):
+    """ll_pt_run_full: three whole iterations on the full-grid likelihood (Module 1) with the counter-based
+    uniforms, against the oracle's loop: identical positions and acceptance counts."""
+    from oracle import sampler as sm
+    tc = torch_cuda
+    wl = wlm.make_workload(0)
+    d, run = oracle_setup_full(orc, wl)
+    ctx = make_ctx(wl)
+    g = wl.grid
+    ctx.set_data(g.n_f, g.k_min, g.df, dev(tc, d), dev(tc, wl.W))
+    n_t, n_w = 2, 32
+    x = wl.params[:n_t * n_w].reshape(n_t, n_w, -1).copy()
+    x[:, :, 5:] = wl.params[0, 5:]
+    ll = lambda rows: (run(rows, d)["logL"], {})
+    betas = np.array([1.0, 0.01])
+    lo, hi = _prior_box(wl, wl.params, 0.6)
+    logL = ll(x.reshape(n_t * n_w, -1))[0].reshape(n_t, n_w).copy()
+    gx, gl = dev(tc, x), dev(tc, logL)
+    acc_g = tc.zeros(n_t, dtype=tc.int64, device="cuda")
+    n_acc = sm.run(x, logL, betas, lo, hi, 5, 2.0, 194, 7, 3, ll)
+    ctx.pt_run(gx, gl, None, None, dev(tc, betas), dev(tc, lo), dev(tc, hi), 5, 194, 7, 3, n_accepted=acc_g, f_nodes=wl.f_nodes)
+    assert np.array_equal(gx.cpu().numpy(), x) and np.array_equal(acc_g.cpu().numpy(), n_acc) and n_acc.sum() > 10
+    err = np.abs(gl.cpu().numpy() - logL) / np.maximum(1.0, np.abs(logL))
+    assert err.max() <= 1e-6
+    ctx.destroy()
