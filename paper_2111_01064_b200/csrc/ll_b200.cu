@@ -698,7 +698,7 @@ int launch_het_standin1(ll_ctx *ctx, int64_t n_w, const double *params, double *
                         cudaStream_t st)
 {
     const int n_groups = ceil_div(n_w, 32), n_e = ctx->ht1.n_e;
-    constexpr int WY = 16;
+    constexpr int WY = LL_HET1_WY;
     const size_t smem = sizeof(double) * ((size_t)n_e * kHet1Stride + (size_t)WY * 192);
     static bool attr_set = false;
     if (!attr_set) {
@@ -716,7 +716,8 @@ int launch_het_standin1(ll_ctx *ctx, int64_t n_w, const double *params, double *
     const int max_blocks = ctx->sm_count * bps;
     int S = 1, grid = 1;
     double best = 1e300;
-    for (int s = 1; s <= WY; s <<= 1) {
+    for (int s = 1; s <= WY; ++s) {
+        if (WY % s) continue;
         if (s > 1 && n_e / s < 8) break;
         const int G = WY / s;
         const long long passes = ceil_div(n_groups, G);

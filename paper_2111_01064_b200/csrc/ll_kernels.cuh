@@ -2193,7 +2193,10 @@ struct Het1Table {
     int n_e, n_b;
 };
 
-__global__ void __launch_bounds__(512)
+#ifndef LL_HET1_WY
+#define LL_HET1_WY 16 // warps per block of the single-mode kernel (one block per SM shares the table copy)
+#endif
+__global__ void __launch_bounds__(32 * LL_HET1_WY)
 k_het_standin1(Het1Table T, StandinInfo si, const double *__restrict__ params, int P, int n_w, int n_groups, int S,
                const double *__restrict__ dd, double *__restrict__ logL, double *__restrict__ d_h,
                double *__restrict__ h_h)
