@@ -786,7 +786,7 @@ int launch_het_standin(ll_ctx *ctx, int64_t n_w, const double *params, double *l
 // =====================================================================================================
 extern "C" {
 
-int ll_abi_version(void) { return 1; }
+int ll_abi_version(void) { return 2; } // 2: ll_config.spline_bc, ll_standin_nodes band output, the SURVEY 8(f) entry points
 
 int ll_create(const ll_config *cfg, ll_ctx **out)
 {

@@ -39,7 +39,7 @@ def test_library_exports_every_declared_symbol(so_path):
     assert sorted(binding.SYMBOLS) == names
     for n in names:
         assert hasattr(lib, n), n
-    assert lib.ll_abi_version() == 1
+    assert lib.ll_abi_version() == 2
 
 
 def test_library_is_sm100a_only(so_path):
