@@ -86,9 +86,16 @@ struct ll_ctx {
     bool nodes_valid = false;
     std::vector<int> bstart_host;  // bin -> interval table of the current node set (host copy)
     long long nodes_version = 0;   // bumped whenever the node tables are rebuilt
-    DevBuf tile_tab;               // frequency-tile boundaries of the fused kernel [n_tiles + 1]
-    long long tile_key_version = -1;
-    int tile_key_TB = -1, tile_key_small = -1, tile_n = 0, tile2_off = 0, tile2_n = 0;
+    // frequency-tile boundaries of the fused kernels [n_tiles + 1] (+ the chunk boundaries of the two-stage finalize):
+    // one cached table per kind (0: uniform tiles, 1: small batches, tiles limited by the spline intervals they cross,
+    // 2: per-walker node grids, uniform), keyed by (data version, node-set version, TB)
+    struct TileCache {
+        DevBuf tab;
+        long long data_version = -1, nodes_version = -1;
+        int TB = -1, n = 0, off2 = 0, n2 = 0;
+    } tiles[3];
+    TileCache *tile_cur = nullptr; // the table of the call in progress
+    long long data_version = 0;    // bumped by every ll_set_data
     DevBuf part2;                  // chunk partials of the two-stage finalize
     DevBuf pw_x;                   // per-walker node grids: X [n_nodes][n_wp], then the effective bands [n_w][2]
     DevBuf node_tab; // doubles then ints
@@ -105,6 +112,13 @@ struct ll_ctx {
     DevBuf pt_u;                // ll_pt_run_*: the uniforms of one iteration
     DevBuf pt_y, pt_out, pt_in; // sampler step: proposals [n][P], (log L, <d|h>, <h|h>, (d-1) ln z) [4][n], inside flags
     DevBuf ref_idx, ref_dense, ref_edges; // ll_het_refresh_standin: argmax slot, h0 on the grid, h0 and f at the edges
+    // launch shapes of the heterodyne kernels, per context (the shared-memory opt-in is per device, the
+    // grid depends on this device's SM count)
+    bool het1_attr = false, hetn_attr = false, heta_attr = false;
+    size_t het1_bps_smem = 0;
+    int het1_bps = 0;
+    long long hetn_key_groups = -1;
+    int hetn_key_total = -1, hetn_S = 1, hetn_grid = 1;
     HetTable ht{};
     Het1Table ht1{}; // single-mode regrouped table (k_het_standin1); base == nullptr when not built
     std::vector<double> raw_host; // [n_b][13]
@@ -309,8 +323,11 @@ constexpr int kTileChunk = 64;
 int ensure_tiles(ll_ctx *ctx, FullPlan &pl, cudaStream_t st, bool uniform = false)
 {
     const int small = uniform ? 2 : (pl.n_wp <= 1024 ? 1 : 0); // 2: per-walker node grids, no shared interval table
-    if (ctx->tile_key_version == ctx->nodes_version && ctx->tile_key_TB == pl.TB && ctx->tile_key_small == small) {
-        pl.n_tiles = ctx->tile_n;
+    ll_ctx::TileCache &tc = ctx->tiles[small];
+    ctx->tile_cur = &tc;
+    // kinds 0 and 2 depend on the grid only; kind 1 also on the node set (its interval table)
+    if (tc.data_version == ctx->data_version && tc.TB == pl.TB && (small != 1 || tc.nodes_version == ctx->nodes_version)) {
+        pl.n_tiles = tc.n;
         return LL_OK;
     }
     const int n_f = (int)ctx->n_f, n = (int)ctx->bstart_host.size();
@@ -340,17 +357,18 @@ int ensure_tiles(ll_ctx *ctx, FullPlan &pl, cudaStream_t st, bool uniform = fals
     ts.push_back(n_f);
     pl.n_tiles = (int)ts.size() - 1;
     // chunk boundaries for the two-stage finalize of small batches: tile_start2[z] = tile_start[z * kTileChunk]
-    ctx->tile2_off = (int)ts.size();
-    ctx->tile2_n = ceil_div(pl.n_tiles, kTileChunk);
-    for (int z = 0; z < ctx->tile2_n; ++z) ts.push_back(ts[(size_t)z * kTileChunk]);
+    tc.off2 = (int)ts.size();
+    tc.n2 = ceil_div(pl.n_tiles, kTileChunk);
+    for (int z = 0; z < tc.n2; ++z) ts.push_back(ts[(size_t)z * kTileChunk]);
     ts.push_back(n_f);
-    CK(ctx->tile_tab.ensure(sizeof(int) * ts.size()));
-    CK(cudaMemcpyAsync(ctx->tile_tab.p, ts.data(), sizeof(int) * ts.size(), cudaMemcpyHostToDevice, st));
+    tc.data_version = -1; // not valid until the copy below has been enqueued
+    CK(tc.tab.ensure(sizeof(int) * ts.size()));
+    CK(cudaMemcpyAsync(tc.tab.p, ts.data(), sizeof(int) * ts.size(), cudaMemcpyHostToDevice, st));
     CK(cudaStreamSynchronize(st)); // ts goes out of scope
-    ctx->tile_key_version = ctx->nodes_version;
-    ctx->tile_key_TB = pl.TB;
-    ctx->tile_key_small = small;
-    ctx->tile_n = pl.n_tiles;
+    tc.data_version = ctx->data_version;
+    tc.nodes_version = ctx->nodes_version;
+    tc.TB = pl.TB;
+    tc.n = pl.n_tiles;
     return LL_OK;
 }
 
@@ -439,7 +457,7 @@ int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, cons
     fa.xj = ctx->nt.xj; fa.bstart = ctx->nt.bstart; fa.ilo = ctx->ilo_s.as<int>(); fa.ihi = ctx->ihi_s.as<int>();
     fa.part = ctx->part.as<double>(); fa.k_min = ctx->k_min; fa.df = ctx->df; fa.n_f = (int)ctx->n_f; fa.n_wp = n_wp;
     fa.n_nodes = n_nodes; fa.n_m = n_m; fa.TB = pl.TB; fa.CH = pl.CH;
-    fa.tile_start = ctx->tile_tab.as<int>();
+    fa.tile_start = ctx->tile_cur->tab.as<int>();
     if (template_only) {
         // sorted position of walker 0 of a one-walker batch is 0
         k_full_template<<<ceil_div(ctx->n_f, 256), 256, 0, st>>>(fa, 0, h_out);
@@ -463,11 +481,11 @@ int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, cons
         ctx->last_n_blocks = (int)(grid.x * grid.y);
     }
     const double *fin_part = ctx->part.as<double>();
-    const int *fin_tiles = ctx->tile_tab.as<int>();
+    const int *fin_tiles = ctx->tile_cur->tab.as<int>();
     int fin_n = pl.n_tiles;
     if (n_wp <= 1024 && pl.n_tiles >= 8 * kTileChunk) { // thousands of tiles, a handful of walker blocks: two stages
-        CK(ctx->part2.ensure(sizeof(double) * (size_t)ctx->tile2_n * NQ * n_wp));
-        dim3 grid(ceil_div(n_wp, 32), ctx->tile2_n);
+        CK(ctx->part2.ensure(sizeof(double) * (size_t)ctx->tile_cur->n2 * NQ * n_wp));
+        dim3 grid(ceil_div(n_wp, 32), ctx->tile_cur->n2);
         if (NQ == 5)
             k_reduce_tiles<5><<<grid, dim3(32, 32), 0, st>>>(fin_part, ctx->ilo_s.as<int>(), ctx->ihi_s.as<int>(), n_wp, fin_tiles,
                                                             fin_n, kTileChunk, ctx->part2.as<double>());
@@ -476,8 +494,8 @@ int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, cons
                                                             fin_n, kTileChunk, ctx->part2.as<double>());
         LAUNCHED(ctx);
         fin_part = ctx->part2.as<double>();
-        fin_tiles = ctx->tile_tab.as<int>() + ctx->tile2_off;
-        fin_n = ctx->tile2_n;
+        fin_tiles = ctx->tile_cur->tab.as<int>() + ctx->tile_cur->off2;
+        fin_n = ctx->tile_cur->n2;
     }
     if (nm1 && !tfp)
         k_finalize<1><<<ceil_div(n_wp, 32), dim3(32, kFinY), 0, st>>>(fin_part, ctx->TF.as<double>(), ctx->perm.as<int>(),
@@ -556,7 +574,7 @@ int run_full_pw(ll_ctx *ctx, long long n_w, int n_nodes, const double *f_nodes_w
     fa.xj = nullptr; fa.bstart = nullptr; fa.ilo = ctx->ilo_s.as<int>(); fa.ihi = ctx->ihi_s.as<int>();
     fa.part = ctx->part.as<double>(); fa.k_min = ctx->k_min; fa.df = ctx->df; fa.n_f = (int)ctx->n_f; fa.n_wp = n_wp;
     fa.n_nodes = n_nodes; fa.n_m = n_m; fa.TB = pl.TB; fa.CH = pl.CH;
-    fa.tile_start = ctx->tile_tab.as<int>();
+    fa.tile_start = ctx->tile_cur->tab.as<int>();
     {
         dim3 grid(n_wp / pl.WB, pl.n_tiles);
         const size_t smem = (size_t)2 * pl.CH * 40;
@@ -568,7 +586,7 @@ int run_full_pw(ll_ctx *ctx, long long n_w, int n_nodes, const double *f_nodes_w
     }
     k_finalize<0><<<ceil_div(n_wp, 32), dim3(32, kFinY), 0, st>>>(ctx->part.as<double>(), ctx->TF.as<double>(), ctx->perm.as<int>(),
                                                                  ctx->ilo_s.as<int>(), ctx->ihi_s.as<int>(), n_wp,
-                                                                 ctx->tile_tab.as<int>(), pl.n_tiles, ctx->dd.as<double>(), logL,
+                                                                 ctx->tile_cur->tab.as<int>(), pl.n_tiles, ctx->dd.as<double>(), logL,
                                                                  d_h, h_h);
     LAUNCHED(ctx);
     return LL_OK;
@@ -700,20 +718,18 @@ int launch_het_standin1(ll_ctx *ctx, int64_t n_w, const double *params, double *
     const int n_groups = ceil_div(n_w, 32), n_e = ctx->ht1.n_e;
     constexpr int WY = LL_HET1_WY;
     const size_t smem = sizeof(double) * ((size_t)n_e * kHet1Stride + (size_t)WY * 192);
-    static bool attr_set = false;
-    if (!attr_set) {
+    if (!ctx->het1_attr) {
         CK(cudaFuncSetAttribute(k_het_standin1, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
-        attr_set = true;
+        ctx->het1_attr = true;
     }
     if (smem > 227 * 1024) return ctx->fail(LL_ERR_UNSUPPORTED, "heterodyne tables exceed shared memory (too many bins)");
-    static size_t bps_smem = 0;
-    static int bps = 0;
-    if (bps == 0 || bps_smem != smem) {
+    if (ctx->het1_bps == 0 || ctx->het1_bps_smem != smem) {
+        int bps = 0;
         CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, k_het_standin1, 32 * WY, smem));
-        bps = std::max(1, bps);
-        bps_smem = smem;
+        ctx->het1_bps = std::max(1, bps);
+        ctx->het1_bps_smem = smem;
     }
-    const int max_blocks = ctx->sm_count * bps;
+    const int max_blocks = ctx->sm_count * ctx->het1_bps;
     int S = 1, grid = 1;
     double best = 1e300;
     for (int s = 1; s <= WY; ++s) {
@@ -741,17 +757,15 @@ int launch_het_standin(ll_ctx *ctx, int64_t n_w, const double *params, double *l
     constexpr int WY = LL_HET_WY; // warps per block, all sharing one table copy
     // table + [WY][2][32] segment partials + -(m/pi) + the staged parameter rows of the G = WY/S walker groups
     auto smem_of = [&](int s) { return sizeof(double) * ((size_t)ctx->ht.total + (size_t)WY * 64 + 8 + (size_t)(WY / s) * 32 * (5 + 4 * NM)); };
-    static bool attr_set = false;
-    if (!attr_set) {
+    if (!ctx->hetn_attr) { // a context has one n_modes, so one instantiation
         CK(cudaFuncSetAttribute(k_het_standin<NM>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
-        attr_set = true;
+        ctx->hetn_attr = true;
     }
     if (smem_of(WY) > 227 * 1024) return ctx->fail(LL_ERR_UNSUPPORTED, "heterodyne tables exceed shared memory (too many bins x modes)");
     // S = frequency segments per walker group (G = WY/S groups per block pass): pick the split whose busiest SM
     // has the least work, work = resident blocks x passes per block x warp-edges per pass
-    static long long key_groups = -1; // decision cached per (batch size, table size)
-    static int key_total = -1, S = 1, grid = 1;
-    if (key_groups != n_groups || key_total != ctx->ht.total) {
+    int &S = ctx->hetn_S, &grid = ctx->hetn_grid; // decision cached per (batch size, table size)
+    if (ctx->hetn_key_groups != n_groups || ctx->hetn_key_total != ctx->ht.total) {
         double best = 1e300;
         for (int s = 1; s <= WY; ++s) {
             if (WY % s) continue;
@@ -767,8 +781,8 @@ int launch_het_standin(ll_ctx *ctx, int64_t n_w, const double *params, double *l
             if (work < best * 0.999) { best = work; S = s; grid = gr; }
         }
         if (best == 1e300) { S = WY; grid = (int)std::min<long long>(n_groups, ctx->sm_count); }
-        key_groups = n_groups;
-        key_total = ctx->ht.total;
+        ctx->hetn_key_groups = n_groups;
+        ctx->hetn_key_total = ctx->ht.total;
     }
     const size_t smem = smem_of(S);
     const int P = 5 + 2 * kNC * ctx->n_m;
@@ -836,7 +850,7 @@ int ll_destroy(ll_ctx *ctx)
                          &ctx->key_w, &ctx->hist, &ctx->perm, &ctx->ilo_s, &ctx->ihi_s, &ctx->Y, &ctx->C, &ctx->TF,
                          &ctx->part, &ctx->prow, &ctx->het_tab, &ctx->het_tab1, &ctx->het_raw, &ctx->het_idx, &ctx->het_fb,
                          &ctx->stage_in, &ctx->stage_out, &ctx->g4f, &ctx->Wf, &ctx->scale, &ctx->wmax, &ctx->ref_idx,
-                         &ctx->ref_dense, &ctx->ref_edges, &ctx->tile_tab, &ctx->part2, &ctx->pw_x, &ctx->pt_y, &ctx->pt_out, &ctx->pt_in, &ctx->pt_u};
+                         &ctx->ref_dense, &ctx->ref_edges, &ctx->tiles[0].tab, &ctx->tiles[1].tab, &ctx->tiles[2].tab, &ctx->part2, &ctx->pw_x, &ctx->pt_y, &ctx->pt_out, &ctx->pt_in, &ctx->pt_u};
         for (DevBuf *b : all) b->release();
         for (auto &e : ctx->ev) cudaEventDestroy(e);
     }
@@ -860,6 +874,7 @@ int ll_set_data(ll_ctx *ctx, int64_t n_f, int64_t k_min, double df, const double
     ctx->have_data = false;
     ctx->have_het = false;
     ctx->nodes_valid = false;
+    ctx->data_version += 1; // the cached frequency-tile tables and the bin -> interval table belong to the old grid
     const long long n_pad = round_up(n_f, 512);
     CK(ctx->g4.ensure(sizeof(double) * 4 * n_pad));
     CK(ctx->Wd.ensure(sizeof(double) * n_pad));
@@ -1263,10 +1278,9 @@ int ll_het_batch(ll_ctx *ctx, int64_t n_w, const double *amp_e, const double *ph
     DeviceGuard dg(ctx->device);
     const size_t smem = sizeof(double) * (size_t)ctx->ht.total;
     if (smem > 227 * 1024) return ctx->fail(LL_ERR_UNSUPPORTED, "heterodyne tables exceed shared memory");
-    static bool attr_set = false;
-    if (!attr_set) {
+    if (!ctx->heta_attr) {
         CK(cudaFuncSetAttribute(k_het_arrays, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
-        attr_set = true;
+        ctx->heta_attr = true;
     }
     const int wpb = 8;
     int blocks_per_sm = std::max(1, std::min(8, (int)((220 * 1024) / std::max<size_t>(smem, 1))));

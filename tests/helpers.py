@@ -19,6 +19,26 @@ def assert_close_ll(got, ref, what=""):
                           f"at {int(err.argmax())} (ref {ref[err.argmax()]:.6e})"
 
 
+def dev(torch, a):
+    return torch.as_tensor(np.ascontiguousarray(a, dtype=np.float64), device="cuda")
+
+
+def make_ctx(wl, precision=0):
+    from paper_2111_01064_b200 import binding
+    ctx = binding.Context(n_modes=wl.n_m, precision=precision, n_channels=wl.n_c)
+    ctx.standin_config(wl.modes_l, wl.modes_m, wl.c_lm, wl.kappa)
+    return ctx
+
+
+def check_triplet(got, ref, what):
+    """log L at the north_star bar; d_h and h_h separately at 1e-6 max(1, |h_h|) so that a cancelling pair cannot hide"""
+    logL, d_h, h_h = (x.cpu().numpy() for x in got)
+    assert_close_ll(logL, ref["logL"], what + " logL")
+    scale = np.maximum(1.0, np.abs(ref["h_h"]))
+    assert np.all(np.abs(d_h - ref["d_h"]) <= 1e-6 * np.maximum(scale, np.abs(ref["d_h"]))), what + " d_h"
+    assert np.all(np.abs(h_h - ref["h_h"]) <= 1e-6 * scale), what + " h_h"
+
+
 def oracle_setup_full(orc, wl: wlm.Workload):
     g = wl.grid
     run = lambda params, d, tmpl=False: orc.full_batch_standin(

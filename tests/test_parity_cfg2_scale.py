@@ -1,0 +1,177 @@
+"""GPU parity tests (-m gpu) at BASELINE.json config 2's FULL size for every full-grid kernel bench.py times there
+(`per_config.cfg2`, `cfg2_tf`, `cfg2_pw`, `cfg2_hm6`, `module1_iteration`): the one-year grid (1 574 725 bins), 1024
+nodes, LISA-scale phases (up to ~1e7 rad, several quarter cycles per bin), the launch configuration of the bench, and
+the oracle recomputing sampled walkers one by one.  Each of those kernels carries its own copy of the rotation
+recurrence (ll_kernels.cuh), so each needs its own test at this scale.
+
+Tolerance (BASELINE.json north_star): |delta log L| <= 1e-6 max(1, |log L|), d_h and h_h separately
+at 1e-6 max(1, |h_h|).  Inputs: the seeded config-2 workload (workloads.py), completed with the oracle (helpers.py);
+node arrays for the array entry points come from a numpy generator in this file, never from the CUDA path.
+"""
+import numpy as np
+import pytest
+
+from paper_2111_01064_b200 import workloads as wlm
+from helpers import check_triplet, dev, make_ctx, oracle_setup_full
+
+pytestmark = pytest.mark.gpu
+
+
+def _np_triplet(got, idx):
+    import torch
+    return [torch.as_tensor(x[idx]) for x in got]
+
+
+def sample_walkers(n_w, fis, extra=(), stride=None, wb=128):
+    """walker 0, min / max f_ISCO (shortest / longest band), walker-block boundaries of the launch, every `stride`-th"""
+    s = {0, 1, int(fis.argmin()), int(fis.argmax()), wb - 1, wb, n_w - wb - 1, n_w - wb, n_w - 1} | set(extra)
+    if stride:
+        s |= set(range(stride // 3, n_w, stride))
+    return np.array(sorted(i for i in s if 0 <= i < n_w))
+
+
+def lisa_node_arrays(params, x, kappa=wlm.KAPPA):
+    """INPUT GENERATOR for the array entry points (ll_full_batch / _tf / _pw take whatever amplitude and phase they are
+    given): smooth node arrays with the magnitude and the phase scale of a LISA massive-black-hole binary — amplitude
+    ~ f^(-7/6)/D rolled off above a walker-dependent frequency, phase 2 pi f t_c + K f^(-5/3) + const reaching ~1e7
+    rad — at the nodes x [n_w][n_nodes] (or [n_nodes]).  numpy float64; both the oracle and the library get these arrays."""
+    x = np.broadcast_to(np.asarray(x, dtype=np.float64), (params.shape[0], np.shape(x)[-1]))
+    mc, q, tc, phic, inv_d = (params[:, k][:, None] for k in range(5))
+    eta = q / (1.0 + q) ** 2
+    mtot = mc * eta ** -0.6
+    f_roll = 6.0 ** -1.5 / (np.pi * mtot)
+    s = np.clip((1.0 + kappa - x / f_roll) / kappa, 0.0, 1.0)
+    amp = x ** (-7.0 / 6.0) * inv_d * s ** 3 * (10.0 - 15.0 * s + 6.0 * s * s)
+    phase = 2.0 * np.pi * x * tc - phic - 0.25 * np.pi + 3.0 / (128.0 * eta) * (np.pi * mtot * x) ** (-5.0 / 3.0)
+    band_top = np.minimum((1.0 + kappa) * f_roll[:, 0], wlm.F_HI)
+    return np.ascontiguousarray(amp[:, None, :]), np.ascontiguousarray(phase[:, None, :]), band_top
+
+
+@pytest.fixture(scope="module")
+def cfg2(orc, torch_cuda):
+    wl = wlm.make_workload(2)
+    d, run = oracle_setup_full(orc, wl)
+    ctx = make_ctx(wl)
+    g = wl.grid
+    ctx.set_data(g.n_f, g.k_min, g.df, dev(torch_cuda, d), dev(torch_cuda, wl.W))
+    fis = np.array([orc.standin_fisco(p) for p in wl.params])
+    yield wl, d, run, ctx, fis
+    ctx.destroy()
+
+
+def test_cfg2_full_size_128_walkers(cfg2, torch_cuda):
+    """k_full_fused<1> (bench headline, per_config.cfg2): >= 128 sampled walkers of the full 16384-walker batch
+    against the oracle (BASELINE.md §3 planned a 512-walker subset; the oracle does ~38 walkers/s on 16 cores)."""
+    wl, d, run, ctx, fis = cfg2
+    got = [x.cpu().numpy() for x in ctx.full_batch_standin(wl.f_nodes, dev(torch_cuda, wl.params))]
+    sample = sample_walkers(wl.n_w, fis, stride=128)
+    assert len(sample) >= 128
+    ref = run(wl.params[sample], d)
+    check_triplet(_np_triplet(got, sample), ref, "cfg2 full size, 128+ walkers")
+
+
+@pytest.mark.parametrize("n_small", [37, 160, 320])
+def test_module1_sized_batches_against_oracle(cfg2, torch_cuda, n_small):
+    """Module-1 sized batches on the one-year grid (80 walkers x 4 temperatures; a half update is 160
+    proposals, a whole population 320): the small-batch route (per_config.module1_iteration) against the ORACLE, not
+    only against the large-batch route."""
+    wl, d, run, ctx, fis = cfg2
+    rng = np.random.default_rng(194 + n_small)
+    idx = rng.choice(wl.n_w, n_small, replace=False)
+    idx[0] = 0                                              # the injection: log L ~ -n_f (noise), <d|h> = 2.5e5
+    params = wl.params[idx]
+    got = [x.cpu().numpy() for x in ctx.full_batch_standin(wl.f_nodes, dev(torch_cuda, params))]
+    sample = np.arange(n_small) if n_small <= 40 else np.unique(np.r_[0, 31, 32, n_small - 1, rng.integers(0, n_small, 36)])
+    ref = run(params[sample], d)
+    check_triplet(_np_triplet(got, sample), ref, f"module-1 sized batch of {n_small}")
+
+
+def _smooth_tf_at_nodes(params, f_nodes, n_c=2):
+    """smooth complex T^c(f_j) per walker (the response's formula is in the paper's ref. [44], not in PAPER.md):
+    the walker's constant factor times (1 + 0.2 x) e^{2 i x}(1 + 0.1 sin(5 x + phi_c)), x = log-frequency in [0, 1]"""
+    x = np.log(f_nodes / f_nodes[0]) / np.log(f_nodes[-1] / f_nodes[0])
+    n_w = params.shape[0]
+    t0 = params[:, 5:5 + 2 * n_c].reshape(n_w, 1, n_c, 1, 2)
+    mod = (1.0 + 0.2 * x)[None, :] * (1.0 + 0.1 * np.sin(5.0 * x[None, :] + params[:, 3:4]))
+    cr, ci = (mod * np.cos(2.0 * x))[:, None, None, :], (mod * np.sin(2.0 * x))[:, None, None, :]
+    out = np.stack([t0[..., 0] * cr - t0[..., 1] * ci, t0[..., 0] * ci + t0[..., 1] * cr], axis=-1)
+    return np.ascontiguousarray(out)
+
+
+def test_cfg2_tf_full_size_sampled(cfg2, orc, torch_cuda):
+    """k_full_fused_tf<1> (per_config.cfg2_tf): frequency-dependent transfer function (Eq. 8-9) on the full
+    16384-walker batch, one-year grid, LISA-scale phases, the walkers' own bands; 18 sampled walkers vs oracle.full_batch_tf."""
+    wl, d, run, ctx, fis = cfg2
+    amp, ph, top = lisa_node_arrays(wl.params, wl.f_nodes)
+    tfn = _smooth_tf_at_nodes(wl.params, wl.f_nodes)
+    g = wl.grid
+    band = np.ascontiguousarray(np.stack([np.full(wl.n_w, g.k_min * g.df), top], axis=1))
+    tc = torch_cuda
+    got = [x.cpu().numpy() for x in ctx.full_batch_tf(wl.f_nodes, dev(tc, amp), dev(tc, ph), dev(tc, tfn), dev(tc, band))]
+    sample = sample_walkers(wl.n_w, fis, stride=2048)
+    assert len(sample) >= 16
+    ref = orc.full_batch_tf(wl.f_nodes, amp[sample], ph[sample], tfn[sample], band[sample], g.k_min, g.df, d, wl.W)
+    assert np.abs(ph).max() > 5e6                          # LISA-scale phases (2 pi f t_c at 0.05 Hz, t_c ~ 0.9 yr)
+    check_triplet(_np_triplet(got, sample), ref, "cfg2 tf sampled")
+    assert np.all(np.isfinite(got[0]))
+
+
+def test_cfg2_pw_full_size_sampled(cfg2, orc, torch_cuda):
+    """k_full_fused_pw<1> (per_config.cfg2_pw): per-walker node grids on the full 16384-walker batch.  Even walkers
+    carry a copy of the shared 1024 nodes, odd walkers 1024 log-spaced nodes over their OWN span (starting above the
+    grid's first bin, ending near their band top), so lanes of one warp sit in different intervals of different
+    widths; 20 sampled walkers vs oracle.per_walker.full_batch_pw."""
+    from oracle import per_walker as pw
+    wl, d, run, ctx, fis = cfg2
+    g = wl.grid
+    rng = np.random.default_rng(30)
+    _, _, top = lisa_node_arrays(wl.params, wl.f_nodes)
+    x = np.tile(wl.f_nodes, (wl.n_w, 1))
+    odd = np.arange(1, wl.n_w, 2)
+    lo = wlm.F_LO * rng.uniform(1.0, 3.0, len(odd))
+    hi = np.minimum(top[odd] * rng.uniform(0.7, 1.1, len(odd)), wlm.F_HI)
+    t = np.linspace(0.0, 1.0, len(wl.f_nodes))
+    x[odd] = np.exp(np.log(lo)[:, None] + (np.log(hi) - np.log(lo))[:, None] * t[None, :])
+    x[odd, 0], x[odd, -1] = lo, hi
+    amp, ph, _ = lisa_node_arrays(wl.params, x)
+    tf = np.ascontiguousarray(wl.params[:, 5:9].reshape(wl.n_w, 1, 2, 2))
+    band = np.ascontiguousarray(np.stack([np.full(wl.n_w, g.k_min * g.df), top], axis=1))
+    tc = torch_cuda
+    got = [v.cpu().numpy() for v in ctx.full_batch_pw(dev(tc, x), dev(tc, amp), dev(tc, ph), dev(tc, tf), dev(tc, band))]
+    sample = sample_walkers(wl.n_w, fis, extra=(2, 3, 4097, 4098), stride=2048)
+    assert len(sample) >= 16 and (sample % 2 == 1).sum() >= 6 and (sample % 2 == 0).sum() >= 6
+    ref = pw.full_batch_pw(x[sample], amp[sample], ph[sample], tf[sample], band[sample], g.k_min, g.df, d, wl.W)
+    check_triplet(_np_triplet(got, sample), ref, "cfg2 per-walker nodes sampled")
+    assert np.all(np.isfinite(got[0]))
+
+
+def test_cfg2_hm6_full_size_sampled(orc, torch_cuda):
+    """k_full_fused<0> (per_config.cfg2_hm6): config 3's six modes through the FULL-GRID path on config 2's one-year
+    grid and 1024 nodes, 2048 prior-draw walkers (the bench's batch); data = walker 0's six-mode template + noise;
+    16 sampled walkers vs the oracle."""
+    n_w = 2048
+    wl6, wl2 = wlm.make_workload(3, n_w=8), wlm.make_workload(2, n_w=n_w)
+    rng = np.random.default_rng(wlm.SEED_BASE + 232)
+    params = np.empty((n_w, 5 + 4 * wl6.n_m))
+    params[:, :5] = wl2.params[:, :5]
+    ang = rng.uniform(0, 2 * np.pi, (n_w, 2 * wl6.n_m))
+    params[:, 5::2], params[:, 6::2] = np.cos(ang), np.sin(ang)
+    g = wl2.grid
+    run = lambda p, dd, t=False: orc.full_batch_standin(wl6.modes_m, wl6.c_lm, wl6.kappa, p, wl2.f_nodes, g.k_min, g.df,
+                                                        g.n_f, dd, wl2.W, want_template=t)
+    hh = run(params[:1], None)["h_h"][0]
+    params[:, 4] *= wlm.SNR_TARGET / np.sqrt(hh)            # walker 0 at SNR 500 (reading R18)
+    d = run(params[:1], None, True)["h"] + wl2.noise
+    from paper_2111_01064_b200 import binding
+    ctx = binding.Context(n_modes=wl6.n_m)
+    ctx.standin_config(wl6.modes_l, wl6.modes_m, wl6.c_lm, wl6.kappa)
+    tc = torch_cuda
+    ctx.set_data(g.n_f, g.k_min, g.df, dev(tc, d), dev(tc, wl2.W))
+    got = [x.cpu().numpy() for x in ctx.full_batch_standin(wl2.f_nodes, dev(tc, params))]
+    fis = np.array([orc.standin_fisco(p) for p in params])
+    sample = sample_walkers(n_w, fis, stride=256, wb=64)
+    assert len(sample) >= 16
+    ref = run(params[sample], d)
+    check_triplet(_np_triplet(got, sample), ref, "cfg2 six modes sampled")
+    assert abs(np.sqrt(got[2][0]) - 500.0) < 1e-3
+    ctx.destroy()

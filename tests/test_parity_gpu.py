@@ -7,36 +7,10 @@ import numpy as np
 import pytest
 
 from paper_2111_01064_b200 import workloads as wlm
-from helpers import (assert_close_ll, oracle_setup_full, oracle_setup_het, rand_smooth_nodes, tol_ll, unit_tf)
+from helpers import (assert_close_ll, check_triplet, dev, make_ctx, oracle_setup_full, oracle_setup_het, rand_smooth_nodes,
+                     tol_ll, unit_tf)
 
 pytestmark = pytest.mark.gpu
-
-
-@pytest.fixture(scope="module")
-def torch_cuda():
-    import torch
-    if not torch.cuda.is_available():
-        pytest.fail("GPU tests need a CUDA device; there is no CPU fallback to test instead")
-    return torch
-
-
-def dev(torch, a):
-    return torch.as_tensor(np.ascontiguousarray(a, dtype=np.float64), device="cuda")
-
-
-def make_ctx(wl, precision=0):
-    from paper_2111_01064_b200 import binding
-    ctx = binding.Context(n_modes=wl.n_m, precision=precision)
-    ctx.standin_config(wl.modes_l, wl.modes_m, wl.c_lm, wl.kappa)
-    return ctx
-
-
-def check_triplet(got, ref, what):
-    logL, d_h, h_h = (x.cpu().numpy() for x in got)
-    assert_close_ll(logL, ref["logL"], what + " logL")
-    scale = np.maximum(1.0, np.abs(ref["h_h"]))
-    assert np.all(np.abs(d_h - ref["d_h"]) <= 1e-6 * np.maximum(scale, np.abs(ref["d_h"]))), what + " d_h"
-    assert np.all(np.abs(h_h - ref["h_h"]) <= 1e-6 * scale), what + " h_h"
 
 
 # ------------------------------------------------------------------------------------------- full grid
@@ -743,6 +717,32 @@ def test_full_per_walker_nodes(orc, torch_cuda, n_m, banded, n_w, n_nodes):
     for u, v in zip(a, b):
         un, vn = u.cpu().numpy(), v.cpu().numpy()
         assert np.all(np.abs(un - vn) <= 1e-9 * np.maximum(1.0, np.abs(vn)))
+    ctx.destroy()
+
+
+def test_set_data_again_invalidates_cached_tiles(orc, torch_cuda):
+    """ll_set_data "may be called again at any time" (include/ll.h): a second data stream with MORE bins in the same
+    tile-size bucket must not reuse the frequency-tile table of the first (the per-walker path never rebuilds the node
+    tables, so nothing else would invalidate it), and alternating per-walker and shared-node calls must stay right."""
+    from oracle import per_walker as pw
+    from paper_2111_01064_b200 import binding
+    from helpers import pw_case
+    tc = torch_cuda
+    rng = np.random.default_rng(312)
+    k_min, df, n_w, n_nodes = 40, 1e-5, 40, 33
+    ctx = binding.Context(n_modes=1)
+    for n_f in (3000, 5000, 4000):
+        f, x, amp, ph, tf, W, d = pw_case(rng, n_w, 1, n_nodes, n_f, k_min, df)
+        ctx.set_data(n_f, k_min, df, dev(tc, d), dev(tc, W))
+        got = ctx.full_batch_pw(dev(tc, x), dev(tc, amp), dev(tc, ph), dev(tc, tf))
+        ref = pw.full_batch_pw(x, amp, ph, tf, None, k_min, df, d, W)
+        check_triplet(got, ref, f"per-walker nodes after set_data(n_f={n_f})")
+        xs = np.geomspace(f[0] * 0.9, f[-1] * 1.05, n_nodes)
+        got = ctx.full_batch(xs, dev(tc, amp), dev(tc, ph), dev(tc, tf))
+        ref = orc.full_batch(xs, amp, ph, tf, None, k_min, df, d, W)
+        check_triplet(got, ref, f"shared nodes after set_data(n_f={n_f})")
+        got = ctx.full_batch_pw(dev(tc, x), dev(tc, amp), dev(tc, ph), dev(tc, tf))
+        check_triplet(got, pw.full_batch_pw(x, amp, ph, tf, None, k_min, df, d, W), "per-walker nodes, alternating")
     ctx.destroy()
 
 
