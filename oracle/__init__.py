@@ -99,10 +99,26 @@ def standin_fisco(p) -> float:
     return out.value
 
 
-def standin_nodes(params, mode_m, c_lm, kappa, f, f_grid_lo, f_grid_hi, n_c=2):
-    """-> amp, phase [n_w][n_m][n_freq], tf [n_w][n_m][n_c][2], band [n_w][2]"""
+def _n_c_of(P: int, n_m: int) -> int:
+    n_c, rem = divmod(P - 5, 2 * n_m)
+    assert rem == 0 and n_c in (1, 2, 3), (P, n_m)
+    return n_c
+
+
+def _w_rows(W: np.ndarray, n_c: int) -> int:
+    """W [n_f]: one weight row for every channel; W [n_c][n_f]: one row per channel"""
+    if W.ndim == 1:
+        return 1
+    assert W.ndim == 2 and W.shape[0] == n_c, (W.shape, n_c)
+    return n_c
+
+
+def standin_nodes(params, mode_m, c_lm, kappa, f, f_grid_lo, f_grid_hi, n_c=None, split_tc=False):
+    """-> amp, phase [n_w][n_m][n_freq], tf [n_w][n_m][n_c][2], band [n_w][2]; n_c from the row length by default.
+    split_tc: the phase without its linear term 2 pi f t_c (pass t_shift = params[:, 2] alongside, reading R32)"""
     params, f, c_lm, mode_m = _f64(params), _f64(f), _f64(c_lm), _i32(mode_m)
     n_w, n_m, n = params.shape[0], len(mode_m), len(f)
+    n_c = _n_c_of(params.shape[1], n_m) if n_c is None else n_c
     assert params.shape[1] == 5 + 2 * n_c * n_m
     amp = np.empty((n_w, n_m, n))
     phase = np.empty((n_w, n_m, n))
@@ -110,15 +126,16 @@ def standin_nodes(params, mode_m, c_lm, kappa, f, f_grid_lo, f_grid_hi, n_c=2):
     band = np.empty((n_w, 2))
     _check(lib().orc_standin_nodes(C.c_int64(n_w), C.c_int(n_m), C.c_int(n_c), _p(mode_m, np.int32), _p(c_lm),
                                    C.c_double(kappa), _p(params), C.c_int(n), _p(f),
-                                   C.c_double(f_grid_lo), C.c_double(f_grid_hi),
+                                   C.c_double(f_grid_lo), C.c_double(f_grid_hi), C.c_int(1 if split_tc else 0),
                                    _p(amp), _p(phase), _p(tf), _p(band)), "standin_nodes")
     return amp, phase, tf, band
 
 
-def standin_direct(p, mode_m, c_lm, kappa, f, f_lo, f_hi, n_c=2) -> np.ndarray:
+def standin_direct(p, mode_m, c_lm, kappa, f, f_lo, f_hi, n_c=None) -> np.ndarray:
     """stand-in template of ONE parameter row evaluated directly at f: [n_c][n_freq][2]"""
     p, f, c_lm, mode_m = _f64(p), _f64(f), _f64(c_lm), _i32(mode_m)
     n_m = len(mode_m)
+    n_c = _n_c_of(p.shape[0], n_m) if n_c is None else n_c
     assert p.shape == (5 + 2 * n_c * n_m,)
     h = np.empty((n_c, len(f), 2))
     _check(lib().orc_standin_direct(C.c_int(n_m), C.c_int(n_c), _p(mode_m, np.int32), _p(c_lm), C.c_double(kappa),
@@ -131,7 +148,8 @@ def standin_direct(p, mode_m, c_lm, kappa, f, f_lo, f_hi, n_c=2) -> np.ndarray:
 def dd(d, W) -> float:
     d, W = _f64(d), _f64(W)
     out = C.c_double()
-    _check(lib().orc_dd(C.c_int(d.shape[0]), C.c_int64(d.shape[1]), _p(d), _p(W), C.byref(out)), "dd")
+    _check(lib().orc_dd(C.c_int(d.shape[0]), C.c_int64(d.shape[1]), _p(d), _p(W), C.c_int(_w_rows(W, d.shape[0])),
+                        C.byref(out)), "dd")
     return out.value
 
 
@@ -139,45 +157,52 @@ def inner(a, b, W) -> complex:
     """sum_c sum_k W_k conj(a_k) b_k; the real part is <a|b> (Eq. 3)."""
     a, b, W = _f64(a), _f64(b), _f64(W)
     re, im = C.c_double(), C.c_double()
-    _check(lib().orc_inner(C.c_int(a.shape[0]), C.c_int64(a.shape[1]), _p(a), _p(b), _p(W), C.byref(re), C.byref(im)),
-           "inner")
+    _check(lib().orc_inner(C.c_int(a.shape[0]), C.c_int64(a.shape[1]), _p(a), _p(b), _p(W),
+                           C.c_int(_w_rows(W, a.shape[0])), C.byref(re), C.byref(im)), "inner")
     return complex(re.value, im.value)
 
 
 # ------------------------------------------------------------------ full-grid path
-def full_batch(f_nodes, amp, phase, tf, band, k_min, df, d, W, want_template=False):
-    """-> dict(logL, d_h, h_h, logL_direct[, h]) for amp/phase [n_w][n_m][n_nodes]."""
+def full_batch(f_nodes, amp, phase, tf, band, k_min, df, d, W, want_template=False, t_shift=None):
+    """-> dict(logL, d_h, h_h, logL_direct[, h]) for amp/phase [n_w][n_m][n_nodes]; W [n_f] or [n_c][n_f];
+    t_shift [n_w] or None: Psi_m(f) = spline_m(f) + 2 pi f t_shift (reading R32)."""
     f_nodes, amp, phase, tf, W = _f64(f_nodes), _f64(amp), _f64(phase), _f64(tf), _f64(W)
     n_w, n_m, n_nodes = amp.shape
     n_c = tf.shape[2]
-    n_f = W.shape[0]
+    n_f = W.shape[-1]
+    t_shift = None if t_shift is None else _f64(t_shift)
+    assert t_shift is None or t_shift.shape == (n_w,)
     band = None if band is None else _f64(band)
     d = None if d is None else _f64(d)
     out = {k: np.empty(n_w) for k in ("logL", "d_h", "h_h", "logL_direct")}
     h = np.empty((n_c, n_f, 2)) if want_template else None
     _check(lib().orc_full_batch(C.c_int64(n_w), C.c_int(n_m), C.c_int(n_c), C.c_int(n_nodes), _p(f_nodes),
                                 _p(amp), _p(phase), _p(tf), _p(band), C.c_int64(n_f), C.c_int64(k_min),
-                                C.c_double(df), _p(d), _p(W), _p(out["logL"]), _p(out["d_h"]), _p(out["h_h"]),
+                                C.c_double(df), _p(d), _p(W), C.c_int(_w_rows(W, n_c)), _p(t_shift),
+                                _p(out["logL"]), _p(out["d_h"]), _p(out["h_h"]),
                                 _p(out["logL_direct"]), _p(h)), "full_batch")
     if want_template:
         out["h"] = h
     return out
 
 
-def full_batch_tf(f_nodes, amp, phase, tf_nodes, band, k_min, df, d, W, want_template=False):
+def full_batch_tf(f_nodes, amp, phase, tf_nodes, band, k_min, df, d, W, want_template=False, t_shift=None):
     """frequency-dependent transfer function T [n_w][n_m][n_c][n_nodes][2] splined alongside amp/phase (Eq. 8-9)."""
     f_nodes, amp, phase, tf_nodes, W = _f64(f_nodes), _f64(amp), _f64(phase), _f64(tf_nodes), _f64(W)
     n_w, n_m, n_nodes = amp.shape
     n_c = tf_nodes.shape[2]
     assert tf_nodes.shape == (n_w, n_m, n_c, n_nodes, 2)
-    n_f = W.shape[0]
+    n_f = W.shape[-1]
+    t_shift = None if t_shift is None else _f64(t_shift)
+    assert t_shift is None or t_shift.shape == (n_w,)
     band = None if band is None else _f64(band)
     d = None if d is None else _f64(d)
     out = {k: np.empty(n_w) for k in ("logL", "d_h", "h_h", "logL_direct")}
     h = np.empty((n_c, n_f, 2)) if want_template else None
     _check(lib().orc_full_batch_tf(C.c_int64(n_w), C.c_int(n_m), C.c_int(n_c), C.c_int(n_nodes), _p(f_nodes),
                                    _p(amp), _p(phase), _p(tf_nodes), _p(band), C.c_int64(n_f), C.c_int64(k_min),
-                                   C.c_double(df), _p(d), _p(W), _p(out["logL"]), _p(out["d_h"]), _p(out["h_h"]),
+                                   C.c_double(df), _p(d), _p(W), C.c_int(_w_rows(W, n_c)), _p(t_shift),
+                                   _p(out["logL"]), _p(out["d_h"]), _p(out["h_h"]),
                                    _p(out["logL_direct"]), _p(h)), "full_batch_tf")
     if want_template:
         out["h"] = h
@@ -194,11 +219,15 @@ def tlm_nodes(f_nodes, phase, t_ref) -> np.ndarray:
     return out
 
 
-def full_batch_standin(wl_modes_m, c_lm, kappa, params, f_nodes, k_min, df, n_f, d, W, want_template=False):
-    """parameters -> node arrays (stand-in, rounded to fp64) -> full_batch."""
+def full_batch_standin(wl_modes_m, c_lm, kappa, params, f_nodes, k_min, df, n_f, d, W, want_template=False,
+                       split_tc=False):
+    """parameters -> node arrays (stand-in, rounded to fp64) -> full_batch.  split_tc: the linear phase term
+    2 pi f t_c stays outside the spline (t_shift = t_c, reading R32)."""
+    params = _f64(params)
     f_lo, f_hi = float(k_min) * df, float(k_min + n_f - 1) * df
-    amp, phase, tf, band = standin_nodes(params, wl_modes_m, c_lm, kappa, f_nodes, f_lo, f_hi)
-    return full_batch(f_nodes, amp, phase, tf, band, k_min, df, d, W, want_template)
+    amp, phase, tf, band = standin_nodes(params, wl_modes_m, c_lm, kappa, f_nodes, f_lo, f_hi, split_tc=split_tc)
+    t_shift = np.ascontiguousarray(params[:, 2]) if split_tc else None
+    return full_batch(f_nodes, amp, phase, tf, band, k_min, df, d, W, want_template, t_shift=t_shift)
 
 
 # ------------------------------------------------------------------ heterodyned path
@@ -210,18 +239,21 @@ def het_prepare(k_min, df, d, W, h0_dense, f_edges):
     B0, B1, B2 = np.empty((n_c, n_b)), np.empty((n_c, n_b)), np.empty((n_c, n_b))
     ddb = C.c_double()
     _check(lib().orc_het_prepare(C.c_int(n_c), C.c_int64(n_f), C.c_int64(k_min), C.c_double(df), _p(d), _p(W),
-                                 _p(h0_dense), C.c_int(len(f_edges)), _p(f_edges),
+                                 C.c_int(_w_rows(W, n_c)), _p(h0_dense), C.c_int(len(f_edges)), _p(f_edges),
                                  _p(A0), _p(A1), _p(B0), _p(B1), _p(B2), C.byref(ddb)), "het_prepare")
     return dict(A0=A0, A1=A1, B0=B0, B1=B1, B2=B2, dd_band=ddb.value)
 
 
-def het_batch(f_edges, amp_e, phase_e, tf, h0_edges, summ):
+def het_batch(f_edges, amp_e, phase_e, tf, h0_edges, summ, t_shift=None):
+    """t_shift [n_w] or None: Psi_m(f_e) = phase_e + 2 pi f_e t_shift (reading R32)"""
     f_edges, amp_e, phase_e, tf, h0_edges = _f64(f_edges), _f64(amp_e), _f64(phase_e), _f64(tf), _f64(h0_edges)
     n_w, n_m, n_e = amp_e.shape
     n_c = tf.shape[2]
+    t_shift = None if t_shift is None else _f64(t_shift)
+    assert t_shift is None or t_shift.shape == (n_w,)
     out = {k: np.empty(n_w) for k in ("logL", "d_h", "h_h")}
     _check(lib().orc_het_batch(C.c_int64(n_w), C.c_int(n_m), C.c_int(n_c), C.c_int(n_e), _p(f_edges),
-                               _p(amp_e), _p(phase_e), _p(tf), _p(h0_edges),
+                               _p(amp_e), _p(phase_e), _p(tf), _p(t_shift), _p(h0_edges),
                                _p(_f64(summ["A0"])), _p(_f64(summ["A1"])), _p(_f64(summ["B0"])), _p(_f64(summ["B1"])),
                                C.c_double(summ["dd_band"]), _p(out["logL"]), _p(out["d_h"]), _p(out["h_h"])),
            "het_batch")

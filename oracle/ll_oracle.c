@@ -31,15 +31,22 @@
  * inputs; summary-data partition exactness; het exactness for r linear in f and its known B2
  * deficit; het == full at h = h0; the frequency-dependent-T path against the constant-T path, a template
  * whose T is linear in f against direct numpy evaluation, SciPy on tiny inputs; t_lm against SciPy's spline
- * derivative and the stand-in's analytic d Psi/df.  No function here is "parity unpinned".
+ * derivative and the stand-in's analytic d Psi/df; three channels with per-channel weights against SciPy + numpy channel
+ * by channel, the closed-form <h|h> under three different flat PSDs, additivity over channels and equality with the
+ * shared-weight path when the rows are equal; the linear phase term outside the spline (t_shift) against splining the
+ * full phase (a natural spline reproduces linear functions) and SciPy.  No function here is "parity unpinned".
  *
  * Layouts (all row-major, fp64):
  *   d, h, h0_dense, noise : [n_c][n_f][2]  (re, im)
- *   W                     : [n_f]          W_k = 4 df w_k / S_n(f_k)
+ *   W                     : [n_f] (w_rows = 1: one PSD for every channel) or [n_c][n_f] (w_rows = n_c: W^c_k =
+ *                           4 df w_k / S^c_n(f_k), each TDI channel with its own noise PSD; Eq. 3 sums over A, E, T and
+ *                           "A=E identical, T different")
  *   amp, phase            : [n_w][n_m][n_nodes]   (phase in radians)
  *   tf                    : [n_w][n_m][n_c][2]
  *   tf_nodes              : [n_w][n_m][n_c][n_nodes][2]   (frequency-dependent transfer function, Eq. 8-9)
  *   band                  : [n_w][2] (f_lo, f_hi) or NULL
+ *   t_shift               : [n_w] seconds or NULL: a linear phase term kept OUTSIDE the spline:
+ *                           Psi_m(f) = spline_m(f) + 2 pi f t_shift, the same for every mode (reading R32)
  *   params                : [n_w][P], P = 5 + 2 n_c n_m:
  *                           Mc[s], q, t_c[s], phi_c[rad], 1/D, then T^c_m (re, im), m-major, c-minor
  *   A0, A1                : [n_c][n_b][2];  B0, B1 : [n_c][n_b];  h0_edges : [n_c][n_e][2]
@@ -241,12 +248,13 @@ static void standin_masses(const double *p, ld *Mtot, ld *eta, ld *f_isco)
     *f_isco = powl(6.0L, -1.5L) / (PI_L * (*Mtot));
 }
 
-/* amplitude and phase (radians) of mode (l,m) at frequency f for parameter row p */
-static void standin_mode(const double *p, int m, double c_lm, double kappa, double f, ld *amp, ld *phase)
+/* amplitude and phase (radians) of mode (l,m) at frequency f for parameter row p.  split_tc: the phase WITHOUT its
+ * linear term 2 pi f t_c ((m/2) 2 pi (2f/m) t_c = 2 pi f t_c for every mode), which then travels as t_shift = t_c */
+static void standin_mode(const double *p, int m, double c_lm, double kappa, double f, int split_tc, ld *amp, ld *phase)
 {
     ld Mtot, eta, f_isco;
     standin_masses(p, &Mtot, &eta, &f_isco);
-    ld t_c = (ld)p[2], phi_c = (ld)p[3], invD = (ld)p[4];
+    ld t_c = split_tc ? 0.0L : (ld)p[2], phi_c = (ld)p[3], invD = (ld)p[4];
     ld fl = (ld)f, mh = (ld)m / 2.0L;
     *amp = (ld)c_lm * powl(fl, -7.0L / 6.0L) * invD * taper_l(2.0L * fl / ((ld)m * f_isco), (ld)kappa);
     *phase = mh * psi22_l(fl / mh, Mtot, eta, t_c, phi_c);
@@ -265,7 +273,7 @@ int orc_standin_fisco(const double *p, double *f_isco_out)
  * band = [k_min df, min(k_max df, (1+kappa) f_ISCO max_m(m/2))]. */
 int orc_standin_nodes(int64_t n_w, int n_m, int n_c, const int32_t *mode_m, const double *c_lm, double kappa,
                       const double *params, int n_freq, const double *f,
-                      double f_grid_lo, double f_grid_hi,
+                      double f_grid_lo, double f_grid_hi, int split_tc,
                       double *amp, double *phase, double *tf, double *band)
 {
     const int P = 5 + 2 * n_c * n_m;
@@ -277,7 +285,7 @@ int orc_standin_nodes(int64_t n_w, int n_m, int n_c, const int32_t *mode_m, cons
         for (int im = 0; im < n_m; ++im)
             for (int j = 0; j < n_freq; ++j) {
                 ld a, ph;
-                standin_mode(p, mode_m[im], c_lm[im], kappa, f[j], &a, &ph);
+                standin_mode(p, mode_m[im], c_lm[im], kappa, f[j], split_tc, &a, &ph);
                 amp[(w * n_m + im) * n_freq + j] = (double)a;
                 phase[(w * n_m + im) * n_freq + j] = (double)ph;
             }
@@ -296,27 +304,35 @@ int orc_standin_nodes(int64_t n_w, int n_m, int n_c, const int32_t *mode_m, cons
 /* ---------------------------------------------------------------------------------------------
  * <d|d> = sum_c sum_k W_k |d^c_k|^2     (Eq. 3 with W_k = 4 df w_k / S_n)
  * ------------------------------------------------------------------------------------------- */
-static ld inner_dd(int n_c, int64_t n_f, const double *d, const double *W, int64_t i_lo, int64_t i_hi)
+/* weight of channel c at bin i: one row shared by all channels (w_rows = 1) or one row per channel */
+static ld wgt(const double *W, int w_rows, int64_t n_f, int c, int64_t i)
+{
+    return (ld)W[(w_rows > 1 ? (int64_t)c * n_f : 0) + i];
+}
+
+static ld inner_dd(int n_c, int64_t n_f, const double *d, const double *W, int w_rows, int64_t i_lo, int64_t i_hi)
 {
     ld s = 0.0L;
     for (int c = 0; c < n_c; ++c)
         for (int64_t i = i_lo; i < i_hi; ++i) {
             ld re = d[(c * n_f + i) * 2], im = d[(c * n_f + i) * 2 + 1];
-            s += (ld)W[i] * (re * re + im * im);
+            s += wgt(W, w_rows, n_f, c, i) * (re * re + im * im);
         }
     return s;
 }
 
-int orc_inner(int n_c, int64_t n_f, const double *a, const double *b, const double *W, double *re_out, double *im_out)
+int orc_inner(int n_c, int64_t n_f, const double *a, const double *b, const double *W, int w_rows, double *re_out,
+              double *im_out)
 {
+    if (w_rows != 1 && w_rows != n_c) return -1;
     /* sum_c sum_k W_k conj(a_k) b_k : real part is <a|b> */
     ld sr = 0.0L, si = 0.0L;
     for (int c = 0; c < n_c; ++c)
         for (int64_t i = 0; i < n_f; ++i) {
             ld ar = a[(c * n_f + i) * 2], ai = a[(c * n_f + i) * 2 + 1];
             ld br = b[(c * n_f + i) * 2], bi = b[(c * n_f + i) * 2 + 1];
-            sr += (ld)W[i] * (ar * br + ai * bi);
-            si += (ld)W[i] * (ar * bi - ai * br);
+            sr += wgt(W, w_rows, n_f, c, i) * (ar * br + ai * bi);
+            si += wgt(W, w_rows, n_f, c, i) * (ar * bi - ai * br);
         }
     *re_out = (double)sr; *im_out = (double)si;
     return 0;
@@ -332,12 +348,14 @@ int orc_inner(int n_c, int64_t n_f, const double *a, const double *b, const doub
  * ------------------------------------------------------------------------------------------- */
 int orc_full_batch(int64_t n_w, int n_m, int n_c, int n_nodes, const double *f_nodes,
                    const double *amp, const double *phase, const double *tf, const double *band,
-                   int64_t n_f, int64_t k_min, double df, const double *d, const double *W,
+                   int64_t n_f, int64_t k_min, double df, const double *d, const double *W, int w_rows,
+                   const double *t_shift,
                    double *logL, double *d_h, double *h_h, double *logL_direct, double *h_out)
 {
     if (n_nodes < 3 || n_m < 1 || n_c < 1 || n_c > 3) return -1;
+    if (w_rows != 1 && w_rows != n_c) return -1;
     if (h_out && n_w != 1) return -1;
-    const ld dd = d ? inner_dd(n_c, n_f, d, W, 0, n_f) : 0.0L;
+    const ld dd = d ? inner_dd(n_c, n_f, d, W, w_rows, 0, n_f) : 0.0L;
     int fail = 0;
     #pragma omp parallel for schedule(dynamic, 1)
     for (int64_t w = 0; w < n_w; ++w) {
@@ -354,16 +372,19 @@ int orc_full_batch(int64_t n_w, int n_m, int n_c, int n_nodes, const double *f_n
             spline_ld(n_nodes, f_nodes, yP + m * nn, MP + m * nn);
         }
         const double f_lo = band ? band[2 * w] : -HUGE_VAL, f_hi = band ? band[2 * w + 1] : HUGE_VAL;
+        const ld tsh = t_shift ? (ld)t_shift[w] : 0.0L;
         ld s_dh = 0.0L, s_hh = 0.0L, s_res = 0.0L;
         for (int c = 0; c < n_c; ++c)
             for (int64_t i = 0; i < n_f; ++i) {
                 const double f = (double)(k_min + i) * df;
+                const ld Wi = wgt(W, w_rows, n_f, c, i);
                 ld hr = 0.0L, hi = 0.0L;
                 if (f >= f_lo && f <= f_hi) {
                     const int j = find_interval(n_nodes, f_nodes, f);
                     for (int m = 0; m < n_m; ++m) {
                         ld A = spline_eval_ld(f_nodes, yA + m * nn, MA + m * nn, j, f);
                         ld Psi = spline_eval_ld(f_nodes, yP + m * nn, MP + m * nn, j, f);
+                        if (t_shift) Psi += 2.0L * PI_L * (ld)f * tsh;        /* linear term outside the spline (R32) */
                         ld mr = A * cosl(Psi), mi = -A * sinl(Psi);          /* Eq. 7: A e^{-i Psi} */
                         ld tr = tf[((w * n_m + m) * n_c + c) * 2], ti = tf[((w * n_m + m) * n_c + c) * 2 + 1];
                         hr += tr * mr - ti * mi;                             /* Eq. 9 */
@@ -373,10 +394,10 @@ int orc_full_batch(int64_t n_w, int n_m, int n_c, int n_nodes, const double *f_n
                 if (h_out) { h_out[(c * n_f + i) * 2] = (double)hr; h_out[(c * n_f + i) * 2 + 1] = (double)hi; }
                 if (d) {
                     ld dr = d[(c * n_f + i) * 2], di = d[(c * n_f + i) * 2 + 1];
-                    s_dh += (ld)W[i] * (dr * hr + di * hi);                  /* Re[conj(d) h] */
-                    s_res += (ld)W[i] * ((dr - hr) * (dr - hr) + (di - hi) * (di - hi));
+                    s_dh += Wi * (dr * hr + di * hi);                        /* Re[conj(d) h] */
+                    s_res += Wi * ((dr - hr) * (dr - hr) + (di - hi) * (di - hi));
                 }
-                s_hh += (ld)W[i] * (hr * hr + hi * hi);
+                s_hh += Wi * (hr * hr + hi * hi);
             }
         if (logL) logL[w] = (double)(s_dh - 0.5L * s_hh - 0.5L * dd);
         if (d_h) d_h[w] = (double)s_dh;
@@ -397,12 +418,14 @@ int orc_full_batch(int64_t n_w, int n_m, int n_c, int n_nodes, const double *f_n
  * ------------------------------------------------------------------------------------------- */
 int orc_full_batch_tf(int64_t n_w, int n_m, int n_c, int n_nodes, const double *f_nodes,
                       const double *amp, const double *phase, const double *tf_nodes, const double *band,
-                      int64_t n_f, int64_t k_min, double df, const double *d, const double *W,
+                      int64_t n_f, int64_t k_min, double df, const double *d, const double *W, int w_rows,
+                      const double *t_shift,
                       double *logL, double *d_h, double *h_h, double *logL_direct, double *h_out)
 {
     if (n_nodes < 3 || n_m < 1 || n_c < 1 || n_c > 3) return -1;
+    if (w_rows != 1 && w_rows != n_c) return -1;
     if (h_out && n_w != 1) return -1;
-    const ld dd = d ? inner_dd(n_c, n_f, d, W, 0, n_f) : 0.0L;
+    const ld dd = d ? inner_dd(n_c, n_f, d, W, w_rows, 0, n_f) : 0.0L;
     int fail = 0;
     #pragma omp parallel for schedule(dynamic, 1)
     for (int64_t w = 0; w < n_w; ++w) {
@@ -425,10 +448,12 @@ int orc_full_batch_tf(int64_t n_w, int n_m, int n_c, int n_nodes, const double *
             for (int s = 0; s < 2 + 2 * n_c; ++s) spline_ld(n_nodes, f_nodes, ym + s * nn, Mm + s * nn);
         }
         const double f_lo = band ? band[2 * w] : -HUGE_VAL, f_hi = band ? band[2 * w + 1] : HUGE_VAL;
+        const ld tsh = t_shift ? (ld)t_shift[w] : 0.0L;
         ld s_dh = 0.0L, s_hh = 0.0L, s_res = 0.0L;
         for (int c = 0; c < n_c; ++c)
             for (int64_t i = 0; i < n_f; ++i) {
                 const double f = (double)(k_min + i) * df;
+                const ld Wi = wgt(W, w_rows, n_f, c, i);
                 ld hr = 0.0L, hi = 0.0L;
                 if (f >= f_lo && f <= f_hi) {
                     const int j = find_interval(n_nodes, f_nodes, f);
@@ -438,6 +463,7 @@ int orc_full_batch_tf(int64_t n_w, int n_m, int n_c, int n_nodes, const double *
                         ld Psi = spline_eval_ld(f_nodes, ym + nn, Mm + nn, j, f);
                         ld tr = spline_eval_ld(f_nodes, ym + (2 + 2 * c) * nn, Mm + (2 + 2 * c) * nn, j, f);
                         ld ti = spline_eval_ld(f_nodes, ym + (3 + 2 * c) * nn, Mm + (3 + 2 * c) * nn, j, f);
+                        if (t_shift) Psi += 2.0L * PI_L * (ld)f * tsh;        /* linear term outside the spline (R32) */
                         ld mr = A * cosl(Psi), mi = -A * sinl(Psi);          /* Eq. 7: A e^{-i Psi} */
                         hr += tr * mr - ti * mi;                             /* Eq. 9 */
                         hi += tr * mi + ti * mr;
@@ -446,10 +472,10 @@ int orc_full_batch_tf(int64_t n_w, int n_m, int n_c, int n_nodes, const double *
                 if (h_out) { h_out[(c * n_f + i) * 2] = (double)hr; h_out[(c * n_f + i) * 2 + 1] = (double)hi; }
                 if (d) {
                     ld dr = d[(c * n_f + i) * 2], di = d[(c * n_f + i) * 2 + 1];
-                    s_dh += (ld)W[i] * (dr * hr + di * hi);
-                    s_res += (ld)W[i] * ((dr - hr) * (dr - hr) + (di - hi) * (di - hi));
+                    s_dh += Wi * (dr * hr + di * hi);
+                    s_res += Wi * ((dr - hr) * (dr - hr) + (di - hi) * (di - hi));
                 }
-                s_hh += (ld)W[i] * (hr * hr + hi * hi);
+                s_hh += Wi * (hr * hr + hi * hi);
             }
         if (logL) logL[w] = (double)(s_dh - 0.5L * s_hh - 0.5L * dd);
         if (d_h) d_h[w] = (double)s_dh;
@@ -496,9 +522,10 @@ int orc_tlm_nodes(int64_t n_w, int n_m, int n_nodes, const double *f_nodes, cons
     return fail ? -4 : 0;
 }
 
-int orc_dd(int n_c, int64_t n_f, const double *d, const double *W, double *dd_out)
+int orc_dd(int n_c, int64_t n_f, const double *d, const double *W, int w_rows, double *dd_out)
 {
-    *dd_out = (double)inner_dd(n_c, n_f, d, W, 0, n_f);
+    if (w_rows != 1 && w_rows != n_c) return -1;
+    *dd_out = (double)inner_dd(n_c, n_f, d, W, w_rows, 0, n_f);
     return 0;
 }
 
@@ -515,7 +542,7 @@ int orc_standin_direct(int n_m, int n_c, const int32_t *mode_m, const double *c_
             if (f[i] >= f_lo && f[i] <= f_hi)
                 for (int m = 0; m < n_m; ++m) {
                     ld A, Psi;
-                    standin_mode(p, mode_m[m], c_lm[m], kappa, f[i], &A, &Psi);
+                    standin_mode(p, mode_m[m], c_lm[m], kappa, f[i], 0, &A, &Psi);
                     ld mr = A * cosl(Psi), mi = -A * sinl(Psi);
                     ld tr = p[5 + (m * n_c + c) * 2], ti = p[5 + (m * n_c + c) * 2 + 1];
                     hr += tr * mr - ti * mi;
@@ -535,11 +562,12 @@ int orc_standin_direct(int n_m, int n_c, const int32_t *mode_m, const double *c_
  *   B0 = sum W |h0|^2,      B1 = sum W |h0|^2 (f - f_b),     dd_band = sum_c sum_{k in any bin} W |d|^2.
  * B2 = sum W |h0|^2 (f-f_b)^2 is returned for the pin on the term Eq. 17 drops (may be NULL).
  * ------------------------------------------------------------------------------------------- */
-int orc_het_prepare(int n_c, int64_t n_f, int64_t k_min, double df, const double *d, const double *W,
+int orc_het_prepare(int n_c, int64_t n_f, int64_t k_min, double df, const double *d, const double *W, int w_rows,
                     const double *h0, int n_e, const double *e,
                     double *A0, double *A1, double *B0, double *B1, double *B2, double *dd_band)
 {
     if (n_e < 2) return -1;
+    if (w_rows != 1 && w_rows != n_c) return -1;
     const int n_b = n_e - 1;
     ld ddb = 0.0L;
     for (int c = 0; c < n_c; ++c)
@@ -552,7 +580,7 @@ int orc_het_prepare(int n_c, int64_t n_f, int64_t k_min, double df, const double
                 if (!inside) continue;
                 ld dr = d[(c * n_f + i) * 2], di = d[(c * n_f + i) * 2 + 1];
                 ld hr = h0[(c * n_f + i) * 2], hi = h0[(c * n_f + i) * 2 + 1];
-                ld w = (ld)W[i], t = (ld)f - fb;
+                ld w = wgt(W, w_rows, n_f, c, i), t = (ld)f - fb;
                 ld pr = dr * hr + di * hi, pi = di * hr - dr * hi;     /* d conj(h0) */
                 ld h2 = hr * hr + hi * hi;
                 a0r += w * pr;      a0i += w * pi;
@@ -579,7 +607,7 @@ int orc_het_prepare(int n_c, int64_t n_f, int64_t k_min, double df, const double
  * Returns -6 if h0 is exactly zero (or non-finite) at an edge.
  * ------------------------------------------------------------------------------------------- */
 int orc_het_batch(int64_t n_w, int n_m, int n_c, int n_e, const double *e,
-                  const double *amp_e, const double *phase_e, const double *tf, const double *h0_e,
+                  const double *amp_e, const double *phase_e, const double *tf, const double *t_shift, const double *h0_e,
                   const double *A0, const double *A1, const double *B0, const double *B1, double dd_band,
                   double *logL, double *d_h, double *h_h)
 {
@@ -601,6 +629,7 @@ int orc_het_batch(int64_t n_w, int n_m, int n_c, int n_e, const double *e,
                 ld hr = 0.0L, hi = 0.0L;
                 for (int m = 0; m < n_m; ++m) {
                     ld A = amp_e[(w * n_m + m) * n_e + j], Psi = phase_e[(w * n_m + m) * n_e + j];
+                    if (t_shift) Psi += 2.0L * PI_L * (ld)e[j] * (ld)t_shift[w];  /* linear term kept apart (R32) */
                     ld mr = A * cosl(Psi), mi = -A * sinl(Psi);
                     ld tr = tf[((w * n_m + m) * n_c + c) * 2], ti = tf[((w * n_m + m) * n_c + c) * 2 + 1];
                     hr += tr * mr - ti * mi;

@@ -21,8 +21,9 @@ import numpy as np
 import oracle as orc
 
 
-def full_batch_pw(f_nodes_w, amp, phase, tf, band, k_min, df, d, W):
-    """f_nodes_w [n_w][n_nodes]; amp, phase [n_w][n_m][n_nodes]; tf [n_w][n_m][n_c][2]; band [n_w][2] or None."""
+def full_batch_pw(f_nodes_w, amp, phase, tf, band, k_min, df, d, W, t_shift=None):
+    """f_nodes_w [n_w][n_nodes]; amp, phase [n_w][n_m][n_nodes]; tf [n_w][n_m][n_c][2]; band [n_w][2] or None;
+    W [n_f] or [n_c][n_f]; t_shift [n_w] or None (linear phase term outside the spline, reading R32)."""
     f_nodes_w = np.asarray(f_nodes_w, dtype=np.float64)
     n_w = f_nodes_w.shape[0]
     out = {k: np.empty(n_w) for k in ("logL", "d_h", "h_h", "logL_direct")}
@@ -31,7 +32,8 @@ def full_batch_pw(f_nodes_w, amp, phase, tf, band, k_min, df, d, W):
         lo, hi = x[0], x[-1]
         if band is not None:
             lo, hi = max(lo, band[w][0]), min(hi, band[w][1])
-        r = orc.full_batch(x, amp[w:w + 1], phase[w:w + 1], tf[w:w + 1], np.array([[lo, hi]]), k_min, df, d, W)
+        r = orc.full_batch(x, amp[w:w + 1], phase[w:w + 1], tf[w:w + 1], np.array([[lo, hi]]), k_min, df, d, W,
+                           t_shift=None if t_shift is None else np.asarray(t_shift, dtype=np.float64)[w:w + 1])
         for k in out:
             out[k][w] = r[k][0]
     return out

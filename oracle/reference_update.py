@@ -63,7 +63,7 @@ def audit(params, mode_m, c_lm, kappa, k_min, df, n_f, d, W, f_edges):
     form -1/2 sum W |d-h|^2 (reading R8)."""
     f = (k_min + np.arange(n_f, dtype=np.int64)).astype(np.float64) * df
     m = (f >= f_edges[0]) & (f <= f_edges[-1])
-    fm, Wm = np.ascontiguousarray(f[m]), np.ascontiguousarray(W[m])
+    fm, Wm = np.ascontiguousarray(f[m]), np.ascontiguousarray(np.asarray(W)[..., m])   # W [n_f] or [n_c][n_f]
     dm = np.ascontiguousarray(np.asarray(d)[:, m, :])
     ddb = orc.dd(dm, Wm)
     params = np.atleast_2d(np.asarray(params, dtype=np.float64))
@@ -74,5 +74,5 @@ def audit(params, mode_m, c_lm, kappa, k_min, df, n_f, d, W, f_edges):
         out["h_h"][w] = orc.inner(h, h, Wm).real
         out["logL"][w] = out["d_h"][w] - 0.5 * out["h_h"][w] - 0.5 * ddb
         r = dm - h
-        out["logL_direct"][w] = -0.5 * float(np.sum(Wm[None, :] * (r[..., 0] ** 2 + r[..., 1] ** 2)))
+        out["logL_direct"][w] = -0.5 * float(np.sum((Wm if Wm.ndim == 2 else Wm[None, :]) * (r[..., 0] ** 2 + r[..., 1] ** 2)))
     return out

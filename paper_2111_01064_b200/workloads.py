@@ -38,6 +38,21 @@ def psd_sn(f: np.ndarray) -> np.ndarray:
     return s_oms + s_acc * (1.0 + (0.4e-3 / f) ** 2) * (1.0 + (f / 8e-3) ** 4)
 
 
+def psd_sn_T(f: np.ndarray) -> np.ndarray:
+    """Analytic PSD of the T channel for the three-channel variants (Eq. 3 sums over A, E and T; "A=E identical, T
+    different").  A stand-in like psd_sn (the paper's SciRDv1 curves are not in PAPER.md): twice the
+    optical-metrology floor and a tenth of the acceleration noise, so its shape differs from psd_sn at both ends."""
+    f = np.asarray(f, dtype=np.float64)
+    s_oms = (15e-12) ** 2
+    s_acc = (3e-15) ** 2 / (2.0 * np.pi * f) ** 4
+    return 2.0 * s_oms + 0.1 * s_acc * (1.0 + (0.4e-3 / f) ** 2)
+
+
+def channel_psds(f: np.ndarray, n_c: int) -> np.ndarray:
+    """[n_c][n_f]: channels 0, 1 (A, E) share psd_sn, channel 2 (T) has psd_sn_T"""
+    return np.stack([psd_sn(f) if c < 2 else psd_sn_T(f) for c in range(n_c)])
+
+
 @dataclasses.dataclass
 class Grid:
     """rfft grid f_k = k*df, k = k_min .. k_min+n_f-1 (reading (c)3)."""
@@ -61,13 +76,16 @@ def make_grid(t_obs: float) -> Grid:
     return Grid(t_obs=float(t_obs), df=df, k_min=k_min, n_f=k_max - k_min + 1)
 
 
-def trapezoid_weights(grid: Grid, rule: str = "trapezoid") -> np.ndarray:
-    """W_k = 4 df w_k / S_n(f_k) (Eq. 3 discretised; reading (c)4)."""
+def trapezoid_weights(grid: Grid, rule: str = "trapezoid", n_c: int = 2) -> np.ndarray:
+    """W_k = 4 df w_k / S_n(f_k) (Eq. 3 discretised; reading (c)4).  n_c = 2: one row [n_f] (A and E share their
+    PSD); n_c = 3: one row per channel [3][n_f], the T channel with its own PSD."""
     w = np.ones(grid.n_f)
     if rule == "trapezoid":
         w[0] = 0.5
         w[-1] = 0.5
-    return 4.0 * grid.df * w / psd_sn(grid.freqs())
+    if n_c == 2:
+        return 4.0 * grid.df * w / psd_sn(grid.freqs())
+    return np.ascontiguousarray(4.0 * grid.df * w[None, :] / channel_psds(grid.freqs(), n_c))
 
 
 def geomspace_exact(lo: float, hi: float, n: int) -> np.ndarray:
@@ -99,7 +117,7 @@ class Workload:
     kappa: float
     params: np.ndarray              # f64 [n_w][P], P = 5 + 2 n_c n_m; 1/D column relative to D_inj until finished
     inj: np.ndarray                 # f64 [P] injection row (1/D = 1 until finished)
-    W: np.ndarray                   # f64 [n_f]
+    W: np.ndarray                   # f64 [n_f] (n_c = 2) or [n_c][n_f] (n_c = 3: per-channel PSDs)
     noise: Optional[np.ndarray]     # f64 [n_c][n_f][2] or None (noiseless)
     f_nodes: Optional[np.ndarray] = None    # full path
     f_edges: Optional[np.ndarray] = None    # het path
@@ -164,9 +182,9 @@ def _draw_ball(rng: np.random.Generator, n: int, inj: np.ndarray, frac: float) -
 def _draw_noise(seed: int, grid: Grid, n_c: int) -> np.ndarray:
     """Re, Im of n_k ~ N(0, S_n(f_k)/(4 df)) (reading (c)16)."""
     rng = np.random.default_rng([seed, 1])
-    sigma = np.sqrt(psd_sn(grid.freqs()) / (4.0 * grid.df))
+    sigma = np.sqrt(channel_psds(grid.freqs(), n_c) / (4.0 * grid.df))
     n = rng.standard_normal((n_c, grid.n_f, 2))
-    n *= sigma[None, :, None]
+    n *= sigma[:, :, None]
     return n
 
 
@@ -183,15 +201,16 @@ _NAMES = {0: "cfg0_full_tiny", 1: "cfg1_het", 2: "cfg2_full_search", 3: "cfg3_he
 
 def make_workload(index: int, n_w: Optional[int] = None, t_obs: Optional[float] = None,
                   n_knots: Optional[int] = None, seed_offset: int = 0,
-                  noisy: Optional[bool] = None) -> Workload:
+                  noisy: Optional[bool] = None, n_c: int = 2) -> Workload:
     """Build config `index`; the keyword overrides give scaled-down / ragged variants for tests and
-    rank-specific draws (seed_offset) for multi-GPU weak scaling."""
+    rank-specific draws (seed_offset) for multi-GPU weak scaling.  n_c = 3: the three-channel variant of the
+    config (A, E, T with per-channel weights; its own draws, since a parameter row is longer)."""
     path, t0, nw0, n_m, nk0, noisy0, ball, n_temps = _SPEC[index]
     t_obs = t0 if t_obs is None else float(t_obs)
     n_w = nw0 if n_w is None else int(n_w)
     n_knots = nk0 if n_knots is None else int(n_knots)
     noisy = noisy0 if noisy is None else bool(noisy)
-    n_c = 2
+    assert n_c in (2, 3)
     seed = SEED_BASE + index + 1000 * seed_offset
     grid = make_grid(t_obs)
     rng = np.random.default_rng(seed)
@@ -211,7 +230,7 @@ def make_workload(index: int, n_w: Optional[int] = None, t_obs: Optional[float] 
     wl = Workload(index=index, name=_NAMES[index], path=path, grid=grid, n_w=n_w, n_m=n_m, n_c=n_c,
                   modes_l=l, modes_m=m, c_lm=c_lm, kappa=KAPPA,
                   params=np.ascontiguousarray(params), inj=inj,
-                  W=trapezoid_weights(grid), noise=_draw_noise(seed, grid, n_c) if noisy else None,
+                  W=trapezoid_weights(grid, n_c=n_c), noise=_draw_noise(seed, grid, n_c) if noisy else None,
                   n_temps=n_temps)
     f_kmin, f_kmax = grid.k_min * grid.df, grid.k_max * grid.df
     if path == "full":

@@ -968,3 +968,235 @@ def test_sampler_run_keeps_gaussian_target():
     s = np.concatenate(keep)
     np.testing.assert_allclose(np.cov(s.T), C, rtol=0.2, atol=0.15)
     np.testing.assert_allclose(logL[0], ll(x[0])[0], rtol=1e-12)
+
+
+# ------------------------------------------- three channels, per-channel weights (Eq. 3)
+def _brute_full_wc(f_nodes, amp, phase, tf, band, k_min, df, d, Wc, t_shift=None):
+    """_brute_full with one weight row per channel and an optional linear phase term outside the spline: SciPy natural
+    spline + numpy complex arithmetic + math.fsum, the sums taken channel by channel."""
+    n_w, n_m, _ = amp.shape
+    n_c, n_f = Wc.shape
+    f = np.arange(k_min, k_min + n_f, dtype=np.float64) * df
+    dc = d[..., 0] + 1j * d[..., 1]
+    out = {k: np.zeros(n_w) for k in ("logL", "d_h", "h_h")}
+    dd = math.fsum(math.fsum(Wc[c] * np.abs(dc[c]) ** 2) for c in range(n_c))
+    for w in range(n_w):
+        mask = np.ones(n_f, bool) if band is None else (f >= band[w, 0]) & (f <= band[w, 1])
+        dh = hh = 0.0
+        for c in range(n_c):
+            h = np.zeros(n_f, complex)
+            for m in range(n_m):
+                A = CubicSpline(f_nodes, amp[w, m], bc_type="natural")(f)
+                P = CubicSpline(f_nodes, phase[w, m], bc_type="natural")(f)
+                if t_shift is not None:
+                    P = P + TWO_PI * f * t_shift[w]
+                h += (tf[w, m, c, 0] + 1j * tf[w, m, c, 1]) * A * np.exp(-1j * P)
+            h[~mask] = 0.0
+            dh += math.fsum(Wc[c] * (np.conj(dc[c]) * h).real)
+            hh += math.fsum(Wc[c] * np.abs(h) ** 2)
+        out["d_h"][w], out["h_h"][w], out["logL"][w] = dh, hh, dh - 0.5 * hh - 0.5 * dd
+    return out
+
+
+def _tiny_case(rng, n_w, n_m, n_c, n_nodes, n_f):
+    k_min, df = 7, 1.0 / 512.0
+    f = np.arange(k_min, k_min + n_f) * df
+    f_nodes = np.sort(np.concatenate([[f[0] * 0.9, f[-1] * 1.1], rng.uniform(f[1], f[-2], n_nodes - 2)]))
+    amp, ph = _rand_smooth_nodes(rng, n_w, n_m, f_nodes)
+    tf = _unit_tf(rng, n_w, n_m, n_c)
+    d = rng.standard_normal((n_c, n_f, 2))
+    Wc = rng.uniform(0.5, 2.0, (n_c, n_f)) * np.array([1.0, 3.0, 0.2])[:n_c, None]     # three different "PSDs"
+    band = np.stack([rng.uniform(f[0], f[n_f // 3], n_w), rng.uniform(f[n_f // 2], f[-1], n_w)], axis=1)
+    return k_min, df, f, f_nodes, amp, ph, tf, d, np.ascontiguousarray(Wc), band
+
+
+def test_three_channels_equal_rows_reduce_to_shared_weights(orc):
+    """W [n_c][n_f] with equal rows is the shared-W problem: every entry point that takes weights returns the same numbers."""
+    rng = np.random.default_rng(41)
+    k_min, df, f, f_nodes, amp, ph, tf, d, Wc, band = _tiny_case(rng, 4, 2, 3, 7, 48)
+    W1 = np.ascontiguousarray(Wc[1])
+    W3 = np.ascontiguousarray(np.tile(W1, (3, 1)))
+    a = orc.full_batch(f_nodes, amp, ph, tf, band, k_min, df, d, W1)
+    b = orc.full_batch(f_nodes, amp, ph, tf, band, k_min, df, d, W3)
+    for k in ("logL", "d_h", "h_h", "logL_direct"):
+        assert np.array_equal(a[k], b[k]), k
+    tfn = _rand_tf_nodes(rng, 4, 2, 3, f_nodes)
+    a = orc.full_batch_tf(f_nodes, amp, ph, tfn, band, k_min, df, d, W1)
+    b = orc.full_batch_tf(f_nodes, amp, ph, tfn, band, k_min, df, d, W3)
+    for k in ("logL", "d_h", "h_h", "logL_direct"):
+        assert np.array_equal(a[k], b[k]), k
+    assert orc.dd(d, W1) == orc.dd(d, W3) and orc.inner(d, d[::-1].copy(), W1) == orc.inner(d, d[::-1].copy(), W3)
+    h0 = rng.standard_normal((3, 48, 2)) + 2.0
+    e = np.array([f[2] - 0.1 * df, f[20], f[40] + 0.2 * df])
+    sa, sb = orc.het_prepare(k_min, df, d, W1, h0, e), orc.het_prepare(k_min, df, d, W3, h0, e)
+    for k in ("A0", "A1", "B0", "B1", "B2"):
+        assert np.array_equal(sa[k], sb[k]), k
+    assert sa["dd_band"] == sb["dd_band"]
+
+
+@pytest.mark.parametrize("n_m,n_nodes,n_f", [(1, 5, 24), (3, 8, 49)])
+def test_three_channels_three_psds_brute_force(orc, n_m, n_nodes, n_f):
+    """n_c = 3 with three different weight rows against SciPy + numpy, channel by channel (Eq. 3: 4 Re sum over A, E, T
+    of int a* b / S^c_n); a swapped or shared weight row fails it (the rows differ by factors 3 and 15)."""
+    rng = np.random.default_rng(300 + n_m)
+    k_min, df, f, f_nodes, amp, ph, tf, d, Wc, band = _tiny_case(rng, 3, n_m, 3, n_nodes, n_f)
+    o = orc.full_batch(f_nodes, amp, ph, tf, band, k_min, df, d, Wc)
+    r = _brute_full_wc(f_nodes, amp, ph, tf, band, k_min, df, d, Wc)
+    for k in ("logL", "d_h", "h_h"):
+        np.testing.assert_allclose(o[k], r[k], rtol=1e-11, atol=1e-11, err_msg=k)
+    np.testing.assert_allclose(o["logL_direct"], o["logL"], rtol=1e-11, atol=1e-10)
+    # the likelihood is additive over channels: three one-channel problems, each with its own row
+    parts = [orc.full_batch(f_nodes, amp, ph, np.ascontiguousarray(tf[:, :, c:c + 1]), band, k_min, df,
+                            np.ascontiguousarray(d[c:c + 1]), np.ascontiguousarray(Wc[c])) for c in range(3)]
+    for k in ("logL", "d_h", "h_h"):
+        np.testing.assert_allclose(o[k], sum(p[k] for p in parts), rtol=1e-12, atol=1e-12, err_msg=k)
+    # frequency-dependent transfer function, same three rows
+    tfn = _rand_tf_nodes(rng, 3, n_m, 3, f_nodes)
+    o = orc.full_batch_tf(f_nodes, amp, ph, tfn, band, k_min, df, d, Wc)
+    dc = _c(d)
+    for w in range(3):
+        mask = (f >= band[w, 0]) & (f <= band[w, 1])
+        dh = hh = 0.0
+        for c in range(3):
+            h = np.zeros(n_f, complex)
+            for m in range(n_m):
+                A = CubicSpline(f_nodes, amp[w, m], bc_type="natural")(f)
+                P = CubicSpline(f_nodes, ph[w, m], bc_type="natural")(f)
+                T = CubicSpline(f_nodes, tfn[w, m, c, :, 0], bc_type="natural")(f) + 1j * CubicSpline(
+                    f_nodes, tfn[w, m, c, :, 1], bc_type="natural")(f)
+                h += T * A * np.exp(-1j * P)
+            h[~mask] = 0.0
+            dh += (Wc[c] * (np.conj(dc[c]) * h).real).sum()
+            hh += (Wc[c] * np.abs(h) ** 2).sum()
+        assert o["d_h"][w] == pytest.approx(dh, rel=1e-11, abs=1e-11) and o["h_h"][w] == pytest.approx(hh, rel=1e-11)
+
+
+def test_hh_closed_form_three_flat_psds(orc):
+    """<h|h> = sum_c |T^c|^2 (6/(D^2 S_c)) (f_lo^{-4/3} - f_hi^{-4/3}) (+ the Euler-Maclaurin term of the trapezoid
+    sum) for three channels under three different flat PSDs, directly and through the spline path."""
+    S = np.array([3.0e-40, 1.1e-39, 4.0e-41])
+    tmod = np.array([1.0, 0.7, 1.6])
+    grid = wlm.make_grid(2.0 ** 17)
+    f = grid.freqs()
+    w = np.ones(grid.n_f)
+    w[0] = w[-1] = 0.5
+    Wc = np.ascontiguousarray(4.0 * grid.df * w[None, :] / S[:, None])
+    ang = np.array([0.3, 2.0, -1.1])
+    p = np.concatenate([_row(mc_msun=50.0, q=1.0, t_c=0.6 * 2.0 ** 17, inv_d=1.0)[:5],
+                        np.stack([tmod * np.cos(ang), tmod * np.sin(ang)], axis=1).ravel()])
+    h = orc.standin_direct(p, [2], [1.0], 0.5, f, f[0], f[-1])
+    assert h.shape == (3, grid.n_f, 2)
+    hh = orc.inner(h, h, Wc).real
+    gp = lambda x: -7.0 / 3.0 * x ** (-10.0 / 3.0)
+    per_unit = 3.0 * (f[0] ** (-4.0 / 3.0) - f[-1] ** (-4.0 / 3.0)) + 4.0 * grid.df ** 2 / 12.0 * (gp(f[-1]) - gp(f[0]))
+    expect = (tmod ** 2 / S).sum() * per_unit
+    assert hh == pytest.approx(expect, rel=5e-6)
+    f_nodes = wlm.geomspace_exact(1e-4, 0.05, 256)
+    r = orc.full_batch_standin([2], [1.0], 0.5, p[None], f_nodes, grid.k_min, grid.df, grid.n_f, None, Wc)
+    assert r["h_h"][0] == pytest.approx(expect, rel=2e-4)
+    # one channel at a time: each term of the sum separately (a row applied to the wrong channel changes these)
+    for c in range(3):
+        hc = np.zeros_like(h)
+        hc[c] = h[c]
+        assert orc.inner(hc, hc, Wc).real == pytest.approx(tmod[c] ** 2 / S[c] * per_unit, rel=5e-6)
+
+
+def test_het_three_channels_three_psds(orc):
+    """heterodyne with per-channel weights: partition exactness of A0, B0 channel by channel against numpy, and
+    het = full at h = h0 (north_star invariant) with three different PSDs."""
+    wl = wlm.make_workload(1, n_w=8, t_obs=2.0 ** 17, n_knots=24, n_c=3)
+    g = wl.grid
+    f = g.freqs()
+    assert wl.W.shape == (3, g.n_f) and not np.allclose(wl.W[0], wl.W[2])
+    direct = lambda p, ff: orc.standin_direct(p, wl.modes_m, wl.c_lm, wl.kappa, ff, f[0], f[-1])
+    h1 = direct(wl.inj, f)
+    wl.finish_distance(orc.inner(h1, h1, wl.W).real)
+    h0 = direct(wl.inj, f)
+    d = wl.make_data(h0)
+    h0e = direct(wl.inj, wl.f_edges)
+    s = orc.het_prepare(g.k_min, g.df, d, wl.W, h0, wl.f_edges)
+    m = _band_mask(f, wl.f_edges)
+    dc, hc = _c(d), _c(h0)
+    np.testing.assert_allclose(_c(s["A0"]).sum(axis=1), (wl.W * dc * np.conj(hc))[:, m].sum(axis=1), rtol=1e-12)
+    np.testing.assert_allclose(s["B0"].sum(axis=1), (wl.W * np.abs(hc) ** 2)[:, m].sum(axis=1), rtol=1e-12)
+    assert s["dd_band"] == pytest.approx((wl.W * np.abs(dc) ** 2)[:, m].sum(), rel=1e-12)
+    amp, ph, tf, _ = orc.standin_nodes(wl.inj[None], wl.modes_m, wl.c_lm, wl.kappa, wl.f_edges, f[0], f[-1])
+    assert tf.shape == (1, 1, 3, 2)
+    r = orc.het_batch(wl.f_edges, amp, ph, tf, h0e, s)
+    direct_ll = -0.5 * (wl.W[:, m] * np.abs(dc[:, m] - hc[:, m]) ** 2).sum()
+    assert r["logL"][0] == pytest.approx(direct_ll, rel=1e-10)
+    # near the reference the heterodyned value tracks the dense three-channel likelihood (method accuracy, PAPER.md:276)
+    amp, ph, tf, _ = orc.standin_nodes(wl.params, wl.modes_m, wl.c_lm, wl.kappa, wl.f_edges, f[0], f[-1])
+    het = orc.het_batch(wl.f_edges, amp, ph, tf, h0e, s)
+    for w in range(3):
+        hw = _c(direct(wl.params[w], f))
+        dense = (wl.W[:, m] * (np.conj(dc[:, m]) * hw[:, m]).real).sum() - 0.5 * (wl.W[:, m] * np.abs(hw[:, m]) ** 2).sum() \
+            - 0.5 * s["dd_band"]
+        assert abs(het["logL"][w] - dense) < 0.05 * max(1.0, abs(dense - direct_ll))
+
+
+# ------------------------------------------- linear phase term outside the spline (SURVEY 8(f) item 2; reading R32)
+def test_t_shift_equals_splining_the_full_phase(orc):
+    """A natural cubic spline reproduces a linear function exactly, so Psi = spline(phase) + 2 pi f t_shift is the same
+    function as spline(phase + 2 pi f_j t_shift): the two calls agree to the rounding of the larger phase."""
+    rng = np.random.default_rng(52)
+    k_min, df, f, f_nodes, amp, ph, tf, d, Wc, band = _tiny_case(rng, 5, 2, 2, 9, 64)
+    W = np.ascontiguousarray(Wc[0])
+    t = rng.uniform(-3e3, 3e3, 5)
+    ph_full = ph + TWO_PI * f_nodes[None, None, :] * t[:, None, None]
+    a = orc.full_batch(f_nodes, amp, ph, tf, band, k_min, df, d, W, t_shift=t)
+    b = orc.full_batch(f_nodes, amp, ph_full, tf, band, k_min, df, d, W)
+    scale = np.abs(ph_full).max()
+    assert scale > 1e3
+    for k in ("d_h", "h_h", "logL"):
+        np.testing.assert_allclose(a[k], b[k], rtol=0, atol=1e-15 * scale * np.abs(b["h_h"]).max() * 50, err_msg=k)
+    assert np.abs(a["d_h"] - orc.full_batch(f_nodes, amp, ph, tf, band, k_min, df, d, W)["d_h"]).max() > 1e-3   # it does something
+    # SciPy + numpy with the term added after the spline
+    r = _brute_full_wc(f_nodes, amp, ph, tf, band, k_min, df, d, np.ascontiguousarray(np.tile(W, (2, 1))), t_shift=t)
+    for k in ("logL", "d_h", "h_h"):
+        np.testing.assert_allclose(a[k], r[k], rtol=1e-10, atol=1e-10, err_msg=k)
+    # frequency-dependent-T path and per-walker nodes take the same term
+    tfn = _rand_tf_nodes(rng, 5, 2, 2, f_nodes)
+    a = orc.full_batch_tf(f_nodes, amp, ph, tfn, band, k_min, df, d, W, t_shift=t)
+    b = orc.full_batch_tf(f_nodes, amp, ph_full, tfn, band, k_min, df, d, W)
+    np.testing.assert_allclose(a["logL"], b["logL"], rtol=0, atol=1e-15 * scale * np.abs(b["h_h"]).max() * 50)
+    from oracle import per_walker as pw
+    xw = np.tile(f_nodes, (5, 1))
+    a = pw.full_batch_pw(xw, amp, ph, tf, band, k_min, df, d, W, t_shift=t)
+    b = orc.full_batch(f_nodes, amp, ph, tf, band, k_min, df, d, W, t_shift=t)
+    np.testing.assert_allclose(a["logL"], b["logL"], rtol=1e-13)
+
+
+def test_t_shift_standin_split_and_het(orc):
+    """stand-in: node phase without 2 pi f t_c, plus t_shift = t_c, is the stand-in's phase (for every mode: the linear
+    term of (m/2) Psi(2f/m) is 2 pi f t_c); heterodyne: phase_e + 2 pi f_e t_shift enters exactly like a phase."""
+    wl = wlm.make_workload(3, n_w=6, t_obs=2.0 ** 16, n_knots=12)
+    f_nodes = wlm.geomspace_exact(wlm.F_LO, wlm.F_HI, 40)
+    g = wl.grid
+    f = g.freqs()
+    a_full, p_full, tf, band = orc.standin_nodes(wl.params, wl.modes_m, wl.c_lm, wl.kappa, f_nodes, f[0], f[-1])
+    a_spl, p_spl, tf2, band2 = orc.standin_nodes(wl.params, wl.modes_m, wl.c_lm, wl.kappa, f_nodes, f[0], f[-1], split_tc=True)
+    assert np.array_equal(a_full, a_spl) and np.array_equal(tf, tf2) and np.array_equal(band, band2)
+    lin = TWO_PI * f_nodes[None, None, :] * wl.params[:, 2][:, None, None]
+    np.testing.assert_allclose(p_spl + lin, p_full, rtol=0, atol=1e-15 * np.abs(p_full).max() * 4)
+    assert np.all(np.abs(p_spl[..., -1]) < 0.01 * np.abs(p_full[..., -1]))   # at the top of the band almost nothing is left to spline
+    rng = np.random.default_rng(8)
+    d = rng.standard_normal((2, g.n_f, 2)) * 1e-19
+    run = lambda split: orc.full_batch_standin(wl.modes_m, wl.c_lm, wl.kappa, wl.params, f_nodes, g.k_min, g.df, g.n_f, d,
+                                               wl.W, split_tc=split)
+    a, b = run(True), run(False)
+    np.testing.assert_allclose(a["h_h"], b["h_h"], rtol=1e-9)
+    np.testing.assert_allclose(a["d_h"], b["d_h"], rtol=0, atol=1e-9 * np.sqrt(np.abs(b["h_h"]).max() * orc.dd(d, wl.W)))
+    # heterodyne array entry: t_shift against the same term added to the edge phases
+    e = wl.f_edges
+    h0 = rng.standard_normal((2, g.n_f, 2)) + 2.0
+    h0e = rng.standard_normal((2, len(e), 2)) + 2.0
+    s = orc.het_prepare(g.k_min, g.df, rng.standard_normal((2, g.n_f, 2)), rng.uniform(0.5, 2.0, g.n_f), h0, e)   # O(1) scales
+    amp_e = rng.uniform(0.5, 2.0, (6, wl.n_m, len(e)))
+    ph_e = rng.uniform(-20, 20, (6, wl.n_m, len(e)))
+    t = rng.uniform(-50.0, 50.0, 6)
+    a = orc.het_batch(e, amp_e, ph_e, tf, h0e, s, t_shift=t)
+    b = orc.het_batch(e, amp_e, ph_e + TWO_PI * e[None, None, :] * t[:, None, None], tf, h0e, s)
+    for k in ("logL", "d_h", "h_h"):
+        np.testing.assert_allclose(a[k], b[k], rtol=1e-11, atol=1e-11 * np.abs(b["h_h"]).max(), err_msg=k)
+    assert np.abs(a["d_h"] - orc.het_batch(e, amp_e, ph_e, tf, h0e, s)["d_h"]).max() > 1e-3 * np.abs(b["d_h"]).max()
