@@ -19,6 +19,7 @@
  *     The caller owns every pointer it passes.  The library copies what it keeps (pre-weighted data,
  *     weights, summary tables) and holds no caller pointer once the stream has reached the end of the call.
  *   - All arrays are row-major fp64.  Complex numbers are (re, im) pairs in the last axis.
+ *   - n_c = ll_config.n_channels: 2 (TDI A, E) or 3 (A, E, T; Eq. 3 sums over all three).
  *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Batch calls are
  *     asynchronous on it, never synchronise, and do not allocate in steady state (scratch grows on the
  *     first call at a larger shape; growing synchronises the device once).
@@ -31,6 +32,9 @@
  * Weights (reading R4):    W_i = 4 df w_i / S_n(f_i), w_i the quadrature weight (trapezoid or rectangle).
  * Parameter row of the stand-in waveform (reading R9; BASELINE.json config 0/3), P = 5 + 2 n_c n_m doubles:
  *   Mc [s], q, t_c [s], phi_c [rad], 1/D, then T^c_m (re, im) mode-major, channel-minor.
+ * t_shift (reading R32): an optional per-walker linear phase term kept OUTSIDE the spline,
+ *   Psi_m(f) = spline_m(f) + 2 pi f t_shift for every mode m; DEV [n_w] seconds, or NULL.  With the node phases given
+ *   without their 2 pi f t_c term the spline carries ~1e4 rad instead of ~1e7 at the top of a one-year band.
  */
 #ifndef LL_B200_H
 #define LL_B200_H
@@ -57,11 +61,11 @@ enum { LL_PREC_FP64 = 0, LL_PREC_FP32_ACC = 1 };
 enum { LL_BC_NATURAL = 0, LL_BC_NOT_A_KNOT = 1 }; /* not-a-knot needs n_nodes >= 4; ll_tlm_nodes is natural-only */
 
 #define LL_MAX_MODES 8
-#define LL_N_CHANNELS 2
+#define LL_MAX_CHANNELS 3
 
 typedef struct {
     int32_t device;     /* CUDA device ordinal                                                              */
-    int32_t n_channels; /* must be 2 (TDI A and E; reading R5)                                 */
+    int32_t n_channels; /* 2 (TDI A, E) or 3 (A, E, T: Eq. 3; reading R5)                   */
     int32_t n_modes;    /* 1..LL_MAX_MODES harmonics (l,m) summed per channel (Eq. 9)                       */
     int32_t precision;  /* LL_PREC_FP64, or LL_PREC_FP32_ACC (full-grid path only; reading R15)             */
     int32_t spline_bc;  /* LL_BC_NATURAL (reading R1) or LL_BC_NOT_A_KNOT: boundary condition of every node spline   */
@@ -76,10 +80,14 @@ const char *ll_last_error(const ll_ctx *ctx);
 int ll_abi_version(void);
 
 /* F0 — fix the data stream and the noise weights (Eq. 3; "prior to the analysis, we transform the data",
- * PAPER.md:91).  Builds g^c_i = W_i conj(d^c_i) (interleaved [n_f][A re, A im, E re, E im]) and
- * <d|d> = sum_c sum_i W_i |d^c_i|^2.  May be called again at any time; invalidates ll_het_prepare.
- *   d : DEV [n_c][n_f][2]     W : DEV [n_f]                                                               */
-int ll_set_data(ll_ctx *ctx, int64_t n_f, int64_t k_min, double df, const double *d, const double *W,
+ * PAPER.md:91).  Builds g^c_i = W^c_i conj(d^c_i) (interleaved [n_f][n_c][re, im]) and
+ * <d|d> = sum_c sum_i W^c_i |d^c_i|^2.  May be called again at any time; invalidates ll_het_prepare and every
+ * table cached for the previous grid.
+ *   d : DEV [n_c][n_f][2]
+ *   W : DEV [n_f] when w_shared != 0 (one PSD for every channel: "A=E identical"), else DEV [n_c][n_f]
+ *       (W^c_i = 4 df w_i / S^c_n(f_i): every channel its own PSD, "T different").
+ * FP32-accumulate contexts take two channels with w_shared != 0 only (LL_ERR_UNSUPPORTED otherwise).       */
+int ll_set_data(ll_ctx *ctx, int64_t n_f, int64_t k_min, double df, const double *d, const double *W, int32_t w_shared,
                 void *stream);
 
 /* <d|d> over the whole grid and over the heterodyne band (0 before ll_het_prepare).  HOST out.
@@ -90,16 +98,21 @@ int ll_get_dd(ll_ctx *ctx, double *dd_full, double *dd_het_band, void *stream);
  *   l, m, c_lm : HOST [n_modes]   (n_modes must equal the context's)                                      */
 int ll_standin_config(ll_ctx *ctx, int32_t n_modes, const int32_t *l, const int32_t *m, const double *c_lm,
                       double taper_kappa);
+/* on != 0: the stand-in entry points of the full-grid path (ll_full_batch_standin, ll_full_template_standin,
+ * ll_standin_nodes, ll_pt_*_full) build the node phases WITHOUT the linear term 2 pi f t_c and carry it as
+ * t_shift = t_c outside the spline (reading R32).  Same template up to rounding; off by default (reading R2).   */
+int ll_standin_split_tc(ll_ctx *ctx, int32_t on);
 
 /* F2-F4 — full-grid log-likelihood of n_w walkers given node arrays (Eq. 2, 3, 7, 9; spline: reading R1).
  *   f_nodes : HOST [n_nodes] strictly ascending, n_nodes >= 3, f_nodes[0] <= f_0, f_nodes[last] >= f_{n_f-1}
  *   amp, phase : DEV [n_w][n_m][n_nodes]  (phase in radians; h_lm = amp exp(-i phase))
  *   tf   : DEV [n_w][n_m][n_c][2]         transfer factors T^c_lm (Eq. 8-9 as per-walker constants, R5/R11)
  *   band : DEV [n_w][2] (f_lo, f_hi) or NULL (whole grid); template is zero outside (reading R10)
+ *   t_shift : DEV [n_w] or NULL (see the top of this file; reading R32)
  *   logL, d_h, h_h : DEV [n_w]; d_h and/or h_h may be NULL.  n_w = 0 is a no-op.                          */
 int ll_full_batch(ll_ctx *ctx, int64_t n_w, int32_t n_nodes, const double *f_nodes, const double *amp,
-                  const double *phase, const double *tf, const double *band, double *logL, double *d_h,
-                  double *h_h, void *stream);
+                  const double *phase, const double *tf, const double *band, const double *t_shift, double *logL,
+                  double *d_h, double *h_h, void *stream);
 
 /* F2-F4 with a frequency-dependent transfer function — h^c(f) = sum_lm T^c_lm(f, t_lm(f)) h_lm(f) (Eq. 8-9,
  * PAPER.md:100-110).  The transfer function's formula is in the paper's ref. [44], so T arrives at the nodes:
@@ -107,8 +120,8 @@ int ll_full_batch(ll_ctx *ctx, int64_t n_w, int32_t n_nodes, const double *f_nod
  *              (natural cubic in f) and evaluated at every dense bin.  Other arguments as ll_full_batch.
  * FP64 contexts only (LL_ERR_UNSUPPORTED otherwise).                                                        */
 int ll_full_batch_tf(ll_ctx *ctx, int64_t n_w, int32_t n_nodes, const double *f_nodes, const double *amp,
-                     const double *phase, const double *tf_nodes, const double *band, double *logL, double *d_h,
-                     double *h_h, void *stream);
+                     const double *phase, const double *tf_nodes, const double *band, const double *t_shift, double *logL,
+                     double *d_h, double *h_h, void *stream);
 
 /* F2-F4 with PER-WALKER node grids: every walker brings its own nodes, spanning its own band,
  * so each walker has its own tridiagonal system (a true batched solve) and its own bin -> interval map.
@@ -117,8 +130,8 @@ int ll_full_batch_tf(ll_ctx *ctx, int64_t n_w, int32_t n_nodes, const double *f_
  *   zero outside [f_nodes_w[w][0], f_nodes_w[w][n_nodes-1]] (intersected with `band` when given; reading R30).
  * FP64 contexts only.                                                                                        */
 int ll_full_batch_pw(ll_ctx *ctx, int64_t n_w, int32_t n_nodes, const double *f_nodes_w, const double *amp,
-                     const double *phase, const double *tf, const double *band, double *logL, double *d_h, double *h_h,
-                     void *stream);
+                     const double *phase, const double *tf, const double *band, const double *t_shift, double *logL,
+                     double *d_h, double *h_h, void *stream);
 
 /* F1 utility — the stand-in's node arrays in the caller layout (what ll_full_batch_standin builds internally):
  *   params : DEV [n_w][P];  amp, phase : DEV out [n_w][n_m][n_nodes] (phase in radians);
@@ -187,9 +200,10 @@ int ll_het_audit_standin(ll_ctx *ctx, int64_t n_w, const double *params, double 
 int ll_het_get_summary(ll_ctx *ctx, double *A0, double *A1, double *B0, double *B1, void *stream);
 
 /* H1-H3 — heterodyned log-likelihood given amplitude/phase at the bin edges (Eq. 11, 14, 17).
- *   amp_e, phase_e : DEV [n_w][n_m][n_edges]   tf : DEV [n_w][n_m][n_c][2]   outputs as ll_full_batch     */
+ *   amp_e, phase_e : DEV [n_w][n_m][n_edges]   tf : DEV [n_w][n_m][n_c][2]   outputs as ll_full_batch
+ *   t_shift : DEV [n_w] or NULL: Psi_m(f_e) = phase_e + 2 pi f_e t_shift (reading R32)                    */
 int ll_het_batch(ll_ctx *ctx, int64_t n_w, const double *amp_e, const double *phase_e, const double *tf,
-                 double *logL, double *d_h, double *h_h, void *stream);
+                 const double *t_shift, double *logL, double *d_h, double *h_h, void *stream);
 
 /* H1-H3 with the stand-in waveform evaluated at the edges on the device.   params : DEV [n_w][P]          */
 int ll_het_batch_standin(ll_ctx *ctx, int64_t n_w, const double *params, double *logL, double *d_h,

@@ -63,6 +63,7 @@ struct FullPlan {
 
 struct ll_ctx {
     int device = 0, n_c = 2, n_m = 1, precision = 0, spline_bc = 0;
+    int w_rows = 1; // weight rows kept on the device: 1 (two channels sharing their PSD) or n_c
     int sm_count = 148;
     std::string err;
     int64_t launches = 0;
@@ -71,7 +72,7 @@ struct ll_ctx {
     bool have_data = false;
     long long n_f = 0, n_f_pad = 0, k_min = 0;
     double df = 0.0;
-    DevBuf g4, Wd, dd_part, dd; // dd: [0] full grid, [1] het band
+    DevBuf g, Wc, dd_part, dd;  // g [n_f_pad][2 n_c], Wc [w_rows][n_f_pad]; dd: [0] full grid, [1] het band
     DevBuf g4f, Wf, scale, wmax; // FP32-accumulate variant: g/sigma in binary32, W/sigma^2 in FP64, (sigma, 1/sigma, 1/sigma^2)
     DevBuf pairs;               // unsigned long long [1]
 
@@ -121,7 +122,7 @@ struct ll_ctx {
     int hetn_key_total = -1, hetn_S = 1, hetn_grid = 1;
     HetTable ht{};
     Het1Table ht1{}; // single-mode regrouped table (k_het_standin1); base == nullptr when not built
-    std::vector<double> raw_host; // [n_b][13]
+    std::vector<double> raw_host; // [n_b][6 n_c + 1]
 
     // host staging for the *_host entry points
     DevBuf stage_in, stage_out;
@@ -196,6 +197,18 @@ struct ProfScope { // records an event pair around one launch when profiling is 
 };
 
 inline int ceil_div(long long a, long long b) { return (int)((a + b - 1) / b); }
+
+// the three data layouts the kernels are built for: (channels, one weight row shared by all of them?)
+#define LL_LAYOUT(ctx, CALL)                                      \
+    do {                                                          \
+        if ((ctx)->n_c == 2 && (ctx)->w_rows == 1) { CALL(2, true); } \
+        else if ((ctx)->n_c == 2) { CALL(2, false); }             \
+        else { CALL(3, false); }                                  \
+    } while (0)
+#define LL_CHANNELS(ctx, CALL)                                    \
+    do {                                                          \
+        if ((ctx)->n_c == 2) { CALL(2); } else { CALL(3); }       \
+    } while (0)
 inline long long round_up(long long a, long long b) { return (a + b - 1) / b * b; }
 
 // ---------------------------------------------------------------------------------------------------
@@ -372,38 +385,19 @@ int ensure_tiles(ll_ctx *ctx, FullPlan &pl, cudaStream_t st, bool uniform = fals
     return LL_OK;
 }
 
-// the whole full-grid pipeline for walkers [0, n_w) given either stand-in params or caller arrays
-int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, const double *amp, const double *phase,
-             const double *tf, const double *band, double *logL, double *d_h, double *h_h, cudaStream_t st,
-             bool template_only, double *h_out, const double *tf_nodes = nullptr)
+// band -> bin range per walker, sort by band top (F1 prologue shared by every full-grid entry point)
+int band_sort(ll_ctx *ctx, const FullPlan &pl, long long n_w, bool standin, const double *params, int P, const double *band,
+              cudaStream_t st)
 {
-    const bool standin = params != nullptr;
-    const bool tfp = tf_nodes != nullptr; // frequency-dependent transfer function: 6 splines per mode
-    const int ns = tfp ? 6 : 2;
-    const int n_m = ctx->n_m;
-    const int P = 5 + 2 * kNC * n_m;
-    FullPlan pl = make_plan(ctx, n_w);
-    {
-        const int rc_t = ensure_tiles(ctx, pl, st);
-        if (rc_t != LL_OK) return rc_t;
-    }
     const int n_wp = pl.n_wp;
-    const bool nm1 = (n_m == 1);
-    const int NQ = (nm1 && !tfp) ? 5 : 2;
-
     CK(ctx->ilo_w.ensure(sizeof(int) * n_wp));
     CK(ctx->ihi_w.ensure(sizeof(int) * n_wp));
-    CK(ctx->key_w.ensure(sizeof(int) * n_wp));
+    CK(ctx->key_w.ensure(sizeof(int) * 2 * n_wp)); // keys, then the unordered buckets
     CK(ctx->perm.ensure(sizeof(int) * n_wp));
     CK(ctx->ilo_s.ensure(sizeof(int) * n_wp));
     CK(ctx->ihi_s.ensure(sizeof(int) * n_wp));
-    CK(ctx->hist.ensure(sizeof(int) * 8192));
+    CK(ctx->hist.ensure(sizeof(int) * (2 * 8192 + 1))); // cursors, then the bucket starts
     CK(ctx->pairs.ensure(sizeof(unsigned long long)));
-    CK(ctx->Y.ensure(sizeof(double) * (size_t)n_m * ns * n_nodes * n_wp));
-    CK(ctx->C.ensure(sizeof(double) * (size_t)(n_nodes - 1) * n_m * ns * 4 * n_wp));
-    CK(ctx->TF.ensure(sizeof(double) * (size_t)n_m * 4 * n_wp));
-    if (!template_only) CK(ctx->part.ensure(sizeof(double) * (size_t)pl.n_tiles * NQ * n_wp));
-
     const GridInfo g{ctx->k_min, ctx->n_f, ctx->df};
     if (n_w <= 1024 && n_wp <= 1024) {
         k_band_sort_small<<<1, 1024, 0, st>>>(standin ? 1 : 0, params, P, band, (int)n_w, n_wp, g, ctx->si, ctx->perm.as<int>(),
@@ -416,24 +410,115 @@ int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, cons
                                                         ctx->ilo_w.as<int>(), ctx->ihi_w.as<int>(), ctx->key_w.as<int>(),
                                                         ctx->hist.as<int>(), ctx->pairs.as<unsigned long long>());
         LAUNCHED(ctx);
-        k_scan_hist<<<1, 1024, 0, st>>>(ctx->hist.as<int>(), pl.n_keys);
+        int *starts = ctx->hist.as<int>() + 8192, *bucket = ctx->key_w.as<int>() + n_wp;
+        k_scan_hist<<<1, 1024, 0, st>>>(ctx->hist.as<int>(), pl.n_keys, starts);
         LAUNCHED(ctx);
-        k_scatter<<<ceil_div(n_wp, 256), 256, 0, st>>>((int)n_w, n_wp, ctx->key_w.as<int>(), ctx->ilo_w.as<int>(),
-                                                       ctx->ihi_w.as<int>(), ctx->hist.as<int>(), ctx->perm.as<int>(),
-                                                       ctx->ilo_s.as<int>(), ctx->ihi_s.as<int>());
+        k_scatter<<<ceil_div(n_w, 256), 256, 0, st>>>((int)n_w, ctx->key_w.as<int>(), ctx->hist.as<int>(), bucket);
         LAUNCHED(ctx);
+        k_sort_buckets<<<pl.n_keys + 1, kSortThreads, 0, st>>>((int)n_w, n_wp, pl.n_keys, starts, bucket, ctx->key_w.as<int>(),
+                                                               ctx->ilo_w.as<int>(), ctx->ihi_w.as<int>(), ctx->perm.as<int>(),
+                                                               ctx->ilo_s.as<int>(), ctx->ihi_s.as<int>());
+        LAUNCHED(ctx);
+    }
+    return LL_OK;
+}
+
+FusedArgs fused_args(ll_ctx *ctx, const FullPlan &pl, int n_nodes, const double *t_shift, int ts_stride)
+{
+    FusedArgs fa;
+    fa.g = ctx->g.as<double>(); fa.Wc = ctx->Wc.as<double>(); fa.C = ctx->C.as<double>(); fa.TF = ctx->TF.as<double>();
+    fa.xj = ctx->nt.xj; fa.bstart = ctx->nt.bstart; fa.ilo = ctx->ilo_s.as<int>(); fa.ihi = ctx->ihi_s.as<int>();
+    fa.perm = ctx->perm.as<int>(); fa.t_shift = t_shift; fa.ts_stride = ts_stride;
+    fa.part = ctx->part.as<double>(); fa.k_min = ctx->k_min; fa.n_f_pad = ctx->n_f_pad; fa.df = ctx->df;
+    fa.n_f = (int)ctx->n_f; fa.n_wp = pl.n_wp; fa.n_nodes = n_nodes; fa.n_m = ctx->n_m; fa.TB = pl.TB; fa.CH = pl.CH;
+    fa.tile_start = ctx->tile_cur->tab.as<int>();
+    return fa;
+}
+
+// F4: partial sums over tiles (two stages for small batches with thousands of tiles) -> log L
+int finalize(ll_ctx *ctx, const FullPlan &pl, bool single_mode_sums, double *logL, double *d_h, double *h_h, cudaStream_t st)
+{
+    const int n_wp = pl.n_wp, n_c = ctx->n_c, nw = ctx->w_rows;
+    const int NQ = single_mode_sums ? 2 * n_c + nw : 2;
+    const double *fin_part = ctx->part.as<double>();
+    const int *fin_tiles = ctx->tile_cur->tab.as<int>();
+    int fin_n = pl.n_tiles;
+    if (n_wp <= 1024 && pl.n_tiles >= 8 * kTileChunk) { // thousands of tiles, a handful of walker blocks: two stages
+        CK(ctx->part2.ensure(sizeof(double) * (size_t)ctx->tile_cur->n2 * NQ * n_wp));
+        dim3 grid(ceil_div(n_wp, 32), ctx->tile_cur->n2);
+#define LL_REDUCE(Q)                                                                                                     \
+    k_reduce_tiles<Q><<<grid, dim3(32, fin_slices(Q)), 0, st>>>(fin_part, ctx->ilo_s.as<int>(), ctx->ihi_s.as<int>(), n_wp, fin_tiles, \
+                                                     fin_n, kTileChunk, ctx->part2.as<double>())
+        switch (NQ) {
+        case 2: LL_REDUCE(2); break;
+        case 5: LL_REDUCE(5); break;
+        case 6: LL_REDUCE(6); break;
+        default: LL_REDUCE(9); break;
+        }
+#undef LL_REDUCE
+        LAUNCHED(ctx);
+        fin_part = ctx->part2.as<double>();
+        fin_tiles = ctx->tile_cur->tab.as<int>() + ctx->tile_cur->off2;
+        fin_n = ctx->tile_cur->n2;
+    }
+#define LL_FIN(NC, WS)                                                                                                    \
+    do {                                                                                                                  \
+        if (single_mode_sums)                                                                                             \
+            k_finalize<1, NC, (WS ? 1 : NC)><<<ceil_div(n_wp, 32), dim3(32, fin_slices(2 * NC + (WS ? 1 : NC))), 0, st>>>(                             \
+                fin_part, ctx->TF.as<double>(), ctx->perm.as<int>(), ctx->ilo_s.as<int>(), ctx->ihi_s.as<int>(), n_wp,    \
+                fin_tiles, fin_n, ctx->dd.as<double>(), logL, d_h, h_h);                                                  \
+        else                                                                                                              \
+            k_finalize<0, NC, (WS ? 1 : NC)><<<ceil_div(n_wp, 32), dim3(32, fin_slices(2)), 0, st>>>(                             \
+                fin_part, ctx->TF.as<double>(), ctx->perm.as<int>(), ctx->ilo_s.as<int>(), ctx->ihi_s.as<int>(), n_wp,    \
+                fin_tiles, fin_n, ctx->dd.as<double>(), logL, d_h, h_h);                                                  \
+    } while (0)
+    LL_LAYOUT(ctx, LL_FIN);
+#undef LL_FIN
+    LAUNCHED(ctx);
+    return LL_OK;
+}
+
+// the whole full-grid pipeline for walkers [0, n_w) given either stand-in params or caller arrays
+int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, const double *amp, const double *phase,
+             const double *tf, const double *band, const double *t_shift, double *logL, double *d_h, double *h_h,
+             cudaStream_t st, bool template_only, double *h_out, const double *tf_nodes = nullptr)
+{
+    const bool standin = params != nullptr;
+    const bool tfp = tf_nodes != nullptr; // frequency-dependent transfer function: 2 + 2 n_c splines per mode
+    const int n_m = ctx->n_m, n_c = ctx->n_c, nw = ctx->w_rows;
+    const int ns = tfp ? 2 + 2 * n_c : 2;
+    const int P = 5 + 2 * n_c * n_m;
+    FullPlan pl = make_plan(ctx, n_w);
+    {
+        const int rc_t = ensure_tiles(ctx, pl, st);
+        if (rc_t != LL_OK) return rc_t;
+    }
+    const int n_wp = pl.n_wp;
+    const bool nm1 = (n_m == 1);
+    const bool sums1 = nm1 && !tfp; // the single-mode kernel leaves S^c, H^c and k_finalize applies T^c
+    const int NQ = sums1 ? 2 * n_c + nw : 2;
+    int ts_stride = 1;
+    if (standin && ctx->si.split_tc) { t_shift = params + 2; ts_stride = P; } // the stand-in's own linear term (R32)
+
+    CK(ctx->Y.ensure(sizeof(double) * (size_t)n_m * ns * n_nodes * n_wp));
+    CK(ctx->C.ensure(sizeof(double) * (size_t)(n_nodes - 1) * n_m * ns * 4 * n_wp));
+    CK(ctx->TF.ensure(sizeof(double) * (size_t)n_m * 2 * n_c * n_wp));
+    if (!template_only) CK(ctx->part.ensure(sizeof(double) * (size_t)pl.n_tiles * NQ * n_wp));
+    {
+        const int rc_b = band_sort(ctx, pl, n_w, standin, params, P, band, st);
+        if (rc_b != LL_OK) return rc_b;
     }
     if (standin) {
         dim3 grid(ceil_div(n_wp, 128), ceil_div(n_nodes, kNodesPerThread));
         k_nodes_standin<<<grid, 128, 0, st>>>(params, P, ctx->perm.as<int>(), n_wp, n_nodes, ctx->si, ctx->nt,
                                               ctx->Y.as<double>(), ctx->TF.as<double>());
     } else if (tfp) {
-        dim3 grid(n_wp / 32, ceil_div(n_nodes, 32), n_m * 6);
-        k_nodes_arrays_tf<<<grid, 256, 0, st>>>(amp, phase, tf_nodes, ctx->perm.as<int>(), n_wp, n_nodes, n_m,
+        dim3 grid(n_wp / 32, ceil_div(n_nodes, 32), n_m * ns);
+        k_nodes_arrays_tf<<<grid, 256, 0, st>>>(amp, phase, tf_nodes, ctx->perm.as<int>(), n_wp, n_nodes, n_m, n_c,
                                                 ctx->Y.as<double>());
     } else {
         dim3 grid(n_wp / 32, ceil_div(n_nodes, 32), n_m);
-        k_nodes_arrays<<<grid, 256, 0, st>>>(amp, phase, tf, ctx->perm.as<int>(), n_wp, n_nodes, n_m,
+        k_nodes_arrays<<<grid, 256, 0, st>>>(amp, phase, tf, ctx->perm.as<int>(), n_wp, n_nodes, n_m, n_c,
                                              ctx->Y.as<double>(), ctx->TF.as<double>());
     }
     LAUNCHED(ctx);
@@ -452,68 +537,45 @@ int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, cons
         }
         LAUNCHED(ctx);
     }
-    FusedArgs fa;
-    fa.g4 = ctx->g4.as<double>(); fa.Wd = ctx->Wd.as<double>(); fa.C = ctx->C.as<double>(); fa.TF = ctx->TF.as<double>();
-    fa.xj = ctx->nt.xj; fa.bstart = ctx->nt.bstart; fa.ilo = ctx->ilo_s.as<int>(); fa.ihi = ctx->ihi_s.as<int>();
-    fa.part = ctx->part.as<double>(); fa.k_min = ctx->k_min; fa.df = ctx->df; fa.n_f = (int)ctx->n_f; fa.n_wp = n_wp;
-    fa.n_nodes = n_nodes; fa.n_m = n_m; fa.TB = pl.TB; fa.CH = pl.CH;
-    fa.tile_start = ctx->tile_cur->tab.as<int>();
+    const FusedArgs fa = fused_args(ctx, pl, n_nodes, t_shift, ts_stride);
     if (template_only) {
         // sorted position of walker 0 of a one-walker batch is 0
-        k_full_template<<<ceil_div(ctx->n_f, 256), 256, 0, st>>>(fa, 0, h_out);
+        k_full_template<<<ceil_div(ctx->n_f, 256), 256, 0, st>>>(fa, 0, n_c, h_out);
         LAUNCHED(ctx);
         return LL_OK;
     }
     {
         dim3 grid(n_wp / pl.WB, pl.n_tiles);
         const bool mixed = ctx->precision == LL_PREC_FP32_ACC && !tfp;
-        const size_t smem = (size_t)2 * pl.CH * (mixed ? 24 : 40);
+        const size_t smem = (size_t)2 * pl.CH * (mixed ? 24 : 8 * (2 * n_c + nw));
         ProfScope prof(ctx, st);
-        if (tfp) {
-            if (nm1) k_full_fused_tf<1><<<grid, pl.WB, smem, st>>>(fa);
-            else k_full_fused_tf<0><<<grid, pl.WB, smem, st>>>(fa);
-        } else if (mixed) {
+        if (mixed) {
             const FusedArgsF32 fm{ctx->g4f.as<float>(), ctx->Wf.as<double>(), ctx->scale.as<double>()};
             k_full_fused_mixed<<<grid, pl.WB, smem, st>>>(fa, fm);
-        } else if (nm1) k_full_fused<1><<<grid, pl.WB, smem, st>>>(fa);
-        else k_full_fused<0><<<grid, pl.WB, smem, st>>>(fa);
+        } else {
+#define LL_FUSED(NC, WS)                                                              \
+    do {                                                                              \
+        if (tfp) {                                                                    \
+            if (nm1) k_full_fused_tf<1, NC, WS><<<grid, pl.WB, smem, st>>>(fa);       \
+            else k_full_fused_tf<0, NC, WS><<<grid, pl.WB, smem, st>>>(fa);           \
+        } else if (nm1) k_full_fused<1, NC, WS><<<grid, pl.WB, smem, st>>>(fa);       \
+        else k_full_fused<0, NC, WS><<<grid, pl.WB, smem, st>>>(fa);                  \
+    } while (0)
+            LL_LAYOUT(ctx, LL_FUSED);
+#undef LL_FUSED
+        }
         LAUNCHED(ctx);
         ctx->last_n_blocks = (int)(grid.x * grid.y);
     }
-    const double *fin_part = ctx->part.as<double>();
-    const int *fin_tiles = ctx->tile_cur->tab.as<int>();
-    int fin_n = pl.n_tiles;
-    if (n_wp <= 1024 && pl.n_tiles >= 8 * kTileChunk) { // thousands of tiles, a handful of walker blocks: two stages
-        CK(ctx->part2.ensure(sizeof(double) * (size_t)ctx->tile_cur->n2 * NQ * n_wp));
-        dim3 grid(ceil_div(n_wp, 32), ctx->tile_cur->n2);
-        if (NQ == 5)
-            k_reduce_tiles<5><<<grid, dim3(32, 32), 0, st>>>(fin_part, ctx->ilo_s.as<int>(), ctx->ihi_s.as<int>(), n_wp, fin_tiles,
-                                                            fin_n, kTileChunk, ctx->part2.as<double>());
-        else
-            k_reduce_tiles<2><<<grid, dim3(32, 32), 0, st>>>(fin_part, ctx->ilo_s.as<int>(), ctx->ihi_s.as<int>(), n_wp, fin_tiles,
-                                                            fin_n, kTileChunk, ctx->part2.as<double>());
-        LAUNCHED(ctx);
-        fin_part = ctx->part2.as<double>();
-        fin_tiles = ctx->tile_cur->tab.as<int>() + ctx->tile_cur->off2;
-        fin_n = ctx->tile_cur->n2;
-    }
-    if (nm1 && !tfp)
-        k_finalize<1><<<ceil_div(n_wp, 32), dim3(32, kFinY), 0, st>>>(fin_part, ctx->TF.as<double>(), ctx->perm.as<int>(),
-                                                           ctx->ilo_s.as<int>(), ctx->ihi_s.as<int>(), n_wp, fin_tiles, fin_n,
-                                                           ctx->dd.as<double>(), logL, d_h, h_h);
-    else
-        k_finalize<0><<<ceil_div(n_wp, 32), dim3(32, kFinY), 0, st>>>(fin_part, ctx->TF.as<double>(), ctx->perm.as<int>(),
-                                                           ctx->ilo_s.as<int>(), ctx->ihi_s.as<int>(), n_wp, fin_tiles, fin_n,
-                                                           ctx->dd.as<double>(), logL, d_h, h_h);
-    LAUNCHED(ctx);
-    return LL_OK;
+    return finalize(ctx, pl, sums1, logL, d_h, h_h, st);
 }
 
 // full-grid pipeline with per-walker node grids (reading R30)
 int run_full_pw(ll_ctx *ctx, long long n_w, int n_nodes, const double *f_nodes_w, const double *amp, const double *phase,
-                const double *tf, const double *band, double *logL, double *d_h, double *h_h, cudaStream_t st)
+                const double *tf, const double *band, const double *t_shift, double *logL, double *d_h, double *h_h,
+                cudaStream_t st)
 {
-    const int n_m = ctx->n_m;
+    const int n_m = ctx->n_m, n_c = ctx->n_c, nw = ctx->w_rows;
     FullPlan pl = make_plan(ctx, n_w);
     {
         const int rc_t = ensure_tiles(ctx, pl, st, true);
@@ -521,45 +583,22 @@ int run_full_pw(ll_ctx *ctx, long long n_w, int n_nodes, const double *f_nodes_w
     }
     const int n_wp = pl.n_wp;
     const int NQ = 2;
-    CK(ctx->ilo_w.ensure(sizeof(int) * n_wp));
-    CK(ctx->ihi_w.ensure(sizeof(int) * n_wp));
-    CK(ctx->key_w.ensure(sizeof(int) * n_wp));
-    CK(ctx->perm.ensure(sizeof(int) * n_wp));
-    CK(ctx->ilo_s.ensure(sizeof(int) * n_wp));
-    CK(ctx->ihi_s.ensure(sizeof(int) * n_wp));
-    CK(ctx->hist.ensure(sizeof(int) * 8192));
-    CK(ctx->pairs.ensure(sizeof(unsigned long long)));
     CK(ctx->Y.ensure(sizeof(double) * (size_t)n_m * 2 * n_nodes * n_wp));
     CK(ctx->C.ensure(sizeof(double) * (size_t)(n_nodes - 1) * n_m * 8 * n_wp));
-    CK(ctx->TF.ensure(sizeof(double) * (size_t)n_m * 4 * n_wp));
+    CK(ctx->TF.ensure(sizeof(double) * (size_t)n_m * 2 * n_c * n_wp));
     CK(ctx->part.ensure(sizeof(double) * (size_t)pl.n_tiles * NQ * n_wp));
     CK(ctx->pw_x.ensure(sizeof(double) * ((size_t)n_nodes * n_wp + 2 * (size_t)n_w)));
     double *X = ctx->pw_x.as<double>(), *band_w = X + (size_t)n_nodes * n_wp;
 
-    const GridInfo g{ctx->k_min, ctx->n_f, ctx->df};
     k_pw_band<<<ceil_div(n_w, 256), 256, 0, st>>>(f_nodes_w, band, (int)n_w, n_nodes, band_w);
     LAUNCHED(ctx);
-    if (n_w <= 1024 && n_wp <= 1024) {
-        k_band_sort_small<<<1, 1024, 0, st>>>(0, nullptr, 0, band_w, (int)n_w, n_wp, g, ctx->si, ctx->perm.as<int>(),
-                                              ctx->ilo_s.as<int>(), ctx->ihi_s.as<int>(), ctx->pairs.as<unsigned long long>());
-        LAUNCHED(ctx);
-    } else {
-        CK(cudaMemsetAsync(ctx->hist.p, 0, sizeof(int) * pl.n_keys, st));
-        CK(cudaMemsetAsync(ctx->pairs.p, 0, sizeof(unsigned long long), st));
-        k_band_prep<<<ceil_div(n_w, 256), 256, 0, st>>>(0, nullptr, 0, band_w, (int)n_w, g, ctx->si, pl.key_gran,
-                                                        ctx->ilo_w.as<int>(), ctx->ihi_w.as<int>(), ctx->key_w.as<int>(),
-                                                        ctx->hist.as<int>(), ctx->pairs.as<unsigned long long>());
-        LAUNCHED(ctx);
-        k_scan_hist<<<1, 1024, 0, st>>>(ctx->hist.as<int>(), pl.n_keys);
-        LAUNCHED(ctx);
-        k_scatter<<<ceil_div(n_wp, 256), 256, 0, st>>>((int)n_w, n_wp, ctx->key_w.as<int>(), ctx->ilo_w.as<int>(),
-                                                       ctx->ihi_w.as<int>(), ctx->hist.as<int>(), ctx->perm.as<int>(),
-                                                       ctx->ilo_s.as<int>(), ctx->ihi_s.as<int>());
-        LAUNCHED(ctx);
+    {
+        const int rc_b = band_sort(ctx, pl, n_w, false, nullptr, 0, band_w, st);
+        if (rc_b != LL_OK) return rc_b;
     }
     {
         dim3 grid(n_wp / 32, ceil_div(n_nodes, 32), n_m);
-        k_nodes_arrays<<<grid, 256, 0, st>>>(amp, phase, tf, ctx->perm.as<int>(), n_wp, n_nodes, n_m, ctx->Y.as<double>(),
+        k_nodes_arrays<<<grid, 256, 0, st>>>(amp, phase, tf, ctx->perm.as<int>(), n_wp, n_nodes, n_m, n_c, ctx->Y.as<double>(),
                                              ctx->TF.as<double>());
         LAUNCHED(ctx);
         dim3 gx(n_wp / 32, ceil_div(n_nodes, 32));
@@ -569,27 +608,23 @@ int run_full_pw(ll_ctx *ctx, long long n_w, int n_nodes, const double *f_nodes_w
         k_spline_pw<<<gs, 128, 0, st>>>(ctx->Y.as<double>(), X, ctx->C.as<double>(), n_wp, n_nodes, n_m, ctx->spline_bc);
         LAUNCHED(ctx);
     }
-    FusedArgs fa;
-    fa.g4 = ctx->g4.as<double>(); fa.Wd = ctx->Wd.as<double>(); fa.C = ctx->C.as<double>(); fa.TF = ctx->TF.as<double>();
-    fa.xj = nullptr; fa.bstart = nullptr; fa.ilo = ctx->ilo_s.as<int>(); fa.ihi = ctx->ihi_s.as<int>();
-    fa.part = ctx->part.as<double>(); fa.k_min = ctx->k_min; fa.df = ctx->df; fa.n_f = (int)ctx->n_f; fa.n_wp = n_wp;
-    fa.n_nodes = n_nodes; fa.n_m = n_m; fa.TB = pl.TB; fa.CH = pl.CH;
-    fa.tile_start = ctx->tile_cur->tab.as<int>();
+    FusedArgs fa = fused_args(ctx, pl, n_nodes, t_shift, 1);
+    fa.xj = nullptr; fa.bstart = nullptr;
     {
         dim3 grid(n_wp / pl.WB, pl.n_tiles);
-        const size_t smem = (size_t)2 * pl.CH * 40;
+        const size_t smem = (size_t)2 * pl.CH * 8 * (2 * n_c + nw);
         ProfScope prof(ctx, st);
-        if (n_m == 1) k_full_fused_pw<1><<<grid, pl.WB, smem, st>>>(fa, X);
-        else k_full_fused_pw<0><<<grid, pl.WB, smem, st>>>(fa, X);
+#define LL_FUSED_PW(NC, WS)                                                            \
+    do {                                                                               \
+        if (n_m == 1) k_full_fused_pw<1, NC, WS><<<grid, pl.WB, smem, st>>>(fa, X);    \
+        else k_full_fused_pw<0, NC, WS><<<grid, pl.WB, smem, st>>>(fa, X);             \
+    } while (0)
+        LL_LAYOUT(ctx, LL_FUSED_PW);
+#undef LL_FUSED_PW
         LAUNCHED(ctx);
         ctx->last_n_blocks = (int)(grid.x * grid.y);
     }
-    k_finalize<0><<<ceil_div(n_wp, 32), dim3(32, kFinY), 0, st>>>(ctx->part.as<double>(), ctx->TF.as<double>(), ctx->perm.as<int>(),
-                                                                 ctx->ilo_s.as<int>(), ctx->ihi_s.as<int>(), n_wp,
-                                                                 ctx->tile_cur->tab.as<int>(), pl.n_tiles, ctx->dd.as<double>(), logL,
-                                                                 d_h, h_h);
-    LAUNCHED(ctx);
-    return LL_OK;
+    return finalize(ctx, pl, false, logL, d_h, h_h, st);
 }
 
 int check_full_common(ll_ctx *ctx, int64_t n_w, const double *f_nodes, const double *logL)
@@ -600,8 +635,8 @@ int check_full_common(ll_ctx *ctx, int64_t n_w, const double *f_nodes, const dou
     if (!f_nodes) return ctx->fail(LL_ERR_ARG, "f_nodes is NULL");
     if (n_w > 0 && !logL) return ctx->fail(LL_ERR_ARG, "logL is NULL");
     if (!ctx->have_data) return ctx->fail(LL_ERR_STATE, "ll_set_data has not been called");
-    if (ctx->precision == LL_PREC_FP32_ACC && ctx->n_m != 1)
-        return ctx->fail(LL_ERR_UNSUPPORTED, "the FP32-accumulate variant is built for n_modes = 1 only");
+    if (ctx->precision == LL_PREC_FP32_ACC && (ctx->n_m != 1 || ctx->n_c != 2 || ctx->w_rows != 1))
+        return ctx->fail(LL_ERR_UNSUPPORTED, "the FP32-accumulate variant is built for n_modes = 1, two channels, one shared weight row only");
     return LL_OK;
 }
 
@@ -609,19 +644,19 @@ int check_full_common(ll_ctx *ctx, int64_t n_w, const double *f_nodes, const dou
 int build_het_table(ll_ctx *ctx, int n_e, const double *e, const std::vector<double> &h0e, std::vector<double> &tab)
 {
     typedef long double ld;
-    const int n_b = n_e - 1, n_m = ctx->n_m;
+    const int n_b = n_e - 1, n_m = ctx->n_m, n_c = ctx->n_c, NR = 6 * n_c + 1;
     HetTable T;
-    T.base = nullptr; T.n_e = n_e; T.n_b = n_b; T.n_m = n_m;
-    T.total = 5 * n_e + 3 * n_m * n_e + 12 * n_b;
+    T.base = nullptr; T.n_e = n_e; T.n_b = n_b; T.n_m = n_m; T.n_c = n_c;
+    T.total = (1 + 2 * n_c) * n_e + 3 * n_m * n_e + 6 * n_c * n_b;
     tab.assign(T.total, 0.0);
     for (int j = 0; j < n_e; ++j) {
         tab[T.off_f4() + j] = 4.0 * e[j];
-        for (int c = 0; c < kNC; ++c) {
+        for (int c = 0; c < n_c; ++c) {
             const ld gr = h0e[((size_t)c * n_e + j) * 2], gi = h0e[((size_t)c * n_e + j) * 2 + 1];
             const ld den = gr * gr + gi * gi;
             if (!(den > 0.0L) || !std::isfinite((double)den)) return ctx->fail(LL_ERR_REF_ZERO, "h0 is zero or non-finite at a bin edge");
-            tab[T.off_ih0() + 4 * j + 2 * c] = (double)(gr / den);
-            tab[T.off_ih0() + 4 * j + 2 * c + 1] = (double)(-gi / den);
+            tab[T.off_ih0() + 2 * n_c * j + 2 * c] = (double)(gr / den);
+            tab[T.off_ih0() + 2 * n_c * j + 2 * c + 1] = (double)(-gi / den);
         }
         if (ctx->have_standin)
             for (int m = 0; m < n_m; ++m) {
@@ -636,28 +671,30 @@ int build_het_table(ll_ctx *ctx, int n_e, const double *e, const std::vector<dou
     const std::vector<double> &raw = ctx->raw_host;
     for (int b = 0; b < n_b; ++b) {
         const ld invw = 1.0L / ((ld)e[b + 1] - (ld)e[b]);
-        double *t = &tab[T.off_bins() + 12 * b];
-        const double *r = &raw[(size_t)b * 13];
-        // raw: A: (A0r, A0i, A1r, A1i, B0, B1) at 0..5, E at 6..11
-        t[0] = 0.5 * r[0]; t[1] = 0.5 * r[1]; t[2] = 0.5 * r[6]; t[3] = 0.5 * r[7];
-        t[4] = (double)((ld)r[2] * invw); t[5] = (double)((ld)r[3] * invw);
-        t[6] = (double)((ld)r[8] * invw); t[7] = (double)((ld)r[9] * invw);
-        t[8] = 0.25 * r[4]; t[9] = 0.25 * r[10];
-        t[10] = (double)((ld)r[5] * invw); t[11] = (double)((ld)r[11] * invw);
+        double *t = &tab[T.off_bins() + 6 * n_c * b];
+        // raw: per channel (A0r, A0i, A1r, A1i, B0, B1); table: A0/2 [2 n_c], A1/width [2 n_c], B0/4 [n_c], B1/width [n_c]
+        for (int c = 0; c < n_c; ++c) {
+            const double *r = &raw[(size_t)b * NR + 6 * c];
+            t[2 * c] = 0.5 * r[0]; t[2 * c + 1] = 0.5 * r[1];
+            t[2 * n_c + 2 * c] = (double)((ld)r[2] * invw); t[2 * n_c + 2 * c + 1] = (double)((ld)r[3] * invw);
+            t[4 * n_c + c] = 0.25 * r[4];
+            t[5 * n_c + c] = (double)((ld)r[5] * invw);
+        }
     }
     ctx->ht = T;
     return LL_OK;
 }
 
-// single-mode regrouped table (k_het_standin1): 14 doubles per edge, see ll_kernels.cuh
+// single-mode regrouped table (k_het_standin1): 4 + 5 n_c doubles per edge, see ll_kernels.cuh
 void build_het1_table(ll_ctx *ctx, int n_e, const double *e, const std::vector<double> &h0e, std::vector<double> &tab)
 {
     typedef long double ld;
-    const int n_b = n_e - 1;
-    const std::vector<double> &raw = ctx->raw_host; // [n_b][13]: per channel (A0r, A0i, A1r, A1i, B0, B1), then dd
-    tab.assign((size_t)n_e * kHet1Stride, 0.0);
-    std::vector<ld> ihr((size_t)kNC * n_e), ihi((size_t)kNC * n_e);
-    for (int c = 0; c < kNC; ++c)
+    const int n_b = n_e - 1, n_c = ctx->n_c, NR = 6 * n_c + 1, ST = het1_stride(n_c);
+    const int oQ = 4, oP = 4 + 2 * n_c, oX = 4 + 3 * n_c;
+    const std::vector<double> &raw = ctx->raw_host; // [n_b][6 n_c + 1]: per channel (A0r, A0i, A1r, A1i, B0, B1), then dd
+    tab.assign((size_t)n_e * ST, 0.0);
+    std::vector<ld> ihr((size_t)n_c * n_e), ihi((size_t)n_c * n_e);
+    for (int c = 0; c < n_c; ++c)
         for (int j = 0; j < n_e; ++j) {
             const ld gr = h0e[((size_t)c * n_e + j) * 2], gi = h0e[((size_t)c * n_e + j) * 2 + 1];
             const ld den = gr * gr + gi * gi;
@@ -665,36 +702,36 @@ void build_het1_table(ll_ctx *ctx, int n_e, const double *e, const std::vector<d
             ihi[(size_t)c * n_e + j] = -gi / den;
         }
     for (int j = 0; j < n_e; ++j) {
-        double *t = &tab[(size_t)j * kHet1Stride];
+        double *t = &tab[(size_t)j * ST];
         const ld f = (ld)e[j], fp = 2.0L * f / (ld)ctx->si.mode_m[0];
         t[0] = 4.0 * e[j];
         t[1] = (double)powl(fp, -5.0L / 3.0L);
         t[2] = (double)((ld)ctx->c_lm[0] * powl(f, -7.0L / 6.0L));
         t[3] = (double)fp;
-        for (int c = 0; c < kNC; ++c) {
+        for (int c = 0; c < n_c; ++c) {
             ld Gr = 0, Gi = 0, Pc = 0;
             if (j >= 1) { // bin j - 1 ends at this edge
-                const double *r = &raw[(size_t)(j - 1) * 13 + 6 * c];
+                const double *r = &raw[(size_t)(j - 1) * NR + 6 * c];
                 const ld invw = 1.0L / ((ld)e[j] - (ld)e[j - 1]);
                 Gr += 0.5L * r[0] + r[2] * invw; Gi += 0.5L * r[1] + r[3] * invw;
                 Pc += 0.25L * r[4] + r[5] * invw;
             }
             if (j < n_b) { // bin j starts at this edge
-                const double *r = &raw[(size_t)j * 13 + 6 * c];
+                const double *r = &raw[(size_t)j * NR + 6 * c];
                 const ld invw = 1.0L / ((ld)e[j + 1] - (ld)e[j]);
                 Gr += 0.5L * r[0] - r[2] * invw; Gi += 0.5L * r[1] - r[3] * invw;
                 Pc += 0.25L * r[4] - r[5] * invw;
             }
             const ld ar = ihr[(size_t)c * n_e + j], ai = ihi[(size_t)c * n_e + j];
             // Q = G conj(1/h0)
-            t[4 + 2 * c] = (double)(Gr * ar + Gi * ai);
-            t[5 + 2 * c] = (double)(Gi * ar - Gr * ai);
-            t[8 + c] = (double)(Pc * (ar * ar + ai * ai));
+            t[oQ + 2 * c] = (double)(Gr * ar + Gi * ai);
+            t[oQ + 2 * c + 1] = (double)(Gi * ar - Gr * ai);
+            t[oP + c] = (double)(Pc * (ar * ar + ai * ai));
             if (j < n_b) { // X = (B0/2) (1/h0_j) conj(1/h0_{j+1})
                 const ld br = ihr[(size_t)c * n_e + j + 1], bi = ihi[(size_t)c * n_e + j + 1];
-                const ld hb = 0.5L * raw[(size_t)j * 13 + 6 * c + 4];
-                t[10 + 2 * c] = (double)(hb * (ar * br + ai * bi));
-                t[11 + 2 * c] = (double)(hb * (ai * br - ar * bi));
+                const ld hb = 0.5L * raw[(size_t)j * NR + 6 * c + 4];
+                t[oX + 2 * c] = (double)(hb * (ar * br + ai * bi));
+                t[oX + 2 * c + 1] = (double)(hb * (ai * br - ar * bi));
             }
         }
     }
@@ -712,20 +749,22 @@ int het_check(ll_ctx *ctx, int64_t n_w, const double *logL)
 }
 
 // single mode: the regrouped kernel (one table copy per block, WY warps = G walker groups x S edge segments)
+template <int NC>
 int launch_het_standin1(ll_ctx *ctx, int64_t n_w, const double *params, double *logL, double *d_h, double *h_h,
                         cudaStream_t st)
 {
     const int n_groups = ceil_div(n_w, 32), n_e = ctx->ht1.n_e;
     constexpr int WY = LL_HET1_WY;
-    const size_t smem = sizeof(double) * ((size_t)n_e * kHet1Stride + (size_t)WY * 192);
+    const size_t tab_d = (size_t)n_e * het1_stride(NC);
+    const size_t smem = sizeof(double) * (tab_d + (tab_d & 1) + (size_t)WY * 32 * 3 * NC);
     if (!ctx->het1_attr) {
-        CK(cudaFuncSetAttribute(k_het_standin1, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+        CK(cudaFuncSetAttribute(k_het_standin1<NC>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
         ctx->het1_attr = true;
     }
     if (smem > 227 * 1024) return ctx->fail(LL_ERR_UNSUPPORTED, "heterodyne tables exceed shared memory (too many bins)");
     if (ctx->het1_bps == 0 || ctx->het1_bps_smem != smem) {
         int bps = 0;
-        CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, k_het_standin1, 32 * WY, smem));
+        CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, k_het_standin1<NC>, 32 * WY, smem));
         ctx->het1_bps = std::max(1, bps);
         ctx->het1_bps_smem = smem;
     }
@@ -741,24 +780,24 @@ int launch_het_standin1(ll_ctx *ctx, int64_t n_w, const double *params, double *
         const double work = (double)ceil_div(gr, ctx->sm_count) * (double)ceil_div(passes, gr) * WY * (ceil_div(n_e, s) + 1.0);
         if (work < best * 0.999) { best = work; S = s; grid = gr; }
     }
-    const int P = 5 + 2 * kNC;
+    const int P = 5 + 2 * NC;
     ProfScope prof(ctx, st);
-    k_het_standin1<<<grid, dim3(32, WY), smem, st>>>(ctx->ht1, ctx->si, params, P, (int)n_w, n_groups, S,
-                                                     ctx->dd.as<double>(), logL, d_h, h_h);
+    k_het_standin1<NC><<<grid, dim3(32, WY), smem, st>>>(ctx->ht1, ctx->si, params, P, (int)n_w, n_groups, S,
+                                                         ctx->dd.as<double>(), logL, d_h, h_h);
     LAUNCHED(ctx);
     return LL_OK;
 }
 
-template <int NM>
+template <int NM, int NC>
 int launch_het_standin(ll_ctx *ctx, int64_t n_w, const double *params, double *logL, double *d_h, double *h_h,
                        cudaStream_t st)
 {
     const int n_groups = ceil_div(n_w, 32), n_b = ctx->ht.n_b;
     constexpr int WY = LL_HET_WY; // warps per block, all sharing one table copy
     // table + [WY][2][32] segment partials + -(m/pi) + the staged parameter rows of the G = WY/S walker groups
-    auto smem_of = [&](int s) { return sizeof(double) * ((size_t)ctx->ht.total + (size_t)WY * 64 + 8 + (size_t)(WY / s) * 32 * (5 + 4 * NM)); };
-    if (!ctx->hetn_attr) { // a context has one n_modes, so one instantiation
-        CK(cudaFuncSetAttribute(k_het_standin<NM>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+    auto smem_of = [&](int s) { return sizeof(double) * ((size_t)ctx->ht.total + (size_t)WY * 64 + 8 + (size_t)(WY / s) * 32 * (5 + 2 * NC * NM)); };
+    if (!ctx->hetn_attr) { // a context has one n_modes and one n_channels, so one instantiation
+        CK(cudaFuncSetAttribute(k_het_standin<NM, NC>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
         ctx->hetn_attr = true;
     }
     if (smem_of(WY) > 227 * 1024) return ctx->fail(LL_ERR_UNSUPPORTED, "heterodyne tables exceed shared memory (too many bins x modes)");
@@ -772,7 +811,7 @@ int launch_het_standin(ll_ctx *ctx, int64_t n_w, const double *params, double *l
             if (s > 1 && n_b / s < 8) break;
             if (smem_of(s) > 227 * 1024) continue;
             int bps = 0;
-            CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, k_het_standin<NM>, 32 * WY, smem_of(s)));
+            CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, k_het_standin<NM, NC>, 32 * WY, smem_of(s)));
             bps = std::max(1, bps);
             const int G = WY / s;
             const long long passes = ceil_div(n_groups, G);
@@ -785,12 +824,31 @@ int launch_het_standin(ll_ctx *ctx, int64_t n_w, const double *params, double *l
         ctx->hetn_key_total = ctx->ht.total;
     }
     const size_t smem = smem_of(S);
-    const int P = 5 + 2 * kNC * ctx->n_m;
+    const int P = 5 + 2 * NC * ctx->n_m;
     ProfScope prof(ctx, st);
-    k_het_standin<NM><<<grid, dim3(32, WY), smem, st>>>(ctx->ht, ctx->si, params, P, (int)n_w, n_groups, S,
-                                                          ctx->dd.as<double>(), logL, d_h, h_h);
+    k_het_standin<NM, NC><<<grid, dim3(32, WY), smem, st>>>(ctx->ht, ctx->si, params, P, (int)n_w, n_groups, S,
+                                                              ctx->dd.as<double>(), logL, d_h, h_h);
     LAUNCHED(ctx);
     return LL_OK;
+}
+
+template <int NC>
+int launch_het_standin_modes(ll_ctx *ctx, int64_t n_w, const double *params, double *logL, double *d_h, double *h_h,
+                             cudaStream_t st)
+{
+    switch (ctx->n_m) {
+    case 1:
+        if (ctx->ht1.base) return launch_het_standin1<NC>(ctx, n_w, params, logL, d_h, h_h, st);
+        return launch_het_standin<1, NC>(ctx, n_w, params, logL, d_h, h_h, st);
+    case 2: return launch_het_standin<2, NC>(ctx, n_w, params, logL, d_h, h_h, st);
+    case 3: return launch_het_standin<3, NC>(ctx, n_w, params, logL, d_h, h_h, st);
+    case 4: return launch_het_standin<4, NC>(ctx, n_w, params, logL, d_h, h_h, st);
+    case 5: return launch_het_standin<5, NC>(ctx, n_w, params, logL, d_h, h_h, st);
+    case 6: return launch_het_standin<6, NC>(ctx, n_w, params, logL, d_h, h_h, st);
+    case 7: return launch_het_standin<7, NC>(ctx, n_w, params, logL, d_h, h_h, st);
+    case 8: return launch_het_standin<8, NC>(ctx, n_w, params, logL, d_h, h_h, st);
+    default: return ctx->fail(LL_ERR_UNSUPPORTED, "n_modes");
+    }
 }
 
 } // namespace
@@ -800,13 +858,14 @@ int launch_het_standin(ll_ctx *ctx, int64_t n_w, const double *params, double *l
 // =====================================================================================================
 extern "C" {
 
-int ll_abi_version(void) { return 2; } // 2: ll_config.spline_bc, ll_standin_nodes band output, the SURVEY 8(f) entry points
+int ll_abi_version(void) { return 3; } // 3: n_channels 2 or 3 and ll_set_data w_shared (per-channel weights), t_shift on the array
+                                       // entry points, ll_standin_split_tc, ll_pt_run_het_fused
 
 int ll_create(const ll_config *cfg, ll_ctx **out)
 {
     if (!cfg || !out) return LL_ERR_ARG;
     *out = nullptr;
-    if (cfg->n_channels != LL_N_CHANNELS) return LL_ERR_UNSUPPORTED;
+    if (cfg->n_channels != 2 && cfg->n_channels != 3) return LL_ERR_UNSUPPORTED;
     if (cfg->n_modes < 1 || cfg->n_modes > LL_MAX_MODES) return LL_ERR_UNSUPPORTED;
     if (cfg->precision != LL_PREC_FP64 && cfg->precision != LL_PREC_FP32_ACC) return LL_ERR_UNSUPPORTED;
     if (cfg->spline_bc != LL_BC_NATURAL && cfg->spline_bc != LL_BC_NOT_A_KNOT) return LL_ERR_UNSUPPORTED;
@@ -836,6 +895,8 @@ int ll_create(const ll_config *cfg, ll_ctx **out)
     // default stand-in description: the (2,2) mode only, kappa = 1/2; overwritten by ll_standin_config
     ctx->si.n_m = ctx->n_m;
     ctx->si.kappa = 0.5;
+    ctx->si.n_c = ctx->n_c;
+    ctx->si.split_tc = 0;
     *out = ctx;
     return LL_OK;
 }
@@ -846,7 +907,7 @@ int ll_destroy(ll_ctx *ctx)
     {
         DeviceGuard dg(ctx->device);
         cudaDeviceSynchronize();
-        DevBuf *all[] = {&ctx->g4, &ctx->Wd, &ctx->dd_part, &ctx->dd, &ctx->pairs, &ctx->node_tab, &ctx->ilo_w, &ctx->ihi_w,
+        DevBuf *all[] = {&ctx->g, &ctx->Wc, &ctx->dd_part, &ctx->dd, &ctx->pairs, &ctx->node_tab, &ctx->ilo_w, &ctx->ihi_w,
                          &ctx->key_w, &ctx->hist, &ctx->perm, &ctx->ilo_s, &ctx->ihi_s, &ctx->Y, &ctx->C, &ctx->TF,
                          &ctx->part, &ctx->prow, &ctx->het_tab, &ctx->het_tab1, &ctx->het_raw, &ctx->het_idx, &ctx->het_fb,
                          &ctx->stage_in, &ctx->stage_out, &ctx->g4f, &ctx->Wf, &ctx->scale, &ctx->wmax, &ctx->ref_idx,
@@ -862,29 +923,40 @@ const char *ll_last_error(const ll_ctx *ctx) { return ctx ? ctx->err.c_str() : "
 
 int64_t ll_kernel_launches(const ll_ctx *ctx) { return ctx ? ctx->launches : 0; }
 
-int ll_set_data(ll_ctx *ctx, int64_t n_f, int64_t k_min, double df, const double *d, const double *W, void *stream)
+int ll_set_data(ll_ctx *ctx, int64_t n_f, int64_t k_min, double df, const double *d, const double *W, int32_t w_shared,
+                void *stream)
 {
     if (!ctx) return LL_ERR_ARG;
     if (!d || !W) return ctx->fail(LL_ERR_ARG, "d or W is NULL");
     if (n_f < 1 || n_f > (1LL << 30)) return ctx->fail(LL_ERR_ARG, "n_f out of range [1, 2^30]");
     if (k_min < 0 || !(df > 0.0) || !std::isfinite(df)) return ctx->fail(LL_ERR_ARG, "k_min < 0 or df not positive");
     if (k_min + n_f >= (1LL << 31)) return ctx->fail(LL_ERR_ARG, "k_min + n_f must stay below 2^31 (bin numbers are int32 on the device)");
+    if (ctx->precision == LL_PREC_FP32_ACC && (ctx->n_c != 2 || !w_shared))
+        return ctx->fail(LL_ERR_UNSUPPORTED, "the FP32-accumulate variant is built for two channels sharing one weight row");
     DeviceGuard dg(ctx->device);
     cudaStream_t st = (cudaStream_t)stream;
     ctx->have_data = false;
     ctx->have_het = false;
     ctx->nodes_valid = false;
     ctx->data_version += 1; // the cached frequency-tile tables and the bin -> interval table belong to the old grid
+    // weight rows kept: one for two channels sharing their PSD; otherwise one per channel (a shared row is replicated)
+    const int w_rows_in = w_shared ? 1 : ctx->n_c;
+    const int nw = (ctx->n_c == 2 && w_shared) ? 1 : ctx->n_c;
+    ctx->w_rows = nw;
     const long long n_pad = round_up(n_f, 512);
-    CK(ctx->g4.ensure(sizeof(double) * 4 * n_pad));
-    CK(ctx->Wd.ensure(sizeof(double) * n_pad));
+    CK(ctx->g.ensure(sizeof(double) * 2 * ctx->n_c * n_pad));
+    CK(ctx->Wc.ensure(sizeof(double) * nw * n_pad));
     CK(ctx->dd.ensure(sizeof(double) * 2));
     const int nb = std::min(1024, ceil_div(n_f, 256));
     CK(ctx->dd_part.ensure(sizeof(double) * 1024));
-    CK(cudaMemsetAsync(ctx->g4.as<double>() + 4 * n_f, 0, sizeof(double) * 4 * (n_pad - n_f), st));
-    CK(cudaMemsetAsync(ctx->Wd.as<double>() + n_f, 0, sizeof(double) * (n_pad - n_f), st));
+    CK(cudaMemsetAsync(ctx->g.as<double>() + 2 * ctx->n_c * n_f, 0, sizeof(double) * 2 * ctx->n_c * (n_pad - n_f), st));
+    for (int r = 0; r < nw; ++r)
+        CK(cudaMemsetAsync(ctx->Wc.as<double>() + (size_t)r * n_pad + n_f, 0, sizeof(double) * (n_pad - n_f), st));
     CK(cudaMemsetAsync(ctx->dd.p, 0, sizeof(double) * 2, st));
-    k_preweight<<<nb, 256, 0, st>>>(d, W, n_f, ctx->g4.as<double>(), ctx->Wd.as<double>(), ctx->dd_part.as<double>());
+#define LL_PREWEIGHT(NC) \
+    k_preweight<NC><<<nb, 256, 0, st>>>(d, W, w_rows_in, nw, n_f, n_pad, ctx->g.as<double>(), ctx->Wc.as<double>(), ctx->dd_part.as<double>())
+    LL_CHANNELS(ctx, LL_PREWEIGHT);
+#undef LL_PREWEIGHT
     LAUNCHED(ctx);
     k_sum_parts<<<1, 256, 0, st>>>(ctx->dd_part.as<double>(), nb, ctx->dd.as<double>());
     LAUNCHED(ctx);
@@ -898,7 +970,7 @@ int ll_set_data(ll_ctx *ctx, int64_t n_f, int64_t k_min, double df, const double
         LAUNCHED(ctx);
         k_scale_from_wmax<<<1, 1, 0, st>>>(ctx->wmax.as<unsigned long long>(), ctx->scale.as<double>());
         LAUNCHED(ctx);
-        k_prescale_f32<<<ceil_div(n_pad, 256), 256, 0, st>>>(ctx->g4.as<double>(), ctx->Wd.as<double>(), n_pad,
+        k_prescale_f32<<<ceil_div(n_pad, 256), 256, 0, st>>>(ctx->g.as<double>(), ctx->Wc.as<double>(), n_pad,
                                                              ctx->scale.as<double>(), ctx->g4f.as<float>(), ctx->Wf.as<double>());
         LAUNCHED(ctx);
     }
@@ -937,6 +1009,7 @@ int ll_standin_config(ll_ctx *ctx, int32_t n_modes, const int32_t *l, const int3
     ctx->si.n_m = n_modes;
     ctx->si.m_max = m_max;
     ctx->si.kappa = taper_kappa;
+    ctx->si.n_c = ctx->n_c;
     for (int i = 0; i < kMaxModes; ++i) {
         ctx->si.mode_m[i] = i < n_modes ? m[i] : 2;
         ctx->mode_l[i] = i < n_modes ? l[i] : 2;
@@ -948,8 +1021,16 @@ int ll_standin_config(ll_ctx *ctx, int32_t n_modes, const int32_t *l, const int3
     return LL_OK;
 }
 
+int ll_standin_split_tc(ll_ctx *ctx, int32_t on)
+{
+    if (!ctx) return LL_ERR_ARG;
+    ctx->si.split_tc = on ? 1 : 0;
+    return LL_OK;
+}
+
 int ll_full_batch(ll_ctx *ctx, int64_t n_w, int32_t n_nodes, const double *f_nodes, const double *amp, const double *phase,
-                  const double *tf, const double *band, double *logL, double *d_h, double *h_h, void *stream)
+                  const double *tf, const double *band, const double *t_shift, double *logL, double *d_h, double *h_h,
+                  void *stream)
 {
     int rc = check_full_common(ctx, n_w, f_nodes, logL);
     if (rc != LL_OK) return rc;
@@ -959,12 +1040,12 @@ int ll_full_batch(ll_ctx *ctx, int64_t n_w, int32_t n_nodes, const double *f_nod
     rc = prepare_nodes(ctx, n_nodes, f_nodes, st);
     if (rc != LL_OK) return rc;
     if (n_w == 0) return LL_OK;
-    return run_full(ctx, n_w, n_nodes, nullptr, amp, phase, tf, band, logL, d_h, h_h, st, false, nullptr);
+    return run_full(ctx, n_w, n_nodes, nullptr, amp, phase, tf, band, t_shift, logL, d_h, h_h, st, false, nullptr);
 }
 
 int ll_full_batch_pw(ll_ctx *ctx, int64_t n_w, int32_t n_nodes, const double *f_nodes_w, const double *amp,
-                     const double *phase, const double *tf, const double *band, double *logL, double *d_h, double *h_h,
-                     void *stream)
+                     const double *phase, const double *tf, const double *band, const double *t_shift, double *logL,
+                     double *d_h, double *h_h, void *stream)
 {
     if (!ctx) return LL_ERR_ARG;
     if (n_w < 0) return ctx->fail(LL_ERR_ARG, "n_w < 0");
@@ -976,12 +1057,12 @@ int ll_full_batch_pw(ll_ctx *ctx, int64_t n_w, int32_t n_nodes, const double *f_
     if (ctx->precision != LL_PREC_FP64) return ctx->fail(LL_ERR_UNSUPPORTED, "ll_full_batch_pw is FP64 only");
     if (n_w == 0) return LL_OK;
     DeviceGuard dg(ctx->device);
-    return run_full_pw(ctx, n_w, n_nodes, f_nodes_w, amp, phase, tf, band, logL, d_h, h_h, (cudaStream_t)stream);
+    return run_full_pw(ctx, n_w, n_nodes, f_nodes_w, amp, phase, tf, band, t_shift, logL, d_h, h_h, (cudaStream_t)stream);
 }
 
 int ll_full_batch_tf(ll_ctx *ctx, int64_t n_w, int32_t n_nodes, const double *f_nodes, const double *amp,
-                     const double *phase, const double *tf_nodes, const double *band, double *logL, double *d_h,
-                     double *h_h, void *stream)
+                     const double *phase, const double *tf_nodes, const double *band, const double *t_shift, double *logL,
+                     double *d_h, double *h_h, void *stream)
 {
     int rc = check_full_common(ctx, n_w, f_nodes, logL);
     if (rc != LL_OK) return rc;
@@ -992,7 +1073,7 @@ int ll_full_batch_tf(ll_ctx *ctx, int64_t n_w, int32_t n_nodes, const double *f_
     rc = prepare_nodes(ctx, n_nodes, f_nodes, st);
     if (rc != LL_OK) return rc;
     if (n_w == 0) return LL_OK;
-    return run_full(ctx, n_w, n_nodes, nullptr, amp, phase, nullptr, band, logL, d_h, h_h, st, false, nullptr, tf_nodes);
+    return run_full(ctx, n_w, n_nodes, nullptr, amp, phase, nullptr, band, t_shift, logL, d_h, h_h, st, false, nullptr, tf_nodes);
 }
 
 int ll_standin_nodes(ll_ctx *ctx, int64_t n_w, int32_t n_nodes, const double *f_nodes, const double *params,
@@ -1009,7 +1090,7 @@ int ll_standin_nodes(ll_ctx *ctx, int64_t n_w, int32_t n_nodes, const double *f_
     int rc = prepare_nodes(ctx, n_nodes, f_nodes, st);
     if (rc != LL_OK) return rc;
     if (n_w == 0) return LL_OK;
-    k_standin_nodes_out<<<(unsigned)n_w, 128, 0, st>>>(params, 5 + 2 * kNC * ctx->n_m, n_nodes, ctx->si, ctx->nt,
+    k_standin_nodes_out<<<(unsigned)n_w, 128, 0, st>>>(params, 5 + 2 * ctx->n_c * ctx->n_m, n_nodes, ctx->si, ctx->nt,
                                                         GridInfo{ctx->k_min, ctx->n_f, ctx->df}, amp, phase, band);
     LAUNCHED(ctx);
     return LL_OK;
@@ -1049,7 +1130,7 @@ int ll_full_batch_standin(ll_ctx *ctx, int64_t n_w, int32_t n_nodes, const doubl
     rc = prepare_nodes(ctx, n_nodes, f_nodes, st);
     if (rc != LL_OK) return rc;
     if (n_w == 0) return LL_OK;
-    return run_full(ctx, n_w, n_nodes, params, nullptr, nullptr, nullptr, nullptr, logL, d_h, h_h, st, false, nullptr);
+    return run_full(ctx, n_w, n_nodes, params, nullptr, nullptr, nullptr, nullptr, nullptr, logL, d_h, h_h, st, false, nullptr);
 }
 
 int ll_full_batch_standin_host(ll_ctx *ctx, int64_t n_w, int32_t n_nodes, const double *f_nodes, const double *params_host,
@@ -1061,7 +1142,7 @@ int ll_full_batch_standin_host(ll_ctx *ctx, int64_t n_w, int32_t n_nodes, const 
     if (!params_host) return ctx->fail(LL_ERR_ARG, "params_host is NULL");
     DeviceGuard dg(ctx->device);
     cudaStream_t st = (cudaStream_t)stream;
-    const size_t P = 5 + 2 * kNC * (size_t)ctx->n_m;
+    const size_t P = 5 + 2 * (size_t)ctx->n_c * (size_t)ctx->n_m;
     CK(ctx->stage_in.ensure(sizeof(double) * P * n_w));
     CK(ctx->stage_out.ensure(sizeof(double) * 3 * n_w));
     CK(cudaMemcpyAsync(ctx->stage_in.p, params_host, sizeof(double) * P * n_w, cudaMemcpyHostToDevice, st));
@@ -1086,12 +1167,12 @@ int ll_full_template_standin(ll_ctx *ctx, int32_t n_nodes, const double *f_nodes
     cudaStream_t st = (cudaStream_t)stream;
     int rc = prepare_nodes(ctx, n_nodes, f_nodes, st);
     if (rc != LL_OK) return rc;
-    const size_t P = 5 + 2 * kNC * (size_t)ctx->n_m;
+    const size_t P = 5 + 2 * (size_t)ctx->n_c * (size_t)ctx->n_m;
     CK(ctx->prow.ensure(sizeof(double) * P));
     CK(cudaMemcpyAsync(ctx->prow.p, params_row, sizeof(double) * P, cudaMemcpyHostToDevice, st));
     CK(cudaStreamSynchronize(st)); // params_row is pageable caller memory
-    return run_full(ctx, 1, n_nodes, ctx->prow.as<double>(), nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, st,
-                    true, h_out);
+    return run_full(ctx, 1, n_nodes, ctx->prow.as<double>(), nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr,
+                    nullptr, st, true, h_out);
 }
 
 int ll_template_standin(ll_ctx *ctx, const double *params_row, int64_t n_freq, const double *f, double f_lo, double f_hi,
@@ -1105,7 +1186,7 @@ int ll_template_standin(ll_ctx *ctx, const double *params_row, int64_t n_freq, c
     DeviceGuard dg(ctx->device);
     DirectRow row;
     memset(&row, 0, sizeof(row));
-    const int P = 5 + 2 * kNC * ctx->n_m;
+    const int P = 5 + 2 * ctx->n_c * ctx->n_m;
     memcpy(row.p, params_row, sizeof(double) * P);
     memcpy(row.c_lm, ctx->c_lm, sizeof(row.c_lm));
     k_template_direct<<<ceil_div(n_freq, 256), 256, 0, (cudaStream_t)stream>>>(row, ctx->si, n_freq, f, GridInfo{0, 0, 0.0},
@@ -1137,16 +1218,20 @@ int ll_het_prepare(ll_ctx *ctx, int32_t n_edges, const double *f_edges, const do
     es[n_b] = (int)first_bin_gt(f_edges[n_b], ctx->k_min, ctx->n_f, ctx->df);
     CK(ctx->het_idx.ensure(sizeof(int) * n_e));
     CK(ctx->het_fb.ensure(sizeof(double) * n_b));
-    CK(ctx->het_raw.ensure(sizeof(double) * 13 * n_b));
+    const int NR = 6 * ctx->n_c + 1; // raw sums per bin: per channel (A0r, A0i, A1r, A1i, B0, B1), then <d|d>
+    CK(ctx->het_raw.ensure(sizeof(double) * NR * n_b));
     CK(cudaMemcpyAsync(ctx->het_idx.p, es.data(), sizeof(int) * n_e, cudaMemcpyHostToDevice, st));
     CK(cudaMemcpyAsync(ctx->het_fb.p, fb.data(), sizeof(double) * n_b, cudaMemcpyHostToDevice, st));
     const GridInfo g{ctx->k_min, ctx->n_f, ctx->df};
-    k_het_prepare<<<n_b, 256, 0, st>>>(ctx->g4.as<double>(), ctx->Wd.as<double>(), h0_dense, g, ctx->het_idx.as<int>(),
-                                       ctx->het_fb.as<double>(), ctx->het_raw.as<double>());
+#define LL_HETPREP(NC)                                                                                                 \
+    k_het_prepare<NC><<<n_b, 256, 0, st>>>(ctx->g.as<double>(), ctx->Wc.as<double>(), ctx->w_rows, ctx->n_f_pad, h0_dense, g, \
+                                           ctx->het_idx.as<int>(), ctx->het_fb.as<double>(), ctx->het_raw.as<double>())
+    LL_CHANNELS(ctx, LL_HETPREP);
+#undef LL_HETPREP
     LAUNCHED(ctx);
-    ctx->raw_host.assign((size_t)13 * n_b, 0.0);
-    std::vector<double> h0e((size_t)kNC * n_e * 2);
-    CK(cudaMemcpyAsync(ctx->raw_host.data(), ctx->het_raw.p, sizeof(double) * 13 * n_b, cudaMemcpyDeviceToHost, st));
+    ctx->raw_host.assign((size_t)NR * n_b, 0.0);
+    std::vector<double> h0e((size_t)ctx->n_c * n_e * 2);
+    CK(cudaMemcpyAsync(ctx->raw_host.data(), ctx->het_raw.p, sizeof(double) * NR * n_b, cudaMemcpyDeviceToHost, st));
     CK(cudaMemcpyAsync(h0e.data(), h0_edges, sizeof(double) * h0e.size(), cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
     std::vector<double> tab;
@@ -1154,7 +1239,7 @@ int ll_het_prepare(ll_ctx *ctx, int32_t n_edges, const double *f_edges, const do
     if (rc != LL_OK) return rc;
     // <d|d> over the band: bins in a fixed order, compensated
     long double ddb = 0.0L;
-    for (int b = 0; b < n_b; ++b) ddb += (long double)ctx->raw_host[(size_t)b * 13 + 12];
+    for (int b = 0; b < n_b; ++b) ddb += (long double)ctx->raw_host[(size_t)b * NR + NR - 1];
     const double ddb_d = (double)ddb;
     CK(ctx->het_tab.ensure(sizeof(double) * tab.size()));
     CK(cudaMemcpyAsync(ctx->het_tab.p, tab.data(), sizeof(double) * tab.size(), cudaMemcpyHostToDevice, st));
@@ -1187,7 +1272,7 @@ int ll_het_refresh_standin(ll_ctx *ctx, int64_t n_w, const double *params, const
     if (!ctx->have_standin) return ctx->fail(LL_ERR_STATE, "ll_standin_config has not been called");
     DeviceGuard dg(ctx->device);
     cudaStream_t st = (cudaStream_t)stream;
-    const int P = 5 + 2 * kNC * ctx->n_m;
+    const int P = 5 + 2 * ctx->n_c * ctx->n_m;
     CK(ctx->ref_idx.ensure(sizeof(long long)));
     k_argmax<<<1, 1024, 0, st>>>(logL, (long long)n_w, ctx->ref_idx.as<long long>());
     LAUNCHED(ctx);
@@ -1212,9 +1297,9 @@ int ll_het_refresh_standin(ll_ctx *ctx, int64_t n_w, const double *params, const
     for (int j = 0; j < n_edges; ++j) e[j] = (double)std::exp(l0 + (l1 - l0) * (long double)j / (long double)(n_edges - 1));
     e[0] = f_first;
     e[n_edges - 1] = f_top;
-    CK(ctx->ref_dense.ensure(sizeof(double) * 2 * kNC * (size_t)ctx->n_f));
-    CK(ctx->ref_edges.ensure(sizeof(double) * (2 * kNC + 1) * (size_t)n_edges));
-    double *fe_dev = ctx->ref_edges.as<double>() + (size_t)2 * kNC * n_edges;
+    CK(ctx->ref_dense.ensure(sizeof(double) * 2 * ctx->n_c * (size_t)ctx->n_f));
+    CK(ctx->ref_edges.ensure(sizeof(double) * (2 * ctx->n_c + 1) * (size_t)n_edges));
+    double *fe_dev = ctx->ref_edges.as<double>() + (size_t)2 * ctx->n_c * n_edges;
     CK(cudaMemcpyAsync(fe_dev, e.data(), sizeof(double) * n_edges, cudaMemcpyHostToDevice, st));
     const GridInfo g{ctx->k_min, ctx->n_f, ctx->df};
     k_template_direct<<<ceil_div(ctx->n_f, 256), 256, 0, st>>>(row, ctx->si, ctx->n_f, nullptr, g, f_first, f_last,
@@ -1243,10 +1328,13 @@ int ll_het_audit_standin(ll_ctx *ctx, int64_t n_w, const double *params, double 
     DirectClm cl;
     memcpy(cl.c_lm, ctx->c_lm, sizeof(cl.c_lm));
     const GridInfo g{ctx->k_min, ctx->n_f, ctx->df};
-    k_het_audit<<<(unsigned)n_w, 256, 0, (cudaStream_t)stream>>>(params, 5 + 2 * kNC * ctx->n_m, cl, ctx->si,
-                                                                 ctx->g4.as<double>(), ctx->Wd.as<double>(), g,
-                                                                 ctx->het_idx.as<int>(), ctx->n_e - 1, ctx->dd.as<double>(),
-                                                                 logL, d_h, h_h);
+#define LL_AUDIT(NC)                                                                                                   \
+    k_het_audit<NC><<<(unsigned)n_w, 256, 0, (cudaStream_t)stream>>>(params, 5 + 2 * ctx->n_c * ctx->n_m, cl, ctx->si,   \
+                                                                     ctx->g.as<double>(), ctx->Wc.as<double>(), ctx->w_rows, \
+                                                                     ctx->n_f_pad, g, ctx->het_idx.as<int>(), ctx->n_e - 1, \
+                                                                     ctx->dd.as<double>(), logL, d_h, h_h)
+    LL_CHANNELS(ctx, LL_AUDIT);
+#undef LL_AUDIT
     LAUNCHED(ctx);
     return LL_OK;
 }
@@ -1256,10 +1344,10 @@ int ll_het_get_summary(ll_ctx *ctx, double *A0, double *A1, double *B0, double *
     (void)stream;
     if (!ctx) return LL_ERR_ARG;
     if (!ctx->have_het) return ctx->fail(LL_ERR_STATE, "ll_het_prepare has not been called");
-    const int n_b = ctx->n_e - 1;
-    for (int c = 0; c < kNC; ++c)
+    const int n_b = ctx->n_e - 1, NR = 6 * ctx->n_c + 1;
+    for (int c = 0; c < ctx->n_c; ++c)
         for (int b = 0; b < n_b; ++b) {
-            const double *r = &ctx->raw_host[(size_t)b * 13 + 6 * c];
+            const double *r = &ctx->raw_host[(size_t)b * NR + 6 * c];
             if (A0) { A0[((size_t)c * n_b + b) * 2] = r[0]; A0[((size_t)c * n_b + b) * 2 + 1] = r[1]; }
             if (A1) { A1[((size_t)c * n_b + b) * 2] = r[2]; A1[((size_t)c * n_b + b) * 2 + 1] = r[3]; }
             if (B0) B0[(size_t)c * n_b + b] = r[4];
@@ -1268,8 +1356,8 @@ int ll_het_get_summary(ll_ctx *ctx, double *A0, double *A1, double *B0, double *
     return LL_OK;
 }
 
-int ll_het_batch(ll_ctx *ctx, int64_t n_w, const double *amp_e, const double *phase_e, const double *tf, double *logL,
-                 double *d_h, double *h_h, void *stream)
+int ll_het_batch(ll_ctx *ctx, int64_t n_w, const double *amp_e, const double *phase_e, const double *tf, const double *t_shift,
+                 double *logL, double *d_h, double *h_h, void *stream)
 {
     int rc = het_check(ctx, n_w, logL);
     if (rc != LL_OK) return rc;
@@ -1279,15 +1367,20 @@ int ll_het_batch(ll_ctx *ctx, int64_t n_w, const double *amp_e, const double *ph
     const size_t smem = sizeof(double) * (size_t)ctx->ht.total;
     if (smem > 227 * 1024) return ctx->fail(LL_ERR_UNSUPPORTED, "heterodyne tables exceed shared memory");
     if (!ctx->heta_attr) {
-        CK(cudaFuncSetAttribute(k_het_arrays, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+#define LL_HETA_ATTR(NC) CK(cudaFuncSetAttribute(k_het_arrays<NC>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024))
+        LL_CHANNELS(ctx, LL_HETA_ATTR);
+#undef LL_HETA_ATTR
         ctx->heta_attr = true;
     }
     const int wpb = 8;
     int blocks_per_sm = std::max(1, std::min(8, (int)((220 * 1024) / std::max<size_t>(smem, 1))));
     const int grid = std::min(ceil_div(n_w, wpb), ctx->sm_count * blocks_per_sm);
     ProfScope prof(ctx, (cudaStream_t)stream);
-    k_het_arrays<<<grid, wpb * 32, smem, (cudaStream_t)stream>>>(ctx->ht, amp_e, phase_e, tf, (int)n_w, ctx->dd.as<double>(),
-                                                                  logL, d_h, h_h);
+#define LL_HETA(NC)                                                                                                       \
+    k_het_arrays<NC><<<grid, wpb * 32, smem, (cudaStream_t)stream>>>(ctx->ht, amp_e, phase_e, tf, t_shift, (int)n_w,       \
+                                                                      ctx->dd.as<double>(), logL, d_h, h_h)
+    LL_CHANNELS(ctx, LL_HETA);
+#undef LL_HETA
     LAUNCHED(ctx);
     return LL_OK;
 }
@@ -1301,19 +1394,8 @@ int ll_het_batch_standin(ll_ctx *ctx, int64_t n_w, const double *params, double 
     if (!params) return ctx->fail(LL_ERR_ARG, "params is NULL");
     DeviceGuard dg(ctx->device);
     cudaStream_t st = (cudaStream_t)stream;
-    switch (ctx->n_m) {
-    case 1:
-        if (ctx->ht1.base) return launch_het_standin1(ctx, n_w, params, logL, d_h, h_h, st);
-        return launch_het_standin<1>(ctx, n_w, params, logL, d_h, h_h, st);
-    case 2: return launch_het_standin<2>(ctx, n_w, params, logL, d_h, h_h, st);
-    case 3: return launch_het_standin<3>(ctx, n_w, params, logL, d_h, h_h, st);
-    case 4: return launch_het_standin<4>(ctx, n_w, params, logL, d_h, h_h, st);
-    case 5: return launch_het_standin<5>(ctx, n_w, params, logL, d_h, h_h, st);
-    case 6: return launch_het_standin<6>(ctx, n_w, params, logL, d_h, h_h, st);
-    case 7: return launch_het_standin<7>(ctx, n_w, params, logL, d_h, h_h, st);
-    case 8: return launch_het_standin<8>(ctx, n_w, params, logL, d_h, h_h, st);
-    default: return ctx->fail(LL_ERR_UNSUPPORTED, "n_modes");
-    }
+    if (ctx->n_c == 2) return launch_het_standin_modes<2>(ctx, n_w, params, logL, d_h, h_h, st);
+    return launch_het_standin_modes<3>(ctx, n_w, params, logL, d_h, h_h, st);
 }
 
 int ll_het_batch_standin_host(ll_ctx *ctx, int64_t n_w, const double *params_host, double *logL_host, double *d_h_host,
@@ -1325,7 +1407,7 @@ int ll_het_batch_standin_host(ll_ctx *ctx, int64_t n_w, const double *params_hos
     if (!params_host) return ctx->fail(LL_ERR_ARG, "params_host is NULL");
     DeviceGuard dg(ctx->device);
     cudaStream_t st = (cudaStream_t)stream;
-    const size_t P = 5 + 2 * kNC * (size_t)ctx->n_m;
+    const size_t P = 5 + 2 * (size_t)ctx->n_c * (size_t)ctx->n_m;
     CK(ctx->stage_in.ensure(sizeof(double) * P * n_w));
     CK(ctx->stage_out.ensure(sizeof(double) * 3 * n_w));
     CK(cudaMemcpyAsync(ctx->stage_in.p, params_host, sizeof(double) * P * n_w, cudaMemcpyHostToDevice, st));
@@ -1355,7 +1437,7 @@ int pt_half(ll_ctx *ctx, bool full, int32_t n_nodes, const double *f_nodes, int3
     if (!ctx->have_standin) return ctx->fail(LL_ERR_STATE, "ll_standin_config has not been called");
     DeviceGuard dg(ctx->device);
     cudaStream_t st = (cudaStream_t)stream;
-    const int P = 5 + 2 * kNC * ctx->n_m;
+    const int P = 5 + 2 * ctx->n_c * ctx->n_m;
     const int64_t np = (int64_t)n_t * (n_w / 2);
     CK(ctx->pt_y.ensure(sizeof(double) * (size_t)np * P));
     CK(ctx->pt_out.ensure(sizeof(double) * (size_t)np * 4));
@@ -1400,7 +1482,7 @@ int ll_pt_swap(ll_ctx *ctx, int32_t n_temps, int32_t n_walkers, double *x, doubl
     if (!x || !logL || !betas || (n_temps > 1 && !u_swap)) return ctx->fail(LL_ERR_ARG, "NULL argument");
     if (n_temps == 1) return LL_OK;
     DeviceGuard dg(ctx->device);
-    const int P = 5 + 2 * kNC * ctx->n_m;
+    const int P = 5 + 2 * ctx->n_c * ctx->n_m;
     if (n_temps <= 32 && P <= 64)
         k_pt_swap_warp<<<(int)ceil_div(n_walkers, 4), 128, 0, (cudaStream_t)stream>>>(x, logL, d_h, h_h, n_temps, n_walkers, P,
                                                                                      betas, u_swap, swapped);

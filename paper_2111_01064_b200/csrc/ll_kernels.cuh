@@ -2,12 +2,15 @@
 //
 // Device layouts ("sorted position" p = index of a walker after the band-top counting sort; n_wp = n_w
 // rounded up to the walker-block size):
-//   g4   [n_f_pad][4]   W_i * conj(d^c_i): (A re, A im, E re, E im); im already negated          (F0)
-//   Wd   [n_f_pad]      W_i, zero in the padding
+//   g    [n_f_pad][2 NC]  W^c_i * conj(d^c_i): (re, im) per channel c = A, E(, T); im already negated       (F0)
+//   Wc   [NW][n_f_pad]    W^c_i, zero in the padding; NW = 1 (one row shared by all channels) or NC (one per channel)
 //   Y    [n_m*2][n_nodes][n_wp]   node values, sys = 2 m + kind (0 amplitude, 1 phase in quarter cycles)
 //   C    [n_nodes-1][n_m][8][n_wp] cubic coefficients per interval: (y, b, c, d) amplitude, then phase
-//   TF   [n_m][2][2][n_wp]         transfer factors T^c_m (re, im)
+//   TF   [n_m][NC][2][n_wp]        transfer factors T^c_m (re, im)
 //   part [n_tiles][NQ][n_wp]       per-(frequency tile, walker) partial sums
+// Kernels that touch the data tile or the channels are templates on NC (2: A, E; 3: A, E, T — Eq. 3 sums over all
+// three) and, where the weights enter, on WS (true: one weight row for every channel, "A=E identical";
+// false: one row per channel, "T different").
 #pragma once
 #include <limits.h>
 #include "ll_device.cuh"
@@ -15,7 +18,7 @@
 namespace ll {
 
 constexpr int kMaxModes = 8;
-constexpr int kNC = 2;
+constexpr int kMaxNC = 3;
 
 // ---------------------------------------------------------------------------------------------------
 // F0: pre-weighted data and <d|d>          (Eq. 3; "we transform the data")
@@ -35,19 +38,25 @@ __device__ __forceinline__ double block_sum_256(double v, double *sh)
     return r; // valid in warp 0
 }
 
-__global__ void __launch_bounds__(256) k_preweight(const double *__restrict__ d, const double *__restrict__ W,
-                                                   long long n_f, double *__restrict__ g4,
-                                                   double *__restrict__ Wd, double *__restrict__ dd_part)
+template <int NC>
+__global__ void __launch_bounds__(256) k_preweight(const double *__restrict__ d, const double *__restrict__ W, int w_rows,
+                                                   int nw_out, long long n_f, long long n_f_pad, double *__restrict__ g,
+                                                   double *__restrict__ Wc, double *__restrict__ dd_part)
 {
+    // d [NC][n_f][2]; W [w_rows][n_f], w_rows = 1 (shared) or NC; g [n_f_pad][2 NC]; Wc [nw_out][n_f_pad] (nw_out = 1
+    // needs w_rows = 1; nw_out = NC with w_rows = 1 replicates the row)
     __shared__ double sh[8];
     double acc = 0.0, comp = 0.0; // Neumaier-compensated per-thread sum
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n_f; i += (long long)gridDim.x * blockDim.x) {
-        const double w = W[i];
-        const double2 a = reinterpret_cast<const double2 *>(d)[i];
-        const double2 e = reinterpret_cast<const double2 *>(d)[n_f + i];
-        reinterpret_cast<double4 *>(g4)[i] = make_double4(w * a.x, -(w * a.y), w * e.x, -(w * e.y));
-        Wd[i] = w;
-        const double term = w * (a.x * a.x + a.y * a.y + e.x * e.x + e.y * e.y);
+        double term = 0.0;
+#pragma unroll
+        for (int c = 0; c < NC; ++c) {
+            const double w = W[(w_rows > 1 ? (long long)c * n_f : 0) + i];
+            const double2 a = reinterpret_cast<const double2 *>(d)[(long long)c * n_f + i];
+            reinterpret_cast<double2 *>(g)[i * NC + c] = make_double2(w * a.x, -(w * a.y));
+            if (c < nw_out) Wc[(long long)c * n_f_pad + i] = w;
+            term = fma(w, a.x * a.x + a.y * a.y, term);
+        }
         const double t = acc + term;
         comp += (fabs(acc) >= fabs(term)) ? ((acc - t) + term) : ((term - t) + acc);
         acc = t;
@@ -80,6 +89,9 @@ struct StandinInfo {
     int m_max;
     int mode_m[kMaxModes];
     double kappa;
+    int n_c;      // channels: a parameter row is Mc, q, t_c, phi_c, 1/D, then T^c_m (re, im) mode-major, channel-minor
+    int split_tc; // 1: the full-grid node phases are built WITHOUT the linear term 2 pi f t_c, which travels as
+                  // t_shift = t_c outside the spline (reading R32)
 };
 
 __device__ __forceinline__ void standin_masses(double Mc, double q, double &Mtot, double &eta, double &f_isco)
@@ -179,8 +191,9 @@ k_band_sort_small(int use_standin, const double *__restrict__ params, int P, con
     }
 }
 
-// exclusive scan of hist[0..n) in place (single block of 1024 threads, n <= 1024*8)
-__global__ void __launch_bounds__(1024) k_scan_hist(int *__restrict__ hist, int n)
+// exclusive scan of hist[0..n) in place (single block of 1024 threads, n <= 1024*8); starts[0..n] keeps a copy of the
+// bucket starts (starts[n] = total), since k_scatter uses hist as its cursors
+__global__ void __launch_bounds__(1024) k_scan_hist(int *__restrict__ hist, int n, int *__restrict__ starts)
 {
     __shared__ int wsum[32];
     const int per = (n + 1023) / 1024;
@@ -217,25 +230,70 @@ __global__ void __launch_bounds__(1024) k_scan_hist(int *__restrict__ hist, int 
     for (int k = 0; k < 8; ++k)
         if (k < per && b + k < n) {
             hist[b + k] = run;
+            starts[b + k] = run;
             run += loc[k];
         }
+    if (threadIdx.x == 1023) starts[n] = wsum[31];
 }
 
-// scatter walkers to sorted positions; padding positions get perm = -1 and an empty band
+// scatter walkers into their key buckets (order inside a bucket = order of the atomics: NOT reproducible) ...
 __global__ void __launch_bounds__(256)
-k_scatter(int n_w, int n_wp, const int *__restrict__ key_w, const int *__restrict__ ilo_w, const int *__restrict__ ihi_w,
-          int *__restrict__ offs, int *__restrict__ perm, int *__restrict__ ilo_s, int *__restrict__ ihi_s)
+k_scatter(int n_w, const int *__restrict__ key_w, int *__restrict__ offs, int *__restrict__ bucket)
 {
     const int w = blockIdx.x * blockDim.x + threadIdx.x;
-    if (w < n_w) {
-        const int pos = atomicAdd(&offs[key_w[w]], 1);
-        perm[pos] = w;
-        ilo_s[pos] = ilo_w[w];
-        ihi_s[pos] = ihi_w[w];
-    } else if (w < n_wp) {
-        perm[w] = -1;
-        ilo_s[w] = 0;
-        ihi_s[w] = 0;
+    if (w < n_w) bucket[atomicAdd(&offs[key_w[w]], 1)] = w;
+}
+// ... and put every bucket into walker order (rank = number of smaller walker indices in the bucket; buckets hold a
+// few walkers each), so that the sorted order — hence which walkers share a warp, hence every rounding — is a pure
+// function of the inputs and reruns are bit-identical.  One block per bucket; padding positions get perm = -1 and
+// an empty band.
+constexpr int kSortThreads = 128;
+__global__ void __launch_bounds__(kSortThreads)
+k_sort_buckets(int n_w, int n_wp, int n_keys, const int *__restrict__ starts, const int *__restrict__ bucket,
+               const int *__restrict__ key_w, const int *__restrict__ ilo_w, const int *__restrict__ ihi_w,
+               int *__restrict__ perm, int *__restrict__ ilo_s, int *__restrict__ ihi_s)
+{
+    __shared__ int wtot[kSortThreads / 32];
+    const int b = blockIdx.x;
+    if (b == n_keys) { // one extra block for the padding
+        for (int p = n_w + threadIdx.x; p < n_wp; p += blockDim.x) { perm[p] = -1; ilo_s[p] = 0; ihi_s[p] = 0; }
+        return;
+    }
+    const int s0 = starts[b], s1 = starts[b + 1];
+    if (s1 - s0 <= 256) {
+        for (int e = s0 + threadIdx.x; e < s1; e += blockDim.x) {
+            const int w = bucket[e];
+            int rank = 0;
+            for (int k = s0; k < s1; ++k) rank += bucket[k] < w;
+            perm[s0 + rank] = w;
+            ilo_s[s0 + rank] = ilo_w[w];
+            ihi_s[s0 + rank] = ihi_w[w];
+        }
+        return;
+    }
+    // a big bucket (e.g. every walker with the whole grid as its band): one pass over all walkers in index order,
+    // position = start + number of earlier walkers with this key (block-wide running count)
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    int base = s0;
+    for (int w0 = 0; w0 < n_w; w0 += kSortThreads) {
+        const int w = w0 + threadIdx.x;
+        const bool mine = w < n_w && key_w[w] == b;
+        const unsigned m = __ballot_sync(0xffffffffu, mine);
+        if (lane == 0) wtot[wid] = __popc(m);
+        __syncthreads();
+        int before = __popc(m & ((1u << lane) - 1u)), total = 0;
+#pragma unroll
+        for (int k = 0; k < kSortThreads / 32; ++k) {
+            if (k < wid) before += wtot[k];
+            total += wtot[k];
+        }
+        if (mine) {
+            perm[base + before] = w;
+            ilo_s[base + before] = ilo_w[w];
+            ihi_s[base + before] = ihi_w[w];
+        }
+        base += total;
+        __syncthreads();
     }
 }
 
@@ -313,15 +371,16 @@ k_nodes_standin(const double *__restrict__ params, int P, const int *__restrict_
             if (w >= 0) {
                 const size_t t = (size_t)m * n_nodes + j;
                 a = nt.cfp[t] * c.invD * taper(nt.f2m[t] * c.inv_fisco, si.kappa, inv_kappa);
-                y = fma(nt.f4[j], c.tc, fma(Kq, nt.fm53[t], -phq));
+                y = fma(Kq, nt.fm53[t], -phq);
+                if (!si.split_tc) y = fma(nt.f4[j], c.tc, y);
             }
             ya[(size_t)j * n_wp] = a;
             yp[(size_t)j * n_wp] = y;
         }
         if (blockIdx.y == 0) {
-#pragma unroll
-            for (int q = 0; q < 4; ++q)
-                TF[((size_t)m * 4 + q) * n_wp + p] = (w >= 0) ? row[5 + m * 4 + q] : 0.0;
+            const int nq = 2 * si.n_c;
+            for (int q = 0; q < nq; ++q)
+                TF[((size_t)m * nq + q) * n_wp + p] = (w >= 0) ? row[5 + m * nq + q] : 0.0;
         }
     }
 }
@@ -351,7 +410,9 @@ k_standin_nodes_out(const double *__restrict__ params, int P, int n_nodes, Stand
             const size_t t = (size_t)m * n_nodes + j;
             const size_t o = (w * si.n_m + m) * n_nodes + j;
             amp[o] = nt.cfp[t] * c.invD * taper(nt.f2m[t] * c.inv_fisco, si.kappa, inv_kappa);
-            phase[o] = fma(nt.f4[j], c.tc, fma(Kq, nt.fm53[t], -phq)) * kPio2_1; // quarter cycles -> radians
+            double y = fma(Kq, nt.fm53[t], -phq);
+            if (!si.split_tc) y = fma(nt.f4[j], c.tc, y);
+            phase[o] = y * kPio2_1; // quarter cycles -> radians
         }
     }
 }
@@ -359,7 +420,7 @@ k_standin_nodes_out(const double *__restrict__ params, int P, int n_nodes, Stand
 // F1 (array entry point): transpose caller arrays [n_w][n_m][n_nodes] into Y; phase radians -> quarter cycles
 __global__ void __launch_bounds__(256)
 k_nodes_arrays(const double *__restrict__ amp, const double *__restrict__ phase, const double *__restrict__ tf,
-               const int *__restrict__ perm, int n_wp, int n_nodes, int n_m, double *__restrict__ Y,
+               const int *__restrict__ perm, int n_wp, int n_nodes, int n_m, int n_c, double *__restrict__ Y,
                double *__restrict__ TF)
 {
     __shared__ double ta[32][33], tp[32][33];
@@ -388,21 +449,22 @@ k_nodes_arrays(const double *__restrict__ amp, const double *__restrict__ phase,
     }
     if (blockIdx.y == 0 && threadIdx.x < 32) {
         const int w = perm[p0 + tx];
-#pragma unroll
-        for (int q = 0; q < 4; ++q)
-            TF[((size_t)m * 4 + q) * n_wp + p0 + tx] = (w >= 0) ? tf[((size_t)w * n_m + m) * 4 + q] : 0.0;
+        const int nq = 2 * n_c;
+        for (int q = 0; q < nq; ++q)
+            TF[((size_t)m * nq + q) * n_wp + p0 + tx] = (w >= 0) ? tf[((size_t)w * n_m + m) * nq + q] : 0.0;
     }
 }
 
-// F1 (array entry point with a frequency-dependent transfer function, Eq. 8-9): six splines per mode,
-// sys = 6 m + s with s = 0 amplitude, 1 phase (radians -> quarter cycles), 2 + 2c Re T^c, 3 + 2c Im T^c;
+// F1 (array entry point with a frequency-dependent transfer function, Eq. 8-9): ns = 2 + 2 n_c splines per mode,
+// sys = ns m + s with s = 0 amplitude, 1 phase (radians -> quarter cycles), 2 + 2c Re T^c, 3 + 2c Im T^c;
 // tf_nodes is [n_w][n_m][n_c][n_nodes][2].  One 32 x 32 transpose tile per block, blockIdx.z = sys.
 __global__ void __launch_bounds__(256)
 k_nodes_arrays_tf(const double *__restrict__ amp, const double *__restrict__ phase, const double *__restrict__ tf_nodes,
-                  const int *__restrict__ perm, int n_wp, int n_nodes, int n_m, double *__restrict__ Y)
+                  const int *__restrict__ perm, int n_wp, int n_nodes, int n_m, int n_c, double *__restrict__ Y)
 {
     __shared__ double tt[32][33];
-    const int sys = blockIdx.z, m = sys / 6, s = sys % 6;
+    const int ns = 2 + 2 * n_c;
+    const int sys = blockIdx.z, m = sys / ns, s = sys % ns;
     const int p0 = blockIdx.x * 32, j0 = blockIdx.y * 32;
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5; // 32 x 8
     for (int r = ty; r < 32; r += 8) {
@@ -413,7 +475,7 @@ k_nodes_arrays_tf(const double *__restrict__ amp, const double *__restrict__ pha
             const size_t wm = (size_t)w * n_m + m;
             if (s == 0) v = amp[wm * n_nodes + j];
             else if (s == 1) v = phase[wm * n_nodes + j] * kTwoOverPi;
-            else v = tf_nodes[((wm * kNC + ((s - 2) >> 1)) * n_nodes + j) * 2 + ((s - 2) & 1)];
+            else v = tf_nodes[((wm * n_c + ((s - 2) >> 1)) * n_nodes + j) * 2 + ((s - 2) & 1)];
         }
         tt[r][tx] = v;
     }
@@ -437,7 +499,7 @@ constexpr int kSplineBlk = 16;
 __global__ void __launch_bounds__(128)
 k_spline(const double *__restrict__ Y, double *__restrict__ C, int n_wp, int n_nodes, int n_m, int ns, NodeTables nt)
 {
-    // ns = splines per mode: 2 (amplitude, phase) or 6 (+ Re/Im of T^A, T^E: frequency-dependent transfer function)
+    // ns = splines per mode: 2 (amplitude, phase) or 2 + 2 n_c (+ Re/Im of every T^c: frequency-dependent transfer function)
     const int p = blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= n_wp) return;
     const int sys = blockIdx.y, m = sys / ns, kind = sys % ns;
@@ -625,23 +687,27 @@ k_spline_block(const double *__restrict__ Y, double *__restrict__ C, int n_wp, i
 
 // ---------------------------------------------------------------------------------------------------
 // F3: fused spline evaluation / channel response / inner products           (Eq. 3, 7, 9)
-// One thread = one walker; a warp = 32 walkers walking the SAME dense bins, so the data tile (g4, W) is a
-// shared-memory broadcast and no cross-thread reduction exists.  Tiles of g4/W arrive by 1-D bulk TMA into
+// One thread = one walker; a warp = 32 walkers walking the SAME dense bins, so the data tile (g, W) is a
+// shared-memory broadcast and no cross-thread reduction exists.  Tiles of g/W arrive by 1-D bulk TMA into
 // a two-stage ring guarded by mbarriers.  The dense template is never written anywhere.
 // Single-mode specialisation: T^c is constant per walker, so the kernel accumulates the complex sums
 // S^c = sum_i g^c_i A e^{-i Psi} and H = sum_i W_i A^2; k_finalize applies T^c.
 // ---------------------------------------------------------------------------------------------------
 struct FusedArgs {
-    const double *g4;
-    const double *Wd;
+    const double *g;       // [n_f_pad][2 NC]
+    const double *Wc;      // [NW][n_f_pad]
     const double *C;
     const double *TF;
     const double *xj;
     const int *bstart;
     const int *ilo;
     const int *ihi;
+    const int *perm;       // sorted position -> walker index (t_shift is in the caller's order), -1 in the padding
+    const double *t_shift; // t_shift of walker w at t_shift[w * ts_stride] (seconds), or nullptr:
+    int ts_stride;         // Psi_m(f) = spline_m(f) + 2 pi f t_shift (reading R32); the stand-in passes params + 2, P
     double *part;
     long long k_min;
+    long long n_f_pad;     // row stride of Wc
     double df;
     const int *tile_start; // [n_tiles + 1]: frequency tile t covers dense bins [tile_start[t], tile_start[t+1])
     int n_f, n_wp, n_nodes, n_m, TB, CH;
@@ -669,6 +735,121 @@ __device__ __forceinline__ int find_interval_of_bin(const int *__restrict__ bsta
     return lo;
 }
 
+// One stage of the data ring in shared memory: the g tile [CH][2 NC], then NW weight rows [CH] — (2 NC + NW) doubles
+// per bin, 1 + NW bulk copies per stage, all completing on the stage's mbarrier.
+template <int NC, bool WS>
+struct Tile {
+    static constexpr int NW = WS ? 1 : NC;
+    static constexpr int DPB = 2 * NC + NW; // doubles per bin
+    __device__ static __forceinline__ void issue(const FusedArgs &a, double *dst, int c, int CH, uint64_t *bar)
+    {
+        mbar_expect_tx(bar, (uint32_t)CH * 8u * DPB);
+        tma_load_1d(dst, a.g + (size_t)c * CH * 2 * NC, (uint32_t)CH * 16u * NC, bar);
+#pragma unroll
+        for (int r = 0; r < NW; ++r)
+            tma_load_1d(dst + (size_t)CH * (2 * NC + r), a.Wc + (size_t)r * a.n_f_pad + (size_t)c * CH, (uint32_t)CH * 8u, bar);
+    }
+};
+
+// g of bin ii from a tile pointer that has been moved back by the tile's first bin (sgc = tile - cb * 2 NC)
+template <int NC>
+__device__ __forceinline__ void load_g(const double *__restrict__ sgc, int ii, double (&g)[2 * NC])
+{
+    if (NC == 2) {
+        const double4 v = reinterpret_cast<const double4 *>(sgc)[ii];
+        g[0] = v.x; g[1] = v.y; g[2] = v.z; g[3] = v.w;
+    } else {
+#pragma unroll
+        for (int c = 0; c < NC; ++c) {
+            const double2 v = reinterpret_cast<const double2 *>(sgc)[ii * NC + c];
+            g[2 * c] = v.x; g[2 * c + 1] = v.y;
+        }
+    }
+}
+
+// accumulators of the single-mode kernel: S^c = sum_i g^c_i A e^{-i Psi} (complex, per channel) and
+// H = sum_i W_i A^2 (one for a shared weight row, one per channel otherwise); k_finalize applies T^c.
+template <int NC, bool WS>
+struct Acc1 {
+    static constexpr int NW = WS ? 1 : NC;
+    double S[2 * NC];
+    double H[NW];
+    __device__ __forceinline__ void zero()
+    {
+#pragma unroll
+        for (int q = 0; q < 2 * NC; ++q) S[q] = 0.0;
+#pragma unroll
+        for (int q = 0; q < NW; ++q) H[q] = 0.0;
+    }
+    // h = u - i v = A e^{-i Psi} at bin ii
+    __device__ __forceinline__ void add(const double *__restrict__ sgc, const double *__restrict__ sWc, int CH, int ii,
+                                        double u, double v, double A)
+    {
+        double g[2 * NC];
+        load_g<NC>(sgc, ii, g);
+#pragma unroll
+        for (int c = 0; c < NC; ++c) {
+            S[2 * c] = fma(g[2 * c], u, S[2 * c]); S[2 * c] = fma(g[2 * c + 1], v, S[2 * c]);
+            S[2 * c + 1] = fma(g[2 * c + 1], u, S[2 * c + 1]); S[2 * c + 1] = fma(-g[2 * c], v, S[2 * c + 1]);
+        }
+        if (WS) {
+            H[0] = fma(sWc[ii] * A, A, H[0]);
+        } else {
+            const double A2 = A * A;
+#pragma unroll
+            for (int c = 0; c < NC; ++c) H[c] = fma(sWc[c * CH + ii], A2, H[c]);
+        }
+    }
+};
+
+// <d|h> and <h|h> contributions of one bin given the channel responses h^c = (hr, hi) (kernels that apply T^c per bin)
+template <int NC, bool WS>
+__device__ __forceinline__ void accumulate_bin(const double *__restrict__ sgc, const double *__restrict__ sWc, int CH, int ii,
+                                               const double (&h)[2 * NC], double &s_dh, double &s_hh)
+{
+    double g[2 * NC];
+    load_g<NC>(sgc, ii, g);
+#pragma unroll
+    for (int c = 0; c < NC; ++c) {
+        s_dh = fma(g[2 * c], h[2 * c], s_dh);
+        s_dh = fma(-g[2 * c + 1], h[2 * c + 1], s_dh);
+    }
+    if (WS) {
+        double q = fma(h[0], h[0], h[1] * h[1]);
+#pragma unroll
+        for (int c = 1; c < NC; ++c) q += fma(h[2 * c], h[2 * c], h[2 * c + 1] * h[2 * c + 1]);
+        s_hh = fma(sWc[ii], q, s_hh);
+    } else {
+#pragma unroll
+        for (int c = 0; c < NC; ++c)
+            s_hh = fma(sWc[c * CH + ii], fma(h[2 * c], h[2 * c], h[2 * c + 1] * h[2 * c + 1]), s_hh);
+    }
+}
+
+// h^c += T^c (u - i v) for every channel; T^c = (tf[2c], tf[2c+1])
+template <int NC>
+__device__ __forceinline__ void apply_tf(const double (&tf)[2 * NC], double u, double v, double (&h)[2 * NC])
+{
+#pragma unroll
+    for (int c = 0; c < NC; ++c) {
+        h[2 * c] = fma(tf[2 * c], u, h[2 * c]); h[2 * c] = fma(tf[2 * c + 1], v, h[2 * c]);
+        h[2 * c + 1] = fma(tf[2 * c + 1], u, h[2 * c + 1]); h[2 * c + 1] = fma(-tf[2 * c], v, h[2 * c + 1]);
+    }
+}
+
+// Linear phase term outside the spline (reading R32): Psi(f) = spline(f) + 2 pi f t_shift, i.e. 4 f t_shift quarter
+// cycles.  It is folded into the phase cubic of the current interval: with f = x_j + t,
+//   c0 += 4 t_shift x_j (taken modulo one cycle: e^{-i Psi} does not see whole cycles),   c1 += 4 t_shift,
+// so neither route pays anything per bin.  The product is formed exactly (hi + lo by FMA) and the whole cycles are
+// removed from hi before the sum, so the large linear phase (1e7 quarter cycles at the top of a one-year band) never
+// costs the low bits of the small splined one.
+__device__ __forceinline__ double qc_linear_mod_cycle(double x, double ts4 /* 4 t_shift */)
+{
+    const double hi = ts4 * x, lo = fma(ts4, x, -hi);
+    const double n4 = 4.0 * rint(0.25 * hi); // whole cycles, in quarter cycles; hi - n4 is exact
+    return (hi - n4) + lo;
+}
+
 #ifndef LL_FUSED_UNROLL
 #define LL_FUSED_UNROLL 3 // bins in flight per thread in the hot loop (tuned on B200, profiles/)
 #endif
@@ -676,14 +857,13 @@ __device__ __forceinline__ int find_interval_of_bin(const int *__restrict__ bsta
 #define LL_FUSED_MINB 4 // resident 128-thread blocks per SM the register budget is held to
 #endif
 constexpr int kFusedUnroll = LL_FUSED_UNROLL;
-// bins [b0, b1) of one spline interval for the single-mode kernel: t, the two cubics, A e^{-i Psi}, the two
-// complex MACs with g^A, g^E and W A^2.  MASK = per-lane band test (only at the ragged ends of a warp's band).
-template <bool MASK>
+// bins [b0, b1) of one spline interval for the single-mode kernel: t, the two cubics, A e^{-i Psi}, the complex MACs
+// with g^c and W A^2.  MASK = per-lane band test (only at the ragged ends of a warp's band).
+template <bool MASK, int NC, bool WS>
 __device__ __forceinline__ void fused_bins_nm1(int b0, int b1, int tlo, int thi, int kbase, double df, double nxj,
                                                double cA0, double cA1, double cA2, double cA3, double cP0, double cP1,
-                                               double cP2, double cP3, const double4 *__restrict__ sg4,
-                                               const double *__restrict__ sWc, double &sAr, double &sAi, double &sEr,
-                                               double &sEi, double &sH)
+                                               double cP2, double cP3, const double *__restrict__ sgc,
+                                               const double *__restrict__ sWc, int CH, Acc1<NC, WS> &acc)
 {
 #pragma unroll kFusedUnroll
     for (int ii = b0; ii < b1; ++ii) {
@@ -693,13 +873,7 @@ __device__ __forceinline__ void fused_bins_nm1(int b0, int b1, int tlo, int thi,
         if (MASK) A = ((ii >= tlo) && (ii < thi)) ? A : 0.0;
         double u, v; // h = u - i v
         amp_expi_qc(A, y, u, v);
-        const double4 g = sg4[ii];
-        const double w = sWc[ii];
-        sAr = fma(g.x, u, sAr); sAr = fma(g.y, v, sAr);
-        sAi = fma(g.y, u, sAi); sAi = fma(-g.x, v, sAi);
-        sEr = fma(g.z, u, sEr); sEr = fma(g.w, v, sEr);
-        sEi = fma(g.w, u, sEi); sEi = fma(-g.z, v, sEi);
-        sH = fma(w * A, A, sH);
+        acc.add(sgc, sWc, CH, ii, u, v, A);
     }
 }
 
@@ -709,8 +883,9 @@ __device__ __forceinline__ void fused_bins_nm1(int b0, int b1, int tlo, int thi,
 // and the amplitude cubic by its forward differences; every kRotSync bins everything is re-evaluated from the cubic
 // coefficients (the exact route above), which bounds the accumulated rounding: with D1 Psi <= a few quarter cycles
 // known to 1 ulp, the phase drifts by < kRotSync^2/2 ulp ~ 1e-13 quarter cycles between re-syncs, far below the
-// rounding of Psi itself (1e-9 at 1e7 quarter cycles).  Per bin: 12 (rotations) + 3 (amplitude) + 2 (A z) + 8
-// (MACs) + 2 (W A^2) = 27 FP64 instructions and no sincos, no quadrant fix-up, no bin-number conversion, instead of
+// rounding of Psi itself (1e-9 at 1e7 quarter cycles).  Per bin: 12 (rotations) + 3 (amplitude) + 2 (A z) + 4 NC
+// (MACs) + 2 (W A^2; 1 + NC with per-channel weights) = 27 FP64 instructions for two channels and a shared weight row
+// (33 for three channels with their own rows), no sincos, no quadrant fix-up, no bin-number conversion, instead of
 // 34 + 18 others.
 #ifndef LL_FUSED_ROT
 #define LL_FUSED_ROT 1
@@ -734,10 +909,11 @@ __device__ __forceinline__ void unit_modulus(double &c, double &s)
     c *= k;
     s *= k;
 }
+template <int NC, bool WS>
 __device__ __forceinline__ void fused_bins_rot(int b0, int b1, int kbase, double df, double nxj, double cA0, double cA1,
                                                double cA2, double cA3, double cP0, double cP1, double cP2, double cP3,
-                                               const double4 *__restrict__ sg4, const double *__restrict__ sWc,
-                                               double &sAr, double &sAi, double &sEr, double &sEi, double &sH)
+                                               const double *__restrict__ sgc, const double *__restrict__ sWc, int CH,
+                                               Acc1<NC, WS> &acc)
 {
     const double df2 = df * df, df3 = df2 * df;
     const double d3A = 6.0 * cA3 * df3;
@@ -762,13 +938,7 @@ __device__ __forceinline__ void fused_bins_rot(int b0, int b1, int kbase, double
 #pragma unroll kRotUnroll
         for (int ii = k0; ii < k1; ++ii) {
             const double u = A * cz, v = A * sz; // h = u - i v
-            const double4 g = sg4[ii];
-            const double w = sWc[ii];
-            sAr = fma(g.x, u, sAr); sAr = fma(g.y, v, sAr);
-            sAi = fma(g.y, u, sAi); sAi = fma(-g.x, v, sAi);
-            sEr = fma(g.z, u, sEr); sEr = fma(g.w, v, sEr);
-            sEi = fma(g.w, u, sEi); sEi = fma(-g.z, v, sEi);
-            sH = fma(w * A, A, sH);
+            acc.add(sgc, sWc, CH, ii, u, v, A);
             const double nzc = fma(cz, cw, -(sz * sw)), nzs = fma(sz, cw, cz * sw);
             const double nwc = fma(cw, cv, -(sw * sv)), nws = fma(sw, cv, cw * sv);
             const double nvc = fma(cv, cu, -(sv * su)), nvs = fma(sv, cu, cv * su);
@@ -778,9 +948,11 @@ __device__ __forceinline__ void fused_bins_rot(int b0, int b1, int kbase, double
     }
 }
 
-template <int NM1> // NM1 = 1: single-mode specialisation (NQ = 5); 0: any n_m (NQ = 2)
-__global__ void __launch_bounds__(128, LL_FUSED_MINB) k_full_fused(FusedArgs a)
+// NM1 = 1: single-mode specialisation (NQ = 2 NC + NW partial sums per walker and tile); 0: any n_m (NQ = 2)
+template <int NM1, int NC, bool WS>
+__global__ void __launch_bounds__(128, (NC == 2 && WS) ? LL_FUSED_MINB : 3) k_full_fused(FusedArgs a)
 {
+    using TL = Tile<NC, WS>;
     extern __shared__ __align__(128) double sm[];
     __shared__ __align__(8) uint64_t bar[2];
     __shared__ int s_lo, s_hi;
@@ -808,14 +980,7 @@ __global__ void __launch_bounds__(128, LL_FUSED_MINB) k_full_fused(FusedArgs a)
 
     const int CH = a.CH;
     const int c_begin = blo / CH, c_end = (bhi + CH - 1) / CH;
-    const uint32_t stage_bytes = (uint32_t)CH * 40u;
-    auto issue = [&](int c, int st) {
-        double *dst = sm + (size_t)st * CH * 5;
-        mbar_expect_tx(&bar[st], stage_bytes);
-        tma_load_1d(dst, a.g4 + (size_t)c * CH * 4, (uint32_t)CH * 32u, &bar[st]);
-        tma_load_1d(dst + (size_t)CH * 4, a.Wd + (size_t)c * CH, (uint32_t)CH * 8u, &bar[st]);
-    };
-    if (tid == 0) issue(c_begin, 0);
+    if (tid == 0) TL::issue(a, sm, c_begin, CH, &bar[0]);
 
     const size_t sw = (size_t)a.n_wp;
     const size_t cj = (size_t)a.n_m * 8 * sw;
@@ -823,16 +988,23 @@ __global__ void __launch_bounds__(128, LL_FUSED_MINB) k_full_fused(FusedArgs a)
     int jl = -1;
     double cA0 = 0, cA1 = 0, cA2 = 0, cA3 = 0, cP0 = 0, cP1 = 0, cP2 = 0, cP3 = 0, nxj = 0;
     const int kbase = (int)a.k_min; // k_min + n_f < 2^31 is checked on the host
-    double sAr = 0, sAi = 0, sEr = 0, sEi = 0, sH = 0; // NM1: S^A, S^E, H;  generic: sAr = d_h, sH = h_h
+    double ts4 = 0.0;               // 4 t_shift: the linear phase term in quarter cycles per Hz
+    if (a.t_shift) {
+        const int w = a.perm[p];
+        if (w >= 0) ts4 = 4.0 * a.t_shift[(size_t)w * a.ts_stride];
+    }
+    Acc1<NC, WS> acc; // NM1: S^c, H;  generic: S[0] = d_h, S[1] = h_h
+    acc.zero();
 
     for (int c = c_begin; c < c_end; ++c) {
         const int st = (c - c_begin) & 1;
         const uint32_t ph = (uint32_t)((c - c_begin) >> 1) & 1u;
-        if (tid == 0 && c + 1 < c_end) issue(c + 1, st ^ 1);
+        if (tid == 0 && c + 1 < c_end) TL::issue(a, sm + (size_t)(st ^ 1) * CH * TL::DPB, c + 1, CH, &bar[st ^ 1]);
         mbar_wait(&bar[st], ph);
-        const double *sg = sm + (size_t)st * CH * 5;
-        const double *sW = sg + (size_t)CH * 4;
+        const double *sg = sm + (size_t)st * CH * TL::DPB;
         const int cb = c * CH;
+        const double *sgc = sg - (size_t)cb * 2 * NC;      // addressed by global bin
+        const double *sWc = sg + (size_t)CH * 2 * NC - cb; // weight row r of bin ii: sWc[r CH + ii]
         const int ce = min(cb + CH, bhi);
         int i = max(cb, blo);
         while (i < ce) {
@@ -848,41 +1020,44 @@ __global__ void __launch_bounds__(128, LL_FUSED_MINB) k_full_fused(FusedArgs a)
                         const double *cc = a.C + (size_t)j * cj + p;
                         cA0 = cc[0]; cA1 = cc[sw]; cA2 = cc[2 * sw]; cA3 = cc[3 * sw];
                         cP0 = cc[4 * sw]; cP1 = cc[5 * sw]; cP2 = cc[6 * sw]; cP3 = cc[7 * sw];
-                        nxj = -__ldg(a.xj + j);
+                        const double xj = __ldg(a.xj + j);
+                        nxj = -xj;
+                        if (a.t_shift) { cP0 += qc_linear_mod_cycle(xj, ts4); cP1 += ts4; }
                         jl = j;
                     }
                     // bins every lane of the warp has inside its band run without the per-lane mask
                     const int flo = __reduce_max_sync(0xffffffffu, max(lo, i));
                     const int fhi = __reduce_min_sync(0xffffffffu, min(hi, seg_end));
-                    const double4 *sg4 = reinterpret_cast<const double4 *>(sg) - cb;
-                    const double *sWc = sW - cb;
                     if (flo < fhi) {
-                        fused_bins_nm1<true>(wlo, flo, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1, cP2, cP3,
-                                             sg4, sWc, sAr, sAi, sEr, sEi, sH);
+                        fused_bins_nm1<true, NC, WS>(wlo, flo, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1, cP2,
+                                                     cP3, sgc, sWc, CH, acc);
                         if (LL_FUSED_ROT && fhi - flo >= 8)
-                            fused_bins_rot(flo, fhi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1, cP2, cP3, sg4, sWc,
-                                           sAr, sAi, sEr, sEi, sH);
+                            fused_bins_rot<NC, WS>(flo, fhi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1, cP2, cP3, sgc, sWc,
+                                                   CH, acc);
                         else
-                            fused_bins_nm1<false>(flo, fhi, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1, cP2, cP3,
-                                                  sg4, sWc, sAr, sAi, sEr, sEi, sH);
-                        fused_bins_nm1<true>(fhi, whi, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1, cP2, cP3,
-                                             sg4, sWc, sAr, sAi, sEr, sEi, sH);
+                            fused_bins_nm1<false, NC, WS>(flo, fhi, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1,
+                                                          cP2, cP3, sgc, sWc, CH, acc);
+                        fused_bins_nm1<true, NC, WS>(fhi, whi, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1, cP2,
+                                                     cP3, sgc, sWc, CH, acc);
                     } else {
-                        fused_bins_nm1<true>(wlo, whi, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1, cP2, cP3,
-                                             sg4, sWc, sAr, sAi, sEr, sEi, sH);
+                        fused_bins_nm1<true, NC, WS>(wlo, whi, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1, cP2,
+                                                     cP3, sgc, sWc, CH, acc);
                     }
                 } else {
                     // any number of modes: chunks of four bins with the MODE loop outside the bins, so that a mode's
-                    // 8 coefficients and 4 transfer factors are read once per chunk (not once per bin) and the four
+                    // 8 coefficients and 2 NC transfer factors are read once per chunk (not once per bin) and the four
                     // bins are four independent cubic -> sincos -> T^c h chains in flight per thread
-                    nxj = -__ldg(a.xj + j);
+                    const double xj = __ldg(a.xj + j);
+                    nxj = -xj;
+                    const double sh0 = a.t_shift ? qc_linear_mod_cycle(xj, ts4) : 0.0;
                     const double *cc0 = a.C + (size_t)j * cj + p;
                     for (int c4 = wlo; c4 < whi; c4 += 4) {
-                        double t4[4], h4[4][4];
+                        double t4[4], h4[4][2 * NC];
 #pragma unroll
                         for (int k = 0; k < 4; ++k) {
                             t4[k] = fma((double)(kbase + c4 + k), a.df, nxj);
-                            h4[k][0] = h4[k][1] = h4[k][2] = h4[k][3] = 0.0;
+#pragma unroll
+                            for (int q = 0; q < 2 * NC; ++q) h4[k][q] = 0.0;
                         }
 #pragma unroll 1
                         for (int m = 0; m < a.n_m; ++m) {
@@ -890,30 +1065,24 @@ __global__ void __launch_bounds__(128, LL_FUSED_MINB) k_full_fused(FusedArgs a)
                             double co[8];
 #pragma unroll
                             for (int q = 0; q < 8; ++q) co[q] = cc[(size_t)q * sw];
-                            const double *tf = a.TF + (size_t)m * 4 * sw + p;
-                            const double tar = tf[0], tai = tf[sw], ter = tf[2 * sw], tei = tf[3 * sw];
+                            if (a.t_shift) { co[4] += sh0; co[5] += ts4; }
+                            const double *tfp = a.TF + (size_t)m * 2 * NC * sw + p;
+                            double tf[2 * NC];
+#pragma unroll
+                            for (int q = 0; q < 2 * NC; ++q) tf[q] = tfp[(size_t)q * sw];
 #pragma unroll
                             for (int k = 0; k < 4; ++k) {
                                 const double A = fma(fma(fma(co[3], t4[k], co[2]), t4[k], co[1]), t4[k], co[0]);
                                 const double y = fma(fma(fma(co[7], t4[k], co[6]), t4[k], co[5]), t4[k], co[4]);
                                 double u, v; // h_m = u - i v
                                 amp_expi_qc(A, y, u, v);
-                                h4[k][0] = fma(tar, u, h4[k][0]); h4[k][0] = fma(tai, v, h4[k][0]);
-                                h4[k][1] = fma(tai, u, h4[k][1]); h4[k][1] = fma(-tar, v, h4[k][1]);
-                                h4[k][2] = fma(ter, u, h4[k][2]); h4[k][2] = fma(tei, v, h4[k][2]);
-                                h4[k][3] = fma(tei, u, h4[k][3]); h4[k][3] = fma(-ter, v, h4[k][3]);
+                                apply_tf<NC>(tf, u, v, h4[k]);
                             }
                         }
 #pragma unroll
                         for (int k = 0; k < 4; ++k) {
                             const int ii = c4 + k;
-                            if (ii < whi && ii >= tlo && ii < thi) {
-                                const double4 g = reinterpret_cast<const double4 *>(sg)[ii - cb];
-                                const double w = sW[ii - cb];
-                                sAr = fma(g.x, h4[k][0], sAr); sAr = fma(-g.y, h4[k][1], sAr);
-                                sAr = fma(g.z, h4[k][2], sAr); sAr = fma(-g.w, h4[k][3], sAr);
-                                sH = fma(w, h4[k][0] * h4[k][0] + h4[k][1] * h4[k][1] + h4[k][2] * h4[k][2] + h4[k][3] * h4[k][3], sH);
-                            }
+                            if (ii < whi && ii >= tlo && ii < thi) accumulate_bin<NC, WS>(sgc, sWc, CH, ii, h4[k], acc.S[0], acc.S[1]);
                         }
                     }
                 }
@@ -923,11 +1092,15 @@ __global__ void __launch_bounds__(128, LL_FUSED_MINB) k_full_fused(FusedArgs a)
         __syncthreads(); // everyone is done with stage st before it is refilled two chunks later
     }
     if (NM1) {
-        double *o = a.part + ((size_t)tile * 5) * sw + p;
-        o[0] = sAr; o[sw] = sAi; o[2 * sw] = sEr; o[3 * sw] = sEi; o[4 * sw] = sH;
+        constexpr int NQ = 2 * NC + Acc1<NC, WS>::NW;
+        double *o = a.part + ((size_t)tile * NQ) * sw + p;
+#pragma unroll
+        for (int q = 0; q < 2 * NC; ++q) o[(size_t)q * sw] = acc.S[q];
+#pragma unroll
+        for (int q = 0; q < Acc1<NC, WS>::NW; ++q) o[(size_t)(2 * NC + q) * sw] = acc.H[q];
     } else {
         double *o = a.part + ((size_t)tile * 2) * sw + p;
-        o[0] = sAr; o[sw] = sH;
+        o[0] = acc.S[0]; o[sw] = acc.S[1];
     }
 }
 
@@ -1112,6 +1285,11 @@ __global__ void __launch_bounds__(128, 4) k_full_fused_mixed(FusedArgs a, FusedA
     const size_t cj = (size_t)8 * sw;
     const double sigma = m.scale[0];
     const int kbase = (int)a.k_min;
+    double ts4 = 0.0; // 4 t_shift (reading R32), folded into the phase cubic of the current interval
+    if (a.t_shift) {
+        const int w = a.perm[p];
+        if (w >= 0) ts4 = 4.0 * a.t_shift[(size_t)w * a.ts_stride];
+    }
     int j = find_interval_of_bin(a.bstart, a.n_nodes, blo);
     int jl = -1;
     double cA0 = 0, cA1 = 0, cA2 = 0, cA3 = 0, cP0 = 0, cP1 = 0, cP2 = 0, cP3 = 0, nxj = 0;
@@ -1139,7 +1317,9 @@ __global__ void __launch_bounds__(128, 4) k_full_fused_mixed(FusedArgs a, FusedA
                     const double *cc = a.C + (size_t)j * cj + p;
                     cA0 = cc[0] * sigma; cA1 = cc[sw] * sigma; cA2 = cc[2 * sw] * sigma; cA3 = cc[3 * sw] * sigma;
                     cP0 = cc[4 * sw]; cP1 = cc[5 * sw]; cP2 = cc[6 * sw]; cP3 = cc[7 * sw];
-                    nxj = -__ldg(a.xj + j);
+                    const double xj = __ldg(a.xj + j);
+                    nxj = -xj;
+                    if (a.t_shift) { cP0 += qc_linear_mod_cycle(xj, ts4); cP1 += ts4; }
                     jl = j;
                 }
                 const int flo = __reduce_max_sync(0xffffffffu, max(lo, i));
@@ -1169,19 +1349,21 @@ __global__ void __launch_bounds__(128, 4) k_full_fused_mixed(FusedArgs a, FusedA
 
 // ---------------------------------------------------------------------------------------------------
 // F3 with a frequency-dependent transfer function (Eq. 8-9).  Same mapping, staging and
-// band logic as k_full_fused; per (walker, bin, mode) six cubics (amplitude, phase, Re/Im of T^A and T^E), then
-// h^c += T^c(f) A e^{-i Psi}.  Coefficient block per (interval, mode): 24 doubles, walker fastest.
-// NM1 = 1: the 24 coefficients of the current interval live in registers; 0: any n_m, coefficients re-read per
-// bin through L1 (they would not fit in registers for several modes).
+// band logic as k_full_fused; per (walker, bin, mode) 2 + 2 NC cubics (amplitude, phase, Re/Im of every T^c), then
+// h^c += T^c(f) A e^{-i Psi}.  Coefficient block per (interval, mode): 8 + 8 NC doubles, walker fastest.
+// NM1 = 1: the coefficients of the current interval live in registers; 0: any n_m, coefficients re-read per
+// chunk of bins through L1 (they would not fit in registers for several modes).
 // ---------------------------------------------------------------------------------------------------
 __device__ __forceinline__ double cubic4(const double *c4, double t)
 {
     return fma(fma(fma(c4[3], t, c4[2]), t, c4[1]), t, c4[0]);
 }
 
-template <int NM1>
-__global__ void __launch_bounds__(128, 3) k_full_fused_tf(FusedArgs a)
+template <int NM1, int NC, bool WS>
+__global__ void __launch_bounds__(128, NC == 2 ? 3 : 2) k_full_fused_tf(FusedArgs a)
 {
+    using TL = Tile<NC, WS>;
+    constexpr int NCO = 8 + 8 * NC; // coefficients per (interval, mode)
     extern __shared__ __align__(128) double sm[];
     __shared__ __align__(8) uint64_t bar[2];
     __shared__ int s_lo, s_hi;
@@ -1209,32 +1391,31 @@ __global__ void __launch_bounds__(128, 3) k_full_fused_tf(FusedArgs a)
 
     const int CH = a.CH;
     const int c_begin = blo / CH, c_end = (bhi + CH - 1) / CH;
-    const uint32_t stage_bytes = (uint32_t)CH * 40u;
-    auto issue = [&](int c, int st) {
-        double *dst = sm + (size_t)st * CH * 5;
-        mbar_expect_tx(&bar[st], stage_bytes);
-        tma_load_1d(dst, a.g4 + (size_t)c * CH * 4, (uint32_t)CH * 32u, &bar[st]);
-        tma_load_1d(dst + (size_t)CH * 4, a.Wd + (size_t)c * CH, (uint32_t)CH * 8u, &bar[st]);
-    };
-    if (tid == 0) issue(c_begin, 0);
+    if (tid == 0) TL::issue(a, sm, c_begin, CH, &bar[0]);
 
     const size_t sw = (size_t)a.n_wp;
-    const size_t cm = (size_t)24 * sw;          // one mode's block
+    const size_t cm = (size_t)NCO * sw;         // one mode's block
     const size_t cj = (size_t)a.n_m * cm;       // one interval's block
     const int kbase = (int)a.k_min;
     int j = find_interval_of_bin(a.bstart, a.n_nodes, blo);
     int jl = -1;
-    double co[24];
-    double nxj = 0.0, s_dh = 0.0, s_hh = 0.0;
+    double co[NCO];
+    double nxj = 0.0, sh0 = 0.0, s_dh = 0.0, s_hh = 0.0;
+    double ts4 = 0.0; // 4 t_shift (reading R32)
+    if (a.t_shift) {
+        const int w = a.perm[p];
+        if (w >= 0) ts4 = 4.0 * a.t_shift[(size_t)w * a.ts_stride];
+    }
 
     for (int c = c_begin; c < c_end; ++c) {
         const int st = (c - c_begin) & 1;
         const uint32_t ph = (uint32_t)((c - c_begin) >> 1) & 1u;
-        if (tid == 0 && c + 1 < c_end) issue(c + 1, st ^ 1);
+        if (tid == 0 && c + 1 < c_end) TL::issue(a, sm + (size_t)(st ^ 1) * CH * TL::DPB, c + 1, CH, &bar[st ^ 1]);
         mbar_wait(&bar[st], ph);
-        const double *sg = sm + (size_t)st * CH * 5;
-        const double *sW = sg + (size_t)CH * 4;
+        const double *sg = sm + (size_t)st * CH * TL::DPB;
         const int cb = c * CH;
+        const double *sgc = sg - (size_t)cb * 2 * NC;
+        const double *sWc = sg + (size_t)CH * 2 * NC - cb;
         const int ce = min(cb + CH, bhi);
         int i = max(cb, blo);
         while (i < ce) {
@@ -1247,55 +1428,50 @@ __global__ void __launch_bounds__(128, 3) k_full_fused_tf(FusedArgs a)
             if (wlo < whi) {
                 const double *cc0 = a.C + (size_t)j * cj + p;
                 if (j != jl) {
-                    nxj = -__ldg(a.xj + j);
+                    const double xj = __ldg(a.xj + j);
+                    nxj = -xj;
+                    sh0 = a.t_shift ? qc_linear_mod_cycle(xj, ts4) : 0.0;
                     if (NM1) {
 #pragma unroll
-                        for (int q = 0; q < 24; ++q) co[q] = cc0[(size_t)q * sw];
+                        for (int q = 0; q < NCO; ++q) co[q] = cc0[(size_t)q * sw];
+                        if (a.t_shift) { co[4] += sh0; co[5] += ts4; }
                     }
                     jl = j;
                 }
-                const double4 *sg4 = reinterpret_cast<const double4 *>(sg) - cb;
-                const double *sWc = sW - cb;
+                // h^c of one mode at offset t from the interval's node, added into h
+                auto mode_at = [&](double t, double (&h)[2 * NC]) {
+                    const double A = cubic4(co, t), y = cubic4(co + 4, t);
+                    double tf[2 * NC];
+#pragma unroll
+                    for (int q = 0; q < 2 * NC; ++q) tf[q] = cubic4(co + 8 + 4 * q, t);
+                    double u, v; // h_m = u - i v
+                    amp_expi_qc(A, y, u, v);
+                    apply_tf<NC>(tf, u, v, h);
+                };
                 auto direct_bins = [&](int b0, int b1) {
                     if (!NM1) {
-                        // several modes: chunks of four bins, mode loop outside (24 coefficients read once per chunk)
+                        // several modes: chunks of four bins, mode loop outside (the coefficients read once per chunk)
                         for (int c4 = b0; c4 < b1; c4 += 4) {
-                            double t4[4], h4[4][4];
+                            double t4[4], h4[4][2 * NC];
 #pragma unroll
                             for (int k = 0; k < 4; ++k) {
                                 t4[k] = fma((double)(kbase + c4 + k), a.df, nxj);
-                                h4[k][0] = h4[k][1] = h4[k][2] = h4[k][3] = 0.0;
+#pragma unroll
+                                for (int q = 0; q < 2 * NC; ++q) h4[k][q] = 0.0;
                             }
 #pragma unroll 1
                             for (int m = 0; m < a.n_m; ++m) {
                                 const double *cc = cc0 + (size_t)m * cm;
 #pragma unroll
-                                for (int q = 0; q < 24; ++q) co[q] = cc[(size_t)q * sw];
+                                for (int q = 0; q < NCO; ++q) co[q] = cc[(size_t)q * sw];
+                                if (a.t_shift) { co[4] += sh0; co[5] += ts4; }
 #pragma unroll
-                                for (int k = 0; k < 4; ++k) {
-                                    const double t = t4[k];
-                                    const double A = cubic4(co, t), y = cubic4(co + 4, t);
-                                    const double tar = cubic4(co + 8, t), tai = cubic4(co + 12, t);
-                                    const double ter = cubic4(co + 16, t), tei = cubic4(co + 20, t);
-                                    double u, v; // h_m = u - i v
-                                    amp_expi_qc(A, y, u, v);
-                                    h4[k][0] = fma(tar, u, h4[k][0]); h4[k][0] = fma(tai, v, h4[k][0]);
-                                    h4[k][1] = fma(tai, u, h4[k][1]); h4[k][1] = fma(-tar, v, h4[k][1]);
-                                    h4[k][2] = fma(ter, u, h4[k][2]); h4[k][2] = fma(tei, v, h4[k][2]);
-                                    h4[k][3] = fma(tei, u, h4[k][3]); h4[k][3] = fma(-ter, v, h4[k][3]);
-                                }
+                                for (int k = 0; k < 4; ++k) mode_at(t4[k], h4[k]);
                             }
 #pragma unroll
                             for (int k = 0; k < 4; ++k) {
                                 const int ii = c4 + k;
-                                if (ii < b1 && ii >= tlo && ii < thi) {
-                                    const double4 g = sg4[ii];
-                                    const double w = sWc[ii];
-                                    s_dh = fma(g.x, h4[k][0], s_dh); s_dh = fma(-g.y, h4[k][1], s_dh);
-                                    s_dh = fma(g.z, h4[k][2], s_dh); s_dh = fma(-g.w, h4[k][3], s_dh);
-                                    s_hh = fma(w, fma(h4[k][0], h4[k][0], h4[k][1] * h4[k][1]) +
-                                                      fma(h4[k][2], h4[k][2], h4[k][3] * h4[k][3]), s_hh);
-                                }
+                                if (ii < b1 && ii >= tlo && ii < thi) accumulate_bin<NC, WS>(sgc, sWc, CH, ii, h4[k], s_dh, s_hh);
                             }
                         }
                         return;
@@ -1304,31 +1480,11 @@ __global__ void __launch_bounds__(128, 3) k_full_fused_tf(FusedArgs a)
                     for (int ii = b0; ii < b1; ++ii) {
                         const bool act = (ii >= tlo) && (ii < thi);
                         const double t = fma((double)(kbase + ii), a.df, nxj);
-                        double hAr = 0, hAi = 0, hEr = 0, hEi = 0;
-                        const int n_m = NM1 ? 1 : a.n_m;
-                        for (int m = 0; m < n_m; ++m) {
-                            if (!NM1) {
-                                const double *cc = cc0 + (size_t)m * cm;
+                        double h[2 * NC];
 #pragma unroll
-                                for (int q = 0; q < 24; ++q) co[q] = cc[(size_t)q * sw];
-                            }
-                            const double A = cubic4(co, t), y = cubic4(co + 4, t);
-                            const double tar = cubic4(co + 8, t), tai = cubic4(co + 12, t);
-                            const double ter = cubic4(co + 16, t), tei = cubic4(co + 20, t);
-                            double u, v; // h_m = u - i v
-                            amp_expi_qc(A, y, u, v);
-                            hAr = fma(tar, u, hAr); hAr = fma(tai, v, hAr);
-                            hAi = fma(tai, u, hAi); hAi = fma(-tar, v, hAi);
-                            hEr = fma(ter, u, hEr); hEr = fma(tei, v, hEr);
-                            hEi = fma(tei, u, hEi); hEi = fma(-ter, v, hEi);
-                        }
-                        if (act) {
-                            const double4 g = sg4[ii];
-                            const double w = sWc[ii];
-                            s_dh = fma(g.x, hAr, s_dh); s_dh = fma(-g.y, hAi, s_dh);
-                            s_dh = fma(g.z, hEr, s_dh); s_dh = fma(-g.w, hEi, s_dh);
-                            s_hh = fma(w, fma(hAr, hAr, hAi * hAi) + fma(hEr, hEr, hEi * hEi), s_hh);
-                        }
+                        for (int q = 0; q < 2 * NC; ++q) h[q] = 0.0;
+                        mode_at(t, h);
+                        if (act) accumulate_bin<NC, WS>(sgc, sWc, CH, ii, h, s_dh, s_hh);
                     }
                 };
                 // bins inside every lane's band: e^{-i Psi} and A by the recurrence of fused_bins_rot, T^c(f) by Horner
@@ -1356,16 +1512,15 @@ __global__ void __launch_bounds__(128, 3) k_full_fused_tf(FusedArgs a)
 #pragma unroll 2
                         for (int ii = k0; ii < k1; ++ii) {
                             const double t = fma((double)(kbase + ii), df, nxj);
-                            const double tar = cubic4(co + 8, t), tai = cubic4(co + 12, t);
-                            const double ter = cubic4(co + 16, t), tei = cubic4(co + 20, t);
                             const double u = A * cz, v = A * sz; // h = u - i v
-                            const double hAr = fma(tar, u, tai * v), hAi = fma(tai, u, -(tar * v));
-                            const double hEr = fma(ter, u, tei * v), hEi = fma(tei, u, -(ter * v));
-                            const double4 g = sg4[ii];
-                            const double w = sWc[ii];
-                            s_dh = fma(g.x, hAr, s_dh); s_dh = fma(-g.y, hAi, s_dh);
-                            s_dh = fma(g.z, hEr, s_dh); s_dh = fma(-g.w, hEi, s_dh);
-                            s_hh = fma(w, fma(hAr, hAr, hAi * hAi) + fma(hEr, hEr, hEi * hEi), s_hh);
+                            double h[2 * NC];
+#pragma unroll
+                            for (int cch = 0; cch < NC; ++cch) {
+                                const double tr = cubic4(co + 8 + 8 * cch, t), ti = cubic4(co + 12 + 8 * cch, t);
+                                h[2 * cch] = fma(tr, u, ti * v);
+                                h[2 * cch + 1] = fma(ti, u, -(tr * v));
+                            }
+                            accumulate_bin<NC, WS>(sgc, sWc, CH, ii, h, s_dh, s_hh);
                             const double nzc = fma(cz, cw, -(sz * sw_)), nzs = fma(sz, cw, cz * sw_);
                             const double nwc = fma(cw, cv, -(sw_ * sv)), nws = fma(sw_, cv, cw * sv);
                             const double nvc = fma(cv, cu, -(sv * su)), nvs = fma(sv, cu, cv * su);
@@ -1499,9 +1654,10 @@ k_spline_pw(const double *__restrict__ Y, const double *__restrict__ X, double *
 // g/W tiles broadcast from shared memory); every lane tracks its own interval: the bins go up, so the interval index
 // only moves forward, by a comparison with the lane's next node per bin.  NM1: the 8 coefficients of the lane's
 // current interval live in registers; otherwise they are re-read per bin through L1.
-template <int NM1>
+template <int NM1, int NC, bool WS>
 __global__ void __launch_bounds__(128, 3) k_full_fused_pw(FusedArgs a, const double *__restrict__ X)
 {
+    using TL = Tile<NC, WS>;
     extern __shared__ __align__(128) double sm[];
     __shared__ __align__(8) uint64_t bar[2];
     __shared__ int s_lo, s_hi;
@@ -1529,30 +1685,30 @@ __global__ void __launch_bounds__(128, 3) k_full_fused_pw(FusedArgs a, const dou
 
     const int CH = a.CH;
     const int c_begin = blo / CH, c_end = (bhi + CH - 1) / CH;
-    const uint32_t stage_bytes = (uint32_t)CH * 40u;
-    auto issue = [&](int c, int st) {
-        double *dst = sm + (size_t)st * CH * 5;
-        mbar_expect_tx(&bar[st], stage_bytes);
-        tma_load_1d(dst, a.g4 + (size_t)c * CH * 4, (uint32_t)CH * 32u, &bar[st]);
-        tma_load_1d(dst + (size_t)CH * 4, a.Wd + (size_t)c * CH, (uint32_t)CH * 8u, &bar[st]);
-    };
-    if (tid == 0) issue(c_begin, 0);
+    if (tid == 0) TL::issue(a, sm, c_begin, CH, &bar[0]);
 
     const size_t sw = (size_t)a.n_wp;
     const size_t cm = (size_t)8 * sw, cj = (size_t)a.n_m * cm;
     const int n = a.n_nodes;
     const double *x = X + p;
+    double ts4 = 0.0; // 4 t_shift (reading R32), folded into the phase cubic of the lane's current interval
+    if (a.t_shift) {
+        const int w = a.perm[p];
+        if (w >= 0) ts4 = 4.0 * a.t_shift[(size_t)w * a.ts_stride];
+    }
     // this lane's interval at its first bin: largest j in [0, n-2] with x_j <= f
     int j = 0;
-    double xj = 0.0, xnext = INFINITY;
+    double xj = 0.0, xnext = INFINITY, sh0 = 0.0;
     double co[8];
     auto load_interval = [&](int jj) {
         xj = __ldg(x + (size_t)jj * sw);
         xnext = (jj < n - 2) ? __ldg(x + (size_t)(jj + 1) * sw) : INFINITY;
+        sh0 = a.t_shift ? qc_linear_mod_cycle(xj, ts4) : 0.0;
         if (NM1) {
             const double *cc = a.C + (size_t)jj * cj + p;
 #pragma unroll
             for (int q = 0; q < 8; ++q) co[q] = cc[(size_t)q * sw];
+            if (a.t_shift) { co[4] += sh0; co[5] += ts4; }
         }
     };
     if (lo < hi) {
@@ -1565,49 +1721,43 @@ __global__ void __launch_bounds__(128, 3) k_full_fused_pw(FusedArgs a, const dou
         j = l;
         load_interval(j);
     }
-    double tf1[4] = {0, 0, 0, 0}; // single mode: the walker's transfer factors stay in registers
-    if (NM1) { tf1[0] = a.TF[p]; tf1[1] = a.TF[sw + p]; tf1[2] = a.TF[2 * sw + p]; tf1[3] = a.TF[3 * sw + p]; }
+    double tf1[2 * NC]; // single mode: the walker's transfer factors stay in registers
+#pragma unroll
+    for (int q = 0; q < 2 * NC; ++q) tf1[q] = NM1 ? a.TF[(size_t)q * sw + p] : 0.0;
     double s_dh = 0.0, s_hh = 0.0;
 
     for (int c = c_begin; c < c_end; ++c) {
         const int st = (c - c_begin) & 1;
         const uint32_t ph = (uint32_t)((c - c_begin) >> 1) & 1u;
-        if (tid == 0 && c + 1 < c_end) issue(c + 1, st ^ 1);
+        if (tid == 0 && c + 1 < c_end) TL::issue(a, sm + (size_t)(st ^ 1) * CH * TL::DPB, c + 1, CH, &bar[st ^ 1]);
         mbar_wait(&bar[st], ph);
-        const double *sg = sm + (size_t)st * CH * 5;
-        const double *sW = sg + (size_t)CH * 4;
+        const double *sg = sm + (size_t)st * CH * TL::DPB;
         const int cb = c * CH;
+        const double *sgc = sg - (size_t)cb * 2 * NC;
+        const double *sWc = sg + (size_t)CH * 2 * NC - cb;
         const int tlo = max(cb, lo), thi = min(cb + CH, hi);
-        const double4 *sg4 = reinterpret_cast<const double4 *>(sg) - cb;
-        const double *sWc = sW - cb;
         auto one_bin = [&](int ii, double f) {
             const double t = f - xj;
-            double hAr = 0, hAi = 0, hEr = 0, hEi = 0;
+            double h[2 * NC];
+#pragma unroll
+            for (int q = 0; q < 2 * NC; ++q) h[q] = 0.0;
             const int n_m = NM1 ? 1 : a.n_m;
             for (int m = 0; m < n_m; ++m) {
                 if (!NM1) {
                     const double *cc = a.C + (size_t)j * cj + (size_t)m * cm + p;
 #pragma unroll
                     for (int q = 0; q < 8; ++q) co[q] = cc[(size_t)q * sw];
+                    if (a.t_shift) { co[4] += sh0; co[5] += ts4; }
+                    const double *tf = a.TF + (size_t)m * 2 * NC * sw + p;
+#pragma unroll
+                    for (int q = 0; q < 2 * NC; ++q) tf1[q] = tf[(size_t)q * sw];
                 }
                 const double A = cubic4(co, t), y = cubic4(co + 4, t);
                 double u, v; // h_m = u - i v
                 amp_expi_qc(A, y, u, v);
-                double tar = tf1[0], tai = tf1[1], ter = tf1[2], tei = tf1[3];
-                if (!NM1) {
-                    const double *tf = a.TF + (size_t)m * 4 * sw + p;
-                    tar = tf[0]; tai = tf[sw]; ter = tf[2 * sw]; tei = tf[3 * sw];
-                }
-                hAr = fma(tar, u, hAr); hAr = fma(tai, v, hAr);
-                hAi = fma(tai, u, hAi); hAi = fma(-tar, v, hAi);
-                hEr = fma(ter, u, hEr); hEr = fma(tei, v, hEr);
-                hEi = fma(tei, u, hEi); hEi = fma(-ter, v, hEi);
+                apply_tf<NC>(tf1, u, v, h);
             }
-            const double4 g = sg4[ii];
-            const double w = sWc[ii];
-            s_dh = fma(g.x, hAr, s_dh); s_dh = fma(-g.y, hAi, s_dh);
-            s_dh = fma(g.z, hEr, s_dh); s_dh = fma(-g.w, hEi, s_dh);
-            s_hh = fma(w, fma(hAr, hAr, hAi * hAi) + fma(hEr, hEr, hEi * hEi), s_hh);
+            accumulate_bin<NC, WS>(sgc, sWc, CH, ii, h, s_dh, s_hh);
         };
         int ii = tlo;
         while (ii < thi) {
@@ -1637,13 +1787,13 @@ __global__ void __launch_bounds__(128, 3) k_full_fused_pw(FusedArgs a, const dou
 #pragma unroll 2
                 for (int k = 0; k < m; ++k) {
                     const double u = A * cz, v = A * sz; // h = u - i v
-                    const double hAr = fma(tf1[0], u, tf1[1] * v), hAi = fma(tf1[1], u, -(tf1[0] * v));
-                    const double hEr = fma(tf1[2], u, tf1[3] * v), hEi = fma(tf1[3], u, -(tf1[2] * v));
-                    const double4 g = sg4[ii + k];
-                    const double w = sWc[ii + k];
-                    s_dh = fma(g.x, hAr, s_dh); s_dh = fma(-g.y, hAi, s_dh);
-                    s_dh = fma(g.z, hEr, s_dh); s_dh = fma(-g.w, hEi, s_dh);
-                    s_hh = fma(w, fma(hAr, hAr, hAi * hAi) + fma(hEr, hEr, hEi * hEi), s_hh);
+                    double h[2 * NC];
+#pragma unroll
+                    for (int cch = 0; cch < NC; ++cch) {
+                        h[2 * cch] = fma(tf1[2 * cch], u, tf1[2 * cch + 1] * v);
+                        h[2 * cch + 1] = fma(tf1[2 * cch + 1], u, -(tf1[2 * cch] * v));
+                    }
+                    accumulate_bin<NC, WS>(sgc, sWc, CH, ii + k, h, s_dh, s_hh);
                     const double nzc = fma(cz, cw, -(sz * sw_)), nzs = fma(sz, cw, cz * sw_);
                     const double nwc = fma(cw, cv, -(sw_ * sv)), nws = fma(sw_, cv, cw * sv);
                     const double nvc = fma(cv, cu, -(sv * su)), nvs = fma(sv, cu, cv * su);
@@ -1701,12 +1851,17 @@ k_tlm_nodes(const double *__restrict__ phase, int n_sys, int n_nodes, double t_r
 // F4, first stage for small batches with thousands of tiles: block (x, z) adds, for its 32 walkers, the partials of
 // the tiles of chunk z = [z cs, (z+1) cs) that lie in the walker's band, in a fixed order, into part2[z][NQ][n_wp];
 // k_finalize then runs over the chunks as if they were tiles (tile_start2[z] = tile_start[z cs]).
+// tile slices per block of the two F4 kernels: 32, or 16 when a walker has more than 5 partial sums (the slices meet in
+// shared memory, [slices][NQ][32] doubles <= 48 KB)
+__host__ __device__ constexpr int fin_slices(int nq) { return nq > 5 ? 16 : 32; }
+
 template <int NQ>
-__global__ void __launch_bounds__(32 * 32)
+__global__ void __launch_bounds__(32 * fin_slices(NQ))
 k_reduce_tiles(const double *__restrict__ part, const int *__restrict__ ilo, const int *__restrict__ ihi, int n_wp,
                const int *__restrict__ tile_start, int n_tiles, int cs, double *__restrict__ part2)
 {
-    __shared__ double red[32][NQ][32];
+    constexpr int FY = fin_slices(NQ);
+    __shared__ double red[FY][NQ][32];
     const int p = blockIdx.x * 32 + threadIdx.x, ty = threadIdx.y, z = blockIdx.y;
     const bool in = p < n_wp;
     const size_t sw = (size_t)n_wp;
@@ -1719,7 +1874,7 @@ k_reduce_tiles(const double *__restrict__ part, const int *__restrict__ ilo, con
         const int t0 = max(tile_of_bin(tile_start, n_tiles, lo), z * cs);
         const int t1 = min(tile_of_bin(tile_start, n_tiles, hi - 1), min((z + 1) * cs, n_tiles) - 1);
         any = t0 <= t1;
-        for (int t = t0 + ty; t <= t1; t += 32) {
+        for (int t = t0 + ty; t <= t1; t += FY) {
             const double *o = part + ((size_t)t * NQ) * sw + p;
 #pragma unroll
             for (int q = 0; q < NQ; ++q) acc[q] += o[q * sw];
@@ -1733,7 +1888,7 @@ k_reduce_tiles(const double *__restrict__ part, const int *__restrict__ ilo, con
     for (int q = 0; q < NQ; ++q) {
         double v = red[0][q][threadIdx.x];
 #pragma unroll
-        for (int k = 1; k < 32; ++k) v += red[k][q][threadIdx.x];
+        for (int k = 1; k < FY; ++k) v += red[k][q][threadIdx.x];
         part2[((size_t)z * NQ + q) * sw + p] = v;
     }
 }
@@ -1741,15 +1896,15 @@ k_reduce_tiles(const double *__restrict__ part, const int *__restrict__ ilo, con
 // F4: reduce the per-tile partials in a fixed order, apply T^c (single mode), form log L        (Eq. 2)
 // Block = 32 walkers x kFinY tile slices: slice ty sums tiles t0 + ty, t0 + ty + kFinY, ... of its walker, the
 // slices meet in shared memory and are added in slice order (deterministic: reruns are bit-identical).
-constexpr int kFinY = 32;
-template <int NM1>
-__global__ void __launch_bounds__(32 * kFinY)
+template <int NM1, int NC, int NW> // NW: weight rows behind the single-mode H sums (1 shared, NC per channel)
+__global__ void __launch_bounds__(32 * fin_slices(NM1 ? 2 * NC + NW : 2))
 k_finalize(const double *__restrict__ part, const double *__restrict__ TF, const int *__restrict__ perm,
            const int *__restrict__ ilo, const int *__restrict__ ihi, int n_wp, const int *__restrict__ tile_start,
            int n_tiles, const double *__restrict__ dd, double *__restrict__ logL, double *__restrict__ d_h,
            double *__restrict__ h_h)
 {
-    constexpr int NQ = NM1 ? 5 : 2;
+    constexpr int NQ = NM1 ? 2 * NC + NW : 2;
+    constexpr int kFinY = fin_slices(NQ);
     __shared__ double red[kFinY][NQ][32];
     const int p = blockIdx.x * 32 + threadIdx.x, ty = threadIdx.y;
     const bool in = p < n_wp;
@@ -1782,10 +1937,17 @@ k_finalize(const double *__restrict__ part, const double *__restrict__ TF, const
     }
     double dh, hh;
     if (NM1) {
-        const double tar = TF[p], tai = TF[sw + p], ter = TF[2 * sw + p], tei = TF[3 * sw + p];
-        // Re[T^A S^A + T^E S^E],  (|T^A|^2 + |T^E|^2) H
-        dh = (tar * acc[0] - tai * acc[1]) + (ter * acc[2] - tei * acc[3]);
-        hh = (tar * tar + tai * tai + ter * ter + tei * tei) * acc[4];
+        // Re sum_c T^c S^c,  sum_c |T^c|^2 H^c (one H for a shared weight row)
+        dh = 0.0; hh = 0.0;
+        double t2 = 0.0;
+#pragma unroll
+        for (int c = 0; c < NC; ++c) {
+            const double tr = TF[(size_t)(2 * c) * sw + p], ti = TF[(size_t)(2 * c + 1) * sw + p];
+            dh += tr * acc[2 * c] - ti * acc[2 * c + 1];
+            if (NW == 1) t2 += tr * tr + ti * ti;
+            else hh += (tr * tr + ti * ti) * acc[2 * NC + c];
+        }
+        if (NW == 1) hh = t2 * acc[2 * NC];
     } else {
         dh = acc[0];
         hh = acc[1];
@@ -1797,51 +1959,59 @@ k_finalize(const double *__restrict__ part, const double *__restrict__ TF, const
 
 // dense template of the walker at sorted position p (setup utility; same arithmetic as k_full_fused)
 __global__ void __launch_bounds__(256)
-k_full_template(FusedArgs a, int p, double *__restrict__ h_out)
+k_full_template(FusedArgs a, int p, int n_c, double *__restrict__ h_out)
 {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= a.n_f) return;
-    double hAr = 0, hAi = 0, hEr = 0, hEi = 0;
+    double h[2 * kMaxNC];
+#pragma unroll
+    for (int q = 0; q < 2 * kMaxNC; ++q) h[q] = 0.0;
     if (i >= a.ilo[p] && i < a.ihi[p]) {
         const int j = find_interval_of_bin(a.bstart, a.n_nodes, (int)i);
         const size_t sw = (size_t)a.n_wp;
         const double t = fma((double)(a.k_min + i), a.df, -a.xj[j]);
+        double ysh = 0.0;
+        if (a.t_shift && a.perm[p] >= 0) ysh = qc_linear_mod_cycle((double)(a.k_min + i) * a.df, 4.0 * a.t_shift[(size_t)a.perm[p] * a.ts_stride]);
         for (int m = 0; m < a.n_m; ++m) {
             const double *cc = a.C + ((size_t)j * a.n_m + m) * 8 * sw + p;
             const double A = fma(fma(fma(cc[3 * sw], t, cc[2 * sw]), t, cc[sw]), t, cc[0]);
-            const double y = fma(fma(fma(cc[7 * sw], t, cc[6 * sw]), t, cc[5 * sw]), t, cc[4 * sw]);
+            const double y = fma(fma(fma(cc[7 * sw], t, cc[6 * sw]), t, cc[5 * sw]), t, cc[4 * sw]) + ysh;
             double sn, cs;
             sincos_qc(y, sn, cs);
             const double u = A * cs, v = A * sn;
-            const double *tf = a.TF + (size_t)m * 4 * sw + p;
-            const double tar = tf[0], tai = tf[sw], ter = tf[2 * sw], tei = tf[3 * sw];
-            hAr = fma(tar, u, hAr); hAr = fma(tai, v, hAr);
-            hAi = fma(tai, u, hAi); hAi = fma(-tar, v, hAi);
-            hEr = fma(ter, u, hEr); hEr = fma(tei, v, hEr);
-            hEi = fma(tei, u, hEi); hEi = fma(-ter, v, hEi);
+            const double *tf = a.TF + (size_t)m * 2 * n_c * sw + p;
+#pragma unroll
+            for (int c = 0; c < kMaxNC; ++c)
+                if (c < n_c) {
+                    const double tr = tf[(size_t)(2 * c) * sw], ti = tf[(size_t)(2 * c + 1) * sw];
+                    h[2 * c] = fma(tr, u, h[2 * c]); h[2 * c] = fma(ti, v, h[2 * c]);
+                    h[2 * c + 1] = fma(ti, u, h[2 * c + 1]); h[2 * c + 1] = fma(-tr, v, h[2 * c + 1]);
+                }
         }
     }
-    reinterpret_cast<double2 *>(h_out)[i] = make_double2(hAr, hAi);
-    reinterpret_cast<double2 *>(h_out)[a.n_f + i] = make_double2(hEr, hEi);
+#pragma unroll
+    for (int c = 0; c < kMaxNC; ++c)
+        if (c < n_c) reinterpret_cast<double2 *>(h_out)[(size_t)c * a.n_f + i] = make_double2(h[2 * c], h[2 * c + 1]);
 }
 
 // stand-in template of one parameter row evaluated directly at arbitrary frequencies (no spline, no tables)
 struct DirectRow {
-    double p[5 + 4 * kMaxModes];
+    double p[5 + 2 * kMaxNC * kMaxModes];
     double c_lm[kMaxModes];
 };
 struct DirectClm {
     double c_lm[kMaxModes];
 };
 
-// h^A, h^E of one stand-in parameter row at frequency fi, evaluated directly (Eq. 7, 9; reading R9)
+// h^c (re, im per channel) of one stand-in parameter row at frequency fi, evaluated directly (Eq. 7, 9; reading R9)
 __device__ __forceinline__ void direct_template_at(const double *__restrict__ rp, const double *__restrict__ c_lm,
                                                    const StandinInfo &si, double Mtot, double eta, double fisco,
-                                                   double fi, double &hAr, double &hAi, double &hEr, double &hEi)
+                                                   double fi, double (&h)[2 * kMaxNC])
 {
     const double tc = rp[2], phic = rp[3], invD = rp[4];
     const double inv_kappa = 1.0 / si.kappa;
-    hAr = hAi = hEr = hEi = 0.0;
+#pragma unroll
+    for (int q = 0; q < 2 * kMaxNC; ++q) h[q] = 0.0;
     for (int m = 0; m < si.n_m; ++m) {
         const double mh = 0.5 * (double)si.mode_m[m];
         const double fp = fi / mh;
@@ -1852,11 +2022,14 @@ __device__ __forceinline__ void direct_template_at(const double *__restrict__ rp
         double sn, cs;
         sincos_rad(psi, sn, cs);
         const double u = A * cs, vv = A * sn;
-        const double tar = rp[5 + m * 4], tai = rp[6 + m * 4], ter = rp[7 + m * 4], tei = rp[8 + m * 4];
-        hAr = fma(tar, u, hAr); hAr = fma(tai, vv, hAr);
-        hAi = fma(tai, u, hAi); hAi = fma(-tar, vv, hAi);
-        hEr = fma(ter, u, hEr); hEr = fma(tei, vv, hEr);
-        hEi = fma(tei, u, hEi); hEi = fma(-ter, vv, hEi);
+        const double *tf = rp + 5 + m * 2 * si.n_c;
+#pragma unroll
+        for (int c = 0; c < kMaxNC; ++c)
+            if (c < si.n_c) {
+                const double tr = tf[2 * c], ti = tf[2 * c + 1];
+                h[2 * c] = fma(tr, u, h[2 * c]); h[2 * c] = fma(ti, vv, h[2 * c]);
+                h[2 * c + 1] = fma(ti, u, h[2 * c + 1]); h[2 * c + 1] = fma(-tr, vv, h[2 * c + 1]);
+            }
     }
 }
 
@@ -1868,14 +2041,17 @@ k_template_direct(DirectRow row, StandinInfo si, long long n_freq, const double 
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n_freq) return;
     const double fi = f ? f[i] : bin_freq(g.k_min, i, g.df);
-    double hAr = 0, hAi = 0, hEr = 0, hEi = 0;
+    double h[2 * kMaxNC];
+#pragma unroll
+    for (int q = 0; q < 2 * kMaxNC; ++q) h[q] = 0.0;
     if (fi >= f_lo && fi <= f_hi) {
         double Mtot, eta, fisco;
         standin_masses(row.p[0], row.p[1], Mtot, eta, fisco);
-        direct_template_at(row.p, row.c_lm, si, Mtot, eta, fisco, fi, hAr, hAi, hEr, hEi);
+        direct_template_at(row.p, row.c_lm, si, Mtot, eta, fisco, fi, h);
     }
-    reinterpret_cast<double2 *>(h_out)[i] = make_double2(hAr, hAi);
-    reinterpret_cast<double2 *>(h_out)[n_freq + i] = make_double2(hEr, hEi);
+#pragma unroll
+    for (int c = 0; c < kMaxNC; ++c)
+        if (c < si.n_c) reinterpret_cast<double2 *>(h_out)[(size_t)c * n_freq + i] = make_double2(h[2 * c], h[2 * c + 1]);
 }
 
 // PAPER.md:210 "replacing it with the highest Likelihood point in the population": index of the largest finite
@@ -1919,10 +2095,12 @@ __global__ void __launch_bounds__(1024) k_argmax(const double *__restrict__ v, l
 // PAPER.md:276 "the brute-force Likelihood can ... verify the Heterodyning results": dense log L of each walker
 // over the dense bins [i_lo, i_hi) the heterodyne bins cover, template evaluated directly at every bin (no spline,
 // no heterodyne), three-term form (Eq. 2-3).  One block per walker; fixed-order reduction.
+template <int NC>
 __global__ void __launch_bounds__(256)
-k_het_audit(const double *__restrict__ params, int P, DirectClm cl, StandinInfo si, const double *__restrict__ g4,
-            const double *__restrict__ Wd, GridInfo g, const int *__restrict__ estart, int n_b,
-            const double *__restrict__ dd, double *__restrict__ logL, double *__restrict__ d_h, double *__restrict__ h_h)
+k_het_audit(const double *__restrict__ params, int P, DirectClm cl, StandinInfo si, const double *__restrict__ g,
+            const double *__restrict__ Wc, int w_rows, long long n_f_pad, GridInfo gi, const int *__restrict__ estart,
+            int n_b, const double *__restrict__ dd, double *__restrict__ logL, double *__restrict__ d_h,
+            double *__restrict__ h_h)
 {
     __shared__ double sh[8];
     const size_t w = blockIdx.x;
@@ -1932,11 +2110,14 @@ k_het_audit(const double *__restrict__ params, int P, DirectClm cl, StandinInfo 
     standin_masses(rp[0], rp[1], Mtot, eta, fisco);
     double a_dh = 0.0, a_hh = 0.0;
     for (int i = i_lo + threadIdx.x; i < i_hi; i += blockDim.x) {
-        double hAr, hAi, hEr, hEi;
-        direct_template_at(rp, cl.c_lm, si, Mtot, eta, fisco, bin_freq(g.k_min, i, g.df), hAr, hAi, hEr, hEi);
-        const double4 gg = reinterpret_cast<const double4 *>(g4)[i]; // W conj(d)
-        a_dh += (gg.x * hAr - gg.y * hAi) + (gg.z * hEr - gg.w * hEi);
-        a_hh = fma(Wd[i], (hAr * hAr + hAi * hAi) + (hEr * hEr + hEi * hEi), a_hh);
+        double h[2 * kMaxNC];
+        direct_template_at(rp, cl.c_lm, si, Mtot, eta, fisco, bin_freq(gi.k_min, i, gi.df), h);
+#pragma unroll
+        for (int c = 0; c < NC; ++c) {
+            const double2 gg = reinterpret_cast<const double2 *>(g)[(size_t)i * NC + c]; // W conj(d)
+            a_dh += gg.x * h[2 * c] - gg.y * h[2 * c + 1];
+            a_hh = fma(Wc[(w_rows > 1 ? (size_t)c * n_f_pad : 0) + i], h[2 * c] * h[2 * c] + h[2 * c + 1] * h[2 * c + 1], a_hh);
+        }
     }
     const double t_dh = block_sum_256(a_dh, sh);
     const double t_hh = block_sum_256(a_hh, sh);
@@ -1950,76 +2131,85 @@ k_het_audit(const double *__restrict__ params, int P, DirectClm cl, StandinInfo 
 // ---------------------------------------------------------------------------------------------------
 // H0: heterodyne summary data, one block per bin                   (Eq. 15, 16, 18, 19)
 //   A0 = sum W d conj(h0), A1 = sum W d conj(h0)(f - f_b), B0 = sum W |h0|^2, B1 = sum W |h0|^2 (f - f_b)
-// raw[b][13]: per channel (A0r, A0i, A1r, A1i, B0, B1), then sum_c W |d|^2 over the bin.
+// raw[b][6 NC + 1]: per channel (A0r, A0i, A1r, A1i, B0, B1), then sum_c W^c |d^c|^2 over the bin.
 // ---------------------------------------------------------------------------------------------------
+template <int NC>
 __global__ void __launch_bounds__(256)
-k_het_prepare(const double *__restrict__ g4, const double *__restrict__ Wd, const double *__restrict__ h0, GridInfo g,
-              const int *__restrict__ estart, const double *__restrict__ fb, double *__restrict__ raw)
+k_het_prepare(const double *__restrict__ g, const double *__restrict__ Wc, int w_rows, long long n_f_pad,
+              const double *__restrict__ h0, GridInfo gi, const int *__restrict__ estart, const double *__restrict__ fb,
+              double *__restrict__ raw)
 {
+    constexpr int NR = 6 * NC + 1;
     __shared__ double sh[8];
     const int b = blockIdx.x;
     const int i_lo = estart[b], i_hi = estart[b + 1];
     const double f_b = fb[b];
-    double acc[13];
+    double acc[NR];
 #pragma unroll
-    for (int q = 0; q < 13; ++q) acc[q] = 0.0;
+    for (int q = 0; q < NR; ++q) acc[q] = 0.0;
     for (int i = i_lo + threadIdx.x; i < i_hi; i += blockDim.x) {
-        const double4 gg = reinterpret_cast<const double4 *>(g4)[i]; // W conj(d): (W dAr, -W dAi, W dEr, -W dEi)
-        const double w = Wd[i];
-        const double t = bin_freq(g.k_min, i, g.df) - f_b;
-        const double2 ha = reinterpret_cast<const double2 *>(h0)[i];
-        const double2 he = reinterpret_cast<const double2 *>(h0)[g.n_f + i];
-        // W d conj(h0) = conj( (W conj d) h0 )
-        const double par = gg.x * ha.x - gg.y * ha.y, pai = -(gg.x * ha.y + gg.y * ha.x);
-        const double per = gg.z * he.x - gg.w * he.y, pei = -(gg.z * he.y + gg.w * he.x);
-        const double qa = w * (ha.x * ha.x + ha.y * ha.y), qe = w * (he.x * he.x + he.y * he.y);
-        acc[0] += par; acc[1] += pai; acc[2] = fma(par, t, acc[2]); acc[3] = fma(pai, t, acc[3]);
-        acc[4] += qa; acc[5] = fma(qa, t, acc[5]);
-        acc[6] += per; acc[7] += pei; acc[8] = fma(per, t, acc[8]); acc[9] = fma(pei, t, acc[9]);
-        acc[10] += qe; acc[11] = fma(qe, t, acc[11]);
-        // W |d|^2 = |W conj d|^2 / W
-        if (w > 0.0) acc[12] += (gg.x * gg.x + gg.y * gg.y + gg.z * gg.z + gg.w * gg.w) / w;
+        const double t = bin_freq(gi.k_min, i, gi.df) - f_b;
+#pragma unroll
+        for (int c = 0; c < NC; ++c) {
+            const double2 gg = reinterpret_cast<const double2 *>(g)[(size_t)i * NC + c]; // W conj(d): (W d_re, -W d_im)
+            const double w = Wc[(w_rows > 1 ? (size_t)c * n_f_pad : 0) + i];
+            const double2 hc = reinterpret_cast<const double2 *>(h0)[(size_t)c * gi.n_f + i];
+            // W d conj(h0) = conj( (W conj d) h0 )
+            const double pr = gg.x * hc.x - gg.y * hc.y, pi = -(gg.x * hc.y + gg.y * hc.x);
+            const double q = w * (hc.x * hc.x + hc.y * hc.y);
+            double *o = acc + 6 * c;
+            o[0] += pr; o[1] += pi; o[2] = fma(pr, t, o[2]); o[3] = fma(pi, t, o[3]);
+            o[4] += q; o[5] = fma(q, t, o[5]);
+            // W |d|^2 = |W conj d|^2 / W
+            if (w > 0.0) acc[6 * NC] += (gg.x * gg.x + gg.y * gg.y) / w;
+        }
     }
 #pragma unroll
-    for (int q = 0; q < 13; ++q) {
+    for (int q = 0; q < NR; ++q) {
         const double tot = block_sum_256(acc[q], sh);
-        if (threadIdx.x == 0) raw[(size_t)b * 13 + q] = tot;
+        if (threadIdx.x == 0) raw[(size_t)b * NR + q] = tot;
     }
 }
 
 // ---------------------------------------------------------------------------------------------------
 // H1-H3: heterodyned likelihood.  Packed table (host-built by ll_het_prepare), all in shared memory:
-//   edge e : f4[e] = 4 f_e; ih0[e][4] = 1/h0^A (re, im), 1/h0^E (re, im);
-//            per mode m: cfp[m][e] = c_lm f_e^(-7/6), f2m[m][e] = 2 f_e/m, fm53[m][e] = (2 f_e/m)^(-5/3)
-//   bin b  : A0h[4] = A0/2 (A re, im, E re, im), A1w[4] = A1/(e_{b+1}-e_b), B0q[2] = B0/4, B1w[2] = B1/(e_{b+1}-e_b)
+//   edge e : f4[e] = 4 f_e; ih0[e][2 NC] = 1/h0^c (re, im) per channel;
+//            per mode m: cfp[m][e] = c_lm f_e^(-7/6), f2m[m][e] = 2 f_e/m, fm53[m][e] = (m/pi) (2 f_e/m)^(-5/3)
+//   bin b  : [6 NC] = A0h[2 NC] = A0/2 (re, im per channel), A1w[2 NC] = A1/(e_{b+1}-e_b), B0q[NC] = B0/4,
+//            B1w[NC] = B1/(e_{b+1}-e_b)
 // With s = r_lo + r_hi and dlt = r_hi - r_lo:  r0 = s/2, r1 = dlt/width                         (Eq. 11), so
 //   Z[d,h] term = Re[A0 conj r0 + A1 conj r1] = A0h . s + A1w . dlt                              (Eq. 14)
 //   Z[h,h] term = B0 |r0|^2 + 2 B1 Re[r0 conj r1] = B0q |s|^2 + B1w (s . dlt)                    (Eq. 17)
+// The per-channel weights (reading R5) enter only through the summary data, i.e. through ll_het_prepare.
 // ---------------------------------------------------------------------------------------------------
 struct HetTable {
     const double *base; // device copy of the packed table
-    int n_e, n_b, n_m;
+    int n_e, n_b, n_m, n_c;
     int total;          // doubles
     __host__ __device__ int off_f4() const { return 0; }
     __host__ __device__ int off_ih0() const { return n_e; }
-    __host__ __device__ int off_cfp() const { return 5 * n_e; }
-    __host__ __device__ int off_f2m() const { return 5 * n_e + n_m * n_e; }
-    __host__ __device__ int off_fm53() const { return 5 * n_e + 2 * n_m * n_e; }
-    __host__ __device__ int off_bins() const { return 5 * n_e + 3 * n_m * n_e; }
+    __host__ __device__ int off_cfp() const { return (1 + 2 * n_c) * n_e; }
+    __host__ __device__ int off_f2m() const { return (1 + 2 * n_c) * n_e + n_m * n_e; }
+    __host__ __device__ int off_fm53() const { return (1 + 2 * n_c) * n_e + 2 * n_m * n_e; }
+    __host__ __device__ int off_bins() const { return (1 + 2 * n_c) * n_e + 3 * n_m * n_e; }
+    __host__ __device__ int bin_stride() const { return 6 * n_c; }
 };
 
-__device__ __forceinline__ void het_bin_contract(const double *__restrict__ tb, double lAr, double lAi, double lEr,
-                                                 double lEi, double hAr, double hAi, double hEr, double hEi,
-                                                 double &dh, double &hh)
+template <int NC>
+__device__ __forceinline__ void het_bin_contract(const double *__restrict__ tb, const double (&l)[2 * NC],
+                                                 const double (&h)[2 * NC], double &dh, double &hh)
 {
-    const double sAr = lAr + hAr, sAi = lAi + hAi, sEr = lEr + hEr, sEi = lEi + hEi;
-    const double dAr = hAr - lAr, dAi = hAi - lAi, dEr = hEr - lEr, dEi = hEi - lEi;
-    dh = fma(tb[0], sAr, dh); dh = fma(tb[1], sAi, dh); dh = fma(tb[2], sEr, dh); dh = fma(tb[3], sEi, dh);
-    dh = fma(tb[4], dAr, dh); dh = fma(tb[5], dAi, dh); dh = fma(tb[6], dEr, dh); dh = fma(tb[7], dEi, dh);
-    hh = fma(tb[8], fma(sAr, sAr, sAi * sAi), hh);
-    hh = fma(tb[9], fma(sEr, sEr, sEi * sEi), hh);
-    hh = fma(tb[10], fma(sAr, dAr, sAi * dAi), hh);
-    hh = fma(tb[11], fma(sEr, dEr, sEi * dEi), hh);
+    double s[2 * NC], d[2 * NC];
+#pragma unroll
+    for (int q = 0; q < 2 * NC; ++q) { s[q] = l[q] + h[q]; d[q] = h[q] - l[q]; }
+#pragma unroll
+    for (int q = 0; q < 2 * NC; ++q) dh = fma(tb[q], s[q], dh);
+#pragma unroll
+    for (int q = 0; q < 2 * NC; ++q) dh = fma(tb[2 * NC + q], d[q], dh);
+#pragma unroll
+    for (int c = 0; c < NC; ++c) hh = fma(tb[4 * NC + c], fma(s[2 * c], s[2 * c], s[2 * c + 1] * s[2 * c + 1]), hh);
+#pragma unroll
+    for (int c = 0; c < NC; ++c) hh = fma(tb[5 * NC + c], fma(s[2 * c], d[2 * c], s[2 * c + 1] * d[2 * c + 1]), hh);
 }
 
 // Stand-in parameters -> log L.  Block = 32 lanes x (G walker groups x S frequency segments) warps sharing ONE
@@ -2028,32 +2218,35 @@ __device__ __forceinline__ void het_bin_contract(const double *__restrict__ tb, 
 // G groups; the S partial sums of a group meet in shared memory in segment order (deterministic).
 //
 // Inside a segment the edges go in chunks of E = 4 with the MODE loop outside the edge loop: the transfer factors
-// of a mode are read once per chunk (from a lane-major shared copy, so they do not occupy 4 n_m registers for
+// of a mode are read once per chunk (from a lane-major shared copy, so they do not occupy 2 NC n_m registers for
 // the whole kernel), and the four edges of a chunk are four independent phase -> sincos -> T^c h chains in
 // flight per thread (with 16 warps per SM the FP64 pipe needs that instruction-level parallelism).  Whether any
 // lane needs the taper polynomial is decided once per chunk (warp-uniform), below f_ISCO m_min/2 it is 1.
 struct HetEdgeCtx {
     const double *f4, *ih0, *cfp, *f2m, *fm53;
-    const double *tfs; // shared: this lane's staged parameter row + 5, i.e. T^c_m (re, im) mode-major, [n_m][4]
+    const double *tfs; // shared: this lane's staged parameter row + 5, i.e. T^c_m (re, im) mode-major, [n_m][2 NC]
     const double *nmq; // shared, [n_m]: -(m/pi)
     int n_e;
     double tc, invD, inv_fisco, K, phi0, kappa, inv_kappa;
 };
 
-template <int NM, int E, bool TAPER>
-__device__ __forceinline__ void het_eval_edges(const HetEdgeCtx &x, const StandinInfo &si, int e, double (&r)[E][4])
+template <int NM, int NC, int E, bool TAPER>
+__device__ __forceinline__ void het_eval_edges(const HetEdgeCtx &x, const StandinInfo &si, int e, double (&r)[E][2 * NC])
 {
-    double h[E][4], ftc[E];
+    double h[E][2 * NC], ftc[E];
 #pragma unroll
     for (int k = 0; k < E; ++k) {
-        h[k][0] = h[k][1] = h[k][2] = h[k][3] = 0.0;
+#pragma unroll
+        for (int q = 0; q < 2 * NC; ++q) h[k][q] = 0.0;
         ftc[k] = x.f4[e + k] * x.tc;
     }
 #pragma unroll 1
     for (int m = 0; m < NM; ++m) {
         const double nmq = x.nmq[m]; // -(m/pi), shared
-        const double *tq = x.tfs + m * 4;
-        const double t0 = tq[0], t1 = tq[1], t2 = tq[2], t3 = tq[3];
+        const double *tq = x.tfs + m * 2 * NC;
+        double tf[2 * NC];
+#pragma unroll
+        for (int q = 0; q < 2 * NC; ++q) tf[q] = tq[q];
         const int t = m * x.n_e + e;
 #pragma unroll
         for (int k = 0; k < E; ++k) {
@@ -2063,19 +2256,17 @@ __device__ __forceinline__ void het_eval_edges(const HetEdgeCtx &x, const Standi
             if (TAPER) A *= taper_nobranch(x.f2m[t + k] * x.inv_fisco, x.kappa, x.inv_kappa);
             double u, v; // h_m = u - i v
             amp_expi_qc(A, y, u, v);
-            h[k][0] = fma(t0, u, h[k][0]); h[k][0] = fma(t1, v, h[k][0]);
-            h[k][1] = fma(t1, u, h[k][1]); h[k][1] = fma(-t0, v, h[k][1]);
-            h[k][2] = fma(t2, u, h[k][2]); h[k][2] = fma(t3, v, h[k][2]);
-            h[k][3] = fma(t3, u, h[k][3]); h[k][3] = fma(-t2, v, h[k][3]);
+            apply_tf<NC>(tf, u, v, h[k]);
         }
     }
 #pragma unroll
     for (int k = 0; k < E; ++k) { // r = h * (1/h0)
-        const double *g = x.ih0 + 4 * (e + k);
-        r[k][0] = h[k][0] * g[0] - h[k][1] * g[1];
-        r[k][1] = h[k][0] * g[1] + h[k][1] * g[0];
-        r[k][2] = h[k][2] * g[2] - h[k][3] * g[3];
-        r[k][3] = h[k][2] * g[3] + h[k][3] * g[2];
+        const double *g = x.ih0 + 2 * NC * (e + k);
+#pragma unroll
+        for (int c = 0; c < NC; ++c) {
+            r[k][2 * c] = h[k][2 * c] * g[2 * c] - h[k][2 * c + 1] * g[2 * c + 1];
+            r[k][2 * c + 1] = h[k][2 * c] * g[2 * c + 1] + h[k][2 * c + 1] * g[2 * c];
+        }
     }
 }
 
@@ -2085,13 +2276,14 @@ __device__ __forceinline__ void het_eval_edges(const HetEdgeCtx &x, const Standi
 #ifndef LL_HET_WY
 #define LL_HET_WY 16 // warps per block (one block per SM: the table copy is shared by all of them)
 #endif
-template <int NM>
+template <int NM, int NC>
 __global__ void __launch_bounds__(32 * LL_HET_WY)
 k_het_standin(HetTable T, StandinInfo si, const double *__restrict__ params, int P, int n_w, int n_groups, int S,
               const double *__restrict__ dd, double *__restrict__ logL, double *__restrict__ d_h,
               double *__restrict__ h_h)
 {
     constexpr int E = LL_HET_E;
+    constexpr int BS = 6 * NC; // table doubles per bin
     extern __shared__ __align__(16) double tab[];
     const int G = blockDim.y / S, seg = threadIdx.y % S, gslot = threadIdx.y / S, lane = threadIdx.x;
     double *red = tab + T.total;                 // [G][S][2][32]
@@ -2119,7 +2311,7 @@ k_het_standin(HetTable T, StandinInfo si, const double *__restrict__ params, int
         const bool valid = grp < n_groups && w < n_w;
         __syncthreads(); // table staged (first pass) / previous pass done with the staged rows and red
         {   // the G x 32 parameter rows of this pass are contiguous in memory: the whole block stages them with
-            // coalesced loads (instead of one warp reading 4 n_m strided values per lane while the others wait)
+            // coalesced loads (instead of one warp reading 2 NC n_m strided values per lane while the others wait)
             const long long r0 = (long long)base * 32 * P, r1 = min((long long)(base + G) * 32, (long long)n_w) * P;
             for (long long i = r0 + threadIdx.x + threadIdx.y * 32; i < r1; i += 32 * blockDim.y) tfs_all[i - r0] = params[i];
         }
@@ -2133,27 +2325,31 @@ k_het_standin(HetTable T, StandinInfo si, const double *__restrict__ params, int
         const double x_scale = c.inv_fisco * (0.5 / (double)m_min);
         double dh = 0.0, hh = 0.0;
         if (grp < n_groups && b0 < b1) {
-            double pr[1][4];
-            if (__any_sync(0xffffffffu, x.f4[b0] * x_scale > 1.0)) het_eval_edges<NM, 1, true>(x, si, b0, pr);
-            else het_eval_edges<NM, 1, false>(x, si, b0, pr);
-            double pAr = pr[0][0], pAi = pr[0][1], pEr = pr[0][2], pEi = pr[0][3];
+            double pr[1][2 * NC];
+            if (__any_sync(0xffffffffu, x.f4[b0] * x_scale > 1.0)) het_eval_edges<NM, NC, 1, true>(x, si, b0, pr);
+            else het_eval_edges<NM, NC, 1, false>(x, si, b0, pr);
+            double prev[2 * NC];
+#pragma unroll
+            for (int q = 0; q < 2 * NC; ++q) prev[q] = pr[0][q];
             int e = b0 + 1;
             for (; e + E <= b1 + 1; e += E) {
-                double r[E][4];
-                if (__any_sync(0xffffffffu, x.f4[e + E - 1] * x_scale > 1.0)) het_eval_edges<NM, E, true>(x, si, e, r);
-                else het_eval_edges<NM, E, false>(x, si, e, r);
+                double r[E][2 * NC];
+                if (__any_sync(0xffffffffu, x.f4[e + E - 1] * x_scale > 1.0)) het_eval_edges<NM, NC, E, true>(x, si, e, r);
+                else het_eval_edges<NM, NC, E, false>(x, si, e, r);
 #pragma unroll
                 for (int k = 0; k < E; ++k) {
-                    het_bin_contract(bins + 12 * (e + k - 1), pAr, pAi, pEr, pEi, r[k][0], r[k][1], r[k][2], r[k][3], dh, hh);
-                    pAr = r[k][0]; pAi = r[k][1]; pEr = r[k][2]; pEi = r[k][3];
+                    het_bin_contract<NC>(bins + BS * (e + k - 1), prev, r[k], dh, hh);
+#pragma unroll
+                    for (int q = 0; q < 2 * NC; ++q) prev[q] = r[k][q];
                 }
             }
             for (; e <= b1; ++e) {
-                double r[1][4];
-                if (__any_sync(0xffffffffu, x.f4[e] * x_scale > 1.0)) het_eval_edges<NM, 1, true>(x, si, e, r);
-                else het_eval_edges<NM, 1, false>(x, si, e, r);
-                het_bin_contract(bins + 12 * (e - 1), pAr, pAi, pEr, pEi, r[0][0], r[0][1], r[0][2], r[0][3], dh, hh);
-                pAr = r[0][0]; pAi = r[0][1]; pEr = r[0][2]; pEi = r[0][3];
+                double r[1][2 * NC];
+                if (__any_sync(0xffffffffu, x.f4[e] * x_scale > 1.0)) het_eval_edges<NM, NC, 1, true>(x, si, e, r);
+                else het_eval_edges<NM, NC, 1, false>(x, si, e, r);
+                het_bin_contract<NC>(bins + BS * (e - 1), prev, r[0], dh, hh);
+#pragma unroll
+                for (int q = 0; q < 2 * NC; ++q) prev[q] = r[0][q];
             }
         }
         if (S > 1) {
@@ -2176,7 +2372,7 @@ k_het_standin(HetTable T, StandinInfo si, const double *__restrict__ params, int
 
 // ---------------------------------------------------------------------------------------------------
 // H1-H3, single mode, regrouped by edge.  With one mode and constant T^c, r^c_e = T^c z_e / h0^c_e with
-// z_e = A(f_e) e^{-i Psi(f_e)} common to both channels, and Eq. 14 / Eq. 17 regroup exactly into sums over edges:
+// z_e = A(f_e) e^{-i Psi(f_e)} common to all channels, and Eq. 14 / Eq. 17 regroup exactly into sums over edges:
 //   Z[d,h] = Re sum_c conj(T^c) sum_e conj(z_e) Q^c_e,
 //            Q^c_e = conj(1/h0^c_e) (A0_{e-1}/2 + A1_{e-1}/D_{e-1} + A0_e/2 - A1_e/D_e)            (Eq. 11, 14)
 //   Z[h,h] = sum_c |T^c|^2 ( sum_e |z_e|^2 P^c_e + sum_b Re[z_b conj(z_{b+1}) X^c_b] ),
@@ -2184,9 +2380,10 @@ k_het_standin(HetTable T, StandinInfo si, const double *__restrict__ params, int
 //            X^c_b = (B0_b/2) (1/h0^c_b) conj(1/h0^c_{b+1})                                         (Eq. 11, 17)
 // (D_b = f_{b+1} - f_b; terms whose bin index falls outside [0, n_b) are absent; 2 Re[r0 conj r1] =
 // (|r_hi|^2 - |r_lo|^2)/D.)  Same arithmetic as the bin-by-bin form up to rounding; 48 instead of 73 FP64 slots
-// per (walker, bin).  Table: 14 doubles per edge, resident in shared memory, every read a broadcast.
+// per (walker, bin) for two channels.  Table: 4 + 5 NC doubles per edge (f4, fm53, cfp, f2m, then Q^c (re, im) per
+// channel, P^c per channel, X^c (re, im) per channel), resident in shared memory, every read a broadcast.
 // ---------------------------------------------------------------------------------------------------
-constexpr int kHet1Stride = 14; // f4, fm53, cfp, f2m, QAr, QAi, QEr, QEi, PA, PE, XAr, XAi, XEr, XEi
+__host__ __device__ constexpr int het1_stride(int n_c) { return 4 + 5 * n_c; }
 
 struct Het1Table {
     const double *base;
@@ -2196,19 +2393,19 @@ struct Het1Table {
 #ifndef LL_HET1_WY
 #define LL_HET1_WY 16 // warps per block of the single-mode kernel (one block per SM shares the table copy)
 #endif
+template <int NC>
 __global__ void __launch_bounds__(32 * LL_HET1_WY)
 k_het_standin1(Het1Table T, StandinInfo si, const double *__restrict__ params, int P, int n_w, int n_groups, int S,
                const double *__restrict__ dd, double *__restrict__ logL, double *__restrict__ d_h,
                double *__restrict__ h_h)
 {
+    constexpr int ST = het1_stride(NC);
+    constexpr int oQ = 4, oP = 4 + 2 * NC, oX = 4 + 3 * NC; // offsets of Q, P, X inside an edge's row
+    constexpr int NR = 3 * NC;                               // partial sums per walker: D^c (re, im), H^c
     extern __shared__ __align__(16) double tab[];
-    const int total = T.n_e * kHet1Stride;
-    double *red = tab + total; // [G][S][6][32]
-    {
-        const double2 *src = reinterpret_cast<const double2 *>(T.base);
-        double2 *dst = reinterpret_cast<double2 *>(tab);
-        for (int i = threadIdx.x + threadIdx.y * 32; i < total / 2; i += 32 * blockDim.y) dst[i] = src[i];
-    }
+    const int total = T.n_e * ST;
+    double *red = tab + total + (total & 1); // [G][S][NR][32]
+    for (int i = threadIdx.x + threadIdx.y * 32; i < total; i += 32 * blockDim.y) tab[i] = T.base[i];
     __syncthreads();
     const int G = blockDim.y / S, seg = threadIdx.y % S, gslot = threadIdx.y / S, lane = threadIdx.x;
     const int per = (T.n_e + S - 1) / S;
@@ -2224,41 +2421,49 @@ k_het_standin1(Het1Table T, StandinInfo si, const double *__restrict__ params, i
         const double *row = params + (size_t)(valid ? w : 0) * P;
         const WalkerConst c = standin_consts(row);
         const double Kq = mh_pi * c.K, nphq = -mh_pi * (c.phi + 0.25 * kPi);
-        double DAr = 0, DAi = 0, DEr = 0, DEi = 0, HA = 0, HE = 0;
+        double D[2 * NC], H[NC];
+#pragma unroll
+        for (int q = 0; q < 2 * NC; ++q) D[q] = 0.0;
+#pragma unroll
+        for (int q = 0; q < NC; ++q) H[q] = 0.0;
         if (grp < n_groups && e0 < e1) {
             auto edge = [&](const double *t, double &u, double &v, double &amp) {
                 const double y = fma(t[0], c.tc, fma(Kq, t[1], nphq));
                 amp = t[2] * c.invD * taper(t[3] * c.inv_fisco, si.kappa, inv_kappa);
                 amp_expi_qc(amp, y, u, v); // z = u - i v
             };
-            const double *t = tab + (size_t)e0 * kHet1Stride;
+            const double *t = tab + (size_t)e0 * ST;
             double up, vp, ap;
             edge(t, up, vp, ap);
             const int last = min(e1, T.n_b); // one past the last bin whose cross term this segment owns
             auto edge_terms = [&](const double *tt, double u, double v, double a) { // conj(z) Q and |z|^2 P of one edge
-                DAr = fma(u, tt[4], DAr); DAr = fma(-v, tt[5], DAr);
-                DAi = fma(u, tt[5], DAi); DAi = fma(v, tt[4], DAi);
-                DEr = fma(u, tt[6], DEr); DEr = fma(-v, tt[7], DEr);
-                DEi = fma(u, tt[7], DEi); DEi = fma(v, tt[6], DEi);
                 const double a2 = a * a;
-                HA = fma(a2, tt[8], HA);
-                HE = fma(a2, tt[9], HE);
+#pragma unroll
+                for (int cc = 0; cc < NC; ++cc) {
+                    const double qr = tt[oQ + 2 * cc], qi = tt[oQ + 2 * cc + 1];
+                    D[2 * cc] = fma(u, qr, D[2 * cc]); D[2 * cc] = fma(-v, qi, D[2 * cc]);
+                    D[2 * cc + 1] = fma(u, qi, D[2 * cc + 1]); D[2 * cc + 1] = fma(v, qr, D[2 * cc + 1]);
+                    H[cc] = fma(a2, tt[oP + cc], H[cc]);
+                }
             };
             auto cross_terms = [&](const double *tt, double u0, double v0, double u1, double v1) { // z_e conj(z_{e+1}) X
                 const double wr = fma(u0, u1, v0 * v1), wi = fma(u0, v1, -(v0 * u1));
-                HA = fma(wr, tt[10], HA); HA = fma(-wi, tt[11], HA);
-                HE = fma(wr, tt[12], HE); HE = fma(-wi, tt[13], HE);
+#pragma unroll
+                for (int cc = 0; cc < NC; ++cc) {
+                    H[cc] = fma(wr, tt[oX + 2 * cc], H[cc]);
+                    H[cc] = fma(-wi, tt[oX + 2 * cc + 1], H[cc]);
+                }
             };
             int e = e0;
             // chunks of kE bins: the kE next edges are kE independent phase -> sincos chains in flight per thread;
             // the taper polynomial is needed only where some lane is above its f_ISCO (one warp-uniform test per chunk)
             constexpr int kE = 4;
-            for (; e + kE <= last; e += kE, t += kE * kHet1Stride) {
+            for (; e + kE <= last; e += kE, t += kE * ST) {
                 double un[kE], vn[kE], an[kE];
-                const bool tapered = __any_sync(0xffffffffu, t[kE * kHet1Stride + 3] * c.inv_fisco > 1.0);
+                const bool tapered = __any_sync(0xffffffffu, t[kE * ST + 3] * c.inv_fisco > 1.0);
 #pragma unroll
                 for (int k = 0; k < kE; ++k) {
-                    const double *tn = t + (k + 1) * kHet1Stride;
+                    const double *tn = t + (k + 1) * ST;
                     const double y = fma(tn[0], c.tc, fma(Kq, tn[1], nphq));
                     double a = tn[2] * c.invD;
                     if (tapered) a *= taper_nobranch(tn[3] * c.inv_fisco, si.kappa, inv_kappa);
@@ -2267,41 +2472,54 @@ k_het_standin1(Het1Table T, StandinInfo si, const double *__restrict__ params, i
                 }
 #pragma unroll
                 for (int k = 0; k < kE; ++k) {
-                    const double *tt = t + k * kHet1Stride;
+                    const double *tt = t + k * ST;
                     const double u0 = k ? un[k - 1] : up, v0 = k ? vn[k - 1] : vp, a0 = k ? an[k - 1] : ap;
                     edge_terms(tt, u0, v0, a0);
                     cross_terms(tt, u0, v0, un[k], vn[k]);
                 }
                 up = un[kE - 1]; vp = vn[kE - 1]; ap = an[kE - 1];
             }
-            for (; e < e1; ++e, t += kHet1Stride) {
+            for (; e < e1; ++e, t += ST) {
                 edge_terms(t, up, vp, ap);
                 if (e < last) { // bin e = [e, e + 1]: needs z at e + 1 (the next segment's first edge at the boundary)
                     double un, vn, an;
-                    edge(t + kHet1Stride, un, vn, an);
+                    edge(t + ST, un, vn, an);
                     cross_terms(t, up, vp, un, vn);
                     up = un; vp = vn; ap = an;
                 }
             }
         }
         if (S > 1) {
-            double *rg = red + (size_t)gslot * S * 192;
-            double *q = rg + seg * 192 + lane;
-            q[0] = DAr; q[32] = DAi; q[64] = DEr; q[96] = DEi; q[128] = HA; q[160] = HE;
+            double *rg = red + (size_t)gslot * S * (NR * 32);
+            double *q = rg + seg * (NR * 32) + lane;
+#pragma unroll
+            for (int k = 0; k < 2 * NC; ++k) q[32 * k] = D[k];
+#pragma unroll
+            for (int k = 0; k < NC; ++k) q[32 * (2 * NC + k)] = H[k];
             __syncthreads();
             if (seg == 0) {
-                DAr = DAi = DEr = DEi = HA = HE = 0.0;
+#pragma unroll
+                for (int k = 0; k < 2 * NC; ++k) D[k] = 0.0;
+#pragma unroll
+                for (int k = 0; k < NC; ++k) H[k] = 0.0;
                 for (int s = 0; s < S; ++s) {
-                    const double *r = rg + s * 192 + lane;
-                    DAr += r[0]; DAi += r[32]; DEr += r[64]; DEi += r[96]; HA += r[128]; HE += r[160];
+                    const double *r = rg + s * (NR * 32) + lane;
+#pragma unroll
+                    for (int k = 0; k < 2 * NC; ++k) D[k] += r[32 * k];
+#pragma unroll
+                    for (int k = 0; k < NC; ++k) H[k] += r[32 * (2 * NC + k)];
                 }
             }
         }
         if (seg == 0 && valid) {
-            const double tar = row[5], tai = row[6], ter = row[7], tei = row[8];
-            // Re[conj(T^A) D^A + conj(T^E) D^E],  |T^A|^2 H^A + |T^E|^2 H^E
-            const double dh = (tar * DAr + tai * DAi) + (ter * DEr + tei * DEi);
-            const double hh = (tar * tar + tai * tai) * HA + (ter * ter + tei * tei) * HE;
+            // Re sum_c conj(T^c) D^c,  sum_c |T^c|^2 H^c
+            double dh = 0.0, hh = 0.0;
+#pragma unroll
+            for (int cc = 0; cc < NC; ++cc) {
+                const double tr = row[5 + 2 * cc], ti = row[6 + 2 * cc];
+                dh += tr * D[2 * cc] + ti * D[2 * cc + 1];
+                hh += (tr * tr + ti * ti) * H[cc];
+            }
             logL[w] = dh - 0.5 * hh - 0.5 * ddb;
             if (d_h) d_h[w] = dh;
             if (h_h) h_h[w] = hh;
@@ -2310,46 +2528,72 @@ k_het_standin1(Het1Table T, StandinInfo si, const double *__restrict__ params, i
     }
 }
 
+// sin and cos of (x radians + lin quarter cycles): x is reduced by Cody-Waite, the small second term is added to the
+// reduced argument (the linear phase term of reading R32 arrives already reduced modulo one cycle)
+__device__ __forceinline__ void sincos_rad_plus_qc(double x, double lin, double &sn, double &cs)
+{
+    const double sh = __dadd_rn(x * kTwoOverPi, kMagic);
+    const int q = __double2loint(sh);
+    const double nd = __dadd_rn(sh, -kMagic);
+    double r = fma(-nd, kPio2_1, x);
+    r = fma(-nd, kPio2_2, r);
+    r = fma(-nd, kPio2_3, r);
+    sincos_qc(fma(r, kTwoOverPi, lin) + (double)(q & 3), sn, cs);
+}
+
 // Array entry point: amp_e, phase_e [n_w][n_m][n_e] (radians).  One warp per walker, lanes over edges (the
 // arrays are walker-major, so this is the coalesced direction); neighbouring edges meet through a shuffle.
+// t_shift [n_w] or nullptr: Psi_m(f_e) = phase_e + 2 pi f_e t_shift (reading R32).
+template <int NC>
 __global__ void __launch_bounds__(256)
 k_het_arrays(HetTable T, const double *__restrict__ amp_e, const double *__restrict__ phase_e,
-             const double *__restrict__ tf, int n_w, const double *__restrict__ dd, double *__restrict__ logL,
-             double *__restrict__ d_h, double *__restrict__ h_h)
+             const double *__restrict__ tf, const double *__restrict__ t_shift, int n_w, const double *__restrict__ dd,
+             double *__restrict__ logL, double *__restrict__ d_h, double *__restrict__ h_h)
 {
+    constexpr int BS = 6 * NC;
     extern __shared__ __align__(16) double tab[];
     for (int i = threadIdx.x; i < T.total; i += blockDim.x) tab[i] = T.base[i];
     __syncthreads();
-    const double *ih0 = tab + T.off_ih0(), *bins = tab + T.off_bins();
+    const double *ih0 = tab + T.off_ih0(), *bins = tab + T.off_bins(), *f4 = tab + T.off_f4();
     const int lane = threadIdx.x & 31, wpb = blockDim.x >> 5;
     const double ddb = dd[1];
     for (int w = blockIdx.x * wpb + (threadIdx.x >> 5); w < n_w; w += gridDim.x * wpb) {
         double dh = 0.0, hh = 0.0;
+        const double ts = t_shift ? t_shift[w] : 0.0;
         for (int base = 0; base < T.n_b; base += 31) {
             const int e = base + lane;
-            double rAr = 0, rAi = 0, rEr = 0, rEi = 0;
+            double r[2 * NC];
+#pragma unroll
+            for (int q = 0; q < 2 * NC; ++q) r[q] = 0.0;
             if (e < T.n_e) {
-                double hAr = 0, hAi = 0, hEr = 0, hEi = 0;
+                double h[2 * NC];
+#pragma unroll
+                for (int q = 0; q < 2 * NC; ++q) h[q] = 0.0;
+                const double lin = t_shift ? qc_linear_mod_cycle(f4[e], ts) : 0.0; // 4 f_e t_shift quarter cycles
                 for (int m = 0; m < T.n_m; ++m) {
                     const size_t idx = ((size_t)w * T.n_m + m) * T.n_e + e;
                     const double A = amp_e[idx];
                     double sn, cs;
-                    sincos_rad(phase_e[idx], sn, cs);
+                    if (t_shift) sincos_rad_plus_qc(phase_e[idx], lin, sn, cs);
+                    else sincos_rad(phase_e[idx], sn, cs);
                     const double u = A * cs, v = A * sn;
-                    const double *t4 = tf + ((size_t)w * T.n_m + m) * 4;
-                    const double tar = __ldg(t4), tai = __ldg(t4 + 1), ter = __ldg(t4 + 2), tei = __ldg(t4 + 3);
-                    hAr = fma(tar, u, hAr); hAr = fma(tai, v, hAr);
-                    hAi = fma(tai, u, hAi); hAi = fma(-tar, v, hAi);
-                    hEr = fma(ter, u, hEr); hEr = fma(tei, v, hEr);
-                    hEi = fma(tei, u, hEi); hEi = fma(-ter, v, hEi);
+                    const double *t4 = tf + ((size_t)w * T.n_m + m) * 2 * NC;
+                    double tfr[2 * NC];
+#pragma unroll
+                    for (int q = 0; q < 2 * NC; ++q) tfr[q] = __ldg(t4 + q);
+                    apply_tf<NC>(tfr, u, v, h);
                 }
-                const double *g = ih0 + 4 * e;
-                rAr = hAr * g[0] - hAi * g[1]; rAi = hAr * g[1] + hAi * g[0];
-                rEr = hEr * g[2] - hEi * g[3]; rEi = hEr * g[3] + hEi * g[2];
+                const double *g = ih0 + 2 * NC * e;
+#pragma unroll
+                for (int c = 0; c < NC; ++c) {
+                    r[2 * c] = h[2 * c] * g[2 * c] - h[2 * c + 1] * g[2 * c + 1];
+                    r[2 * c + 1] = h[2 * c] * g[2 * c + 1] + h[2 * c + 1] * g[2 * c];
+                }
             }
-            const double nAr = __shfl_down_sync(0xffffffffu, rAr, 1), nAi = __shfl_down_sync(0xffffffffu, rAi, 1);
-            const double nEr = __shfl_down_sync(0xffffffffu, rEr, 1), nEi = __shfl_down_sync(0xffffffffu, rEi, 1);
-            if (lane < 31 && e < T.n_b) het_bin_contract(bins + 12 * e, rAr, rAi, rEr, rEi, nAr, nAi, nEr, nEi, dh, hh);
+            double nx[2 * NC];
+#pragma unroll
+            for (int q = 0; q < 2 * NC; ++q) nx[q] = __shfl_down_sync(0xffffffffu, r[q], 1);
+            if (lane < 31 && e < T.n_b) het_bin_contract<NC>(bins + BS * e, r, nx, dh, hh);
         }
         dh = warp_sum(dh);
         hh = warp_sum(hh);

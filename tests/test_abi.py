@@ -39,7 +39,7 @@ def test_library_exports_every_declared_symbol(so_path):
     assert sorted(binding.SYMBOLS) == names
     for n in names:
         assert hasattr(lib, n), n
-    assert lib.ll_abi_version() == 2
+    assert lib.ll_abi_version() == 3
 
 
 def test_library_is_sm100a_only(so_path):
@@ -51,13 +51,14 @@ def test_library_is_sm100a_only(so_path):
 
 
 def test_tma_and_mbarrier_in_fused_kernel_sass(so_path):
-    out = subprocess.run(["cuobjdump", "-sass", "-fun", "_ZN2ll12k_full_fusedILi1EEEvNS_9FusedArgsE", so_path],
-                         capture_output=True, text=True)
-    if out.returncode != 0 or not out.stdout:
-        pytest.skip("cuobjdump unavailable")
-    assert "UBLKCP" in out.stdout          # cp.async.bulk (1-D TMA)
-    assert "SYNCS" in out.stdout           # mbarrier
-    assert "DFMA" in out.stdout
+    # k_full_fused<1, 2, true> (two channels, shared weight row: the bench's kernel) and <1, 3, false> (A, E, T)
+    for fun in ("_ZN2ll12k_full_fusedILi1ELi2ELb1EEEvNS_9FusedArgsE", "_ZN2ll12k_full_fusedILi1ELi3ELb0EEEvNS_9FusedArgsE"):
+        out = subprocess.run(["cuobjdump", "-sass", "-fun", fun, so_path], capture_output=True, text=True)
+        if out.returncode != 0 or not out.stdout:
+            pytest.skip("cuobjdump unavailable")
+        assert "UBLKCP" in out.stdout          # cp.async.bulk (1-D TMA)
+        assert "SYNCS" in out.stdout           # mbarrier
+        assert "DFMA" in out.stdout
 
 
 def test_no_cpu_fallback_without_gpu(so_path):
@@ -77,7 +78,7 @@ def test_create_rejects_bad_config(so_path):
     from paper_2111_01064_b200 import binding
     lib = binding.load_library()
     h = C.c_void_p()
-    for dev, nc, nm, prec, bc in ((0, 3, 1, 0, 0), (0, 2, 0, 0, 0), (0, 2, 9, 0, 0), (0, 2, 1, 7, 0), (0, 2, 1, 0, 2)):
+    for dev, nc, nm, prec, bc in ((0, 4, 1, 0, 0), (0, 1, 1, 0, 0), (0, 2, 0, 0, 0), (0, 2, 9, 0, 0), (0, 2, 1, 7, 0), (0, 2, 1, 0, 2)):
         cfg = binding.ll_config(dev, nc, nm, prec, bc, (C.c_int32 * 3)(0, 0, 0))
         assert lib.ll_create(C.byref(cfg), C.byref(h)) == binding.LL_ERR_UNSUPPORTED
     assert lib.ll_create(None, C.byref(h)) == binding.LL_ERR_ARG
