@@ -32,20 +32,26 @@ from paper_2111_01064_b200 import workloads as wlm  # noqa: E402
 
 METRIC = "log-likelihood evals/sec"
 UNIT = "evals/s"
-# algorithmic FP64 issue slots per active (walker, bin, mode) of the full-grid path.  Direct formulation (DESIGN.md §6:
-# t 1, two cubics 6, reduce 3, sincos 18, A e^{-i Psi} 2, two complex MACs 8, W A^2 2 => 40; SURVEY.md §8(d) uses 39).
-# The single-mode FP64 kernel advances e^{-i Psi} and A by recurrence (three complex rotations and three additions per
-# bin, re-synchronised from the cubics every 32 bins), and SURVEY §8(d) asks that such a build quote ITS count:
-# 12 + 3 + 2 + 8 + 2 = 27 per bin plus (2 cubics 6 + differences 16 + 3 sincos 54 + 3 normalisations 15 + 1)/32 = 2.9 => 30
+# Algorithmic FP64 issue slots per unit (1 DFMA | DMUL | DADD = 1 slot).
+# Full grid, per active (walker, bin, mode).  Direct formulation: t 1, two cubics 6, reduce 3, sincos 18, A e^{-i Psi} 2,
+# two complex MACs 8, W A^2 2 => 39.  The single-mode FP64 kernels advance e^{-i Psi} and A by recurrence, and
+# SURVEY §8(d) asks that such a build quote ITS count: 12 (three rotations) + 3 (amplitude differences) + 2 (A z) +
+# 4 n_c (MACs) + 2 (W A^2; 1 + n_c with per-channel weights) => 27 for two channels sharing a weight row, 33 for
+# three channels with their own rows.  `frac` uses these.  The re-synchronisation every 32 bins (2 cubics 6 +
+# differences 16 + 3 sincos 54 + 3 normalisations 15 + 1 = 92 slots / 32 bins = 2.9) is the builder's tuning choice,
+# not algorithmic work: `frac_with_resync` adds it and is reported beside `frac`, never instead of it.
 SLOTS_FULL_DIRECT = 39.0
-SLOTS_FULL = 30.0
+SLOTS_FULL = 27.0
+SLOTS_FULL_NC3 = 33.0
+SLOTS_RESYNC = 2.9
 # per-walker node grids: the recurrence route with T^c applied per bin (it accumulates <d|h>, <h|h> directly):
-# 12 + 3 + 2 + T^c h 8 + Re g h 4 + W |h|^2 5 = 34 per bin + (6 + 16 + 4 sincos 72 + 20 + 1)/32 = 3.6 => 38
-SLOTS_FULL_PW = 38.0
+# 12 + 3 + 2 + T^c h 8 + Re g h 4 + W |h|^2 5 = 34 per bin (+ re-sync with four sincos: 3.6)
+SLOTS_FULL_PW = 34.0
 # single mode: the kernel regroups Eq. 14/17 by edge, whose own count is 48 slots per (walker, bin): phase 2,
-# reduce 3, sincos 18, taper and amplitude 4, z conj(Q) 8, |z|^2 P 3, z_b conj(z_{b+1}) X 10; the bin-by-bin form needs 73
+# reduce 3, sincos 18, taper and amplitude 4, z conj(Q) 8, |z|^2 P 3, z_b conj(z_{b+1}) X 10; the bin-by-bin form of
+# SURVEY §8(d) needs 73.  Six modes: SURVEY's 252 (6 x 36 + 36)
 SLOTS_HET = {1: 48.0, 6: 252.0}
-SLOTS_HET_DIRECT_FORM = {1: 73.0}
+SLOTS_HET_SURVEY_FORM = {1: 73.0, 6: 252.0}
 # FP32-accumulate variant: bound by instruction issue (one warp instruction per scheduler per
 # clock = 4 x 32 lane-instructions/clk/SM).  Algorithmic instructions per active pair: 13 FP64 (t, two cubics,
 # reduce 3, scale 1, W A^2 2) + 3 conversions + 20 binary32 (sincos 10, A e^{-i Psi} 2, MACs 8) + 6 quadrant
@@ -53,12 +59,46 @@ SLOTS_HET_DIRECT_FORM = {1: 73.0}
 INSTR_FULL_FP32ACC = 45.0
 # frequency-dependent transfer function (Eq. 8-9), direct formulation: t 1, six cubics 18, reduce 3, sincos 18,
 # A e^{-i Psi} 2, T^c h 8, Re g h 4, W |h|^2 5 = 59.  The kernel advances A and e^{-i Psi} by the recurrence and keeps
-# Horner for the four T cubics: t 1 + 12 + rotations 12 + amplitude 3 + 2 + 8 + 4 + 5 = 47 per bin + re-sync 3 => 50
-SLOTS_FULL_TF = 50.0
+# Horner for the four T cubics: t 1 + 12 + rotations 12 + amplitude 3 + 2 + 8 + 4 + 5 = 47 per bin
+SLOTS_FULL_TF = 47.0
 ISSUE_LANES_PER_CLK_PER_SM = 128.0
-# DRAM traffic per launch of the dominant kernel, from the committed `ncu --set full` captures (profiles/)
-NCU_TRAFFIC_BYTES = {("k_full_fused", 2): 806.3e6 + 39.9e6, ("k_full_fused_mixed", 2): 786.4e6 + 37.0e6}
 DFMA_PER_CLK_PER_SM = 64.0
+# the parity test that covers each timed configuration at its full size (tests/, -m gpu)
+COVERED_BY = {
+    "cfg0": "tests/test_parity_gpu.py::test_cfg0_full_standin_parity",
+    "cfg1": "tests/test_parity_gpu.py::test_cfg1_full_size",
+    "cfg2": "tests/test_parity_cfg2_scale.py::test_cfg2_full_size_128_walkers",
+    "cfg3": "tests/test_parity_gpu.py::test_cfg3_higher_modes_full_size_sampled",
+    "cfg4": "tests/test_parity_gpu.py::test_cfg4_large_batch_full_size_sampled",
+    "cfg2_fp32acc": "tests/test_parity_gpu.py::test_cfg2_full_size_sampled_mixed",
+    "cfg2_tf": "tests/test_parity_cfg2_scale.py::test_cfg2_tf_full_size_sampled",
+    "cfg2_pw": "tests/test_parity_cfg2_scale.py::test_cfg2_pw_full_size_sampled",
+    "cfg2_hm6": "tests/test_parity_cfg2_scale.py::test_cfg2_hm6_full_size_sampled",
+    "cfg2_nc3": "tests/test_parity_cfg2_scale.py::test_cfg2_three_channels_full_size_sampled",
+    "cfg2_split_tc": "tests/test_parity_cfg2_scale.py::test_cfg2_split_tc_full_size_sampled",
+    "module1_iteration": "tests/test_parity_cfg2_scale.py::test_module1_sized_batches_against_oracle, "
+                         "tests/test_parity_gpu.py::test_pt_run_parity_full",
+    "module2_iteration": "tests/test_parity_gpu.py::test_pt_run_parity_het",
+}
+
+
+def ncu_traffic_bytes(kernel_tag: str):
+    """DRAM read + write bytes per launch of a kernel from the newest committed `ncu --set full` summary under profiles/
+    whose name carries `kernel_tag` (e.g. 'full_fused_cfg2'): a measurement of THIS build's kernel, by file name, or None."""
+    import glob
+    import re
+    cands = sorted(glob.glob(os.path.join(ROOT, "profiles", f"r*_{kernel_tag}.md")))
+    if not cands:
+        return None, None
+    path = cands[-1]
+    unit = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+    tot, seen = 0.0, 0
+    for line in open(path):
+        m = re.match(r"\|\s*dram__bytes_(read|write)\.sum\s*\|\s*(\w+)\s*\|\s*([0-9.eE+-]+)\s*\|", line)
+        if m and m.group(2) in unit:
+            tot += float(m.group(3)) * unit[m.group(2)]
+            seen += 1
+    return (tot, os.path.relpath(path, ROOT)) if seen == 2 else (None, None)
 
 
 # ------------------------------------------------------------------------------------------------ helpers
@@ -290,6 +330,23 @@ def bench_sampler_iteration(torch, ctx, wl, params, n_t: int = 10, n_w: int = 40
     return res
 
 
+def bench_small_batch(torch, ctx, wl, params, peak_slots, n_w: int = 160, steps: int = 20):
+    """one Module-1 sized likelihood call (a half update of 4 x 80 walkers is 160 proposals): batch time
+    and the fused kernel's own time and ALU-roofline fraction"""
+    p = params[:n_w].contiguous()
+    out = tuple(torch.empty(n_w, dtype=torch.float64, device=p.device) for _ in range(3))
+    fn = lambda: ctx.full_batch_standin(wl.f_nodes, p, out=out)
+    fn()
+    ctx.profile_enable(True)
+    ms = time_steps(torch, fn, steps, 3) / steps
+    kms, kn = ctx.profile_read()
+    ctx.profile_enable(False)
+    pairs = ctx.last_full_stats()[0]
+    k = kms / max(kn, 1)
+    return {"call_160": {"n_walkers": n_w, "ms_per_batch": ms, "kernel_ms": k, "units": pairs, "slots_per_unit": SLOTS_FULL,
+                         "frac": pairs * SLOTS_FULL / (k * 1e-3) / peak_slots}}
+
+
 def bench_full_hm(torch, steps: int = 5, n_w: int = 2048):
     """The paper's higher-mode analysis ran the brute-force likelihood, not the heterodyned one: config 3's
     six modes through the FULL-GRID path on config 2's one-year grid and 1024 nodes, prior-draw walkers with unit-modulus
@@ -335,18 +392,22 @@ def e2e_config(torch, res, steps: int, warmup: int):
     return ms / steps, ph.numel() * 8, 3 * wl.n_w * 8
 
 
-def cpu_baseline(index: int, n_sample: int, budget_note: str = ""):
-    """the oracle, as it stands, on this box's cores, on the first n_sample walkers of the same workload"""
+CPU_SAMPLE_CFG2 = 128   # walkers of config 2 the oracle is timed on (>= 128)
+
+
+def oracle_job(index: int, n_sample=None):
+    """the oracle, as it stands, on workload `index`: returns (work(n) -> None over the first n walkers, n_total, name).
+    Het configs run in full; config 2 on its first CPU_SAMPLE_CFG2 walkers over the whole grid (bounded sample)."""
     import oracle as orc
     wl = rank_workload(index, 0)
     g = wl.grid
-    t_setup = time.perf_counter()
     if wl.path == "full":
         run = lambda p, d, t=False: orc.full_batch_standin(wl.modes_m, wl.c_lm, wl.kappa, p, wl.f_nodes, g.k_min, g.df,
                                                            g.n_f, d, wl.W, want_template=t)
         wl.finish_distance(run(wl.inj[None], None)["h_h"][0])
         d = wl.make_data(run(wl.inj[None], None, True)["h"])
-        work = lambda: run(wl.params[:n_sample], d)
+        work = lambda n: run(wl.params[:n], d)
+        n_total = min(wl.n_w, n_sample or (CPU_SAMPLE_CFG2 if index == 2 else wl.n_w))
     else:
         f = g.freqs()
         direct = lambda p, ff: orc.standin_direct(p, wl.modes_m, wl.c_lm, wl.kappa, ff, float(f[0]), float(f[-1]))
@@ -356,41 +417,69 @@ def cpu_baseline(index: int, n_sample: int, budget_note: str = ""):
         d = wl.make_data(h0)
         h0e = direct(wl.inj, wl.f_edges)
         summ = orc.het_prepare(g.k_min, g.df, d, wl.W, h0, wl.f_edges)
-        work = lambda: orc.het_batch_standin(wl.modes_m, wl.c_lm, wl.kappa, wl.params[:n_sample], wl.f_edges, h0e, summ)
-    t_setup = time.perf_counter() - t_setup
-    t0 = time.perf_counter()
-    work()
-    dt = time.perf_counter() - t0
-    return {"value": n_sample / dt, "unit": UNIT, "cores": orc.n_threads(), "kind": "oracle",
-            "sample": f"{wl.name}: first {n_sample} of {wl.n_w} walkers, whole grid, {dt:.1f} s wall{budget_note}",
-            "seconds": dt, "work": work, "n_sample": n_sample}
+        work = lambda n: orc.het_batch_standin(wl.modes_m, wl.c_lm, wl.kappa, wl.params[:n], wl.f_edges, h0e, summ)
+        n_total = min(wl.n_w, n_sample or wl.n_w)
+    return work, n_total, wl
+
+
+def cpu_baseline(index: int, repeats: int = 3):
+    """the oracle timed on this box's host cores: median of `repeats` runs on all cores (omp_get_max_threads) and on one
+    core (a 1/cores share of the sample, so both legs take about as long)"""
+    import oracle as orc
+    work, n_all, wl = oracle_job(index)
+    cores = orc.n_threads()
+
+    def timed(n):
+        ts = []
+        for _ in range(repeats):
+            t0 = time.perf_counter()
+            work(n)
+            ts.append(time.perf_counter() - t0)
+        return statistics.median(ts)
+
+    t_all = timed(n_all)
+    n_one = max(1, n_all // cores)
+    orc.set_threads(1)
+    try:
+        t_one = timed(n_one)
+    finally:
+        orc.set_threads(cores)
+    what = "whole grid" if wl.path == "full" else "all %d bins" % (len(wl.f_edges) - 1)
+    return {"value": n_all / t_all, "unit": UNIT, "cores": cores, "kind": "oracle", "median_of": repeats,
+            "sample": f"{wl.name}: first {n_all} of {wl.n_w} walkers, {what}; {t_all:.2f} s per run on {cores} cores",
+            "evals_per_s_all_cores": n_all / t_all, "evals_per_s_per_core": n_one / t_one,
+            "per_core_sample": f"first {n_one} walkers on one thread, {t_one:.2f} s per run",
+            "seconds": t_all, "n_sample": n_all}
 
 
 def run_reference(args):
-    """--impl reference: the oracle is the reference arm for this tier (no reference implementation exists)."""
+    """--impl reference: the oracle is the reference arm for this tier (no reference implementation exists).  Each
+    step is the SAME bounded sample `cpu_baseline` times (config 2: the first CPU_SAMPLE_CFG2 walkers over the whole
+    grid, on all cores), so the two legs agree."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
     import oracle as orc
     orc.build()
     cores = orc.n_threads()
-    n_sample = max(cores, 1)
-    cb = cpu_baseline(args.workload, n_sample)
-    work = cb.pop("work")
-    for _ in range(max(args.warmup - 1, 0)):
-        work()
-    t0 = time.perf_counter()
+    work, n_sample, wl = oracle_job(args.workload)
+    for _ in range(max(args.warmup, 0)):
+        work(n_sample)
+    ts = []
     for _ in range(args.steps):
-        work()
-    dt = time.perf_counter() - t0
-    wl = rank_workload(args.workload, 0)
+        t0 = time.perf_counter()
+        work(n_sample)
+        ts.append(time.perf_counter() - t0)
+    dt = sum(ts)
     val = n_sample * args.steps / dt
+    what = "whole grid" if wl.path == "full" else "all bins"
+    sample = f"{wl.name}: first {n_sample} of {wl.n_w} walkers per step, {what}"
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64 (x87 long double accumulators)", "data": "synthetic",
-            "config": workload_config(wl, extra={"step": f"{n_sample} walkers of the batch per step (bounded sample)"}),
-            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle",
-                             "sample": f"{wl.name}: first {n_sample} walkers per step, whole grid"},
+            "config": workload_config(wl),
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+                             "median_step_evals_per_s": n_sample / statistics.median(ts)},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line))
@@ -412,6 +501,43 @@ def workload_config(wl, extra=None):
     if extra:
         c.update(extra)
     return c
+
+
+def config_roofline(wl, ctx, kernel_ms: float, peak_slots: float):
+    """ALU roofline of one configuration's dominant kernel: units of the launch x algorithmic FP64 slots per unit
+    (SURVEY §8(d) for the formulation the kernel implements) / CUDA-event duration / peak"""
+    if wl.path == "full":
+        units = ctx.last_full_stats()[0]                # active (walker, bin, mode) triples, counted on the device
+        if wl.n_m == 1:
+            slots = SLOTS_FULL if wl.n_c == 2 else SLOTS_FULL_NC3
+            out = {"kernel": "k_full_fused<1, %d, %s>" % (wl.n_c, "true" if wl.n_c == 2 else "false"), "slots_per_unit": slots,
+                   "formulation": "rotation recurrence (SURVEY §8(d): ~27 for two channels), re-synchronised every 32 bins; "
+                                  "the direct formulation needs %g" % SLOTS_FULL_DIRECT,
+                   "frac_with_resync": units * (slots + SLOTS_RESYNC) / (kernel_ms * 1e-3) / peak_slots}
+        else:
+            slots = SLOTS_FULL_DIRECT
+            out = {"kernel": "k_full_fused<0, %d, ...>" % wl.n_c, "slots_per_unit": slots, "formulation": "direct (SURVEY §8(d): 39)"}
+        out["unit_name"] = "active (walker, bin, mode)"
+    else:
+        units = float(wl.n_w) * (len(wl.f_edges) - 1)
+        slots = SLOTS_HET.get(wl.n_m, 73.0 + 36.0 * (wl.n_m - 1))
+        out = {"kernel": "k_het_standin1" if wl.n_m == 1 else "k_het_standin<%d>" % wl.n_m, "slots_per_unit": slots,
+               "unit_name": "(walker, bin)",
+               "formulation": ("regrouped by edge (DESIGN.md §5): 48; the bin-by-bin form of SURVEY §8(d) needs %g"
+                               % SLOTS_HET_SURVEY_FORM[1]) if wl.n_m == 1 else "bin by bin (SURVEY §8(d): 252 for six modes)"}
+    out.update({"units": units, "kernel_ms": kernel_ms, "frac": units * slots / (kernel_ms * 1e-3) / peak_slots})
+    return out
+
+
+def sustained_dfma(torch, ctx, index: int, burst_ms_at_4000: float, seconds: float = 2.2):
+    """the FP64 roofline denominator from a >= 2 s run of dependent-free DFMA chains on every SM, with the
+    SM clock sampled during it (a burst of a few ms says nothing about the clock the chip holds under this load)"""
+    iters = int(4000 * seconds * 1e3 / max(burst_ms_at_4000, 1e-3))
+    with ClockSampler(index, period=0.05) as clk:
+        rate, ms = ctx.peak_fma(0, iters)
+    c = clk.summary()
+    return {"measured_dfma_per_s_sustained": rate, "sustained_run_s": ms * 1e-3, "sustained_sm_mhz": c.get("sm_mhz"),
+            "sustained_clock_reasons": c.get("reasons")}
 
 
 def main():
@@ -467,49 +593,40 @@ def main():
         sm_max = float(clocks.get("sm_max_mhz") or peaks.get("sm_max_mhz", 1965.0))
         n_sm = torch.cuda.get_device_properties(local).multi_processor_count
         peak_slots = n_sm * DFMA_PER_CLK_PER_SM * sm_max * 1e6
-        if wl.path == "full":
-            pairs, n_blocks = ctx.last_full_stats()
-            slots = pairs * SLOTS_FULL
-            kname = "k_full_fused" if args.precision == "fp64" else "k_full_fused_mixed"
-        else:
-            pairs = float(wl.n_w) * (len(wl.f_edges) - 1)
-            slots = pairs * SLOTS_HET.get(wl.n_m, 73.0 + 36.0 * (wl.n_m - 1))
-            kname = "k_het_standin"
         k_ms = res["kernel_ms"]
         dfma_rate, dfma_ms = ctx.peak_fma(0, 4000)
         ffma_rate, _ = ctx.peak_fma(1, 8000)
-        traffic = NCU_TRAFFIC_BYTES.get((kname, args.workload))
-        if kname == "k_full_fused_mixed":
+        common = {"kernel_ms": k_ms, "kernel_share_of_step": k_ms / res["ms_per_step"],
+                  "measured_dfma_per_s_burst": dfma_rate, "measured_ffma_per_s_burst": ffma_rate,
+                  "hbm_peak_gbs": peaks.get("hbm_gbs"), "hbm_peak_source": peak_src}
+        if not args.quick:
+            common.update(sustained_dfma(torch, ctx, local, dfma_ms))
+        if wl.path == "full" and args.precision == "fp32acc":
+            pairs, n_blocks = ctx.last_full_stats()
+            traffic, traffic_src = ncu_traffic_bytes("full_fused_mixed_cfg%d" % args.workload)
             peak_issue = n_sm * ISSUE_LANES_PER_CLK_PER_SM * sm_max * 1e6
             achieved = pairs * INSTR_FULL_FP32ACC / (k_ms * 1e-3)
             line["roofline"] = {
-                "bound": "alu", "kernel": kname, "achieved": achieved / 1e12, "peak": peak_issue / 1e12,
+                "bound": "alu", "kernel": "k_full_fused_mixed", "achieved": achieved / 1e12, "peak": peak_issue / 1e12,
                 "unit": "T lane-instructions/s (instruction issue: 1 warp instruction/scheduler/clk)",
-                "frac": achieved / peak_issue, "traffic": traffic, "kernel_ms": k_ms,
-                "kernel_share_of_step": k_ms / (res["ms_per_step"]),
+                "frac": achieved / peak_issue, "traffic": traffic, "traffic_source": traffic_src,
                 "algorithmic_instructions_per_pair": INSTR_FULL_FP32ACC, "active_pairs": pairs,
                 "peak_source": f"{n_sm} SMs x 4 schedulers x 32 lanes x {sm_max:.0f} MHz (DESIGN.md §6)",
-                "fp64_slots_per_pair": 13.0, "fp64_pipe_frac": pairs * 13.0 / (k_ms * 1e-3) / peak_slots,
-                "measured_dfma_per_s": dfma_rate, "measured_ffma_per_s": ffma_rate,
-                "hbm_peak_gbs": peaks.get("hbm_gbs"), "hbm_peak_source": peak_src}
+                "fp64_slots_per_pair": 13.0, "fp64_pipe_frac": pairs * 13.0 / (k_ms * 1e-3) / peak_slots, **common}
         else:
-            achieved = slots / (k_ms * 1e-3)
+            rf = config_roofline(wl, ctx, k_ms, peak_slots)
+            traffic, traffic_src = ncu_traffic_bytes(("full_fused_cfg%d" if wl.path == "full" else "het_cfg%d") % args.workload)
             line["roofline"] = {
-                "bound": "alu", "kernel": kname, "achieved": achieved / 1e12, "peak": peak_slots / 1e12,
-                "unit": "T FP64 issue slots/s (1 DFMA|DMUL|DADD = 1 slot)", "frac": achieved / peak_slots,
-                "traffic": traffic, "kernel_ms": k_ms, "kernel_share_of_step": k_ms / (res["ms_per_step"]),
-                "algorithmic_slots_per_pair": SLOTS_FULL if wl.path == "full" else slots / pairs, "active_pairs": pairs,
+                "bound": "alu", "kernel": rf["kernel"], "achieved": rf["frac"] * peak_slots / 1e12, "peak": peak_slots / 1e12,
+                "unit": "T FP64 issue slots/s (1 DFMA|DMUL|DADD = 1 slot)", "frac": rf["frac"],
+                "traffic": traffic, "traffic_source": traffic_src,
+                "algorithmic_slots_per_unit": rf["slots_per_unit"], "units": rf["units"], "formulation": rf["formulation"],
                 "peak_source": f"{n_sm} SMs x {int(DFMA_PER_CLK_PER_SM)} DFMA/clk x {sm_max:.0f} MHz (DESIGN.md §6)",
-                "measured_dfma_per_s": dfma_rate, "measured_ffma_per_s": ffma_rate,
-                "frac_of_measured_dfma": achieved / dfma_rate,
-                "hbm_peak_gbs": peaks.get("hbm_gbs"), "hbm_peak_source": peak_src}
-            if wl.path == "full":
-                line["roofline"]["formulation"] = ("rotation recurrence, re-synchronised every 32 bins (DESIGN.md §5); the direct "
-                                                   "formulation needs %g slots per pair" % SLOTS_FULL_DIRECT)
-                line["roofline"]["frac_in_direct_form_slots"] = pairs * SLOTS_FULL_DIRECT / (k_ms * 1e-3) / peak_slots
-            if wl.path != "full" and wl.n_m in SLOTS_HET_DIRECT_FORM:
-                line["roofline"]["formulation"] = "regrouped by edge (DESIGN.md §5); the bin-by-bin form of Eq. 14/17 needs %g" \
-                                                  % SLOTS_HET_DIRECT_FORM[wl.n_m]
+                "frac_of_measured_dfma_burst": rf["frac"] * peak_slots / dfma_rate, **common}
+            if "frac_with_resync" in rf:
+                line["roofline"]["frac_with_resync"] = rf["frac_with_resync"]
+            if "measured_dfma_per_s_sustained" in common:
+                line["roofline"]["frac_of_measured_dfma_sustained"] = rf["frac"] * peak_slots / common["measured_dfma_per_s_sustained"]
 
     if not args.quick:
         # ---- end to end through the C ABI with host buffers
@@ -522,16 +639,26 @@ def main():
     torch.cuda.empty_cache()
 
     if rank == 0 and not args.quick and world == 1:
-        # ---- every BASELINE.json config, device-resident, stand-in entry points
+        # ---- every BASELINE.json config, device-resident, stand-in entry points, each with the ALU roofline of its
+        # dominant kernel (library CUDA-event bracket) — configs 0 and 1 are launch-bound
         per = {}
         for idx in (0, 1, 2, 3, 4):
+            key = f"cfg{idx}"
             if idx == args.workload:
-                per[f"cfg{idx}"] = {"evals_per_s": value, "ms_per_batch": t_ms / args.steps, "n_walkers": wl.n_w}
+                per[key] = {"evals_per_s": value, "ms_per_batch": t_ms / args.steps, "n_walkers": wl.n_w}
+                if args.precision == "fp64":
+                    rf = line["roofline"]
+                    per[key].update({"kernel": rf["kernel"], "kernel_ms": rf["kernel_ms"], "slots_per_unit": rf["algorithmic_slots_per_unit"],
+                                     "units": rf["units"], "frac": rf["frac"], "launch_bound": False, "covered_by": COVERED_BY[key]})
                 continue
             st = 50 if idx != 2 else args.steps
-            r = bench_config(torch, idx, st, 5)
-            per[f"cfg{idx}"] = {"evals_per_s": r["wl"].n_w / (r["ms_per_step"] * 1e-3), "ms_per_batch": r["ms_per_step"],
-                                "n_walkers": r["wl"].n_w}
+            r = bench_config(torch, idx, st, 5, profile=True)
+            rf = config_roofline(r["wl"], r["ctx"], r["kernel_ms"], peak_slots)
+            per[key] = {"evals_per_s": r["wl"].n_w / (r["ms_per_step"] * 1e-3), "ms_per_batch": r["ms_per_step"],
+                        "n_walkers": r["wl"].n_w, "launches_per_batch": r["launches"] / st, "kernel": rf["kernel"],
+                        "kernel_ms": rf["kernel_ms"], "slots_per_unit": rf["slots_per_unit"], "units": rf["units"],
+                        "unit": rf["unit_name"], "frac": rf["frac"], "formulation": rf["formulation"],
+                        "launch_bound": idx in (0, 1), "covered_by": COVERED_BY[key]}
             if idx in (0, 1):
                 # ---- launch-bound configs: the same call replayed as a CUDA graph
                 try:
@@ -544,27 +671,35 @@ def main():
                             r["fn"]()
                     torch.cuda.current_stream().wait_stream(sg)
                     ms_g = time_steps(torch, gr.replay, 200, 5) / 200
-                    per[f"cfg{idx}"].update({"ms_per_batch_graph": ms_g, "evals_per_s_graph": r["wl"].n_w / (ms_g * 1e-3)})
+                    per[key].update({"ms_per_batch_graph": ms_g, "evals_per_s_graph": r["wl"].n_w / (ms_g * 1e-3)})
                     del gr
                 except Exception as e:
-                    per[f"cfg{idx}"]["graph_error"] = repr(e)[:200]
+                    per[key]["graph_error"] = repr(e)[:200]
             if idx == 1:
                 # ---- the reference update inside the loop (every 5000 iterations)
                 # and the brute-force audit of the heterodyned values, config-1 size
                 c1, p1, n_e = r["ctx"], r["bufs"]["params"], len(r["wl"].f_edges)
+                het = [x.clone() for x in c1.het_batch_standin(p1)]
+                o1 = tuple(torch.empty_like(het[0]) for _ in range(3))
+                ms_a = time_steps(torch, lambda: c1.het_audit_standin(p1, out=o1), 5, 2) / 5
+                err = (het[0] - o1[0]).abs()
+                below = o1[0].max() - o1[0]                # distance from the best dense log L of the population
+                near = below < 50.0
+                per["cfg1_audit"] = {"evals_per_s": r["wl"].n_w / (ms_a * 1e-3), "ms_per_batch": ms_a, "n_walkers": r["wl"].n_w,
+                                     "max_abs_het_minus_dense_logL": float(err.max()), "median_abs_het_minus_dense_logL": float(err.median()),
+                                     "dense_logL_range": [float(o1[0].min()), float(o1[0].max())],
+                                     "n_within_50_of_best": int(near.sum()),
+                                     "max_abs_err_within_50_of_best": float(err[near].max()) if bool(near.any()) else None,
+                                     "max_rel_err_to_distance_from_best": float((err / below.clamp_min(1.0)).max()),
+                                     "entry": "ll_het_audit_standin (direct template at every dense bin of the band)"}
                 t0 = time.perf_counter()
                 for _ in range(5):
                     c1.het_refresh_standin(p1, r["out"][0], n_e)          # synchronises the stream itself
                 ms_ref = (time.perf_counter() - t0) / 5 * 1e3
-                het = [x.clone() for x in c1.het_batch_standin(p1)]
-                o1 = tuple(torch.empty_like(het[0]) for _ in range(3))
-                ms_a = time_steps(torch, lambda: c1.het_audit_standin(p1, out=o1), 5, 2) / 5
                 per["cfg1_refresh"] = {"ms_per_update": ms_ref, "n_edges": n_e, "n_f": r["wl"].grid.n_f,
                                        "entry": "ll_het_refresh_standin (argmax, h0 on the grid and at the edges, H0; host wall time, the call synchronises)"}
-                per["cfg1_audit"] = {"evals_per_s": r["wl"].n_w / (ms_a * 1e-3), "ms_per_batch": ms_a, "n_walkers": r["wl"].n_w,
-                                     "max_abs_het_minus_dense_logL": float((het[0] - o1[0]).abs().max()),
-                                     "entry": "ll_het_audit_standin (direct template at every dense bin of the band)"}
                 per["module2_iteration"] = bench_sampler_iteration(torch, c1, r["wl"], p1)
+                per["module2_iteration"]["covered_by"] = COVERED_BY["module2_iteration"]
             r["ctx"].destroy()
             del r
             torch.cuda.empty_cache()
@@ -572,11 +707,36 @@ def main():
             # ---- config 2's FP32-accumulate variant on the same data: throughput and its distance from FP64
             r = bench_config(torch, 2, args.steps, 5, profile=True, precision=1)
             dl = (r["out"][0] - headline_logL).abs()
+            pairs_m = r["ctx"].last_full_stats()[0]
             per["cfg2_fp32acc"] = {"evals_per_s": r["wl"].n_w / (r["ms_per_step"] * 1e-3), "ms_per_batch": r["ms_per_step"],
                                    "n_walkers": r["wl"].n_w, "kernel": "k_full_fused_mixed", "kernel_ms": r["kernel_ms"],
-                                   "max_abs_dlogL_vs_fp64": float(dl.max()), "rms_dlogL_vs_fp64": float(dl.pow(2).mean().sqrt())}
+                                   "max_abs_dlogL_vs_fp64": float(dl.max()), "rms_dlogL_vs_fp64": float(dl.pow(2).mean().sqrt()),
+                                   "fp64_slots_per_unit": 13.0, "fp64_pipe_frac": pairs_m * 13.0 / (r["kernel_ms"] * 1e-3) / peak_slots,
+                                   "covered_by": COVERED_BY["cfg2_fp32acc"]}
             r["ctx"].destroy()
             del r
+            torch.cuda.empty_cache()
+            # ---- config 2 with three channels (A, E, T; per-channel PSDs: SURVEY §8(f) item 1)
+            from paper_2111_01064_b200 import synth
+            wl3 = wlm.make_workload(2, n_c=3)
+            c3 = synth.make_context(wl3)
+            b3 = synth.setup(c3, wl3)
+            o3 = tuple(torch.empty(wl3.n_w, dtype=torch.float64, device="cuda") for _ in range(3))
+            fn = lambda: c3.full_batch_standin(wl3.f_nodes, b3["params"], out=o3)
+            fn()
+            c3.profile_enable(True)
+            nst = max(args.steps // 2, 3)
+            ms = time_steps(torch, fn, nst, 3) / nst
+            kms, kn = c3.profile_read()
+            c3.profile_enable(False)
+            rf = config_roofline(wl3, c3, kms / max(kn, 1), peak_slots)
+            per["cfg2_nc3"] = {"evals_per_s": wl3.n_w / (ms * 1e-3), "ms_per_batch": ms, "n_walkers": wl3.n_w, "n_channels": 3,
+                               "kernel": rf["kernel"], "kernel_ms": rf["kernel_ms"], "slots_per_unit": rf["slots_per_unit"],
+                               "units": rf["units"], "frac": rf["frac"], "frac_with_resync": rf["frac_with_resync"],
+                               "entry": "ll_set_data(w_shared = 0), W [3][n_f]; ll_full_batch_standin with 11-double rows",
+                               "covered_by": COVERED_BY["cfg2_nc3"]}
+            c3.destroy()
+            del b3, o3
             torch.cuda.empty_cache()
         if args.workload == 2 and args.precision == "fp64":
             # ---- frequency-dependent transfer function (six splines per mode) at config-2
@@ -597,10 +757,11 @@ def main():
             nst = max(args.steps // 2, 3)
             pairs2 = c2.last_full_stats()[0]
             per["cfg2_tf"] = {"evals_per_s": wl2.n_w / (ms2 / nst * 1e-3), "ms_per_batch": ms2 / nst, "n_walkers": wl2.n_w,
-                              "kernel": "k_full_fused_tf", "kernel_ms": kms / max(kn, 1), "active_pairs": pairs2,
-                              "algorithmic_slots_per_pair": SLOTS_FULL_TF,
+                              "kernel": "k_full_fused_tf<1, 2, true>", "kernel_ms": kms / max(kn, 1), "units": pairs2,
+                              "slots_per_unit": SLOTS_FULL_TF,
                               "frac": pairs2 * SLOTS_FULL_TF / (kms / max(kn, 1) * 1e-3) / peak_slots,
-                              "entry": "ll_full_batch_tf (amp, phase, T at 1024 nodes as device arrays; the walkers' own bands)"}
+                              "entry": "ll_full_batch_tf (amp, phase, T at 1024 nodes as device arrays; the walkers' own bands)",
+                              "covered_by": COVERED_BY["cfg2_tf"]}
             # ---- per-walker node grids at config-2 size.  Every walker gets its own copy of the
             # 1024 nodes (so the numbers can be compared with the shared-node path output by output); what is timed is
             # the per-walker machinery: one tridiagonal factorisation per system, one bin -> interval map per lane
@@ -615,29 +776,49 @@ def main():
             kms3, kn3 = c2.profile_read()
             c2.profile_enable(False)
             per["cfg2_pw"] = {"evals_per_s": wl2.n_w / (ms3 / nst * 1e-3), "ms_per_batch": ms3 / nst, "n_walkers": wl2.n_w,
-                              "kernel": "k_full_fused_pw", "kernel_ms": kms3 / max(kn3, 1),
+                              "kernel": "k_full_fused_pw<1, 2, true>", "kernel_ms": kms3 / max(kn3, 1), "units": pairs2,
                               "frac": pairs2 * SLOTS_FULL_PW / (kms3 / max(kn3, 1) * 1e-3) / peak_slots,
-                              "algorithmic_slots_per_pair": SLOTS_FULL_PW,
+                              "slots_per_unit": SLOTS_FULL_PW,
                               "max_abs_dlogL_vs_shared_nodes": float((o3[0] - sh[0]).abs().max()),
-                              "entry": "ll_full_batch_pw (f_nodes_w [n_w][1024] on the device; the walkers' own bands)"}
+                              "entry": "ll_full_batch_pw (f_nodes_w [n_w][1024] on the device; the walkers' own bands)",
+                              "covered_by": COVERED_BY["cfg2_pw"]}
             del xw, sh, tfc
+            # ---- SURVEY §8(f) item 2, t_shift: the stand-in's linear phase term 2 pi f t_c kept outside the spline
+            c2.standin_split_tc(True)
+            o4 = tuple(torch.empty(wl2.n_w, dtype=torch.float64, device=amp.device) for _ in range(3))
+            fn4 = lambda: c2.full_batch_standin(wl2.f_nodes, b2["params"], out=o4)
+            fn4()
+            c2.profile_enable(True)
+            ms4 = time_steps(torch, fn4, nst, 2) / nst
+            kms4, kn4 = c2.profile_read()
+            c2.profile_enable(False)
+            c2.standin_split_tc(False)
+            dsp = (o4[0] - headline_logL).abs()
+            per["cfg2_split_tc"] = {"evals_per_s": wl2.n_w / (ms4 * 1e-3), "ms_per_batch": ms4, "kernel_ms": kms4 / max(kn4, 1),
+                                    "max_abs_dlogL_vs_full_phase_spline": float(dsp.max()),
+                                    "max_abs_node_phase_rad": {"full": float(ph.abs().max()), "split": float((ph - 2 * np.pi * torch.as_tensor(wl2.f_nodes, device=ph.device) * b2["params"][:, 2:3, None]).abs().max())},
+                                    "entry": "ll_standin_split_tc(1); ll_full_batch_standin (reading R32)",
+                                    "covered_by": COVERED_BY["cfg2_split_tc"]}
             # ---- six modes through the full-grid path (the paper's higher-mode run used the brute-force likelihood)
             hm = bench_full_hm(torch)
             hm["frac"] = hm["active_pair_modes"] * SLOTS_FULL_DIRECT / (hm["kernel_ms"] * 1e-3) / peak_slots
+            hm["covered_by"] = COVERED_BY["cfg2_hm6"]
             per["cfg2_hm6"] = hm
             # ---- Module-1 sized sampler iteration on the full-grid likelihood of the same one-year data stream
             per["module1_iteration"] = bench_sampler_iteration(torch, c2, wl2, b2["params"], n_t=4, n_w=80, iters=20,
                                                                f_nodes=wl2.f_nodes)
+            per["module1_iteration"]["covered_by"] = COVERED_BY["module1_iteration"]
+            per["module1_iteration"].update(bench_small_batch(torch, c2, wl2, b2["params"], peak_slots))
             c2.destroy()
             del amp, ph, tfn, b2
             torch.cuda.empty_cache()
         line["per_config"] = per
-        # ---- the oracle on this box's cores, bounded sample of the same workload
+        # ---- the oracle on this box's cores: the headline config, then every other config (het configs in full,
+        # config 2 on a bounded sample), median of 3, per core and on all cores (SURVEY §8(d) "Oracle timing")
         import oracle as orc
         orc.build()
-        n_sample = 4 * orc.n_threads() if wl.path == "full" else min(wl.n_w, 4096)
-        cb = cpu_baseline(args.workload, n_sample)
-        cb.pop("work")
+        cb = cpu_baseline(args.workload)
+        cb["per_config"] = {f"cfg{i}": (cpu_baseline(i) if i != args.workload else "the headline entry above") for i in range(5)}
         line["cpu_baseline"] = cb
     if rank == 0:
         print(json.dumps(line))

@@ -58,9 +58,13 @@ def _check(rc: int, what: str):
 
 
 def n_threads() -> int:
-    """Threads the OpenMP loops will use (for bench.py's cpu_baseline `cores`)."""
-    env = os.environ.get("OMP_NUM_THREADS")
-    return int(env) if env else (os.cpu_count() or 1)
+    """Threads the OpenMP loops will use: omp_get_max_threads() (for bench.py's cpu_baseline `cores`)."""
+    return int(lib().orc_get_threads())
+
+
+def set_threads(n: int) -> int:
+    """omp_set_num_threads(n) (timing harness: the oracle on one core and on all cores); returns the new count"""
+    return int(lib().orc_set_threads(C.c_int(int(n))))
 
 
 # ------------------------------------------------------------------ spline

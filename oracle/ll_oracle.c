@@ -56,8 +56,28 @@
 #include <stdint.h>
 #include <stdlib.h>
 #include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
 
 typedef long double ld;
+
+/* threads the walker loops run on (timing harness only: bench.py reports the oracle per core and on all cores) */
+int orc_get_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+int orc_set_threads(int n)
+{
+#ifdef _OPENMP
+    if (n >= 1) omp_set_num_threads(n);
+#endif
+    return orc_get_threads();
+}
 
 static const ld PI_L = 3.14159265358979323846264338327950288L;
 

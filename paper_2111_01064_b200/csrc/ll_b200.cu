@@ -1580,7 +1580,9 @@ int ll_peak_fma(ll_ctx *ctx, int32_t which, int64_t iters, double *fma_per_s, do
     CK(cudaEventCreate(&e0));
     CK(cudaEventCreate(&e1));
     const int blocks = ctx->sm_count * 8, threads = 256;
-    for (int rep = 0; rep < 2; ++rep) { // first pass warms up
+    const int64_t iters_timed = iters;
+    for (int rep = 0; rep < 2; ++rep) { // first pass warms up (a short one when the timed pass runs for seconds)
+        iters = rep == 0 ? std::min<int64_t>(iters_timed, 4000) : iters_timed;
         CK(cudaEventRecord(e0, st));
         if (which == 0) k_peak_fma<double><<<blocks, threads, 0, st>>>(iters, ctx->prow.as<double>());
         else if (which == 1) k_peak_fma<float><<<blocks, threads, 0, st>>>(iters, ctx->prow.as<float>());

@@ -175,3 +175,47 @@ def test_cfg2_hm6_full_size_sampled(orc, torch_cuda):
     check_triplet(_np_triplet(got, sample), ref, "cfg2 six modes sampled")
     assert abs(np.sqrt(got[2][0]) - 500.0) < 1e-3
     ctx.destroy()
+
+
+def test_cfg2_three_channels_full_size_sampled(orc, torch_cuda):
+    """k_full_fused<1, 3, false> (per_config.cfg2_nc3): config 2 with three channels (A, E, T; the T channel with its own
+    PSD) at full size, 16 384 walkers with 11-double rows; 18 sampled walkers vs the oracle."""
+    wl = wlm.make_workload(2, n_c=3)
+    d, run = oracle_setup_full(orc, wl)
+    ctx = make_ctx(wl)
+    g = wl.grid
+    tc = torch_cuda
+    ctx.set_data(g.n_f, g.k_min, g.df, dev(tc, d), dev(tc, wl.W))
+    got = [x.cpu().numpy() for x in ctx.full_batch_standin(wl.f_nodes, dev(tc, wl.params))]
+    fis = np.array([orc.standin_fisco(p) for p in wl.params])
+    sample = sample_walkers(wl.n_w, fis, stride=2048)
+    assert len(sample) >= 16
+    ref = run(wl.params[sample], d)
+    check_triplet(_np_triplet(got, sample), ref, "cfg2 three channels sampled")
+    assert np.all(np.isfinite(got[0])) and abs(np.sqrt(got[2][0]) - 500.0) < 1e-3
+    ctx.destroy()
+
+
+def test_cfg2_split_tc_full_size_sampled(cfg2, orc, torch_cuda):
+    """per_config.cfg2_split_tc: the stand-in's linear term 2 pi f t_c (up to ~9e6 rad) kept outside the spline as
+    t_shift (reading R32) on the full config-2 batch; sampled walkers vs the oracle doing the same (long-double sum of the
+    two phase terms), and vs the oracle splining the full phase (the same template up to rounding)."""
+    wl, d, run, ctx, fis = cfg2
+    g = wl.grid
+    ctx.standin_split_tc(True)
+    try:
+        got = [x.cpu().numpy() for x in ctx.full_batch_standin(wl.f_nodes, dev(torch_cuda, wl.params))]
+    finally:
+        ctx.standin_split_tc(False)
+    sample = sample_walkers(wl.n_w, fis, stride=1024)
+    ref = orc.full_batch_standin(wl.modes_m, wl.c_lm, wl.kappa, wl.params[sample], wl.f_nodes, g.k_min, g.df, g.n_f, d, wl.W,
+                                 split_tc=True)
+    check_triplet(_np_triplet(got, sample), ref, "cfg2 split t_c sampled")
+    ref_full = run(wl.params[sample], d)
+    check_triplet(_np_triplet(got, sample), ref_full, "cfg2 split t_c vs the full-phase spline")
+    # what the split buys: distance of <d|h> from the oracle, split vs full-phase (reported in DESIGN.md §6)
+    plain = [x.cpu().numpy() for x in ctx.full_batch_standin(wl.f_nodes, dev(torch_cuda, wl.params[sample]))]
+    e_split = np.abs(got[1][sample] - ref["d_h"]).max()
+    e_plain = np.abs(plain[1] - ref_full["d_h"]).max()
+    print(f"max |d_h - oracle|: split t_c {e_split:.3e}, full-phase spline {e_plain:.3e}; "
+          f"oracle split vs oracle full {np.abs(ref['d_h'] - ref_full['d_h']).max():.3e}")
