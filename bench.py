@@ -219,12 +219,13 @@ def time_steps(torch, fn, steps: int, warmup: int):
     return e0.elapsed_time(e1)
 
 
-def bench_config(torch, index: int, steps: int, warmup: int, rank: int = 0, profile: bool = False, precision: int = 0):
+def bench_config(torch, index: int, steps: int, warmup: int, rank: int = 0, profile: bool = False, precision: int = 0,
+                 n_w=None):
     """device-resident timing of one config through the stand-in entry point (parameters -> log L).
     precision = 1: the FP32-accumulate variant of the full-grid path on the SAME data (the data stream is built
     by an FP64 context first, so the two variants can be compared output by output)."""
     from paper_2111_01064_b200 import synth
-    wl = rank_workload(index, rank)
+    wl = rank_workload(index, rank, n_w=n_w)
     ctx = synth.make_context(wl)
     bufs = synth.setup(ctx, wl)
     if precision:
@@ -548,10 +549,15 @@ def main():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--workload", type=int, default=2, help="BASELINE.json config index of the headline step")
     ap.add_argument("--quick", action="store_true", help="skip per_config, e2e and cpu_baseline (profiling runs)")
+    ap.add_argument("--n-walkers", type=int, default=None,
+                    help="profiling aid: the headline workload with this many walkers (e.g. 160: one Module-1 sized call); "
+                         "implies --quick, and the line's config says so")
     ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32acc"],
                     help="fp32acc: time the FP32-accumulate variant of the full-grid path as the headline step")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
+    if args.n_walkers is not None:
+        args.quick = True
 
     if args.impl == "reference":
         return run_reference(args)
@@ -574,7 +580,7 @@ def main():
     peaks, peak_src = measured_peaks()
     with ClockSampler(local) as clk:
         res = bench_config(torch, args.workload, args.steps, args.warmup, rank=rank, profile=True,
-                           precision=1 if args.precision == "fp32acc" else 0)
+                           precision=1 if args.precision == "fp32acc" else 0, n_w=args.n_walkers)
     wl, ctx = res["wl"], res["ctx"]
     headline_logL = res["out"][0].clone()
     t_ms = allreduce_max(res["ms_total"])

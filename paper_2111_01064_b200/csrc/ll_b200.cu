@@ -8,6 +8,7 @@
 #include <math.h>
 #include <stdint.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <algorithm>
@@ -98,6 +99,7 @@ struct ll_ctx {
     TileCache *tile_cur = nullptr; // the table of the call in progress
     long long data_version = 0;    // bumped by every ll_set_data
     DevBuf part2;                  // chunk partials of the two-stage finalize
+    DevBuf grp_tab;                // small batches: work items per group of 32 walkers (k_band_sort_small)
     DevBuf pw_x;                   // per-walker node grids: X [n_nodes][n_wp], then the effective bands [n_w][2]
     DevBuf node_tab; // doubles then ints
     NodeTables nt{};
@@ -316,12 +318,15 @@ FullPlan make_plan(const ll_ctx *ctx, long long n_w)
     // aim at ~16 blocks per SM over the whole grid, tiles between 64 and 4096 bins.  Small batches (blocks of one
     // warp, most tiles beyond the walkers' bands and exiting at once): 8x as many, smaller tiles, so that the active
     // ones still fill the SMs (measured on 160 walkers x 1.57e6 bins: TB 4096 -> 512 halves the fused kernel's time)
-    const long long target = (long long)ctx->sm_count * (pl.n_wp <= 1024 ? 128 : 16);
+    static const int small_factor = getenv("LL_SMALL_TILE_FACTOR") ? atoi(getenv("LL_SMALL_TILE_FACTOR")) : 128;
+    const long long target = (long long)ctx->sm_count * (pl.n_wp <= 1024 ? small_factor : 16);
     long long tb = ctx->n_f * n_wb / target;
     int TB = 64;
     while (TB < 4096 && TB < tb) TB <<= 1;
     pl.TB = TB;
-    pl.CH = std::min(TB, LL_FUSED_CH);
+    // bins per TMA stage: blocks of one warp (small batches) take 64-bin stages, 5 KB of shared memory per block, so
+    // that shared memory does not hold an SM to 11 resident warps (ncu r02a: 12 % warps active with 256-bin stages)
+    pl.CH = std::min(TB, pl.WB == 32 ? 64 : LL_FUSED_CH);
     pl.n_tiles = ceil_div(ctx->n_f, TB);
     pl.key_gran = std::max(1, ceil_div(ctx->n_f, 4096));
     pl.n_keys = (int)(ctx->n_f / pl.key_gran) + 2;
@@ -333,6 +338,7 @@ FullPlan make_plan(const ll_ctx *ctx, long long n_w)
 // change costs one dependent global load of the coefficients (~14 bins' worth of arithmetic) and log-spaced nodes
 // put dozens of intervals into the first tiles of the grid; cost = bins + 14 per interval <= TB.
 constexpr int kTileChunk = 64;
+constexpr int kSmallWarpsPerSM = 16; // one-warp blocks of the small-batch fused kernel resident per SM (register limit)
 int ensure_tiles(ll_ctx *ctx, FullPlan &pl, cudaStream_t st, bool uniform = false)
 {
     const int small = uniform ? 2 : (pl.n_wp <= 1024 ? 1 : 0); // 2: per-walker node grids, no shared interval table
@@ -387,7 +393,7 @@ int ensure_tiles(ll_ctx *ctx, FullPlan &pl, cudaStream_t st, bool uniform = fals
 
 // band -> bin range per walker, sort by band top (F1 prologue shared by every full-grid entry point)
 int band_sort(ll_ctx *ctx, const FullPlan &pl, long long n_w, bool standin, const double *params, int P, const double *band,
-              cudaStream_t st)
+              cudaStream_t st, int n_items = 0)
 {
     const int n_wp = pl.n_wp;
     CK(ctx->ilo_w.ensure(sizeof(int) * n_wp));
@@ -400,8 +406,11 @@ int band_sort(ll_ctx *ctx, const FullPlan &pl, long long n_w, bool standin, cons
     CK(ctx->pairs.ensure(sizeof(unsigned long long)));
     const GridInfo g{ctx->k_min, ctx->n_f, ctx->df};
     if (n_w <= 1024 && n_wp <= 1024) {
+        if (n_items) CK(ctx->grp_tab.ensure(sizeof(int) * kGrpInts));
         k_band_sort_small<<<1, 1024, 0, st>>>(standin ? 1 : 0, params, P, band, (int)n_w, n_wp, g, ctx->si, ctx->perm.as<int>(),
-                                              ctx->ilo_s.as<int>(), ctx->ihi_s.as<int>(), ctx->pairs.as<unsigned long long>());
+                                              ctx->ilo_s.as<int>(), ctx->ihi_s.as<int>(), ctx->pairs.as<unsigned long long>(),
+                                              n_items, n_items ? ctx->grp_tab.as<int>() : nullptr, ctx->nt.bstart,
+                                              (int)ctx->nodes_host.size());
         LAUNCHED(ctx);
     } else {
         CK(cudaMemsetAsync(ctx->hist.p, 0, sizeof(int) * pl.n_keys, st));
@@ -431,7 +440,8 @@ FusedArgs fused_args(ll_ctx *ctx, const FullPlan &pl, int n_nodes, const double 
     fa.perm = ctx->perm.as<int>(); fa.t_shift = t_shift; fa.ts_stride = ts_stride;
     fa.part = ctx->part.as<double>(); fa.k_min = ctx->k_min; fa.n_f_pad = ctx->n_f_pad; fa.df = ctx->df;
     fa.n_f = (int)ctx->n_f; fa.n_wp = pl.n_wp; fa.n_nodes = n_nodes; fa.n_m = ctx->n_m; fa.TB = pl.TB; fa.CH = pl.CH;
-    fa.tile_start = ctx->tile_cur->tab.as<int>();
+    fa.tile_start = ctx->tile_cur ? ctx->tile_cur->tab.as<int>() : nullptr;
+    fa.grp_tab = ctx->grp_tab.as<int>();
     return fa;
 }
 
@@ -489,7 +499,11 @@ int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, cons
     const int ns = tfp ? 2 + 2 * n_c : 2;
     const int P = 5 + 2 * n_c * n_m;
     FullPlan pl = make_plan(ctx, n_w);
-    {
+    // small batches (Module-1 sized): blocks of one warp, the work dealt out by active bins (k_band_sort_small)
+    const bool small = pl.n_wp <= 1024 && !tfp && !template_only && ctx->precision == LL_PREC_FP64;
+    static const int small_wps = getenv("LL_SMALL_WPS") ? atoi(getenv("LL_SMALL_WPS")) : kSmallWarpsPerSM;
+    const int n_items = small ? ctx->sm_count * small_wps : 0;
+    if (!small) {
         const int rc_t = ensure_tiles(ctx, pl, st);
         if (rc_t != LL_OK) return rc_t;
     }
@@ -503,9 +517,10 @@ int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, cons
     CK(ctx->Y.ensure(sizeof(double) * (size_t)n_m * ns * n_nodes * n_wp));
     CK(ctx->C.ensure(sizeof(double) * (size_t)(n_nodes - 1) * n_m * ns * 4 * n_wp));
     CK(ctx->TF.ensure(sizeof(double) * (size_t)n_m * 2 * n_c * n_wp));
-    if (!template_only) CK(ctx->part.ensure(sizeof(double) * (size_t)pl.n_tiles * NQ * n_wp));
+    if (small) CK(ctx->part.ensure(sizeof(double) * (size_t)(n_items + 32) * NQ * 32));
+    else if (!template_only) CK(ctx->part.ensure(sizeof(double) * (size_t)pl.n_tiles * NQ * n_wp));
     {
-        const int rc_b = band_sort(ctx, pl, n_w, standin, params, P, band, st);
+        const int rc_b = band_sort(ctx, pl, n_w, standin, params, P, band, st, n_items);
         if (rc_b != LL_OK) return rc_b;
     }
     if (standin) {
@@ -544,6 +559,37 @@ int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, cons
         LAUNCHED(ctx);
         return LL_OK;
     }
+    if (small) {
+        const int grid = n_items + 32; // rounding gives every non-empty group at least one item: up to 32 more than n_items
+        const size_t smem = (size_t)2 * pl.CH * 8 * (2 * n_c + nw);
+        {
+            ProfScope prof(ctx, st);
+#define LL_FUSED_SMALL(NC, WS)                                                        \
+    do {                                                                              \
+        if (nm1) k_full_fused<1, NC, WS, 1><<<grid, 32, smem, st>>>(fa);              \
+        else k_full_fused<0, NC, WS, 1><<<grid, 32, smem, st>>>(fa);                  \
+    } while (0)
+            LL_LAYOUT(ctx, LL_FUSED_SMALL);
+#undef LL_FUSED_SMALL
+            LAUNCHED(ctx);
+        }
+        ctx->last_n_blocks = grid;
+#define LL_FIN_SMALL(NC, WS)                                                                                               \
+    do {                                                                                                                   \
+        if (sums1)                                                                                                         \
+            k_finalize_small<1, NC, (WS ? 1 : NC)><<<n_wp / 32, dim3(32, fin_slices(2 * NC + (WS ? 1 : NC))), 0, st>>>(    \
+                ctx->part.as<double>(), ctx->TF.as<double>(), ctx->perm.as<int>(), ctx->ilo_s.as<int>(), ctx->ihi_s.as<int>(), \
+                n_wp, ctx->grp_tab.as<int>(), ctx->nt.bstart, n_nodes, ctx->dd.as<double>(), logL, d_h, h_h);              \
+        else                                                                                                               \
+            k_finalize_small<0, NC, (WS ? 1 : NC)><<<n_wp / 32, dim3(32, fin_slices(2)), 0, st>>>(                         \
+                ctx->part.as<double>(), ctx->TF.as<double>(), ctx->perm.as<int>(), ctx->ilo_s.as<int>(), ctx->ihi_s.as<int>(), \
+                n_wp, ctx->grp_tab.as<int>(), ctx->nt.bstart, n_nodes, ctx->dd.as<double>(), logL, d_h, h_h);              \
+    } while (0)
+        LL_LAYOUT(ctx, LL_FIN_SMALL);
+#undef LL_FIN_SMALL
+        LAUNCHED(ctx);
+        return LL_OK;
+    }
     {
         dim3 grid(n_wp / pl.WB, pl.n_tiles);
         const bool mixed = ctx->precision == LL_PREC_FP32_ACC && !tfp;
@@ -558,8 +604,8 @@ int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, cons
         if (tfp) {                                                                    \
             if (nm1) k_full_fused_tf<1, NC, WS><<<grid, pl.WB, smem, st>>>(fa);       \
             else k_full_fused_tf<0, NC, WS><<<grid, pl.WB, smem, st>>>(fa);           \
-        } else if (nm1) k_full_fused<1, NC, WS><<<grid, pl.WB, smem, st>>>(fa);       \
-        else k_full_fused<0, NC, WS><<<grid, pl.WB, smem, st>>>(fa);                  \
+        } else if (nm1) k_full_fused<1, NC, WS, 0><<<grid, pl.WB, smem, st>>>(fa);    \
+        else k_full_fused<0, NC, WS, 0><<<grid, pl.WB, smem, st>>>(fa);               \
     } while (0)
             LL_LAYOUT(ctx, LL_FUSED);
 #undef LL_FUSED
@@ -911,7 +957,7 @@ int ll_destroy(ll_ctx *ctx)
                          &ctx->key_w, &ctx->hist, &ctx->perm, &ctx->ilo_s, &ctx->ihi_s, &ctx->Y, &ctx->C, &ctx->TF,
                          &ctx->part, &ctx->prow, &ctx->het_tab, &ctx->het_tab1, &ctx->het_raw, &ctx->het_idx, &ctx->het_fb,
                          &ctx->stage_in, &ctx->stage_out, &ctx->g4f, &ctx->Wf, &ctx->scale, &ctx->wmax, &ctx->ref_idx,
-                         &ctx->ref_dense, &ctx->ref_edges, &ctx->tiles[0].tab, &ctx->tiles[1].tab, &ctx->tiles[2].tab, &ctx->part2, &ctx->pw_x, &ctx->pt_y, &ctx->pt_out, &ctx->pt_in, &ctx->pt_u};
+                         &ctx->ref_dense, &ctx->ref_edges, &ctx->tiles[0].tab, &ctx->tiles[1].tab, &ctx->tiles[2].tab, &ctx->grp_tab, &ctx->part2, &ctx->pw_x, &ctx->pt_y, &ctx->pt_out, &ctx->pt_in, &ctx->pt_u};
         for (DevBuf *b : all) b->release();
         for (auto &e : ctx->ev) cudaEventDestroy(e);
     }

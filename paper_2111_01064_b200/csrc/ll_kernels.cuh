@@ -84,6 +84,37 @@ struct GridInfo {
     double df;
 };
 
+// Cost model of the small-batch work partition: one unit per dense bin plus kIntervalCost per spline interval entered
+// (an interval change is a dependent load of the coefficients and a re-synchronisation of the recurrence; log-spaced
+// nodes put dozens of intervals into the first few hundred bins of the grid).  C(b) = b + K j(b), j(b) = interval of bin b.
+constexpr int kIntervalCost = 14;
+__device__ __forceinline__ int interval_of_bin_tab(const int *__restrict__ bstart, int n_nodes, int i)
+{
+    int lo = 0, hi = n_nodes - 2; // largest j in [0, n-2] with bstart[j] <= i
+    while (lo < hi) {
+        const int mid = (lo + hi + 1) >> 1;
+        if (__ldg(bstart + mid) <= i) lo = mid; else hi = mid - 1;
+    }
+    return lo;
+}
+__device__ __forceinline__ int cost_of_bin(const int *__restrict__ bstart, int n_nodes, int b)
+{
+    return bstart ? b + kIntervalCost * interval_of_bin_tab(bstart, n_nodes, b) : b;
+}
+// smallest bin b with C(b) >= X
+__device__ __forceinline__ int first_bin_with_cost(const int *__restrict__ bstart, int n_nodes, int X)
+{
+    if (!bstart) return X;
+    int lo = 0, hi = n_nodes - 2; // largest j with C(bstart[j]) = bstart[j] + K j <= X
+    while (lo < hi) {
+        const int mid = (lo + hi + 1) >> 1;
+        if (__ldg(bstart + mid) + kIntervalCost * mid <= X) lo = mid; else hi = mid - 1;
+    }
+    const int b = max(__ldg(bstart + lo), X - kIntervalCost * lo);
+    const int end = (lo < n_nodes - 2) ? __ldg(bstart + lo + 1) : INT_MAX;
+    return min(b, end);
+}
+
 struct StandinInfo {
     int n_m;
     int m_max;
@@ -153,12 +184,24 @@ k_band_prep(int use_standin, const double *__restrict__ params, int P, const dou
 // The same three steps (band -> bin range, sort by band top, scatter) for batches of up to 1024 walkers in ONE
 // block (Module-1 sized batches are latency-bound: one launch instead of three plus two memsets).  Rank of a walker
 // = number of walkers with a smaller (top bin, index): an O(n^2) count over shared memory, n <= 1024.
+// It also deals the fused kernel's work out by ACTIVE bins (grp_tab, when not null): a group = the 32 walkers of one
+// warp (consecutive sorted positions), its bin range [glo, ghi) = union of its walkers' bands, and the n_items blocks
+// of the fused kernel are shared among the groups in proportion to ghi - glo, so that every block gets the same
+// number of bins of ONE group and all of them start and finish together (no empty tiles, no tail).
+// "Bins" are counted in cost units C(b) (above), so that an item of the first, densely noded part of the grid holds
+// fewer bins: item t of group g = the bins b of [glo, ghi) with cg + t len <= C(b) < cg + (t + 1) len.
+constexpr int kGrpStride = 33; // grp_tab: [0..32] first item of group g (entry 32 = total), then glo, ghi, cg, len [32] each
+constexpr int kGrpInts = kGrpStride + 4 * 32;
+constexpr int kMinItemCost = 256;
 __global__ void __launch_bounds__(1024)
 k_band_sort_small(int use_standin, const double *__restrict__ params, int P, const double *__restrict__ band, int n_w,
                   int n_wp, GridInfo g, StandinInfo si, int *__restrict__ perm, int *__restrict__ ilo_s,
-                  int *__restrict__ ihi_s, unsigned long long *__restrict__ pairs)
+                  int *__restrict__ ihi_s, unsigned long long *__restrict__ pairs, int n_items, int *__restrict__ grp_tab,
+                  const int *__restrict__ bstart, int n_nodes)
 {
     __shared__ int s_hi[1024];
+    __shared__ int s_slo[1024], s_shi[1024]; // bands in sorted order
+    __shared__ long long s_U[32];
     __shared__ unsigned long long s_span[32];
     const int w = threadIdx.x;
     long long lo = 0, hi = 0;
@@ -184,10 +227,54 @@ k_band_sort_small(int use_standin, const double *__restrict__ params, int P, con
         perm[rank] = w;
         ilo_s[rank] = (int)lo;
         ihi_s[rank] = (int)hi;
-    } else if (w < n_wp) {
-        perm[w] = -1;
-        ilo_s[w] = 0;
-        ihi_s[w] = 0;
+        s_slo[rank] = (int)lo;
+        s_shi[rank] = (int)hi;
+    } else {
+        if (w < n_wp) {
+            perm[w] = -1;
+            ilo_s[w] = 0;
+            ihi_s[w] = 0;
+        }
+        s_slo[w] = 0;
+        s_shi[w] = 0;
+    }
+    if (!grp_tab) return;
+    __syncthreads();
+    const int n_groups = n_wp >> 5;
+    if (w < 32) {
+        int glo = INT_MAX, ghi = INT_MIN;
+        if (w < n_groups)
+            for (int k = 0; k < 32; ++k) {
+                const int l = s_slo[w * 32 + k], h = s_shi[w * 32 + k];
+                if (h > l) { glo = min(glo, l); ghi = max(ghi, h); }
+            }
+        int cg = 0;
+        if (glo >= ghi) { glo = 0; ghi = 0; s_U[w] = 0; }
+        else {
+            cg = cost_of_bin(bstart, n_nodes, glo);
+            s_U[w] = (long long)(cost_of_bin(bstart, n_nodes, ghi - 1) - cg + 1);
+        }
+        grp_tab[kGrpStride + w] = glo;
+        grp_tab[kGrpStride + 32 + w] = ghi;
+        grp_tab[kGrpStride + 64 + w] = cg;
+    }
+    __syncthreads();
+    if (w == 0) {
+        long long U = 0;
+        int n_live = 0;
+        for (int k = 0; k < n_groups; ++k) { U += s_U[k]; n_live += s_U[k] > 0; }
+        // tiny problems (config 0: 64 walkers x 6.5k bins) take fewer items than the grid has blocks — at least
+        // kMinItemCost units each — and the blocks beyond them exit at once
+        n_items = (int)min((long long)n_items, max((long long)n_live, U / kMinItemCost));
+        int first = 0;
+        for (int k = 0; k < 32; ++k) {
+            grp_tab[k] = first;
+            int n_g = 0;
+            if (k < n_groups && s_U[k] > 0) n_g = (int)max(1LL, (long long)n_items * s_U[k] / U);
+            grp_tab[kGrpStride + 96 + k] = n_g ? (int)((s_U[k] + n_g - 1) / n_g) : 1;
+            first += n_g;
+        }
+        grp_tab[32] = first;
     }
 }
 
@@ -710,6 +797,7 @@ struct FusedArgs {
     long long n_f_pad;     // row stride of Wc
     double df;
     const int *tile_start; // [n_tiles + 1]: frequency tile t covers dense bins [tile_start[t], tile_start[t+1])
+    const int *grp_tab;    // small batches (k_full_fused<.., SMALL = 1>): work dealt out by active bins, see k_band_sort_small
     int n_f, n_wp, n_nodes, n_m, TB, CH;
 };
 
@@ -909,11 +997,13 @@ __device__ __forceinline__ void unit_modulus(double &c, double &s)
     c *= k;
     s *= k;
 }
-template <int NC, bool WS>
-__device__ __forceinline__ void fused_bins_rot(int b0, int b1, int kbase, double df, double nxj, double cA0, double cA1,
-                                               double cA2, double cA3, double cP0, double cP1, double cP2, double cP3,
-                                               const double *__restrict__ sgc, const double *__restrict__ sWc, int CH,
-                                               Acc1<NC, WS> &acc)
+// MASK: lanes outside their own band [tlo, thi) ride along with amplitude 0 (the ragged end of a warp's band: a
+// few bins in a large sorted batch, but a third of all bins when a whole batch is only a handful of warps).
+template <bool MASK, int NC, bool WS>
+__device__ __forceinline__ void fused_bins_rot(int b0, int b1, int tlo, int thi, int kbase, double df, double nxj, double cA0,
+                                               double cA1, double cA2, double cA3, double cP0, double cP1, double cP2,
+                                               double cP3, const double *__restrict__ sgc, const double *__restrict__ sWc,
+                                               int CH, Acc1<NC, WS> &acc)
 {
     const double df2 = df * df, df3 = df2 * df;
     const double d3A = 6.0 * cA3 * df3;
@@ -937,8 +1027,9 @@ __device__ __forceinline__ void fused_bins_rot(int b0, int b1, int kbase, double
         unit_modulus(cv, sv);
 #pragma unroll kRotUnroll
         for (int ii = k0; ii < k1; ++ii) {
-            const double u = A * cz, v = A * sz; // h = u - i v
-            acc.add(sgc, sWc, CH, ii, u, v, A);
+            const double Am = (!MASK || ((ii >= tlo) && (ii < thi))) ? A : 0.0;
+            const double u = Am * cz, v = Am * sz; // h = u - i v
+            acc.add(sgc, sWc, CH, ii, u, v, Am);
             const double nzc = fma(cz, cw, -(sz * sw)), nzs = fma(sz, cw, cz * sw);
             const double nwc = fma(cw, cv, -(sw * sv)), nws = fma(sw, cv, cw * sv);
             const double nvc = fma(cv, cu, -(sv * su)), nvs = fma(sv, cu, cv * su);
@@ -948,8 +1039,11 @@ __device__ __forceinline__ void fused_bins_rot(int b0, int b1, int kbase, double
     }
 }
 
-// NM1 = 1: single-mode specialisation (NQ = 2 NC + NW partial sums per walker and tile); 0: any n_m (NQ = 2)
-template <int NM1, int NC, bool WS>
+// NM1 = 1: single-mode specialisation (NQ = 2 NC + NW partial sums per walker and tile); 0: any n_m (NQ = 2).
+// SMALL = 1 (batches of up to 1024 walkers; blocks of ONE warp): block b is item b of the group table — bins
+// [i0, i1) of one group of 32 walkers, an equal share of the batch's active bins — instead of (walker block, tile);
+// its partial sums go to part[b][NQ][32].
+template <int NM1, int NC, bool WS, int SMALL>
 __global__ void __launch_bounds__(128, (NC == 2 && WS) ? LL_FUSED_MINB : 3) k_full_fused(FusedArgs a)
 {
     using TL = Tile<NC, WS>;
@@ -958,9 +1052,25 @@ __global__ void __launch_bounds__(128, (NC == 2 && WS) ? LL_FUSED_MINB : 3) k_fu
     __shared__ int s_lo, s_hi;
 
     const int tid = threadIdx.x;
-    const int p = blockIdx.x * blockDim.x + tid;
-    const int tile = blockIdx.y;
-    const int i0 = __ldg(a.tile_start + tile), i1 = __ldg(a.tile_start + tile + 1); // tile = dense bins [i0, i1)
+    int p, tile, i0, i1;
+    if (SMALL) {
+        tile = blockIdx.x;
+        if (tile >= __ldg(a.grp_tab + 32)) return;
+        int grp = 0;
+        while (grp < 31 && __ldg(a.grp_tab + grp + 1) <= tile) ++grp;
+        const int first = __ldg(a.grp_tab + grp);
+        const int glo = __ldg(a.grp_tab + kGrpStride + grp), ghi = __ldg(a.grp_tab + kGrpStride + 32 + grp);
+        const int cg = __ldg(a.grp_tab + kGrpStride + 64 + grp), len = __ldg(a.grp_tab + kGrpStride + 96 + grp);
+        const int c0 = cg + (tile - first) * len;
+        i0 = min(max(first_bin_with_cost(a.bstart, a.n_nodes, c0), glo), ghi);
+        i1 = min(max(first_bin_with_cost(a.bstart, a.n_nodes, c0 + len), glo), ghi);
+        p = grp * 32 + tid;
+    } else {
+        p = blockIdx.x * blockDim.x + tid;
+        tile = blockIdx.y;
+        i0 = __ldg(a.tile_start + tile);
+        i1 = __ldg(a.tile_start + tile + 1); // tile = dense bins [i0, i1)
+    }
     const int lo = max(a.ilo[p], i0), hi = min(a.ihi[p], i1);
     if (tid == 0) {
         s_lo = INT_MAX;
@@ -976,7 +1086,14 @@ __global__ void __launch_bounds__(128, (NC == 2 && WS) ? LL_FUSED_MINB : 3) k_fu
     }
     __syncthreads();
     const int blo = s_lo, bhi = s_hi;
-    if (blo >= bhi) return; // no walker of this block has bins in this tile; k_finalize never reads it
+    if (blo >= bhi) { // no walker of this block has bins in this tile
+        if (SMALL) {  // an item of the cost partition may hold no bin at all, and k_finalize_small does read it
+            constexpr int NQ0 = NM1 ? 2 * NC + Acc1<NC, WS>::NW : 2;
+#pragma unroll
+            for (int q = 0; q < NQ0; ++q) a.part[((size_t)tile * NQ0 + q) * 32 + tid] = 0.0;
+        }
+        return; // large batches: k_finalize never reads it
+    }
 
     const int CH = a.CH;
     const int c_begin = blo / CH, c_end = (bhi + CH - 1) / CH;
@@ -1028,20 +1145,26 @@ __global__ void __launch_bounds__(128, (NC == 2 && WS) ? LL_FUSED_MINB : 3) k_fu
                     // bins every lane of the warp has inside its band run without the per-lane mask
                     const int flo = __reduce_max_sync(0xffffffffu, max(lo, i));
                     const int fhi = __reduce_min_sync(0xffffffffu, min(hi, seg_end));
+                    // masked stretch [b0, b1): by recurrence with the mask when it is long enough, else bin by bin
+                    auto masked = [&](int b0, int b1) {
+                        if (LL_FUSED_ROT && b1 - b0 >= 8)
+                            fused_bins_rot<true, NC, WS>(b0, b1, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1, cP2, cP3,
+                                                         sgc, sWc, CH, acc);
+                        else
+                            fused_bins_nm1<true, NC, WS>(b0, b1, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1, cP2, cP3,
+                                                         sgc, sWc, CH, acc);
+                    };
                     if (flo < fhi) {
-                        fused_bins_nm1<true, NC, WS>(wlo, flo, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1, cP2,
-                                                     cP3, sgc, sWc, CH, acc);
+                        masked(wlo, flo);
                         if (LL_FUSED_ROT && fhi - flo >= 8)
-                            fused_bins_rot<NC, WS>(flo, fhi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1, cP2, cP3, sgc, sWc,
-                                                   CH, acc);
+                            fused_bins_rot<false, NC, WS>(flo, fhi, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1, cP2,
+                                                          cP3, sgc, sWc, CH, acc);
                         else
                             fused_bins_nm1<false, NC, WS>(flo, fhi, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1,
                                                           cP2, cP3, sgc, sWc, CH, acc);
-                        fused_bins_nm1<true, NC, WS>(fhi, whi, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1, cP2,
-                                                     cP3, sgc, sWc, CH, acc);
+                        masked(fhi, whi);
                     } else {
-                        fused_bins_nm1<true, NC, WS>(wlo, whi, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1, cP2,
-                                                     cP3, sgc, sWc, CH, acc);
+                        masked(wlo, whi);
                     }
                 } else {
                     // any number of modes: chunks of four bins with the MODE loop outside the bins, so that a mode's
@@ -1091,16 +1214,16 @@ __global__ void __launch_bounds__(128, (NC == 2 && WS) ? LL_FUSED_MINB : 3) k_fu
         }
         __syncthreads(); // everyone is done with stage st before it is refilled two chunks later
     }
+    constexpr int NQ = NM1 ? 2 * NC + Acc1<NC, WS>::NW : 2;
+    const size_t so = SMALL ? 32 : sw; // stride between the partial sums of one record
+    double *o = SMALL ? a.part + (size_t)tile * NQ * 32 + tid : a.part + ((size_t)tile * NQ) * sw + p;
     if (NM1) {
-        constexpr int NQ = 2 * NC + Acc1<NC, WS>::NW;
-        double *o = a.part + ((size_t)tile * NQ) * sw + p;
 #pragma unroll
-        for (int q = 0; q < 2 * NC; ++q) o[(size_t)q * sw] = acc.S[q];
+        for (int q = 0; q < 2 * NC; ++q) o[(size_t)q * so] = acc.S[q];
 #pragma unroll
-        for (int q = 0; q < Acc1<NC, WS>::NW; ++q) o[(size_t)(2 * NC + q) * sw] = acc.H[q];
+        for (int q = 0; q < Acc1<NC, WS>::NW; ++q) o[(size_t)(2 * NC + q) * so] = acc.H[q];
     } else {
-        double *o = a.part + ((size_t)tile * 2) * sw + p;
-        o[0] = acc.S[0]; o[sw] = acc.S[1];
+        o[0] = acc.S[0]; o[so] = acc.S[1];
     }
 }
 
@@ -1939,6 +2062,69 @@ k_finalize(const double *__restrict__ part, const double *__restrict__ TF, const
     if (NM1) {
         // Re sum_c T^c S^c,  sum_c |T^c|^2 H^c (one H for a shared weight row)
         dh = 0.0; hh = 0.0;
+        double t2 = 0.0;
+#pragma unroll
+        for (int c = 0; c < NC; ++c) {
+            const double tr = TF[(size_t)(2 * c) * sw + p], ti = TF[(size_t)(2 * c + 1) * sw + p];
+            dh += tr * acc[2 * c] - ti * acc[2 * c + 1];
+            if (NW == 1) t2 += tr * tr + ti * ti;
+            else hh += (tr * tr + ti * ti) * acc[2 * NC + c];
+        }
+        if (NW == 1) hh = t2 * acc[2 * NC];
+    } else {
+        dh = acc[0];
+        hh = acc[1];
+    }
+    logL[w] = dh - 0.5 * hh - 0.5 * dd[0];
+    if (d_h) d_h[w] = dh;
+    if (h_h) h_h[w] = hh;
+}
+
+// F4 for small batches (k_full_fused<.., SMALL = 1>): one block per group of 32 walkers; the items of the group that
+// overlap a walker's band are summed by 32 slices in a fixed order, T^c applied, log L formed.
+template <int NM1, int NC, int NW>
+__global__ void __launch_bounds__(32 * fin_slices(NM1 ? 2 * NC + NW : 2))
+k_finalize_small(const double *__restrict__ part, const double *__restrict__ TF, const int *__restrict__ perm,
+                 const int *__restrict__ ilo, const int *__restrict__ ihi, int n_wp, const int *__restrict__ grp_tab,
+                 const int *__restrict__ bstart, int n_nodes, const double *__restrict__ dd, double *__restrict__ logL,
+                 double *__restrict__ d_h, double *__restrict__ h_h)
+{
+    constexpr int NQ = NM1 ? 2 * NC + NW : 2;
+    constexpr int FY = fin_slices(NQ);
+    __shared__ double red[FY][NQ][32];
+    const int grp = blockIdx.x, lane = threadIdx.x, ty = threadIdx.y;
+    const int p = grp * 32 + lane;
+    const size_t sw = (size_t)n_wp;
+    const int lo = ilo[p], hi = ihi[p];
+    double acc[NQ];
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) acc[q] = 0.0;
+    const int first = grp_tab[grp], n_g = grp_tab[grp + 1] - first;
+    if (hi > lo && n_g > 0) {
+        const int cg = grp_tab[kGrpStride + 64 + grp], len = grp_tab[kGrpStride + 96 + grp];
+        const int t0 = (cost_of_bin(bstart, n_nodes, lo) - cg) / len;
+        const int t1 = min((cost_of_bin(bstart, n_nodes, hi - 1) - cg) / len, n_g - 1);
+        for (int t = t0 + ty; t <= t1; t += FY) {
+            const double *o = part + (size_t)(first + t) * NQ * 32 + lane;
+#pragma unroll
+            for (int q = 0; q < NQ; ++q) acc[q] += o[q * 32];
+        }
+    }
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) red[ty][q][lane] = acc[q];
+    __syncthreads();
+    if (ty != 0) return;
+    const int w = perm[p];
+    if (w < 0) return;
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) {
+        double v = red[0][q][lane];
+#pragma unroll
+        for (int k = 1; k < FY; ++k) v += red[k][q][lane];
+        acc[q] = v;
+    }
+    double dh = 0.0, hh = 0.0;
+    if (NM1) {
         double t2 = 0.0;
 #pragma unroll
         for (int c = 0; c < NC; ++c) {
