@@ -406,11 +406,12 @@ int band_sort(ll_ctx *ctx, const FullPlan &pl, long long n_w, bool standin, cons
     CK(ctx->pairs.ensure(sizeof(unsigned long long)));
     const GridInfo g{ctx->k_min, ctx->n_f, ctx->df};
     if (n_w <= 1024 && n_wp <= 1024) {
-        if (n_items) CK(ctx->grp_tab.ensure(sizeof(int) * kGrpInts));
+        const int max_items = n_items ? n_items + 32 : 0; // = the fused kernel's grid (every live group gets >= 1 item)
+        if (n_items) CK(ctx->grp_tab.ensure(sizeof(int) * (grp_off_items() + 4 * (size_t)max_items)));
         k_band_sort_small<<<1, 1024, 0, st>>>(standin ? 1 : 0, params, P, band, (int)n_w, n_wp, g, ctx->si, ctx->perm.as<int>(),
                                               ctx->ilo_s.as<int>(), ctx->ihi_s.as<int>(), ctx->pairs.as<unsigned long long>(),
-                                              n_items, n_items ? ctx->grp_tab.as<int>() : nullptr, ctx->nt.bstart,
-                                              (int)ctx->nodes_host.size());
+                                              n_items, max_items, n_items ? ctx->grp_tab.as<int>() : nullptr,
+                                              n_items ? ctx->nt.bstart : nullptr, (int)ctx->nodes_host.size());
         LAUNCHED(ctx);
     } else {
         CK(cudaMemsetAsync(ctx->hist.p, 0, sizeof(int) * pl.n_keys, st));
@@ -578,12 +579,12 @@ int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, cons
     do {                                                                                                                   \
         if (sums1)                                                                                                         \
             k_finalize_small<1, NC, (WS ? 1 : NC)><<<n_wp / 32, dim3(32, fin_slices(2 * NC + (WS ? 1 : NC))), 0, st>>>(    \
-                ctx->part.as<double>(), ctx->TF.as<double>(), ctx->perm.as<int>(), ctx->ilo_s.as<int>(), ctx->ihi_s.as<int>(), \
-                n_wp, ctx->grp_tab.as<int>(), ctx->nt.bstart, n_nodes, ctx->dd.as<double>(), logL, d_h, h_h);              \
+                ctx->part.as<double>(), ctx->TF.as<double>(), ctx->perm.as<int>(), n_wp, ctx->grp_tab.as<int>(),           \
+                ctx->dd.as<double>(), logL, d_h, h_h);                                                                     \
         else                                                                                                               \
             k_finalize_small<0, NC, (WS ? 1 : NC)><<<n_wp / 32, dim3(32, fin_slices(2)), 0, st>>>(                         \
-                ctx->part.as<double>(), ctx->TF.as<double>(), ctx->perm.as<int>(), ctx->ilo_s.as<int>(), ctx->ihi_s.as<int>(), \
-                n_wp, ctx->grp_tab.as<int>(), ctx->nt.bstart, n_nodes, ctx->dd.as<double>(), logL, d_h, h_h);              \
+                ctx->part.as<double>(), ctx->TF.as<double>(), ctx->perm.as<int>(), n_wp, ctx->grp_tab.as<int>(),           \
+                ctx->dd.as<double>(), logL, d_h, h_h);                                                                     \
     } while (0)
         LL_LAYOUT(ctx, LL_FIN_SMALL);
 #undef LL_FIN_SMALL

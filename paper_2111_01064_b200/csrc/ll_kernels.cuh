@@ -88,30 +88,31 @@ struct GridInfo {
 // (an interval change is a dependent load of the coefficients and a re-synchronisation of the recurrence; log-spaced
 // nodes put dozens of intervals into the first few hundred bins of the grid).  C(b) = b + K j(b), j(b) = interval of bin b.
 constexpr int kIntervalCost = 14;
-__device__ __forceinline__ int interval_of_bin_tab(const int *__restrict__ bstart, int n_nodes, int i)
+// (bstart may point to global memory or to a shared-memory copy; nullptr = no shared interval table: C(b) = b)
+__device__ __forceinline__ int interval_of_bin_tab(const int *bstart, int n_nodes, int i)
 {
     int lo = 0, hi = n_nodes - 2; // largest j in [0, n-2] with bstart[j] <= i
     while (lo < hi) {
         const int mid = (lo + hi + 1) >> 1;
-        if (__ldg(bstart + mid) <= i) lo = mid; else hi = mid - 1;
+        if (bstart[mid] <= i) lo = mid; else hi = mid - 1;
     }
     return lo;
 }
-__device__ __forceinline__ int cost_of_bin(const int *__restrict__ bstart, int n_nodes, int b)
+__device__ __forceinline__ int cost_of_bin(const int *bstart, int n_nodes, int b)
 {
     return bstart ? b + kIntervalCost * interval_of_bin_tab(bstart, n_nodes, b) : b;
 }
 // smallest bin b with C(b) >= X
-__device__ __forceinline__ int first_bin_with_cost(const int *__restrict__ bstart, int n_nodes, int X)
+__device__ __forceinline__ int first_bin_with_cost(const int *bstart, int n_nodes, int X)
 {
     if (!bstart) return X;
     int lo = 0, hi = n_nodes - 2; // largest j with C(bstart[j]) = bstart[j] + K j <= X
     while (lo < hi) {
         const int mid = (lo + hi + 1) >> 1;
-        if (__ldg(bstart + mid) + kIntervalCost * mid <= X) lo = mid; else hi = mid - 1;
+        if (bstart[mid] + kIntervalCost * mid <= X) lo = mid; else hi = mid - 1;
     }
-    const int b = max(__ldg(bstart + lo), X - kIntervalCost * lo);
-    const int end = (lo < n_nodes - 2) ? __ldg(bstart + lo + 1) : INT_MAX;
+    const int b = max(bstart[lo], X - kIntervalCost * lo);
+    const int end = (lo < n_nodes - 2) ? bstart[lo + 1] : INT_MAX;
     return min(b, end);
 }
 
@@ -190,20 +191,34 @@ k_band_prep(int use_standin, const double *__restrict__ params, int P, const dou
 // number of bins of ONE group and all of them start and finish together (no empty tiles, no tail).
 // "Bins" are counted in cost units C(b) (above), so that an item of the first, densely noded part of the grid holds
 // fewer bins: item t of group g = the bins b of [glo, ghi) with cg + t len <= C(b) < cg + (t + 1) len.
+// The kernel is the planner of the whole small-batch call: besides the group table it writes, per item, (group, first
+// bin, end bin, interval of the first bin) and, per walker, the first and last item its band touches, so that neither
+// the fused kernel's blocks nor k_finalize_small search anything.
 constexpr int kGrpStride = 33; // grp_tab: [0..32] first item of group g (entry 32 = total), then glo, ghi, cg, len [32] each
 constexpr int kGrpInts = kGrpStride + 4 * 32;
-constexpr int kMinItemCost = 256;
+// after them: t0[1024], t1[1024] (items of sorted position p), then item[4][max_items] (group, i0, i1, j0)
+__host__ __device__ constexpr int grp_off_t0() { return kGrpInts; }
+__host__ __device__ constexpr int grp_off_t1() { return kGrpInts + 1024; }
+__host__ __device__ constexpr int grp_off_items() { return kGrpInts + 2048; }
+constexpr int kMinItemCost = 64;
 __global__ void __launch_bounds__(1024)
 k_band_sort_small(int use_standin, const double *__restrict__ params, int P, const double *__restrict__ band, int n_w,
                   int n_wp, GridInfo g, StandinInfo si, int *__restrict__ perm, int *__restrict__ ilo_s,
-                  int *__restrict__ ihi_s, unsigned long long *__restrict__ pairs, int n_items, int *__restrict__ grp_tab,
-                  const int *__restrict__ bstart, int n_nodes)
+                  int *__restrict__ ihi_s, unsigned long long *__restrict__ pairs, int n_items, int max_items,
+                  int *__restrict__ grp_tab, const int *__restrict__ bstart_g, int n_nodes)
 {
     __shared__ int s_hi[1024];
     __shared__ int s_slo[1024], s_shi[1024]; // bands in sorted order
+    __shared__ int s_bs[1024];               // the bin -> interval table, when it fits
+    __shared__ int s_first[33], s_glo[32], s_ghi[32], s_cg[32], s_len[32];
     __shared__ long long s_U[32];
     __shared__ unsigned long long s_span[32];
     const int w = threadIdx.x;
+    const int *bstart = bstart_g;
+    if (grp_tab && bstart_g && n_nodes <= 1024) {
+        if (w < n_nodes) s_bs[w] = bstart_g[w];
+        bstart = s_bs; // visible after the first barrier below
+    }
     long long lo = 0, hi = 0;
     if (w < n_w) band_bins(use_standin, params, P, band, w, g, si, lo, hi);
     s_hi[w] = (w < n_w) ? (int)hi : INT_MAX;
@@ -257,6 +272,7 @@ k_band_sort_small(int use_standin, const double *__restrict__ params, int P, con
         grp_tab[kGrpStride + w] = glo;
         grp_tab[kGrpStride + 32 + w] = ghi;
         grp_tab[kGrpStride + 64 + w] = cg;
+        s_glo[w] = glo; s_ghi[w] = ghi; s_cg[w] = cg;
     }
     __syncthreads();
     if (w == 0) {
@@ -269,12 +285,43 @@ k_band_sort_small(int use_standin, const double *__restrict__ params, int P, con
         int first = 0;
         for (int k = 0; k < 32; ++k) {
             grp_tab[k] = first;
+            s_first[k] = first;
             int n_g = 0;
             if (k < n_groups && s_U[k] > 0) n_g = (int)max(1LL, (long long)n_items * s_U[k] / U);
-            grp_tab[kGrpStride + 96 + k] = n_g ? (int)((s_U[k] + n_g - 1) / n_g) : 1;
+            const int len = n_g ? (int)((s_U[k] + n_g - 1) / n_g) : 1;
+            grp_tab[kGrpStride + 96 + k] = len;
+            s_len[k] = len;
             first += n_g;
         }
         grp_tab[32] = first;
+        s_first[32] = first;
+    }
+    __syncthreads();
+    // per item: group, bins [i0, i1), interval of i0
+    const int total = min(s_first[32], max_items);
+    int *it = grp_tab + grp_off_items();
+    for (int id = w; id < total; id += 1024) {
+        int grp = 0;
+        while (grp < 31 && s_first[grp + 1] <= id) ++grp;
+        const int c0 = s_cg[grp] + (id - s_first[grp]) * s_len[grp];
+        const int i0 = min(max(first_bin_with_cost(bstart, n_nodes, c0), s_glo[grp]), s_ghi[grp]);
+        const int i1 = min(max(first_bin_with_cost(bstart, n_nodes, c0 + s_len[grp]), s_glo[grp]), s_ghi[grp]);
+        it[id] = grp;
+        it[max_items + id] = i0;
+        it[2 * max_items + id] = i1;
+        it[3 * max_items + id] = bstart ? interval_of_bin_tab(bstart, n_nodes, i0) : 0;
+    }
+    // per sorted position: first and last item its band touches
+    if (w < n_wp) {
+        const int grp = w >> 5, l = s_slo[w], h = s_shi[w];
+        const int n_g = s_first[grp + 1] - s_first[grp];
+        int t0 = 0, t1 = -1;
+        if (h > l && n_g > 0) {
+            t0 = (cost_of_bin(bstart, n_nodes, l) - s_cg[grp]) / s_len[grp];
+            t1 = min((cost_of_bin(bstart, n_nodes, h - 1) - s_cg[grp]) / s_len[grp], n_g - 1);
+        }
+        grp_tab[grp_off_t0() + w] = s_first[grp] + t0;
+        grp_tab[grp_off_t1() + w] = s_first[grp] + t1;
     }
 }
 
@@ -1052,19 +1099,16 @@ __global__ void __launch_bounds__(128, (NC == 2 && WS) ? LL_FUSED_MINB : 3) k_fu
     __shared__ int s_lo, s_hi;
 
     const int tid = threadIdx.x;
-    int p, tile, i0, i1;
+    int p, tile, i0, i1, j_hint = 0;
     if (SMALL) {
         tile = blockIdx.x;
         if (tile >= __ldg(a.grp_tab + 32)) return;
-        int grp = 0;
-        while (grp < 31 && __ldg(a.grp_tab + grp + 1) <= tile) ++grp;
-        const int first = __ldg(a.grp_tab + grp);
-        const int glo = __ldg(a.grp_tab + kGrpStride + grp), ghi = __ldg(a.grp_tab + kGrpStride + 32 + grp);
-        const int cg = __ldg(a.grp_tab + kGrpStride + 64 + grp), len = __ldg(a.grp_tab + kGrpStride + 96 + grp);
-        const int c0 = cg + (tile - first) * len;
-        i0 = min(max(first_bin_with_cost(a.bstart, a.n_nodes, c0), glo), ghi);
-        i1 = min(max(first_bin_with_cost(a.bstart, a.n_nodes, c0 + len), glo), ghi);
-        p = grp * 32 + tid;
+        const int *it = a.grp_tab + grp_off_items() + tile;
+        const int mi = gridDim.x; // the table's row length = the grid
+        i0 = __ldg(it + mi);
+        i1 = __ldg(it + 2 * mi);
+        j_hint = __ldg(it + 3 * mi);
+        p = __ldg(it) * 32 + tid;
     } else {
         p = blockIdx.x * blockDim.x + tid;
         tile = blockIdx.y;
@@ -1101,7 +1145,7 @@ __global__ void __launch_bounds__(128, (NC == 2 && WS) ? LL_FUSED_MINB : 3) k_fu
 
     const size_t sw = (size_t)a.n_wp;
     const size_t cj = (size_t)a.n_m * 8 * sw;
-    int j = find_interval_of_bin(a.bstart, a.n_nodes, blo);
+    int j = SMALL ? j_hint : find_interval_of_bin(a.bstart, a.n_nodes, blo); // the bin loop moves a hint up to its interval
     int jl = -1;
     double cA0 = 0, cA1 = 0, cA2 = 0, cA3 = 0, cP0 = 0, cP1 = 0, cP2 = 0, cP3 = 0, nxj = 0;
     const int kbase = (int)a.k_min; // k_min + n_f < 2^31 is checked on the host
@@ -2085,8 +2129,7 @@ k_finalize(const double *__restrict__ part, const double *__restrict__ TF, const
 template <int NM1, int NC, int NW>
 __global__ void __launch_bounds__(32 * fin_slices(NM1 ? 2 * NC + NW : 2))
 k_finalize_small(const double *__restrict__ part, const double *__restrict__ TF, const int *__restrict__ perm,
-                 const int *__restrict__ ilo, const int *__restrict__ ihi, int n_wp, const int *__restrict__ grp_tab,
-                 const int *__restrict__ bstart, int n_nodes, const double *__restrict__ dd, double *__restrict__ logL,
+                 int n_wp, const int *__restrict__ grp_tab, const double *__restrict__ dd, double *__restrict__ logL,
                  double *__restrict__ d_h, double *__restrict__ h_h)
 {
     constexpr int NQ = NM1 ? 2 * NC + NW : 2;
@@ -2095,20 +2138,15 @@ k_finalize_small(const double *__restrict__ part, const double *__restrict__ TF,
     const int grp = blockIdx.x, lane = threadIdx.x, ty = threadIdx.y;
     const int p = grp * 32 + lane;
     const size_t sw = (size_t)n_wp;
-    const int lo = ilo[p], hi = ihi[p];
     double acc[NQ];
 #pragma unroll
     for (int q = 0; q < NQ; ++q) acc[q] = 0.0;
-    const int first = grp_tab[grp], n_g = grp_tab[grp + 1] - first;
-    if (hi > lo && n_g > 0) {
-        const int cg = grp_tab[kGrpStride + 64 + grp], len = grp_tab[kGrpStride + 96 + grp];
-        const int t0 = (cost_of_bin(bstart, n_nodes, lo) - cg) / len;
-        const int t1 = min((cost_of_bin(bstart, n_nodes, hi - 1) - cg) / len, n_g - 1);
-        for (int t = t0 + ty; t <= t1; t += FY) {
-            const double *o = part + (size_t)(first + t) * NQ * 32 + lane;
+    const int t0 = grp_tab[grp_off_t0() + p], t1 = grp_tab[grp_off_t1() + p]; // items the walker's band touches
+#pragma unroll 4
+    for (int t = t0 + ty; t <= t1; t += FY) {
+        const double *o = part + (size_t)t * NQ * 32 + lane;
 #pragma unroll
-            for (int q = 0; q < NQ; ++q) acc[q] += o[q * 32];
-        }
+        for (int q = 0; q < NQ; ++q) acc[q] += o[q * 32];
     }
 #pragma unroll
     for (int q = 0; q < NQ; ++q) red[ty][q][lane] = acc[q];
