@@ -258,6 +258,12 @@ int ll_pt_run_het(ll_ctx *ctx, int32_t n_temps, int32_t n_walkers, double *x, do
 int ll_pt_run_full(ll_ctx *ctx, int32_t n_nodes, const double *f_nodes, int32_t n_temps, int32_t n_walkers, double *x,
                    double *logL, double *d_h, double *h_h, const double *betas, const double *lo, const double *hi,
                    int32_t n_dim, double a, uint64_t seed, int64_t iter0, int64_t n_iter, uint64_t *n_accepted, void *stream);
+/* ll_pt_run_het runs the WHOLE loop as one cooperative launch (a grid of one block per SM that keeps the summary table
+ * in shared memory and separates the half updates and the swap sweep by grid barriers) when the context has one mode,
+ * n_temps <= 32, and the device supports cooperative launches; otherwise — and always after ll_pt_fused(ctx, 0) — it
+ * enqueues 9 launches per iteration.  Both forms are the same function of (seed, iter0, state): same uniforms, same
+ * arithmetic, same decisions.                                                                                        */
+int ll_pt_fused(ll_ctx *ctx, int32_t on);
 typedef struct {
     int32_t n_checks; /* consecutive unchanged checks needed to stop (30 in the paper)   */
     int32_t count;    /* consecutive unchanged checks so far                             */

@@ -26,7 +26,7 @@ SYMBOLS = (
     "ll_full_batch", "ll_full_batch_pw", "ll_full_batch_tf", "ll_tlm_nodes", "ll_standin_nodes", "ll_full_batch_standin", "ll_full_batch_standin_host",
     "ll_full_template_standin",
     "ll_template_standin", "ll_het_prepare", "ll_het_refresh_standin", "ll_het_audit_standin",
-    "ll_pt_stretch_half_het", "ll_pt_stretch_half_full", "ll_pt_swap", "ll_pt_stats", "ll_pt_run_het", "ll_pt_run_full", "ll_stop_snr", "ll_stop_converged", "ll_het_get_summary", "ll_het_batch", "ll_het_batch_standin",
+    "ll_pt_stretch_half_het", "ll_pt_stretch_half_full", "ll_pt_swap", "ll_pt_stats", "ll_pt_run_het", "ll_pt_run_full", "ll_pt_fused", "ll_stop_snr", "ll_stop_converged", "ll_het_get_summary", "ll_het_batch", "ll_het_batch_standin",
     "ll_het_batch_standin_host", "ll_peak_fma", "ll_kernel_launches", "ll_last_full_stats",
     "ll_profile_enable", "ll_profile_read",
 )
@@ -89,6 +89,7 @@ def load_library(path: Optional[str] = None):
         "ll_pt_run_full": (C.c_int, [vp, i32, vp, i32, i32, vp, vp, vp, vp, vp, vp, vp, i32, dbl, C.c_uint64, i64, i64, vp,
                                      vp]),
         "ll_pt_stats": (C.c_int, [vp, i64, vp, vp, vp, vp, vp]),
+        "ll_pt_fused": (C.c_int, [vp, i32]),
         "ll_stop_snr": (C.c_int, [dbl, dbl]),
         "ll_stop_converged": (C.c_int, [vp, dbl]),
         "ll_het_batch_standin_host": (C.c_int, [vp, i64, vp, vp, vp, vp, vp]),
@@ -481,6 +482,10 @@ class Context:
             f_nodes = _host_f64(f_nodes, "f_nodes")
             self._check(self._lib.ll_pt_run_full(self._h, len(f_nodes), f_nodes.ctypes.data_as(C.c_void_p), *tail),
                         "ll_pt_run_full")
+
+    def pt_fused(self, on: bool = True):
+        """ll_pt_run_het as one cooperative launch (default) or as 9 launches per iteration"""
+        self._check(self._lib.ll_pt_fused(self._h, 1 if on else 0), "ll_pt_fused")
 
     def pt_swap(self, x, logL, d_h, h_h, betas, u_swap, swapped=None, stream=None):
         n_t, n_w = int(x.shape[0]), int(x.shape[1])

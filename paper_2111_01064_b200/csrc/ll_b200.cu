@@ -122,6 +122,9 @@ struct ll_ctx {
     int het1_bps = 0;
     long long hetn_key_groups = -1;
     int hetn_key_total = -1, hetn_S = 1, hetn_grid = 1;
+    bool pt_fused = true;          // ll_pt_run_het: the one-launch cooperative kernel when the population fits it
+    int coop = -1;                 // device supports cooperative launches (-1: not asked yet)
+    bool ptrun_attr = false;
     HetTable ht{};
     Het1Table ht1{}; // single-mode regrouped table (k_het_standin1); base == nullptr when not built
     std::vector<double> raw_host; // [n_b][6 n_c + 1]
@@ -898,6 +901,44 @@ int launch_het_standin_modes(ll_ctx *ctx, int64_t n_w, const double *params, dou
     }
 }
 
+// the heterodyned loop as ONE cooperative launch (k_pt_run_het1): single mode with the edge-regrouped table, up to 32
+// temperatures.  Returns LL_ERR_UNSUPPORTED when the population or the device does not fit (the caller falls back).
+template <int NC>
+int pt_run_fused(ll_ctx *ctx, int32_t n_t, int32_t n_w, double *x, double *logL, double *d_h, double *h_h, const double *betas,
+                 const double *lo, const double *hi, int32_t n_dim, double a, uint64_t seed, int64_t iter0, int64_t n_iter,
+                 uint64_t *n_accepted, cudaStream_t st)
+{
+    constexpr int WY = LL_HET1_WY;
+    if (ctx->coop < 0) {
+        int v = 0;
+        if (cudaDeviceGetAttribute(&v, cudaDevAttrCooperativeLaunch, ctx->device) != cudaSuccess) v = 0;
+        ctx->coop = v;
+    }
+    if (!ctx->coop) return LL_ERR_UNSUPPORTED;
+    const size_t tab_d = (size_t)ctx->ht1.n_e * het1_stride(NC);
+    const size_t smem = sizeof(double) * (tab_d + (tab_d & 1) + (size_t)WY * 32 * 3 * NC + 7 * 32);
+    if (smem > 227 * 1024) return LL_ERR_UNSUPPORTED;
+    if (!ctx->ptrun_attr) {
+        CK(cudaFuncSetAttribute(k_pt_run_het1<NC>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+        ctx->ptrun_attr = true;
+    }
+    int bps = 0;
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, k_pt_run_het1<NC>, 32 * WY, smem));
+    if (bps < 1) return LL_ERR_UNSUPPORTED;
+    const int n_pass = ceil_div((long long)n_t * (n_w / 2), 32);
+    const int grid = std::max(1, std::min(std::max(n_pass, ceil_div(n_w, WY)), ctx->sm_count * bps));
+    PtRunArgs pa;
+    pa.x = x; pa.logL = logL; pa.d_h = d_h; pa.h_h = h_h; pa.betas = betas; pa.lo = lo; pa.hi = hi;
+    pa.dd = ctx->dd.as<double>(); pa.n_acc = (unsigned long long *)n_accepted; pa.seed = seed; pa.iter0 = iter0;
+    pa.n_iter = n_iter; pa.n_t = n_t; pa.n_w = n_w; pa.n_dim = n_dim; pa.a = a;
+    Het1Table tab = ctx->ht1;
+    StandinInfo si = ctx->si;
+    void *args[] = {&tab, &si, &pa};
+    CK(cudaLaunchCooperativeKernel((const void *)k_pt_run_het1<NC>, dim3(grid), dim3(32, WY), args, smem, st));
+    LAUNCHED(ctx);
+    return LL_OK;
+}
+
 } // namespace
 
 // =====================================================================================================
@@ -906,7 +947,7 @@ int launch_het_standin_modes(ll_ctx *ctx, int64_t n_w, const double *params, dou
 extern "C" {
 
 int ll_abi_version(void) { return 3; } // 3: n_channels 2 or 3 and ll_set_data w_shared (per-channel weights), t_shift on the array
-                                       // entry points, ll_standin_split_tc, ll_pt_run_het_fused
+                                       // entry points, ll_standin_split_tc, ll_pt_fused
 
 int ll_create(const ll_config *cfg, ll_ctx **out)
 {
@@ -1553,6 +1594,19 @@ int pt_run(ll_ctx *ctx, bool full, int32_t n_nodes, const double *f_nodes, int32
     if ((int64_t)n_t * n_w > (1LL << 28)) return ctx->fail(LL_ERR_ARG, "n_temps * n_walkers too large");
     DeviceGuard dg(ctx->device);
     cudaStream_t st = (cudaStream_t)stream;
+    if (!full && ctx->pt_fused && ctx->n_m == 1 && n_t <= 32 && n_iter > 0) {
+        // the same checks pt_half makes, then the whole loop in one cooperative launch
+        if (!x || !logL || !betas || !lo || !hi) return ctx->fail(LL_ERR_ARG, "NULL argument");
+        if (n_dim < 1 || !(a > 1.0)) return ctx->fail(LL_ERR_ARG, "n_dim >= 1 and a > 1 are required");
+        int rc = het_check(ctx, (int64_t)n_t * n_w, logL);
+        if (rc != LL_OK) return rc;
+        if (!ctx->have_standin) return ctx->fail(LL_ERR_STATE, "ll_standin_config has not been called");
+        if (ctx->ht1.base) {
+            rc = ctx->n_c == 2 ? pt_run_fused<2>(ctx, n_t, n_w, x, logL, d_h, h_h, betas, lo, hi, n_dim, a, seed, iter0, n_iter, n_accepted, st)
+                               : pt_run_fused<3>(ctx, n_t, n_w, x, logL, d_h, h_h, betas, lo, hi, n_dim, a, seed, iter0, n_iter, n_accepted, st);
+            if (rc != LL_ERR_UNSUPPORTED) return rc;
+        }
+    }
     const int n_half = n_t * (n_w / 2), n_swap = (n_t - 1) * n_w;
     CK(ctx->pt_u.ensure(sizeof(double) * (size_t)(6 * n_half + n_swap)));
     double *u = ctx->pt_u.as<double>();
@@ -1588,6 +1642,13 @@ int ll_pt_run_full(ll_ctx *ctx, int32_t n_nodes, const double *f_nodes, int32_t 
 {
     return pt_run(ctx, true, n_nodes, f_nodes, n_temps, n_walkers, x, logL, d_h, h_h, betas, lo, hi, n_dim, a, seed, iter0,
                   n_iter, n_accepted, stream);
+}
+
+int ll_pt_fused(ll_ctx *ctx, int32_t on)
+{
+    if (!ctx) return LL_ERR_ARG;
+    ctx->pt_fused = on != 0;
+    return LL_OK;
 }
 
 int ll_pt_stats(ll_ctx *ctx, int64_t n, const double *logL, const double *d_h, const double *h_h, double *out3, void *stream)

@@ -13,6 +13,7 @@
 // false: one row per channel, "T different").
 #pragma once
 #include <limits.h>
+#include <cooperative_groups.h>
 #include "ll_device.cuh"
 
 namespace ll {
@@ -2614,6 +2615,80 @@ struct Het1Table {
     int n_e, n_b;
 };
 
+// the sums of one walker over the edges [e0, e1) of the table (and the bins [e0, min(e1, n_b))): D^c = sum conj(z) Q^c
+// (re, im), H^c = sum |z|^2 P^c + Re[z_b conj(z_{b+1}) X^c_b]; lanes of the warp are 32 walkers at the same edges
+template <int NC>
+__device__ __forceinline__ void het1_segment(const double *__restrict__ tab, int n_b, const StandinInfo &si,
+                                             const WalkerConst &c, int e0, int e1, double (&D)[2 * NC], double (&H)[NC])
+{
+    constexpr int ST = het1_stride(NC);
+    constexpr int oQ = 4, oP = 4 + 2 * NC, oX = 4 + 3 * NC; // offsets of Q, P, X inside an edge's row
+    const double inv_kappa = 1.0 / si.kappa;
+    const double mh_pi = (double)si.mode_m[0] / kPi;
+    const double Kq = mh_pi * c.K, nphq = -mh_pi * (c.phi + 0.25 * kPi);
+    auto edge = [&](const double *t, double &u, double &v, double &amp) {
+        const double y = fma(t[0], c.tc, fma(Kq, t[1], nphq));
+        amp = t[2] * c.invD * taper(t[3] * c.inv_fisco, si.kappa, inv_kappa);
+        amp_expi_qc(amp, y, u, v); // z = u - i v
+    };
+    const double *t = tab + (size_t)e0 * ST;
+    double up, vp, ap;
+    edge(t, up, vp, ap);
+    const int last = min(e1, n_b); // one past the last bin whose cross term this segment owns
+    auto edge_terms = [&](const double *tt, double u, double v, double a) { // conj(z) Q and |z|^2 P of one edge
+        const double a2 = a * a;
+#pragma unroll
+        for (int cc = 0; cc < NC; ++cc) {
+            const double qr = tt[oQ + 2 * cc], qi = tt[oQ + 2 * cc + 1];
+            D[2 * cc] = fma(u, qr, D[2 * cc]); D[2 * cc] = fma(-v, qi, D[2 * cc]);
+            D[2 * cc + 1] = fma(u, qi, D[2 * cc + 1]); D[2 * cc + 1] = fma(v, qr, D[2 * cc + 1]);
+            H[cc] = fma(a2, tt[oP + cc], H[cc]);
+        }
+    };
+    auto cross_terms = [&](const double *tt, double u0, double v0, double u1, double v1) { // z_e conj(z_{e+1}) X
+        const double wr = fma(u0, u1, v0 * v1), wi = fma(u0, v1, -(v0 * u1));
+#pragma unroll
+        for (int cc = 0; cc < NC; ++cc) {
+            H[cc] = fma(wr, tt[oX + 2 * cc], H[cc]);
+            H[cc] = fma(-wi, tt[oX + 2 * cc + 1], H[cc]);
+        }
+    };
+    int e = e0;
+    // chunks of kE bins: the kE next edges are kE independent phase -> sincos chains in flight per thread;
+    // the taper polynomial is needed only where some lane is above its f_ISCO (one warp-uniform test per chunk)
+    constexpr int kE = 4;
+    for (; e + kE <= last; e += kE, t += kE * ST) {
+        double un[kE], vn[kE], an[kE];
+        const bool tapered = __any_sync(0xffffffffu, t[kE * ST + 3] * c.inv_fisco > 1.0);
+#pragma unroll
+        for (int k = 0; k < kE; ++k) {
+            const double *tn = t + (k + 1) * ST;
+            const double y = fma(tn[0], c.tc, fma(Kq, tn[1], nphq));
+            double a = tn[2] * c.invD;
+            if (tapered) a *= taper_nobranch(tn[3] * c.inv_fisco, si.kappa, inv_kappa);
+            an[k] = a;
+            amp_expi_qc(a, y, un[k], vn[k]);
+        }
+#pragma unroll
+        for (int k = 0; k < kE; ++k) {
+            const double *tt = t + k * ST;
+            const double u0 = k ? un[k - 1] : up, v0 = k ? vn[k - 1] : vp, a0 = k ? an[k - 1] : ap;
+            edge_terms(tt, u0, v0, a0);
+            cross_terms(tt, u0, v0, un[k], vn[k]);
+        }
+        up = un[kE - 1]; vp = vn[kE - 1]; ap = an[kE - 1];
+    }
+    for (; e < e1; ++e, t += ST) {
+        edge_terms(t, up, vp, ap);
+        if (e < last) { // bin e = [e, e + 1]: needs z at e + 1 (the next segment's first edge at the boundary)
+            double un, vn, an;
+            edge(t + ST, un, vn, an);
+            cross_terms(t, up, vp, un, vn);
+            up = un; vp = vn; ap = an;
+        }
+    }
+}
+
 #ifndef LL_HET1_WY
 #define LL_HET1_WY 16 // warps per block of the single-mode kernel (one block per SM shares the table copy)
 #endif
@@ -2624,7 +2699,6 @@ k_het_standin1(Het1Table T, StandinInfo si, const double *__restrict__ params, i
                double *__restrict__ h_h)
 {
     constexpr int ST = het1_stride(NC);
-    constexpr int oQ = 4, oP = 4 + 2 * NC, oX = 4 + 3 * NC; // offsets of Q, P, X inside an edge's row
     constexpr int NR = 3 * NC;                               // partial sums per walker: D^c (re, im), H^c
     extern __shared__ __align__(16) double tab[];
     const int total = T.n_e * ST;
@@ -2634,9 +2708,7 @@ k_het_standin1(Het1Table T, StandinInfo si, const double *__restrict__ params, i
     const int G = blockDim.y / S, seg = threadIdx.y % S, gslot = threadIdx.y / S, lane = threadIdx.x;
     const int per = (T.n_e + S - 1) / S;
     const int e0 = seg * per, e1 = min(e0 + per, T.n_e); // this segment owns edges [e0, e1) and bins [e0, min(e1, n_b))
-    const double inv_kappa = 1.0 / si.kappa;
     const double ddb = dd[1];
-    const double mh_pi = (double)si.mode_m[0] / kPi;
 
     for (int base = blockIdx.x * G; base < n_groups; base += gridDim.x * G) {
         const int grp = base + gslot;
@@ -2644,75 +2716,12 @@ k_het_standin1(Het1Table T, StandinInfo si, const double *__restrict__ params, i
         const bool valid = grp < n_groups && w < n_w;
         const double *row = params + (size_t)(valid ? w : 0) * P;
         const WalkerConst c = standin_consts(row);
-        const double Kq = mh_pi * c.K, nphq = -mh_pi * (c.phi + 0.25 * kPi);
         double D[2 * NC], H[NC];
 #pragma unroll
         for (int q = 0; q < 2 * NC; ++q) D[q] = 0.0;
 #pragma unroll
         for (int q = 0; q < NC; ++q) H[q] = 0.0;
-        if (grp < n_groups && e0 < e1) {
-            auto edge = [&](const double *t, double &u, double &v, double &amp) {
-                const double y = fma(t[0], c.tc, fma(Kq, t[1], nphq));
-                amp = t[2] * c.invD * taper(t[3] * c.inv_fisco, si.kappa, inv_kappa);
-                amp_expi_qc(amp, y, u, v); // z = u - i v
-            };
-            const double *t = tab + (size_t)e0 * ST;
-            double up, vp, ap;
-            edge(t, up, vp, ap);
-            const int last = min(e1, T.n_b); // one past the last bin whose cross term this segment owns
-            auto edge_terms = [&](const double *tt, double u, double v, double a) { // conj(z) Q and |z|^2 P of one edge
-                const double a2 = a * a;
-#pragma unroll
-                for (int cc = 0; cc < NC; ++cc) {
-                    const double qr = tt[oQ + 2 * cc], qi = tt[oQ + 2 * cc + 1];
-                    D[2 * cc] = fma(u, qr, D[2 * cc]); D[2 * cc] = fma(-v, qi, D[2 * cc]);
-                    D[2 * cc + 1] = fma(u, qi, D[2 * cc + 1]); D[2 * cc + 1] = fma(v, qr, D[2 * cc + 1]);
-                    H[cc] = fma(a2, tt[oP + cc], H[cc]);
-                }
-            };
-            auto cross_terms = [&](const double *tt, double u0, double v0, double u1, double v1) { // z_e conj(z_{e+1}) X
-                const double wr = fma(u0, u1, v0 * v1), wi = fma(u0, v1, -(v0 * u1));
-#pragma unroll
-                for (int cc = 0; cc < NC; ++cc) {
-                    H[cc] = fma(wr, tt[oX + 2 * cc], H[cc]);
-                    H[cc] = fma(-wi, tt[oX + 2 * cc + 1], H[cc]);
-                }
-            };
-            int e = e0;
-            // chunks of kE bins: the kE next edges are kE independent phase -> sincos chains in flight per thread;
-            // the taper polynomial is needed only where some lane is above its f_ISCO (one warp-uniform test per chunk)
-            constexpr int kE = 4;
-            for (; e + kE <= last; e += kE, t += kE * ST) {
-                double un[kE], vn[kE], an[kE];
-                const bool tapered = __any_sync(0xffffffffu, t[kE * ST + 3] * c.inv_fisco > 1.0);
-#pragma unroll
-                for (int k = 0; k < kE; ++k) {
-                    const double *tn = t + (k + 1) * ST;
-                    const double y = fma(tn[0], c.tc, fma(Kq, tn[1], nphq));
-                    double a = tn[2] * c.invD;
-                    if (tapered) a *= taper_nobranch(tn[3] * c.inv_fisco, si.kappa, inv_kappa);
-                    an[k] = a;
-                    amp_expi_qc(a, y, un[k], vn[k]);
-                }
-#pragma unroll
-                for (int k = 0; k < kE; ++k) {
-                    const double *tt = t + k * ST;
-                    const double u0 = k ? un[k - 1] : up, v0 = k ? vn[k - 1] : vp, a0 = k ? an[k - 1] : ap;
-                    edge_terms(tt, u0, v0, a0);
-                    cross_terms(tt, u0, v0, un[k], vn[k]);
-                }
-                up = un[kE - 1]; vp = vn[kE - 1]; ap = an[kE - 1];
-            }
-            for (; e < e1; ++e, t += ST) {
-                edge_terms(t, up, vp, ap);
-                if (e < last) { // bin e = [e, e + 1]: needs z at e + 1 (the next segment's first edge at the boundary)
-                    double un, vn, an;
-                    edge(t + ST, un, vn, an);
-                    cross_terms(t, up, vp, un, vn);
-                    up = un; vp = vn; ap = an;
-                }
-            }
-        }
+        if (grp < n_groups && e0 < e1) het1_segment<NC>(tab, T.n_b, si, c, e0, e1, D, H);
         if (S > 1) {
             double *rg = red + (size_t)gslot * S * (NR * 32);
             double *q = rg + seg * (NR * 32) + lane;
@@ -3003,6 +3012,239 @@ k_pt_uniforms(unsigned long long seed, long long it, int n_half, int n_swap, dou
     const unsigned long long k = splitmix_mix(seed + G * (unsigned long long)(8 * it + kind + 1));
     const unsigned long long r = splitmix_mix(k + G * (unsigned long long)(index + 1));
     u[i] = (double)(r >> 11) * 0x1.0p-53;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// The whole sampler loop on the heterodyned likelihood in ONE launch (4e8 heterodyned evaluations
+// are the paper's whole cost, a Module-2 iteration is 4000 of them).  A cooperative grid of one block per SM keeps the
+// single-mode summary table (k_het_standin1's Q, P, X form) in shared memory for all n_iter iterations and runs, per
+// iteration: [uniforms -> propose -> H1-H3 -> accept] for half 0, grid barrier, the same for half 1, grid barrier,
+// the temperature-swap sweep (one warp per walker column), grid barrier.  Uniforms are the counter-based ones of
+// reading R31, computed where they are used (no buffer), every arithmetic step is the one of k_pt_propose /
+// k_het_standin1 / k_pt_accept / k_pt_swap_warp, so a run is the same pure function of (seed, iter0, state).
+// Block = 32 lanes x WY warps: lanes are 32 proposals, warp s takes edge segment s of the table (S = WY segments).
+// ---------------------------------------------------------------------------------------------------
+struct PtRunArgs {
+    double *x, *logL, *d_h, *h_h;       // [n_t][n_w][P], [n_t][n_w] (d_h, h_h may be null): read AND written in the loop
+    const double *betas, *lo, *hi, *dd; // [n_t], [P], [P], dd[1] = <d|d> over the band
+    unsigned long long *n_acc;          // [n_t] or null
+    unsigned long long seed;
+    long long iter0, n_iter;
+    int n_t, n_w, n_dim;
+    double a;
+};
+
+__device__ __forceinline__ double pt_uniform(unsigned long long seed, long long it, int kind, long long index)
+{
+    const unsigned long long G = 0x9E3779B97F4A7C15ull;
+    const unsigned long long k = splitmix_mix(seed + G * (unsigned long long)(8 * it + kind + 1));
+    const unsigned long long r = splitmix_mix(k + G * (unsigned long long)(index + 1));
+    return (double)(r >> 11) * 0x1.0p-53;
+}
+
+template <int NC>
+__global__ void __launch_bounds__(32 * LL_HET1_WY, 1)
+k_pt_run_het1(Het1Table T, StandinInfo si, PtRunArgs a)
+{
+    constexpr int ST = het1_stride(NC);
+    constexpr int NR = 3 * NC;
+    constexpr int P = 5 + 2 * NC;
+    constexpr int S = LL_HET1_WY;
+    cooperative_groups::grid_group grid = cooperative_groups::this_grid();
+    extern __shared__ __align__(16) double tab[];
+    const int total = T.n_e * ST;
+    double *red = tab + total + (total & 1); // [S][NR][32]
+    double *wc_s = red + S * NR * 32;        // [7][32]: the walker constants of the pass's 32 proposals, ln u_accept, (d-1) ln z
+    for (int i = threadIdx.x + threadIdx.y * 32; i < total; i += 32 * blockDim.y) tab[i] = T.base[i];
+    __syncthreads();
+    const int seg = threadIdx.y, lane = threadIdx.x;
+    const int per = (T.n_e + S - 1) / S;
+    const int e0 = seg * per, e1 = min(e0 + per, T.n_e);
+    const double ddb = a.dd[1];
+    const int n_t = a.n_t, n_w = a.n_w, nh = n_w / 2, n_half = n_t * nh;
+    const int n_pass = (n_half + 31) / 32;
+    // the loop state is rewritten between grid barriers: plain (coherent) loads only, never the read-only path
+    double *x = a.x, *logL = a.logL;
+
+#ifdef LL_PT_TIMING // build-time debugging aid: where an iteration's time goes, as seen by block 0
+    long long tm[4] = {0, 0, 0, 0}, t_a = 0, t_b = 0;
+    auto now = []() { long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; };
+#define LL_PT_TICK(v) v = now()
+#define LL_PT_ADD(k, d) tm[k] += (d)
+#else
+#define LL_PT_TICK(v)
+#define LL_PT_ADD(k, d)
+#endif
+    for (long long it = a.iter0; it < a.iter0 + a.n_iter; ++it) {
+        for (int half = 0; half < 2; ++half) {
+            LL_PT_TICK(t_a);
+            const int k0 = half == 0 ? 0 : nh, j0 = half == 0 ? nh : 0;
+            for (int pass = blockIdx.x; pass < n_pass; pass += gridDim.x) {
+                const int i = pass * 32 + lane;
+                const bool valid = i < n_half;
+                const int ii = valid ? i : 0;
+                const int t = ii / nh, k = ii - t * nh;
+                // ---- proposal (k_pt_propose) and the walker constants, ONCE per proposal, by the first warp (with 16
+                // segment warps each redoing pow, cbrt and three divisions for its 8 edges, the constants were more
+                // than half of the block's FP64 instructions); the others pick the five constants up from shared memory
+                double y[P], z = 1.0;
+                bool in = true;
+                const size_t wk = (size_t)t * n_w + k0 + k;
+                WalkerConst c;
+                if (seg == 0) {
+                    const double tt = __dadd_rn(__dmul_rn(a.a - 1.0, pt_uniform(a.seed, it, 3 * half, ii)), 1.0);
+                    z = __ddiv_rn(__dmul_rn(tt, tt), a.a);
+                    int j = (int)(pt_uniform(a.seed, it, 3 * half + 1, ii) * (double)nh);
+                    j = min(max(j, 0), nh - 1);
+                    const double *xk = x + wk * P;
+                    const double *xj = x + ((size_t)t * n_w + j0 + j) * P;
+#pragma unroll
+                    for (int q = 0; q < P; ++q) {
+                        const double xkq = xk[q], xjq = xj[q], lq = a.lo[q], hq = a.hi[q];
+                        const double v = __dadd_rn(xjq, __dmul_rn(z, __dadd_rn(xkq, -xjq)));
+                        in = in & (v >= lq) & (v <= hq);
+                        y[q] = v;
+                    }
+                    if (!in) {
+#pragma unroll
+                        for (int q = 0; q < P; ++q) y[q] = xk[q];
+                    }
+                    c = standin_consts(y);
+                    wc_s[lane] = c.tc; wc_s[32 + lane] = c.invD; wc_s[64 + lane] = c.inv_fisco; wc_s[96 + lane] = c.K;
+                    wc_s[128 + lane] = c.phi;
+                } else if (seg == 1) {
+                    // the two logarithms of the acceptance test depend on the uniforms only: the second warp has them
+                    // ready in shared memory before the first one needs them
+                    const double tt = __dadd_rn(__dmul_rn(a.a - 1.0, pt_uniform(a.seed, it, 3 * half, ii)), 1.0);
+                    const double zz = __ddiv_rn(__dmul_rn(tt, tt), a.a);
+                    wc_s[160 + lane] = log(pt_uniform(a.seed, it, 3 * half + 2, ii));
+                    wc_s[192 + lane] = (double)(a.n_dim - 1) * log(zz);
+                }
+                __syncthreads();
+                if (seg != 0) {
+                    c.tc = wc_s[lane]; c.invD = wc_s[32 + lane]; c.inv_fisco = wc_s[64 + lane]; c.K = wc_s[96 + lane];
+                    c.phi = wc_s[128 + lane];
+                }
+                // ---- H1-H3 on the proposal (k_het_standin1)
+                double D[2 * NC], H[NC];
+#pragma unroll
+                for (int q = 0; q < 2 * NC; ++q) D[q] = 0.0;
+#pragma unroll
+                for (int q = 0; q < NC; ++q) H[q] = 0.0;
+                if (e0 < e1) het1_segment<NC>(tab, T.n_b, si, c, e0, e1, D, H);
+                double *qd = red + seg * (NR * 32) + lane;
+#pragma unroll
+                for (int q = 0; q < 2 * NC; ++q) qd[32 * q] = D[q];
+#pragma unroll
+                for (int q = 0; q < NC; ++q) qd[32 * (2 * NC + q)] = H[q];
+                __syncthreads();
+                if (seg == 0 && valid) {
+#pragma unroll
+                    for (int q = 0; q < 2 * NC; ++q) D[q] = 0.0;
+#pragma unroll
+                    for (int q = 0; q < NC; ++q) H[q] = 0.0;
+                    for (int s = 0; s < S; ++s) {
+                        const double *r = red + s * (NR * 32) + lane;
+#pragma unroll
+                        for (int q = 0; q < 2 * NC; ++q) D[q] += r[32 * q];
+#pragma unroll
+                        for (int q = 0; q < NC; ++q) H[q] += r[32 * (2 * NC + q)];
+                    }
+                    double dh = 0.0, hh = 0.0;
+#pragma unroll
+                    for (int cc = 0; cc < NC; ++cc) {
+                        const double tr = y[5 + 2 * cc], ti = y[6 + 2 * cc];
+                        dh += tr * D[2 * cc] + ti * D[2 * cc + 1];
+                        hh += (tr * tr + ti * ti) * H[cc];
+                    }
+                    const double l_new = dh - 0.5 * hh - 0.5 * ddb;
+                    // ---- accept (k_pt_accept)
+                    bool acc = false;
+                    if (in && l_new == l_new && fabs(l_new) != INFINITY) {
+                        const double lnq = __dadd_rn(wc_s[192 + lane], __dmul_rn(a.betas[t], __dadd_rn(l_new, -logL[wk])));
+                        acc = wc_s[160 + lane] < lnq;
+                    }
+                    if (acc) {
+                        double *xo = x + wk * P;
+#pragma unroll
+                        for (int q = 0; q < P; ++q) xo[q] = y[q];
+                        logL[wk] = l_new;
+                        if (a.d_h) a.d_h[wk] = dh;
+                        if (a.h_h) a.h_h[wk] = hh;
+                        if (a.n_acc) atomicAdd(a.n_acc + t, 1ull); // integer: order-independent
+                    }
+                }
+                __syncthreads(); // red is reused by the next pass
+            }
+            LL_PT_TICK(t_b);
+            grid.sync(); // the other half reads what this one wrote
+            LL_PT_ADD(0, t_b - t_a);
+            LL_PT_ADD(1, now() - t_b);
+        }
+        if (n_t > 1) {
+            LL_PT_TICK(t_a);
+            // ---- temperature swaps (reading R27; same decisions as k_pt_swap_warp): one warp per walker column.
+            // Going down from the hottest rung, the cold partner of step t is always the ORIGINAL rung t - 1 (nothing has
+            // touched it yet) and the hot one is whatever has been carried down so far, so the sweep is a scalar
+            // recurrence on (carried log L, its source rung) — two FP64 operations and a compare per rung — after
+            // which every rung knows which original row it ends up with and only the rows that moved are copied.
+            for (int col = blockIdx.x * S + seg; col < n_w; col += gridDim.x * S) {
+                const bool has = lane < n_t;
+                const size_t cidx = (size_t)(has ? lane : 0) * n_w + col;
+                const double l = has ? logL[cidx] : 0.0;
+                const double dh = (has && a.d_h) ? a.d_h[cidx] : 0.0, hh = (has && a.h_h) ? a.h_h[cidx] : 0.0;
+                const double beta = has ? a.betas[lane] : 0.0;
+                const double lnu = (lane >= 1 && has) ? log(pt_uniform(a.seed, it, 6, (long long)(lane - 1) * n_w + col)) : 0.0;
+                const double db = __dadd_rn(beta, -__shfl_up_sync(0xffffffffu, beta, 1)); // beta_t - beta_{t-1}
+                const double lprev = __shfl_up_sync(0xffffffffu, l, 1);                  // ln L of rung t - 1
+                double carried = __shfl_sync(0xffffffffu, l, n_t - 1);
+                int csrc = n_t - 1, my_src = lane;
+                for (int t = n_t - 1; t >= 1; --t) {
+                    const double lu = __shfl_sync(0xffffffffu, lnu, t), d = __shfl_sync(0xffffffffu, db, t);
+                    const double lc = __shfl_sync(0xffffffffu, lprev, t);
+                    const bool sw = lu < __dmul_rn(d, __dadd_rn(lc, -carried));
+                    if (lane == t) my_src = sw ? t - 1 : csrc;
+                    if (!sw) { carried = lc; csrc = t - 1; }
+                }
+                if (lane == 0) my_src = csrc;
+                // rows: every read before any write
+                double xv[32];
+#pragma unroll
+                for (int t = 0; t < 32; ++t) {
+                    xv[t] = 0.0;
+                    if (t < n_t) { // uniform
+                        const int src = __shfl_sync(0xffffffffu, my_src, t);
+                        if (src != t && lane < P) xv[t] = x[((size_t)src * n_w + col) * P + lane];
+                    }
+                }
+                const double l_new = __shfl_sync(0xffffffffu, l, my_src & 31);
+                const double dh_new = __shfl_sync(0xffffffffu, dh, my_src & 31), hh_new = __shfl_sync(0xffffffffu, hh, my_src & 31);
+                __syncwarp();
+#pragma unroll
+                for (int t = 0; t < 32; ++t)
+                    if (t < n_t) {
+                        const int src = __shfl_sync(0xffffffffu, my_src, t);
+                        if (src != t && lane < P) x[((size_t)t * n_w + col) * P + lane] = xv[t];
+                    }
+                if (has && my_src != lane) {
+                    logL[cidx] = l_new;
+                    if (a.d_h) a.d_h[cidx] = dh_new;
+                    if (a.h_h) a.h_h[cidx] = hh_new;
+                }
+            }
+            LL_PT_TICK(t_b);
+            grid.sync();
+            LL_PT_ADD(2, t_b - t_a);
+            LL_PT_ADD(3, now() - t_b);
+        }
+    }
+#ifdef LL_PT_TIMING
+    if (blockIdx.x == 0 && threadIdx.x == 0 && threadIdx.y == 0)
+        printf("pt_run phases per iteration (ns): half %.0f  sync %.0f  swap %.0f  sync %.0f\n", (double)tm[0] / (2.0 * a.n_iter),
+               (double)tm[1] / (2.0 * a.n_iter), (double)tm[2] / a.n_iter, (double)tm[3] / a.n_iter);
+#endif
+#undef LL_PT_TICK
+#undef LL_PT_ADD
 }
 
 // what the stopping tests look at: out[0] = max finite log L, out[1] = its index (lowest on

@@ -51,8 +51,8 @@ def test_library_is_sm100a_only(so_path):
 
 
 def test_tma_and_mbarrier_in_fused_kernel_sass(so_path):
-    # k_full_fused<1, 2, true> (two channels, shared weight row: the bench's kernel) and <1, 3, false> (A, E, T)
-    for fun in ("_ZN2ll12k_full_fusedILi1ELi2ELb1EEEvNS_9FusedArgsE", "_ZN2ll12k_full_fusedILi1ELi3ELb0EEEvNS_9FusedArgsE"):
+    # k_full_fused<1, 2, true, 0> (two channels, shared weight row: the bench kernel) and <1, 3, false, 0> (A, E, T)
+    for fun in ("_ZN2ll12k_full_fusedILi1ELi2ELb1ELi0EEEvNS_9FusedArgsE", "_ZN2ll12k_full_fusedILi1ELi3ELb0ELi0EEEvNS_9FusedArgsE"):
         out = subprocess.run(["cuobjdump", "-sass", "-fun", fun, so_path], capture_output=True, text=True)
         if out.returncode != 0 or not out.stdout:
             pytest.skip("cuobjdump unavailable")

@@ -854,6 +854,86 @@ def test_pt_run_parity_het(orc, het_small, torch_cuda):
     assert tc.equal(gx2, gx) and tc.equal(gl2, gl)
 
 
+def test_pt_run_fused_150_iterations_and_both_forms(orc, het_small, torch_cuda):
+    """ll_pt_run_het as ONE cooperative launch (k_pt_run_het1: the whole loop on the device, grid barriers between the
+    half updates and the swap sweep): 150 iterations (the paper's check cadence) against the oracle's
+    loop — identical positions, equal acceptance counters — and against the 9-launches-per-iteration form of the same
+    entry point (ll_pt_fused(0)): same positions, log L equal to rounding."""
+    from oracle import sampler as sm
+    wl, d, h0, h0e, summ, ctx = het_small
+    tc = torch_cuda
+    n_t, n_w = 3, 64
+    x = wl.params[:n_t * n_w].reshape(n_t, n_w, -1).copy()
+    x[:, :, 5:] = wl.inj[5:]
+    betas = np.array([1.0, 0.3, 0.05])
+    lo, hi = _prior_box(wl, wl.params, 0.35)
+    ll = _oracle_loglike_het(orc, wl, h0e, summ)
+    logL = ll(x.reshape(n_t * n_w, -1))[0].reshape(n_t, n_w).copy()
+    out0 = ctx.het_batch_standin(dev(tc, x.reshape(n_t * n_w, -1)))
+    gx, gl, gd, gh = dev(tc, x), dev(tc, logL), out0[1].reshape(n_t, n_w).clone(), out0[2].reshape(n_t, n_w).clone()
+    ux, ul, ud, uh = gx.clone(), gl.clone(), gd.clone(), gh.clone()
+    acc_g = tc.zeros(n_t, dtype=tc.int64, device="cuda")
+    acc_u = tc.zeros(n_t, dtype=tc.int64, device="cuda")
+    seed, n_iter = 2111, 150
+    n_acc = sm.run(x, logL, betas, lo, hi, 5, 2.0, seed, 40, n_iter, ll)
+    launches0 = ctx.kernel_launches()
+    ctx.pt_run(gx, gl, gd, gh, dev(tc, betas), dev(tc, lo), dev(tc, hi), 5, seed, 40, n_iter, n_accepted=acc_g)
+    assert ctx.kernel_launches() - launches0 == 1                       # the whole run is one launch
+    assert np.array_equal(gx.cpu().numpy(), x)
+    assert np.array_equal(acc_g.cpu().numpy(), n_acc) and n_acc.sum() > 5000
+    err = np.abs(gl.cpu().numpy() - logL) / np.maximum(1.0, np.abs(logL))
+    assert err.max() <= 1e-6
+    # the carried <d|h>, <h|h> belong to the positions
+    chk = ctx.het_batch_standin(gx.reshape(n_t * n_w, -1))
+    assert np.allclose(gd.cpu().numpy().ravel(), chk[1].cpu().numpy(), rtol=1e-9, atol=1e-9)
+    assert np.allclose(gh.cpu().numpy().ravel(), chk[2].cpu().numpy(), rtol=1e-9)
+    ctx.pt_fused(False)
+    try:
+        launches0 = ctx.kernel_launches()
+        ctx.pt_run(ux, ul, ud, uh, dev(tc, betas), dev(tc, lo), dev(tc, hi), 5, seed, 40, n_iter, n_accepted=acc_u)
+        assert ctx.kernel_launches() - launches0 == 8 * n_iter          # uniforms, 2 x (propose, H1-H3, accept), swaps
+    finally:
+        ctx.pt_fused(True)
+    assert tc.equal(ux, gx) and tc.equal(acc_u, acc_g)
+    assert np.allclose(ul.cpu().numpy(), gl.cpu().numpy(), rtol=1e-12, atol=1e-9)
+
+
+def test_pt_run_fused_module2_size(orc, torch_cuda):
+    """Module-2 size (10 temperatures x 400 walkers) on the config-1 recipe: the one-launch loop and the
+    multi-launch loop end at the same positions after 40 iterations; sampled log L against the oracle."""
+    tc = torch_cuda
+    wl = wlm.make_workload(1, n_w=4000, t_obs=2.0 ** 18, n_knots=128)
+    d, h0, h0e, summ = oracle_setup_het(orc, wl)
+    ctx = make_ctx(wl)
+    g = wl.grid
+    ctx.set_data(g.n_f, g.k_min, g.df, dev(tc, d), dev(tc, wl.W))
+    ctx.het_prepare(wl.f_edges, dev(tc, h0), dev(tc, h0e))
+    n_t, n_w = 10, 400
+    x = wl.params.reshape(n_t, n_w, -1).copy()
+    x[:, :, 5:] = wl.inj[5:]
+    betas = np.array([0.5 ** t for t in range(n_t - 1)] + [0.0])
+    lo, hi = _prior_box(wl, wl.params, 3.0)
+    gx = dev(tc, x)
+    out0 = ctx.het_batch_standin(gx.reshape(n_t * n_w, -1))
+    gl, gd, gh = (v.reshape(n_t, n_w).clone() for v in out0)
+    ux, ul, ud, uh = gx.clone(), gl.clone(), gd.clone(), gh.clone()
+    args = (dev(tc, betas), dev(tc, lo), dev(tc, hi), 5, 77, 0, 40)
+    acc_g = tc.zeros(n_t, dtype=tc.int64, device="cuda")
+    acc_u = tc.zeros(n_t, dtype=tc.int64, device="cuda")
+    ctx.pt_run(gx, gl, gd, gh, *args, n_accepted=acc_g)
+    ctx.pt_fused(False)
+    ctx.pt_run(ux, ul, ud, uh, *args, n_accepted=acc_u)
+    ctx.pt_fused(True)
+    assert tc.equal(ux, gx) and tc.equal(acc_u, acc_g) and int(acc_g.sum()) > 0.2 * 40 * n_t * n_w
+    assert not tc.equal(gx, dev(tc, x))
+    sample = np.r_[0:8, 1990:2010, 3990:4000]
+    rows = gx.reshape(n_t * n_w, -1).cpu().numpy()[sample]
+    ref = orc.het_batch_standin(wl.modes_m, wl.c_lm, wl.kappa, rows, wl.f_edges, h0e, summ)
+    got = gl.reshape(-1).cpu().numpy()[sample]
+    assert np.all(np.abs(got - ref["logL"]) <= 1e-6 * np.maximum(1.0, np.abs(ref["logL"])))
+    ctx.destroy()
+
+
 def test_module2_loop_with_reference_update(orc, torch_cuda):
     """The Module-2 loop in miniature: sample, update the reference to the best walker, re-evaluate
     the population against the new reference, sample on, read the stopping statistics — library calls only on one
