@@ -324,9 +324,20 @@ def bench_sampler_iteration(torch, ctx, wl, params, n_t: int = 10, n_w: int = 40
         st3 = ctx.pt_stats(logL[0], d_h[0], h_h[0], out3=out3).cpu()                        # synchronises
         stopped = binding.stop_converged(stop, float(st3[0])) or binding.stop_snr(float(st3[2]), float("inf"))
     ms_run = (time.perf_counter() - t0) * 1e3 / (blocks * per_block)
+    if f_nodes is None:
+        # the same loop as 8 launches per iteration (ll_pt_fused(0)), for comparison with the one-launch form above
+        ctx.pt_fused(False)
+        ctx.pt_run(x, logL, d_h, h_h, betas, lo, hi, 5, 2111, 5, 5)
+        torch.cuda.synchronize()
+        t1 = time.perf_counter()
+        ctx.pt_run(x, logL, d_h, h_h, betas, lo, hi, 5, 2111, 1000, per_block)
+        torch.cuda.synchronize()
+        res["ms_per_iteration_run_multi_launch"] = (time.perf_counter() - t1) * 1e3 / per_block
+        ctx.pt_fused(True)
     res.update({"ms_per_iteration_run": ms_run, "evals_per_s_run": n_t * n_w / (ms_run * 1e-3),
-                "run": "ll_pt_run_%s, %d blocks of %d iterations, stopping statistics read back after each (host wall time)"
-                       % ("het" if f_nodes is None else "full", blocks, per_block),
+                "run": "ll_pt_run_%s%s, %d blocks of %d iterations, stopping statistics read back after each (host wall time)"
+                       % ("het" if f_nodes is None else "full", " (one cooperative launch per block of iterations)" if f_nodes is None else "",
+                          blocks, per_block),
                 "acceptance_fraction_run": float(n_acc64.sum()) / (blocks * per_block * n_t * n_w), "stopped": bool(stopped)})
     return res
 

@@ -908,7 +908,7 @@ int pt_run_fused(ll_ctx *ctx, int32_t n_t, int32_t n_w, double *x, double *logL,
                  const double *lo, const double *hi, int32_t n_dim, double a, uint64_t seed, int64_t iter0, int64_t n_iter,
                  uint64_t *n_accepted, cudaStream_t st)
 {
-    constexpr int WY = LL_HET1_WY;
+    constexpr int WY = LL_PT_WY;
     if (ctx->coop < 0) {
         int v = 0;
         if (cudaDeviceGetAttribute(&v, cudaDevAttrCooperativeLaunch, ctx->device) != cudaSuccess) v = 0;

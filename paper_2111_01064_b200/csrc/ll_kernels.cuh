@@ -3042,14 +3042,19 @@ __device__ __forceinline__ double pt_uniform(unsigned long long seed, long long 
     return (double)(r >> 11) * 0x1.0p-53;
 }
 
+#ifndef LL_PT_WY
+#define LL_PT_WY 8 // warps (= edge segments) per block of the one-launch sampler: a pass of 32 proposals is bound by the FP64
+                   // issue rate of ONE SM, so more warps only add barrier and reduction cost (measured at Module-2 size,
+                   // half update: 16 warps 5.2 us, 8 warps 4.8 us)
+#endif
 template <int NC>
-__global__ void __launch_bounds__(32 * LL_HET1_WY, 1)
+__global__ void __launch_bounds__(32 * LL_PT_WY, 1)
 k_pt_run_het1(Het1Table T, StandinInfo si, PtRunArgs a)
 {
     constexpr int ST = het1_stride(NC);
     constexpr int NR = 3 * NC;
     constexpr int P = 5 + 2 * NC;
-    constexpr int S = LL_HET1_WY;
+    constexpr int S = LL_PT_WY;
     cooperative_groups::grid_group grid = cooperative_groups::this_grid();
     extern __shared__ __align__(16) double tab[];
     const int total = T.n_e * ST;
