@@ -275,6 +275,11 @@ typedef struct {
 int ll_stop_snr(double extracted_snr, double limit);
 int ll_stop_converged(ll_stop_state *s, double max_logL);
 
+/* Memory check (no part of the method): every internal device buffer has a canary-filled guard band behind it;
+ * this synchronises the device, reads the bands back and returns in *n_bad the number of buffers whose band was
+ * written (an out-of-bounds store by a kernel; ll_last_error names them).  HOST out.                          */
+int ll_debug_check(ll_ctx *ctx, int32_t *n_bad);
+
 /* Measurement helpers (no part of the method).
  * ll_peak_fma: runs `iters` dependent-free FMA chains on every SM and returns the achieved rate in
  *   FMA/s (HOST out); which = 0 -> FP64 DFMA (two loop-invariant register operands), 1 -> FP32 FFMA,

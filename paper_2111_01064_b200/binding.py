@@ -21,7 +21,7 @@ LL_BC_NATURAL, LL_BC_NOT_A_KNOT = 0, 1
 
 # every symbol include/ll.h declares (tests/test_abi.py checks header and library against this list)
 SYMBOLS = (
-    "ll_create", "ll_destroy", "ll_last_error", "ll_abi_version", "ll_set_data", "ll_get_dd", "ll_standin_config",
+    "ll_create", "ll_destroy", "ll_last_error", "ll_abi_version", "ll_debug_check", "ll_set_data", "ll_get_dd", "ll_standin_config",
     "ll_standin_split_tc",
     "ll_full_batch", "ll_full_batch_pw", "ll_full_batch_tf", "ll_tlm_nodes", "ll_standin_nodes", "ll_full_batch_standin", "ll_full_batch_standin_host",
     "ll_full_template_standin",
@@ -62,6 +62,7 @@ def load_library(path: Optional[str] = None):
         "ll_destroy": (C.c_int, [vp]),
         "ll_last_error": (C.c_char_p, [vp]),
         "ll_abi_version": (C.c_int, []),
+        "ll_debug_check": (C.c_int, [vp, C.POINTER(i32)]),
         "ll_set_data": (C.c_int, [vp, i64, i64, dbl, vp, vp, i32, vp]),
         "ll_standin_split_tc": (C.c_int, [vp, i32]),
         "ll_get_dd": (C.c_int, [vp, C.POINTER(dbl), C.POINTER(dbl), vp]),
@@ -192,6 +193,12 @@ class Context:
 
     def last_error(self) -> str:
         return (self._lib.ll_last_error(self._h) or b"").decode()
+
+    def debug_check(self) -> int:
+        """number of internal buffers whose guard band was written (out-of-bounds stores); 0 = clean"""
+        n = C.c_int32(-1)
+        self._check(self._lib.ll_debug_check(self._h, C.byref(n)), "ll_debug_check")
+        return int(n.value)
 
     def destroy(self):
         if getattr(self, "_h", None) is not None and self._h.value:

@@ -23,9 +23,22 @@ using namespace ll;
 
 namespace {
 
+// Every internal device buffer carries a guard band behind its capacity, filled with a canary byte when the block is
+// allocated; ll_debug_check() reads the bands back and reports the buffers whose band was written (an out-of-bounds
+// store by a kernel).  compute-sanitizer is closed on this pool, so this and the poisoned-stage build (LL_POISON_STAGES,
+// ll_kernels.cuh) are the memory checks the tests run.
+constexpr size_t kGuardBytes = 256;
+constexpr int kGuardByte = 0xA5;
 struct DevBuf {
     void *p = nullptr;
     size_t cap = 0;
+    cudaError_t alloc(size_t bytes)
+    {
+        cudaError_t e = cudaMalloc(&p, bytes + kGuardBytes);
+        if (e != cudaSuccess) { p = nullptr; return e; }
+        cap = bytes;
+        return cudaMemset((char *)p + cap, kGuardByte, kGuardBytes); // legacy stream: ordered before any later kernel
+    }
     cudaError_t ensure(size_t bytes)
     {
         if (bytes <= cap) return cudaSuccess;
@@ -35,17 +48,20 @@ struct DevBuf {
             cap = 0;
             if (e != cudaSuccess) return e;
         }
-        const size_t want = bytes + bytes / 8;
-        cudaError_t e = cudaMalloc(&p, want);
-        if (e != cudaSuccess) {
-            (void)cudaGetLastError();
-            e = cudaMalloc(&p, bytes);
-            if (e != cudaSuccess) { p = nullptr; return e; }
-            cap = bytes;
-            return cudaSuccess;
-        }
-        cap = want;
-        return cudaSuccess;
+        const size_t want = (bytes + bytes / 8 + 255) & ~(size_t)255;
+        if (alloc(want) == cudaSuccess) return cudaSuccess;
+        (void)cudaGetLastError();
+        return alloc((bytes + 255) & ~(size_t)255);
+    }
+    // 0: guard band intact (or nothing allocated), 1: written, -1: the read-back failed
+    int guard_state() const
+    {
+        if (!p) return 0;
+        unsigned char h[kGuardBytes];
+        if (cudaMemcpy(h, (const char *)p + cap, kGuardBytes, cudaMemcpyDeviceToHost) != cudaSuccess) return -1;
+        for (size_t i = 0; i < kGuardBytes; ++i)
+            if (h[i] != kGuardByte) return 1;
+        return 0;
     }
     void release()
     {
@@ -137,6 +153,17 @@ struct ll_ctx {
     std::vector<cudaEvent_t> ev; // pairs
     int ev_used = 0;             // pairs recorded since enable (ring)
 
+    std::vector<std::pair<const char *, DevBuf *>> buffers()
+    {
+#define LL_B(x) {#x, &x}
+        return {LL_B(g), LL_B(Wc), LL_B(dd_part), LL_B(dd), LL_B(pairs), LL_B(node_tab), LL_B(ilo_w), LL_B(ihi_w), LL_B(key_w),
+                LL_B(hist), LL_B(perm), LL_B(ilo_s), LL_B(ihi_s), LL_B(Y), LL_B(C), LL_B(TF), LL_B(part), LL_B(prow),
+                LL_B(het_tab), LL_B(het_tab1), LL_B(het_raw), LL_B(het_idx), LL_B(het_fb), LL_B(stage_in), LL_B(stage_out),
+                LL_B(g4f), LL_B(Wf), LL_B(scale), LL_B(wmax), LL_B(ref_idx), LL_B(ref_dense), LL_B(ref_edges),
+                LL_B(tiles[0].tab), LL_B(tiles[1].tab), LL_B(tiles[2].tab), LL_B(grp_tab), LL_B(part2), LL_B(pw_x), LL_B(pt_y),
+                LL_B(pt_out), LL_B(pt_in), LL_B(pt_u)};
+#undef LL_B
+    }
     int fail(int code, const std::string &msg)
     {
         err = msg;
@@ -995,12 +1022,7 @@ int ll_destroy(ll_ctx *ctx)
     {
         DeviceGuard dg(ctx->device);
         cudaDeviceSynchronize();
-        DevBuf *all[] = {&ctx->g, &ctx->Wc, &ctx->dd_part, &ctx->dd, &ctx->pairs, &ctx->node_tab, &ctx->ilo_w, &ctx->ihi_w,
-                         &ctx->key_w, &ctx->hist, &ctx->perm, &ctx->ilo_s, &ctx->ihi_s, &ctx->Y, &ctx->C, &ctx->TF,
-                         &ctx->part, &ctx->prow, &ctx->het_tab, &ctx->het_tab1, &ctx->het_raw, &ctx->het_idx, &ctx->het_fb,
-                         &ctx->stage_in, &ctx->stage_out, &ctx->g4f, &ctx->Wf, &ctx->scale, &ctx->wmax, &ctx->ref_idx,
-                         &ctx->ref_dense, &ctx->ref_edges, &ctx->tiles[0].tab, &ctx->tiles[1].tab, &ctx->tiles[2].tab, &ctx->grp_tab, &ctx->part2, &ctx->pw_x, &ctx->pt_y, &ctx->pt_out, &ctx->pt_in, &ctx->pt_u};
-        for (DevBuf *b : all) b->release();
+        for (auto &nb : ctx->buffers()) nb.second->release();
         for (auto &e : ctx->ev) cudaEventDestroy(e);
     }
     delete ctx;
@@ -1008,6 +1030,23 @@ int ll_destroy(ll_ctx *ctx)
 }
 
 const char *ll_last_error(const ll_ctx *ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+
+int ll_debug_check(ll_ctx *ctx, int32_t *n_bad)
+{
+    if (!ctx) return LL_ERR_ARG;
+    DeviceGuard dg(ctx->device);
+    CK(cudaDeviceSynchronize());
+    int bad = 0;
+    std::string names;
+    for (auto &nb : ctx->buffers()) {
+        const int st = nb.second->guard_state();
+        if (st < 0) return ctx->fail(LL_ERR_CUDA, "guard band read-back failed");
+        if (st > 0) { ++bad; names += std::string(names.empty() ? "" : ", ") + nb.first; }
+    }
+    if (n_bad) *n_bad = bad;
+    if (bad) ctx->err = "guard band written behind: " + names;
+    return LL_OK;
+}
 
 int64_t ll_kernel_launches(const ll_ctx *ctx) { return ctx ? ctx->launches : 0; }
 

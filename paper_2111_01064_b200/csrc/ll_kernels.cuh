@@ -887,6 +887,23 @@ struct Tile {
     }
 };
 
+// LL_POISON_STAGES (a test build; compute-sanitizer is closed on this pool): when a block has finished with a stage of
+// the ring, it overwrites the stage with NaNs before the barrier that frees it for the next bulk copy.  A thread that
+// read a stage before its copy had landed — a wrong mbarrier phase, a missing wait — would then see NaNs instead of the
+// previous tile's plausible numbers, and every parity test would fail.  The generic-proxy stores are ordered before
+// the async-proxy copy that refills the stage by fence.proxy.async.
+__device__ __forceinline__ void poison_stage(const double *stage, int n_doubles)
+{
+#ifdef LL_POISON_STAGES
+    __syncthreads(); // the other warps of the block may still be reading the stage
+    double *w = const_cast<double *>(stage);
+    for (int i = threadIdx.x; i < n_doubles; i += blockDim.x) w[i] = __longlong_as_double(0x7ff8000000000000LL);
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+#else
+    (void)stage; (void)n_doubles;
+#endif
+}
+
 // g of bin ii from a tile pointer that has been moved back by the tile's first bin (sgc = tile - cb * 2 NC)
 template <int NC>
 __device__ __forceinline__ void load_g(const double *__restrict__ sgc, int ii, double (&g)[2 * NC])
@@ -1257,6 +1274,7 @@ __global__ void __launch_bounds__(128, (NC == 2 && WS) ? LL_FUSED_MINB : 3) k_fu
             }
             i = seg_end;
         }
+        poison_stage(sg, CH * TL::DPB);
         __syncthreads(); // everyone is done with stage st before it is refilled two chunks later
     }
     constexpr int NQ = NM1 ? 2 * NC + Acc1<NC, WS>::NW : 2;
@@ -1509,6 +1527,7 @@ __global__ void __launch_bounds__(128, 4) k_full_fused_mixed(FusedArgs a, FusedA
             }
             i = seg_end;
         }
+        poison_stage(sg, CH * 3);
         __syncthreads();
     }
     double *o = a.part + ((size_t)tile * 5) * sw + p;
@@ -1703,6 +1722,7 @@ __global__ void __launch_bounds__(128, NC == 2 ? 3 : 2) k_full_fused_tf(FusedArg
             }
             i = seg_end;
         }
+        poison_stage(sg, CH * TL::DPB);
         __syncthreads();
     }
     double *o = a.part + ((size_t)tile * 2) * sw + p;
@@ -1974,6 +1994,7 @@ __global__ void __launch_bounds__(128, 3) k_full_fused_pw(FusedArgs a, const dou
                 ii += 1;
             }
         }
+        poison_stage(sg, CH * TL::DPB);
         __syncthreads();
     }
     double *o = a.part + ((size_t)tile * 2) * sw + p;

@@ -296,3 +296,10 @@ def test_unsupported_layouts_are_errors(torch_cuda):
         ctx.set_data(100, 10, 1e-5, tc.zeros((3, 100, 2), dtype=tc.float64, device="cuda"),
                      tc.ones((2, 100), dtype=tc.float64, device="cuda"))
     ctx.destroy()
+
+
+def test_memory_checks(torch_cuda):
+    """every kernel family once (both channel counts, small and large routes, the sampler in both forms), then the guard
+    bands behind every internal device buffer must be intact (ll_debug_check); outputs must be finite"""
+    from paper_2111_01064_b200 import sanitize_smoke
+    assert sanitize_smoke.main() == 0
