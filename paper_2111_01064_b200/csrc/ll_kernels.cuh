@@ -1300,6 +1300,14 @@ __global__ void __launch_bounds__(128, (NC == 2 && WS) ? LL_FUSED_MINB : 3) k_fu
 // so that every binary32 quantity is O(1): k_prescale_f32.
 // ---------------------------------------------------------------------------------------------------
 constexpr int kMixedChain = 8;
+#ifndef LL_MIXED_ROT
+#define LL_MIXED_ROT 0 // 1: the phase by the FP64 rotation recurrence, the rest in binary32 (fused_pairs_rot_mixed).  Measured at
+                       // config 2 (ncu r02, profiles/r02_full_fused_mixed_cfg2.md): 9.6 ms against 9.98 ms for the direct
+                       // binary32 sincos route and 10.8 ms for the FP64 kernel, FP64 pipe 50 % busy, XU pipe 40 % busy —
+                       // the three FP64 -> binary32 conversions per bin (cos, sin, W A^2 hand-off) run on the XU pipe at a
+                       // quarter of the FP64 rate and stall dispatch — and max |delta log L| 1.07e-3 against FP64, over
+                       // the 1e-3 bar.  Off: the variant cannot pay on this chip.
+#endif
 
 // scale[0] = sigma = 2^ceil(log2(max W)/2), scale[1] = 1/sigma, scale[2] = 1/sigma^2 (exact powers of two)
 __global__ void __launch_bounds__(256) k_wmax(const double *__restrict__ W, long long n_f, unsigned long long *__restrict__ wmax_bits)
@@ -1422,6 +1430,80 @@ __device__ __forceinline__ void fused_pairs_mixed(int b0, int b1, int kbase, dou
     }
 }
 
+// The same pairs with the phase advanced by the FP64 rotation recurrence of fused_bins_rot (z <- z w, w <- w v,
+// v <- v u: 12 FP64 instructions per bin, re-synchronised every kRotSync bins) and everything else in binary32:
+// the amplitude as its Taylor cubic around the re-sync point (the offset is at most 32 bins, so the binary32 rounding
+// is relative to A itself and not cumulative), A e^{-i Psi}, the MACs with the binary32 data tile and W A^2, two bins
+// per f32x2 instruction, partial sums of 8 terms per accumulator lane flushed into the FP64 accumulators.
+// The FP64 pipe carries 12 of the FP64 kernel's 27 instructions per bin.
+__device__ __forceinline__ void fused_pairs_rot_mixed(int b0, int b1, int kbase, double df, double nxj, double cA0, double cA1,
+                                                      double cA2, double cA3, double cP0, double cP1, double cP2, double cP3,
+                                                      const float *__restrict__ sgp, const double *__restrict__ sWc,
+                                                      MixedAcc &acc)
+{
+    const double df2 = df * df, df3 = df2 * df;
+    const float dff = __double2float_rn(df);
+    double su, cu;
+    sincos_qc(6.0 * cP3 * df3, su, cu);
+    unit_modulus(cu, su);
+    const f32x2 dS = pack2(2.0f * dff, 2.0f * dff), one2 = pack2(1.0f, 1.0f);
+    for (int k0 = b0; k0 < b1; k0 += kRotSync) {
+        const int k1 = min(k0 + kRotSync, b1);
+        const double t = fma((double)(kbase + k0), df, nxj);
+        const double tt = fma(2.0, t, df), q3 = fma(3.0 * t, t + df, df2), t1 = t + df;
+        // amplitude: Taylor coefficients at t, in binary32
+        const float a0 = __double2float_rn(fma(fma(fma(cA3, t, cA2), t, cA1), t, cA0));
+        const float a1 = __double2float_rn(fma(fma(3.0 * cA3, t, 2.0 * cA2), t, cA1));
+        const float a2 = __double2float_rn(fma(3.0 * cA3, t, cA2));
+        const float a3 = __double2float_rn(cA3);
+        const f32x2 A0 = pack2(a0, a0), A1 = pack2(a1, a1), A2 = pack2(a2, a2), A3 = pack2(a3, a3);
+        double sz, cz, sw, cw, sv, cv;
+        sincos_qc(fma(fma(fma(cP3, t, cP2), t, cP1), t, cP0), sz, cz);
+        sincos_qc(df * fma(cP3, q3, fma(cP2, tt, cP1)), sw, cw);
+        sincos_qc(df2 * fma(6.0 * cP3, t1, 2.0 * cP2), sv, cv);
+        unit_modulus(cz, sz);
+        unit_modulus(cw, sw);
+        unit_modulus(cv, sv);
+        f32x2 S = pack2(0.0f, dff); // offsets of the pair's two bins from the re-sync point
+        for (int base = k0; base < k1; base += 2 * kMixedChain) {
+            const int end = min(base + 2 * kMixedChain, k1);
+            f32x2 aXU = 0, aYV = 0, aYU = 0, aXV = 0, eXU = 0, eYV = 0, eYU = 0, eXV = 0; // +0.0f in both lanes
+#pragma unroll 2
+            for (int ii = base; ii < end; ii += 2) {
+                const float c0 = __double2float_rn(cz), s0 = __double2float_rn(sz);
+                double nzc = fma(cz, cw, -(sz * sw)), nzs = fma(sz, cw, cz * sw);
+                double nwc = fma(cw, cv, -(sw * sv)), nws = fma(sw, cv, cw * sv);
+                double nvc = fma(cv, cu, -(sv * su)), nvs = fma(sv, cu, cv * su);
+                cz = nzc; sz = nzs; cw = nwc; sw = nws; cv = nvc; sv = nvs;
+                const float c1 = __double2float_rn(cz), s1 = __double2float_rn(sz);
+                nzc = fma(cz, cw, -(sz * sw)); nzs = fma(sz, cw, cz * sw);
+                nwc = fma(cw, cv, -(sw * sv)); nws = fma(sw, cv, cw * sv);
+                nvc = fma(cv, cu, -(sv * su)); nvs = fma(sv, cu, cv * su);
+                cz = nzc; sz = nzs; cw = nwc; sw = nws; cv = nvc; sv = nvs;
+                const f32x2 Af = fma2(fma2(fma2(A3, S, A2), S, A1), S, A0);
+                S = fma2(dS, one2, S);
+                const f32x2 U = mul2(Af, pack2(c0, c1)), V = mul2(Af, pack2(s0, s1)); // h = u - i v per lane
+                const ulonglong2 gA = *reinterpret_cast<const ulonglong2 *>(sgp + (ii >> 1) * 8);
+                const ulonglong2 gE = *reinterpret_cast<const ulonglong2 *>(sgp + (ii >> 1) * 8 + 4);
+                aXU = fma2(gA.x, U, aXU); aYV = fma2(gA.y, V, aYV); aYU = fma2(gA.y, U, aYU); aXV = fma2(gA.x, V, aXV);
+                eXU = fma2(gE.x, U, eXU); eYV = fma2(gE.y, V, eYV); eYU = fma2(gE.y, U, eYU); eXV = fma2(gE.x, V, eXV);
+                // <h|h> = sum W A^2 stays in FP64 (all terms positive: binary32 sums lose ~1e-8 of 2.5e5, reading R15)
+                const double2 w = *reinterpret_cast<const double2 *>(sWc + ii);
+                float al, ah;
+                unpack2(Af, al, ah);
+                const double ald = (double)al, ahd = (double)ah;
+                acc.sH = fma(w.x * ald, ald, acc.sH);
+                acc.sH = fma(w.y * ahd, ahd, acc.sH);
+            }
+            float l0, h0, l1, h1;
+            unpack2(aXU, l0, h0); unpack2(aYV, l1, h1); acc.sAr += (double)((l0 + h0) + (l1 + h1));
+            unpack2(aYU, l0, h0); unpack2(aXV, l1, h1); acc.sAi += (double)((l0 + h0) - (l1 + h1));
+            unpack2(eXU, l0, h0); unpack2(eYV, l1, h1); acc.sEr += (double)((l0 + h0) + (l1 + h1));
+            unpack2(eYU, l0, h0); unpack2(eXV, l1, h1); acc.sEi += (double)((l0 + h0) - (l1 + h1));
+        }
+    }
+}
+
 struct FusedArgsF32 {
     const float *g4f;   // [n_f_pad][4] binary32, g / sigma
     const double *Wds;  // [n_f_pad] FP64, W / sigma^2
@@ -1517,7 +1599,10 @@ __global__ void __launch_bounds__(128, 4) k_full_fused_mixed(FusedArgs a, FusedA
                 if (plo < phi) {
                     fused_bins_mixed<true>(wlo, plo, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1,
                                            cP2, cP3, sgp, sWc, acc);
-                    fused_pairs_mixed(plo, phi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1, cP2, cP3, sgp, sWc, acc);
+                    if (LL_MIXED_ROT && phi - plo >= 16)
+                        fused_pairs_rot_mixed(plo, phi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1, cP2, cP3, sgp, sWc, acc);
+                    else
+                        fused_pairs_mixed(plo, phi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1, cP2, cP3, sgp, sWc, acc);
                     fused_bins_mixed<true>(phi, whi, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1,
                                            cP2, cP3, sgp, sWc, acc);
                 } else {
