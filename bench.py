@@ -37,13 +37,13 @@ UNIT = "evals/s"
 # two complex MACs 8, W A^2 2 => 39.  The single-mode FP64 kernels advance e^{-i Psi} and A by recurrence, and
 # SURVEY §8(d) asks that such a build quote ITS count: 12 (three rotations) + 3 (amplitude differences) + 2 (A z) +
 # 4 n_c (MACs) + 2 (W A^2; 1 + n_c with per-channel weights) => 27 for two channels sharing a weight row, 33 for
-# three channels with their own rows.  `frac` uses these.  The re-synchronisation every 32 bins (2 cubics 6 +
-# differences 16 + 3 sincos 54 + 3 normalisations 15 + 1 = 92 slots / 32 bins = 2.9) is the builder's tuning choice,
-# not algorithmic work: `frac_with_resync` adds it and is reported beside `frac`, never instead of it.
+# three channels with their own rows.  `frac` uses these.  The re-synchronisation every 128 bins (2 cubics 6 +
+# differences 16 + 3 degree-7 sincos 57 + 3 normalisations 15 + 1 = 95 slots / 128 bins = 0.74) is the builder's tuning
+# choice, not algorithmic work: `frac_with_resync` adds it and is reported beside `frac`, never instead of it.
 SLOTS_FULL_DIRECT = 39.0
 SLOTS_FULL = 27.0
 SLOTS_FULL_NC3 = 33.0
-SLOTS_RESYNC = 2.9
+SLOTS_RESYNC = 0.74
 # per-walker node grids: the recurrence route with T^c applied per bin (it accumulates <d|h>, <h|h> directly):
 # 12 + 3 + 2 + T^c h 8 + Re g h 4 + W |h|^2 5 = 34 per bin (+ re-sync with four sincos: 3.6)
 SLOTS_FULL_PW = 34.0
@@ -523,7 +523,7 @@ def config_roofline(wl, ctx, kernel_ms: float, peak_slots: float):
         if wl.n_m == 1:
             slots = SLOTS_FULL if wl.n_c == 2 else SLOTS_FULL_NC3
             out = {"kernel": "k_full_fused<1, %d, %s>" % (wl.n_c, "true" if wl.n_c == 2 else "false"), "slots_per_unit": slots,
-                   "formulation": "rotation recurrence (SURVEY §8(d): ~27 for two channels), re-synchronised every 32 bins; "
+                   "formulation": "rotation recurrence (SURVEY §8(d): ~27 for two channels), re-synchronised every 128 bins; "
                                   "the direct formulation needs %g" % SLOTS_FULL_DIRECT,
                    "frac_with_resync": units * (slots + SLOTS_RESYNC) / (kernel_ms * 1e-3) / peak_slots}
         else:

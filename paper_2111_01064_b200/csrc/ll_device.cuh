@@ -45,6 +45,29 @@ __device__ __forceinline__ void sincos_poly_qc(double r, double &s, double &c)
     c = pc;
 }
 
+// The same functions to the rounding of the arithmetic (degree 7 in r^2: max error 3.4e-17 (sin), 1.5e-17 (cos), and
+// C(0) = 1 exactly), for the few evaluations per re-synchronisation of the rotation recurrence whose error is
+// AMPLIFIED: a phase error delta in the per-bin rotation w = e^{i D1 Psi} becomes k delta in z after k bins, and
+// because D1 Psi drifts slowly the degree-5 polynomial's error (5.6e-14 in cos) has the same sign over thousands of
+// consecutive blocks — it was what made the distance from the oracle grow like the re-sync length squared.
+__constant__ double kSinA[8] = {0x1.921fb54442d18p+0, -0x1.4abbce625be53p-1, 0x1.466bc6775aad9p-4, -0x1.32d2cce62ac22p-8,
+                                0x1.50783485cbd83p-13, -0x1.e3074b4ff3058p-19, 0x1.e8eed12ee00a3p-25, -0x1.6c5b875d4e739p-31};
+__constant__ double kCosA[8] = {0x1.0000000000000p+0, -0x1.3bd3cc9be45dep+0, 0x1.03c1f081b5aacp-2, -0x1.55d3c7e3c90f8p-6,
+                                0x1.e1f5068355e15p-11, -0x1.a6d1ec7906c20p-16, 0x1.f9cc41140bb60p-22, -0x1.b264ba152378ap-28};
+__device__ __forceinline__ void sincos_poly_qc_acc(double r, double &s, double &c)
+{
+    const double r2 = r * r;
+    double ps = fma(kSinA[7], r2, kSinA[6]);
+    double pc = fma(kCosA[7], r2, kCosA[6]);
+#pragma unroll
+    for (int k = 5; k >= 0; --k) {
+        ps = fma(ps, r2, kSinA[k]);
+        pc = fma(pc, r2, kCosA[k]);
+    }
+    s = ps * r;
+    c = pc;
+}
+
 // quadrant bookkeeping: angle = (pi/2)(n + r); q = n mod 4.  Integer-pipe only (selects and sign-bit XORs on
 // the high words), so it costs no FP64 issue slot.
 __device__ __forceinline__ double flip_sign_if(double x, unsigned mask /* 0 or 0x80000000 */)
@@ -82,6 +105,17 @@ __device__ __forceinline__ void sincos_qc(double y, double &sn, double &cs)
     const double r = __dadd_rn(y, -nd);
     double s, c;
     sincos_poly_qc(r, s, c);
+    quadrant_fix(q, s, c, sn, cs);
+}
+// the same with the degree-7 polynomials (re-synchronisation of the rotation recurrence)
+__device__ __forceinline__ void sincos_qc_acc(double y, double &sn, double &cs)
+{
+    const double sh = __dadd_rn(y, kMagic);
+    const int q = __double2loint(sh);
+    const double nd = __dadd_rn(sh, -kMagic);
+    const double r = __dadd_rn(y, -nd);
+    double s, c;
+    sincos_poly_qc_acc(r, s, c);
     quadrant_fix(q, s, c, sn, cs);
 }
 // u - i v = amp * exp(-i (pi/2) y)

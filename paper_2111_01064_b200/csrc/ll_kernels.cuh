@@ -1034,9 +1034,9 @@ __device__ __forceinline__ void fused_bins_nm1(int b0, int b1, int tlo, int thi,
 // grid the phase cubic has constant third differences, so e^{-i Psi_k} advances by three complex rotations per bin,
 //   z_{k+1} = z_k w_k,  w_{k+1} = w_k v_k,  v_{k+1} = v_k u,   w = e^{i D1 Psi}, v = e^{i D2 Psi}, u = e^{i D3 Psi},
 // and the amplitude cubic by its forward differences; every kRotSync bins everything is re-evaluated from the cubic
-// coefficients (the exact route above), which bounds the accumulated rounding: with D1 Psi <= a few quarter cycles
-// known to 1 ulp, the phase drifts by < kRotSync^2/2 ulp ~ 1e-13 quarter cycles between re-syncs, far below the
-// rounding of Psi itself (1e-9 at 1e7 quarter cycles).  Per bin: 12 (rotations) + 3 (amplitude) + 2 (A z) + 4 NC
+// coefficients, which bounds the accumulated rounding: with D1 Psi <= a few quarter cycles known to 1 ulp, the phase
+// drifts by < kRotSync^2/2 ulp ~ 1e-12 quarter cycles between re-syncs, far below the rounding of Psi itself (1e-9 at
+// 1e7 quarter cycles) — PROVIDED the rotations w, v, u themselves carry no systematic error (LL_ROT_ACC, ll_device.cuh).  Per bin: 12 (rotations) + 3 (amplitude) + 2 (A z) + 4 NC
 // (MACs) + 2 (W A^2; 1 + NC with per-channel weights) = 27 FP64 instructions for two channels and a shared weight row
 // (33 for three channels with their own rows), no sincos, no quadrant fix-up, no bin-number conversion, instead of
 // 34 + 18 others.
@@ -1044,11 +1044,24 @@ __device__ __forceinline__ void fused_bins_nm1(int b0, int b1, int tlo, int thi,
 #define LL_FUSED_ROT 1
 #endif
 #ifndef LL_ROT_SYNC
-#define LL_ROT_SYNC 32 // measured at config 2 (max |error of <d|h>| over sampled walkers, kernel time): 32: 8e-8, 10.7 ms
-                       // (the exact route: 7e-8, 13.0 ms); 64: 3e-7, 10.2 ms; 128: 2e-6, 10.0 ms; 256: 1.3e-5, 9.9 ms
+#define LL_ROT_SYNC 128 // bins between re-synchronisations.  Measured at config 2 (max |<d|h> - oracle| over 25 sampled
+                        // walkers at <d|h> up to 2.5e5; kernel time).  Round 1, rotations from the degree-5 polynomials:
+                        // 32: 8e-8, 10.7 ms; 64: 3e-7; 128: 2e-6; 256: 1.3e-5 — the error grew like the length squared
+                        // because the polynomial's phase error in w is amplified k-fold in z and has the same sign over
+                        // thousands of blocks.  Round 2, rotations from the degree-7 polynomials (LL_ROT_ACC): 32: 9e-8,
+                        // 10.9 ms; 64: 1.1e-7, 10.35; 128: 1.3e-7, 10.09 (chosen; noiseless log L at the truth -1.6e-8);
+                        // 256: 1.2e-7, 9.96 (noiseless -8.7e-8).  The exact route: 7e-8, 13.0 ms.
 #endif
 #ifndef LL_ROT_UNROLL
 #define LL_ROT_UNROLL 2
+#endif
+#ifndef LL_ROT_ACC
+#define LL_ROT_ACC 1 // the rotations of a re-synchronisation from the degree-7 polynomials (ll_device.cuh)
+#endif
+#if LL_ROT_ACC
+#define LL_ROT_SINCOS sincos_qc_acc
+#else
+#define LL_ROT_SINCOS sincos_qc
 #endif
 constexpr int kRotSync = LL_ROT_SYNC;
 constexpr int kRotUnroll = LL_ROT_UNROLL;
@@ -1073,7 +1086,7 @@ __device__ __forceinline__ void fused_bins_rot(int b0, int b1, int tlo, int thi,
     const double df2 = df * df, df3 = df2 * df;
     const double d3A = 6.0 * cA3 * df3;
     double su, cu;
-    sincos_qc(6.0 * cP3 * df3, su, cu);
+    LL_ROT_SINCOS(6.0 * cP3 * df3, su, cu);
     unit_modulus(cu, su);
     for (int k0 = b0; k0 < b1; k0 += kRotSync) {
         const int k1 = min(k0 + kRotSync, b1);
@@ -1084,9 +1097,9 @@ __device__ __forceinline__ void fused_bins_rot(int b0, int b1, int tlo, int thi,
         double d1A = df * fma(cA3, q3, fma(cA2, tt, cA1));
         double d2A = df2 * fma(6.0 * cA3, t1, 2.0 * cA2);
         double sz, cz, sw, cw, sv, cv;
-        sincos_qc(fma(fma(fma(cP3, t, cP2), t, cP1), t, cP0), sz, cz);
-        sincos_qc(df * fma(cP3, q3, fma(cP2, tt, cP1)), sw, cw);
-        sincos_qc(df2 * fma(6.0 * cP3, t1, 2.0 * cP2), sv, cv);
+        LL_ROT_SINCOS(fma(fma(fma(cP3, t, cP2), t, cP1), t, cP0), sz, cz);
+        LL_ROT_SINCOS(df * fma(cP3, q3, fma(cP2, tt, cP1)), sw, cw);
+        LL_ROT_SINCOS(df2 * fma(6.0 * cP3, t1, 2.0 * cP2), sv, cv);
         unit_modulus(cz, sz);
         unit_modulus(cw, sw);
         unit_modulus(cv, sv);
@@ -1444,7 +1457,7 @@ __device__ __forceinline__ void fused_pairs_rot_mixed(int b0, int b1, int kbase,
     const double df2 = df * df, df3 = df2 * df;
     const float dff = __double2float_rn(df);
     double su, cu;
-    sincos_qc(6.0 * cP3 * df3, su, cu);
+    LL_ROT_SINCOS(6.0 * cP3 * df3, su, cu);
     unit_modulus(cu, su);
     const f32x2 dS = pack2(2.0f * dff, 2.0f * dff), one2 = pack2(1.0f, 1.0f);
     for (int k0 = b0; k0 < b1; k0 += kRotSync) {
@@ -1458,9 +1471,9 @@ __device__ __forceinline__ void fused_pairs_rot_mixed(int b0, int b1, int kbase,
         const float a3 = __double2float_rn(cA3);
         const f32x2 A0 = pack2(a0, a0), A1 = pack2(a1, a1), A2 = pack2(a2, a2), A3 = pack2(a3, a3);
         double sz, cz, sw, cw, sv, cv;
-        sincos_qc(fma(fma(fma(cP3, t, cP2), t, cP1), t, cP0), sz, cz);
-        sincos_qc(df * fma(cP3, q3, fma(cP2, tt, cP1)), sw, cw);
-        sincos_qc(df2 * fma(6.0 * cP3, t1, 2.0 * cP2), sv, cv);
+        LL_ROT_SINCOS(fma(fma(fma(cP3, t, cP2), t, cP1), t, cP0), sz, cz);
+        LL_ROT_SINCOS(df * fma(cP3, q3, fma(cP2, tt, cP1)), sw, cw);
+        LL_ROT_SINCOS(df2 * fma(6.0 * cP3, t1, 2.0 * cP2), sv, cv);
         unit_modulus(cz, sz);
         unit_modulus(cw, sw);
         unit_modulus(cv, sv);
@@ -1767,7 +1780,7 @@ __global__ void __launch_bounds__(128, NC == 2 ? 3 : 2) k_full_fused_tf(FusedArg
                     const double df = a.df, df2 = df * df, df3 = df2 * df;
                     const double d3A = 6.0 * co[3] * df3;
                     double su, cu;
-                    sincos_qc(6.0 * co[7] * df3, su, cu);
+                    LL_ROT_SINCOS(6.0 * co[7] * df3, su, cu);
                     unit_modulus(cu, su);
                     for (int k0 = flo; k0 < fhi; k0 += kRotSync) {
                         const int k1 = min(k0 + kRotSync, fhi);
@@ -1777,9 +1790,9 @@ __global__ void __launch_bounds__(128, NC == 2 ? 3 : 2) k_full_fused_tf(FusedArg
                         double d1A = df * fma(co[3], q3, fma(co[2], tt, co[1]));
                         double d2A = df2 * fma(6.0 * co[3], t1, 2.0 * co[2]);
                         double sz, cz, sw_, cw, sv, cv;
-                        sincos_qc(cubic4(co + 4, t0), sz, cz);
-                        sincos_qc(df * fma(co[7], q3, fma(co[6], tt, co[5])), sw_, cw);
-                        sincos_qc(df2 * fma(6.0 * co[7], t1, 2.0 * co[6]), sv, cv);
+                        LL_ROT_SINCOS(cubic4(co + 4, t0), sz, cz);
+                        LL_ROT_SINCOS(df * fma(co[7], q3, fma(co[6], tt, co[5])), sw_, cw);
+                        LL_ROT_SINCOS(df2 * fma(6.0 * co[7], t1, 2.0 * co[6]), sv, cv);
                         unit_modulus(cz, sz); unit_modulus(cw, sw_); unit_modulus(cv, sv);
 #pragma unroll 2
                         for (int ii = k0; ii < k1; ++ii) {
@@ -2052,10 +2065,10 @@ __global__ void __launch_bounds__(128, 3) k_full_fused_pw(FusedArgs a, const dou
                 double d2A = df2 * fma(6.0 * co[3], t1, 2.0 * co[2]);
                 const double d3A = 6.0 * co[3] * df3;
                 double sz, cz, sw_, cw, sv, cv, su, cu;
-                sincos_qc(cubic4(co + 4, t), sz, cz);
-                sincos_qc(df * fma(co[7], q3, fma(co[6], tt, co[5])), sw_, cw);
-                sincos_qc(df2 * fma(6.0 * co[7], t1, 2.0 * co[6]), sv, cv);
-                sincos_qc(6.0 * co[7] * df3, su, cu);
+                LL_ROT_SINCOS(cubic4(co + 4, t), sz, cz);
+                LL_ROT_SINCOS(df * fma(co[7], q3, fma(co[6], tt, co[5])), sw_, cw);
+                LL_ROT_SINCOS(df2 * fma(6.0 * co[7], t1, 2.0 * co[6]), sv, cv);
+                LL_ROT_SINCOS(6.0 * co[7] * df3, su, cu);
                 unit_modulus(cz, sz); unit_modulus(cw, sw_); unit_modulus(cv, sv); unit_modulus(cu, su);
 #pragma unroll 2
                 for (int k = 0; k < m; ++k) {
