@@ -118,6 +118,7 @@ struct ll_ctx {
     DevBuf grp_tab;                // small batches: work items per group of 32 walkers (k_band_sort_small)
     DevBuf pw_x;                   // per-walker node grids: X [n_nodes][n_wp], then the effective bands [n_w][2]
     DevBuf node_tab; // doubles then ints
+    DevBuf wmom;     // [7][n_f_pad] prefix moments of the shared weight row inside the intervals of the current node set
     NodeTables nt{};
 
     // full-grid scratch
@@ -160,7 +161,7 @@ struct ll_ctx {
                 LL_B(hist), LL_B(perm), LL_B(ilo_s), LL_B(ihi_s), LL_B(Y), LL_B(C), LL_B(TF), LL_B(part), LL_B(prow),
                 LL_B(het_tab), LL_B(het_tab1), LL_B(het_raw), LL_B(het_idx), LL_B(het_fb), LL_B(stage_in), LL_B(stage_out),
                 LL_B(g4f), LL_B(Wf), LL_B(scale), LL_B(wmax), LL_B(ref_idx), LL_B(ref_dense), LL_B(ref_edges),
-                LL_B(tiles[0].tab), LL_B(tiles[1].tab), LL_B(tiles[2].tab), LL_B(grp_tab), LL_B(part2), LL_B(pw_x), LL_B(pt_y),
+                LL_B(tiles[0].tab), LL_B(tiles[1].tab), LL_B(tiles[2].tab), LL_B(grp_tab), LL_B(wmom), LL_B(part2), LL_B(pw_x), LL_B(pt_y),
                 LL_B(pt_out), LL_B(pt_in), LL_B(pt_u)};
 #undef LL_B
     }
@@ -332,6 +333,12 @@ int prepare_nodes(ll_ctx *ctx, int n, const double *x, cudaStream_t st)
     ctx->nodes_host.assign(x, x + n);
     ctx->bstart_host = hi;
     ctx->nodes_version += 1;
+    if (ctx->w_rows == 1 && ctx->precision == LL_PREC_FP64) { // <h|h> by weight moments: single-mode kernel, shared weight row
+        CK(ctx->wmom.ensure(sizeof(double) * 7 * (size_t)ctx->n_f_pad));
+        k_w_moments<<<n - 1, 256, 0, st>>>(ctx->Wc.as<double>(), nt.bstart, nt.xj, n, ctx->k_min, ctx->df, ctx->n_f_pad,
+                                           ctx->wmom.as<double>());
+        LAUNCHED(ctx);
+    }
     ctx->nodes_valid = true;
     return LL_OK;
 }
@@ -473,6 +480,7 @@ FusedArgs fused_args(ll_ctx *ctx, const FullPlan &pl, int n_nodes, const double 
     fa.n_f = (int)ctx->n_f; fa.n_wp = pl.n_wp; fa.n_nodes = n_nodes; fa.n_m = ctx->n_m; fa.TB = pl.TB; fa.CH = pl.CH;
     fa.tile_start = ctx->tile_cur ? ctx->tile_cur->tab.as<int>() : nullptr;
     fa.grp_tab = ctx->grp_tab.as<int>();
+    fa.wmom = (ctx->w_rows == 1 && ctx->precision == LL_PREC_FP64 && ctx->n_m == 1) ? ctx->wmom.as<double>() : nullptr;
     return fa;
 }
 

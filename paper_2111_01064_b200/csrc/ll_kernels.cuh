@@ -828,6 +828,62 @@ k_spline_block(const double *__restrict__ Y, double *__restrict__ C, int n_wp, i
 // Single-mode specialisation: T^c is constant per walker, so the kernel accumulates the complex sums
 // S^c = sum_i g^c_i A e^{-i Psi} and H = sum_i W_i A^2; k_finalize applies T^c.
 // ---------------------------------------------------------------------------------------------------
+// Prefix moments of the (shared) weight row inside each spline interval, for the single-mode kernel's <h|h>:
+// inside an interval A(t) is a cubic in t = f - x_j, so sum_k W_k A(t_k)^2 over any stretch of its bins is
+// sum_{p=0..6} q_p M_p with q = the coefficients of A^2 and M_p = sum_k W_k t_k^p — walker-independent sums.
+//   wmom[p][i] = sum over the bins k of bin i's interval, k <= i, of W_k t_k^p          (inclusive prefix)
+// so M_p of a stretch [b0, b1) of one interval is wmom[p][b1 - 1] - wmom[p][b0 - 1] (the second term absent when b0 is
+// the interval's first bin).  One block per interval; t exactly as the fused kernel forms it.  Rebuilt when the node
+// set or the data change.  A prefix over an interval of n bins carries ~sqrt(n) ulp, the difference of two of them the
+// same absolutely: 1e-15 relative to a stretch a fortieth of its interval — the 1e-12 the log L = 0 test needs is far.
+__global__ void __launch_bounds__(256)
+k_w_moments(const double *__restrict__ Wc, const int *__restrict__ bstart, const double *__restrict__ xj, int n_nodes,
+            long long k_min, double df, long long n_f_pad, double *__restrict__ wmom)
+{
+    __shared__ double wtot[8][7];
+    const int j = blockIdx.x;
+    const int i0 = bstart[j], i1 = bstart[j + 1];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const double nx = -xj[j];
+    double carry[7];
+#pragma unroll
+    for (int p = 0; p < 7; ++p) carry[p] = 0.0;
+    for (int base = i0; base < i1; base += 256) {
+        const int i = base + threadIdx.x;
+        double v[7];
+        {
+            const double t = fma((double)(k_min + i), df, nx);
+            double w = (i < i1) ? Wc[i] : 0.0;
+#pragma unroll
+            for (int p = 0; p < 7; ++p) { v[p] = w; w *= t; }
+        }
+#pragma unroll
+        for (int p = 0; p < 7; ++p) { // inclusive scan inside the warp
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const double u = __shfl_up_sync(0xffffffffu, v[p], o);
+                if (lane >= o) v[p] += u;
+            }
+        }
+        if (lane == 31) {
+#pragma unroll
+            for (int p = 0; p < 7; ++p) wtot[wid][p] = v[p];
+        }
+        __syncthreads();
+#pragma unroll
+        for (int p = 0; p < 7; ++p) {
+            double pre = carry[p], tot = carry[p];
+            for (int k = 0; k < 8; ++k) {
+                if (k < wid) pre += wtot[k][p];
+                tot += wtot[k][p];
+            }
+            if (i < i1) wmom[(size_t)p * n_f_pad + i] = pre + v[p];
+            carry[p] = tot;
+        }
+        __syncthreads();
+    }
+}
+
 struct FusedArgs {
     const double *g;       // [n_f_pad][2 NC]
     const double *Wc;      // [NW][n_f_pad]
@@ -846,6 +902,7 @@ struct FusedArgs {
     double df;
     const int *tile_start; // [n_tiles + 1]: frequency tile t covers dense bins [tile_start[t], tile_start[t+1])
     const int *grp_tab;    // small batches (k_full_fused<.., SMALL = 1>): work dealt out by active bins, see k_band_sort_small
+    const double *wmom;    // [7][n_f_pad] prefix moments of the shared weight row inside each spline interval (k_w_moments), or null
     int n_f, n_wp, n_nodes, n_m, TB, CH;
 };
 
@@ -934,7 +991,8 @@ struct Acc1 {
 #pragma unroll
         for (int q = 0; q < NW; ++q) H[q] = 0.0;
     }
-    // h = u - i v = A e^{-i Psi} at bin ii
+    // h = u - i v = A e^{-i Psi} at bin ii; WITH_H = false: the stretch's sum of W A^2 comes from the weight moments
+    template <bool WITH_H = true>
     __device__ __forceinline__ void add(const double *__restrict__ sgc, const double *__restrict__ sWc, int CH, int ii,
                                         double u, double v, double A)
     {
@@ -945,6 +1003,7 @@ struct Acc1 {
             S[2 * c] = fma(g[2 * c], u, S[2 * c]); S[2 * c] = fma(g[2 * c + 1], v, S[2 * c]);
             S[2 * c + 1] = fma(g[2 * c + 1], u, S[2 * c + 1]); S[2 * c + 1] = fma(-g[2 * c], v, S[2 * c + 1]);
         }
+        if (!WITH_H) return;
         if (WS) {
             H[0] = fma(sWc[ii] * A, A, H[0]);
         } else {
@@ -1043,6 +1102,9 @@ __device__ __forceinline__ void fused_bins_nm1(int b0, int b1, int tlo, int thi,
 #ifndef LL_FUSED_ROT
 #define LL_FUSED_ROT 1
 #endif
+#ifndef LL_H_MOMENTS
+#define LL_H_MOMENTS 1 // <h|h> of an unmasked recurrence stretch from prefix moments of the weights (k_w_moments)
+#endif
 #ifndef LL_ROT_SYNC
 #define LL_ROT_SYNC 128 // bins between re-synchronisations.  Measured at config 2 (max |<d|h> - oracle| over 25 sampled
                         // walkers at <d|h> up to 2.5e5; kernel time).  Round 1, rotations from the degree-5 polynomials:
@@ -1077,7 +1139,7 @@ __device__ __forceinline__ void unit_modulus(double &c, double &s)
 }
 // MASK: lanes outside their own band [tlo, thi) ride along with amplitude 0 (the ragged end of a warp's band: a
 // few bins in a large sorted batch, but a third of all bins when a whole batch is only a handful of warps).
-template <bool MASK, int NC, bool WS>
+template <bool MASK, int NC, bool WS, bool WITH_H = true>
 __device__ __forceinline__ void fused_bins_rot(int b0, int b1, int tlo, int thi, int kbase, double df, double nxj, double cA0,
                                                double cA1, double cA2, double cA3, double cP0, double cP1, double cP2,
                                                double cP3, const double *__restrict__ sgc, const double *__restrict__ sWc,
@@ -1107,7 +1169,7 @@ __device__ __forceinline__ void fused_bins_rot(int b0, int b1, int tlo, int thi,
         for (int ii = k0; ii < k1; ++ii) {
             const double Am = (!MASK || ((ii >= tlo) && (ii < thi))) ? A : 0.0;
             const double u = Am * cz, v = Am * sz; // h = u - i v
-            acc.add(sgc, sWc, CH, ii, u, v, Am);
+            acc.template add<WITH_H>(sgc, sWc, CH, ii, u, v, Am);
             const double nzc = fma(cz, cw, -(sz * sw)), nzs = fma(sz, cw, cz * sw);
             const double nwc = fma(cw, cv, -(sw * sv)), nws = fma(sw, cv, cw * sv);
             const double nvc = fma(cv, cu, -(sv * su)), nvs = fma(sv, cu, cv * su);
@@ -1231,10 +1293,32 @@ __global__ void __launch_bounds__(128, (NC == 2 && WS) ? LL_FUSED_MINB : 3) k_fu
                     };
                     if (flo < fhi) {
                         masked(wlo, flo);
-                        if (LL_FUSED_ROT && fhi - flo >= 8)
-                            fused_bins_rot<false, NC, WS>(flo, fhi, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1, cP2,
-                                                          cP3, sgc, sWc, CH, acc);
-                        else
+                        if (LL_FUSED_ROT && fhi - flo >= 8) {
+                            if (WS && LL_H_MOMENTS && a.wmom) {
+                                // sum_k W_k A(t_k)^2 over the stretch from the weight moments (two of the 27 slots per bin):
+                                // A^2 = sum_p q_p t^p, M_p = sum_k W_k t_k^p = difference of two prefix entries
+                                double mo[7];
+                                const bool first = flo == __ldg(a.bstart + j);
+#pragma unroll
+                                for (int q = 0; q < 7; ++q) {
+                                    const double *Q = a.wmom + (size_t)q * a.n_f_pad;
+                                    mo[q] = __ldg(Q + fhi - 1) - (first ? 0.0 : __ldg(Q + flo - 1));
+                                }
+                                fused_bins_rot<false, NC, WS, false>(flo, fhi, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0,
+                                                                     cP1, cP2, cP3, sgc, sWc, CH, acc);
+                                double hs = (cA0 * cA0) * mo[0];
+                                hs = fma(2.0 * cA0 * cA1, mo[1], hs);
+                                hs = fma(fma(2.0 * cA0, cA2, cA1 * cA1), mo[2], hs);
+                                hs = fma(2.0 * fma(cA0, cA3, cA1 * cA2), mo[3], hs);
+                                hs = fma(fma(2.0 * cA1, cA3, cA2 * cA2), mo[4], hs);
+                                hs = fma(2.0 * cA2 * cA3, mo[5], hs);
+                                hs = fma(cA3 * cA3, mo[6], hs);
+                                acc.H[0] += hs;
+                            } else {
+                                fused_bins_rot<false, NC, WS>(flo, fhi, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1,
+                                                              cP2, cP3, sgc, sWc, CH, acc);
+                            }
+                        } else
                             fused_bins_nm1<false, NC, WS>(flo, fhi, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1,
                                                           cP2, cP3, sgc, sWc, CH, acc);
                         masked(fhi, whi);
