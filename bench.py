@@ -632,7 +632,10 @@ def main():
                 "fp64_slots_per_pair": 13.0, "fp64_pipe_frac": pairs * 13.0 / (k_ms * 1e-3) / peak_slots, **common}
         else:
             rf = config_roofline(wl, ctx, k_ms, peak_slots)
-            traffic, traffic_src = ncu_traffic_bytes(("full_fused_cfg%d" if wl.path == "full" else "het_cfg%d") % args.workload)
+            tag = ("full_fused_cfg%d" if wl.path == "full" else "het_cfg%d") % args.workload
+            if args.n_walkers is not None:  # a capture belongs to one batch size: only the committed small-batch one applies
+                tag = "small%d" % args.n_walkers
+            traffic, traffic_src = ncu_traffic_bytes(tag)
             line["roofline"] = {
                 "bound": "alu", "kernel": rf["kernel"], "achieved": rf["frac"] * peak_slots / 1e12, "peak": peak_slots / 1e12,
                 "unit": "T FP64 issue slots/s (1 DFMA|DMUL|DADD = 1 slot)", "frac": rf["frac"],

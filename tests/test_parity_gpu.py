@@ -174,11 +174,12 @@ def test_cfg2_full_size_sampled(orc, torch_cuda):
     assert np.all(got[1] ** 2 <= dd_full * got[2] * (1 + 1e-9))
     np.testing.assert_allclose(got[0], got[1] - 0.5 * got[2] - 0.5 * dd_full, rtol=1e-13)
     # Module-1 sized batches of the same walkers on the same grid (80 walkers x 4 temperatures, half of
-    # them per likelihood call) take the small-batch route (one-block sort, block-per-system spline, interval-limited
-    # tiles, two-stage finalize); every walker must come out as in the big batch, up to summation order
+    # them per likelihood call) take the small-batch route (one-block sort and cost plan, block-per-system spline, one-warp
+    # blocks over cost-balanced work items, k_finalize_small); every walker must come out as in the big batch, up to
+    # summation order
     for n_small in (160, 37):
         sm = [x.cpu().numpy() for x in ctx.full_batch_standin(wl.f_nodes, dev(torch_cuda, wl.params[:n_small]))]
-        assert ctx.last_full_stats()[1] > 8 * 64 * (n_small // 32 + 1) // 2          # thousands of tiles: two-stage finalize
+        assert ctx.last_full_stats()[1] > 8 * 64 * (n_small // 32 + 1) // 2          # thousands of work items, not a handful of walker blocks
         for a, b in zip(sm, got):                          # other tiles -> other re-sync points of the recurrence
             assert np.all(np.abs(a - b[:n_small]) <= 1e-7 * np.maximum(1.0, np.abs(b[:n_small])))
     ctx.destroy()
