@@ -344,7 +344,8 @@ int prepare_nodes(ll_ctx *ctx, int n, const double *x, cudaStream_t st)
 }
 
 #ifndef LL_FUSED_CH
-#define LL_FUSED_CH 256 // bins per TMA stage of the fused kernel (two stages per block)
+#define LL_FUSED_CH 512 // bins per TMA stage of the fused kernels (two stages per block): a block-wide barrier per stage;
+                        // 256 -> 512 bins: 9.17 -> 9.08 ms at config 2 (40 KB per block, five blocks per SM)
 #endif
 FullPlan make_plan(const ll_ctx *ctx, long long n_w)
 {
@@ -363,7 +364,10 @@ FullPlan make_plan(const ll_ctx *ctx, long long n_w)
     pl.TB = TB;
     // bins per TMA stage: blocks of one warp (small batches) take 64-bin stages, 5 KB of shared memory per block, so
     // that shared memory does not hold an SM to 11 resident warps (ncu r02a: 12 % warps active with 256-bin stages)
-    pl.CH = std::min(TB, pl.WB == 32 ? 64 : LL_FUSED_CH);
+    // (other layouts keep 256-bin stages: with 9 doubles per bin two 512-bin stages would pass the 48 KB a launch gets
+    // without opting in, and hold an SM to three blocks;
+    // and the multi-mode kernel measured 24.8 ms with 256-bin stages against 28.0 ms with 512 at six modes)
+    pl.CH = std::min(TB, pl.WB == 32 ? 64 : ((ctx->n_c == 2 && ctx->w_rows == 1 && ctx->n_m == 1) ? LL_FUSED_CH : 256));
     pl.n_tiles = ceil_div(ctx->n_f, TB);
     pl.key_gran = std::max(1, ceil_div(ctx->n_f, 4096));
     pl.n_keys = (int)(ctx->n_f / pl.key_gran) + 2;
@@ -1078,7 +1082,7 @@ int ll_set_data(ll_ctx *ctx, int64_t n_f, int64_t k_min, double df, const double
     const int w_rows_in = w_shared ? 1 : ctx->n_c;
     const int nw = (ctx->n_c == 2 && w_shared) ? 1 : ctx->n_c;
     ctx->w_rows = nw;
-    const long long n_pad = round_up(n_f, 512);
+    const long long n_pad = round_up(n_f, 512) + 512; // a stage of up to 512 bins may start at the grid's last bin
     CK(ctx->g.ensure(sizeof(double) * 2 * ctx->n_c * n_pad));
     CK(ctx->Wc.ensure(sizeof(double) * nw * n_pad));
     CK(ctx->dd.ensure(sizeof(double) * 2));

@@ -1066,7 +1066,11 @@ __device__ __forceinline__ double qc_linear_mod_cycle(double x, double ts4 /* 4 
 #define LL_FUSED_UNROLL 3 // bins in flight per thread in the hot loop (tuned on B200, profiles/)
 #endif
 #ifndef LL_FUSED_MINB
-#define LL_FUSED_MINB 4 // resident 128-thread blocks per SM the register budget is held to
+#define LL_FUSED_MINB 6 // resident 128-thread blocks per SM the register budget of the single-mode large-batch kernel is held
+                        // to: 80 registers (the multi-mode and small-batch instantiations keep 4: 128).  Measured at
+                        // config 2 (round 2, 256-bin stages): 4 blocks (118 registers) 9.37 ms, 5 (96) 9.57, 6 (80, ~50 bytes
+                        // of spills outside the bin loop) 9.17, 7 (72) 9.44; with 512-bin stages (five blocks fit the shared
+                        // memory) and the recurrence loop unrolled four times: 8.99 ms
 #endif
 constexpr int kFusedUnroll = LL_FUSED_UNROLL;
 // bins [b0, b1) of one spline interval for the single-mode kernel: t, the two cubics, A e^{-i Psi}, the complex MACs
@@ -1115,7 +1119,7 @@ __device__ __forceinline__ void fused_bins_nm1(int b0, int b1, int tlo, int thi,
                         // 256: 1.2e-7, 9.96 (noiseless -8.7e-8).  The exact route: 7e-8, 13.0 ms.
 #endif
 #ifndef LL_ROT_UNROLL
-#define LL_ROT_UNROLL 2
+#define LL_ROT_UNROLL 4 // bins per trip of the unmasked recurrence loop in large batches (2 for the masked ends and small batches)
 #endif
 #ifndef LL_ROT_ACC
 #define LL_ROT_ACC 1 // the rotations of a re-synchronisation from the degree-7 polynomials (ll_device.cuh)
@@ -1139,7 +1143,7 @@ __device__ __forceinline__ void unit_modulus(double &c, double &s)
 }
 // MASK: lanes outside their own band [tlo, thi) ride along with amplitude 0 (the ragged end of a warp's band: a
 // few bins in a large sorted batch, but a third of all bins when a whole batch is only a handful of warps).
-template <bool MASK, int NC, bool WS, bool WITH_H = true>
+template <bool MASK, int NC, bool WS, bool WITH_H = true, int UNR = 2>
 __device__ __forceinline__ void fused_bins_rot(int b0, int b1, int tlo, int thi, int kbase, double df, double nxj, double cA0,
                                                double cA1, double cA2, double cA3, double cP0, double cP1, double cP2,
                                                double cP3, const double *__restrict__ sgc, const double *__restrict__ sWc,
@@ -1165,7 +1169,7 @@ __device__ __forceinline__ void fused_bins_rot(int b0, int b1, int tlo, int thi,
         unit_modulus(cz, sz);
         unit_modulus(cw, sw);
         unit_modulus(cv, sv);
-#pragma unroll kRotUnroll
+#pragma unroll UNR
         for (int ii = k0; ii < k1; ++ii) {
             const double Am = (!MASK || ((ii >= tlo) && (ii < thi))) ? A : 0.0;
             const double u = Am * cz, v = Am * sz; // h = u - i v
@@ -1184,9 +1188,10 @@ __device__ __forceinline__ void fused_bins_rot(int b0, int b1, int tlo, int thi,
 // [i0, i1) of one group of 32 walkers, an equal share of the batch's active bins — instead of (walker block, tile);
 // its partial sums go to part[b][NQ][32].
 template <int NM1, int NC, bool WS, int SMALL>
-__global__ void __launch_bounds__(128, (NC == 2 && WS) ? LL_FUSED_MINB : 3) k_full_fused(FusedArgs a)
+__global__ void __launch_bounds__(128, (NC == 2 && WS) ? ((NM1 && !SMALL) ? LL_FUSED_MINB : 4) : 3) k_full_fused(FusedArgs a)
 {
     using TL = Tile<NC, WS>;
+    constexpr int UR = (SMALL || !(NC == 2 && WS)) ? 2 : kRotUnroll; // trip length of the unmasked recurrence loop
     extern __shared__ __align__(128) double sm[];
     __shared__ __align__(8) uint64_t bar[2];
     __shared__ int s_lo, s_hi;
@@ -1304,7 +1309,7 @@ __global__ void __launch_bounds__(128, (NC == 2 && WS) ? LL_FUSED_MINB : 3) k_fu
                                     const double *Q = a.wmom + (size_t)q * a.n_f_pad;
                                     mo[q] = __ldg(Q + fhi - 1) - (first ? 0.0 : __ldg(Q + flo - 1));
                                 }
-                                fused_bins_rot<false, NC, WS, false>(flo, fhi, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0,
+                                fused_bins_rot<false, NC, WS, false, UR>(flo, fhi, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0,
                                                                      cP1, cP2, cP3, sgc, sWc, CH, acc);
                                 double hs = (cA0 * cA0) * mo[0];
                                 hs = fma(2.0 * cA0 * cA1, mo[1], hs);
@@ -1315,8 +1320,8 @@ __global__ void __launch_bounds__(128, (NC == 2 && WS) ? LL_FUSED_MINB : 3) k_fu
                                 hs = fma(cA3 * cA3, mo[6], hs);
                                 acc.H[0] += hs;
                             } else {
-                                fused_bins_rot<false, NC, WS>(flo, fhi, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1,
-                                                              cP2, cP3, sgc, sWc, CH, acc);
+                                fused_bins_rot<false, NC, WS, true, UR>(flo, fhi, tlo, thi, kbase, a.df, nxj, cA0, cA1,
+                                                                                          cA2, cA3, cP0, cP1, cP2, cP3, sgc, sWc, CH, acc);
                             }
                         } else
                             fused_bins_nm1<false, NC, WS>(flo, fhi, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1,
