@@ -353,14 +353,17 @@ FullPlan make_plan(const ll_ctx *ctx, long long n_w)
     pl.WB = (n_w >= 4096) ? 128 : (n_w >= 1024 ? 64 : 32);
     pl.n_wp = (int)round_up(std::max<long long>(n_w, 1), pl.WB);
     const int n_wb = pl.n_wp / pl.WB;
-    // aim at ~16 blocks per SM over the whole grid, tiles between 64 and 4096 bins.  Small batches (blocks of one
+    // aim at ~16 blocks per SM over the whole grid, tiles between 64 and LL_FUSED_TB_MAX bins.  Small batches (blocks of one
     // warp, most tiles beyond the walkers' bands and exiting at once): 8x as many, smaller tiles, so that the active
     // ones still fill the SMs (measured on 160 walkers x 1.57e6 bins: TB 4096 -> 512 halves the fused kernel's time)
     static const int small_factor = getenv("LL_SMALL_TILE_FACTOR") ? atoi(getenv("LL_SMALL_TILE_FACTOR")) : 128;
     const long long target = (long long)ctx->sm_count * (pl.n_wp <= 1024 ? small_factor : 16);
     long long tb = ctx->n_f * n_wb / target;
     int TB = 64;
-    while (TB < 4096 && TB < tb) TB <<= 1;
+#ifndef LL_FUSED_TB_MAX
+#define LL_FUSED_TB_MAX 2048 // config 2: 4096-bin tiles 8.92 ms (step 9.59), 2048: 8.85 (9.54), 1024: 8.81 (9.53), 512: 8.91 (9.68)
+#endif
+    while (TB < LL_FUSED_TB_MAX && TB < tb) TB <<= 1;
     pl.TB = TB;
     // bins per TMA stage: blocks of one warp (small batches) take 64-bin stages, 5 KB of shared memory per block, so
     // that shared memory does not hold an SM to 11 resident warps (ncu r02a: 12 % warps active with 256-bin stages)

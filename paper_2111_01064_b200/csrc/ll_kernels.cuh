@@ -630,7 +630,10 @@ k_nodes_arrays_tf(const double *__restrict__ amp, const double *__restrict__ pha
 //   b_j = (y_{j+1}-y_j)/h_j - h_j (2 M_j + M_{j+1})/6,  c_j = M_j/2,  d_j = (M_{j+1}-M_j)/(6 h_j)
 // dp_j is parked in the b-slot of interval j between the sweeps.
 // ---------------------------------------------------------------------------------------------------
-constexpr int kSplineBlk = 16;
+#ifndef LL_SPLINE_BLK
+#define LL_SPLINE_BLK 24 // rows per register block of both sweeps; config 2: 8 rows 549 us, 16: 518, 24: 447 (254 registers), 32: 477 (spills)
+#endif
+constexpr int kSplineBlk = LL_SPLINE_BLK;
 __global__ void __launch_bounds__(128)
 k_spline(const double *__restrict__ Y, double *__restrict__ C, int n_wp, int n_nodes, int n_m, int ns, NodeTables nt)
 {
@@ -649,7 +652,7 @@ k_spline(const double *__restrict__ Y, double *__restrict__ C, int n_wp, int n_n
     double dpp = 0.0;
     // node values are read through the read-only path (__ldg): the compiler may then hoist the loads of an
     // unrolled group above the stores of the parked dp values instead of paying one memory latency per row
-#pragma unroll 16
+#pragma unroll kSplineBlk
     for (int j = 1; j <= n - 2; ++j) {
         const double ynext = __ldg(y + (size_t)(j + 1) * sw);
         const double s = (ynext - ycur) * __ldg(nt.invh + j);
