@@ -220,12 +220,12 @@ def time_steps(torch, fn, steps: int, warmup: int):
 
 
 def bench_config(torch, index: int, steps: int, warmup: int, rank: int = 0, profile: bool = False, precision: int = 0,
-                 n_w=None):
+                 n_w=None, n_c=None):
     """device-resident timing of one config through the stand-in entry point (parameters -> log L).
     precision = 1: the FP32-accumulate variant of the full-grid path on the SAME data (the data stream is built
     by an FP64 context first, so the two variants can be compared output by output)."""
     from paper_2111_01064_b200 import synth
-    wl = rank_workload(index, rank, n_w=n_w)
+    wl = rank_workload(index, rank, n_w=n_w, **({"n_c": n_c} if n_c else {}))
     ctx = synth.make_context(wl)
     bufs = synth.setup(ctx, wl)
     if precision:
@@ -563,11 +563,13 @@ def main():
     ap.add_argument("--n-walkers", type=int, default=None,
                     help="profiling aid: the headline workload with this many walkers (e.g. 160: one Module-1 sized call); "
                          "implies --quick, and the line's config says so")
+    ap.add_argument("--channels", type=int, default=None, choices=[2, 3],
+                    help="profiling aid: 3 = the headline workload with three channels and per-channel weight rows; implies --quick")
     ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32acc"],
                     help="fp32acc: time the FP32-accumulate variant of the full-grid path as the headline step")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
-    if args.n_walkers is not None:
+    if args.n_walkers is not None or args.channels == 3:
         args.quick = True
 
     if args.impl == "reference":
@@ -591,7 +593,7 @@ def main():
     peaks, peak_src = measured_peaks()
     with ClockSampler(local) as clk:
         res = bench_config(torch, args.workload, args.steps, args.warmup, rank=rank, profile=True,
-                           precision=1 if args.precision == "fp32acc" else 0, n_w=args.n_walkers)
+                           precision=1 if args.precision == "fp32acc" else 0, n_w=args.n_walkers, n_c=args.channels)
     wl, ctx = res["wl"], res["ctx"]
     headline_logL = res["out"][0].clone()
     t_ms = allreduce_max(res["ms_total"])
@@ -635,6 +637,8 @@ def main():
             tag = ("full_fused_cfg%d" if wl.path == "full" else "het_cfg%d") % args.workload
             if args.n_walkers is not None:  # a capture belongs to one batch size: only the committed small-batch one applies
                 tag = "small%d" % args.n_walkers
+            elif args.channels == 3:
+                tag += "_nc3"
             traffic, traffic_src = ncu_traffic_bytes(tag)
             line["roofline"] = {
                 "bound": "alu", "kernel": rf["kernel"], "achieved": rf["frac"] * peak_slots / 1e12, "peak": peak_slots / 1e12,

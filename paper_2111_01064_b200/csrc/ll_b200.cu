@@ -118,7 +118,7 @@ struct ll_ctx {
     DevBuf grp_tab;                // small batches: work items per group of 32 walkers (k_band_sort_small)
     DevBuf pw_x;                   // per-walker node grids: X [n_nodes][n_wp], then the effective bands [n_w][2]
     DevBuf node_tab; // doubles then ints
-    DevBuf wmom;     // [7][n_f_pad] prefix moments of the shared weight row inside the intervals of the current node set
+    DevBuf wmom;     // [w_rows][7][n_f_pad] prefix moments of every weight row inside the intervals of the current node set
     NodeTables nt{};
 
     // full-grid scratch
@@ -333,10 +333,10 @@ int prepare_nodes(ll_ctx *ctx, int n, const double *x, cudaStream_t st)
     ctx->nodes_host.assign(x, x + n);
     ctx->bstart_host = hi;
     ctx->nodes_version += 1;
-    if (ctx->w_rows == 1 && ctx->precision == LL_PREC_FP64) { // <h|h> by weight moments: single-mode kernel, shared weight row
-        CK(ctx->wmom.ensure(sizeof(double) * 7 * (size_t)ctx->n_f_pad));
-        k_w_moments<<<n - 1, 256, 0, st>>>(ctx->Wc.as<double>(), nt.bstart, nt.xj, n, ctx->k_min, ctx->df, ctx->n_f_pad,
-                                           ctx->wmom.as<double>());
+    if (ctx->n_m == 1 && ctx->precision == LL_PREC_FP64) { // <h|h> by weight moments (single-mode kernel): one set per weight row
+        CK(ctx->wmom.ensure(sizeof(double) * 7 * (size_t)ctx->w_rows * (size_t)ctx->n_f_pad));
+        k_w_moments<<<dim3(n - 1, ctx->w_rows), 256, 0, st>>>(ctx->Wc.as<double>(), nt.bstart, nt.xj, n, ctx->k_min, ctx->df,
+                                                              ctx->n_f_pad, ctx->wmom.as<double>());
         LAUNCHED(ctx);
     }
     ctx->nodes_valid = true;
@@ -487,7 +487,7 @@ FusedArgs fused_args(ll_ctx *ctx, const FullPlan &pl, int n_nodes, const double 
     fa.n_f = (int)ctx->n_f; fa.n_wp = pl.n_wp; fa.n_nodes = n_nodes; fa.n_m = ctx->n_m; fa.TB = pl.TB; fa.CH = pl.CH;
     fa.tile_start = ctx->tile_cur ? ctx->tile_cur->tab.as<int>() : nullptr;
     fa.grp_tab = ctx->grp_tab.as<int>();
-    fa.wmom = (ctx->w_rows == 1 && ctx->precision == LL_PREC_FP64 && ctx->n_m == 1) ? ctx->wmom.as<double>() : nullptr;
+    fa.wmom = (ctx->precision == LL_PREC_FP64 && ctx->n_m == 1) ? ctx->wmom.as<double>() : nullptr;
     return fa;
 }
 

@@ -845,6 +845,8 @@ k_w_moments(const double *__restrict__ Wc, const int *__restrict__ bstart, const
 {
     __shared__ double wtot[8][7];
     const int j = blockIdx.x;
+    Wc += (size_t)blockIdx.y * n_f_pad;          // weight row blockIdx.y
+    wmom += (size_t)blockIdx.y * 7 * n_f_pad;    // and its seven prefix rows
     const int i0 = bstart[j], i1 = bstart[j + 1];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const double nx = -xj[j];
@@ -905,7 +907,7 @@ struct FusedArgs {
     double df;
     const int *tile_start; // [n_tiles + 1]: frequency tile t covers dense bins [tile_start[t], tile_start[t+1])
     const int *grp_tab;    // small batches (k_full_fused<.., SMALL = 1>): work dealt out by active bins, see k_band_sort_small
-    const double *wmom;    // [7][n_f_pad] prefix moments of the shared weight row inside each spline interval (k_w_moments), or null
+    const double *wmom;    // [NW][7][n_f_pad] prefix moments of every weight row inside each spline interval (k_w_moments), or null
     int n_f, n_wp, n_nodes, n_m, TB, CH;
 };
 
@@ -1075,6 +1077,9 @@ __device__ __forceinline__ double qc_linear_mod_cycle(double x, double ts4 /* 4 
                         // of spills outside the bin loop) 9.17, 7 (72) 9.44; with 512-bin stages (five blocks fit the shared
                         // memory) and the recurrence loop unrolled four times: 8.99 ms
 #endif
+#ifndef LL_FUSED_MINB_PC
+#define LL_FUSED_MINB_PC 4 // the same for the layouts with per-channel weight rows: three channels at config-2 size 11.08 ms at 3 blocks (160 registers), 10.96 at 4 (128), 11.57 at 5 (96)
+#endif
 constexpr int kFusedUnroll = LL_FUSED_UNROLL;
 // bins [b0, b1) of one spline interval for the single-mode kernel: t, the two cubics, A e^{-i Psi}, the complex MACs
 // with g^c and W A^2.  MASK = per-lane band test (only at the ragged ends of a warp's band).
@@ -1191,10 +1196,14 @@ __device__ __forceinline__ void fused_bins_rot(int b0, int b1, int tlo, int thi,
 // [i0, i1) of one group of 32 walkers, an equal share of the batch's active bins — instead of (walker block, tile);
 // its partial sums go to part[b][NQ][32].
 template <int NM1, int NC, bool WS, int SMALL>
-__global__ void __launch_bounds__(128, (NC == 2 && WS) ? ((NM1 && !SMALL) ? LL_FUSED_MINB : 4) : 3) k_full_fused(FusedArgs a)
+__global__ void __launch_bounds__(128, (NC == 2 && WS) ? ((NM1 && !SMALL) ? LL_FUSED_MINB : 4) : ((NM1 && !SMALL) ? LL_FUSED_MINB_PC : 3))
+k_full_fused(FusedArgs a)
 {
     using TL = Tile<NC, WS>;
-    constexpr int UR = (SMALL || !(NC == 2 && WS)) ? 2 : kRotUnroll; // trip length of the unmasked recurrence loop
+#ifndef LL_ROT_UNROLL_PC
+#define LL_ROT_UNROLL_PC 2
+#endif
+    constexpr int UR = SMALL ? 2 : ((NC == 2 && WS) ? kRotUnroll : LL_ROT_UNROLL_PC); // trip length of the unmasked recurrence loop
     extern __shared__ __align__(128) double sm[];
     __shared__ __align__(8) uint64_t bar[2];
     __shared__ int s_lo, s_hi;
@@ -1302,26 +1311,36 @@ __global__ void __launch_bounds__(128, (NC == 2 && WS) ? ((NM1 && !SMALL) ? LL_F
                     if (flo < fhi) {
                         masked(wlo, flo);
                         if (LL_FUSED_ROT && fhi - flo >= 8) {
-                            if (WS && LL_H_MOMENTS && a.wmom) {
-                                // sum_k W_k A(t_k)^2 over the stretch from the weight moments (two of the 27 slots per bin):
-                                // A^2 = sum_p q_p t^p, M_p = sum_k W_k t_k^p = difference of two prefix entries
-                                double mo[7];
+                            if (LL_H_MOMENTS && a.wmom) {
+                                // sum_k W^r_k A(t_k)^2 over the stretch from the weight moments (two of the 27 slots per bin; 1 + NC
+                                // of the 33 with per-channel rows): A^2 = sum_p q_p t^p, M^r_p = sum_k W^r_k t_k^p = difference of two
+                                // prefix entries
+                                constexpr int NWR = Acc1<NC, WS>::NW;
+                                double mo[NWR][7];
                                 const bool first = flo == __ldg(a.bstart + j);
 #pragma unroll
-                                for (int q = 0; q < 7; ++q) {
-                                    const double *Q = a.wmom + (size_t)q * a.n_f_pad;
-                                    mo[q] = __ldg(Q + fhi - 1) - (first ? 0.0 : __ldg(Q + flo - 1));
-                                }
+                                for (int r = 0; r < NWR; ++r)
+#pragma unroll
+                                    for (int q = 0; q < 7; ++q) {
+                                        const double *Q = a.wmom + (size_t)(r * 7 + q) * a.n_f_pad;
+                                        mo[r][q] = __ldg(Q + fhi - 1) - (first ? 0.0 : __ldg(Q + flo - 1));
+                                    }
                                 fused_bins_rot<false, NC, WS, false, UR>(flo, fhi, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0,
                                                                      cP1, cP2, cP3, sgc, sWc, CH, acc);
-                                double hs = (cA0 * cA0) * mo[0];
-                                hs = fma(2.0 * cA0 * cA1, mo[1], hs);
-                                hs = fma(fma(2.0 * cA0, cA2, cA1 * cA1), mo[2], hs);
-                                hs = fma(2.0 * fma(cA0, cA3, cA1 * cA2), mo[3], hs);
-                                hs = fma(fma(2.0 * cA1, cA3, cA2 * cA2), mo[4], hs);
-                                hs = fma(2.0 * cA2 * cA3, mo[5], hs);
-                                hs = fma(cA3 * cA3, mo[6], hs);
-                                acc.H[0] += hs;
+                                const double q0 = cA0 * cA0, q1 = 2.0 * cA0 * cA1, q2 = fma(2.0 * cA0, cA2, cA1 * cA1);
+                                const double q3 = 2.0 * fma(cA0, cA3, cA1 * cA2), q4 = fma(2.0 * cA1, cA3, cA2 * cA2);
+                                const double q5 = 2.0 * cA2 * cA3, q6 = cA3 * cA3;
+#pragma unroll
+                                for (int r = 0; r < NWR; ++r) {
+                                    double hs = q0 * mo[r][0];
+                                    hs = fma(q1, mo[r][1], hs);
+                                    hs = fma(q2, mo[r][2], hs);
+                                    hs = fma(q3, mo[r][3], hs);
+                                    hs = fma(q4, mo[r][4], hs);
+                                    hs = fma(q5, mo[r][5], hs);
+                                    hs = fma(q6, mo[r][6], hs);
+                                    acc.H[r] += hs;
+                                }
                             } else {
                                 fused_bins_rot<false, NC, WS, true, UR>(flo, fhi, tlo, thi, kbase, a.df, nxj, cA0, cA1,
                                                                                           cA2, cA3, cP0, cP1, cP2, cP3, sgc, sWc, CH, acc);
@@ -1826,7 +1845,7 @@ __global__ void __launch_bounds__(128, NC == 2 ? 3 : 2) k_full_fused_tf(FusedArg
                     apply_tf<NC>(tf, u, v, h);
                 };
                 auto direct_bins = [&](int b0, int b1) {
-                    if (!NM1) {
+                    if constexpr (!NM1) {
                         // several modes: chunks of four bins, mode loop outside (the coefficients read once per chunk)
                         for (int c4 = b0; c4 < b1; c4 += 4) {
                             double t4[4], h4[4][2 * NC];
@@ -1851,17 +1870,17 @@ __global__ void __launch_bounds__(128, NC == 2 ? 3 : 2) k_full_fused_tf(FusedArg
                                 if (ii < b1 && ii >= tlo && ii < thi) accumulate_bin<NC, WS>(sgc, sWc, CH, ii, h4[k], s_dh, s_hh);
                             }
                         }
-                        return;
-                    }
+                    } else {
 #pragma unroll 2
-                    for (int ii = b0; ii < b1; ++ii) {
-                        const bool act = (ii >= tlo) && (ii < thi);
-                        const double t = fma((double)(kbase + ii), a.df, nxj);
-                        double h[2 * NC];
+                        for (int ii = b0; ii < b1; ++ii) {
+                            const bool act = (ii >= tlo) && (ii < thi);
+                            const double t = fma((double)(kbase + ii), a.df, nxj);
+                            double h[2 * NC];
 #pragma unroll
-                        for (int q = 0; q < 2 * NC; ++q) h[q] = 0.0;
-                        mode_at(t, h);
-                        if (act) accumulate_bin<NC, WS>(sgc, sWc, CH, ii, h, s_dh, s_hh);
+                            for (int q = 0; q < 2 * NC; ++q) h[q] = 0.0;
+                            mode_at(t, h);
+                            if (act) accumulate_bin<NC, WS>(sgc, sWc, CH, ii, h, s_dh, s_hh);
+                        }
                     }
                 };
                 // bins inside every lane's band: e^{-i Psi} and A by the recurrence of fused_bins_rot, T^c(f) by Horner
