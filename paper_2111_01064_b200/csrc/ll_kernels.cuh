@@ -1755,8 +1755,11 @@ __device__ __forceinline__ double cubic4(const double *c4, double t)
     return fma(fma(fma(c4[3], t, c4[2]), t, c4[1]), t, c4[0]);
 }
 
+#ifndef LL_TF_MINB
+#define LL_TF_MINB 5 // config-2 size, one mode: 3 blocks per SM (153 registers) 17.33 ms, 4 (128) 17.78, 5 (96, spills outside the bin loop) 16.90, 6 (80) 17.58
+#endif
 template <int NM1, int NC, bool WS>
-__global__ void __launch_bounds__(128, NC == 2 ? 3 : 2) k_full_fused_tf(FusedArgs a)
+__global__ void __launch_bounds__(128, NC == 2 ? (NM1 ? LL_TF_MINB : 3) : 2) k_full_fused_tf(FusedArgs a)
 {
     using TL = Tile<NC, WS>;
     constexpr int NCO = 8 + 8 * NC; // coefficients per (interval, mode)
@@ -2051,8 +2054,11 @@ k_spline_pw(const double *__restrict__ Y, const double *__restrict__ X, double *
 // g/W tiles broadcast from shared memory); every lane tracks its own interval: the bins go up, so the interval index
 // only moves forward, by a comparison with the lane's next node per bin.  NM1: the 8 coefficients of the lane's
 // current interval live in registers; otherwise they are re-read per bin through L1.
+#ifndef LL_PW_MINB
+#define LL_PW_MINB 3
+#endif
 template <int NM1, int NC, bool WS>
-__global__ void __launch_bounds__(128, 3) k_full_fused_pw(FusedArgs a, const double *__restrict__ X)
+__global__ void __launch_bounds__(128, NM1 ? LL_PW_MINB : 3) k_full_fused_pw(FusedArgs a, const double *__restrict__ X)
 {
     using TL = Tile<NC, WS>;
     extern __shared__ __align__(128) double sm[];
@@ -2922,8 +2928,11 @@ __device__ __forceinline__ void het1_segment(const double *__restrict__ tab, int
 #ifndef LL_HET1_WY
 #define LL_HET1_WY 16 // warps per block of the single-mode kernel (one block per SM shares the table copy)
 #endif
+#ifndef LL_HET1_MINB
+#define LL_HET1_MINB 1
+#endif
 template <int NC>
-__global__ void __launch_bounds__(32 * LL_HET1_WY)
+__global__ void __launch_bounds__(32 * LL_HET1_WY, LL_HET1_MINB)
 k_het_standin1(Het1Table T, StandinInfo si, const double *__restrict__ params, int P, int n_w, int n_groups, int S,
                const double *__restrict__ dd, double *__restrict__ logL, double *__restrict__ d_h,
                double *__restrict__ h_h)
