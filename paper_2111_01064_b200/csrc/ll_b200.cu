@@ -360,6 +360,9 @@ FullPlan make_plan(const ll_ctx *ctx, long long n_w)
     const long long target = (long long)ctx->sm_count * (pl.n_wp <= 1024 ? small_factor : 16);
     long long tb = ctx->n_f * n_wb / target;
     int TB = 64;
+#ifndef LL_SMALL_CH
+#define LL_SMALL_CH 128 // bins per TMA stage of the one-warp blocks of small batches (10 KB per block, 16 blocks per SM); 160 walkers on the config-2 grid: 32 bins 0.183 ms, 64: 0.161, 96: 0.153, 128: 0.151, 160: 0.152, 192 and 256 (fewer resident blocks): 0.179
+#endif
 #ifndef LL_FUSED_TB_MAX
 #define LL_FUSED_TB_MAX 2048 // config 2: 4096-bin tiles 8.92 ms (step 9.59), 2048: 8.85 (9.54), 1024: 8.81 (9.53), 512: 8.91 (9.68)
 #endif
@@ -370,7 +373,7 @@ FullPlan make_plan(const ll_ctx *ctx, long long n_w)
     // (other layouts keep 256-bin stages: with 9 doubles per bin two 512-bin stages would pass the 48 KB a launch gets
     // without opting in, and hold an SM to three blocks;
     // and the multi-mode kernel measured 24.8 ms with 256-bin stages against 28.0 ms with 512 at six modes)
-    pl.CH = std::min(TB, pl.WB == 32 ? 64 : ((ctx->n_c == 2 && ctx->w_rows == 1 && ctx->n_m == 1) ? LL_FUSED_CH : 256));
+    pl.CH = std::min(TB, pl.WB == 32 ? LL_SMALL_CH : ((ctx->n_c == 2 && ctx->w_rows == 1 && ctx->n_m == 1) ? LL_FUSED_CH : 256));
     pl.n_tiles = ceil_div(ctx->n_f, TB);
     pl.key_gran = std::max(1, ceil_div(ctx->n_f, 4096));
     pl.n_keys = (int)(ctx->n_f / pl.key_gran) + 2;

@@ -1077,6 +1077,9 @@ __device__ __forceinline__ double qc_linear_mod_cycle(double x, double ts4 /* 4 
                         // of spills outside the bin loop) 9.17, 7 (72) 9.44; with 512-bin stages (five blocks fit the shared
                         // memory) and the recurrence loop unrolled four times: 8.99 ms
 #endif
+#ifndef LL_FUSED_MINB_SMALL
+#define LL_FUSED_MINB_SMALL 4 // register budget of the small-batch instantiation (one-warp blocks), as blocks of 128 threads
+#endif
 #ifndef LL_FUSED_MINB_PC
 #define LL_FUSED_MINB_PC 4 // the same for the layouts with per-channel weight rows: three channels at config-2 size 11.08 ms at 3 blocks (160 registers), 10.96 at 4 (128), 11.57 at 5 (96)
 #endif
@@ -1196,14 +1199,20 @@ __device__ __forceinline__ void fused_bins_rot(int b0, int b1, int tlo, int thi,
 // [i0, i1) of one group of 32 walkers, an equal share of the batch's active bins — instead of (walker block, tile);
 // its partial sums go to part[b][NQ][32].
 template <int NM1, int NC, bool WS, int SMALL>
-__global__ void __launch_bounds__(128, (NC == 2 && WS) ? ((NM1 && !SMALL) ? LL_FUSED_MINB : 4) : ((NM1 && !SMALL) ? LL_FUSED_MINB_PC : 3))
+__global__ void __launch_bounds__(128, (NC == 2 && WS) ? (NM1 ? (SMALL ? LL_FUSED_MINB_SMALL : LL_FUSED_MINB) : 4) : ((NM1 && !SMALL) ? LL_FUSED_MINB_PC : 3))
 k_full_fused(FusedArgs a)
 {
     using TL = Tile<NC, WS>;
 #ifndef LL_ROT_UNROLL_PC
 #define LL_ROT_UNROLL_PC 2
 #endif
-    constexpr int UR = SMALL ? 2 : ((NC == 2 && WS) ? kRotUnroll : LL_ROT_UNROLL_PC); // trip length of the unmasked recurrence loop
+#ifndef LL_ROT_UNROLL_MASKED
+#define LL_ROT_UNROLL_MASKED 2
+#endif
+#ifndef LL_ROT_UNROLL_SMALL
+#define LL_ROT_UNROLL_SMALL 4 // 160 walkers on the config-2 grid: 1: 0.156 ms, 2: 0.151, 3: 0.150, 4: 0.148
+#endif
+    constexpr int UR = SMALL ? LL_ROT_UNROLL_SMALL : ((NC == 2 && WS) ? kRotUnroll : LL_ROT_UNROLL_PC); // trip length of the unmasked recurrence loop
     extern __shared__ __align__(128) double sm[];
     __shared__ __align__(8) uint64_t bar[2];
     __shared__ int s_lo, s_hi;
@@ -1302,8 +1311,8 @@ k_full_fused(FusedArgs a)
                     // masked stretch [b0, b1): by recurrence with the mask when it is long enough, else bin by bin
                     auto masked = [&](int b0, int b1) {
                         if (LL_FUSED_ROT && b1 - b0 >= 8)
-                            fused_bins_rot<true, NC, WS>(b0, b1, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1, cP2, cP3,
-                                                         sgc, sWc, CH, acc);
+                            fused_bins_rot<true, NC, WS, true, LL_ROT_UNROLL_MASKED>(b0, b1, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3,
+                                                                                     cP0, cP1, cP2, cP3, sgc, sWc, CH, acc);
                         else
                             fused_bins_nm1<true, NC, WS>(b0, b1, tlo, thi, kbase, a.df, nxj, cA0, cA1, cA2, cA3, cP0, cP1, cP2, cP3,
                                                          sgc, sWc, CH, acc);
