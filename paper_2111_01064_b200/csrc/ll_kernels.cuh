@@ -3340,11 +3340,13 @@ k_pt_run_het1(Het1Table T, StandinInfo si, PtRunArgs a)
                 // ---- proposal (k_pt_propose) and the walker constants, ONCE per proposal, by the first warp (with 16
                 // segment warps each redoing pow, cbrt and three divisions for its 8 edges, the constants were more
                 // than half of the block's FP64 instructions); the others pick the five constants up from shared memory
-                double y[P], z = 1.0;
+                double y[P], z = 1.0, l_old = 0.0, beta_t = 0.0;
                 bool in = true;
                 const size_t wk = (size_t)t * n_w + k0 + k;
                 WalkerConst c;
                 if (seg == 0) {
+                    l_old = logL[wk];      // for the acceptance test: loaded here, with the rows, not on its critical path
+                    beta_t = a.betas[t];
                     const double tt = __dadd_rn(__dmul_rn(a.a - 1.0, pt_uniform(a.seed, it, 3 * half, ii)), 1.0);
                     z = __ddiv_rn(__dmul_rn(tt, tt), a.a);
                     int j = (int)(pt_uniform(a.seed, it, 3 * half + 1, ii) * (double)nh);
@@ -3414,7 +3416,7 @@ k_pt_run_het1(Het1Table T, StandinInfo si, PtRunArgs a)
                     // ---- accept (k_pt_accept)
                     bool acc = false;
                     if (in && l_new == l_new && fabs(l_new) != INFINITY) {
-                        const double lnq = __dadd_rn(wc_s[192 + lane], __dmul_rn(a.betas[t], __dadd_rn(l_new, -logL[wk])));
+                        const double lnq = __dadd_rn(wc_s[192 + lane], __dmul_rn(beta_t, __dadd_rn(l_new, -l_old)));
                         acc = wc_s[160 + lane] < lnq;
                     }
                     if (acc) {
@@ -3447,6 +3449,11 @@ k_pt_run_het1(Het1Table T, StandinInfo si, PtRunArgs a)
                 const double l = has ? logL[cidx] : 0.0;
                 const double dh = (has && a.d_h) ? a.d_h[cidx] : 0.0, hh = (has && a.h_h) ? a.h_h[cidx] : 0.0;
                 const double beta = has ? a.betas[lane] : 0.0;
+                // every rung's row of this column, loaded with the log L values (one memory round trip for the whole sweep, not
+                // a second one after the cascade): lane q < P holds parameter q of rung s in xv[s]
+                double xv[32];
+#pragma unroll
+                for (int s_ = 0; s_ < 32; ++s_) xv[s_] = (s_ < n_t && lane < P) ? x[((size_t)s_ * n_w + col) * P + lane] : 0.0;
                 const double lnu = (lane >= 1 && has) ? log(pt_uniform(a.seed, it, 6, (long long)(lane - 1) * n_w + col)) : 0.0;
                 const double db = __dadd_rn(beta, -__shfl_up_sync(0xffffffffu, beta, 1)); // beta_t - beta_{t-1}
                 const double lprev = __shfl_up_sync(0xffffffffu, l, 1);                  // ln L of rung t - 1
@@ -3460,24 +3467,17 @@ k_pt_run_het1(Het1Table T, StandinInfo si, PtRunArgs a)
                     if (!sw) { carried = lc; csrc = t - 1; }
                 }
                 if (lane == 0) my_src = csrc;
-                // rows: every read before any write
-                double xv[32];
-#pragma unroll
-                for (int t = 0; t < 32; ++t) {
-                    xv[t] = 0.0;
-                    if (t < n_t) { // uniform
-                        const int src = __shfl_sync(0xffffffffu, my_src, t);
-                        if (src != t && lane < P) xv[t] = x[((size_t)src * n_w + col) * P + lane];
-                    }
-                }
+                // the sweep is a permutation of the column's rungs: rung s goes to the rung whose source it is
+                int my_dst = lane;
+                for (int t = 0; t < n_t; ++t)
+                    if (__shfl_sync(0xffffffffu, my_src, t) == lane) my_dst = t;
                 const double l_new = __shfl_sync(0xffffffffu, l, my_src & 31);
                 const double dh_new = __shfl_sync(0xffffffffu, dh, my_src & 31), hh_new = __shfl_sync(0xffffffffu, hh, my_src & 31);
-                __syncwarp();
 #pragma unroll
-                for (int t = 0; t < 32; ++t)
-                    if (t < n_t) {
-                        const int src = __shfl_sync(0xffffffffu, my_src, t);
-                        if (src != t && lane < P) x[((size_t)t * n_w + col) * P + lane] = xv[t];
+                for (int s_ = 0; s_ < 32; ++s_)
+                    if (s_ < n_t) { // uniform; all rows were read before the cascade
+                        const int dst = __shfl_sync(0xffffffffu, my_dst, s_);
+                        if (dst != s_ && lane < P) x[((size_t)dst * n_w + col) * P + lane] = xv[s_];
                     }
                 if (has && my_src != lane) {
                     logL[cidx] = l_new;
