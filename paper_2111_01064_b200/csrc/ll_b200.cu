@@ -961,7 +961,7 @@ int pt_run_fused(ll_ctx *ctx, int32_t n_t, int32_t n_w, double *x, double *logL,
     }
     if (!ctx->coop) return LL_ERR_UNSUPPORTED;
     const size_t tab_d = (size_t)ctx->ht1.n_e * het1_stride(NC);
-    const size_t smem = sizeof(double) * (tab_d + (tab_d & 1) + (size_t)WY * 32 * 3 * NC + 7 * 32);
+    const size_t smem = sizeof(double) * (tab_d + (tab_d & 1) + (size_t)WY * 32 * 3 * NC + 7 * 32 + (size_t)WY * (32 * (5 + 2 * NC) + 16));
     if (smem > 227 * 1024) return LL_ERR_UNSUPPORTED;
     if (!ctx->ptrun_attr) {
         CK(cudaFuncSetAttribute(k_pt_run_het1<NC>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));

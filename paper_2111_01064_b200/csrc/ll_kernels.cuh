@@ -3308,6 +3308,8 @@ k_pt_run_het1(Het1Table T, StandinInfo si, PtRunArgs a)
     const int total = T.n_e * ST;
     double *red = tab + total + (total & 1); // [S][NR][32]
     double *wc_s = red + S * NR * 32;        // [7][32]: the walker constants of the pass's 32 proposals, ln u_accept, (d-1) ln z
+    constexpr int kSwapSlab = 32 * P + 16;   // per warp: a column's rows [32][P] and the source rung of every rung (swap sweep)
+    double *swp = wc_s + 7 * 32;             // [S][kSwapSlab]
     for (int i = threadIdx.x + threadIdx.y * 32; i < total; i += 32 * blockDim.y) tab[i] = T.base[i];
     __syncthreads();
     const int seg = threadIdx.y, lane = threadIdx.x;
@@ -3450,10 +3452,16 @@ k_pt_run_het1(Het1Table T, StandinInfo si, PtRunArgs a)
                 const double dh = (has && a.d_h) ? a.d_h[cidx] : 0.0, hh = (has && a.h_h) ? a.h_h[cidx] : 0.0;
                 const double beta = has ? a.betas[lane] : 0.0;
                 // every rung's row of this column, loaded with the log L values (one memory round trip for the whole sweep, not
-                // a second one after the cascade): lane q < P holds parameter q of rung s in xv[s]
-                double xv[32];
+                // a second one after the cascade) and parked in the warp's shared-memory slab: element e = rung * P + parameter
+                double *rows = swp + seg * kSwapSlab;
+                int *srcs = reinterpret_cast<int *>(rows + 32 * P);
+                const int ne = n_t * P;
+                double rv[P];
 #pragma unroll
-                for (int s_ = 0; s_ < 32; ++s_) xv[s_] = (s_ < n_t && lane < P) ? x[((size_t)s_ * n_w + col) * P + lane] : 0.0;
+                for (int k = 0; k < P; ++k) {
+                    const int e = lane + 32 * k, t = e / P;
+                    rv[k] = (e < ne) ? x[((size_t)t * n_w + col) * P + (e - t * P)] : 0.0;
+                }
                 const double lnu = (lane >= 1 && has) ? log(pt_uniform(a.seed, it, 6, (long long)(lane - 1) * n_w + col)) : 0.0;
                 const double db = __dadd_rn(beta, -__shfl_up_sync(0xffffffffu, beta, 1)); // beta_t - beta_{t-1}
                 const double lprev = __shfl_up_sync(0xffffffffu, l, 1);                  // ln L of rung t - 1
@@ -3467,18 +3475,23 @@ k_pt_run_het1(Het1Table T, StandinInfo si, PtRunArgs a)
                     if (!sw) { carried = lc; csrc = t - 1; }
                 }
                 if (lane == 0) my_src = csrc;
-                // the sweep is a permutation of the column's rungs: rung s goes to the rung whose source it is
-                int my_dst = lane;
-                for (int t = 0; t < n_t; ++t)
-                    if (__shfl_sync(0xffffffffu, my_src, t) == lane) my_dst = t;
+                if (has) srcs[lane] = my_src;
+#pragma unroll
+                for (int k = 0; k < P; ++k)
+                    if (lane + 32 * k < ne) rows[lane + 32 * k] = rv[k];
+                __syncwarp();
                 const double l_new = __shfl_sync(0xffffffffu, l, my_src & 31);
                 const double dh_new = __shfl_sync(0xffffffffu, dh, my_src & 31), hh_new = __shfl_sync(0xffffffffu, hh, my_src & 31);
+                // only the rows that moved are written (all of them were read before the cascade)
 #pragma unroll
-                for (int s_ = 0; s_ < 32; ++s_)
-                    if (s_ < n_t) { // uniform; all rows were read before the cascade
-                        const int dst = __shfl_sync(0xffffffffu, my_dst, s_);
-                        if (dst != s_ && lane < P) x[((size_t)dst * n_w + col) * P + lane] = xv[s_];
+                for (int k = 0; k < P; ++k) {
+                    const int e = lane + 32 * k;
+                    if (e < ne) {
+                        const int t = e / P, q = e - t * P, src = srcs[t];
+                        if (src != t) x[((size_t)t * n_w + col) * P + q] = rows[src * P + q];
                     }
+                }
+                __syncwarp(); // the slab is reused by the warp's next column
                 if (has && my_src != lane) {
                     logL[cidx] = l_new;
                     if (a.d_h) a.d_h[cidx] = dh_new;
