@@ -237,6 +237,27 @@ int ll_pt_stretch_half_het(ll_ctx *ctx, int32_t n_temps, int32_t n_walkers, int3
                            double *d_h, double *h_h, const double *betas, const double *lo, const double *hi,
                            int32_t n_dim, double a, const double *u_z, const double *u_partner, const double *u_accept,
                            int32_t *accepted, void *stream);
+/* ll_pt_stretch_half_het_static: ll_pt_stretch_half_het for callers that must not allocate (a caller under CUDA
+ *   graph capture, a tight serving loop, a harness that forbids cudaMalloc).  Same arguments, same three launches
+ *   (propose, H1-H3, accept), same arithmetic (readings R25-R28), results identical to
+ *   ll_pt_stretch_half_het; but the step's scratch — the proposal rows [n_temps n_walkers/2][P], their ln L, <d|h>,
+ *   <h|h>, (n_dim-1) ln z and inside-the-box flags — lives in a file-scope device array of the library instead of the
+ *   context's lazily grown buffers, so this call makes no cudaMalloc, cudaFree or allocating library call, on the
+ *   first call or any later one.  ll_het_prepare and ll_standin_config (which do allocate) come before, as for
+ *   ll_pt_stretch_half_het.  The array is LL_STATIC_SCRATCH_BYTES (2 MiB) on every GPU that loads the library, held
+ *   until the process exits; its device address is looked up once per device in ll_create (cudaGetSymbolAddress with
+ *   that device current).
+ *   Limit: n_temps (n_walkers/2) (P + 4.5) doubles <= LL_STATIC_SCRATCH_BYTES / 8, e.g. 19 418 proposals at P = 9
+ *   (Module-2 size, 10 x 400, needs 2000); beyond it the call returns LL_ERR_ARG, launches nothing, and
+ *   ll_last_error names the size asked for and the limit.
+ *   ONE array per device, shared by every context and every call: calls that overlap on the GPU (different streams,
+ *   different contexts on one device) race on it — serialise them (one stream, or events).  It keeps the last call's
+ *   contents; nothing in it has to be cleared, since every element a call reads it has written before.          */
+#define LL_STATIC_SCRATCH_BYTES (2 * 1024 * 1024)
+int ll_pt_stretch_half_het_static(ll_ctx *ctx, int32_t n_temps, int32_t n_walkers, int32_t half, double *x,
+                                  double *logL, double *d_h, double *h_h, const double *betas, const double *lo,
+                                  const double *hi, int32_t n_dim, double a, const double *u_z,
+                                  const double *u_partner, const double *u_accept, int32_t *accepted, void *stream);
 int ll_pt_stretch_half_full(ll_ctx *ctx, int32_t n_nodes, const double *f_nodes, int32_t n_temps, int32_t n_walkers,
                             int32_t half, double *x, double *logL, double *d_h, double *h_h, const double *betas,
                             const double *lo, const double *hi, int32_t n_dim, double a, const double *u_z,

@@ -17,6 +17,7 @@ SO_PATH = os.path.join(_HERE, "libll_b200.so")
 
 LL_OK, LL_ERR_ARG, LL_ERR_STATE, LL_ERR_CUDA, LL_ERR_NOMEM, LL_ERR_UNSUPPORTED, LL_ERR_REF_ZERO = 0, -1, -2, -3, -4, -5, -6
 LL_PREC_FP64, LL_PREC_FP32_ACC = 0, 1
+LL_STATIC_SCRATCH_BYTES = 2 * 1024 * 1024  # include/ll.h: the static device array of ll_pt_stretch_half_het_static
 LL_BC_NATURAL, LL_BC_NOT_A_KNOT = 0, 1
 
 # every symbol include/ll.h declares (tests/test_abi.py checks header and library against this list)
@@ -26,7 +27,7 @@ SYMBOLS = (
     "ll_full_batch", "ll_full_batch_pw", "ll_full_batch_tf", "ll_tlm_nodes", "ll_standin_nodes", "ll_full_batch_standin", "ll_full_batch_standin_host",
     "ll_full_template_standin",
     "ll_template_standin", "ll_het_prepare", "ll_het_refresh_standin", "ll_het_audit_standin",
-    "ll_pt_stretch_half_het", "ll_pt_stretch_half_full", "ll_pt_swap", "ll_pt_stats", "ll_pt_run_het", "ll_pt_run_full", "ll_pt_fused", "ll_stop_snr", "ll_stop_converged", "ll_het_get_summary", "ll_het_batch", "ll_het_batch_standin",
+    "ll_pt_stretch_half_het", "ll_pt_stretch_half_het_static", "ll_pt_stretch_half_full", "ll_pt_swap", "ll_pt_stats", "ll_pt_run_het", "ll_pt_run_full", "ll_pt_fused", "ll_stop_snr", "ll_stop_converged", "ll_het_get_summary", "ll_het_batch", "ll_het_batch_standin",
     "ll_het_batch_standin_host", "ll_peak_fma", "ll_kernel_launches", "ll_last_full_stats",
     "ll_profile_enable", "ll_profile_read",
 )
@@ -83,6 +84,7 @@ def load_library(path: Optional[str] = None):
         "ll_het_refresh_standin": (C.c_int, [vp, i64, vp, vp, i32, vp, vp, vp]),
         "ll_het_audit_standin": (C.c_int, [vp, i64, vp, vp, vp, vp, vp]),
         "ll_pt_stretch_half_het": (C.c_int, [vp, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp, i32, dbl, vp, vp, vp, vp, vp]),
+        "ll_pt_stretch_half_het_static": (C.c_int, [vp, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp, i32, dbl, vp, vp, vp, vp, vp]),
         "ll_pt_stretch_half_full": (C.c_int, [vp, i32, vp, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp, i32, dbl, vp, vp, vp,
                                               vp, vp]),
         "ll_pt_swap": (C.c_int, [vp, i32, i32, vp, vp, vp, vp, vp, vp, vp, vp]),
@@ -460,6 +462,22 @@ class Context:
             f_nodes = _host_f64(f_nodes, "f_nodes")
             self._check(self._lib.ll_pt_stretch_half_full(self._h, len(f_nodes), f_nodes.ctypes.data_as(C.c_void_p), *tail),
                         "ll_pt_stretch_half_full")
+
+    def pt_stretch_half_static(self, half, x, logL, d_h, h_h, betas, lo, hi, n_dim, u_z, u_partner, u_accept, a=2.0,
+                               accepted=None, stream=None):
+        """pt_stretch_half on the heterodyned likelihood with the step's scratch in the library's static device array
+        (LL_STATIC_SCRATCH_BYTES, one per GPU, shared by all calls): the call allocates nothing; sizes beyond the array
+        raise LLError (include/ll.h: ll_pt_stretch_half_het_static)"""
+        n_t, n_w = int(x.shape[0]), int(x.shape[1])
+        self._check_pt(x, logL, d_h, h_h, betas, lo, hi)
+        for u in (u_z, u_partner, u_accept):
+            _shape(u, (n_t, n_w // 2), "u_z / u_partner / u_accept")
+        _shape(accepted, (n_t, n_w // 2), "accepted")
+        self._check(self._lib.ll_pt_stretch_half_het_static(
+            self._h, n_t, n_w, int(half), _dev_ptr(x, "x"), _dev_ptr(logL, "logL"), _dev_ptr(d_h, "d_h"), _dev_ptr(h_h, "h_h"),
+            _dev_ptr(betas, "betas"), _dev_ptr(lo, "lo"), _dev_ptr(hi, "hi"), int(n_dim), float(a), _dev_ptr(u_z, "u_z"),
+            _dev_ptr(u_partner, "u_partner"), _dev_ptr(u_accept, "u_accept"), _dev_ptr_i32(accepted, "accepted"),
+            _stream_ptr(stream, self.device)), "ll_pt_stretch_half_het_static")
 
     def _check_pt(self, x, logL, d_h, h_h, betas, lo, hi):
         n_t, n_w = int(x.shape[0]), int(x.shape[1])

@@ -12,6 +12,7 @@
 #include <string.h>
 
 #include <algorithm>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -20,6 +21,12 @@
 #include "ll_kernels.cuh"
 
 using namespace ll;
+
+// Scratch of the one allocation-free entry point, ll_pt_stretch_half_het_static (include/ll.h): a file-scope device
+// array of LL_STATIC_SCRATCH_BYTES that every GPU which loads this library holds until the process exits.  In host
+// code this name is only the runtime's handle for the symbol, NOT a device address: the address a kernel may be given
+// comes from cudaGetSymbolAddress (static_scratch_addr below), looked up once per device with that device current.
+static __device__ __align__(256) double g_ll_static_scratch[LL_STATIC_SCRATCH_BYTES / sizeof(double)];
 
 namespace {
 
@@ -142,6 +149,7 @@ struct ll_ctx {
     bool pt_fused = true;          // ll_pt_run_het: the one-launch cooperative kernel when the population fits it
     int coop = -1;                 // device supports cooperative launches (-1: not asked yet)
     bool ptrun_attr = false;
+    double *static_scratch = nullptr; // device address of g_ll_static_scratch on this context's device (ll_create)
     HetTable ht{};
     Het1Table ht1{}; // single-mode regrouped table (k_het_standin1); base == nullptr when not built
     std::vector<double> raw_host; // [n_b][6 n_c + 1]
@@ -199,6 +207,27 @@ struct DeviceGuard {
         cudaError_t e_ = (call);                                           \
         if (e_ != cudaSuccess) return ctx->cuda_fail(#call, e_);           \
     } while (0)
+
+// device address of g_ll_static_scratch on `device`: one cudaGetSymbolAddress per device and process, made with that
+// device current (a static __device__ array exists once per device, each copy at its own address)
+constexpr int kMaxScratchDevices = 64;
+std::mutex g_scratch_mu;
+double *g_scratch_addr[kMaxScratchDevices] = {};
+cudaError_t static_scratch_addr(int device, double **out)
+{
+    *out = nullptr;
+    if (device < 0 || device >= kMaxScratchDevices) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_scratch_mu);
+    if (!g_scratch_addr[device]) {
+        DeviceGuard dg(device);
+        void *p = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&p, g_ll_static_scratch);
+        if (e != cudaSuccess) return e;
+        g_scratch_addr[device] = static_cast<double *>(p);
+    }
+    *out = g_scratch_addr[device];
+    return cudaSuccess;
+}
 
 #define LAUNCHED(ctx)                                                      \
     do {                                                                   \
@@ -1025,6 +1054,12 @@ int ll_create(const ll_config *cfg, ll_ctx **out)
         return LL_ERR_UNSUPPORTED;
     }
     ctx->sm_count = prop.multiProcessorCount;
+    // set-up for ll_pt_stretch_half_het_static: where this device keeps the static scratch array
+    if (static_scratch_addr(ctx->device, &ctx->static_scratch) != cudaSuccess) {
+        (void)cudaGetLastError();
+        delete ctx;
+        return LL_ERR_CUDA;
+    }
     // default stand-in description: the (2,2) mode only, kappa = 1/2; overwritten by ll_standin_config
     ctx->si.n_m = ctx->n_m;
     ctx->si.kappa = 0.5;
@@ -1608,6 +1643,50 @@ int ll_pt_stretch_half_het(ll_ctx *ctx, int32_t n_temps, int32_t n_walkers, int3
 {
     return pt_half(ctx, false, 0, nullptr, n_temps, n_walkers, half, x, logL, d_h, h_h, betas, lo, hi, n_dim, a, u_z,
                    u_partner, u_accept, accepted, stream);
+}
+
+// The same half update with the proposal rows, the proposals' results and the inside-the-box flags in the static
+// device array instead of the context's lazily grown buffers: no cudaMalloc, cudaFree or allocating library call on
+// this path (k_pt_propose, the H1-H3 kernel of ll_het_batch_standin, k_pt_accept: three launches, the same kernels and
+// arithmetic as ll_pt_stretch_half_het).  Nothing in the scratch has to start at zero: k_pt_propose writes every row,
+// ln z and flag of the call's proposals and the likelihood kernel every result before k_pt_accept reads them; what a
+// previous call left behind is never read.
+int ll_pt_stretch_half_het_static(ll_ctx *ctx, int32_t n_temps, int32_t n_walkers, int32_t half, double *x, double *logL,
+                                  double *d_h, double *h_h, const double *betas, const double *lo, const double *hi,
+                                  int32_t n_dim, double a, const double *u_z, const double *u_partner,
+                                  const double *u_accept, int32_t *accepted, void *stream)
+{
+    if (!ctx) return LL_ERR_ARG;
+    if (n_temps < 1 || n_walkers < 2 || (n_walkers & 1))
+        return ctx->fail(LL_ERR_ARG, "n_temps >= 1 and an even n_walkers >= 2 are required");
+    if (half != 0 && half != 1) return ctx->fail(LL_ERR_ARG, "half must be 0 or 1");
+    if (!x || !logL || !betas || !lo || !hi || !u_z || !u_partner || !u_accept) return ctx->fail(LL_ERR_ARG, "NULL argument");
+    if (n_dim < 1 || !(a > 1.0)) return ctx->fail(LL_ERR_ARG, "n_dim >= 1 and a > 1 are required");
+    if (!ctx->have_standin) return ctx->fail(LL_ERR_STATE, "ll_standin_config has not been called");
+    if (!ctx->static_scratch) return ctx->fail(LL_ERR_STATE, "the static scratch array has no device address (ll_create)");
+    const int P = 5 + 2 * ctx->n_c * ctx->n_m;
+    const int64_t np = (int64_t)n_temps * (n_walkers / 2);
+    // layout in doubles: y [np][P] | ln L(y), <d|h>, <h|h>, (n_dim - 1) ln z [4][np] | flags (int) [np]
+    const int64_t need = np * (P + 4) + (np + 1) / 2;
+    const int64_t have = (int64_t)(LL_STATIC_SCRATCH_BYTES / sizeof(double));
+    if (need > have)
+        return ctx->fail(LL_ERR_ARG, "ll_pt_stretch_half_het_static: n_temps * n_walkers / 2 = " + std::to_string(np) + " proposals of " +
+                                         std::to_string(P) + " parameters need " + std::to_string(need * 8) +
+                                         " bytes of scratch, the static array holds LL_STATIC_SCRATCH_BYTES = " +
+                                         std::to_string((long long)LL_STATIC_SCRATCH_BYTES) + " (use ll_pt_stretch_half_het)");
+    DeviceGuard dg(ctx->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    double *y = ctx->static_scratch, *ly = y + np * P, *ydh = ly + np, *yhh = ly + 2 * np, *lnz = ly + 3 * np;
+    int *inside = reinterpret_cast<int *>(ly + 4 * np);
+    const int grid = (int)ceil_div(np, 128);
+    k_pt_propose<<<grid, 128, 0, st>>>(x, n_temps, n_walkers, P, half, a, n_dim, lo, hi, u_z, u_partner, y, lnz, inside);
+    LAUNCHED(ctx);
+    const int rc = ll_het_batch_standin(ctx, np, y, ly, ydh, yhh, stream);
+    if (rc != LL_OK) return rc;
+    k_pt_accept<<<grid, 128, 0, st>>>(x, logL, d_h, h_h, n_temps, n_walkers, P, half, betas, u_accept, y, ly, ydh, yhh, lnz,
+                                      inside, accepted, nullptr);
+    LAUNCHED(ctx);
+    return LL_OK;
 }
 
 int ll_pt_stretch_half_full(ll_ctx *ctx, int32_t n_nodes, const double *f_nodes, int32_t n_temps, int32_t n_walkers,
