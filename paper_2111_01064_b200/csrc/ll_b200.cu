@@ -652,16 +652,17 @@ int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, cons
             LAUNCHED(ctx);
         }
         ctx->last_n_blocks = grid;
+        CK(ctx->part2.ensure(sizeof(double) * (size_t)(n_wp / 32) * kFinZ * 9 * 32)); // [group][kFinZ][NQ <= 9][32]
 #define LL_FIN_SMALL(NC, WS)                                                                                               \
     do {                                                                                                                   \
         if (sums1)                                                                                                         \
-            k_finalize_small<1, NC, (WS ? 1 : NC)><<<n_wp / 32, dim3(32, fin_slices(2 * NC + (WS ? 1 : NC))), 0, st>>>(    \
-                ctx->part.as<double>(), ctx->TF.as<double>(), ctx->perm.as<int>(), n_wp, ctx->grp_tab.as<int>(),           \
-                ctx->dd.as<double>(), logL, d_h, h_h);                                                                     \
+            k_finalize_small<1, NC, (WS ? 1 : NC)><<<dim3(n_wp / 32, kFinZ), dim3(32, fin_slices(2 * NC + (WS ? 1 : NC))), 0, st>>>( \
+                ctx->part.as<double>(), ctx->part2.as<double>(), ctx->TF.as<double>(), ctx->perm.as<int>(), n_wp,          \
+                ctx->grp_tab.as<int>(), ctx->dd.as<double>(), logL, d_h, h_h);                                             \
         else                                                                                                               \
-            k_finalize_small<0, NC, (WS ? 1 : NC)><<<n_wp / 32, dim3(32, fin_slices(2)), 0, st>>>(                         \
-                ctx->part.as<double>(), ctx->TF.as<double>(), ctx->perm.as<int>(), n_wp, ctx->grp_tab.as<int>(),           \
-                ctx->dd.as<double>(), logL, d_h, h_h);                                                                     \
+            k_finalize_small<0, NC, (WS ? 1 : NC)><<<dim3(n_wp / 32, kFinZ), dim3(32, fin_slices(2)), 0, st>>>(            \
+                ctx->part.as<double>(), ctx->part2.as<double>(), ctx->TF.as<double>(), ctx->perm.as<int>(), n_wp,          \
+                ctx->grp_tab.as<int>(), ctx->dd.as<double>(), logL, d_h, h_h);                                             \
     } while (0)
         LL_LAYOUT(ctx, LL_FIN_SMALL);
 #undef LL_FIN_SMALL

@@ -195,8 +195,9 @@ k_band_prep(int use_standin, const double *__restrict__ params, int P, const dou
 // The kernel is the planner of the whole small-batch call: besides the group table it writes, per item, (group, first
 // bin, end bin, interval of the first bin) and, per walker, the first and last item its band touches, so that neither
 // the fused kernel's blocks nor k_finalize_small search anything.
-constexpr int kGrpStride = 33; // grp_tab: [0..32] first item of group g (entry 32 = total), then glo, ghi, cg, len [32] each
-constexpr int kGrpInts = kGrpStride + 4 * 32;
+constexpr int kGrpStride = 33; // grp_tab: [0..32] first item of group g (entry 32 = total), then glo, ghi, cg, len [32] each,
+constexpr int kGrpInts = kGrpStride + 5 * 32; // then the tickets of k_finalize_small [32] (zeroed by the planner)
+__host__ __device__ constexpr int grp_off_ticket() { return kGrpStride + 4 * 32; }
 // after them: t0[1024], t1[1024] (items of sorted position p), then item[4][max_items] (group, i0, i1, j0)
 __host__ __device__ constexpr int grp_off_t0() { return kGrpInts; }
 __host__ __device__ constexpr int grp_off_t1() { return kGrpInts + 1024; }
@@ -273,6 +274,7 @@ k_band_sort_small(int use_standin, const double *__restrict__ params, int P, con
         grp_tab[kGrpStride + w] = glo;
         grp_tab[kGrpStride + 32 + w] = ghi;
         grp_tab[kGrpStride + 64 + w] = cg;
+        grp_tab[grp_off_ticket() + w] = 0;
         s_glo[w] = glo; s_ghi[w] = ghi; s_cg[w] = cg;
     }
     __syncthreads();
@@ -2370,26 +2372,32 @@ k_finalize(const double *__restrict__ part, const double *__restrict__ TF, const
     if (h_h) h_h[w] = hh;
 }
 
-// F4 for small batches (k_full_fused<.., SMALL = 1>): one block per group of 32 walkers; the items of the group that
-// overlap a walker's band are summed by 32 slices in a fixed order, T^c applied, log L formed.
+// F4 for small batches (k_full_fused<.., SMALL = 1>).  A group's records are ~1000 x 1.3 KB, and ONE block pulling them
+// through one SM took 19 us (ncu r02: 70 long-scoreboard stalls per issue), so a group is summed by kFinZ blocks: block z
+// takes the items t = z (mod kFinZ) of every walker's range, its 32 slices every 32nd of those, in a fixed order; the
+// block's sums go to part2[group][z], and the block that finishes last (a ticket per group) adds the kFinZ records in z
+// order, applies T^c and forms log L — the same order whichever block comes last, so reruns are bit-identical.
+constexpr int kFinZ = 8;
 template <int NM1, int NC, int NW>
 __global__ void __launch_bounds__(32 * fin_slices(NM1 ? 2 * NC + NW : 2))
-k_finalize_small(const double *__restrict__ part, const double *__restrict__ TF, const int *__restrict__ perm,
-                 int n_wp, const int *__restrict__ grp_tab, const double *__restrict__ dd, double *__restrict__ logL,
-                 double *__restrict__ d_h, double *__restrict__ h_h)
+k_finalize_small(const double *__restrict__ part, double *__restrict__ part2, const double *__restrict__ TF,
+                 const int *__restrict__ perm, int n_wp, int *__restrict__ grp_tab, const double *__restrict__ dd,
+                 double *__restrict__ logL, double *__restrict__ d_h, double *__restrict__ h_h)
 {
     constexpr int NQ = NM1 ? 2 * NC + NW : 2;
     constexpr int FY = fin_slices(NQ);
     __shared__ double red[FY][NQ][32];
-    const int grp = blockIdx.x, lane = threadIdx.x, ty = threadIdx.y;
+    __shared__ int s_last;
+    const int grp = blockIdx.x, z = blockIdx.y, lane = threadIdx.x, ty = threadIdx.y;
     const int p = grp * 32 + lane;
     const size_t sw = (size_t)n_wp;
     double acc[NQ];
 #pragma unroll
     for (int q = 0; q < NQ; ++q) acc[q] = 0.0;
     const int t0 = grp_tab[grp_off_t0() + p], t1 = grp_tab[grp_off_t1() + p]; // items the walker's band touches
+    const int first = t0 + ((z - t0 % kFinZ) + kFinZ) % kFinZ;              // the first of them with t = z (mod kFinZ)
 #pragma unroll 4
-    for (int t = t0 + ty; t <= t1; t += FY) {
+    for (int t = first + ty * kFinZ; t <= t1; t += FY * kFinZ) {
         const double *o = part + (size_t)t * NQ * 32 + lane;
 #pragma unroll
         for (int q = 0; q < NQ; ++q) acc[q] += o[q * 32];
@@ -2397,14 +2405,29 @@ k_finalize_small(const double *__restrict__ part, const double *__restrict__ TF,
 #pragma unroll
     for (int q = 0; q < NQ; ++q) red[ty][q][lane] = acc[q];
     __syncthreads();
-    if (ty != 0) return;
+    double *rec = part2 + (size_t)grp * kFinZ * NQ * 32 + lane; // [z][NQ][32]
+    if (ty == 0) {
+#pragma unroll
+        for (int q = 0; q < NQ; ++q) {
+            double v = red[0][q][lane];
+#pragma unroll
+            for (int k = 1; k < FY; ++k) v += red[k][q][lane];
+            rec[((size_t)z * NQ + q) * 32] = v;
+        }
+        __threadfence(); // the record is visible before the ticket is taken
+    }
+    __syncthreads();
+    if (ty == 0 && lane == 0) s_last = atomicAdd(grp_tab + grp_off_ticket() + grp, 1) == kFinZ - 1;
+    __syncthreads();
+    if (!s_last || ty != 0) return;
+    __threadfence();
     const int w = perm[p];
     if (w < 0) return;
 #pragma unroll
     for (int q = 0; q < NQ; ++q) {
-        double v = red[0][q][lane];
+        double v = 0.0;
 #pragma unroll
-        for (int k = 1; k < FY; ++k) v += red[k][q][lane];
+        for (int k = 0; k < kFinZ; ++k) v += __ldcg(rec + ((size_t)k * NQ + q) * 32); // L2: written by other SMs
         acc[q] = v;
     }
     double dh = 0.0, hh = 0.0;
