@@ -149,6 +149,7 @@ struct ll_ctx {
     bool pt_fused = true;          // ll_pt_run_het: the one-launch cooperative kernel when the population fits it
     int coop = -1;                 // device supports cooperative launches (-1: not asked yet)
     bool ptrun_attr = false;
+    bool spl4_attr = false;
     double *static_scratch = nullptr; // device address of g_ll_static_scratch on this context's device (ll_create)
     HetTable ht{};
     Het1Table ht1{}; // single-mode regrouped table (k_het_standin1); base == nullptr when not built
@@ -601,7 +602,26 @@ int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, cons
         const int rc_b = band_sort(ctx, pl, n_w, standin, params, P, band, st, n_items);
         if (rc_b != LL_OK) return rc_b;
     }
-    if (standin) {
+    // few systems (Module-1 sized batches): a block per four walkers of a system, scan-based sweeps (k_spline_block4), and on
+    // the stand-in path the block evaluates its own node values (no k_nodes_standin launch, no Y); else one thread per system
+    const long long n_sys = (long long)n_wp * ns * n_m;
+    // measured on 160 walkers x 1024 nodes (whole call): 1 walker per block 0.2095 ms (256 threads), 2: 0.2056 (512),
+    // 4: 0.2014 (512 or 1024 threads; 0.2054 with 256) — latency-bound: ~2000 dependent instructions per warp whatever the shape
+    constexpr int NWK4 = 4; // walkers per block of k_spline_block4
+    int T4 = 32 * NWK4;     // its threads: NWK4 walkers x ~8 rows per chunk thread, at most 512
+    while (T4 < 512 && T4 < n_nodes * NWK4 / 8) T4 <<= 1;
+    const size_t smem4 = sizeof(double) * (2 * (size_t)NWK4 * n_nodes + T4);
+    const bool block4 = n_sys <= (long long)ctx->sm_count * 32 && smem4 <= 200 * 1024;
+    if (block4 && !ctx->spl4_attr) {
+#define LL_SPL4_ATTR(S, N) CK(cudaFuncSetAttribute(k_spline_block4<S, N>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024))
+        LL_SPL4_ATTR(true, NWK4);
+        LL_SPL4_ATTR(false, NWK4);
+#undef LL_SPL4_ATTR
+        ctx->spl4_attr = true;
+    }
+    if (standin && block4) {
+        // F1 happens inside F2 (below)
+    } else if (standin) {
         dim3 grid(ceil_div(n_wp, 128), ceil_div(n_nodes, kNodesPerThread));
         k_nodes_standin<<<grid, 128, 0, st>>>(params, P, ctx->perm.as<int>(), n_wp, n_nodes, ctx->si, ctx->nt,
                                               ctx->Y.as<double>(), ctx->TF.as<double>());
@@ -614,16 +634,22 @@ int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, cons
         k_nodes_arrays<<<grid, 256, 0, st>>>(amp, phase, tf, ctx->perm.as<int>(), n_wp, n_nodes, n_m, n_c,
                                              ctx->Y.as<double>(), ctx->TF.as<double>());
     }
-    LAUNCHED(ctx);
+    if (!(standin && block4)) LAUNCHED(ctx);
     {
-        // few systems (Module-1 sized batches): one warp per system, scan-based sweeps; else one thread per system
-        const long long n_sys = (long long)n_wp * ns * n_m;
-        int T = 32;
-        while (T < 256 && T * 4 < n_nodes) T <<= 1; // ~4 rows per thread
-        const size_t smem_w = sizeof(double) * (2 * (size_t)n_nodes + T);
-        if (n_sys <= (long long)ctx->sm_count * 32 && smem_w <= 48 * 1024) {
-            k_spline_block<<<(unsigned)n_sys, T, smem_w, st>>>(ctx->Y.as<double>(), ctx->C.as<double>(), n_wp, n_nodes, n_m, ns,
-                                                             ctx->nt);
+        if (block4) {
+#define LL_SPL4(N)                                                                                                         \
+    do {                                                                                                                   \
+        if (standin)                                                                                                       \
+            k_spline_block4<true, N><<<(unsigned)(n_sys / N), T4, smem4, st>>>(nullptr, ctx->C.as<double>(), n_wp, n_nodes, n_m, ns, \
+                                                                                ctx->nt, params, P, ctx->perm.as<int>(), ctx->si, \
+                                                                                ctx->TF.as<double>());                      \
+        else                                                                                                               \
+            k_spline_block4<false, N><<<(unsigned)(n_sys / N), T4, smem4, st>>>(ctx->Y.as<double>(), ctx->C.as<double>(), n_wp,     \
+                                                                                 n_nodes, n_m, ns, ctx->nt, nullptr, 0, nullptr, \
+                                                                                 ctx->si, nullptr);                         \
+    } while (0)
+            LL_SPL4(NWK4);
+#undef LL_SPL4
         } else {
             dim3 grid(ceil_div(n_wp, 128), ns * n_m);
             k_spline<<<grid, 128, 0, st>>>(ctx->Y.as<double>(), ctx->C.as<double>(), n_wp, n_nodes, n_m, ns, ctx->nt);

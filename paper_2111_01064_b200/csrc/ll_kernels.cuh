@@ -706,7 +706,7 @@ k_spline(const double *__restrict__ Y, double *__restrict__ C, int n_wp, int n_n
 }
 
 // ---------------------------------------------------------------------------------------------------
-// F2 for small batches (Module-1 sized: tens to hundreds of walkers): one warp or block per system.  With
+// F2 for small batches (Module-1 sized: tens to hundreds of walkers): one block per NWK systems.  With
 // few systems the thread-per-system kernel above is a chain of 2 (n-2) dependent steps on a nearly empty GPU.
 // Both Thomas sweeps are first-order linear recurrences x_j = alpha_j + beta_j x_{j-1}, i.e. compositions of
 // affine maps, which are associative: each thread composes the maps of its ceil(n/T) consecutive rows, a scan
@@ -714,61 +714,100 @@ k_spline(const double *__restrict__ Y, double *__restrict__ C, int n_wp, int n_n
 // 2 ceil(n/T) + scan steps instead of n.  Same factorisation tables; results differ from the sequential sweep
 // by rounding only.  Shared memory per warp: node values and dp / M, 2 n doubles.
 // ---------------------------------------------------------------------------------------------------
-// Generalised to one BLOCK of T = 32..256 threads per system (T ~ n/4): the scan runs inside each warp and then
-// across the warps' totals, so 1024 nodes are a chain of 2 x 4 rows + two block scans instead of 2 x 32 rows.
-__device__ __forceinline__ void affine_block_scan_up(double &A, double &B, double *sA, double *sB, int lane, int wid, int nwarp)
+// One block takes NWK (four) neighbouring walkers (sorted positions p0 .. p0 + NWK - 1) of one system: thread =
+// (chunk thread ct = tid / 4, walker wl = tid % 4).  With one walker per block every coefficient store and node-value
+// load was an isolated 8-byte access (ncu r02: 29 sectors per request, the launch 28 us for 320 systems); with four, a
+// row's four walkers are one full 32-byte sector.  STANDIN: the block evaluates its node values from the parameter rows
+// itself (the arithmetic of k_nodes_standin; Y is neither written nor read, one launch less) and the amplitude blocks
+// write the transfer factors.  Shared memory: ys, ds [n][4] and the exchange slots.
+template <int NWK>
+__device__ __forceinline__ void affine_scan4_up(double &A, double &B, double *sA, double *sB, int lane, int wid, int nwarp, int wl)
 {
-    // inclusive scan of maps x -> A + B x in thread order (thread t's map applied after those of threads < t)
 #pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
+    for (int o = NWK; o < 32; o <<= 1) {
         const double Ap = __shfl_up_sync(0xffffffffu, A, o), Bp = __shfl_up_sync(0xffffffffu, B, o);
         if (lane >= o) { A = fma(B, Ap, A); B *= Bp; }
     }
-    if (nwarp > 1) {
-        if (lane == 31) { sA[wid] = A; sB[wid] = B; }
-        __syncthreads();
-        double pa = 0.0, pb = 1.0; // composition of the warps below, in order
-        for (int k = 0; k < wid; ++k) { pa = fma(sB[k], pa, sA[k]); pb *= sB[k]; }
-        A = fma(B, pa, A);
-        B *= pb;
-        __syncthreads();
-    }
+    if (lane >= 32 - NWK) { sA[wid * NWK + wl] = A; sB[wid * NWK + wl] = B; }
+    __syncthreads();
+    double pa = 0.0, pb = 1.0;
+    for (int k = 0; k < wid; ++k) { pa = fma(sB[k * NWK + wl], pa, sA[k * NWK + wl]); pb *= sB[k * NWK + wl]; }
+    A = fma(B, pa, A);
+    B *= pb;
+    __syncthreads();
+    (void)nwarp;
 }
-__device__ __forceinline__ void affine_block_scan_down(double &A, double &B, double *sA, double *sB, int lane, int wid, int nwarp)
+template <int NWK>
+__device__ __forceinline__ void affine_scan4_down(double &A, double &B, double *sA, double *sB, int lane, int wid, int nwarp, int wl)
 {
-    // the mirror image: thread t's map applied after those of threads > t
 #pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
+    for (int o = NWK; o < 32; o <<= 1) {
         const double Ap = __shfl_down_sync(0xffffffffu, A, o), Bp = __shfl_down_sync(0xffffffffu, B, o);
         if (lane + o < 32) { A = fma(B, Ap, A); B *= Bp; }
     }
-    if (nwarp > 1) {
-        if (lane == 0) { sA[wid] = A; sB[wid] = B; }
-        __syncthreads();
-        double pa = 0.0, pb = 1.0;
-        for (int k = nwarp - 1; k > wid; --k) { pa = fma(sB[k], pa, sA[k]); pb *= sB[k]; }
-        A = fma(B, pa, A);
-        B *= pb;
-        __syncthreads();
-    }
+    if (lane < NWK) { sA[wid * NWK + wl] = A; sB[wid * NWK + wl] = B; }
+    __syncthreads();
+    double pa = 0.0, pb = 1.0;
+    for (int k = nwarp - 1; k > wid; --k) { pa = fma(sB[k * NWK + wl], pa, sA[k * NWK + wl]); pb *= sB[k * NWK + wl]; }
+    A = fma(B, pa, A);
+    B *= pb;
+    __syncthreads();
 }
 
-__global__ void __launch_bounds__(256)
-k_spline_block(const double *__restrict__ Y, double *__restrict__ C, int n_wp, int n_nodes, int n_m, int ns, NodeTables nt)
+template <bool STANDIN, int NWK>
+__global__ void __launch_bounds__(1024)
+k_spline_block4(const double *__restrict__ Y, double *__restrict__ C, int n_wp, int n_nodes, int n_m, int ns, NodeTables nt,
+                const double *__restrict__ params, int P, const int *__restrict__ perm, StandinInfo si, double *__restrict__ TF)
 {
-    extern __shared__ double ssm[]; // ys[n], ds[n], then the exchange slots
-    __shared__ double sA[8], sB[8];
+    extern __shared__ double ssm[]; // ys[n][4], ds[n][4], xch[T]
+    __shared__ double sA[128], sB[128];
     const int tid = threadIdx.x, T = blockDim.x, lane = tid & 31, wid = tid >> 5, nwarp = T >> 5;
-    const int sys = blockIdx.x / n_wp, p = blockIdx.x - sys * n_wp;
+    const int wl = tid % NWK, ct = tid / NWK, TT = T / NWK;
+    const int nq4 = n_wp / NWK;
+    const int sys = blockIdx.x / nq4, p0 = (blockIdx.x - sys * nq4) * NWK;
     const int m = sys / ns, kind = sys % ns;
     const int n = n_nodes;
     const size_t sw = (size_t)n_wp;
-    double *ys = ssm, *ds = ys + n, *xch = ds + n; // xch[T]: value handed to the neighbouring thread
-    for (int j = tid; j < n; j += T) ys[j] = __ldg(Y + ((size_t)sys * n + j) * sw + p);
+    double *ys = ssm, *ds = ys + NWK * n, *xch = ds + NWK * n;
+    if (STANDIN) {
+        const int w = perm[p0 + wl];
+        WalkerConst c = {0, 0, 0, 0, 0};
+        const double *row = nullptr;
+        if (w >= 0) {
+            row = params + (size_t)w * P;
+            c = standin_consts(row);
+        }
+        const double inv_kappa = 1.0 / si.kappa;
+        const double mh_pi = (double)si.mode_m[m] / kPi;
+        const double phq = mh_pi * (c.phi + 0.25 * kPi), Kq = mh_pi * c.K;
+        for (int idx = tid; idx < NWK * n; idx += T) { // idx % NWK = wl
+            const int j = idx / NWK;
+            const size_t t = (size_t)m * n + j;
+            double v = 0.0;
+            if (w >= 0) {
+                if (kind == 0) v = __ldg(nt.cfp + t) * c.invD * taper(__ldg(nt.f2m + t) * c.inv_fisco, si.kappa, inv_kappa);
+                else {
+                    v = fma(Kq, __ldg(nt.fm53 + t), -phq);
+                    if (!si.split_tc) v = fma(__ldg(nt.f4 + j), c.tc, v);
+                }
+            }
+            ys[idx] = v;
+        }
+        if (kind == 0) {
+            const int nq = 2 * si.n_c;
+            if (tid < NWK * nq) { // (q = tid / NWK, walker wl)
+                const int q = tid / NWK;
+                TF[((size_t)m * nq + q) * sw + p0 + wl] = (w >= 0) ? row[5 + m * nq + q] : 0.0;
+            }
+        }
+    } else {
+        for (int idx = tid; idx < NWK * n; idx += T) ys[idx] = __ldg(Y + ((size_t)sys * n + idx / NWK) * sw + p0 + wl);
+    }
     __syncthreads();
-    const int L = (n + T - 1) / T;
-    const int j0 = min(tid * L, n), j1 = min(j0 + L, n);
-    auto rhs = [&](int j) { return (ys[j + 1] - ys[j]) * __ldg(nt.invh + j) - (ys[j] - ys[j - 1]) * __ldg(nt.invh + j - 1); };
+    const int L = (n + TT - 1) / TT;
+    const int j0 = min(ct * L, n), j1 = min(j0 + L, n);
+    auto yv = [&](int j) { return ys[NWK * j + wl]; };
+    auto rhs = [&](int j) { return (yv(j + 1) - yv(j)) * __ldg(nt.invh + j) - (yv(j) - yv(j - 1)) * __ldg(nt.invh + j - 1); };
     // ---- forward sweep: dp_j = (r_j - a_j dp_{j-1}) / den_j for j = 1..n-2, dp_0 = 0
     double A = 0.0, B = 1.0;
     for (int j = j0; j < j1; ++j)
@@ -777,13 +816,13 @@ k_spline_block(const double *__restrict__ Y, double *__restrict__ C, int n_wp, i
             A = fma(be, A, rhs(j) * ti);
             B *= be;
         }
-    affine_block_scan_up(A, B, sA, sB, lane, wid, nwarp);
-    xch[tid] = A; // all maps up to and including this thread applied to dp_0 = 0
+    affine_scan4_up<NWK>(A, B, sA, sB, lane, wid, nwarp, wl);
+    xch[tid] = A;
     __syncthreads();
-    double start = tid ? xch[tid - 1] : 0.0;
+    double start = ct ? xch[tid - NWK] : 0.0;
     for (int j = j0; j < j1; ++j) {
         if (j >= 1 && j <= n - 2) start = (rhs(j) - __ldg(nt.ta + j) * start) * __ldg(nt.tinv + j);
-        ds[j] = (j >= 1 && j <= n - 2) ? start : 0.0;
+        ds[NWK * j + wl] = (j >= 1 && j <= n - 2) ? start : 0.0;
     }
     __syncthreads();
     // ---- backward sweep: M_j = dp_j - c'_j M_{j+1} for j = n-2..1, M_0 = M_{n-1} = 0
@@ -791,31 +830,32 @@ k_spline_block(const double *__restrict__ Y, double *__restrict__ C, int n_wp, i
     for (int j = j1 - 1; j >= j0; --j) {
         if (j >= 1 && j <= n - 2) {
             const double be = -__ldg(nt.tcp + j);
-            A = fma(be, A, ds[j]);
+            A = fma(be, A, ds[NWK * j + wl]);
             B *= be;
         } else { A = 0.0; B = 0.0; }
     }
-    affine_block_scan_down(A, B, sA, sB, lane, wid, nwarp);
+    affine_scan4_down<NWK>(A, B, sA, sB, lane, wid, nwarp, wl);
     xch[tid] = A;
     __syncthreads();
-    double Mn = (tid + 1 < T) ? xch[tid + 1] : 0.0;
+    double Mn = (ct + 1 < TT) ? xch[tid + NWK] : 0.0;
     for (int j = j1 - 1; j >= j0; --j) {
-        Mn = (j >= 1 && j <= n - 2) ? fma(-__ldg(nt.tcp + j), Mn, ds[j]) : 0.0;
-        ds[j] = Mn;
+        Mn = (j >= 1 && j <= n - 2) ? fma(-__ldg(nt.tcp + j), Mn, ds[NWK * j + wl]) : 0.0;
+        ds[NWK * j + wl] = Mn;
     }
     __syncthreads();
     if (nt.bc) { // not-a-knot end values from their neighbours
-        if (tid == 0) {
-            ds[0] = (1.0 + nt.rho0) * ds[1] - nt.rho0 * ds[2];
-            ds[n - 1] = (1.0 + nt.rhon) * ds[n - 2] - nt.rhon * ds[n - 3];
+        if (ct == 0) {
+            ds[wl] = (1.0 + nt.rho0) * ds[NWK + wl] - nt.rho0 * ds[2 * NWK + wl];
+            ds[NWK * (n - 1) + wl] = (1.0 + nt.rhon) * ds[NWK * (n - 2) + wl] - nt.rhon * ds[NWK * (n - 3) + wl];
         }
         __syncthreads();
     }
-    // ---- coefficients of interval j (same formulas as k_spline)
-    double *c = C + ((size_t)m * ns * 4 + kind * 4) * sw + p;
+    // ---- coefficients of interval j (same formulas as k_spline): four walkers of a row = one 32-byte sector per store
+    double *c = C + ((size_t)m * ns * 4 + kind * 4) * sw + p0 + wl;
     const size_t cj = (size_t)n_m * ns * 4 * sw;
-    for (int j = tid; j < n - 1; j += T) {
-        const double y0 = ys[j], y1 = ys[j + 1], Mj = ds[j], Mn1 = ds[j + 1];
+    for (int idx = tid; idx < NWK * (n - 1); idx += T) {
+        const int j = idx / NWK;
+        const double y0 = ys[idx], y1 = ys[idx + NWK], Mj = ds[idx], Mn1 = ds[idx + NWK];
         const double h = __ldg(nt.hj + j), ih = __ldg(nt.invh + j);
         double *cc = c + (size_t)j * cj;
         cc[0] = y0;
