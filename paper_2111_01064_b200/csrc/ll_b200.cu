@@ -469,8 +469,10 @@ int ensure_tiles(ll_ctx *ctx, FullPlan &pl, cudaStream_t st, bool uniform = fals
 }
 
 // band -> bin range per walker, sort by band top (F1 prologue shared by every full-grid entry point)
+// defer: (batches of up to 1024 walkers) fill the planner's arguments instead of launching it — the caller runs it as the
+// last block of k_setup_small
 int band_sort(ll_ctx *ctx, const FullPlan &pl, long long n_w, bool standin, const double *params, int P, const double *band,
-              cudaStream_t st, int n_items = 0)
+              cudaStream_t st, int n_items = 0, BandSortArgs *defer = nullptr)
 {
     const int n_wp = pl.n_wp;
     CK(ctx->ilo_w.ensure(sizeof(int) * n_wp));
@@ -485,10 +487,17 @@ int band_sort(ll_ctx *ctx, const FullPlan &pl, long long n_w, bool standin, cons
     if (n_w <= 1024 && n_wp <= 1024) {
         const int max_items = n_items ? n_items + 32 : 0; // = the fused kernel's grid (every live group gets >= 1 item)
         if (n_items) CK(ctx->grp_tab.ensure(sizeof(int) * (grp_off_items() + 4 * (size_t)max_items)));
-        k_band_sort_small<<<1, 1024, 0, st>>>(standin ? 1 : 0, params, P, band, (int)n_w, n_wp, g, ctx->si, ctx->perm.as<int>(),
-                                              ctx->ilo_s.as<int>(), ctx->ihi_s.as<int>(), ctx->pairs.as<unsigned long long>(),
-                                              n_items, max_items, n_items ? ctx->grp_tab.as<int>() : nullptr,
-                                              n_items ? ctx->nt.bstart : nullptr, (int)ctx->nodes_host.size());
+        BandSortArgs ba;
+        ba.use_standin = standin ? 1 : 0; ba.params = params; ba.P = P; ba.band = band; ba.n_w = (int)n_w; ba.n_wp = n_wp;
+        ba.g = g; ba.si = ctx->si; ba.perm = ctx->perm.as<int>(); ba.ilo_s = ctx->ilo_s.as<int>(); ba.ihi_s = ctx->ihi_s.as<int>();
+        ba.pairs = ctx->pairs.as<unsigned long long>(); ba.n_items = n_items; ba.max_items = max_items;
+        ba.grp_tab = n_items ? ctx->grp_tab.as<int>() : nullptr; ba.bstart_g = n_items ? ctx->nt.bstart : nullptr;
+        ba.n_nodes = (int)ctx->nodes_host.size();
+        if (defer) {
+            *defer = ba;
+            return LL_OK;
+        }
+        k_band_sort_small<<<1, 1024, 0, st>>>(ba);
         LAUNCHED(ctx);
     } else {
         CK(cudaMemsetAsync(ctx->hist.p, 0, sizeof(int) * pl.n_keys, st));
@@ -598,10 +607,6 @@ int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, cons
     CK(ctx->TF.ensure(sizeof(double) * (size_t)n_m * 2 * n_c * n_wp));
     if (small) CK(ctx->part.ensure(sizeof(double) * (size_t)(n_items + 32) * NQ * 32));
     else if (!template_only) CK(ctx->part.ensure(sizeof(double) * (size_t)pl.n_tiles * NQ * n_wp));
-    {
-        const int rc_b = band_sort(ctx, pl, n_w, standin, params, P, band, st, n_items);
-        if (rc_b != LL_OK) return rc_b;
-    }
     // few systems (Module-1 sized batches): a block per four walkers of a system, scan-based sweeps (k_spline_block4), and on
     // the stand-in path the block evaluates its own node values (no k_nodes_standin launch, no Y); else one thread per system
     const long long n_sys = (long long)n_wp * ns * n_m;
@@ -617,8 +622,21 @@ int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, cons
         LL_SPL4_ATTR(true, NWK4);
         LL_SPL4_ATTR(false, NWK4);
 #undef LL_SPL4_ATTR
+        CK(cudaFuncSetAttribute(k_setup_small<NWK4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
         ctx->spl4_attr = true;
     }
+    // stand-in batches of up to 1024 walkers: planner, F1 and F2 in one launch (k_setup_small)
+    const bool merged = standin && block4 && n_w <= 1024 && n_wp <= 1024 &&
+                        sizeof(double) * (2 * (size_t)NWK4 * n_nodes + 1024) <= 200 * 1024;
+    BandSortArgs ba;
+    {
+        const int rc_b = band_sort(ctx, pl, n_w, standin, params, P, band, st, n_items, merged ? &ba : nullptr);
+        if (rc_b != LL_OK) return rc_b;
+    }
+    Spline4Args sa;
+    sa.Y = standin ? nullptr : ctx->Y.as<double>(); sa.C = ctx->C.as<double>(); sa.n_wp = n_wp; sa.n_nodes = n_nodes; sa.n_m = n_m;
+    sa.ns = ns; sa.nt = ctx->nt; sa.params = params; sa.P = P; sa.perm = ctx->perm.as<int>(); sa.si = ctx->si;
+    sa.TF = ctx->TF.as<double>();
     if (standin && block4) {
         // F1 happens inside F2 (below)
     } else if (standin) {
@@ -636,20 +654,12 @@ int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, cons
     }
     if (!(standin && block4)) LAUNCHED(ctx);
     {
-        if (block4) {
-#define LL_SPL4(N)                                                                                                         \
-    do {                                                                                                                   \
-        if (standin)                                                                                                       \
-            k_spline_block4<true, N><<<(unsigned)(n_sys / N), T4, smem4, st>>>(nullptr, ctx->C.as<double>(), n_wp, n_nodes, n_m, ns, \
-                                                                                ctx->nt, params, P, ctx->perm.as<int>(), ctx->si, \
-                                                                                ctx->TF.as<double>());                      \
-        else                                                                                                               \
-            k_spline_block4<false, N><<<(unsigned)(n_sys / N), T4, smem4, st>>>(ctx->Y.as<double>(), ctx->C.as<double>(), n_wp,     \
-                                                                                 n_nodes, n_m, ns, ctx->nt, nullptr, 0, nullptr, \
-                                                                                 ctx->si, nullptr);                         \
-    } while (0)
-            LL_SPL4(NWK4);
-#undef LL_SPL4
+        if (merged) {
+            const size_t smem_m = sizeof(double) * (2 * (size_t)NWK4 * n_nodes + 1024);
+            k_setup_small<NWK4><<<(unsigned)(n_sys / NWK4) + 1, 1024, smem_m, st>>>(sa, ba);
+        } else if (block4) {
+            if (standin) k_spline_block4<true, NWK4><<<(unsigned)(n_sys / NWK4), T4, smem4, st>>>(sa);
+            else k_spline_block4<false, NWK4><<<(unsigned)(n_sys / NWK4), T4, smem4, st>>>(sa);
         } else {
             dim3 grid(ceil_div(n_wp, 128), ns * n_m);
             k_spline<<<grid, 128, 0, st>>>(ctx->Y.as<double>(), ctx->C.as<double>(), n_wp, n_nodes, n_m, ns, ctx->nt);

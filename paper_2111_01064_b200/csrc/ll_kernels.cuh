@@ -203,12 +203,36 @@ __host__ __device__ constexpr int grp_off_t0() { return kGrpInts; }
 __host__ __device__ constexpr int grp_off_t1() { return kGrpInts + 1024; }
 __host__ __device__ constexpr int grp_off_items() { return kGrpInts + 2048; }
 constexpr int kMinItemCost = 64;
-__global__ void __launch_bounds__(1024)
-k_band_sort_small(int use_standin, const double *__restrict__ params, int P, const double *__restrict__ band, int n_w,
-                  int n_wp, GridInfo g, StandinInfo si, int *__restrict__ perm, int *__restrict__ ilo_s,
-                  int *__restrict__ ihi_s, unsigned long long *__restrict__ pairs, int n_items, int max_items,
-                  int *__restrict__ grp_tab, const int *__restrict__ bstart_g, int n_nodes)
+struct BandSortArgs {
+    int use_standin;
+    const double *params;
+    int P;
+    const double *band;
+    int n_w, n_wp;
+    GridInfo g;
+    StandinInfo si;
+    int *perm, *ilo_s, *ihi_s;
+    unsigned long long *pairs;
+    int n_items, max_items;
+    int *grp_tab;
+    const int *bstart_g;
+    int n_nodes;
+};
+// the body: one block of 1024 threads (k_band_sort_small, or the last block of k_setup_small)
+__device__ __forceinline__ void band_sort_small_body(const BandSortArgs &a)
 {
+    const int use_standin = a.use_standin, P = a.P, n_w = a.n_w, n_wp = a.n_wp, max_items = a.max_items, n_nodes = a.n_nodes;
+    const double *__restrict__ params = a.params;
+    const double *__restrict__ band = a.band;
+    const GridInfo g = a.g;
+    const StandinInfo &si = a.si;
+    int *__restrict__ perm = a.perm;
+    int *__restrict__ ilo_s = a.ilo_s;
+    int *__restrict__ ihi_s = a.ihi_s;
+    unsigned long long *__restrict__ pairs = a.pairs;
+    int n_items = a.n_items;
+    int *__restrict__ grp_tab = a.grp_tab;
+    const int *__restrict__ bstart_g = a.bstart_g;
     __shared__ int s_hi[1024];
     __shared__ int s_slo[1024], s_shi[1024]; // bands in sorted order
     __shared__ int s_bs[1024];               // the bin -> interval table, when it fits
@@ -327,6 +351,8 @@ k_band_sort_small(int use_standin, const double *__restrict__ params, int P, con
         grp_tab[grp_off_t1() + w] = s_first[grp] + t1;
     }
 }
+
+__global__ void __launch_bounds__(1024) k_band_sort_small(BandSortArgs a) { band_sort_small_body(a); }
 
 // exclusive scan of hist[0..n) in place (single block of 1024 threads, n <= 1024*8); starts[0..n] keeps a copy of the
 // bucket starts (starts[n] = total), since k_scatter uses hist as its cursors
@@ -754,23 +780,40 @@ __device__ __forceinline__ void affine_scan4_down(double &A, double &B, double *
     __syncthreads();
 }
 
+struct Spline4Args {
+    const double *Y;
+    double *C;
+    int n_wp, n_nodes, n_m, ns;
+    NodeTables nt;
+    const double *params;
+    int P;
+    const int *perm;
+    StandinInfo si;
+    double *TF;
+};
+// wsel[NWK]: the walkers at the block's sorted positions (-1: padding), STANDIN only
 template <bool STANDIN, int NWK>
-__global__ void __launch_bounds__(1024)
-k_spline_block4(const double *__restrict__ Y, double *__restrict__ C, int n_wp, int n_nodes, int n_m, int ns, NodeTables nt,
-                const double *__restrict__ params, int P, const int *__restrict__ perm, StandinInfo si, double *__restrict__ TF)
+__device__ __forceinline__ void spline_block4_body(const Spline4Args &a, const int *wsel, int block)
 {
+    const double *__restrict__ Y = a.Y;
+    double *__restrict__ C = a.C;
+    const int n_wp = a.n_wp, n_nodes = a.n_nodes, n_m = a.n_m, ns = a.ns, P = a.P;
+    const NodeTables &nt = a.nt;
+    const double *__restrict__ params = a.params;
+    const StandinInfo &si = a.si;
+    double *__restrict__ TF = a.TF;
     extern __shared__ double ssm[]; // ys[n][4], ds[n][4], xch[T]
     __shared__ double sA[128], sB[128];
     const int tid = threadIdx.x, T = blockDim.x, lane = tid & 31, wid = tid >> 5, nwarp = T >> 5;
     const int wl = tid % NWK, ct = tid / NWK, TT = T / NWK;
     const int nq4 = n_wp / NWK;
-    const int sys = blockIdx.x / nq4, p0 = (blockIdx.x - sys * nq4) * NWK;
+    const int sys = block / nq4, p0 = (block - sys * nq4) * NWK;
     const int m = sys / ns, kind = sys % ns;
     const int n = n_nodes;
     const size_t sw = (size_t)n_wp;
     double *ys = ssm, *ds = ys + NWK * n, *xch = ds + NWK * n;
     if (STANDIN) {
-        const int w = perm[p0 + wl];
+        const int w = wsel[wl];
         WalkerConst c = {0, 0, 0, 0, 0};
         const double *row = nullptr;
         if (w >= 0) {
@@ -863,6 +906,51 @@ k_spline_block4(const double *__restrict__ Y, double *__restrict__ C, int n_wp, 
         cc[2 * sw] = 0.5 * Mj;
         cc[3 * sw] = (Mn1 - Mj) * ih * kSixth;
     }
+}
+
+template <bool STANDIN, int NWK>
+__global__ void __launch_bounds__(1024) k_spline_block4(Spline4Args a)
+{
+    __shared__ int s_wsel[NWK];
+    if (STANDIN) {
+        if (threadIdx.x < NWK) s_wsel[threadIdx.x] = a.perm[(blockIdx.x % (a.n_wp / NWK)) * NWK + threadIdx.x];
+        __syncthreads();
+    }
+    spline_block4_body<STANDIN, NWK>(a, s_wsel, blockIdx.x);
+}
+
+// The whole set-up of a small stand-in batch in ONE launch of 1024-thread blocks: the last block is the planner
+// (band_sort_small_body: bands, sort, cost plan of the fused kernel), every other block is a spline block that does
+// not wait for the planner's sort — it ranks the walkers itself (every thread one band top, the same band_bins and
+// the same (top, index) order as the planner, so the two agree exactly) and keeps the NWK walkers whose ranks are its
+// sorted positions.  Three launches per call (set-up, fused, F4) instead of four.
+template <int NWK>
+__global__ void __launch_bounds__(1024) k_setup_small(Spline4Args a, BandSortArgs b)
+{
+    if (blockIdx.x == gridDim.x - 1) {
+        band_sort_small_body(b);
+        return;
+    }
+    __shared__ int s_top[1024];
+    __shared__ int s_wsel[NWK];
+    const int w = threadIdx.x;
+    long long lo = 0, hi = 0;
+    if (w < b.n_w) band_bins(b.use_standin, b.params, b.P, b.band, w, b.g, b.si, lo, hi);
+    s_top[w] = (w < b.n_w) ? (int)hi : INT_MAX;
+    if (w < NWK) s_wsel[w] = -1;
+    __syncthreads();
+    const int p0 = (blockIdx.x % (a.n_wp / NWK)) * NWK;
+    if (w < b.n_w) {
+        const int mine = (int)hi;
+        int rank = 0;
+        for (int k = 0; k < b.n_w; ++k) {
+            const int other = s_top[k];
+            rank += (other < mine) || (other == mine && k < w);
+        }
+        if (rank >= p0 && rank < p0 + NWK) s_wsel[rank - p0] = w;
+    }
+    __syncthreads();
+    spline_block4_body<true, NWK>(a, s_wsel, blockIdx.x);
 }
 
 // ---------------------------------------------------------------------------------------------------
