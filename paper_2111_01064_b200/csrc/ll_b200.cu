@@ -485,7 +485,9 @@ int band_sort(ll_ctx *ctx, const FullPlan &pl, long long n_w, bool standin, cons
     CK(ctx->pairs.ensure(sizeof(unsigned long long)));
     const GridInfo g{ctx->k_min, ctx->n_f, ctx->df};
     if (n_w <= 1024 && n_wp <= 1024) {
-        const int max_items = n_items ? n_items + 32 : 0; // = the fused kernel's grid (every live group gets >= 1 item)
+        // = the fused kernel's grid: rounding gives every live group at least one group item (up to 32 more than n_items)
+        // and every walker's lanes items one more than its share (up to n_wp more)
+        const int max_items = n_items ? n_items + 32 + n_wp : 0;
         if (n_items) CK(ctx->grp_tab.ensure(sizeof(int) * (grp_off_items() + 4 * (size_t)max_items)));
         BandSortArgs ba;
         ba.use_standin = standin ? 1 : 0; ba.params = params; ba.P = P; ba.band = band; ba.n_w = (int)n_w; ba.n_wp = n_wp;
@@ -493,6 +495,7 @@ int band_sort(ll_ctx *ctx, const FullPlan &pl, long long n_w, bool standin, cons
         ba.pairs = ctx->pairs.as<unsigned long long>(); ba.n_items = n_items; ba.max_items = max_items;
         ba.grp_tab = n_items ? ctx->grp_tab.as<int>() : nullptr; ba.bstart_g = n_items ? ctx->nt.bstart : nullptr;
         ba.n_nodes = (int)ctx->nodes_host.size();
+        ba.lanes = (ctx->n_m == 1 && ctx->precision == LL_PREC_FP64) ? 1 : 0; // the single-mode kernel with weight moments
         if (defer) {
             *defer = ba;
             return LL_OK;
@@ -605,7 +608,7 @@ int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, cons
     CK(ctx->Y.ensure(sizeof(double) * (size_t)n_m * ns * n_nodes * n_wp));
     CK(ctx->C.ensure(sizeof(double) * (size_t)(n_nodes - 1) * n_m * ns * 4 * n_wp));
     CK(ctx->TF.ensure(sizeof(double) * (size_t)n_m * 2 * n_c * n_wp));
-    if (small) CK(ctx->part.ensure(sizeof(double) * (size_t)(n_items + 32) * NQ * 32));
+    if (small) CK(ctx->part.ensure(sizeof(double) * (size_t)(n_items + 32 + pl.n_wp) * NQ * 32));
     else if (!template_only) CK(ctx->part.ensure(sizeof(double) * (size_t)pl.n_tiles * NQ * n_wp));
     // few systems (Module-1 sized batches): a block per four walkers of a system, scan-based sweeps (k_spline_block4), and on
     // the stand-in path the block evaluates its own node values (no k_nodes_standin launch, no Y); else one thread per system
@@ -616,18 +619,18 @@ int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, cons
     int T4 = 32 * NWK4;     // its threads: NWK4 walkers x ~8 rows per chunk thread, at most 512
     while (T4 < 512 && T4 < n_nodes * NWK4 / 8) T4 <<= 1;
     const size_t smem4 = sizeof(double) * (2 * (size_t)NWK4 * n_nodes + T4);
-    const bool block4 = n_sys <= (long long)ctx->sm_count * 32 && smem4 <= 200 * 1024;
+    const bool block4 = n_sys <= (long long)ctx->sm_count * 32 && smem4 <= 160 * 1024;
     if (block4 && !ctx->spl4_attr) {
-#define LL_SPL4_ATTR(S, N) CK(cudaFuncSetAttribute(k_spline_block4<S, N>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024))
+#define LL_SPL4_ATTR(S, N) CK(cudaFuncSetAttribute(k_spline_block4<S, N>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024))
         LL_SPL4_ATTR(true, NWK4);
         LL_SPL4_ATTR(false, NWK4);
 #undef LL_SPL4_ATTR
-        CK(cudaFuncSetAttribute(k_setup_small<NWK4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+        CK(cudaFuncSetAttribute(k_setup_small<NWK4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024));
         ctx->spl4_attr = true;
     }
     // stand-in batches of up to 1024 walkers: planner, F1 and F2 in one launch (k_setup_small)
     const bool merged = standin && block4 && n_w <= 1024 && n_wp <= 1024 &&
-                        sizeof(double) * (2 * (size_t)NWK4 * n_nodes + 1024) <= 200 * 1024;
+                        sizeof(double) * (2 * (size_t)NWK4 * n_nodes + 1024) <= 160 * 1024;
     BandSortArgs ba;
     {
         const int rc_b = band_sort(ctx, pl, n_w, standin, params, P, band, st, n_items, merged ? &ba : nullptr);
@@ -674,7 +677,7 @@ int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, cons
         return LL_OK;
     }
     if (small) {
-        const int grid = n_items + 32; // rounding gives every non-empty group at least one item: up to 32 more than n_items
+        const int grid = n_items + 32 + n_wp; // = max_items of the planner (band_sort)
         const size_t smem = (size_t)2 * pl.CH * 8 * (2 * n_c + nw);
         {
             ProfScope prof(ctx, st);

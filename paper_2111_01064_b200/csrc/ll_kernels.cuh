@@ -198,10 +198,49 @@ k_band_prep(int use_standin, const double *__restrict__ params, int P, const dou
 constexpr int kGrpStride = 33; // grp_tab: [0..32] first item of group g (entry 32 = total), then glo, ghi, cg, len [32] each,
 constexpr int kGrpInts = kGrpStride + 5 * 32; // then the tickets of k_finalize_small [32] (zeroed by the planner)
 __host__ __device__ constexpr int grp_off_ticket() { return kGrpStride + 4 * 32; }
-// after them: t0[1024], t1[1024] (items of sorted position p), then item[4][max_items] (group, i0, i1, j0)
+// after them: t0[1024], t1[1024] (group items of sorted position p), tb0[1024], tb1[1024] (its own lanes items), then
+// item[4][max_items] (group, or -(p + 1) for a lanes item of sorted position p; i0; i1; j0)
 __host__ __device__ constexpr int grp_off_t0() { return kGrpInts; }
 __host__ __device__ constexpr int grp_off_t1() { return kGrpInts + 1024; }
-__host__ __device__ constexpr int grp_off_items() { return kGrpInts + 2048; }
+__host__ __device__ constexpr int grp_off_tb0() { return kGrpInts + 2048; }
+__host__ __device__ constexpr int grp_off_tb1() { return kGrpInts + 3072; }
+__host__ __device__ constexpr int grp_off_items() { return kGrpInts + 4096; }
+// LANES ITEMS (single-mode FP64 kernel).  Inside a group of 32 sorted walkers the band tops differ (by x1.8 in the last
+// group of a 160-walker batch), and in group mode a lane whose band has ended rides along idle: measured 1.32x the warp-bins
+// a packed batch needs.  So a group's range is split at gsp = the lowest band top of its walkers: [glo, gsp) goes to group
+// items as before (every lane active), and the rest goes to lanes items: a SUB-GROUP of kLW neighbouring sorted walkers
+// x kLP = 32 / kLW bin phases (k_full_fused's fused_lanes_item): a row of kLP bins per step, idle lanes only where the tops
+// inside the sub-group differ.  (kLW = 1, a row of 32 bins of one walker, was measured first and lost: a spline interval is
+// then only a few rows long, so the per-lane re-synchronisation is never amortised, and every row pulls 1 KB from L2 for 25
+// FP64 instructions — 82 B/clk/SM, more than an SM can draw.  The fewer phases, the longer a lane stays inside one spline
+// interval and the fewer bytes a row needs.)  Lanes items are used only where the spline intervals are at
+// least kLaneMinInterval bins long.  Cost of a lanes item in the units of the group items: one per row of kLP bins plus
+// kLaneIntervalCost per interval.
+#ifndef LL_SMALL_LANES
+#define LL_SMALL_LANES 1
+#endif
+#ifndef LL_LANES_WALKERS
+#define LL_LANES_WALKERS 16 // 160 walkers on the config-2 grid, fused kernel: no lanes items 0.1454 ms; 4 walkers x 8 phases 0.148
+                            // (0.142 with the row cost at 130 %), 8 x 4: 0.147 (0.142), 16 x 2: 0.1291 (row cost 85 %: 0.154,
+                            // 110 %: 0.132, 130 %: 0.136); reading the data straight from L2 instead of the TMA ring: 0.142-0.156
+#endif
+constexpr int kLW = LL_LANES_WALKERS, kLP = 32 / kLW;
+#ifndef LL_LANE_INTERVAL_COST
+#define LL_LANE_INTERVAL_COST 8
+#endif
+constexpr int kLaneIntervalCost = LL_LANE_INTERVAL_COST;
+#ifndef LL_LANE_ROW_COST
+#define LL_LANE_ROW_COST 100
+#endif
+constexpr int kLaneRowCostPct = LL_LANE_ROW_COST; // cost of a lanes row in percent of a group item's bin
+#ifndef LL_LANE_MIN_BINS
+#define LL_LANE_MIN_BINS 2048
+#endif
+constexpr int kLaneMinBins = LL_LANE_MIN_BINS; // a group is split only when its tops differ by more than this
+#ifndef LL_LANE_MIN_INTERVAL
+#define LL_LANE_MIN_INTERVAL 256
+#endif
+constexpr int kLaneMinInterval = LL_LANE_MIN_INTERVAL; // and only above the first spline interval at least this long
 constexpr int kMinItemCost = 64;
 struct BandSortArgs {
     int use_standin;
@@ -217,6 +256,7 @@ struct BandSortArgs {
     int *grp_tab;
     const int *bstart_g;
     int n_nodes;
+    int lanes; // 1: the fused kernel can take lanes items (single mode, weight moments present)
 };
 // the body: one block of 1024 threads (k_band_sort_small, or the last block of k_setup_small)
 __device__ __forceinline__ void band_sort_small_body(const BandSortArgs &a)
@@ -282,13 +322,27 @@ __device__ __forceinline__ void band_sort_small_body(const BandSortArgs &a)
     if (!grp_tab) return;
     __syncthreads();
     const int n_groups = n_wp >> 5;
+    __shared__ long long s_UB;   // cost of all lanes items
+    __shared__ int s_lenB, s_totalA, s_nb[1024], s_rb0[1024], s_rb1[1024];
+    __shared__ int s_bL; // first bin of the first spline interval of at least kLaneMinInterval bins
+    if (w == 0) { s_UB = 0; s_bL = INT_MAX; }
+    __syncthreads();
+    if (LL_SMALL_LANES && a.lanes && bstart && w < n_nodes - 1 && bstart[w + 1] - bstart[w] >= kLaneMinInterval) atomicMin(&s_bL, bstart[w]);
+    for (int j = w + 1024; LL_SMALL_LANES && a.lanes && bstart && j < n_nodes - 1; j += 1024)
+        if (bstart[j + 1] - bstart[j] >= kLaneMinInterval) atomicMin(&s_bL, bstart[j]);
+    __syncthreads();
     if (w < 32) {
-        int glo = INT_MAX, ghi = INT_MIN;
+        int glo = INT_MAX, ghi = INT_MIN, gmin = INT_MAX;
         if (w < n_groups)
             for (int k = 0; k < 32; ++k) {
                 const int l = s_slo[w * 32 + k], h = s_shi[w * 32 + k];
-                if (h > l) { glo = min(glo, l); ghi = max(ghi, h); }
+                if (h > l) { glo = min(glo, l); ghi = max(ghi, h); gmin = min(gmin, h); }
             }
+        // group items cover [glo, gsp): up to the lowest band top when the tops differ enough to pay for lanes items
+        if (LL_SMALL_LANES && a.lanes && bstart && glo < ghi) {
+            const int gsp = max(gmin, min(ghi, s_bL));
+            if (ghi - gsp >= kLaneMinBins) ghi = gsp;
+        }
         int cg = 0;
         if (glo >= ghi) { glo = 0; ghi = 0; s_U[w] = 0; }
         else {
@@ -302,13 +356,36 @@ __device__ __forceinline__ void band_sort_small_body(const BandSortArgs &a)
         s_glo[w] = glo; s_ghi[w] = ghi; s_cg[w] = cg;
     }
     __syncthreads();
+    // the rest of a sub-group's bands above its group's items: [rb0, rb1), in lanes items (the sub-group's first thread)
+    int rb0 = 0, rb1 = 0, costB = 0;
+    if (w < n_wp && (w % kLW) == 0) {
+        int l = INT_MAX, h = INT_MIN;
+        for (int k = 0; k < kLW; ++k)
+            if (s_shi[w + k] > s_slo[w + k]) { l = min(l, s_slo[w + k]); h = max(h, s_shi[w + k]); }
+        if (h > l) {
+            rb0 = max(l, s_ghi[w >> 5]);
+            rb1 = h;
+            if (rb1 > rb0)
+                costB = (int)(((long long)((rb1 - rb0 + kLP - 1) / kLP) * kLaneRowCostPct) / 100) +
+                        kLaneIntervalCost * (interval_of_bin_tab(bstart, n_nodes, rb1 - 1) - interval_of_bin_tab(bstart, n_nodes, rb0) + 1);
+            else rb1 = rb0;
+        }
+    }
+    {
+        long long cb = costB;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) cb += __shfl_xor_sync(0xffffffffu, cb, o);
+        if ((w & 31) == 0 && cb) atomicAdd((unsigned long long *)&s_UB, (unsigned long long)cb); // integers: order-independent
+    }
+    __syncthreads();
     if (w == 0) {
-        long long U = 0;
+        long long U = s_UB;
         int n_live = 0;
         for (int k = 0; k < n_groups; ++k) { U += s_U[k]; n_live += s_U[k] > 0; }
+        if (U <= 0) U = 1;
         // tiny problems (config 0: 64 walkers x 6.5k bins) take fewer items than the grid has blocks — at least
         // kMinItemCost units each — and the blocks beyond them exit at once
-        n_items = (int)min((long long)n_items, max((long long)n_live, U / kMinItemCost));
+        n_items = (int)max(1LL, min((long long)n_items, max((long long)n_live, U / kMinItemCost)));
         int first = 0;
         for (int k = 0; k < 32; ++k) {
             grp_tab[k] = first;
@@ -320,12 +397,29 @@ __device__ __forceinline__ void band_sort_small_body(const BandSortArgs &a)
             s_len[k] = len;
             first += n_g;
         }
-        grp_tab[32] = first;
         s_first[32] = first;
+        s_totalA = first;
+        s_lenB = (int)max(1LL, (U + n_items - 1) / n_items);
     }
     __syncthreads();
+    // lanes items per walker, and their first index (exclusive scan over the sorted positions)
+    const int nb = costB ? (costB + s_lenB - 1) / s_lenB : 0;
+    s_nb[w] = nb;
+    s_rb0[w] = rb0;
+    s_rb1[w] = rb1;
+    __syncthreads();
+    for (int o = 1; o < 1024; o <<= 1) { // inclusive Hillis-Steele scan in shared memory
+        const int v = (w >= o) ? s_nb[w - o] : 0;
+        __syncthreads();
+        s_nb[w] += v;
+        __syncthreads();
+    }
+    const int totalA = s_totalA;
+    const int baseB = totalA + s_nb[w] - nb;
+    const int total_all = min(totalA + s_nb[1023], max_items);
+    if (w == 0) grp_tab[32] = total_all;
     // per item: group, bins [i0, i1), interval of i0
-    const int total = min(s_first[32], max_items);
+    const int total = min(totalA, max_items);
     int *it = grp_tab + grp_off_items();
     for (int id = w; id < total; id += 1024) {
         int grp = 0;
@@ -338,9 +432,28 @@ __device__ __forceinline__ void band_sort_small_body(const BandSortArgs &a)
         it[2 * max_items + id] = i1;
         it[3 * max_items + id] = bstart ? interval_of_bin_tab(bstart, n_nodes, i0) : 0;
     }
-    // per sorted position: first and last item its band touches
+    // the lanes items: item k of the sub-group led by sorted position L = an equal share of its [rb0, rb1), in multiples of
+    // 32 bins; every thread takes items (the leader of an item by bisection of the scanned counts)
+    for (int id = totalA + w; id < total_all; id += 1024) {
+        const int rel = id - totalA;
+        int lo_ = 0, hi_ = 1023; // smallest L with s_nb[L] > rel
+        while (lo_ < hi_) {
+            const int mid = (lo_ + hi_) >> 1;
+            if (s_nb[mid] > rel) hi_ = mid; else lo_ = mid + 1;
+        }
+        const int L = lo_, before = L ? s_nb[L - 1] : 0;
+        const int nbL = s_nb[L] - before, k = rel - before;
+        const int r0 = s_rb0[L], r1 = s_rb1[L];
+        const int per = ((r1 - r0 + nbL - 1) / nbL + 31) & ~31;
+        const int i0 = min(r0 + k * per, r1), i1 = min(i0 + per, r1);
+        it[id] = -(L + 1);
+        it[max_items + id] = i0;
+        it[2 * max_items + id] = i1;
+        it[3 * max_items + id] = interval_of_bin_tab(bstart, n_nodes, i0);
+    }
+    // per sorted position: first and last group item its band touches, and its own lanes items
     if (w < n_wp) {
-        const int grp = w >> 5, l = s_slo[w], h = s_shi[w];
+        const int grp = w >> 5, l = s_slo[w], h = min(s_shi[w], s_ghi[grp]);
         const int n_g = s_first[grp + 1] - s_first[grp];
         int t0 = 0, t1 = -1;
         if (h > l && n_g > 0) {
@@ -349,6 +462,11 @@ __device__ __forceinline__ void band_sort_small_body(const BandSortArgs &a)
         }
         grp_tab[grp_off_t0() + w] = s_first[grp] + t0;
         grp_tab[grp_off_t1() + w] = s_first[grp] + t1;
+        // its sub-group's lanes items (the scan's values of the sub-group's first thread)
+        const int L = w - w % kLW;
+        const int incl = s_nb[L], before = L ? s_nb[L - 1] : 0;
+        grp_tab[grp_off_tb0() + w] = totalA + before;
+        grp_tab[grp_off_tb1() + w] = min(totalA + incl, max_items) - 1;
     }
 }
 
@@ -1324,6 +1442,148 @@ __device__ __forceinline__ void fused_bins_rot(int b0, int b1, int tlo, int thi,
     }
 }
 
+// A LANES ITEM of the small-batch kernel (planner: band_sort_small_body's lanes items): bins [i0, i1) of the kLW walkers at
+// sorted positions p0 .. p0 + kLW - 1.  Lane = (walker wl = lane % kLW, bin phase ph = lane / kLW): row r holds the bins
+// kLP r .. kLP r + kLP - 1, and a lane always takes the bins = ph (mod kLP) of its walker — a uniform sequence of stride
+// kLP df, so inside one spline interval it advances e^{-i Psi} and A by the recurrence of fused_bins_rot with df -> kLP df
+// (its own z, w, v, u and amplitude differences), re-synchronised from the walker's cubic coefficients every kLaneSync
+// rows and at every interval; outside its walker's band, or the stretch, a lane carries amplitude 0.  <h|h> of a walker's
+// stretch comes from the weight moments (one evaluation per stretch, added by the walker's phase-0 lane).  The data are
+// read straight from L2/L1 (a row is kLP x 2 NC doubles, each broadcast to kLW lanes), not through the TMA ring.  At the
+// end the phases of a walker are added by a butterfly (a fixed order) and its phase-0 lane writes the walker's slot of
+// the item's record.
+constexpr int kLaneSync = 128;
+template <int NC, bool WS>
+__device__ __forceinline__ void fused_lanes_item(const FusedArgs &a, int pw, int lo, int hi, int wlo, int whi, int j, int item,
+                                                 double *sm, uint64_t *bar)
+{
+    // pw: this lane's walker, [lo, hi): its bins in the item (empty: lo >= hi), [wlo, whi): the union over the warp
+    using TL = Tile<NC, WS>;
+    constexpr int NW = Acc1<NC, WS>::NW, NQ = 2 * NC + NW;
+    const int lane = threadIdx.x, ph = lane / kLW;
+    double S[2 * NC], H[NW];
+#pragma unroll
+    for (int q = 0; q < 2 * NC; ++q) S[q] = 0.0;
+#pragma unroll
+    for (int q = 0; q < NW; ++q) H[q] = 0.0;
+    const int CH = a.CH; // a multiple of kLP
+    const int c_begin = wlo / CH, c_end = (whi + CH - 1) / CH;
+    if (lane == 0) TL::issue(a, sm, c_begin, CH, &bar[0]);
+    const size_t sw = (size_t)a.n_wp;
+    const size_t cj = (size_t)a.n_m * 8 * sw;
+    const int kbase = (int)a.k_min;
+    const double df = a.df, h = (double)kLP * df, h2 = h * h, h3 = h2 * h;
+    double ts4 = 0.0;
+    if (a.t_shift) {
+        const int w = a.perm[pw];
+        if (w >= 0) ts4 = 4.0 * a.t_shift[(size_t)w * a.ts_stride];
+    }
+    // the interval's cubics of this lane's walker and the lane's recurrence state: they live across chunks
+    double cA0 = 0, cA1 = 0, cA2 = 0, cA3 = 0, cP0 = 0, cP1 = 0, cP2 = 0, cP3 = 0, nxj = 0;
+    double A = 0, d1A = 0, d2A = 0, d3A = 0, sz = 0, cz = 1, sw_ = 0, cw = 1, sv = 0, cv = 1, su = 0, cu = 1;
+    int jl = -1, steps = kLaneSync; // rows since the last re-synchronisation
+    for (int c = c_begin; c < c_end; ++c) {
+        const int st = (c - c_begin) & 1;
+        const uint32_t par = (uint32_t)((c - c_begin) >> 1) & 1u;
+        if (lane == 0 && c + 1 < c_end) TL::issue(a, sm + (size_t)(st ^ 1) * CH * TL::DPB, c + 1, CH, &bar[st ^ 1]);
+        mbar_wait(&bar[st], par);
+        const double *sg = sm + (size_t)st * CH * TL::DPB;
+        const int cb = c * CH;
+        const double *sgc = sg - (size_t)cb * 2 * NC; // addressed by global bin
+        const int ce = min(cb + CH, whi);
+        int i = max(cb, wlo);
+        while (i < ce) {
+            while (j < a.n_nodes - 2 && __ldg(a.bstart + j + 1) <= i) ++j;
+            const int j_end = (j < a.n_nodes - 2) ? __ldg(a.bstart + j + 1) : INT_MAX; // end of the interval
+            const int seg_end = min(j_end, ce);
+            if (j != jl) {
+                const double *cc = a.C + (size_t)j * cj + pw;
+                cA0 = cc[0]; cA1 = cc[sw]; cA2 = cc[2 * sw]; cA3 = cc[3 * sw];
+                cP0 = cc[4 * sw]; cP1 = cc[5 * sw]; cP2 = cc[6 * sw]; cP3 = cc[7 * sw];
+                const double xj = __ldg(a.xj + j);
+                nxj = -xj;
+                if (a.t_shift) { cP0 += qc_linear_mod_cycle(xj, ts4); cP1 += ts4; }
+                // <h|h> of the walker's whole stretch in this interval, [m0, m1), from the weight moments
+                const int m0 = max(i, lo), m1 = min(min(j_end, whi), hi);
+                if (ph == 0 && m0 < m1) {
+                    const bool first = m0 == __ldg(a.bstart + j);
+                    const double q0 = cA0 * cA0, q1 = 2.0 * cA0 * cA1, q2 = fma(2.0 * cA0, cA2, cA1 * cA1);
+                    const double q3 = 2.0 * fma(cA0, cA3, cA1 * cA2), q4 = fma(2.0 * cA1, cA3, cA2 * cA2);
+                    const double q5 = 2.0 * cA2 * cA3, q6 = cA3 * cA3;
+#pragma unroll
+                    for (int r = 0; r < NW; ++r) {
+                        const double *Q = a.wmom + (size_t)(r * 7) * a.n_f_pad;
+                        auto mo = [&](int q) { return __ldg(Q + (size_t)q * a.n_f_pad + m1 - 1) - (first ? 0.0 : __ldg(Q + (size_t)q * a.n_f_pad + m0 - 1)); };
+                        double hs = q0 * mo(0);
+                        hs = fma(q1, mo(1), hs); hs = fma(q2, mo(2), hs); hs = fma(q3, mo(3), hs);
+                        hs = fma(q4, mo(4), hs); hs = fma(q5, mo(5), hs); hs = fma(q6, mo(6), hs);
+                        H[r] += hs;
+                    }
+                }
+                d3A = 6.0 * cA3 * h3;
+                LL_ROT_SINCOS(6.0 * cP3 * h3, su, cu);
+                unit_modulus(cu, su);
+                steps = kLaneSync; // forces a re-synchronisation below
+                jl = j;
+            }
+            const int b0 = max(i, lo), b1 = min(seg_end, hi); // this lane's walker inside the stretch
+            const int r_end = (seg_end - 1) / kLP;
+            int r = i / kLP;
+            while (r <= r_end) {
+                if (steps >= kLaneSync) { // this lane's state at its bin of row r, from the cubics
+                    const double t = fma((double)(kbase + kLP * r + ph), df, nxj);
+                    const double tt = fma(2.0, t, h), q3 = fma(3.0 * t, t + h, h2), t1 = t + h;
+                    A = fma(fma(fma(cA3, t, cA2), t, cA1), t, cA0);
+                    d1A = h * fma(cA3, q3, fma(cA2, tt, cA1));
+                    d2A = h2 * fma(6.0 * cA3, t1, 2.0 * cA2);
+                    LL_ROT_SINCOS(fma(fma(fma(cP3, t, cP2), t, cP1), t, cP0), sz, cz);
+                    LL_ROT_SINCOS(h * fma(cP3, q3, fma(cP2, tt, cP1)), sw_, cw);
+                    LL_ROT_SINCOS(h2 * fma(6.0 * cP3, t1, 2.0 * cP2), sv, cv);
+                    unit_modulus(cz, sz);
+                    unit_modulus(cw, sw_);
+                    unit_modulus(cv, sv);
+                    steps = 0;
+                }
+                const int r1 = min(r_end, r + (kLaneSync - steps) - 1);
+                steps += r1 - r + 1;
+#pragma unroll 4
+                for (; r <= r1; ++r) {
+                    const int ii = kLP * r + ph;
+                    const double Am = (ii >= b0 && ii < b1) ? A : 0.0;
+                    const double u = Am * cz, v = Am * sz; // h = u - i v
+                    double g[2 * NC];
+                    load_g<NC>(sgc, ii, g);
+#pragma unroll
+                    for (int cch = 0; cch < NC; ++cch) {
+                        S[2 * cch] = fma(g[2 * cch], u, S[2 * cch]); S[2 * cch] = fma(g[2 * cch + 1], v, S[2 * cch]);
+                        S[2 * cch + 1] = fma(g[2 * cch + 1], u, S[2 * cch + 1]); S[2 * cch + 1] = fma(-g[2 * cch], v, S[2 * cch + 1]);
+                    }
+                    const double nzc = fma(cz, cw, -(sz * sw_)), nzs = fma(sz, cw, cz * sw_);
+                    const double nwc = fma(cw, cv, -(sw_ * sv)), nws = fma(sw_, cv, cw * sv);
+                    const double nvc = fma(cv, cu, -(sv * su)), nvs = fma(sv, cu, cv * su);
+                    cz = nzc; sz = nzs; cw = nwc; sw_ = nws; cv = nvc; sv = nvs;
+                    A += d1A; d1A += d2A; d2A += d3A;
+                }
+            }
+            // a row that straddles the end of the interval is taken again by the next interval (complementary mask)
+            i = seg_end;
+        }
+        poison_stage(sg, CH * TL::DPB);
+        __syncthreads(); // (one warp) done with stage st before it is refilled two chunks later
+    }
+#pragma unroll
+    for (int q = 0; q < 2 * NC; ++q)
+#pragma unroll
+        for (int o = kLW; o < 32; o <<= 1) S[q] += __shfl_xor_sync(0xffffffffu, S[q], o); // over the phases of a walker
+    if (ph == 0) {
+        double *o = a.part + (size_t)item * NQ * 32 + (pw & 31);
+#pragma unroll
+        for (int q = 0; q < 2 * NC; ++q) o[q * 32] = S[q];
+#pragma unroll
+        for (int q = 0; q < NW; ++q) o[(2 * NC + q) * 32] = H[q];
+    }
+}
+
 // NM1 = 1: single-mode specialisation (NQ = 2 NC + NW partial sums per walker and tile); 0: any n_m (NQ = 2).
 // SMALL = 1 (batches of up to 1024 walkers; blocks of ONE warp): block b is item b of the group table — bins
 // [i0, i1) of one group of 32 walkers, an equal share of the batch's active bins — instead of (walker block, tile);
@@ -1349,6 +1609,7 @@ k_full_fused(FusedArgs a)
 
     const int tid = threadIdx.x;
     int p, tile, i0, i1, j_hint = 0;
+    bool lanes_item = false;
     if (SMALL) {
         tile = blockIdx.x;
         if (tile >= __ldg(a.grp_tab + 32)) return;
@@ -1357,7 +1618,9 @@ k_full_fused(FusedArgs a)
         i0 = __ldg(it + mi);
         i1 = __ldg(it + 2 * mi);
         j_hint = __ldg(it + 3 * mi);
-        p = __ldg(it) * 32 + tid;
+        const int code = __ldg(it);
+        lanes_item = NM1 && LL_SMALL_LANES && code < 0; // kLW walkers from sorted position -code - 1 on, lanes = (walker, phase)
+        p = lanes_item ? (-code - 1) + tid % kLW : code * 32 + tid;
     } else {
         p = blockIdx.x * blockDim.x + tid;
         tile = blockIdx.y;
@@ -1388,6 +1651,10 @@ k_full_fused(FusedArgs a)
         return; // large batches: k_finalize never reads it
     }
 
+    if (SMALL && NM1 && LL_SMALL_LANES && lanes_item) {
+        fused_lanes_item<NC, WS>(a, p, lo, hi, blo, bhi, j_hint, tile, sm, bar);
+        return;
+    }
     const int CH = a.CH;
     const int c_begin = blo / CH, c_end = (bhi + CH - 1) / CH;
     if (tid == 0) TL::issue(a, sm, c_begin, CH, &bar[0]);
@@ -2522,13 +2789,17 @@ k_finalize_small(const double *__restrict__ part, double *__restrict__ part2, co
     double acc[NQ];
 #pragma unroll
     for (int q = 0; q < NQ; ++q) acc[q] = 0.0;
-    const int t0 = grp_tab[grp_off_t0() + p], t1 = grp_tab[grp_off_t1() + p]; // items the walker's band touches
-    const int first = t0 + ((z - t0 % kFinZ) + kFinZ) % kFinZ;              // the first of them with t = z (mod kFinZ)
-#pragma unroll 4
-    for (int t = first + ty * kFinZ; t <= t1; t += FY * kFinZ) {
-        const double *o = part + (size_t)t * NQ * 32 + lane;
+    // the group items the walker's band touches, then its own lanes items (its slot of their records)
 #pragma unroll
-        for (int q = 0; q < NQ; ++q) acc[q] += o[q * 32];
+    for (int range = 0; range < 2; ++range) {
+        const int t0 = grp_tab[(range ? grp_off_tb0() : grp_off_t0()) + p], t1 = grp_tab[(range ? grp_off_tb1() : grp_off_t1()) + p];
+        const int first = t0 + ((z - t0 % kFinZ) + kFinZ) % kFinZ; // the first of them with t = z (mod kFinZ)
+#pragma unroll 4
+        for (int t = first + ty * kFinZ; t <= t1; t += FY * kFinZ) {
+            const double *o = part + (size_t)t * NQ * 32 + lane;
+#pragma unroll
+            for (int q = 0; q < NQ; ++q) acc[q] += o[q * 32];
+        }
     }
 #pragma unroll
     for (int q = 0; q < NQ; ++q) red[ty][q][lane] = acc[q];
