@@ -415,7 +415,10 @@ FullPlan make_plan(const ll_ctx *ctx, long long n_w)
 // change costs one dependent global load of the coefficients (~14 bins' worth of arithmetic) and log-spaced nodes
 // put dozens of intervals into the first tiles of the grid; cost = bins + 14 per interval <= TB.
 constexpr int kTileChunk = 64;
-constexpr int kSmallWarpsPerSM = 16; // one-warp blocks of the small-batch fused kernel resident per SM (register limit)
+// work items of the small-batch fused kernel per SM (16 one-warp blocks are resident per SM, by registers).  160 walkers on the
+// config-2 grid with lanes items: 12 per SM 0.161 ms, 16: 0.129, 20: 0.138, 24: 0.1249, 28: 0.1249, 32: 0.1254, 48: 0.1265, 64: 0.128
+// (the plan and F4 grow with the item count: whole call 0.1705 at 16, 0.1667 at 24, 0.175 at 48)
+constexpr int kSmallWarpsPerSM = 24;
 int ensure_tiles(ll_ctx *ctx, FullPlan &pl, cudaStream_t st, bool uniform = false)
 {
     const int small = uniform ? 2 : (pl.n_wp <= 1024 ? 1 : 0); // 2: per-walker node grids, no shared interval table
