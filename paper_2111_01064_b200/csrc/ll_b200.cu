@@ -632,7 +632,9 @@ int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, cons
         ctx->spl4_attr = true;
     }
     // stand-in batches of up to 1024 walkers: planner, F1 and F2 in one launch (k_setup_small)
-    const bool merged = standin && block4 && n_w <= 1024 && n_wp <= 1024 &&
+    // (up to 512 walkers: every spline block ranks all walkers itself, O(n_w) per thread — measured whole call, merged against
+    // separate launches: 160 walkers 0.167 / 0.190 ms, 320: 0.287 / 0.298, 480: 0.444 / 0.453, 640: 0.605 / 0.587, 1024: 1.00 / 0.91)
+    const bool merged = standin && block4 && n_w <= 512 && n_wp <= 1024 &&
                         sizeof(double) * (2 * (size_t)NWK4 * n_nodes + 1024) <= 160 * 1024;
     BandSortArgs ba;
     {
