@@ -380,7 +380,9 @@ int prepare_nodes(ll_ctx *ctx, int n, const double *x, cudaStream_t st)
 FullPlan make_plan(const ll_ctx *ctx, long long n_w)
 {
     FullPlan pl;
-    pl.WB = (n_w >= 4096) ? 128 : (n_w >= 1024 ? 64 : 32);
+    // blocks of 128 walkers above 1024 walkers (64-walker blocks between 1024 and 4096, as in round 1, measured worse: 2048
+    // walkers on the config-2 grid frac 0.60 with 64 x 512-bin stages, 0.69 with 64 x 256, 0.73 with 128 x 512; 3072: 0.63 / 0.73 / 0.76)
+    pl.WB = (n_w > 1024) ? 128 : (n_w >= 1024 ? 64 : 32);
     pl.n_wp = (int)round_up(std::max<long long>(n_w, 1), pl.WB);
     const int n_wb = pl.n_wp / pl.WB;
     // aim at ~16 blocks per SM over the whole grid, tiles between 64 and LL_FUSED_TB_MAX bins.  Small batches (blocks of one
@@ -403,7 +405,8 @@ FullPlan make_plan(const ll_ctx *ctx, long long n_w)
     // (other layouts keep 256-bin stages: with 9 doubles per bin two 512-bin stages would pass the 48 KB a launch gets
     // without opting in, and hold an SM to three blocks;
     // and the multi-mode kernel measured 24.8 ms with 256-bin stages against 28.0 ms with 512 at six modes)
-    pl.CH = std::min(TB, pl.WB == 32 ? LL_SMALL_CH : ((ctx->n_c == 2 && ctx->w_rows == 1 && ctx->n_m == 1) ? LL_FUSED_CH : 256));
+    constexpr int mid_ch = 256; // 64-walker blocks (exactly 1024 walkers that do not take the small route)
+    pl.CH = std::min(TB, pl.WB == 32 ? LL_SMALL_CH : ((ctx->n_c == 2 && ctx->w_rows == 1 && ctx->n_m == 1) ? (pl.WB == 64 ? mid_ch : LL_FUSED_CH) : 256));
     pl.n_tiles = ceil_div(ctx->n_f, TB);
     pl.key_gran = std::max(1, ceil_div(ctx->n_f, 4096));
     pl.n_keys = (int)(ctx->n_f / pl.key_gran) + 2;
