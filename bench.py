@@ -355,8 +355,8 @@ def bench_small_batch(torch, ctx, wl, params, peak_slots, n_w: int = 160, steps:
     ctx.profile_enable(False)
     pairs = ctx.last_full_stats()[0]
     k = kms / max(kn, 1)
-    return {"call_160": {"n_walkers": n_w, "ms_per_batch": ms, "kernel_ms": k, "units": pairs, "slots_per_unit": SLOTS_FULL,
-                         "frac": pairs * SLOTS_FULL / (k * 1e-3) / peak_slots}}
+    return {"call_%d" % n_w: {"n_walkers": n_w, "ms_per_batch": ms, "kernel_ms": k, "units": pairs, "slots_per_unit": SLOTS_FULL,
+                              "frac": pairs * SLOTS_FULL / (k * 1e-3) / peak_slots}}
 
 
 def bench_full_hm(torch, steps: int = 5, n_w: int = 2048):
@@ -833,6 +833,12 @@ def main():
                                                                f_nodes=wl2.f_nodes)
             per["module1_iteration"]["covered_by"] = COVERED_BY["module1_iteration"]
             per["module1_iteration"].update(bench_small_batch(torch, c2, wl2, b2["params"], peak_slots))
+            # ---- the same likelihood call over the batch sizes between Module 1's and config 2's (first n walkers of config 2):
+            # the small-batch route up to 1024 walkers, the large-batch route above
+            sizes = {}
+            for n in (37, 320, 1024, 2048, 4096):
+                sizes.update(bench_small_batch(torch, c2, wl2, b2["params"], peak_slots, n_w=n, steps=10))
+            per["cfg2_batch_sizes"] = sizes
             c2.destroy()
             del amp, ph, tfn, b2
             torch.cuda.empty_cache()
