@@ -219,3 +219,59 @@ def test_cfg2_split_tc_full_size_sampled(cfg2, orc, torch_cuda):
     e_plain = np.abs(plain[1] - ref_full["d_h"]).max()
     print(f"max |d_h - oracle|: split t_c {e_split:.3e}, full-phase spline {e_plain:.3e}; "
           f"oracle split vs oracle full {np.abs(ref['d_h'] - ref_full['d_h']).max():.3e}")
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# The small-batch route's LANES ITEMS (ll_kernels.cuh: a group's range above its lowest band top goes to sub-groups of 16
+# walkers x 2 bin phases) exist only where the spline intervals are long, i.e. on this grid; the tests above cover them for
+# the stand-in entry point with two channels.  The other ways into the same kernel, at Module-1 size:
+def test_small_batch_three_channels_against_oracle(orc, torch_cuda):
+    """160 walkers, three channels with per-channel PSDs (k_full_fused<1, 3, false, SMALL>: the lanes items' <h|h> from the
+    moments of every weight row), one-year grid, against the oracle."""
+    wl = wlm.make_workload(2, n_c=3)
+    d, run = oracle_setup_full(orc, wl)
+    ctx = make_ctx(wl)
+    g = wl.grid
+    tc = torch_cuda
+    ctx.set_data(g.n_f, g.k_min, g.df, dev(tc, d), dev(tc, wl.W))
+    rng = np.random.default_rng(1943)
+    idx = rng.choice(wl.n_w, 160, replace=False)
+    idx[0] = 0
+    params = wl.params[idx]
+    got = [x.cpu().numpy() for x in ctx.full_batch_standin(wl.f_nodes, dev(tc, params))]
+    sample = np.unique(np.r_[0, 15, 16, 31, 32, 159, rng.integers(0, 160, 18)])
+    check_triplet(_np_triplet(got, sample), run(params[sample], d), "three channels, 160 walkers")
+    ctx.destroy()
+
+
+def test_small_batch_split_tc_and_arrays_against_oracle(cfg2, orc, torch_cuda):
+    """160 walkers through (i) the stand-in entry point with 2 pi f t_c kept outside the spline (t_shift folded into the
+    lanes items' phase cubic) and (ii) the array entry point ll_full_batch with per-walker bands and t_shift (planner, node
+    transposition and spline as separate launches; bands with different bottoms), both against the oracle."""
+    wl, d, run, ctx, fis = cfg2
+    g = wl.grid
+    tc = torch_cuda
+    rng = np.random.default_rng(1944)
+    idx = rng.choice(wl.n_w, 160, replace=False)
+    params = wl.params[idx]
+    sample = np.unique(np.r_[0, 15, 16, 31, 32, 159, rng.integers(0, 160, 14)])
+    # (i)
+    ctx.standin_split_tc(True)
+    try:
+        got = [x.cpu().numpy() for x in ctx.full_batch_standin(wl.f_nodes, dev(tc, params))]
+    finally:
+        ctx.standin_split_tc(False)
+    ref = orc.full_batch_standin(wl.modes_m, wl.c_lm, wl.kappa, params[sample], wl.f_nodes, g.k_min, g.df, g.n_f, d, wl.W,
+                                 split_tc=True)
+    check_triplet(_np_triplet(got, sample), ref, "split t_c, 160 walkers")
+    # (ii) numpy-generated node arrays, the linear term as t_shift, bands starting at different bins
+    amp, phase, top = lisa_node_arrays(params, wl.f_nodes)
+    phase = phase - 2.0 * np.pi * wl.f_nodes[None, None, :] * params[:, 2][:, None, None]
+    band = np.stack([wlm.F_LO * (1.0 + 3.0 * rng.random(160)), top], axis=1)
+    tf = np.ascontiguousarray(params[:, 5:9].reshape(160, 1, 2, 2))
+    ts = np.ascontiguousarray(params[:, 2])
+    got = [x.cpu().numpy() for x in ctx.full_batch(wl.f_nodes, dev(tc, amp), dev(tc, phase), dev(tc, tf), dev(tc, band),
+                                                   t_shift=dev(tc, ts))]
+    ref = orc.full_batch(wl.f_nodes, amp[sample], phase[sample], tf[sample], band[sample], g.k_min, g.df, d, wl.W,
+                         t_shift=ts[sample])
+    check_triplet(_np_triplet(got, sample), ref, "array entry point, 160 walkers")
