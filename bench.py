@@ -838,6 +838,7 @@ def main():
             sizes = {}
             for n in (37, 320, 1024, 2048, 4096):
                 sizes.update(bench_small_batch(torch, c2, wl2, b2["params"], peak_slots, n_w=n, steps=10))
+            sizes["covered_by"] = "tests/test_parity_cfg2_scale.py::test_module1_sized_batches_against_oracle (37 ... 2048), test_cfg2_full_size_128_walkers"
             per["cfg2_batch_sizes"] = sizes
             c2.destroy()
             del amp, ph, tfn, b2

@@ -70,11 +70,12 @@ def test_cfg2_full_size_128_walkers(cfg2, torch_cuda):
     check_triplet(_np_triplet(got, sample), ref, "cfg2 full size, 128+ walkers")
 
 
-@pytest.mark.parametrize("n_small", [37, 160, 320])
+@pytest.mark.parametrize("n_small", [37, 160, 320, 1024, 2048])
 def test_module1_sized_batches_against_oracle(cfg2, torch_cuda, n_small):
     """Module-1 sized batches on the one-year grid (80 walkers x 4 temperatures; a half update is 160
     proposals, a whole population 320): the small-batch route (per_config.module1_iteration) against the ORACLE, not
-    only against the large-batch route."""
+    only against the large-batch route.  1024: the largest batch of the small-batch route (32 groups); 2048: the
+    large-batch route just above it (per_config.cfg2_batch_sizes)."""
     wl, d, run, ctx, fis = cfg2
     rng = np.random.default_rng(194 + n_small)
     idx = rng.choice(wl.n_w, n_small, replace=False)
