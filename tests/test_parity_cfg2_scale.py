@@ -276,3 +276,33 @@ def test_small_batch_split_tc_and_arrays_against_oracle(cfg2, orc, torch_cuda):
     ref = orc.full_batch(wl.f_nodes, amp[sample], phase[sample], tf[sample], band[sample], g.k_min, g.df, d, wl.W,
                          t_shift=ts[sample])
     check_triplet(_np_triplet(got, sample), ref, "array entry point, 160 walkers")
+
+
+@pytest.mark.parametrize("n", [1, 17, 33, 49, 257, 513])
+def test_small_batch_odd_sizes_and_bands(cfg2, orc, torch_cuda, n):
+    """The planner's corner cases on the one-year grid: batch sizes that leave sub-groups and groups partly empty, walkers
+    with identical bands (no ragged part: n divisible by 3), and — through the array entry point — bands that are empty,
+    a few bins wide, or start high on the grid; 513 walkers take the separate-launch set-up.  Sampled walkers vs the oracle;
+    the guard bands of every internal buffer afterwards."""
+    wl, d, run, ctx, fis = cfg2
+    g = wl.grid
+    tc = torch_cuda
+    rng = np.random.default_rng(3000 + n)
+    p = wl.params[rng.choice(wl.n_w, n, replace=False)].copy()
+    if n % 3 == 0:
+        p[:, 0], p[:, 1] = p[0, 0], p[0, 1]
+    s = np.unique(np.r_[0, n - 1, rng.integers(0, n, 8)])
+    got = [x.cpu().numpy() for x in ctx.full_batch_standin(wl.f_nodes, dev(tc, p))]
+    check_triplet(_np_triplet(got, s), run(p[s], d), f"stand-in entry, {n} walkers")
+    amp, phase, top = lisa_node_arrays(p, wl.f_nodes)
+    lo = wlm.F_LO * (1.0 + 20.0 * rng.random(n) ** 3)
+    hi = np.where(rng.random(n) < 0.1, 0.5 * lo, np.minimum(top, lo * (1.0 + 50.0 * rng.random(n))))  # 10 % empty bands
+    if n >= 4:
+        hi[1] = lo[1] * 1.0001          # a handful of bins
+        lo[2], hi[2] = 0.03, 0.05       # only the top of the grid
+    band = np.stack([lo, hi], axis=1)
+    tf = np.ascontiguousarray(p[:, 5:9].reshape(n, 1, 2, 2))
+    got = [x.cpu().numpy() for x in ctx.full_batch(wl.f_nodes, dev(tc, amp), dev(tc, phase), dev(tc, tf), dev(tc, band))]
+    ref = orc.full_batch(wl.f_nodes, amp[s], phase[s], tf[s], band[s], g.k_min, g.df, d, wl.W)
+    check_triplet(_np_triplet(got, s), ref, f"array entry, {n} walkers")
+    assert ctx.debug_check() == 0
