@@ -150,6 +150,7 @@ struct ll_ctx {
     int coop = -1;                 // device supports cooperative launches (-1: not asked yet)
     bool ptrun_attr = false;
     bool spl4_attr = false;
+    bool hm_attr = false;
     double *static_scratch = nullptr; // device address of g_ll_static_scratch on this context's device (ll_create)
     HetTable ht{};
     Het1Table ht1{}; // single-mode regrouped table (k_het_standin1); base == nullptr when not built
@@ -720,6 +721,15 @@ int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, cons
         dim3 grid(n_wp / pl.WB, pl.n_tiles);
         const bool mixed = ctx->precision == LL_PREC_FP32_ACC && !tfp;
         const size_t smem = (size_t)2 * pl.CH * (mixed ? 24 : 8 * (2 * n_c + nw));
+        // several modes, the BASELINE layout, FP64, blocks of 128 walkers: the recurrence kernel (instantiated for 3 and 6 modes)
+        const int hm_rot = (!nm1 && !tfp && !mixed && ctx->precision == LL_PREC_FP64 && n_c == 2 && nw == 1 && pl.WB == 128 &&
+                            (n_m == 3 || n_m == 6)) ? n_m : 0;
+        const size_t smem_hm = smem + sizeof(double) * (size_t)n_m * (3 + 2 * n_c) * 128;
+        if (hm_rot && !ctx->hm_attr) {
+            CK(cudaFuncSetAttribute(k_full_fused_hm<6, 2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
+            CK(cudaFuncSetAttribute(k_full_fused_hm<3, 2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
+            ctx->hm_attr = true;
+        }
         ProfScope prof(ctx, st);
         if (mixed) {
             const FusedArgsF32 fm{ctx->g4f.as<float>(), ctx->Wf.as<double>(), ctx->scale.as<double>()};
@@ -731,6 +741,8 @@ int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, cons
             if (nm1) k_full_fused_tf<1, NC, WS><<<grid, pl.WB, smem, st>>>(fa);       \
             else k_full_fused_tf<0, NC, WS><<<grid, pl.WB, smem, st>>>(fa);           \
         } else if (nm1) k_full_fused<1, NC, WS, 0><<<grid, pl.WB, smem, st>>>(fa);    \
+        else if (hm_rot == 6) k_full_fused_hm<6, 2, true><<<grid, pl.WB, smem_hm, st>>>(fa); \
+        else if (hm_rot == 3) k_full_fused_hm<3, 2, true><<<grid, pl.WB, smem_hm, st>>>(fa); \
         else k_full_fused<0, NC, WS, 0><<<grid, pl.WB, smem, st>>>(fa);               \
     } while (0)
             LL_LAYOUT(ctx, LL_FUSED);

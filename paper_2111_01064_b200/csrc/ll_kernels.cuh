@@ -1821,6 +1821,163 @@ k_full_fused(FusedArgs a)
 }
 
 // ---------------------------------------------------------------------------------------------------
+// F3 for several modes, large batches, by the rotation recurrence (the paper's higher-mode analysis ran this brute-force
+// likelihood).  k_full_fused<0> evaluates every (bin, mode) directly: two cubics and a sincos, 37 FP64
+// instructions + T^c h.  Here every mode carries its own recurrence state (z, w, v and the amplitude with its two
+// differences: 9 doubles in registers per mode), exactly as fused_bins_rot does for one mode: per (bin, mode) 12
+// (rotations) + 3 (amplitude) + 2 (A z) + 4 NC (T^c h) = 25 for two channels, plus per bin Re(g^c h^c) and W |h^c|^2.  What
+// is constant inside a re-synchronisation stretch — u = e^{i D3 Psi}, D3 A, T^c_m: 3 + 2 NC doubles per mode — lives in
+// shared memory (per thread, [q][thread]: conflict-free).  The modes are NM independent chains per bin, so a thread has
+// plenty of instruction-level parallelism although only three blocks fit an SM.  Same mapping, staging, tiles and band
+// logic as k_full_fused; bins outside a lane's band advance the recurrence but are not accumulated.
+// ---------------------------------------------------------------------------------------------------
+#ifndef LL_HM_MINB
+#define LL_HM_MINB 2 // six modes keep 54 doubles of recurrence state: at three blocks per SM (168 registers) the bin loop spills and the kernel takes 36.5 ms at config-2 size with 2048 walkers; at two (255 registers) 16.4 ms (direct route: 24.2 ms)
+#endif
+#ifndef LL_HM_UNROLL
+#define LL_HM_UNROLL 1
+#endif
+constexpr int kHmUnroll = LL_HM_UNROLL;
+template <int NM, int NC, bool WS>
+__global__ void __launch_bounds__(128, LL_HM_MINB) k_full_fused_hm(FusedArgs a)
+{
+    using TL = Tile<NC, WS>;
+    constexpr int NK = 3 + 2 * NC; // constants per mode in shared memory: cu, su, d3A, T^c (re, im)
+    extern __shared__ __align__(128) double sm[];
+    __shared__ __align__(8) uint64_t bar[2];
+    __shared__ int s_lo, s_hi;
+    const int tid = threadIdx.x;
+    const int p = blockIdx.x * blockDim.x + tid;
+    const int tile = blockIdx.y;
+    const int i0 = __ldg(a.tile_start + tile), i1 = __ldg(a.tile_start + tile + 1);
+    const int lo = max(a.ilo[p], i0), hi = min(a.ihi[p], i1);
+    if (tid == 0) {
+        s_lo = INT_MAX;
+        s_hi = INT_MIN;
+        mbar_init(&bar[0], 1);
+        mbar_init(&bar[1], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    if (lo < hi) {
+        atomicMin(&s_lo, lo);
+        atomicMax(&s_hi, hi);
+    }
+    __syncthreads();
+    const int blo = s_lo, bhi = s_hi;
+    if (blo >= bhi) return; // k_finalize never reads a tile no walker of the block touches
+
+    const int CH = a.CH;
+    double *kst = sm + (size_t)2 * CH * TL::DPB + tid; // this thread's constants: kst[(m * NK + q) * 128]
+    const int c_begin = blo / CH, c_end = (bhi + CH - 1) / CH;
+    if (tid == 0) TL::issue(a, sm, c_begin, CH, &bar[0]);
+    const size_t sw = (size_t)a.n_wp;
+    const size_t cj = (size_t)a.n_m * 8 * sw;
+    const int kbase = (int)a.k_min;
+    const double df = a.df, df2 = df * df, df3 = df2 * df;
+    double ts4 = 0.0;
+    if (a.t_shift) {
+        const int w = a.perm[p];
+        if (w >= 0) ts4 = 4.0 * a.t_shift[(size_t)w * a.ts_stride];
+    }
+    int j = find_interval_of_bin(a.bstart, a.n_nodes, blo);
+    int jl = -1, steps = kRotSync, expect = -1;
+    double cz[NM], sz[NM], cw[NM], sw_[NM], cv[NM], sv[NM], A[NM], d1A[NM], d2A[NM];
+#pragma unroll
+    for (int m = 0; m < NM; ++m) { cz[m] = 1; sz[m] = 0; cw[m] = 1; sw_[m] = 0; cv[m] = 1; sv[m] = 0; A[m] = 0; d1A[m] = 0; d2A[m] = 0; }
+    double s_dh = 0.0, s_hh = 0.0;
+
+    for (int c = c_begin; c < c_end; ++c) {
+        const int st = (c - c_begin) & 1;
+        const uint32_t ph = (uint32_t)((c - c_begin) >> 1) & 1u;
+        if (tid == 0 && c + 1 < c_end) TL::issue(a, sm + (size_t)(st ^ 1) * CH * TL::DPB, c + 1, CH, &bar[st ^ 1]);
+        mbar_wait(&bar[st], ph);
+        const double *sg = sm + (size_t)st * CH * TL::DPB;
+        const int cb = c * CH;
+        const double *sgc = sg - (size_t)cb * 2 * NC;
+        const double *sWc = sg + (size_t)CH * 2 * NC - cb;
+        const int ce = min(cb + CH, bhi);
+        int i = max(cb, blo);
+        while (i < ce) {
+            while (j < a.n_nodes - 2 && __ldg(a.bstart + j + 1) <= i) ++j;
+            const int seg_end = (j < a.n_nodes - 2) ? min(__ldg(a.bstart + j + 1), ce) : ce;
+            int tlo = max(i, lo), thi = min(seg_end, hi);
+            if (tlo >= thi) { tlo = INT_MAX; thi = INT_MIN; }
+            const int wlo = __reduce_min_sync(0xffffffffu, tlo);
+            const int whi = __reduce_max_sync(0xffffffffu, thi);
+            if (j != jl) { steps = kRotSync; jl = j; } // a new interval: re-synchronise at its first bin
+            if (wlo != expect) steps = kRotSync;       // the warp's bins are not contiguous with the last stretch
+            int ii = wlo;
+            while (ii < whi) {
+                if (steps >= kRotSync) { // every mode's state at bin ii, from its cubics
+                    const double nxj = -__ldg(a.xj + j);
+                    const double sh0 = a.t_shift ? qc_linear_mod_cycle(-nxj, ts4) : 0.0;
+                    const double t = fma((double)(kbase + ii), df, nxj);
+                    const double tt = fma(2.0, t, df), q3 = fma(3.0 * t, t + df, df2), t1 = t + df;
+                    const double *cc0 = a.C + (size_t)j * cj + p;
+#pragma unroll
+                    for (int m = 0; m < NM; ++m) {
+                        const double *cc = cc0 + (size_t)m * 8 * sw;
+                        const double cA0 = cc[0], cA1 = cc[sw], cA2 = cc[2 * sw], cA3 = cc[3 * sw];
+                        const double cP0 = cc[4 * sw] + sh0, cP1 = cc[5 * sw] + ts4, cP2 = cc[6 * sw], cP3 = cc[7 * sw];
+                        A[m] = fma(fma(fma(cA3, t, cA2), t, cA1), t, cA0);
+                        d1A[m] = df * fma(cA3, q3, fma(cA2, tt, cA1));
+                        d2A[m] = df2 * fma(6.0 * cA3, t1, 2.0 * cA2);
+                        double su, cu;
+                        LL_ROT_SINCOS(fma(fma(fma(cP3, t, cP2), t, cP1), t, cP0), sz[m], cz[m]);
+                        LL_ROT_SINCOS(df * fma(cP3, q3, fma(cP2, tt, cP1)), sw_[m], cw[m]);
+                        LL_ROT_SINCOS(df2 * fma(6.0 * cP3, t1, 2.0 * cP2), sv[m], cv[m]);
+                        LL_ROT_SINCOS(6.0 * cP3 * df3, su, cu);
+                        unit_modulus(cz[m], sz[m]);
+                        unit_modulus(cw[m], sw_[m]);
+                        unit_modulus(cv[m], sv[m]);
+                        unit_modulus(cu, su);
+                        double *k = kst + (size_t)(m * NK) * 128;
+                        k[0] = cu; k[128] = su; k[256] = 6.0 * cA3 * df3;
+                        const double *tfp = a.TF + (size_t)m * 2 * NC * sw + p;
+#pragma unroll
+                        for (int q = 0; q < 2 * NC; ++q) k[(3 + q) * 128] = tfp[(size_t)q * sw];
+                    }
+                    steps = 0;
+                }
+                const int ie = min(whi, ii + (kRotSync - steps));
+                steps += ie - ii;
+#pragma unroll kHmUnroll
+                for (; ii < ie; ++ii) {
+                    double h[2 * NC];
+#pragma unroll
+                    for (int q = 0; q < 2 * NC; ++q) h[q] = 0.0;
+#pragma unroll
+                    for (int m = 0; m < NM; ++m) {
+                        const double *k = kst + (size_t)(m * NK) * 128;
+                        const double u = A[m] * cz[m], v = A[m] * sz[m]; // h_m = u - i v
+#pragma unroll
+                        for (int cch = 0; cch < NC; ++cch) {
+                            const double tr = k[(3 + 2 * cch) * 128], ti = k[(4 + 2 * cch) * 128];
+                            h[2 * cch] = fma(tr, u, h[2 * cch]); h[2 * cch] = fma(ti, v, h[2 * cch]);
+                            h[2 * cch + 1] = fma(ti, u, h[2 * cch + 1]); h[2 * cch + 1] = fma(-tr, v, h[2 * cch + 1]);
+                        }
+                        const double cu = k[0], su = k[128];
+                        const double nzc = fma(cz[m], cw[m], -(sz[m] * sw_[m])), nzs = fma(sz[m], cw[m], cz[m] * sw_[m]);
+                        const double nwc = fma(cw[m], cv[m], -(sw_[m] * sv[m])), nws = fma(sw_[m], cv[m], cw[m] * sv[m]);
+                        const double nvc = fma(cv[m], cu, -(sv[m] * su)), nvs = fma(sv[m], cu, cv[m] * su);
+                        cz[m] = nzc; sz[m] = nzs; cw[m] = nwc; sw_[m] = nws; cv[m] = nvc; sv[m] = nvs;
+                        A[m] += d1A[m]; d1A[m] += d2A[m]; d2A[m] += k[256];
+                    }
+                    if (ii >= tlo && ii < thi) accumulate_bin<NC, WS>(sgc, sWc, CH, ii, h, s_dh, s_hh);
+                }
+            }
+            if (wlo < whi) expect = whi;
+            i = seg_end;
+        }
+        poison_stage(sg, CH * TL::DPB);
+        __syncthreads();
+    }
+    double *o = a.part + ((size_t)tile * 2) * sw + p;
+    o[0] = s_dh; o[sw] = s_hh;
+}
+
+// ---------------------------------------------------------------------------------------------------
 // F3, FP32-accumulate variant (BASELINE.json config 2; reading R15), single mode.
 // FP64: bin frequency offset t, phase and amplitude cubics, reduction of the phase to [-1/2, 1/2] quarter
 // cycles and its scaling to radians, <h|h> = sum W A^2 (all terms positive: binary32 partial sums would lose

@@ -146,12 +146,15 @@ def test_cfg2_pw_full_size_sampled(cfg2, orc, torch_cuda):
     assert np.all(np.isfinite(got[0]))
 
 
-def test_cfg2_hm6_full_size_sampled(orc, torch_cuda):
-    """k_full_fused<0> (per_config.cfg2_hm6): config 3's six modes through the FULL-GRID path on config 2's one-year
-    grid and 1024 nodes, 2048 prior-draw walkers (the bench's batch); data = walker 0's six-mode template + noise;
-    16 sampled walkers vs the oracle."""
+@pytest.mark.parametrize("n_m", [6, 3])
+def test_cfg2_hm6_full_size_sampled(orc, torch_cuda, n_m):
+    """k_full_fused_hm<6 | 3, 2, true> (per_config.cfg2_hm6: every mode by its own rotation recurrence): config 3's six
+    modes (or the first three) through the FULL-GRID path on config 2's one-year grid and 1024 nodes, 2048 prior-draw
+    walkers (the bench's batch); data = walker 0's template + noise; 16 sampled walkers vs the oracle; with three modes
+    also with 2 pi f t_c kept outside the splines (t_shift in every mode's phase cubic)."""
     n_w = 2048
     wl6, wl2 = wlm.make_workload(3, n_w=8), wlm.make_workload(2, n_w=n_w)
+    wl6.n_m, wl6.modes_l, wl6.modes_m, wl6.c_lm = n_m, wl6.modes_l[:n_m], wl6.modes_m[:n_m], wl6.c_lm[:n_m]
     rng = np.random.default_rng(wlm.SEED_BASE + 232)
     params = np.empty((n_w, 5 + 4 * wl6.n_m))
     params[:, :5] = wl2.params[:, :5]
@@ -173,8 +176,14 @@ def test_cfg2_hm6_full_size_sampled(orc, torch_cuda):
     sample = sample_walkers(n_w, fis, stride=256, wb=64)
     assert len(sample) >= 16
     ref = run(params[sample], d)
-    check_triplet(_np_triplet(got, sample), ref, "cfg2 six modes sampled")
+    check_triplet(_np_triplet(got, sample), ref, f"cfg2 {n_m} modes sampled")
     assert abs(np.sqrt(got[2][0]) - 500.0) < 1e-3
+    if n_m == 3:
+        ctx.standin_split_tc(True)
+        got = [x.cpu().numpy() for x in ctx.full_batch_standin(wl2.f_nodes, dev(tc, params))]
+        ref = orc.full_batch_standin(wl6.modes_m, wl6.c_lm, wl6.kappa, params[sample], wl2.f_nodes, g.k_min, g.df, g.n_f, d,
+                                     wl2.W, split_tc=True)
+        check_triplet(_np_triplet(got, sample), ref, "cfg2 3 modes, t_c outside the spline")
     ctx.destroy()
 
 
@@ -306,3 +315,33 @@ def test_small_batch_odd_sizes_and_bands(cfg2, orc, torch_cuda, n):
     ref = orc.full_batch(wl.f_nodes, amp[s], phase[s], tf[s], band[s], g.k_min, g.df, d, wl.W)
     check_triplet(_np_triplet(got, s), ref, f"array entry, {n} walkers")
     assert ctx.debug_check() == 0
+
+
+def test_multi_mode_arrays_with_scattered_bands(orc, torch_cuda):
+    """k_full_fused_hm through the array entry point: 1100 walkers, three modes, bands scattered over the grid (narrow, low,
+    high, empty), so that the union of a warp's bands has holes and the kernel's recurrence has to restart where the bins
+    stop being contiguous; sampled walkers vs the oracle."""
+    n_w, n_m = 1100, 3
+    wl = wlm.make_workload(2, n_w=n_w)
+    g = wl.grid
+    rng = np.random.default_rng(2320)
+    a1, p1, top = lisa_node_arrays(wl.params, wl.f_nodes)
+    scale = np.array([1.0, 0.4, 0.25])[None, :, None]
+    amp = np.ascontiguousarray(a1 * scale)
+    phase = np.ascontiguousarray(p1 * np.array([1.0, 0.5, 1.5])[None, :, None])
+    ang = rng.uniform(0, 2 * np.pi, (n_w, n_m, 2))
+    tf = np.ascontiguousarray(np.stack([np.cos(ang), np.sin(ang)], axis=-1))
+    lo = wlm.F_LO * (1.0 + 200.0 * rng.random(n_w) ** 2)
+    hi = np.where(rng.random(n_w) < 0.05, 0.5 * lo, np.minimum(0.05, lo * (1.0 + 0.5 * rng.random(n_w))))
+    band = np.stack([lo, hi], axis=1)
+    d = wl.noise
+    from paper_2111_01064_b200 import binding
+    ctx = binding.Context(n_modes=n_m)
+    tc = torch_cuda
+    ctx.set_data(g.n_f, g.k_min, g.df, dev(tc, d), dev(tc, wl.W))
+    got = [x.cpu().numpy() for x in ctx.full_batch(wl.f_nodes, dev(tc, amp), dev(tc, phase), dev(tc, tf), dev(tc, band))]
+    s_ = np.unique(np.r_[0, 127, 128, n_w - 1, rng.integers(0, n_w, 20)])
+    ref = orc.full_batch(wl.f_nodes, amp[s_], phase[s_], tf[s_], band[s_], g.k_min, g.df, d, wl.W)
+    check_triplet(_np_triplet(got, s_), ref, "three modes, scattered bands")
+    assert ctx.debug_check() == 0
+    ctx.destroy()
