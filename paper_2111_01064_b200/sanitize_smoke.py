@@ -71,7 +71,10 @@ def _full_families(n_c: int, log):
     tf = b["params"][:, 5:].reshape(70, 3, n_c, 2).contiguous()
     xw = torch.as_tensor(np.ascontiguousarray(wl.f_nodes), device=dev).repeat(70, 1).contiguous()
     ctx.full_batch_pw(xw, amp, ph, tf, band)
-    log.append(f"n_c={n_c}: full-grid three modes (generic, tf, per-walker nodes): {ctx.kernel_launches()} launches")
+    if n_c == 2:  # more than 1024 walkers, three modes, the BASELINE layout: k_full_fused_hm (every mode by its own recurrence)
+        big = b["params"].repeat(16, 1)[:1100].contiguous()
+        ctx.full_batch_standin(wl.f_nodes, big)
+    log.append(f"n_c={n_c}: full-grid three modes (generic, recurrence, tf, per-walker nodes): {ctx.kernel_launches()} launches")
     assert ctx.debug_check() == 0, ctx.last_error()
     ctx.destroy()
 
