@@ -479,7 +479,7 @@ int ensure_tiles(ll_ctx *ctx, FullPlan &pl, cudaStream_t st, bool uniform = fals
 // defer: (batches of up to 1024 walkers) fill the planner's arguments instead of launching it — the caller runs it as the
 // last block of k_setup_small
 int band_sort(ll_ctx *ctx, const FullPlan &pl, long long n_w, bool standin, const double *params, int P, const double *band,
-              cudaStream_t st, int n_items = 0, BandSortArgs *defer = nullptr)
+              cudaStream_t st, int n_items = 0, BandSortArgs *defer = nullptr, bool allow_lanes = true)
 {
     const int n_wp = pl.n_wp;
     CK(ctx->ilo_w.ensure(sizeof(int) * n_wp));
@@ -502,7 +502,7 @@ int band_sort(ll_ctx *ctx, const FullPlan &pl, long long n_w, bool standin, cons
         ba.pairs = ctx->pairs.as<unsigned long long>(); ba.n_items = n_items; ba.max_items = max_items;
         ba.grp_tab = n_items ? ctx->grp_tab.as<int>() : nullptr; ba.bstart_g = n_items ? ctx->nt.bstart : nullptr;
         ba.n_nodes = (int)ctx->nodes_host.size();
-        ba.lanes = (ctx->n_m == 1 && ctx->precision == LL_PREC_FP64) ? 1 : 0; // the single-mode kernel with weight moments
+        ba.lanes = (allow_lanes && ctx->n_m == 1 && ctx->precision == LL_PREC_FP64) ? 1 : 0; // the single-mode kernel with weight moments
         if (defer) {
             *defer = ba;
             return LL_OK;
@@ -598,7 +598,9 @@ int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, cons
     const int P = 5 + 2 * n_c * n_m;
     FullPlan pl = make_plan(ctx, n_w);
     // small batches (Module-1 sized): blocks of one warp, the work dealt out by active bins (k_band_sort_small)
-    const bool small = pl.n_wp <= 1024 && !tfp && !template_only && ctx->precision == LL_PREC_FP64;
+    // (the T(f) kernel has group items only, which pay up to ~640 walkers: 160 walkers on the one-year grid 0.397 -> 0.325 ms,
+    // 320: 0.667 -> 0.547, 1024: 1.58 -> 1.66)
+    const bool small = pl.n_wp <= (tfp ? 640 : 1024) && !template_only && ctx->precision == LL_PREC_FP64;
     static const int small_wps = getenv("LL_SMALL_WPS") ? atoi(getenv("LL_SMALL_WPS")) : kSmallWarpsPerSM;
     const int n_items = small ? ctx->sm_count * small_wps : 0;
     if (!small) {
@@ -642,7 +644,7 @@ int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, cons
                         sizeof(double) * (2 * (size_t)NWK4 * n_nodes + 1024) <= 160 * 1024;
     BandSortArgs ba;
     {
-        const int rc_b = band_sort(ctx, pl, n_w, standin, params, P, band, st, n_items, merged ? &ba : nullptr);
+        const int rc_b = band_sort(ctx, pl, n_w, standin, params, P, band, st, n_items, merged ? &ba : nullptr, !tfp);
         if (rc_b != LL_OK) return rc_b;
     }
     Spline4Args sa;
@@ -692,7 +694,10 @@ int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, cons
             ProfScope prof(ctx, st);
 #define LL_FUSED_SMALL(NC, WS)                                                        \
     do {                                                                              \
-        if (nm1) k_full_fused<1, NC, WS, 1><<<grid, 32, smem, st>>>(fa);              \
+        if (tfp) {                                                                    \
+            if (nm1) k_full_fused_tf<1, NC, WS, 1><<<grid, 32, smem, st>>>(fa);       \
+            else k_full_fused_tf<0, NC, WS, 1><<<grid, 32, smem, st>>>(fa);           \
+        } else if (nm1) k_full_fused<1, NC, WS, 1><<<grid, 32, smem, st>>>(fa);       \
         else k_full_fused<0, NC, WS, 1><<<grid, 32, smem, st>>>(fa);                  \
     } while (0)
             LL_LAYOUT(ctx, LL_FUSED_SMALL);

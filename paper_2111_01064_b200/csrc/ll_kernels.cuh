@@ -2321,8 +2321,10 @@ __device__ __forceinline__ double cubic4(const double *c4, double t)
 #ifndef LL_TF_MINB
 #define LL_TF_MINB 5 // config-2 size, one mode: 3 blocks per SM (153 registers) 17.33 ms, 4 (128) 17.78, 5 (96, spills outside the bin loop) 16.90, 6 (80) 17.58
 #endif
-template <int NM1, int NC, bool WS>
-__global__ void __launch_bounds__(128, NC == 2 ? (NM1 ? LL_TF_MINB : 3) : 2) k_full_fused_tf(FusedArgs a)
+// SMALL = 1 (batches of up to 1024 walkers; blocks of ONE warp): block b is group item b of the planner's table, as in
+// k_full_fused<.., SMALL = 1> (group items only: with T(f) there is no moment form of <h|h>, hence no lanes items).
+template <int NM1, int NC, bool WS, int SMALL = 0>
+__global__ void __launch_bounds__(128, NC == 2 ? (NM1 ? (SMALL ? 4 : LL_TF_MINB) : 3) : 2) k_full_fused_tf(FusedArgs a)
 {
     using TL = Tile<NC, WS>;
     constexpr int NCO = 8 + 8 * NC; // coefficients per (interval, mode)
@@ -2331,9 +2333,22 @@ __global__ void __launch_bounds__(128, NC == 2 ? (NM1 ? LL_TF_MINB : 3) : 2) k_f
     __shared__ int s_lo, s_hi;
 
     const int tid = threadIdx.x;
-    const int p = blockIdx.x * blockDim.x + tid;
-    const int tile = blockIdx.y;
-    const int i0 = __ldg(a.tile_start + tile), i1 = __ldg(a.tile_start + tile + 1); // tile = dense bins [i0, i1)
+    int p, tile, i0, i1, j_hint = 0;
+    if (SMALL) {
+        tile = blockIdx.x;
+        if (tile >= __ldg(a.grp_tab + 32)) return;
+        const int *it = a.grp_tab + grp_off_items() + tile;
+        const int mi = gridDim.x; // the table's row length = the grid
+        i0 = __ldg(it + mi);
+        i1 = __ldg(it + 2 * mi);
+        j_hint = __ldg(it + 3 * mi);
+        p = __ldg(it) * 32 + tid;
+    } else {
+        p = blockIdx.x * blockDim.x + tid;
+        tile = blockIdx.y;
+        i0 = __ldg(a.tile_start + tile);
+        i1 = __ldg(a.tile_start + tile + 1); // tile = dense bins [i0, i1)
+    }
     const int lo = max(a.ilo[p], i0), hi = min(a.ihi[p], i1);
     if (tid == 0) {
         s_lo = INT_MAX;
@@ -2349,7 +2364,10 @@ __global__ void __launch_bounds__(128, NC == 2 ? (NM1 ? LL_TF_MINB : 3) : 2) k_f
     }
     __syncthreads();
     const int blo = s_lo, bhi = s_hi;
-    if (blo >= bhi) return;
+    if (blo >= bhi) {
+        if (SMALL) { a.part[((size_t)tile * 2) * 32 + tid] = 0.0; a.part[((size_t)tile * 2 + 1) * 32 + tid] = 0.0; } // F4 reads every item
+        return;
+    }
 
     const int CH = a.CH;
     const int c_begin = blo / CH, c_end = (bhi + CH - 1) / CH;
@@ -2359,7 +2377,7 @@ __global__ void __launch_bounds__(128, NC == 2 ? (NM1 ? LL_TF_MINB : 3) : 2) k_f
     const size_t cm = (size_t)NCO * sw;         // one mode's block
     const size_t cj = (size_t)a.n_m * cm;       // one interval's block
     const int kbase = (int)a.k_min;
-    int j = find_interval_of_bin(a.bstart, a.n_nodes, blo);
+    int j = SMALL ? j_hint : find_interval_of_bin(a.bstart, a.n_nodes, blo);
     int jl = -1;
     double co[NCO];
     double nxj = 0.0, sh0 = 0.0, s_dh = 0.0, s_hh = 0.0;
@@ -2499,6 +2517,11 @@ __global__ void __launch_bounds__(128, NC == 2 ? (NM1 ? LL_TF_MINB : 3) : 2) k_f
         }
         poison_stage(sg, CH * TL::DPB);
         __syncthreads();
+    }
+    if (SMALL) {
+        a.part[((size_t)tile * 2) * 32 + tid] = s_dh;
+        a.part[((size_t)tile * 2 + 1) * 32 + tid] = s_hh;
+        return;
     }
     double *o = a.part + ((size_t)tile * 2) * sw + p;
     o[0] = s_dh; o[sw] = s_hh;

@@ -345,3 +345,26 @@ def test_multi_mode_arrays_with_scattered_bands(orc, torch_cuda):
     check_triplet(_np_triplet(got, s_), ref, "three modes, scattered bands")
     assert ctx.debug_check() == 0
     ctx.destroy()
+
+
+@pytest.mark.parametrize("n", [160, 333])
+def test_small_batch_tf_against_oracle(cfg2, orc, torch_cuda, n):
+    """The frequency-dependent transfer function (Eq. 8-9) at Module-1 size on the one-year grid: k_full_fused_tf in its
+    small-batch form (one-warp blocks over the planner's cost-balanced group items), bands with different bottoms and a
+    t_shift, against oracle.full_batch_tf."""
+    wl, d, run, ctx, fis = cfg2
+    g = wl.grid
+    tc = torch_cuda
+    rng = np.random.default_rng(8900 + n)
+    p = wl.params[rng.choice(wl.n_w, n, replace=False)]
+    amp, ph, top = lisa_node_arrays(p, wl.f_nodes)
+    ph = ph - 2.0 * np.pi * wl.f_nodes[None, None, :] * p[:, 2][:, None, None]
+    ts = np.ascontiguousarray(p[:, 2])
+    tfn = _smooth_tf_at_nodes(p, wl.f_nodes)
+    band = np.ascontiguousarray(np.stack([wlm.F_LO * (1.0 + 2.0 * rng.random(n)), top], axis=1))
+    got = [x.cpu().numpy() for x in ctx.full_batch_tf(wl.f_nodes, dev(tc, amp), dev(tc, ph), dev(tc, tfn), dev(tc, band),
+                                                      t_shift=dev(tc, ts))]
+    s_ = np.unique(np.r_[0, 31, 32, n - 1, rng.integers(0, n, 12)])
+    ref = orc.full_batch_tf(wl.f_nodes, amp[s_], ph[s_], tfn[s_], band[s_], g.k_min, g.df, d, wl.W, t_shift=ts[s_])
+    check_triplet(_np_triplet(got, s_), ref, f"T(f), {n} walkers")
+    assert ctx.debug_check() == 0
