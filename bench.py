@@ -792,6 +792,20 @@ def main():
                               "frac": pairs2 * SLOTS_FULL_TF / (kms / max(kn, 1) * 1e-3) / peak_slots,
                               "entry": "ll_full_batch_tf (amp, phase, T at 1024 nodes as device arrays; the walkers' own bands)",
                               "covered_by": COVERED_BY["cfg2_tf"]}
+            # the same entry point at Module-1 size (160 walkers: one-warp blocks over the planner's group items)
+            a16, p16, t16, b16 = (v[:160].contiguous() for v in (amp, ph, tfn, bnd))
+            o16 = tuple(torch.empty(160, dtype=torch.float64, device=amp.device) for _ in range(3))
+            fn16 = lambda: c2.full_batch_tf(wl2.f_nodes, a16, p16, t16, band=b16, out=o16)
+            fn16()
+            c2.profile_enable(True)
+            ms16 = time_steps(torch, fn16, 20, 3) / 20
+            kms16, kn16 = c2.profile_read()
+            c2.profile_enable(False)
+            pairs16 = c2.last_full_stats()[0]
+            per["cfg2_tf"]["call_160"] = {"n_walkers": 160, "ms_per_batch": ms16, "kernel_ms": kms16 / max(kn16, 1), "units": pairs16,
+                                          "slots_per_unit": SLOTS_FULL_TF,
+                                          "frac": pairs16 * SLOTS_FULL_TF / (kms16 / max(kn16, 1) * 1e-3) / peak_slots,
+                                          "covered_by": "tests/test_parity_cfg2_scale.py::test_small_batch_tf_against_oracle"}
             # ---- per-walker node grids at config-2 size.  Every walker gets its own copy of the
             # 1024 nodes (so the numbers can be compared with the shared-node path output by output); what is timed is
             # the per-walker machinery: one tridiagonal factorisation per system, one bin -> interval map per lane
