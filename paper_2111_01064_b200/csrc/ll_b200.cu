@@ -598,9 +598,9 @@ int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, cons
     const int P = 5 + 2 * n_c * n_m;
     FullPlan pl = make_plan(ctx, n_w);
     // small batches (Module-1 sized): blocks of one warp, the work dealt out by active bins (k_band_sort_small)
-    // (the T(f) kernel has group items only, which pay up to ~640 walkers: 160 walkers on the one-year grid 0.397 -> 0.325 ms,
-    // 320: 0.667 -> 0.547, 1024: 1.58 -> 1.66)
-    const bool small = pl.n_wp <= (tfp ? 640 : 1024) && !template_only && ctx->precision == LL_PREC_FP64;
+    // (the T(f) entry point too: 160 walkers on the one-year grid, kernel 0.397 ms on the large route's uniform tiles, 0.325 with
+    // group items, 0.236 with lanes items; 1024 walkers 1.58 / 1.66 / 1.47)
+    const bool small = pl.n_wp <= 1024 && !template_only && ctx->precision == LL_PREC_FP64;
     static const int small_wps = getenv("LL_SMALL_WPS") ? atoi(getenv("LL_SMALL_WPS")) : kSmallWarpsPerSM;
     const int n_items = small ? ctx->sm_count * small_wps : 0;
     if (!small) {
@@ -644,7 +644,7 @@ int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, cons
                         sizeof(double) * (2 * (size_t)NWK4 * n_nodes + 1024) <= 160 * 1024;
     BandSortArgs ba;
     {
-        const int rc_b = band_sort(ctx, pl, n_w, standin, params, P, band, st, n_items, merged ? &ba : nullptr, !tfp);
+        const int rc_b = band_sort(ctx, pl, n_w, standin, params, P, band, st, n_items, merged ? &ba : nullptr);
         if (rc_b != LL_OK) return rc_b;
     }
     Spline4Args sa;

@@ -2321,8 +2321,117 @@ __device__ __forceinline__ double cubic4(const double *c4, double t)
 #ifndef LL_TF_MINB
 #define LL_TF_MINB 5 // config-2 size, one mode: 3 blocks per SM (153 registers) 17.33 ms, 4 (128) 17.78, 5 (96, spills outside the bin loop) 16.90, 6 (80) 17.58
 #endif
+// A lanes item (fused_lanes_item above) of the T(f) kernel, single mode: lane = (walker, bin phase); A e^{-i Psi} by the lane's
+// own stride-kLP recurrence, the four T cubics by Horner at the lane's bin, T^c h, Re(g^c h^c) and W |h^c|^2 per row (with T(f)
+// there is no moment form of <h|h>).  The walker's 8 + 8 NC coefficients of the current interval live in registers.
+template <int NC, bool WS>
+__device__ __forceinline__ void fused_lanes_item_tf(const FusedArgs &a, int pw, int lo, int hi, int wlo, int whi, int j, int item,
+                                                    double *sm, uint64_t *bar)
+{
+    using TL = Tile<NC, WS>;
+    constexpr int NCO = 8 + 8 * NC;
+    const int lane = threadIdx.x, ph = lane / kLW;
+    double s_dh = 0.0, s_hh = 0.0;
+    const int CH = a.CH;
+    const int c_begin = wlo / CH, c_end = (whi + CH - 1) / CH;
+    if (lane == 0) TL::issue(a, sm, c_begin, CH, &bar[0]);
+    const size_t sw = (size_t)a.n_wp;
+    const size_t cj = (size_t)a.n_m * NCO * sw;
+    const int kbase = (int)a.k_min;
+    const double df = a.df, h = (double)kLP * df, h2 = h * h, h3 = h2 * h;
+    double ts4 = 0.0;
+    if (a.t_shift) {
+        const int w = a.perm[pw];
+        if (w >= 0) ts4 = 4.0 * a.t_shift[(size_t)w * a.ts_stride];
+    }
+    double co[NCO], nxj = 0;
+    double A = 0, d1A = 0, d2A = 0, d3A = 0, sz = 0, cz = 1, sw_ = 0, cw = 1, sv = 0, cv = 1, su = 0, cu = 1;
+    int jl = -1, steps = kLaneSync;
+    for (int c = c_begin; c < c_end; ++c) {
+        const int st = (c - c_begin) & 1;
+        const uint32_t par = (uint32_t)((c - c_begin) >> 1) & 1u;
+        if (lane == 0 && c + 1 < c_end) TL::issue(a, sm + (size_t)(st ^ 1) * CH * TL::DPB, c + 1, CH, &bar[st ^ 1]);
+        mbar_wait(&bar[st], par);
+        const double *sg = sm + (size_t)st * CH * TL::DPB;
+        const int cb = c * CH;
+        const double *sgc = sg - (size_t)cb * 2 * NC;
+        const double *sWc = sg + (size_t)CH * 2 * NC - cb;
+        const int ce = min(cb + CH, whi);
+        int i = max(cb, wlo);
+        while (i < ce) {
+            while (j < a.n_nodes - 2 && __ldg(a.bstart + j + 1) <= i) ++j;
+            const int seg_end = (j < a.n_nodes - 2) ? min(__ldg(a.bstart + j + 1), ce) : ce;
+            if (j != jl) {
+                const double *cc = a.C + (size_t)j * cj + pw;
+#pragma unroll
+                for (int q = 0; q < NCO; ++q) co[q] = cc[(size_t)q * sw];
+                const double xj = __ldg(a.xj + j);
+                nxj = -xj;
+                if (a.t_shift) { co[4] += qc_linear_mod_cycle(xj, ts4); co[5] += ts4; }
+                d3A = 6.0 * co[3] * h3;
+                LL_ROT_SINCOS(6.0 * co[7] * h3, su, cu);
+                unit_modulus(cu, su);
+                steps = kLaneSync;
+                jl = j;
+            }
+            const int b0 = max(i, lo), b1 = min(seg_end, hi);
+            const int r_end = (seg_end - 1) / kLP;
+            int r = i / kLP;
+            while (r <= r_end) {
+                if (steps >= kLaneSync) {
+                    const double t = fma((double)(kbase + kLP * r + ph), df, nxj);
+                    const double tt = fma(2.0, t, h), q3 = fma(3.0 * t, t + h, h2), t1 = t + h;
+                    A = cubic4(co, t);
+                    d1A = h * fma(co[3], q3, fma(co[2], tt, co[1]));
+                    d2A = h2 * fma(6.0 * co[3], t1, 2.0 * co[2]);
+                    LL_ROT_SINCOS(cubic4(co + 4, t), sz, cz);
+                    LL_ROT_SINCOS(h * fma(co[7], q3, fma(co[6], tt, co[5])), sw_, cw);
+                    LL_ROT_SINCOS(h2 * fma(6.0 * co[7], t1, 2.0 * co[6]), sv, cv);
+                    unit_modulus(cz, sz);
+                    unit_modulus(cw, sw_);
+                    unit_modulus(cv, sv);
+                    steps = 0;
+                }
+                const int r1 = min(r_end, r + (kLaneSync - steps) - 1);
+                steps += r1 - r + 1;
+#pragma unroll 2
+                for (; r <= r1; ++r) {
+                    const int ii = kLP * r + ph;
+                    const double t = fma((double)(kbase + ii), df, nxj);
+                    const double u = A * cz, v = A * sz; // h = u - i v
+                    double hc[2 * NC];
+#pragma unroll
+                    for (int cch = 0; cch < NC; ++cch) {
+                        const double tr = cubic4(co + 8 + 8 * cch, t), ti = cubic4(co + 12 + 8 * cch, t);
+                        hc[2 * cch] = fma(tr, u, ti * v);
+                        hc[2 * cch + 1] = fma(ti, u, -(tr * v));
+                    }
+                    if (ii >= b0 && ii < b1) accumulate_bin<NC, WS>(sgc, sWc, CH, ii, hc, s_dh, s_hh);
+                    const double nzc = fma(cz, cw, -(sz * sw_)), nzs = fma(sz, cw, cz * sw_);
+                    const double nwc = fma(cw, cv, -(sw_ * sv)), nws = fma(sw_, cv, cw * sv);
+                    const double nvc = fma(cv, cu, -(sv * su)), nvs = fma(sv, cu, cv * su);
+                    cz = nzc; sz = nzs; cw = nwc; sw_ = nws; cv = nvc; sv = nvs;
+                    A += d1A; d1A += d2A; d2A += d3A;
+                }
+            }
+            i = seg_end;
+        }
+        poison_stage(sg, CH * TL::DPB);
+        __syncthreads();
+    }
+#pragma unroll
+    for (int o = kLW; o < 32; o <<= 1) { // over the phases of a walker
+        s_dh += __shfl_xor_sync(0xffffffffu, s_dh, o);
+        s_hh += __shfl_xor_sync(0xffffffffu, s_hh, o);
+    }
+    if (ph == 0) {
+        a.part[((size_t)item * 2) * 32 + (pw & 31)] = s_dh;
+        a.part[((size_t)item * 2 + 1) * 32 + (pw & 31)] = s_hh;
+    }
+}
+
 // SMALL = 1 (batches of up to 1024 walkers; blocks of ONE warp): block b is group item b of the planner's table, as in
-// k_full_fused<.., SMALL = 1> (group items only: with T(f) there is no moment form of <h|h>, hence no lanes items).
+// k_full_fused<.., SMALL = 1>; one mode: lanes items too (fused_lanes_item_tf).
 template <int NM1, int NC, bool WS, int SMALL = 0>
 __global__ void __launch_bounds__(128, NC == 2 ? (NM1 ? (SMALL ? 4 : LL_TF_MINB) : 3) : 2) k_full_fused_tf(FusedArgs a)
 {
@@ -2334,6 +2443,7 @@ __global__ void __launch_bounds__(128, NC == 2 ? (NM1 ? (SMALL ? 4 : LL_TF_MINB)
 
     const int tid = threadIdx.x;
     int p, tile, i0, i1, j_hint = 0;
+    bool lanes_item = false;
     if (SMALL) {
         tile = blockIdx.x;
         if (tile >= __ldg(a.grp_tab + 32)) return;
@@ -2342,7 +2452,9 @@ __global__ void __launch_bounds__(128, NC == 2 ? (NM1 ? (SMALL ? 4 : LL_TF_MINB)
         i0 = __ldg(it + mi);
         i1 = __ldg(it + 2 * mi);
         j_hint = __ldg(it + 3 * mi);
-        p = __ldg(it) * 32 + tid;
+        const int code = __ldg(it);
+        lanes_item = NM1 && LL_SMALL_LANES && code < 0;
+        p = lanes_item ? (-code - 1) + tid % kLW : code * 32 + tid;
     } else {
         p = blockIdx.x * blockDim.x + tid;
         tile = blockIdx.y;
@@ -2369,6 +2481,10 @@ __global__ void __launch_bounds__(128, NC == 2 ? (NM1 ? (SMALL ? 4 : LL_TF_MINB)
         return;
     }
 
+    if (SMALL && NM1 && LL_SMALL_LANES && lanes_item) {
+        fused_lanes_item_tf<NC, WS>(a, p, lo, hi, blo, bhi, j_hint, tile, sm, bar);
+        return;
+    }
     const int CH = a.CH;
     const int c_begin = blo / CH, c_end = (bhi + CH - 1) / CH;
     if (tid == 0) TL::issue(a, sm, c_begin, CH, &bar[0]);
