@@ -378,12 +378,17 @@ int prepare_nodes(ll_ctx *ctx, int n, const double *x, cudaStream_t st)
 #define LL_FUSED_CH 512 // bins per TMA stage of the fused kernels (two stages per block): a block-wide barrier per stage;
                         // 256 -> 512 bins: 9.17 -> 9.08 ms at config 2 (40 KB per block, five blocks per SM)
 #endif
-FullPlan make_plan(const ll_ctx *ctx, long long n_w)
+FullPlan make_plan(const ll_ctx *ctx, long long n_w, bool hm_kernel = false) // hm_kernel: the launch may take k_full_fused_hm
 {
     FullPlan pl;
     // blocks of 128 walkers above 1024 walkers (64-walker blocks between 1024 and 4096, as in round 1, measured worse: 2048
     // walkers on the config-2 grid frac 0.60 with 64 x 512-bin stages, 0.69 with 64 x 256, 0.73 with 128 x 512; 3072: 0.63 / 0.73 / 0.76)
     pl.WB = (n_w > 1024) ? 128 : (n_w >= 1024 ? 64 : 32);
+    // three or six modes, the BASELINE layout, FP64: the recurrence kernel of the large route (k_full_fused_hm) beats the direct
+    // kernel of the small route from a few hundred walkers on (six modes on the one-year grid, small / large route: 160 walkers
+    // 2.52 / 3.09 ms, 320: 4.09 / 4.03, 640: 8.70 / 5.94, 1024: 15.4 / 8.92)
+    if (hm_kernel && (ctx->n_m == 3 || ctx->n_m == 6) && ctx->n_c == 2 && ctx->w_rows == 1 && ctx->precision == LL_PREC_FP64 && n_w >= 384)
+        pl.WB = 128;
     pl.n_wp = (int)round_up(std::max<long long>(n_w, 1), pl.WB);
     const int n_wb = pl.n_wp / pl.WB;
     // aim at ~16 blocks per SM over the whole grid, tiles between 64 and LL_FUSED_TB_MAX bins.  Small batches (blocks of one
@@ -596,11 +601,11 @@ int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, cons
     const int n_m = ctx->n_m, n_c = ctx->n_c, nw = ctx->w_rows;
     const int ns = tfp ? 2 + 2 * n_c : 2;
     const int P = 5 + 2 * n_c * n_m;
-    FullPlan pl = make_plan(ctx, n_w);
+    FullPlan pl = make_plan(ctx, n_w, !tfp && !template_only);
     // small batches (Module-1 sized): blocks of one warp, the work dealt out by active bins (k_band_sort_small)
     // (the T(f) entry point too: 160 walkers on the one-year grid, kernel 0.397 ms on the large route's uniform tiles, 0.325 with
     // group items, 0.236 with lanes items; 1024 walkers 1.58 / 1.66 / 1.47)
-    const bool small = pl.n_wp <= 1024 && !template_only && ctx->precision == LL_PREC_FP64;
+    const bool small = pl.n_wp <= 1024 && pl.WB != 128 && !template_only && ctx->precision == LL_PREC_FP64;
     static const int small_wps = getenv("LL_SMALL_WPS") ? atoi(getenv("LL_SMALL_WPS")) : kSmallWarpsPerSM;
     const int n_items = small ? ctx->sm_count * small_wps : 0;
     if (!small) {
