@@ -384,10 +384,10 @@ FullPlan make_plan(const ll_ctx *ctx, long long n_w, bool hm_kernel = false) // 
     // blocks of 128 walkers above 1024 walkers (64-walker blocks between 1024 and 4096, as in round 1, measured worse: 2048
     // walkers on the config-2 grid frac 0.60 with 64 x 512-bin stages, 0.69 with 64 x 256, 0.73 with 128 x 512; 3072: 0.63 / 0.73 / 0.76)
     pl.WB = (n_w > 1024) ? 128 : (n_w >= 1024 ? 64 : 32);
-    // three or six modes, the BASELINE layout, FP64: the recurrence kernel of the large route (k_full_fused_hm) beats the direct
-    // kernel of the small route from a few hundred walkers on (six modes on the one-year grid, small / large route: 160 walkers
-    // 2.52 / 3.09 ms, 320: 4.09 / 4.03, 640: 8.70 / 5.94, 1024: 15.4 / 8.92)
-    if (hm_kernel && (ctx->n_m == 3 || ctx->n_m == 6) && ctx->n_c == 2 && ctx->w_rows == 1 && ctx->precision == LL_PREC_FP64 && n_w >= 384)
+    // three or six modes, the BASELINE layout, FP64 (k_full_fused_hm on both routes): the large route takes over a little below
+    // 1024 walkers (six modes on the one-year grid, kernel on the small / large route: 320 walkers 2.71 / 4.01 ms, 512: 4.30 / 4.87,
+    // 800: 6.71 / 8.63, 1024: 9.71 / 8.89)
+    if (hm_kernel && (ctx->n_m == 3 || ctx->n_m == 6) && ctx->n_c == 2 && ctx->w_rows == 1 && ctx->precision == LL_PREC_FP64 && n_w >= 960)
         pl.WB = 128;
     pl.n_wp = (int)round_up(std::max<long long>(n_w, 1), pl.WB);
     const int n_wb = pl.n_wp / pl.WB;
@@ -694,6 +694,9 @@ int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, cons
     }
     if (small) {
         const int grid = n_items + 32 + n_wp; // = max_items of the planner (band_sort)
+        // three or six modes, the BASELINE layout: every mode by its own recurrence (k_full_fused_hm in item form)
+        const int hm_small = (!nm1 && !tfp && n_c == 2 && nw == 1 && (n_m == 3 || n_m == 6)) ? n_m : 0;
+        const size_t smem_hms = (size_t)2 * pl.CH * 8 * (2 * n_c + nw) + sizeof(double) * (size_t)n_m * (3 + 2 * n_c) * 32;
         const size_t smem = (size_t)2 * pl.CH * 8 * (2 * n_c + nw);
         {
             ProfScope prof(ctx, st);
@@ -703,6 +706,8 @@ int run_full(ll_ctx *ctx, long long n_w, int n_nodes, const double *params, cons
             if (nm1) k_full_fused_tf<1, NC, WS, 1><<<grid, 32, smem, st>>>(fa);       \
             else k_full_fused_tf<0, NC, WS, 1><<<grid, 32, smem, st>>>(fa);           \
         } else if (nm1) k_full_fused<1, NC, WS, 1><<<grid, 32, smem, st>>>(fa);       \
+        else if (hm_small == 6) k_full_fused_hm<6, 2, true, 1><<<grid, 32, smem_hms, st>>>(fa); \
+        else if (hm_small == 3) k_full_fused_hm<3, 2, true, 1><<<grid, 32, smem_hms, st>>>(fa); \
         else k_full_fused<0, NC, WS, 1><<<grid, 32, smem, st>>>(fa);                  \
     } while (0)
             LL_LAYOUT(ctx, LL_FUSED_SMALL);

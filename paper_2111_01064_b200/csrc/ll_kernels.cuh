@@ -1838,7 +1838,8 @@ k_full_fused(FusedArgs a)
 #define LL_HM_UNROLL 1
 #endif
 constexpr int kHmUnroll = LL_HM_UNROLL;
-template <int NM, int NC, bool WS>
+// SMALL = 1: one-warp blocks over the planner's group items (batches below 384 walkers), as k_full_fused<.., SMALL = 1>.
+template <int NM, int NC, bool WS, int SMALL = 0>
 __global__ void __launch_bounds__(128, LL_HM_MINB) k_full_fused_hm(FusedArgs a)
 {
     using TL = Tile<NC, WS>;
@@ -1846,10 +1847,23 @@ __global__ void __launch_bounds__(128, LL_HM_MINB) k_full_fused_hm(FusedArgs a)
     extern __shared__ __align__(128) double sm[];
     __shared__ __align__(8) uint64_t bar[2];
     __shared__ int s_lo, s_hi;
-    const int tid = threadIdx.x;
-    const int p = blockIdx.x * blockDim.x + tid;
-    const int tile = blockIdx.y;
-    const int i0 = __ldg(a.tile_start + tile), i1 = __ldg(a.tile_start + tile + 1);
+    const int tid = threadIdx.x, nthr = blockDim.x;
+    int p, tile, i0, i1, j_hint = 0;
+    if (SMALL) {
+        tile = blockIdx.x;
+        if (tile >= __ldg(a.grp_tab + 32)) return;
+        const int *it = a.grp_tab + grp_off_items() + tile;
+        const int mi = gridDim.x;
+        i0 = __ldg(it + mi);
+        i1 = __ldg(it + 2 * mi);
+        j_hint = __ldg(it + 3 * mi);
+        p = __ldg(it) * 32 + tid;
+    } else {
+        p = blockIdx.x * blockDim.x + tid;
+        tile = blockIdx.y;
+        i0 = __ldg(a.tile_start + tile);
+        i1 = __ldg(a.tile_start + tile + 1);
+    }
     const int lo = max(a.ilo[p], i0), hi = min(a.ihi[p], i1);
     if (tid == 0) {
         s_lo = INT_MAX;
@@ -1865,10 +1879,13 @@ __global__ void __launch_bounds__(128, LL_HM_MINB) k_full_fused_hm(FusedArgs a)
     }
     __syncthreads();
     const int blo = s_lo, bhi = s_hi;
-    if (blo >= bhi) return; // k_finalize never reads a tile no walker of the block touches
+    if (blo >= bhi) { // k_finalize never reads a tile no walker of the block touches; F4 of the small route reads every item
+        if (SMALL) { a.part[((size_t)tile * 2) * 32 + tid] = 0.0; a.part[((size_t)tile * 2 + 1) * 32 + tid] = 0.0; }
+        return;
+    }
 
     const int CH = a.CH;
-    double *kst = sm + (size_t)2 * CH * TL::DPB + tid; // this thread's constants: kst[(m * NK + q) * 128]
+    double *kst = sm + (size_t)2 * CH * TL::DPB + tid; // this thread's constants: kst[(m * NK + q) * nthr]
     const int c_begin = blo / CH, c_end = (bhi + CH - 1) / CH;
     if (tid == 0) TL::issue(a, sm, c_begin, CH, &bar[0]);
     const size_t sw = (size_t)a.n_wp;
@@ -1880,7 +1897,7 @@ __global__ void __launch_bounds__(128, LL_HM_MINB) k_full_fused_hm(FusedArgs a)
         const int w = a.perm[p];
         if (w >= 0) ts4 = 4.0 * a.t_shift[(size_t)w * a.ts_stride];
     }
-    int j = find_interval_of_bin(a.bstart, a.n_nodes, blo);
+    int j = SMALL ? j_hint : find_interval_of_bin(a.bstart, a.n_nodes, blo);
     int jl = -1, steps = kRotSync, expect = -1;
     double cz[NM], sz[NM], cw[NM], sw_[NM], cv[NM], sv[NM], A[NM], d1A[NM], d2A[NM];
 #pragma unroll
@@ -1932,11 +1949,11 @@ __global__ void __launch_bounds__(128, LL_HM_MINB) k_full_fused_hm(FusedArgs a)
                         unit_modulus(cw[m], sw_[m]);
                         unit_modulus(cv[m], sv[m]);
                         unit_modulus(cu, su);
-                        double *k = kst + (size_t)(m * NK) * 128;
-                        k[0] = cu; k[128] = su; k[256] = 6.0 * cA3 * df3;
+                        double *k = kst + (size_t)(m * NK) * nthr;
+                        k[0] = cu; k[nthr] = su; k[2 * nthr] = 6.0 * cA3 * df3;
                         const double *tfp = a.TF + (size_t)m * 2 * NC * sw + p;
 #pragma unroll
-                        for (int q = 0; q < 2 * NC; ++q) k[(3 + q) * 128] = tfp[(size_t)q * sw];
+                        for (int q = 0; q < 2 * NC; ++q) k[(3 + q) * nthr] = tfp[(size_t)q * sw];
                     }
                     steps = 0;
                 }
@@ -1949,20 +1966,20 @@ __global__ void __launch_bounds__(128, LL_HM_MINB) k_full_fused_hm(FusedArgs a)
                     for (int q = 0; q < 2 * NC; ++q) h[q] = 0.0;
 #pragma unroll
                     for (int m = 0; m < NM; ++m) {
-                        const double *k = kst + (size_t)(m * NK) * 128;
+                        const double *k = kst + (size_t)(m * NK) * nthr;
                         const double u = A[m] * cz[m], v = A[m] * sz[m]; // h_m = u - i v
 #pragma unroll
                         for (int cch = 0; cch < NC; ++cch) {
-                            const double tr = k[(3 + 2 * cch) * 128], ti = k[(4 + 2 * cch) * 128];
+                            const double tr = k[(3 + 2 * cch) * nthr], ti = k[(4 + 2 * cch) * nthr];
                             h[2 * cch] = fma(tr, u, h[2 * cch]); h[2 * cch] = fma(ti, v, h[2 * cch]);
                             h[2 * cch + 1] = fma(ti, u, h[2 * cch + 1]); h[2 * cch + 1] = fma(-tr, v, h[2 * cch + 1]);
                         }
-                        const double cu = k[0], su = k[128];
+                        const double cu = k[0], su = k[nthr];
                         const double nzc = fma(cz[m], cw[m], -(sz[m] * sw_[m])), nzs = fma(sz[m], cw[m], cz[m] * sw_[m]);
                         const double nwc = fma(cw[m], cv[m], -(sw_[m] * sv[m])), nws = fma(sw_[m], cv[m], cw[m] * sv[m]);
                         const double nvc = fma(cv[m], cu, -(sv[m] * su)), nvs = fma(sv[m], cu, cv[m] * su);
                         cz[m] = nzc; sz[m] = nzs; cw[m] = nwc; sw_[m] = nws; cv[m] = nvc; sv[m] = nvs;
-                        A[m] += d1A[m]; d1A[m] += d2A[m]; d2A[m] += k[256];
+                        A[m] += d1A[m]; d1A[m] += d2A[m]; d2A[m] += k[2 * nthr];
                     }
                     if (ii >= tlo && ii < thi) accumulate_bin<NC, WS>(sgc, sWc, CH, ii, h, s_dh, s_hh);
                 }
@@ -1972,6 +1989,11 @@ __global__ void __launch_bounds__(128, LL_HM_MINB) k_full_fused_hm(FusedArgs a)
         }
         poison_stage(sg, CH * TL::DPB);
         __syncthreads();
+    }
+    if (SMALL) {
+        a.part[((size_t)tile * 2) * 32 + tid] = s_dh;
+        a.part[((size_t)tile * 2 + 1) * 32 + tid] = s_hh;
+        return;
     }
     double *o = a.part + ((size_t)tile * 2) * sw + p;
     o[0] = s_dh; o[sw] = s_hh;

@@ -146,13 +146,13 @@ def test_cfg2_pw_full_size_sampled(cfg2, orc, torch_cuda):
     assert np.all(np.isfinite(got[0]))
 
 
-@pytest.mark.parametrize("n_m,n_w", [(6, 2048), (3, 2048), (6, 500)])
+@pytest.mark.parametrize("n_m,n_w", [(6, 2048), (3, 2048), (6, 1000), (6, 500), (6, 160), (3, 45)])
 def test_cfg2_hm6_full_size_sampled(orc, torch_cuda, n_m, n_w):
     """k_full_fused_hm<6 | 3, 2, true> (per_config.cfg2_hm6: every mode by its own rotation recurrence): config 3's six
     modes (or the first three) through the FULL-GRID path on config 2's one-year grid and 1024 nodes, 2048 prior-draw
     walkers (the bench's batch); data = walker 0's template + noise; 16 sampled walkers vs the oracle; with three modes
-    also with 2 pi f t_c kept outside the splines (t_shift in every mode's phase cubic); 500 walkers: the smallest batches
-    that take this kernel (from 384 walkers on) instead of the small-batch route."""
+    also with 2 pi f t_c kept outside the splines (t_shift in every mode's phase cubic); 1000 walkers: the smallest batches
+    that take the large route (from 960 walkers on); 500, 160 and 45 walkers: the kernel's item form on the small-batch route."""
     wl6, wl2 = wlm.make_workload(3, n_w=8), wlm.make_workload(2, n_w=n_w)
     wl6.n_m, wl6.modes_l, wl6.modes_m, wl6.c_lm = n_m, wl6.modes_l[:n_m], wl6.modes_m[:n_m], wl6.c_lm[:n_m]
     rng = np.random.default_rng(wlm.SEED_BASE + 232)
@@ -173,8 +173,8 @@ def test_cfg2_hm6_full_size_sampled(orc, torch_cuda, n_m, n_w):
     ctx.set_data(g.n_f, g.k_min, g.df, dev(tc, d), dev(tc, wl2.W))
     got = [x.cpu().numpy() for x in ctx.full_batch_standin(wl2.f_nodes, dev(tc, params))]
     fis = np.array([orc.standin_fisco(p) for p in params])
-    sample = sample_walkers(n_w, fis, stride=256 if n_w > 1000 else 40, wb=64)
-    assert len(sample) >= 16
+    sample = sample_walkers(n_w, fis, stride=256 if n_w > 1000 else (40 if n_w > 300 else (10 if n_w > 100 else 3)), wb=64)
+    assert len(sample) >= min(16, n_w // 3)
     ref = run(params[sample], d)
     check_triplet(_np_triplet(got, sample), ref, f"cfg2 {n_m} modes sampled")
     assert abs(np.sqrt(got[2][0]) - 500.0) < 1e-3
