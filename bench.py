@@ -847,6 +847,10 @@ def main():
             hm = bench_full_hm(torch)
             hm["frac"] = hm["active_pair_modes"] * hm["algorithmic_slots_per_pair_mode"] / (hm["kernel_ms"] * 1e-3) / peak_slots
             hm["covered_by"] = COVERED_BY["cfg2_hm6"]
+            h16 = bench_full_hm(torch, steps=10, n_w=160)   # the same at Module-1 size: the kernel's item form on the small-batch route
+            hm["call_160"] = {"n_walkers": 160, "ms_per_batch": h16["ms_per_batch"], "kernel_ms": h16["kernel_ms"],
+                              "units": h16["active_pair_modes"], "slots_per_unit": h16["algorithmic_slots_per_pair_mode"],
+                              "frac": h16["active_pair_modes"] * h16["algorithmic_slots_per_pair_mode"] / (h16["kernel_ms"] * 1e-3) / peak_slots}
             per["cfg2_hm6"] = hm
             # ---- Module-1 sized sampler iteration on the full-grid likelihood of the same one-year data stream
             per["module1_iteration"] = bench_sampler_iteration(torch, c2, wl2, b2["params"], n_t=4, n_w=80, iters=20,
