@@ -151,6 +151,7 @@ struct ll_ctx {
     bool ptrun_attr = false;
     bool spl4_attr = false;
     bool hm_attr = false;
+    bool splpw_attr = false;
     double *static_scratch = nullptr; // device address of g_ll_static_scratch on this context's device (ll_create)
     HetTable ht{};
     Het1Table ht1{}; // single-mode regrouped table (k_het_standin1); base == nullptr when not built
@@ -803,8 +804,22 @@ int run_full_pw(ll_ctx *ctx, long long n_w, int n_nodes, const double *f_nodes_w
         dim3 gx(n_wp / 32, ceil_div(n_nodes, 32));
         k_pw_nodes_x<<<gx, 256, 0, st>>>(f_nodes_w, ctx->perm.as<int>(), n_wp, n_nodes, X);
         LAUNCHED(ctx);
-        dim3 gs(ceil_div(n_wp, 128), 2 * n_m);
-        k_spline_pw<<<gs, 128, 0, st>>>(ctx->Y.as<double>(), X, ctx->C.as<double>(), n_wp, n_nodes, n_m, ctx->spline_bc);
+        // few systems (Module-1 sized batches): a block per four walkers of a system (k_spline_pw_block); else a thread per system
+        const long long n_sys = (long long)n_wp * 2 * n_m;
+        int Tb = 128;
+        while (Tb < 512 && Tb < n_nodes / 2) Tb <<= 1; // four walkers x ~8 rows per chunk thread
+        const size_t smem_b = sizeof(double) * (16 * (size_t)n_nodes + Tb);
+        if (n_sys <= (long long)ctx->sm_count * 32 && smem_b <= 160 * 1024 && n_nodes >= 4) {
+            if (!ctx->splpw_attr) {
+                CK(cudaFuncSetAttribute(k_spline_pw_block<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024));
+                ctx->splpw_attr = true;
+            }
+            k_spline_pw_block<4><<<(unsigned)(n_sys / 4), Tb, smem_b, st>>>(ctx->Y.as<double>(), X, ctx->C.as<double>(), n_wp, n_nodes,
+                                                                            n_m, ctx->spline_bc);
+        } else {
+            dim3 gs(ceil_div(n_wp, 128), 2 * n_m);
+            k_spline_pw<<<gs, 128, 0, st>>>(ctx->Y.as<double>(), X, ctx->C.as<double>(), n_wp, n_nodes, n_m, ctx->spline_bc);
+        }
         LAUNCHED(ctx);
     }
     FusedArgs fa = fused_args(ctx, pl, n_nodes, t_shift, 1);

@@ -2774,6 +2774,127 @@ k_spline_pw(const double *__restrict__ Y, const double *__restrict__ X, double *
     }
 }
 
+// F2 with per-walker nodes for FEW systems (Module-1 sized batches): k_spline_pw above is one thread per system walking
+// 2 (n - 2) dependent rows, each with a division and a parked value (measured 0.81 ms for 320 systems of 1024 nodes: 760 cycles
+// per row).  Here a block takes NWK neighbouring walkers of one system, thread = (chunk thread, walker), as k_spline_block4:
+//  (a) the elimination factors c'_j = c_j / (b_j - a_j c'_{j-1}): no scan needed — the map contracts by <= 1/12 per row for
+//      ANY node spacing (a_j c_j / den_j^2 with den_j >= h_{j-1}/4 + h_j/3 >= 2 sqrt(h_{j-1} h_j / 12)), so a thread that
+//      starts kPwWarm = 16 rows before its chunk from c' = 0 has its chunk's first factor to 12^-16 < 1e-17 (from row 1 on
+//      exactly: the true start);
+//  (b) dp_j = (r_j - a_j dp_{j-1}) / den_j and (c) M_j = dp_j - c'_j M_{j+1}: first-order linear recurrences, by the scans
+//      of affine maps of k_spline_block4.
+// Same rows (and not-a-knot substitutions) as k_spline_pw; results equal to rounding.  Shared memory: xs, ys, cps, ds [n][NWK].
+constexpr int kPwWarm = 16;
+template <int NWK>
+__global__ void __launch_bounds__(1024)
+k_spline_pw_block(const double *__restrict__ Y, const double *__restrict__ X, double *__restrict__ C, int n_wp, int n_nodes, int n_m,
+                  int bc)
+{
+    extern __shared__ double ssm[];
+    __shared__ double sA[128], sB[128];
+    const int tid = threadIdx.x, T = blockDim.x, lane = tid & 31, wid = tid >> 5, nwarp = T >> 5;
+    const int wl = tid % NWK, ct = tid / NWK, TT = T / NWK;
+    const int nq = n_wp / NWK;
+    const int sys = blockIdx.x / nq, p0 = (blockIdx.x - sys * nq) * NWK;
+    const int m = sys >> 1, kind = sys & 1;
+    const int n = n_nodes;
+    const size_t sw = (size_t)n_wp;
+    double *xs = ssm, *ys = xs + NWK * n, *cps = ys + NWK * n, *ds = cps + NWK * n, *xch = ds + NWK * n;
+    for (int idx = tid; idx < NWK * n; idx += T) {
+        const int j = idx / NWK;
+        xs[idx] = __ldg(X + (size_t)j * sw + p0 + wl);
+        ys[idx] = __ldg(Y + ((size_t)sys * n + j) * sw + p0 + wl);
+    }
+    __syncthreads();
+    auto xv = [&](int j) { return xs[NWK * j + wl]; };
+    auto yv = [&](int j) { return ys[NWK * j + wl]; };
+    // row j (1 <= j <= n - 2) of the walker's system: a, b, c and the right-hand side r
+    auto row = [&](int j, double &a, double &b, double &c, double &r) {
+        const double hm = xv(j) - xv(j - 1), hp = xv(j + 1) - xv(j);
+        a = hm * kSixth; b = (hm + hp) * (1.0 / 3.0); c = hp * kSixth;
+        if (bc) { // not-a-knot: end conditions substituted into rows 1 and n - 2
+            if (j == 1) { const double rho0 = hm / hp; b += a * (1.0 + rho0); c -= a * rho0; }
+            if (j == n - 2) { const double rhon = hp / hm; b += c * (1.0 + rhon); a -= c * rhon; c = 0.0; }
+        }
+        if (j == 1) a = 0.0;
+        r = (yv(j + 1) - yv(j)) / hp - (yv(j) - yv(j - 1)) / hm;
+    };
+    const int L = (n + TT - 1) / TT;
+    const int j0 = min(ct * L, n), j1 = min(j0 + L, n);
+    // ---- (a) c'_j of the chunk, after a warm-up of kPwWarm rows; (b) composed with the chunk's map for dp
+    double cp = 0.0;
+    for (int j = max(1, j0 - kPwWarm); j < min(j0, n - 1); ++j) {
+        double a, b, c, r;
+        row(j, a, b, c, r);
+        cp = c / (b - a * cp);
+    }
+    double A = 0.0, B = 1.0;
+    for (int j = j0; j < j1; ++j) {
+        if (j >= 1 && j <= n - 2) {
+            double a, b, c, r;
+            row(j, a, b, c, r);
+            const double inv = 1.0 / (b - a * cp);
+            cp = c * inv;
+            cps[NWK * j + wl] = cp;
+            const double be = -a * inv;
+            A = fma(be, A, r * inv);
+            B *= be;
+        } else cps[NWK * j + wl] = 0.0;
+    }
+    affine_scan4_up<NWK>(A, B, sA, sB, lane, wid, nwarp, wl);
+    xch[tid] = A;
+    __syncthreads();
+    double dp = ct ? xch[tid - NWK] : 0.0;
+    for (int j = j0; j < j1; ++j) {
+        if (j >= 1 && j <= n - 2) {
+            double a, b, c, r;
+            row(j, a, b, c, r);
+            const double cpm = (j >= 2) ? cps[NWK * (j - 1) + wl] : 0.0;
+            dp = (r - a * dp) / (b - a * cpm);
+            ds[NWK * j + wl] = dp;
+        } else ds[NWK * j + wl] = 0.0;
+    }
+    __syncthreads();
+    // ---- (c) backward sweep: M_j = dp_j - c'_j M_{j+1}
+    A = 0.0; B = 1.0;
+    for (int j = j1 - 1; j >= j0; --j) {
+        if (j >= 1 && j <= n - 2) {
+            const double be = -cps[NWK * j + wl];
+            A = fma(be, A, ds[NWK * j + wl]);
+            B *= be;
+        } else { A = 0.0; B = 0.0; }
+    }
+    affine_scan4_down<NWK>(A, B, sA, sB, lane, wid, nwarp, wl);
+    xch[tid] = A;
+    __syncthreads();
+    double Mn = (ct + 1 < TT) ? xch[tid + NWK] : 0.0;
+    for (int j = j1 - 1; j >= j0; --j) {
+        Mn = (j >= 1 && j <= n - 2) ? fma(-cps[NWK * j + wl], Mn, ds[NWK * j + wl]) : 0.0;
+        ds[NWK * j + wl] = Mn;
+    }
+    __syncthreads();
+    if (bc) {
+        if (ct == 0) {
+            const double rho0 = (xv(1) - xv(0)) / (xv(2) - xv(1)), rhon = (xv(n - 1) - xv(n - 2)) / (xv(n - 2) - xv(n - 3));
+            ds[wl] = (1.0 + rho0) * ds[NWK + wl] - rho0 * ds[2 * NWK + wl];
+            ds[NWK * (n - 1) + wl] = (1.0 + rhon) * ds[NWK * (n - 2) + wl] - rhon * ds[NWK * (n - 3) + wl];
+        }
+        __syncthreads();
+    }
+    double *c = C + ((size_t)m * 8 + kind * 4) * sw + p0 + wl;
+    const size_t cj = (size_t)n_m * 8 * sw;
+    for (int idx = tid; idx < NWK * (n - 1); idx += T) {
+        const int j = idx / NWK;
+        const double y0 = ys[idx], y1 = ys[idx + NWK], Mj = ds[idx], Mn1 = ds[idx + NWK];
+        const double h = xs[idx + NWK] - xs[idx], ih = 1.0 / h;
+        double *cc = c + (size_t)j * cj;
+        cc[0] = y0;
+        cc[sw] = (y1 - y0) * ih - h * (2.0 * Mj + Mn1) * kSixth;
+        cc[2 * sw] = 0.5 * Mj;
+        cc[3 * sw] = (Mn1 - Mj) * ih * kSixth;
+    }
+}
+
 // F3 with per-walker intervals.  Same mapping and data staging as k_full_fused_tf (one thread = one walker, TMA-fed
 // g/W tiles broadcast from shared memory); every lane tracks its own interval: the bins go up, so the interval index
 // only moves forward, by a comparison with the lane's next node per bin.  NM1: the 8 coefficients of the lane's

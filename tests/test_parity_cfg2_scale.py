@@ -368,3 +368,40 @@ def test_small_batch_tf_against_oracle(cfg2, orc, torch_cuda, n):
     ref = orc.full_batch_tf(wl.f_nodes, amp[s_], ph[s_], tfn[s_], band[s_], g.k_min, g.df, d, wl.W, t_shift=ts[s_])
     check_triplet(_np_triplet(got, s_), ref, f"T(f), {n} walkers")
     assert ctx.debug_check() == 0
+
+
+@pytest.mark.parametrize("n,bc", [(160, 0), (333, 1)])
+def test_small_batch_pw_against_oracle(cfg2, orc, torch_cuda, n, bc):
+    """Per-walker node grids at Module-1 size on the one-year grid: k_spline_pw_block (a block per four walkers of a system;
+    elimination factors from a 16-row warm-up, dp and M by scans of affine maps) instead of the thread-per-system sweep, with
+    the natural and the not-a-knot boundary condition; every second walker has 1024 log-spaced nodes over its own span."""
+    from oracle import per_walker as pw
+    from paper_2111_01064_b200 import binding
+    wl, d, run, ctx0, fis = cfg2
+    g = wl.grid
+    tc = torch_cuda
+    rng = np.random.default_rng(5100 + n)
+    p = wl.params[rng.choice(wl.n_w, n, replace=False)]
+    _, _, top = lisa_node_arrays(p, wl.f_nodes)
+    x = np.tile(wl.f_nodes, (n, 1))
+    odd = np.arange(1, n, 2)
+    lo = wlm.F_LO * rng.uniform(1.0, 3.0, len(odd))
+    hi = np.minimum(top[odd] * rng.uniform(0.7, 1.1, len(odd)), wlm.F_HI)
+    t = np.linspace(0.0, 1.0, len(wl.f_nodes))
+    x[odd] = np.exp(np.log(lo)[:, None] + (np.log(hi) - np.log(lo))[:, None] * t[None, :])
+    x[odd, 0], x[odd, -1] = lo, hi
+    amp, ph, _ = lisa_node_arrays(p, x)
+    tf = np.ascontiguousarray(p[:, 5:9].reshape(n, 1, 2, 2))
+    band = np.ascontiguousarray(np.stack([np.full(n, g.k_min * g.df), top], axis=1))
+    ctx = binding.Context(n_modes=1, spline_bc=bc)
+    ctx.set_data(g.n_f, g.k_min, g.df, dev(tc, d), dev(tc, wl.W))
+    got = [v.cpu().numpy() for v in ctx.full_batch_pw(dev(tc, x), dev(tc, amp), dev(tc, ph), dev(tc, tf), dev(tc, band))]
+    s_ = np.unique(np.r_[0, 1, 2, 3, n - 2, n - 1, rng.integers(0, n, 10)])
+    orc.set_spline_bc(bc)
+    try:
+        ref = pw.full_batch_pw(x[s_], amp[s_], ph[s_], tf[s_], band[s_], g.k_min, g.df, d, wl.W)
+    finally:
+        orc.set_spline_bc(0)
+    check_triplet(_np_triplet(got, s_), ref, f"per-walker nodes, {n} walkers, bc {bc}")
+    assert ctx.debug_check() == 0
+    ctx.destroy()
