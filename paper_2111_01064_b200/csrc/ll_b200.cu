@@ -485,7 +485,7 @@ int ensure_tiles(ll_ctx *ctx, FullPlan &pl, cudaStream_t st, bool uniform = fals
 // defer: (batches of up to 1024 walkers) fill the planner's arguments instead of launching it — the caller runs it as the
 // last block of k_setup_small
 int band_sort(ll_ctx *ctx, const FullPlan &pl, long long n_w, bool standin, const double *params, int P, const double *band,
-              cudaStream_t st, int n_items = 0, BandSortArgs *defer = nullptr, bool allow_lanes = true)
+              cudaStream_t st, int n_items = 0, BandSortArgs *defer = nullptr, bool allow_lanes = true, bool shared_nodes = true)
 {
     const int n_wp = pl.n_wp;
     CK(ctx->ilo_w.ensure(sizeof(int) * n_wp));
@@ -506,9 +506,10 @@ int band_sort(ll_ctx *ctx, const FullPlan &pl, long long n_w, bool standin, cons
         ba.use_standin = standin ? 1 : 0; ba.params = params; ba.P = P; ba.band = band; ba.n_w = (int)n_w; ba.n_wp = n_wp;
         ba.g = g; ba.si = ctx->si; ba.perm = ctx->perm.as<int>(); ba.ilo_s = ctx->ilo_s.as<int>(); ba.ihi_s = ctx->ihi_s.as<int>();
         ba.pairs = ctx->pairs.as<unsigned long long>(); ba.n_items = n_items; ba.max_items = max_items;
-        ba.grp_tab = n_items ? ctx->grp_tab.as<int>() : nullptr; ba.bstart_g = n_items ? ctx->nt.bstart : nullptr;
-        ba.n_nodes = (int)ctx->nodes_host.size();
-        ba.lanes = (allow_lanes && ctx->n_m == 1 && ctx->precision == LL_PREC_FP64) ? 1 : 0; // the single-mode kernel with weight moments
+        ba.grp_tab = n_items ? ctx->grp_tab.as<int>() : nullptr;
+        ba.bstart_g = (n_items && shared_nodes) ? ctx->nt.bstart : nullptr; // per-walker node grids: no shared interval table
+        ba.n_nodes = shared_nodes ? (int)ctx->nodes_host.size() : 0;
+        ba.lanes = (allow_lanes && shared_nodes && ctx->n_m == 1 && ctx->precision == LL_PREC_FP64) ? 1 : 0; // the single-mode kernels
         if (defer) {
             *defer = ba;
             return LL_OK;
@@ -777,7 +778,10 @@ int run_full_pw(ll_ctx *ctx, long long n_w, int n_nodes, const double *f_nodes_w
 {
     const int n_m = ctx->n_m, n_c = ctx->n_c, nw = ctx->w_rows;
     FullPlan pl = make_plan(ctx, n_w);
-    {
+    // small batches: one-warp blocks over the planner's group items (as run_full), the split F4
+    const bool small = pl.n_wp <= 1024 && pl.WB != 128 && ctx->precision == LL_PREC_FP64;
+    const int n_items = small ? ctx->sm_count * kSmallWarpsPerSM : 0;
+    if (!small) {
         const int rc_t = ensure_tiles(ctx, pl, st, true);
         if (rc_t != LL_OK) return rc_t;
     }
@@ -786,14 +790,15 @@ int run_full_pw(ll_ctx *ctx, long long n_w, int n_nodes, const double *f_nodes_w
     CK(ctx->Y.ensure(sizeof(double) * (size_t)n_m * 2 * n_nodes * n_wp));
     CK(ctx->C.ensure(sizeof(double) * (size_t)(n_nodes - 1) * n_m * 8 * n_wp));
     CK(ctx->TF.ensure(sizeof(double) * (size_t)n_m * 2 * n_c * n_wp));
-    CK(ctx->part.ensure(sizeof(double) * (size_t)pl.n_tiles * NQ * n_wp));
+    if (small) CK(ctx->part.ensure(sizeof(double) * (size_t)(n_items + 32 + n_wp) * NQ * 32));
+    else CK(ctx->part.ensure(sizeof(double) * (size_t)pl.n_tiles * NQ * n_wp));
     CK(ctx->pw_x.ensure(sizeof(double) * ((size_t)n_nodes * n_wp + 2 * (size_t)n_w)));
     double *X = ctx->pw_x.as<double>(), *band_w = X + (size_t)n_nodes * n_wp;
 
     k_pw_band<<<ceil_div(n_w, 256), 256, 0, st>>>(f_nodes_w, band, (int)n_w, n_nodes, band_w);
     LAUNCHED(ctx);
     {
-        const int rc_b = band_sort(ctx, pl, n_w, false, nullptr, 0, band_w, st);
+        const int rc_b = band_sort(ctx, pl, n_w, false, nullptr, 0, band_w, st, n_items, nullptr, false, false);
         if (rc_b != LL_OK) return rc_b;
     }
     {
@@ -824,6 +829,31 @@ int run_full_pw(ll_ctx *ctx, long long n_w, int n_nodes, const double *f_nodes_w
     }
     FusedArgs fa = fused_args(ctx, pl, n_nodes, t_shift, 1);
     fa.xj = nullptr; fa.bstart = nullptr;
+    if (small) {
+        const int grid = n_items + 32 + n_wp; // = max_items of the planner
+        const size_t smem = (size_t)2 * pl.CH * 8 * (2 * n_c + nw);
+        {
+            ProfScope prof(ctx, st);
+#define LL_FUSED_PW_SMALL(NC, WS)                                                          \
+    do {                                                                                   \
+        if (n_m == 1) k_full_fused_pw<1, NC, WS, 1><<<grid, 32, smem, st>>>(fa, X);        \
+        else k_full_fused_pw<0, NC, WS, 1><<<grid, 32, smem, st>>>(fa, X);                 \
+    } while (0)
+            LL_LAYOUT(ctx, LL_FUSED_PW_SMALL);
+#undef LL_FUSED_PW_SMALL
+            LAUNCHED(ctx);
+        }
+        ctx->last_n_blocks = grid;
+        CK(ctx->part2.ensure(sizeof(double) * (size_t)(n_wp / 32) * kFinZ * 9 * 32));
+#define LL_FIN_PW_SMALL(NC, WS)                                                                                            \
+    k_finalize_small<0, NC, (WS ? 1 : NC)><<<dim3(n_wp / 32, kFinZ), dim3(32, fin_slices(2)), 0, st>>>(                    \
+        ctx->part.as<double>(), ctx->part2.as<double>(), ctx->TF.as<double>(), ctx->perm.as<int>(), n_wp, ctx->grp_tab.as<int>(), \
+        ctx->dd.as<double>(), logL, d_h, h_h)
+        LL_LAYOUT(ctx, LL_FIN_PW_SMALL);
+#undef LL_FIN_PW_SMALL
+        LAUNCHED(ctx);
+        return LL_OK;
+    }
     {
         dim3 grid(n_wp / pl.WB, pl.n_tiles);
         const size_t smem = (size_t)2 * pl.CH * 8 * (2 * n_c + nw);

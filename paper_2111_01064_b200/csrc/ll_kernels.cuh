@@ -2902,7 +2902,8 @@ k_spline_pw_block(const double *__restrict__ Y, const double *__restrict__ X, do
 #ifndef LL_PW_MINB
 #define LL_PW_MINB 3
 #endif
-template <int NM1, int NC, bool WS>
+// SMALL = 1: one-warp blocks over the planner's group items (cost = bins: no interval table is shared by the walkers).
+template <int NM1, int NC, bool WS, int SMALL = 0>
 __global__ void __launch_bounds__(128, NM1 ? LL_PW_MINB : 3) k_full_fused_pw(FusedArgs a, const double *__restrict__ X)
 {
     using TL = Tile<NC, WS>;
@@ -2911,9 +2912,21 @@ __global__ void __launch_bounds__(128, NM1 ? LL_PW_MINB : 3) k_full_fused_pw(Fus
     __shared__ int s_lo, s_hi;
 
     const int tid = threadIdx.x;
-    const int p = blockIdx.x * blockDim.x + tid;
-    const int tile = blockIdx.y;
-    const int i0 = __ldg(a.tile_start + tile), i1 = __ldg(a.tile_start + tile + 1);
+    int p, tile, i0, i1;
+    if (SMALL) {
+        tile = blockIdx.x;
+        if (tile >= __ldg(a.grp_tab + 32)) return;
+        const int *it = a.grp_tab + grp_off_items() + tile;
+        const int mi = gridDim.x;
+        i0 = __ldg(it + mi);
+        i1 = __ldg(it + 2 * mi);
+        p = __ldg(it) * 32 + tid;
+    } else {
+        p = blockIdx.x * blockDim.x + tid;
+        tile = blockIdx.y;
+        i0 = __ldg(a.tile_start + tile);
+        i1 = __ldg(a.tile_start + tile + 1);
+    }
     const int lo = max(a.ilo[p], i0), hi = min(a.ihi[p], i1);
     if (tid == 0) {
         s_lo = INT_MAX;
@@ -2929,7 +2942,10 @@ __global__ void __launch_bounds__(128, NM1 ? LL_PW_MINB : 3) k_full_fused_pw(Fus
     }
     __syncthreads();
     const int blo = s_lo, bhi = s_hi;
-    if (blo >= bhi) return;
+    if (blo >= bhi) {
+        if (SMALL) { a.part[((size_t)tile * 2) * 32 + tid] = 0.0; a.part[((size_t)tile * 2 + 1) * 32 + tid] = 0.0; } // F4 reads every item
+        return;
+    }
 
     const int CH = a.CH;
     const int c_begin = blo / CH, c_end = (bhi + CH - 1) / CH;
@@ -3056,6 +3072,11 @@ __global__ void __launch_bounds__(128, NM1 ? LL_PW_MINB : 3) k_full_fused_pw(Fus
         }
         poison_stage(sg, CH * TL::DPB);
         __syncthreads();
+    }
+    if (SMALL) {
+        a.part[((size_t)tile * 2) * 32 + tid] = s_dh;
+        a.part[((size_t)tile * 2 + 1) * 32 + tid] = s_hh;
+        return;
     }
     double *o = a.part + ((size_t)tile * 2) * sw + p;
     o[0] = s_dh; o[sw] = s_hh;
