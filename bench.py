@@ -826,6 +826,20 @@ def main():
                               "max_abs_dlogL_vs_shared_nodes": float((o3[0] - sh[0]).abs().max()),
                               "entry": "ll_full_batch_pw (f_nodes_w [n_w][1024] on the device; the walkers' own bands)",
                               "covered_by": COVERED_BY["cfg2_pw"]}
+            # the same entry point at Module-1 size (block spline with a warm-up for the elimination factors, work items)
+            x16, a16, p16, t16, b16 = (v[:160].contiguous() for v in (xw, amp, ph, tfc, bnd))
+            o16 = tuple(torch.empty(160, dtype=torch.float64, device=amp.device) for _ in range(3))
+            fn16 = lambda: c2.full_batch_pw(x16, a16, p16, t16, band=b16, out=o16)
+            fn16()
+            c2.profile_enable(True)
+            ms16 = time_steps(torch, fn16, 20, 3) / 20
+            kms16, kn16 = c2.profile_read()
+            c2.profile_enable(False)
+            pairs16 = c2.last_full_stats()[0]
+            per["cfg2_pw"]["call_160"] = {"n_walkers": 160, "ms_per_batch": ms16, "kernel_ms": kms16 / max(kn16, 1), "units": pairs16,
+                                          "slots_per_unit": SLOTS_FULL_PW,
+                                          "frac": pairs16 * SLOTS_FULL_PW / (kms16 / max(kn16, 1) * 1e-3) / peak_slots,
+                                          "covered_by": "tests/test_parity_cfg2_scale.py::test_small_batch_pw_against_oracle"}
             del xw, sh, tfc
             # ---- SURVEY §8(f) item 2, t_shift: the stand-in's linear phase term 2 pi f t_c kept outside the spline
             c2.standin_split_tc(True)
