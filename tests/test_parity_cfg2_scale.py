@@ -405,3 +405,29 @@ def test_small_batch_pw_against_oracle(cfg2, orc, torch_cuda, n, bc):
     check_triplet(_np_triplet(got, s_), ref, f"per-walker nodes, {n} walkers, bc {bc}")
     assert ctx.debug_check() == 0
     ctx.destroy()
+
+
+def test_small_batch_reruns_are_bit_identical(cfg2, torch_cuda):
+    """Every way into the small-batch route on the one-year grid, called again and again with the same inputs: the same bits
+    (the planner's tables, the per-block ranking of k_setup_small, the lanes items' butterflies and the tickets of the split F4
+    must not let timing into the sums)."""
+    wl, d, run, ctx, fis = cfg2
+    tc = torch_cuda
+    rng = np.random.default_rng(77)
+    p = wl.params[rng.choice(wl.n_w, 160, replace=False)]
+    amp, ph, top = lisa_node_arrays(p, wl.f_nodes)
+    g = wl.grid
+    band = dev(tc, np.stack([np.full(160, g.k_min * g.df), top], axis=1))
+    tf = dev(tc, p[:, 5:9].reshape(160, 1, 2, 2))
+    tfn = dev(tc, _smooth_tf_at_nodes(p, wl.f_nodes))
+    xw = dev(tc, np.tile(wl.f_nodes, (160, 1)))
+    gp, ga, gph = dev(tc, p), dev(tc, amp), dev(tc, ph)
+    calls = {"stand-in": lambda: ctx.full_batch_standin(wl.f_nodes, gp),
+             "arrays": lambda: ctx.full_batch(wl.f_nodes, ga, gph, tf, band),
+             "T(f)": lambda: ctx.full_batch_tf(wl.f_nodes, ga, gph, tfn, band),
+             "per-walker nodes": lambda: ctx.full_batch_pw(xw, ga, gph, tf, band)}
+    for name, fn in calls.items():
+        first = [v.clone() for v in fn()]
+        for rep in range(8):
+            again = fn()
+            assert all(tc.equal(a, b) for a, b in zip(first, again)), f"{name}: rerun {rep} differs"
